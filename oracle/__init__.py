@@ -1,0 +1,95 @@
+"""oracle — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+ctypes loader for ``oracle/rta_oracle.cpp``: the plain single-threaded C++
+definition of sliding-window signal extraction (BASELINE.json:north_star
+sentence 2; §5 names the step, nothing more).
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
+``cpu_baseline`` / ``--impl reference`` legs may import this package. It never
+imports ``paper_1307_6489_b200`` and shares no code with it. numpy arrays in,
+numpy arrays out; no torch, no CUDA.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "rta_oracle.cpp")
+_LIB = os.path.join(_HERE, "librta_oracle.so")
+_lock = threading.Lock()
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ -O2 (single-threaded, no fast-math)."""
+    with _lock:
+        stale = (not os.path.exists(_LIB)
+                 or os.path.getmtime(_LIB) < os.path.getmtime(_SRC))
+        if force or stale:
+            tmp = _LIB + ".tmp%d" % os.getpid()
+            subprocess.check_call(
+                ["g++", "-std=c++17", "-O2", "-fPIC", "-shared",
+                 "-ffp-contract=off", "-o", tmp, _SRC])
+            os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        lib.rta_oracle_extract.restype = ctypes.c_int
+        lib.rta_oracle_extract.argtypes = [
+            ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        _lib = lib
+    return _lib
+
+
+def extract(wf: np.ndarray, pedestal: np.ndarray, gain: np.ndarray, W: int):
+    """Run the oracle on ``wf[E][P][S]`` (uint16).
+
+    Returns ``(out_sum int32[E*P], out_start int32[E*P], out_charge
+    float32[E*P], out_time float32[E*P])``.
+    """
+    wf = np.ascontiguousarray(wf, dtype=np.uint16)
+    if wf.ndim != 3:
+        raise ValueError("wf must be [n_events][n_pixels][n_samples]")
+    E, P, S = wf.shape
+    pedestal = np.ascontiguousarray(pedestal, dtype=np.int32)
+    gain = np.ascontiguousarray(gain, dtype=np.float32)
+    if pedestal.shape != (P,) or gain.shape != (P,):
+        raise ValueError("pedestal and gain must be [n_pixels]")
+    n = E * P
+    out_sum = np.empty(n, np.int32)
+    out_start = np.empty(n, np.int32)
+    out_charge = np.empty(n, np.float32)
+    out_time = np.empty(n, np.float32)
+    rc = _load().rta_oracle_extract(
+        wf.ctypes.data, E, P, S, pedestal.ctypes.data, gain.ctypes.data, int(W),
+        out_sum.ctypes.data, out_start.ctypes.data, out_charge.ctypes.data,
+        out_time.ctypes.data)
+    if rc != 0:
+        raise ValueError("rta_oracle_extract: bad shape (S=%d, W=%d)" % (S, W))
+    return out_sum, out_start, out_charge, out_time
+
+
+def extract_threads(wf, pedestal, gain, W, threads: int):
+    """The unmodified oracle function run on disjoint event ranges, one per
+    thread (ctypes releases the GIL). Used only for the all-cores CPU figure."""
+    from concurrent.futures import ThreadPoolExecutor
+    E = wf.shape[0]
+    threads = max(1, min(int(threads), E))
+    bounds = [E * i // threads for i in range(threads + 1)]
+    _load()
+    with ThreadPoolExecutor(threads) as ex:
+        parts = list(ex.map(
+            lambda i: extract(wf[bounds[i]:bounds[i + 1]], pedestal, gain, W),
+            range(threads)))
+    return tuple(np.concatenate([p[k] for p in parts]) for k in range(4))
