@@ -1,0 +1,204 @@
+"""dl0gen — seeded synthetic DL0 camera waveforms (the inputs, nothing else).
+
+Stands in for the paper's "Prod2" simulation (§5), which is not
+available; the five workloads are BASELINE.json:configs[0..4] (C1..C5). This
+package holds none of the extraction arithmetic. It serves both the oracle
+side and the CUDA side of the tests and the bench: ``events_cpu`` (gcc build)
+and ``events_cuda`` (nvcc build) write byte-identical waveforms, so any event
+range generated on the GPU at bench scale can be regenerated on the host for
+the oracle.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_CPU_LIB = os.path.join(_HERE, "libdl0gen_cpu.so")
+_CUDA_LIB = os.path.join(_HERE, "libdl0gen_cuda.so")
+_lock = threading.Lock()
+_cpu = None
+_cuda = None
+
+
+class Params(ctypes.Structure):
+    _fields_ = [
+        ("seed", ctypes.c_uint64),
+        ("n_pixels", ctypes.c_int32), ("n_samples", ctypes.c_int32),
+        ("ped_lo", ctypes.c_int32), ("ped_hi", ctypes.c_int32),
+        ("adc_max", ctypes.c_int32),
+        ("gain_lo", ctypes.c_float), ("gain_hi", ctypes.c_float),
+        ("noise_sigma", ctypes.c_float),
+        ("pulse_frac", ctypes.c_float), ("pulse_sigma", ctypes.c_float),
+        ("peak_lo", ctypes.c_float), ("peak_hi", ctypes.c_float),
+        ("amp_mu", ctypes.c_float), ("amp_sigma", ctypes.c_float),
+    ]
+
+
+@dataclass(frozen=True)
+class Config:
+    """One workload of BASELINE.json:configs."""
+    name: str
+    label: str
+    seed: int
+    n_events: int
+    n_pixels: int
+    n_samples: int
+    W: int
+    ped_lo: int
+    ped_hi: int
+    noise_sigma: float
+    pulse_frac: float
+    pulse_sigma: float
+    peak_lo: float
+    peak_hi: float
+    amp_mu: float
+    amp_sigma: float
+    gain_lo: float = 0.9
+    gain_hi: float = 1.1
+    adc_max: int = 4095
+
+    @property
+    def n_traces(self) -> int:
+        return self.n_events * self.n_pixels
+
+    @property
+    def trace_bytes(self) -> int:
+        return 2 * self.n_samples
+
+    @property
+    def input_bytes(self) -> int:
+        return self.n_traces * self.trace_bytes
+
+    @property
+    def output_bytes(self) -> int:
+        return self.n_traces * 16
+
+    def with_events(self, n_events: int) -> "Config":
+        d = dict(self.__dict__)
+        d["n_events"] = int(n_events)
+        return Config(**d)
+
+    def params(self) -> Params:
+        return Params(self.seed, self.n_pixels, self.n_samples, self.ped_lo,
+                      self.ped_hi, self.adc_max, self.gain_lo, self.gain_hi,
+                      self.noise_sigma, self.pulse_frac, self.pulse_sigma,
+                      self.peak_lo, self.peak_hi, self.amp_mu, self.amp_sigma)
+
+
+# BASELINE.json:configs[0..4]; seeds: C1 = 0 as stated, C2..C5 = 1..4 (unstated).
+CONFIGS = {
+    "C1": Config("C1", "tiny LST-like 64x1855x30 W=7", 0, 64, 1855, 30, 7,
+                 380, 420, 4.0, 0.05, 1.5, 8.0, 22.0, 3.0, 1.0),
+    "C2": Config("C2", "LST-like 10000x1855x40 W=7", 1, 10_000, 1855, 40, 7,
+                 380, 420, 4.0, 0.08, 1.5, 12.0, 28.0, 3.5, 1.2),
+    "C3": Config("C3", "MST-like 20000x1764x25 W=4", 2, 20_000, 1764, 25, 4,
+                 280, 320, 3.0, 0.05, 1.2, 6.0, 18.0, 3.0, 1.0),
+    "C4": Config("C4", "SST-like 20000x2048x128 W=8", 3, 20_000, 2048, 128, 8,
+                 480, 520, 5.0, 0.03, 3.0, 30.0, 100.0, 3.5, 1.3),
+    "C5": Config("C5", "sustained stream 200000x1855x40 W=7", 4, 200_000, 1855,
+                 40, 7, 380, 420, 4.0, 0.08, 1.5, 12.0, 28.0, 3.5, 1.2),
+}
+
+
+def _stale(lib, srcs):
+    return (not os.path.exists(lib)
+            or any(os.path.getmtime(lib) < os.path.getmtime(s) for s in srcs))
+
+
+def build_cpu(force: bool = False) -> str:
+    srcs = [os.path.join(_HERE, "dl0gen_cpu.c"), os.path.join(_HERE, "dl0gen_core.h")]
+    with _lock:
+        if force or _stale(_CPU_LIB, srcs):
+            tmp = _CPU_LIB + ".tmp%d" % os.getpid()
+            subprocess.check_call(
+                ["gcc", "-std=c11", "-O2", "-fPIC", "-shared", "-ffp-contract=off",
+                 "-fno-fast-math", "-o", tmp, srcs[0], "-lm"])
+            os.replace(tmp, _CPU_LIB)
+    return _CPU_LIB
+
+
+def build_cuda(force: bool = False) -> str:
+    srcs = [os.path.join(_HERE, "dl0gen_cuda.cu"), os.path.join(_HERE, "dl0gen_core.h")]
+    with _lock:
+        if force or _stale(_CUDA_LIB, srcs):
+            tmp = _CUDA_LIB + ".tmp%d" % os.getpid()
+            subprocess.check_call(
+                ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3",
+                 "-lineinfo", "-fmad=false", "-shared", "-Xcompiler", "-fPIC",
+                 "-cudart", "shared", "-o", tmp, srcs[0]])
+            os.replace(tmp, _CUDA_LIB)
+    return _CUDA_LIB
+
+
+def _cpu_lib():
+    global _cpu
+    if _cpu is None:
+        lib = ctypes.CDLL(build_cpu())
+        lib.dl0gen_calib.restype = None
+        lib.dl0gen_calib.argtypes = [ctypes.POINTER(Params), ctypes.c_void_p, ctypes.c_void_p]
+        lib.dl0gen_events_cpu.restype = None
+        lib.dl0gen_events_cpu.argtypes = [ctypes.POINTER(Params), ctypes.c_int64,
+                                          ctypes.c_int64, ctypes.c_void_p]
+        _cpu = lib
+    return _cpu
+
+
+def _cuda_lib():
+    global _cuda
+    if _cuda is None:
+        lib = ctypes.CDLL(build_cuda())
+        lib.dl0gen_events_cuda.restype = ctypes.c_int
+        lib.dl0gen_events_cuda.argtypes = [ctypes.POINTER(Params), ctypes.c_longlong,
+                                           ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
+        _cuda = lib
+    return _cuda
+
+
+def calib(cfg: Config):
+    """(pedestal int32[P], gain float32[P]) for a config."""
+    ped = np.empty(cfg.n_pixels, np.int32)
+    gain = np.empty(cfg.n_pixels, np.float32)
+    p = cfg.params()
+    _cpu_lib().dl0gen_calib(ctypes.byref(p), ped.ctypes.data, gain.ctypes.data)
+    return ped, gain
+
+
+def events_cpu(cfg: Config, first_event: int = 0, n_events: int | None = None,
+               threads: int = 1) -> np.ndarray:
+    """uint16 [n_events][P][S] for events first_event.. on the host."""
+    if n_events is None:
+        n_events = cfg.n_events - first_event
+    out = np.empty((n_events, cfg.n_pixels, cfg.n_samples), np.uint16)
+    p = cfg.params()
+    lib = _cpu_lib()
+    threads = max(1, min(int(threads), max(1, n_events)))
+    if threads == 1:
+        lib.dl0gen_events_cpu(ctypes.byref(p), first_event, n_events, out.ctypes.data)
+        return out
+    from concurrent.futures import ThreadPoolExecutor
+    b = [n_events * i // threads for i in range(threads + 1)]
+    ev_bytes = cfg.n_pixels * cfg.n_samples * 2
+
+    def work(i):
+        lib.dl0gen_events_cpu(ctypes.byref(p), first_event + b[i], b[i + 1] - b[i],
+                              out.ctypes.data + b[i] * ev_bytes)
+    with ThreadPoolExecutor(threads) as ex:
+        list(ex.map(work, range(threads)))
+    return out
+
+
+def events_cuda(cfg: Config, wf_dev_ptr: int, first_event: int, n_events: int,
+                stream: int = 0) -> None:
+    """Fill a DEVICE buffer (raw pointer) with events first_event.. ; async on
+    ``stream``. Byte-identical to :func:`events_cpu`."""
+    p = cfg.params()
+    rc = _cuda_lib().dl0gen_events_cuda(ctypes.byref(p), first_event, n_events,
+                                        ctypes.c_void_p(wf_dev_ptr), ctypes.c_void_p(stream))
+    if rc != 0:
+        raise RuntimeError("dl0gen_events_cuda: cudaError %d" % rc)
