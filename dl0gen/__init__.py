@@ -131,7 +131,7 @@ def build_cuda(force: bool = False) -> str:
             subprocess.check_call(
                 ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3",
                  "-lineinfo", "-fmad=false", "-shared", "-Xcompiler", "-fPIC",
-                 "-cudart", "shared", "-o", tmp, srcs[0]])
+                 "-o", tmp, srcs[0]])
             os.replace(tmp, _CUDA_LIB)
     return _CUDA_LIB
 

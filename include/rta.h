@@ -1,0 +1,127 @@
+/* rta.h — C ABI of the B200 sliding-window signal-extraction library (librta.so).
+ *
+ * The operation (BASELINE.json:north_star sentence 2; the paper names the step
+ * only as "signal extraction algorithms [13] ... ported to CUDA"
+ * §5, at the front of RT-RECO's calibration, §4): for every
+ * trace wf[e][p][0..S-1] of digitised camera samples,
+ *
+ *     x[s]      = wf[e][p][s] - pedestal[p]
+ *     Sum(t)    = x[t] + ... + x[t+W-1],   t = 0 .. S-W      (windows inside the trace)
+ *     t*        = smallest t with Sum(t) = max_t Sum(t)       (earliest on ties)
+ *     out_sum   = Sum(t*)                      int32, exact
+ *     out_start = t*                           int32, exact, 0-based
+ *     out_charge= RN32(Sum(t*) * gain[p])      float32
+ *     out_time  = RN32(sum_{s=t*}^{t*+W-1} s*x[s] / Sum(t*))  float32, absolute 0-based
+ *                 sample index; t* + (W-1)/2 when Sum(t*) <= 0
+ *
+ * (DESIGN.md "Readings" R1-R18 lists every point the sources leave open.)
+ *
+ * Conventions for every entry point
+ *  - All functions return an int status (RTA_OK or RTA_ERR_*); they never
+ *    throw, print or exit. Arguments are validated before anything is enqueued.
+ *  - The caller owns every pointer it passes; the library never frees or
+ *    retains them. The library owns only rta_extract_stream's workspace (two
+ *    device chunk buffers, two pinned staging buffers when the source is
+ *    pageable, one copy stream, events), created lazily, reused, and released
+ *    by rta_shutdown().
+ *  - There is no CPU fallback: without a CUDA device every compute call
+ *    returns RTA_ERR_CUDA.
+ *  - The library links the CUDA runtime only (no libtorch).
+ */
+#ifndef RTA_H
+#define RTA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  RTA_OK = 0,
+  RTA_ERR_NULL = 1,        /* a required pointer is NULL while there is work to do */
+  RTA_ERR_SHAPE = 2,       /* n_events < 0, n_pixels < 1, n_samples < 1, W < 1 or W > n_samples */
+  RTA_ERR_UNSUPPORTED = 3, /* n_events*n_pixels >= 2^31, or n_samples*W*65535 >= 2^31 (int32 guard) */
+  RTA_ERR_ALIGN = 4,       /* wf is not 2-byte aligned / an output is not 4-byte aligned */
+  RTA_ERR_CUDA = 5,        /* CUDA runtime failure; see rta_last_cuda_error() */
+  RTA_ERR_NOMEM = 6        /* workspace allocation failed (device or pinned host) */
+};
+
+/* Kernel-only path.
+ *
+ *   wf        DEVICE  uint16 [n_events][n_pixels][n_samples], dense, sample fastest.
+ *                     Any uint16 value is accepted (12-bit data is a property of the
+ *                     configs, not of the ABI). A 16-byte-aligned base pointer takes
+ *                     the staged (TMA / cp.async) kernels; any other 2-byte-aligned
+ *                     pointer takes the generic kernel. Same results either way.
+ *   pedestal  DEVICE  int32  [n_pixels]; may exceed the samples (x can be negative).
+ *   gain      DEVICE  float  [n_pixels]; NaN/Inf propagate into out_charge untouched.
+ *   W         window width in samples, 1 <= W <= n_samples.
+ *   out_*     DEVICE  flat [n_events*n_pixels], index e*n_pixels + p, 4-byte aligned.
+ *   stream    cudaStream_t (NULL = the default stream).
+ *
+ * Asynchronous: validates, enqueues on `stream`, returns without synchronising.
+ * Outputs are valid once `stream` has been synchronised. n_events == 0 is
+ * RTA_OK with nothing enqueued and the outputs untouched. Stateless and
+ * thread-safe across streams. */
+int rta_extract(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
+                int32_t n_samples, const int32_t* pedestal, const float* gain,
+                int32_t W, int32_t* out_sum, int32_t* out_start,
+                float* out_charge, float* out_time, void* stream);
+
+/* Host-fed path (step a8; BASELINE.json:configs[4]; page-locked transfer test
+ * of PAPER.md:133/139 §5). Same operation, but `wf_host` is HOST memory
+ * (pinned, or pageable — then it is staged through library-owned pinned
+ * buffers). The waveforms are cut into chunks of whole events of at most
+ * `chunk_bytes` (0 = 1 GiB; rounded down to whole events, at least one event),
+ * and chunk k+1 is copied host->device on a library-owned copy stream while
+ * chunk k is extracted on `stream` (two device buffers).
+ *
+ *   pedestal, gain, out_*   DEVICE, out_* sized for the whole run.
+ *
+ * Returns after the last kernel has been enqueued and every H2D copy has been
+ * issued; all work is ordered on `stream`, so synchronising `stream` makes the
+ * outputs valid and `wf_host` reusable. Calls are serialised by a library
+ * mutex (single workspace). */
+int rta_extract_stream(const uint16_t* wf_host, int64_t n_events,
+                       int32_t n_pixels, int32_t n_samples,
+                       const int32_t* pedestal, const float* gain, int32_t W,
+                       int32_t* out_sum, int32_t* out_start, float* out_charge,
+                       float* out_time, size_t chunk_bytes, void* stream);
+
+/* Host-to-host convenience on top of rta_extract_stream, the end-to-end call a
+ * user with nothing on the device makes: every pointer is HOST memory
+ * (pedestal/gain/outputs pinned or pageable); outputs are copied back
+ * device->host chunk by chunk on a third stream, overlapping the next chunk.
+ * Synchronous: returns when the outputs are complete in host memory. */
+int rta_extract_host(const uint16_t* wf_host, int64_t n_events, int32_t n_pixels,
+                     int32_t n_samples, const int32_t* pedestal_host,
+                     const float* gain_host, int32_t W, int32_t* out_sum_host,
+                     int32_t* out_start_host, float* out_charge_host,
+                     float* out_time_host, size_t chunk_bytes);
+
+/* Static, never-NULL description of a status code. */
+const char* rta_strerror(int status);
+
+/* The cudaError_t behind this thread's most recent RTA_ERR_CUDA / RTA_ERR_NOMEM
+ * (0 if none). */
+int rta_last_cuda_error(void);
+
+/* Which kernel a shape takes, for tests and profiles: writes a static string
+ * such as "tile<S=40,W=7>" or "generic" for (n_samples, W, 16-byte-aligned?). */
+const char* rta_kernel_name(int32_t n_samples, int32_t W, int aligned16);
+
+/* Number of kernels the library has launched in this process (all threads);
+ * bench.py reports the difference over its timed region as gpu_launches. */
+uint64_t rta_launch_count(void);
+
+/* Frees the library-owned workspace (device buffers, pinned staging, streams,
+ * events). Safe to call at any time no stream call is running; the workspace
+ * is rebuilt on demand. */
+void rta_shutdown(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RTA_H */

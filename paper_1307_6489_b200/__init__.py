@@ -1,0 +1,160 @@
+"""paper_1307_6489_b200 — thin Python binding of librta.so (include/rta.h).
+
+Argument marshalling only: every step of the extraction runs in the CUDA
+kernels of ``csrc/``. PyTorch is used by callers for device memory and streams;
+this module only turns tensors into raw pointers for the C ABI. There is no CPU
+fallback — if the library cannot be built or loaded, importing the entry points
+raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import threading
+
+RTA_OK = 0
+RTA_ERR_NULL = 1
+RTA_ERR_SHAPE = 2
+RTA_ERR_UNSUPPORTED = 3
+RTA_ERR_ALIGN = 4
+RTA_ERR_CUDA = 5
+RTA_ERR_NOMEM = 6
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_lock = threading.Lock()
+_lib = None
+
+_VP = ctypes.c_void_p
+_EXTRACT_ARGS = [_VP, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, _VP, _VP,
+                 ctypes.c_int32, _VP, _VP, _VP, _VP]
+
+
+class RtaError(RuntimeError):
+    def __init__(self, status: int, message: str, cuda_error: int = 0):
+        super().__init__("rta: %s (status %d, cudaError %d)" % (message, status, cuda_error))
+        self.status = status
+        self.cuda_error = cuda_error
+
+
+def lib() -> ctypes.CDLL:
+    """Load (building in-tree if stale) librta.so and declare its symbols."""
+    global _lib
+    with _lock:
+        if _lib is None:
+            from . import build as _build
+            path = _build.build()
+            if not os.path.exists(path):
+                raise ImportError("librta.so is missing and could not be built: " + path)
+            L = ctypes.CDLL(path)
+            for name in ("rta_extract", "rta_extract_generic"):
+                fn = getattr(L, name)
+                fn.restype = ctypes.c_int
+                fn.argtypes = _EXTRACT_ARGS + [_VP]
+            L.rta_extract_stream.restype = ctypes.c_int
+            L.rta_extract_stream.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t, _VP]
+            L.rta_extract_host.restype = ctypes.c_int
+            L.rta_extract_host.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t]
+            L.rta_strerror.restype = ctypes.c_char_p
+            L.rta_strerror.argtypes = [ctypes.c_int]
+            L.rta_last_cuda_error.restype = ctypes.c_int
+            L.rta_last_cuda_error.argtypes = []
+            L.rta_kernel_name.restype = ctypes.c_char_p
+            L.rta_kernel_name.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int]
+            L.rta_launch_count.restype = ctypes.c_uint64
+            L.rta_launch_count.argtypes = []
+            L.rta_shutdown.restype = None
+            L.rta_shutdown.argtypes = []
+            _lib = L
+    return _lib
+
+
+def _ptr(x) -> int | None:
+    """torch tensor / numpy array / int / None -> raw address."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):
+        return x.ctypes.data
+    raise TypeError("expected a tensor, an array, an int address or None")
+
+
+def _check(status: int) -> None:
+    if status != RTA_OK:
+        L = lib()
+        raise RtaError(status, L.rta_strerror(status).decode(), L.rta_last_cuda_error())
+
+
+def _stream_handle(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def rta_extract(wf, n_events, n_pixels, n_samples, pedestal, gain, W,
+                out_sum, out_start, out_charge, out_time, stream=None, *,
+                generic: bool = False) -> None:
+    """include/rta.h:rta_extract. Device pointers (tensors or addresses);
+    asynchronous on ``stream`` (default: torch's current stream)."""
+    fn = lib().rta_extract_generic if generic else lib().rta_extract
+    _check(fn(_ptr(wf), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain), W,
+              _ptr(out_sum), _ptr(out_start), _ptr(out_charge), _ptr(out_time),
+              _stream_handle(stream)))
+
+
+def rta_extract_stream(wf_host, n_events, n_pixels, n_samples, pedestal, gain, W,
+                       out_sum, out_start, out_charge, out_time, chunk_bytes=0,
+                       stream=None) -> None:
+    """include/rta.h:rta_extract_stream. ``wf_host`` is host memory; the rest
+    are device pointers. Outputs valid after ``stream`` is synchronised."""
+    _check(lib().rta_extract_stream(
+        _ptr(wf_host), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain), W,
+        _ptr(out_sum), _ptr(out_start), _ptr(out_charge), _ptr(out_time),
+        int(chunk_bytes), _stream_handle(stream)))
+
+
+def rta_extract_host(wf_host, n_events, n_pixels, n_samples, pedestal_host, gain_host,
+                     W, out_sum_host, out_start_host, out_charge_host, out_time_host,
+                     chunk_bytes=0) -> None:
+    """include/rta.h:rta_extract_host. Every pointer is host memory;
+    synchronous."""
+    _check(lib().rta_extract_host(
+        _ptr(wf_host), n_events, n_pixels, n_samples, _ptr(pedestal_host),
+        _ptr(gain_host), W, _ptr(out_sum_host), _ptr(out_start_host),
+        _ptr(out_charge_host), _ptr(out_time_host), int(chunk_bytes)))
+
+
+def rta_strerror(status: int) -> str:
+    return lib().rta_strerror(status).decode()
+
+
+def rta_last_cuda_error() -> int:
+    return lib().rta_last_cuda_error()
+
+
+def rta_kernel_name(n_samples: int, W: int, aligned16: bool = True) -> str:
+    return lib().rta_kernel_name(n_samples, W, 1 if aligned16 else 0).decode()
+
+
+def rta_launch_count() -> int:
+    return int(lib().rta_launch_count())
+
+
+def rta_shutdown() -> None:
+    lib().rta_shutdown()
+
+
+def shard_events(n_events: int, world_size: int, rank: int) -> tuple[int, int]:
+    """Contiguous event range [first, first+count) of ``rank`` when a batch is
+    split over ``world_size`` independent GPUs (traces are
+    independent, so there is no exchange step and no collective)."""
+    if world_size < 1 or not (0 <= rank < world_size):
+        raise ValueError("bad rank/world_size")
+    first = n_events * rank // world_size
+    last = n_events * (rank + 1) // world_size
+    return first, last - first

@@ -1,0 +1,410 @@
+// rta_api.cu — the C ABI of include/rta.h: validation, error reporting, and the
+// host-fed double-buffered stream path (the
+// page-locked transfer experiment of PAPER.md:133/139 §5 is its ancestor).
+// No CPU fallback exists here: every compute call ends in a kernel launch or
+// in an error code.
+#include "../../include/rta.h"
+
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstring>
+#include <mutex>
+
+#include "rta_internal.h"
+
+namespace {
+
+thread_local int t_last_cuda = 0;
+std::atomic<uint64_t> g_launches{0};
+
+int fail_cuda(cudaError_t e) {
+  t_last_cuda = (int)e;
+  if (e == cudaErrorMemoryAllocation) return RTA_ERR_NOMEM;
+  return RTA_ERR_CUDA;
+}
+
+int validate(const void* wf, int64_t n_events, int32_t n_pixels, int32_t n_samples,
+             const void* pedestal, const void* gain, int32_t W, const void* o0, const void* o1,
+             const void* o2, const void* o3) {
+  if (n_events < 0 || n_pixels < 1 || n_samples < 1 || W < 1 || W > n_samples)
+    return RTA_ERR_SHAPE;
+  if (n_events * (int64_t)n_pixels >= (1ll << 31)) return RTA_ERR_UNSUPPORTED;
+  if ((int64_t)n_samples * (int64_t)W * 65535ll >= (1ll << 31)) return RTA_ERR_UNSUPPORTED;
+  if (n_events == 0) return RTA_OK;
+  if (!wf || !pedestal || !gain || !o0 || !o1 || !o2 || !o3) return RTA_ERR_NULL;
+  if ((uintptr_t)wf % 2 != 0) return RTA_ERR_ALIGN;
+  if (((uintptr_t)o0 | (uintptr_t)o1 | (uintptr_t)o2 | (uintptr_t)o3 | (uintptr_t)pedestal |
+       (uintptr_t)gain) % 4 != 0)
+    return RTA_ERR_ALIGN;
+  return RTA_OK;
+}
+
+// ---- workspace of the stream path -----------------------------------------
+struct Workspace {
+  std::mutex mu;
+  int device = -1;
+  cudaStream_t copy_stream = nullptr;   // H2D
+  cudaStream_t back_stream = nullptr;   // D2H of outputs (rta_extract_host)
+  void* dev_buf[2] = {nullptr, nullptr};
+  size_t dev_cap = 0;
+  void* pin_buf[2] = {nullptr, nullptr};
+  size_t pin_cap = 0;
+  cudaEvent_t copied[2] = {nullptr, nullptr};    // H2D of buffer b finished
+  cudaEvent_t consumed[2] = {nullptr, nullptr};  // kernel reading buffer b finished
+  bool consumed_valid[2] = {false, false};
+  // rta_extract_host only
+  void* out_buf[2] = {nullptr, nullptr};   // 4 arrays x chunk traces
+  size_t out_cap = 0;
+  void* calib_buf = nullptr;
+  size_t calib_cap = 0;
+  cudaEvent_t done[2] = {nullptr, nullptr};      // kernel of slot b finished
+  cudaEvent_t returned[2] = {nullptr, nullptr};  // D2H of slot b finished
+  bool returned_valid[2] = {false, false};
+  cudaStream_t host_stream = nullptr;            // compute stream of rta_extract_host
+};
+Workspace g_ws;
+
+void ws_release(Workspace& w) {
+  for (int b = 0; b < 2; ++b) {
+    if (w.dev_buf[b]) cudaFree(w.dev_buf[b]);
+    if (w.pin_buf[b]) cudaFreeHost(w.pin_buf[b]);
+    if (w.out_buf[b]) cudaFree(w.out_buf[b]);
+    if (w.copied[b]) cudaEventDestroy(w.copied[b]);
+    if (w.consumed[b]) cudaEventDestroy(w.consumed[b]);
+    if (w.done[b]) cudaEventDestroy(w.done[b]);
+    if (w.returned[b]) cudaEventDestroy(w.returned[b]);
+    w.dev_buf[b] = w.pin_buf[b] = w.out_buf[b] = nullptr;
+    w.copied[b] = w.consumed[b] = w.done[b] = w.returned[b] = nullptr;
+    w.consumed_valid[b] = w.returned_valid[b] = false;
+  }
+  if (w.calib_buf) cudaFree(w.calib_buf);
+  w.calib_buf = nullptr;
+  if (w.copy_stream) cudaStreamDestroy(w.copy_stream);
+  if (w.back_stream) cudaStreamDestroy(w.back_stream);
+  if (w.host_stream) cudaStreamDestroy(w.host_stream);
+  w.copy_stream = w.back_stream = w.host_stream = nullptr;
+  w.dev_cap = w.pin_cap = w.out_cap = w.calib_cap = 0;
+  w.device = -1;
+}
+
+cudaError_t ws_prepare(Workspace& w) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (w.device != dev) {
+    if (w.device >= 0) {
+      int cur = dev;
+      cudaSetDevice(w.device);
+      cudaDeviceSynchronize();
+      ws_release(w);
+      cudaSetDevice(cur);
+    }
+    if ((e = cudaStreamCreateWithFlags(&w.copy_stream, cudaStreamNonBlocking)) != cudaSuccess)
+      return e;
+    if ((e = cudaStreamCreateWithFlags(&w.back_stream, cudaStreamNonBlocking)) != cudaSuccess)
+      return e;
+    if ((e = cudaStreamCreateWithFlags(&w.host_stream, cudaStreamNonBlocking)) != cudaSuccess)
+      return e;
+    for (int b = 0; b < 2; ++b) {
+      if ((e = cudaEventCreateWithFlags(&w.copied[b], cudaEventDisableTiming)) != cudaSuccess)
+        return e;
+      if ((e = cudaEventCreateWithFlags(&w.consumed[b], cudaEventDisableTiming)) != cudaSuccess)
+        return e;
+      if ((e = cudaEventCreateWithFlags(&w.done[b], cudaEventDisableTiming)) != cudaSuccess)
+        return e;
+      if ((e = cudaEventCreateWithFlags(&w.returned[b], cudaEventDisableTiming)) != cudaSuccess)
+        return e;
+    }
+    w.device = dev;
+  }
+  return cudaSuccess;
+}
+
+// grow a pair of buffers; waits for outstanding users before freeing
+template <class Alloc, class Free>
+cudaError_t grow_pair(void* buf[2], size_t* cap, size_t need, Alloc alloc, Free release) {
+  if (*cap >= need) return cudaSuccess;
+  cudaError_t e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) return e;
+  for (int b = 0; b < 2; ++b) {
+    if (buf[b]) release(buf[b]);
+    buf[b] = nullptr;
+  }
+  *cap = 0;
+  for (int b = 0; b < 2; ++b) {
+    if ((e = alloc(&buf[b], need)) != cudaSuccess) return e;
+  }
+  *cap = need;
+  return cudaSuccess;
+}
+
+bool is_pageable(const void* p) {
+  cudaPointerAttributes a;
+  cudaError_t e = cudaPointerGetAttributes(&a, p);
+  if (e != cudaSuccess) {
+    cudaGetLastError();  // clear
+    return true;
+  }
+  return a.type == cudaMemoryTypeUnregistered;
+}
+
+struct ChunkPlan {
+  int64_t chunk_events;
+  int64_t n_chunks;
+  size_t event_bytes;
+};
+ChunkPlan plan_chunks(int64_t n_events, int32_t n_pixels, int32_t n_samples, size_t chunk_bytes) {
+  ChunkPlan p;
+  p.event_bytes = (size_t)n_pixels * (size_t)n_samples * 2u;
+  if (chunk_bytes == 0) chunk_bytes = (size_t)1 << 30;
+  int64_t ce = (int64_t)(chunk_bytes / p.event_bytes);  // rounded down to whole events
+  if (ce < 1) ce = 1;
+  if (ce > n_events) ce = n_events > 0 ? n_events : 1;
+  p.chunk_events = ce;
+  p.n_chunks = (n_events + ce - 1) / ce;
+  return p;
+}
+
+// Core of the host-fed path. When `host_out` is set, per-chunk results are
+// written to library-owned device slots and copied back to the host arrays.
+struct HostOut {
+  int32_t* sum;
+  int32_t* start;
+  float* charge;
+  float* time;
+};
+
+int stream_impl(Workspace& w, const uint16_t* wf_host, int64_t n_events, int32_t n_pixels,
+                int32_t n_samples, const int32_t* pedestal, const float* gain, int32_t W,
+                int32_t* out_sum, int32_t* out_start, float* out_charge, float* out_time,
+                size_t chunk_bytes, cudaStream_t stream, const HostOut* host_out) {
+  cudaError_t e;
+  const ChunkPlan plan = plan_chunks(n_events, n_pixels, n_samples, chunk_bytes);
+  const size_t buf_bytes = (size_t)plan.chunk_events * plan.event_bytes;
+  e = grow_pair(
+      w.dev_buf, &w.dev_cap, buf_bytes, [](void** p, size_t n) { return cudaMalloc(p, n); },
+      [](void* p) { cudaFree(p); });
+  if (e != cudaSuccess) return fail_cuda(e);
+  const bool pageable = is_pageable(wf_host);
+  if (pageable) {
+    e = grow_pair(
+        w.pin_buf, &w.pin_cap, buf_bytes,
+        [](void** p, size_t n) { return cudaHostAlloc(p, n, cudaHostAllocDefault); },
+        [](void* p) { cudaFreeHost(p); });
+    if (e != cudaSuccess) return fail_cuda(e);
+  }
+  const size_t chunk_traces = (size_t)plan.chunk_events * (size_t)n_pixels;
+  if (host_out) {
+    e = grow_pair(
+        w.out_buf, &w.out_cap, chunk_traces * 16u,
+        [](void** p, size_t n) { return cudaMalloc(p, n); }, [](void* p) { cudaFree(p); });
+    if (e != cudaSuccess) return fail_cuda(e);
+  }
+
+  for (int64_t k = 0; k < plan.n_chunks; ++k) {
+    const int b = (int)(k & 1);
+    const int64_t ev0 = k * plan.chunk_events;
+    const int64_t nev = (ev0 + plan.chunk_events <= n_events) ? plan.chunk_events : n_events - ev0;
+    const size_t bytes = (size_t)nev * plan.event_bytes;
+    const uint8_t* src = reinterpret_cast<const uint8_t*>(wf_host) + (size_t)ev0 * plan.event_bytes;
+
+    // the device buffer is free once the kernel of chunk k-2 (or of an
+    // earlier call) has finished with it
+    if (w.consumed_valid[b]) {
+      if ((e = cudaStreamWaitEvent(w.copy_stream, w.consumed[b], 0)) != cudaSuccess)
+        return fail_cuda(e);
+    }
+    if (pageable) {
+      // pinned staging slot b is free once its previous H2D copy has finished
+      // (an event never recorded counts as complete)
+      if ((e = cudaEventSynchronize(w.copied[b])) != cudaSuccess) return fail_cuda(e);
+      std::memcpy(w.pin_buf[b], src, bytes);
+      src = reinterpret_cast<const uint8_t*>(w.pin_buf[b]);
+    }
+    if ((e = cudaMemcpyAsync(w.dev_buf[b], src, bytes, cudaMemcpyHostToDevice, w.copy_stream)) !=
+        cudaSuccess)
+      return fail_cuda(e);
+    if ((e = cudaEventRecord(w.copied[b], w.copy_stream)) != cudaSuccess) return fail_cuda(e);
+    if ((e = cudaStreamWaitEvent(stream, w.copied[b], 0)) != cudaSuccess) return fail_cuda(e);
+
+    const size_t t0 = (size_t)ev0 * (size_t)n_pixels;
+    const int64_t ntr = nev * (int64_t)n_pixels;
+    int32_t *o_sum, *o_start;
+    float *o_charge, *o_time;
+    if (host_out) {
+      // output slot b is free once its previous D2H has finished
+      if (w.returned_valid[b]) {
+        if ((e = cudaStreamWaitEvent(stream, w.returned[b], 0)) != cudaSuccess)
+          return fail_cuda(e);
+      }
+      uint8_t* ob = reinterpret_cast<uint8_t*>(w.out_buf[b]);
+      o_sum = reinterpret_cast<int32_t*>(ob);
+      o_start = reinterpret_cast<int32_t*>(ob + chunk_traces * 4u);
+      o_charge = reinterpret_cast<float*>(ob + chunk_traces * 8u);
+      o_time = reinterpret_cast<float*>(ob + chunk_traces * 12u);
+    } else {
+      o_sum = out_sum + t0;
+      o_start = out_start + t0;
+      o_charge = out_charge + t0;
+      o_time = out_time + t0;
+    }
+    e = rta_launch_extract(reinterpret_cast<const uint16_t*>(w.dev_buf[b]), ntr, n_pixels,
+                           n_samples, pedestal, gain, W, o_sum, o_start, o_charge, o_time, stream,
+                           false);
+    if (e != cudaSuccess) return fail_cuda(e);
+    if ((e = cudaEventRecord(w.consumed[b], stream)) != cudaSuccess) return fail_cuda(e);
+    w.consumed_valid[b] = true;
+
+    if (host_out) {
+      if ((e = cudaStreamWaitEvent(w.back_stream, w.consumed[b], 0)) != cudaSuccess)
+        return fail_cuda(e);
+      const size_t nb = (size_t)ntr * 4u;
+      if ((e = cudaMemcpyAsync(host_out->sum + t0, o_sum, nb, cudaMemcpyDeviceToHost,
+                               w.back_stream)) != cudaSuccess)
+        return fail_cuda(e);
+      if ((e = cudaMemcpyAsync(host_out->start + t0, o_start, nb, cudaMemcpyDeviceToHost,
+                               w.back_stream)) != cudaSuccess)
+        return fail_cuda(e);
+      if ((e = cudaMemcpyAsync(host_out->charge + t0, o_charge, nb, cudaMemcpyDeviceToHost,
+                               w.back_stream)) != cudaSuccess)
+        return fail_cuda(e);
+      if ((e = cudaMemcpyAsync(host_out->time + t0, o_time, nb, cudaMemcpyDeviceToHost,
+                               w.back_stream)) != cudaSuccess)
+        return fail_cuda(e);
+      if ((e = cudaEventRecord(w.returned[b], w.back_stream)) != cudaSuccess) return fail_cuda(e);
+      w.returned_valid[b] = true;
+    }
+  }
+  return RTA_OK;
+}
+
+}  // namespace
+
+void rta_count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+
+extern "C" {
+
+int rta_extract(const uint16_t* wf, int64_t n_events, int32_t n_pixels, int32_t n_samples,
+                const int32_t* pedestal, const float* gain, int32_t W, int32_t* out_sum,
+                int32_t* out_start, float* out_charge, float* out_time, void* stream) {
+  const int v = validate(wf, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum, out_start,
+                         out_charge, out_time);
+  if (v != RTA_OK || n_events == 0) return v;
+  const cudaError_t e =
+      rta_launch_extract(wf, n_events * (int64_t)n_pixels, n_pixels, n_samples, pedestal, gain, W,
+                         out_sum, out_start, out_charge, out_time, (cudaStream_t)stream, false);
+  return e == cudaSuccess ? RTA_OK : fail_cuda(e);
+}
+
+// Same as rta_extract but always through the generic kernel. Exported for the
+// tests (two independent device paths must agree); not in the public header.
+int rta_extract_generic(const uint16_t* wf, int64_t n_events, int32_t n_pixels, int32_t n_samples,
+                        const int32_t* pedestal, const float* gain, int32_t W, int32_t* out_sum,
+                        int32_t* out_start, float* out_charge, float* out_time, void* stream) {
+  const int v = validate(wf, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum, out_start,
+                         out_charge, out_time);
+  if (v != RTA_OK || n_events == 0) return v;
+  const cudaError_t e =
+      rta_launch_extract(wf, n_events * (int64_t)n_pixels, n_pixels, n_samples, pedestal, gain, W,
+                         out_sum, out_start, out_charge, out_time, (cudaStream_t)stream, true);
+  return e == cudaSuccess ? RTA_OK : fail_cuda(e);
+}
+
+int rta_extract_stream(const uint16_t* wf_host, int64_t n_events, int32_t n_pixels,
+                       int32_t n_samples, const int32_t* pedestal, const float* gain, int32_t W,
+                       int32_t* out_sum, int32_t* out_start, float* out_charge, float* out_time,
+                       size_t chunk_bytes, void* stream) {
+  const int v = validate(wf_host, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum,
+                         out_start, out_charge, out_time);
+  if (v != RTA_OK || n_events == 0) return v;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  cudaError_t e = ws_prepare(g_ws);
+  if (e != cudaSuccess) return fail_cuda(e);
+  return stream_impl(g_ws, wf_host, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum,
+                     out_start, out_charge, out_time, chunk_bytes, (cudaStream_t)stream, nullptr);
+}
+
+int rta_extract_host(const uint16_t* wf_host, int64_t n_events, int32_t n_pixels,
+                     int32_t n_samples, const int32_t* pedestal_host, const float* gain_host,
+                     int32_t W, int32_t* out_sum_host, int32_t* out_start_host,
+                     float* out_charge_host, float* out_time_host, size_t chunk_bytes) {
+  const int v = validate(wf_host, n_events, n_pixels, n_samples, pedestal_host, gain_host, W,
+                         out_sum_host, out_start_host, out_charge_host, out_time_host);
+  if (v != RTA_OK || n_events == 0) return v;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  Workspace& w = g_ws;
+  cudaError_t e = ws_prepare(w);
+  if (e != cudaSuccess) return fail_cuda(e);
+  const size_t calib_bytes = (size_t)n_pixels * 8u;
+  if (w.calib_cap < calib_bytes) {
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail_cuda(e);
+    if (w.calib_buf) cudaFree(w.calib_buf);
+    w.calib_buf = nullptr;
+    w.calib_cap = 0;
+    if ((e = cudaMalloc(&w.calib_buf, calib_bytes)) != cudaSuccess) return fail_cuda(e);
+    w.calib_cap = calib_bytes;
+  }
+  int32_t* d_ped = reinterpret_cast<int32_t*>(w.calib_buf);
+  float* d_gain = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(w.calib_buf) +
+                                           (size_t)n_pixels * 4u);
+  // calibration constants may still be read by kernels of an earlier call
+  if ((e = cudaStreamSynchronize(w.host_stream)) != cudaSuccess) return fail_cuda(e);
+  if ((e = cudaMemcpyAsync(d_ped, pedestal_host, (size_t)n_pixels * 4u, cudaMemcpyHostToDevice,
+                           w.host_stream)) != cudaSuccess)
+    return fail_cuda(e);
+  if ((e = cudaMemcpyAsync(d_gain, gain_host, (size_t)n_pixels * 4u, cudaMemcpyHostToDevice,
+                           w.host_stream)) != cudaSuccess)
+    return fail_cuda(e);
+  const HostOut ho{out_sum_host, out_start_host, out_charge_host, out_time_host};
+  const int rc = stream_impl(w, wf_host, n_events, n_pixels, n_samples, d_ped, d_gain, W, nullptr,
+                             nullptr, nullptr, nullptr, chunk_bytes, w.host_stream, &ho);
+  // synchronous by contract, also on the error path (nothing may outlive the call)
+  cudaError_t e1 = cudaStreamSynchronize(w.host_stream);
+  cudaError_t e2 = cudaStreamSynchronize(w.back_stream);
+  cudaError_t e3 = cudaStreamSynchronize(w.copy_stream);
+  if (rc != RTA_OK) return rc;
+  if (e1 != cudaSuccess) return fail_cuda(e1);
+  if (e2 != cudaSuccess) return fail_cuda(e2);
+  if (e3 != cudaSuccess) return fail_cuda(e3);
+  return RTA_OK;
+}
+
+const char* rta_strerror(int status) {
+  switch (status) {
+    case RTA_OK: return "ok";
+    case RTA_ERR_NULL: return "null pointer with work to do";
+    case RTA_ERR_SHAPE: return "bad shape: need n_events >= 0, n_pixels >= 1, 1 <= W <= n_samples";
+    case RTA_ERR_UNSUPPORTED:
+      return "unsupported size: n_events*n_pixels >= 2^31 or n_samples*W*65535 >= 2^31";
+    case RTA_ERR_ALIGN: return "misaligned pointer (wf: 2 bytes; calibration and outputs: 4 bytes)";
+    case RTA_ERR_CUDA: return "CUDA runtime error (see rta_last_cuda_error)";
+    case RTA_ERR_NOMEM: return "out of device or pinned host memory";
+    default: return "unknown status";
+  }
+}
+
+int rta_last_cuda_error(void) { return t_last_cuda; }
+
+const char* rta_kernel_name(int32_t n_samples, int32_t W, int aligned16) {
+  return rta_pick_kernel_name(n_samples, W, aligned16 != 0);
+}
+
+uint64_t rta_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+void rta_shutdown(void) {
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  if (g_ws.device >= 0) {
+    int cur = 0;
+    if (cudaGetDevice(&cur) == cudaSuccess) {
+      cudaSetDevice(g_ws.device);
+      cudaDeviceSynchronize();
+      ws_release(g_ws);
+      cudaSetDevice(cur);
+    } else {
+      cudaGetLastError();
+    }
+  }
+}
+
+}  // extern "C"

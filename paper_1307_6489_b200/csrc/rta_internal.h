@@ -1,0 +1,24 @@
+// rta_internal.h — declarations shared by the translation units of librta.so.
+// Not part of the public ABI (that is include/rta.h) and never seen by oracle/.
+#ifndef RTA_INTERNAL_H
+#define RTA_INTERNAL_H
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+// Enqueue the extraction of `n_traces` traces starting at global trace index 0
+// of `wf` on `stream`. Arguments are already validated. Returns a cudaError_t.
+// `force_generic` routes every shape to the generic kernel (tests use it to
+// compare the two paths).
+cudaError_t rta_launch_extract(const uint16_t* wf, int64_t n_traces, int32_t n_pixels,
+                               int32_t n_samples, const int32_t* pedestal,
+                               const float* gain, int32_t W, int32_t* out_sum,
+                               int32_t* out_start, float* out_charge, float* out_time,
+                               cudaStream_t stream, bool force_generic);
+
+// Name of the kernel the dispatcher picks (static string).
+const char* rta_pick_kernel_name(int32_t n_samples, int32_t W, bool aligned16);
+
+void rta_count_launch();
+
+#endif

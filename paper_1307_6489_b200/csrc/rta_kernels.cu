@@ -1,0 +1,492 @@
+// rta_kernels.cu — sm_100a kernels for sliding-window signal extraction.
+//
+// What is computed is BASELINE.json:north_star sentence 2 (steps a1-a7 of
+// SURVEY.md §8(a); the paper names the step at PAPER.md:141 §5). How it is
+// computed is this file's own design:
+//
+//  * a1 ingest: persistent CTAs stream contiguous tiles of whole traces from
+//    HBM into a ring of shared-memory stages. Dense layouts (S = 30, 40, 25)
+//    use one TMA bulk copy per tile (cp.async.bulk + mbarrier complete_tx);
+//    the S = 128 layout, whose 256-byte trace stride would put every lane of
+//    a quarter-warp on the same banks, is copied with 16-byte cp.async into a
+//    layout padded by one 16-byte chunk per trace, completion tracked by the
+//    same mbarriers (cp.async.mbarrier.arrive).
+//  * a2 pedestal: deferred. The pedestal is constant inside a trace, so the
+//    arg-max runs on raw samples and Sum = rawsum - W*ped once per trace.
+//  * a3/a4: one thread owns one trace (two when 2*S is not a multiple of 4),
+//    reads it from shared memory with the widest conflict-free vector load,
+//    slides the window in O(1) per step and keeps the maximum of the key
+//    rawsum * 2^KB + (2^KB - 1 - t): one unsigned max per window yields the
+//    largest sum and, among equals, the smallest t (earliest on ties).
+//  * a5-a7: W-1 re-reads of the winning window from shared memory give the
+//    time numerator; integers stay exact (int64 where a pedestal could
+//    overflow int32), floats are one IEEE multiply / one IEEE divide on
+//    exactly representable operands, with a double-precision path when an
+//    operand exceeds 2^24 (bit-identical to rounding the double result).
+//  * outputs: four coalesced 4-byte (or 8-byte) stores per thread.
+//
+// A generic kernel (any S, W, any 2-byte alignment) reads global memory
+// directly; it is the path for shapes without a specialisation.
+#include "rta_internal.h"
+
+#include <atomic>
+
+namespace {
+
+// ------------------------------------------------------------------ PTX ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+// TMA 1-D bulk copy global -> shared, completion on an mbarrier (bytes % 16 == 0)
+__device__ __forceinline__ void tma_bulk_g2s(uint32_t dst, const void* src, uint32_t bytes,
+                                             uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+      "l"(src), "r"(bytes), "r"(bar)
+      : "memory");
+}
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_mbar_arrive(uint32_t bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+
+// ------------------------------------------------------------ utilities ----
+constexpr int ilog2_ceil(int n) {
+  int b = 0;
+  while ((1 << b) < n) ++b;
+  return b;
+}
+
+// g mod d with inv = min(floor(2^32 / d), 2^32 - 1): the estimate is short by
+// at most one, so one conditional subtract finishes it.
+__device__ __forceinline__ uint32_t fastmod(uint32_t g, uint32_t d, uint32_t inv) {
+  const uint32_t q = __umulhi(g, inv);
+  const uint32_t r = g - q * d;
+  return r >= d ? r - d : r;
+}
+
+struct Result {
+  int sum, start;
+  float charge, time;
+};
+
+// Steps a5-a7 from the raw (pedestal-deferred) quantities of one trace:
+//   rawsum = sum of raw samples in the winning window, tstar = its start,
+//   relnum = sum_k k * raw[tstar + k].
+__device__ __forceinline__ Result finish_trace(const int W, const uint32_t rawsum, const int tstar,
+                                               const uint32_t relnum, const int ped,
+                                               const float gain) {
+  Result r;
+  const long long sum64 = (long long)rawsum - (long long)W * (long long)ped;
+  const int c = W * tstar + (W * (W - 1)) / 2;  // sum of the window's sample indices
+  const long long num64 =
+      (long long)((uint32_t)tstar * rawsum + relnum) - (long long)ped * (long long)c;
+  r.sum = (int)sum64;
+  r.start = tstar;
+  const long long lim = 1ll << 24;
+  if (sum64 > -lim && sum64 < lim && num64 > -lim && num64 < lim) {
+    // every operand is an exactly representable integer: one IEEE operation
+    // each, bit-identical to rounding the double-precision result
+    int n = (int)num64, d = (int)sum64;
+    if (d <= 0) {  // degenerate mean -> window centre = (2 t* + W - 1) / 2
+      n = 2 * tstar + W - 1;
+      d = 2;
+    }
+    r.charge = __fmul_rn((float)(int)sum64, gain);
+    r.time = __fdiv_rn((float)n, (float)d);
+  } else {
+    r.charge = (float)((double)sum64 * (double)gain);
+    r.time = sum64 > 0 ? (float)((double)num64 / (double)sum64)
+                       : (float)((double)tstar + 0.5 * (double)(W - 1));
+  }
+  return r;
+}
+
+// ------------------------------------------------------- tile kernel cfg ----
+template <int S_, int W_, int NT_, int STAGES_>
+struct TileCfg {
+  static constexpr int S = S_, W = W_, NT = NT_, STAGES = STAGES_;
+  static constexpr int TRACE_BYTES = 2 * S;
+  static constexpr int TPT = (TRACE_BYTES % 4 == 0) ? 1 : 2;  // traces per thread
+  static constexpr int UNIT_BYTES = TRACE_BYTES * TPT;        // bytes one thread owns
+  static constexpr int VEC = (UNIT_BYTES % 16 == 0) ? 16 : (UNIT_BYTES % 8 == 0) ? 8 : 4;
+  static constexpr int NVEC = UNIT_BYTES / VEC;
+  // an even number of 16-byte chunks per unit puts the lanes of a quarter-warp
+  // on the same banks: pad each unit by one chunk
+  static constexpr bool PAD = (VEC == 16) && (NVEC % 2 == 0);
+  static constexpr int UNIT_STRIDE = UNIT_BYTES + (PAD ? 16 : 0);
+  static constexpr int NWORDS = UNIT_BYTES / 4;
+  static constexpr int TILE_TRACES = NT * TPT;
+  static constexpr int TILE_BYTES = NT * UNIT_BYTES;
+  static constexpr int STAGE_BYTES = ((NT * UNIT_STRIDE + 127) / 128) * 128;
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES;
+  static constexpr int NWIN = S - W + 1;
+  static constexpr int KB = ilog2_ceil(NWIN);
+  static constexpr uint32_t KM = (1u << KB) - 1u;
+  static_assert(W >= 1 && W <= S, "window must fit the trace");
+  static_assert(NT % 32 == 0, "whole warps");
+  static_assert(TILE_BYTES % 16 == 0, "TMA bulk copies move multiples of 16 bytes");
+  static_assert((unsigned long long)W * 65535ull * (1ull << KB) + KM < (1ull << 32),
+                "arg-max key must fit 32 bits for any uint16 data");
+};
+
+// raw sample h (halfword index inside the thread's unit), h known at compile time
+#define RTA_X(w, h) (((h)&1) ? ((w)[(h) >> 1] >> 16) : ((w)[(h) >> 1] & 0xFFFFu))
+
+template <class C>
+__device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, const uint32_t g0,
+                                             const uint32_t n_valid, const uint32_t n_pixels,
+                                             const uint32_t pix_inv,
+                                             const int* __restrict__ pedestal,
+                                             const float* __restrict__ gain,
+                                             int* __restrict__ out_sum, int* __restrict__ out_start,
+                                             float* __restrict__ out_charge,
+                                             float* __restrict__ out_time, const bool vec_store) {
+  constexpr int S = C::S, W = C::W;
+  uint32_t w[C::NWORDS];
+  if constexpr (C::VEC == 16) {
+#pragma unroll
+    for (int i = 0; i < C::NVEC; ++i) {
+      const uint4 v = *reinterpret_cast<const uint4*>(unit + 16 * i);
+      w[4 * i] = v.x, w[4 * i + 1] = v.y, w[4 * i + 2] = v.z, w[4 * i + 3] = v.w;
+    }
+  } else if constexpr (C::VEC == 8) {
+#pragma unroll
+    for (int i = 0; i < C::NVEC; ++i) {
+      const uint2 v = *reinterpret_cast<const uint2*>(unit + 8 * i);
+      w[2 * i] = v.x, w[2 * i + 1] = v.y;
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < C::NVEC; ++i) w[i] = *reinterpret_cast<const uint32_t*>(unit + 4 * i);
+  }
+
+  Result res[C::TPT];
+  uint32_t p = fastmod(g0, n_pixels, pix_inv);
+#pragma unroll
+  for (int j = 0; j < C::TPT; ++j) {
+    constexpr int dummy = 0;
+    (void)dummy;
+    const int h0 = j * S;  // compile-time after unrolling
+    // a3 + a4 on raw samples: sliding sum, packed (sum, earliest) key
+    uint32_t sum = 0;
+#pragma unroll
+    for (int k = 0; k < W; ++k) sum += RTA_X(w, h0 + k);
+    uint32_t best = (sum << C::KB) | C::KM;
+#pragma unroll
+    for (int t = 1; t < C::NWIN; ++t) {
+      sum = sum + RTA_X(w, h0 + t + W - 1) - RTA_X(w, h0 + t - 1);
+      const uint32_t key = (sum << C::KB) + (C::KM - (uint32_t)t);
+      best = max(best, key);
+    }
+    const int tstar = (int)(C::KM - (best & C::KM));
+    const uint32_t rawsum = best >> C::KB;
+    // a7 numerator: re-read the winning window (dynamic index -> shared memory)
+    const uint16_t* tr = reinterpret_cast<const uint16_t*>(unit) + h0 + tstar;
+    uint32_t relnum = 0;
+#pragma unroll
+    for (int k = 1; k < W; ++k) relnum += (uint32_t)k * (uint32_t)tr[k];
+    const int ped = __ldg(pedestal + p);
+    const float gn = __ldg(gain + p);
+    res[j] = finish_trace(W, rawsum, tstar, relnum, ped, gn);
+    p = (p + 1 == n_pixels) ? 0u : p + 1;
+  }
+
+  if constexpr (C::TPT == 1) {
+    if (n_valid >= 1) {
+      __stcs(out_sum + g0, res[0].sum);
+      __stcs(out_start + g0, res[0].start);
+      __stcs(out_charge + g0, res[0].charge);
+      __stcs(out_time + g0, res[0].time);
+    }
+  } else {
+    if (n_valid >= 2 && vec_store) {  // g0 is even: 8-byte stores
+      __stcs(reinterpret_cast<int2*>(out_sum + g0), make_int2(res[0].sum, res[1].sum));
+      __stcs(reinterpret_cast<int2*>(out_start + g0), make_int2(res[0].start, res[1].start));
+      __stcs(reinterpret_cast<float2*>(out_charge + g0),
+             make_float2(res[0].charge, res[1].charge));
+      __stcs(reinterpret_cast<float2*>(out_time + g0), make_float2(res[0].time, res[1].time));
+    } else {
+#pragma unroll
+      for (int j = 0; j < C::TPT; ++j) {
+        if ((uint32_t)j < n_valid) {
+          __stcs(out_sum + g0 + j, res[j].sum);
+          __stcs(out_start + g0 + j, res[j].start);
+          __stcs(out_charge + g0 + j, res[j].charge);
+          __stcs(out_time + g0 + j, res[j].time);
+        }
+      }
+    }
+  }
+}
+
+template <class C>
+__global__ void __launch_bounds__(C::NT)
+    extract_tile_kernel(const uint16_t* __restrict__ wf, const uint32_t n_traces,
+                        const uint32_t n_pixels, const uint32_t pix_inv,
+                        const int* __restrict__ pedestal, const float* __restrict__ gain,
+                        int* __restrict__ out_sum, int* __restrict__ out_start,
+                        float* __restrict__ out_charge, float* __restrict__ out_time,
+                        const int vec_store) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t full_bar[C::STAGES];
+  const int tid = threadIdx.x;
+  const uint32_t n_full = n_traces / C::TILE_TRACES;
+  const uint32_t rem = n_traces - n_full * C::TILE_TRACES;
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t bar_base = smem_u32(full_bar);
+
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < C::STAGES; ++s) mbar_init(bar_base + 8 * s, C::PAD ? C::NT : 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+
+  auto issue = [&](const uint32_t tile, const int stage) {
+    const uint8_t* src = reinterpret_cast<const uint8_t*>(wf) + (size_t)tile * C::TILE_BYTES;
+    const uint32_t dst = smem_base + stage * C::STAGE_BYTES;
+    const uint32_t bar = bar_base + 8 * stage;
+    if constexpr (!C::PAD) {
+      if (tid == 0) {
+        mbar_expect_tx(bar, C::TILE_BYTES);
+        tma_bulk_g2s(dst, src, C::TILE_BYTES, bar);
+      }
+    } else {
+#pragma unroll 4
+      for (int c = tid; c < C::TILE_BYTES / 16; c += C::NT) {
+        const int u = c / C::NVEC;  // one extra chunk of padding per unit
+        cp_async16(dst + (uint32_t)(c + u) * 16u, src + (size_t)c * 16);
+      }
+      cp_async_mbar_arrive(bar);
+    }
+  };
+
+  // prologue: fill the ring
+#pragma unroll
+  for (int s = 0; s < C::STAGES; ++s) {
+    const uint32_t tile = blockIdx.x + (uint32_t)s * gridDim.x;
+    if (tile < n_full) issue(tile, s);
+  }
+
+  uint32_t j = 0;
+  for (uint32_t tile = blockIdx.x; tile < n_full; tile += gridDim.x, ++j) {
+    const int stage = (int)(j % C::STAGES);
+    const uint32_t parity = (j / C::STAGES) & 1u;
+    mbar_wait(bar_base + 8 * stage, parity);
+    const uint8_t* unit = smem + stage * C::STAGE_BYTES + tid * C::UNIT_STRIDE;
+    const uint32_t g0 = tile * C::TILE_TRACES + (uint32_t)tid * C::TPT;
+    compute_unit<C>(unit, g0, C::TPT, n_pixels, pix_inv, pedestal, gain, out_sum, out_start,
+                    out_charge, out_time, vec_store != 0);
+    __syncthreads();  // every thread is done with this stage
+    const uint32_t next = tile + (uint32_t)C::STAGES * gridDim.x;
+    if (next < n_full) issue(next, stage);
+  }
+
+  // ragged tail (< one tile of traces): plain copies, one CTA
+  if (rem != 0 && blockIdx.x == n_full % gridDim.x) {
+    __syncthreads();
+    const uint16_t* src = wf + (size_t)n_full * C::TILE_TRACES * C::S;
+    uint16_t* dst = reinterpret_cast<uint16_t*>(smem);
+    const uint32_t n_hw = rem * C::S;
+    constexpr uint32_t UNIT_HW = C::UNIT_BYTES / 2, STRIDE_HW = C::UNIT_STRIDE / 2;
+    for (uint32_t i = tid; i < n_hw; i += C::NT) {
+      const uint32_t u = i / UNIT_HW;
+      dst[u * STRIDE_HW + (i - u * UNIT_HW)] = src[i];
+    }
+    __syncthreads();
+    const uint32_t first = (uint32_t)tid * C::TPT;
+    if (first < rem) {
+      const uint8_t* unit = smem + tid * C::UNIT_STRIDE;
+      const uint32_t g0 = n_full * C::TILE_TRACES + first;
+      compute_unit<C>(unit, g0, rem - first, n_pixels, pix_inv, pedestal, gain, out_sum,
+                      out_start, out_charge, out_time, vec_store != 0);
+    }
+  }
+}
+
+// -------------------------------------------------------- generic kernel ----
+// Any (S, W) inside the ABI guards, any 2-byte alignment: one thread per trace,
+// samples read straight from global memory (L1/L2 absorb the re-reads).
+__global__ void __launch_bounds__(256)
+    extract_generic_kernel(const uint16_t* __restrict__ wf, const uint32_t n_traces, const int S,
+                           const int W, const uint32_t n_pixels, const uint32_t pix_inv,
+                           const int* __restrict__ pedestal, const float* __restrict__ gain,
+                           int* __restrict__ out_sum, int* __restrict__ out_start,
+                           float* __restrict__ out_charge, float* __restrict__ out_time) {
+  for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < n_traces;
+       g += gridDim.x * blockDim.x) {
+    const uint16_t* tr = wf + (size_t)g * S;
+    uint32_t sum = 0;
+    for (int k = 0; k < W; ++k) sum += tr[k];
+    uint32_t best = sum;
+    int tstar = 0;
+    for (int t = 1; t + W <= S; ++t) {
+      sum = sum + tr[t + W - 1] - tr[t - 1];
+      if (sum > best) {  // strict: earliest on ties
+        best = sum;
+        tstar = t;
+      }
+    }
+    uint32_t relnum = 0;
+    for (int k = 1; k < W; ++k) relnum += (uint32_t)k * (uint32_t)tr[tstar + k];
+    const uint32_t p = fastmod(g, n_pixels, pix_inv);
+    const Result r = finish_trace(W, best, tstar, relnum, __ldg(pedestal + p), __ldg(gain + p));
+    out_sum[g] = r.sum;
+    out_start[g] = r.start;
+    out_charge[g] = r.charge;
+    out_time[g] = r.time;
+  }
+}
+
+// ------------------------------------------------------------- dispatch ----
+constexpr int kMaxDevices = 32;
+
+struct DeviceInfo {
+  std::atomic<int> ready{0};
+  int sms = 0;
+};
+DeviceInfo g_dev[kMaxDevices];
+
+cudaError_t device_sms(int dev, int* sms) {
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  DeviceInfo& d = g_dev[dev];
+  if (!d.ready.load(std::memory_order_acquire)) {
+    int n = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    d.sms = n;
+    d.ready.store(1, std::memory_order_release);
+  }
+  *sms = d.sms;
+  return cudaSuccess;
+}
+
+template <class C>
+struct TileLauncher {
+  static std::atomic<int> ready[kMaxDevices];
+  static int ctas_per_sm[kMaxDevices];
+
+  static cudaError_t prepare(int dev) {
+    if (ready[dev].load(std::memory_order_acquire)) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(extract_tile_kernel<C>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         C::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, extract_tile_kernel<C>, C::NT,
+                                                      C::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) return cudaErrorLaunchOutOfResources;
+    ctas_per_sm[dev] = occ;
+    ready[dev].store(1, std::memory_order_release);
+    return cudaSuccess;
+  }
+
+  static cudaError_t launch(const uint16_t* wf, uint32_t n_traces, uint32_t n_pixels,
+                            uint32_t pix_inv, const int32_t* pedestal, const float* gain,
+                            int32_t* out_sum, int32_t* out_start, float* out_charge,
+                            float* out_time, cudaStream_t stream) {
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
+    if ((e = prepare(dev)) != cudaSuccess) return e;
+    const uint32_t n_full = n_traces / C::TILE_TRACES;
+    uint32_t grid = (uint32_t)(sms * ctas_per_sm[dev]);
+    if (grid > n_full) grid = n_full;
+    if (grid < 1) grid = 1;
+    const uintptr_t o = (uintptr_t)out_sum | (uintptr_t)out_start | (uintptr_t)out_charge |
+                        (uintptr_t)out_time;
+    const int vec_store = (o % 8 == 0) ? 1 : 0;
+    extract_tile_kernel<C><<<grid, C::NT, C::SMEM_BYTES, stream>>>(
+        wf, n_traces, n_pixels, pix_inv, pedestal, gain, out_sum, out_start, out_charge, out_time,
+        vec_store);
+    rta_count_launch();
+    return cudaGetLastError();
+  }
+};
+template <class C>
+std::atomic<int> TileLauncher<C>::ready[kMaxDevices];
+template <class C>
+int TileLauncher<C>::ctas_per_sm[kMaxDevices];
+
+// The four shapes of BASELINE.json:configs (NT, STAGES tuned on B200; see
+// DESIGN.md "Kernels" for the shared-memory budget of each).
+using CfgS30W7 = TileCfg<30, 7, 256, 3>;
+using CfgS40W7 = TileCfg<40, 7, 256, 3>;
+using CfgS25W4 = TileCfg<25, 4, 256, 3>;
+using CfgS128W8 = TileCfg<128, 8, 128, 2>;
+
+}  // namespace
+
+const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16) {
+  if (aligned16) {
+    if (S == 30 && W == 7) return "tile<S=30,W=7>";
+    if (S == 40 && W == 7) return "tile<S=40,W=7>";
+    if (S == 25 && W == 4) return "tile<S=25,W=4>";
+    if (S == 128 && W == 8) return "tile<S=128,W=8>";
+  }
+  return "generic";
+}
+
+cudaError_t rta_launch_extract(const uint16_t* wf, int64_t n_traces64, int32_t n_pixels,
+                               int32_t S, const int32_t* pedestal, const float* gain, int32_t W,
+                               int32_t* out_sum, int32_t* out_start, float* out_charge,
+                               float* out_time, cudaStream_t stream, bool force_generic) {
+  if (n_traces64 <= 0) return cudaSuccess;
+  const uint32_t n_traces = (uint32_t)n_traces64;
+  const uint32_t P = (uint32_t)n_pixels;
+  const uint64_t inv64 = (1ull << 32) / P;
+  const uint32_t inv = inv64 > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)inv64;
+  const bool aligned16 = ((uintptr_t)wf % 16) == 0;
+  if (!force_generic && aligned16) {
+    if (S == 30 && W == 7)
+      return TileLauncher<CfgS30W7>::launch(wf, n_traces, P, inv, pedestal, gain, out_sum,
+                                            out_start, out_charge, out_time, stream);
+    if (S == 40 && W == 7)
+      return TileLauncher<CfgS40W7>::launch(wf, n_traces, P, inv, pedestal, gain, out_sum,
+                                            out_start, out_charge, out_time, stream);
+    if (S == 25 && W == 4)
+      return TileLauncher<CfgS25W4>::launch(wf, n_traces, P, inv, pedestal, gain, out_sum,
+                                            out_start, out_charge, out_time, stream);
+    if (S == 128 && W == 8)
+      return TileLauncher<CfgS128W8>::launch(wf, n_traces, P, inv, pedestal, gain, out_sum,
+                                             out_start, out_charge, out_time, stream);
+  }
+  int dev = 0, sms = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
+  uint32_t grid = (n_traces + 255u) / 256u;
+  const uint32_t cap = (uint32_t)sms * 8u;
+  if (grid > cap) grid = cap;
+  extract_generic_kernel<<<grid, 256, 0, stream>>>(wf, n_traces, S, W, P, inv, pedestal, gain,
+                                                   out_sum, out_start, out_charge, out_time);
+  rta_count_launch();
+  return cudaGetLastError();
+}

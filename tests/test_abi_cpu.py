@@ -1,0 +1,126 @@
+"""CPU-only checks of the boundary: librta.so builds, loads, exports every
+symbol include/rta.h declares, and rejects bad arguments before touching CUDA
+(pin P17). No compute call is made here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_1307_6489_b200 as rta
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "rta.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(rta_[a-z_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    L = rta.lib()
+    names = declared_symbols()
+    assert {"rta_extract", "rta_extract_stream", "rta_extract_host", "rta_strerror",
+            "rta_last_cuda_error", "rta_kernel_name", "rta_launch_count",
+            "rta_shutdown"} <= set(names)
+    for n in names:
+        assert hasattr(L, n), n
+
+
+def test_library_links_no_torch():
+    import subprocess
+    out = subprocess.run(["ldd", rta.lib()._name], capture_output=True, text=True).stdout
+    assert "torch" not in out and "c10" not in out
+
+
+def _call(n_events=1, n_pixels=4, n_samples=30, W=7, wf=0x1000, ped=0x2000, gain=0x3000,
+          o=(0x4000, 0x5000, 0x6000, 0x7000)):
+    return rta.lib().rta_extract(wf, n_events, n_pixels, n_samples, ped, gain, W, *o, 0)
+
+
+def test_shape_errors_before_any_cuda_call():
+    assert _call(W=0) == rta.RTA_ERR_SHAPE
+    assert _call(W=31) == rta.RTA_ERR_SHAPE               # W > S
+    assert _call(n_samples=0) == rta.RTA_ERR_SHAPE
+    assert _call(n_pixels=0) == rta.RTA_ERR_SHAPE
+    assert _call(n_events=-1) == rta.RTA_ERR_SHAPE
+
+
+def test_unsupported_sizes():
+    assert _call(n_events=2 ** 31, n_pixels=1) == rta.RTA_ERR_UNSUPPORTED
+    assert _call(n_events=2 ** 20, n_pixels=2 ** 11) == rta.RTA_ERR_UNSUPPORTED
+    assert _call(n_samples=2048, W=17) == rta.RTA_ERR_UNSUPPORTED   # 2048*17*65535 >= 2^31
+    assert _call(n_samples=182, W=182) == rta.RTA_ERR_UNSUPPORTED
+
+
+def test_null_and_alignment():
+    assert _call(wf=None) == rta.RTA_ERR_NULL
+    assert _call(ped=None) == rta.RTA_ERR_NULL
+    assert _call(gain=None) == rta.RTA_ERR_NULL
+    assert _call(o=(0x4000, None, 0x6000, 0x7000)) == rta.RTA_ERR_NULL
+    assert _call(wf=0x1001) == rta.RTA_ERR_ALIGN
+    assert _call(o=(0x4002, 0x5000, 0x6000, 0x7000)) == rta.RTA_ERR_ALIGN
+
+
+def test_empty_input_is_ok_and_touches_nothing():
+    # R17: no work -> RTA_OK even with null pointers, nothing enqueued
+    before = rta.rta_launch_count()
+    assert _call(n_events=0, wf=None, ped=None, gain=None, o=(None,) * 4) == rta.RTA_OK
+    L = rta.lib()
+    assert L.rta_extract_stream(None, 0, 4, 30, None, None, 7, None, None, None, None, 0, 0) == rta.RTA_OK
+    assert L.rta_extract_host(None, 0, 4, 30, None, None, 7, None, None, None, None, 0) == rta.RTA_OK
+    assert rta.rta_launch_count() == before
+
+
+def test_stream_and_host_entry_points_validate_too():
+    L = rta.lib()
+    assert L.rta_extract_stream(0x1000, 1, 4, 30, 0x2000, 0x3000, 31, 0x4000, 0x5000,
+                                0x6000, 0x7000, 0, 0) == rta.RTA_ERR_SHAPE
+    assert L.rta_extract_host(0x1000, 1, 4, 30, None, 0x3000, 7, 0x4000, 0x5000,
+                              0x6000, 0x7000, 0) == rta.RTA_ERR_NULL
+
+
+def test_strerror_and_kernel_names():
+    for s in range(0, 8):
+        assert isinstance(rta.rta_strerror(s), str) and rta.rta_strerror(s)
+    assert rta.rta_kernel_name(40, 7) == "tile<S=40,W=7>"
+    assert rta.rta_kernel_name(30, 7) == "tile<S=30,W=7>"
+    assert rta.rta_kernel_name(25, 4) == "tile<S=25,W=4>"
+    assert rta.rta_kernel_name(128, 8) == "tile<S=128,W=8>"
+    assert rta.rta_kernel_name(40, 7, aligned16=False) == "generic"
+    assert rta.rta_kernel_name(41, 7) == "generic"
+
+
+def test_binding_raises_on_error_status():
+    with pytest.raises(rta.RtaError) as ei:
+        rta.rta_extract(0x1000, 1, 4, 30, 0x2000, 0x3000, 99, 0x4000, 0x5000, 0x6000,
+                        0x7000, stream=0)
+    assert ei.value.status == rta.RTA_ERR_SHAPE
+
+
+def test_no_cpu_fallback_without_a_device():
+    """On a box without a GPU a real compute call must fail loudly."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    import numpy as np
+    wf = np.zeros((1, 4, 30), np.uint16)
+    ped = np.zeros(4, np.int32)
+    g = np.ones(4, np.float32)
+    outs = [np.zeros(4, np.int32), np.zeros(4, np.int32), np.zeros(4, np.float32),
+            np.zeros(4, np.float32)]
+    with pytest.raises(rta.RtaError) as ei:
+        rta.rta_extract_host(wf, 1, 4, 30, ped, g, 7, *outs)
+    assert ei.value.status in (rta.RTA_ERR_CUDA, rta.RTA_ERR_NOMEM)
+
+
+def test_shard_events_partitions_exactly():
+    for n in (0, 1, 7, 10_000, 200_000):
+        for w in (1, 2, 3, 8):
+            parts = [rta.shard_events(n, w, r) for r in range(w)]
+            assert parts[0][0] == 0
+            assert sum(c for _, c in parts) == n
+            for (a, ca), (b, _) in zip(parts, parts[1:]):
+                assert a + ca == b
+            assert max(c for _, c in parts) - min(c for _, c in parts) <= 1

@@ -1,0 +1,223 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by
+element on the same seeded inputs. Bar = BASELINE.json:north_star: out_sum and
+out_start bit-exact, charge within relative 1e-6, peak time within absolute
+1e-4 samples. (The kernels are designed to be bit-identical on the floats too;
+`bit_identical` is asserted where the design guarantees it.)"""
+import itertools
+import json
+import os
+
+import numpy as np
+import pytest
+
+import dl0gen
+import oracle
+from tests._checks import check_invariants
+from tests._gpu import alloc_outputs, assert_parity, bit_identical, run_gpu, to_dev_u16
+
+pytestmark = pytest.mark.gpu
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "hand_worked.json")
+SHAPES = [(30, 7), (40, 7), (25, 4), (128, 8)]          # specialised tile kernels
+
+
+def both(wf, ped, gain, W):
+    want = oracle.extract(wf, ped, gain, W)
+    for generic in (False, True):
+        got = run_gpu(wf, ped, gain, W, generic=generic)
+        assert_parity(got, want, "generic" if generic else "dispatch")
+        assert bit_identical(got, want)
+    return want
+
+
+def test_hand_worked_fixtures_on_gpu():
+    for c in json.load(open(GOLD))["cases"]:
+        E, P, S = c["n_events"], c["n_pixels"], c["n_samples"]
+        wf = np.array(c["wf"], np.uint16).reshape(E, P, S)
+        got = run_gpu(wf, np.array(c["pedestal"], np.int32),
+                      np.array(c["gain"], np.float32), c["W"])
+        assert got[0].tolist() == c["out_sum"] and got[1].tolist() == c["out_start"]
+        assert got[2].tolist() == [float(np.float32(v)) for v in c["out_charge"]]
+        want_t = [float(np.float32(np.float64(n) / np.float64(d)))
+                  for n, d in zip(c["time_num"], c["time_den"])]
+        assert got[3].tolist() == want_t
+
+
+@pytest.mark.parametrize("S,Ws,values,ped", [
+    (4, [2], [9, 10, 11], 10), (5, [1, 2, 3, 4, 5], [0, 1, 2, 3], 1), (12, [3], [0, 1], 0)])
+def test_exhaustive_tiny_traces(S, Ws, values, ped):
+    """Pin P10 through the GPU: every trace over a small alphabet."""
+    tr = np.array(list(itertools.product(values, repeat=S)), np.uint16)
+    n = len(tr)
+    P = 4 if n % 4 == 0 else 3
+    wf = tr.reshape(n // P, P, S)
+    pedv = np.full(P, ped, np.int32)
+    gain = np.linspace(0.9, 1.1, P).astype(np.float32)
+    for W in Ws:
+        both(wf, pedv, gain, W)
+
+
+@pytest.mark.parametrize("S,W", SHAPES)
+def test_exhaustive_tie_patterns_in_specialised_shapes(S, W):
+    """All 2^12 on/off patterns of a 12-sample region placed at the start, the
+    middle and the end of the trace — every tie pattern the key must resolve."""
+    pats = np.array(list(itertools.product([0, 1], repeat=12)), np.uint16)  # 4096
+    for off in (0, (S - 12) // 2, S - 12):
+        tr = np.full((4096, S), 100, np.uint16)
+        tr[:, off:off + 12] += pats * 5
+        wf = tr.reshape(64, 64, S)
+        ped = np.full(64, 100, np.int32)
+        ped[::3] = 101                                   # some negative samples
+        both(wf, ped, np.linspace(0.9, 1.1, 64).astype(np.float32), W)
+
+
+@pytest.mark.parametrize("S,W", SHAPES)
+def test_closed_forms_in_specialised_shapes(S, W):
+    P = 3
+    ped = np.array([400, 0, 4095], np.int32)
+    gain = np.array([1.0, 0.5, 1.0625], np.float32)
+    # P1 constant traces: below, at and above pedestal
+    for c in (0, 400, 4095, 65535):
+        wf = np.full((5, P, S), c, np.uint16)
+        s, t, q, tm = run_gpu(wf, ped, gain, W)
+        assert (t == 0).all()
+        assert (s.reshape(5, P) == W * (c - ped.astype(np.int64))).all()
+        assert (tm == np.float32((W - 1) / 2)).all()
+        assert (q.reshape(5, P) == (W * (c - ped.astype(np.float64)) * gain).astype(np.float32)).all()
+    # P2 delta at every position, one event per position
+    A = 57
+    wf = np.broadcast_to(ped.astype(np.uint16)[None, :, None], (S, P, S)).copy()
+    for k in range(S):
+        wf[k, :, k] += A
+    s, t, q, tm = run_gpu(wf, ped, gain, W)
+    ks = np.repeat(np.arange(S), P)
+    assert (s == A).all()
+    assert (t == np.maximum(0, ks - W + 1)).all()
+    assert (tm == ks.astype(np.float32)).all()
+    assert (q == (A * np.tile(gain, S).astype(np.float64)).astype(np.float32)).all()
+    both(wf, ped, gain, W)
+
+
+@pytest.mark.parametrize("S,W", SHAPES + [(31, 5), (64, 16), (7, 7), (9, 1), (200, 3)])
+@pytest.mark.parametrize("n_traces_shape", [(1, 1), (3, 5), (7, 37), (2, 129), (5, 257), (4, 1031)])
+def test_random_full_uint16_range_and_ragged_sizes(S, W, n_traces_shape):
+    """Any uint16 value (R13), sizes around the tile boundaries (128/256/512
+    traces) and pedestals of both signs and beyond the samples (R2)."""
+    E, P = n_traces_shape
+    rng = np.random.default_rng(S * 7919 + W * 31 + E * P)
+    wf = rng.integers(0, 65536, size=(E, P, S)).astype(np.uint16)
+    wf[rng.random((E, P)) < 0.2] = 65535                  # key overflow guard: all-max traces
+    ped = rng.integers(-70000, 70000, P).astype(np.int32)
+    gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
+    both(wf, ped, gain, W)
+
+
+@pytest.mark.parametrize("S,W", SHAPES)
+def test_extreme_pedestals_take_the_wide_path(S, W):
+    """|pedestal| up to 2^30: int64 numerator and the double-precision branch."""
+    rng = np.random.default_rng(S)
+    E, P = 3, 300
+    wf = rng.integers(0, 65536, size=(E, P, S)).astype(np.uint16)
+    ped = rng.integers(-2 ** 30, 2 ** 30, P).astype(np.int32)
+    ped[:50] = rng.integers(-2 ** 26, 2 ** 26, 50)
+    gain = rng.uniform(-3, 3, P).astype(np.float32)
+    gain[0], gain[1], gain[2] = np.float32("nan"), np.float32("inf"), np.float32(1e-42)
+    want = oracle.extract(wf, ped, gain, W)
+    got = run_gpu(wf, ped, gain, W)
+    assert (got[0] == want[0]).all() and (got[1] == want[1]).all()
+    assert bit_identical(got, want)
+
+
+def test_unaligned_input_takes_generic_kernel_and_agrees():
+    import torch
+    import paper_1307_6489_b200 as rta
+    c = dl0gen.CONFIGS["C1"]
+    ped, gain = dl0gen.calib(c)
+    wf = dl0gen.events_cpu(c, 0, 8)
+    want = oracle.extract(wf, ped, gain, c.W)
+    flat = torch.empty(wf.size + 8, dtype=torch.int16, device="cuda")
+    flat[1:1 + wf.size] = torch.from_numpy(wf.reshape(-1).view(np.int16)).cuda()
+    view = flat[1:1 + wf.size]                            # 2-byte aligned only
+    assert view.data_ptr() % 16 != 0
+    d_ped = torch.from_numpy(ped).cuda()
+    d_gain = torch.from_numpy(gain).cuda()
+    outs = alloc_outputs(8 * c.n_pixels)
+    rta.rta_extract(view, 8, c.n_pixels, c.n_samples, d_ped, d_gain, c.W, *outs)
+    torch.cuda.synchronize()
+    assert bit_identical(tuple(o.cpu().numpy() for o in outs), want)
+
+
+def test_odd_output_alignment_takes_scalar_stores():
+    """S=25 pairs traces per thread and prefers 8-byte stores; outputs that are
+    only 4-byte aligned must still be written correctly."""
+    import torch
+    import paper_1307_6489_b200 as rta
+    c = dl0gen.CONFIGS["C3"]
+    ped, gain = dl0gen.calib(c)
+    wf = dl0gen.events_cpu(c, 0, 3)
+    n = 3 * c.n_pixels
+    want = oracle.extract(wf, ped, gain, c.W)
+    d_wf = to_dev_u16(wf)
+    bufs = [torch.zeros(n + 1, dtype=dt, device="cuda")
+            for dt in (torch.int32, torch.int32, torch.float32, torch.float32)]
+    outs = [b[1:] for b in bufs]
+    assert outs[0].data_ptr() % 8 == 4
+    rta.rta_extract(d_wf, 3, c.n_pixels, c.n_samples, torch.from_numpy(ped).cuda(),
+                    torch.from_numpy(gain).cuda(), c.W, *outs)
+    torch.cuda.synchronize()
+    assert bit_identical(tuple(o.cpu().numpy() for o in outs), want)
+    assert all(float(b[0]) == 0 for b in bufs)            # nothing written before the view
+
+
+def test_C1_full_parity():
+    c = dl0gen.CONFIGS["C1"]
+    ped, gain = dl0gen.calib(c)
+    wf = dl0gen.events_cpu(c, threads=4)
+    want = both(wf, ped, gain, c.W)
+    check_invariants(wf, ped, gain, c.W, *want)
+
+
+@pytest.mark.parametrize("name,n_ev", [("C2", 23), ("C3", 19), ("C4", 11)])
+def test_config_models_small_batches(name, n_ev):
+    """The C2-C4 signal models at sizes the oracle finishes at once: several
+    tiles per CTA plus a ragged tail (n_traces is not a multiple of the tile)."""
+    c = dl0gen.CONFIGS[name]
+    ped, gain = dl0gen.calib(c)
+    wf = dl0gen.events_cpu(c, 100, n_ev, threads=4)
+    both(wf, ped, gain, c.W)
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4"])
+def test_full_size_configs_sampled_against_oracle(name):
+    """BASELINE.json's full sizes, in the launch configuration bench.py times
+    (one rta_extract over the whole device-resident batch): generate on the
+    GPU, extract, then compare sampled event blocks with the oracle run on the
+    same bytes regenerated on the host, and check the size-independent
+    invariants (P8/P9) on them."""
+    import torch
+    import paper_1307_6489_b200 as rta
+    c = dl0gen.CONFIGS[name]
+    ped, gain = dl0gen.calib(c)
+    d_wf = torch.empty((c.n_events, c.n_pixels, c.n_samples), dtype=torch.int16, device="cuda")
+    dl0gen.events_cuda(c, d_wf.data_ptr(), 0, c.n_events, torch.cuda.current_stream().cuda_stream)
+    d_ped = torch.from_numpy(ped).cuda()
+    d_gain = torch.from_numpy(gain).cuda()
+    outs = alloc_outputs(c.n_traces)
+    rta.rta_extract(d_wf, c.n_events, c.n_pixels, c.n_samples, d_ped, d_gain, c.W, *outs)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(5)
+    blocks = [0, c.n_events - 12] + sorted(rng.integers(12, c.n_events - 24, 6).tolist())
+    for e0 in blocks:
+        wf = dl0gen.events_cpu(c, e0, 12, threads=4)
+        # the device bytes are the host generator's bytes
+        assert (d_wf[e0:e0 + 12].cpu().numpy().view(np.uint16) == wf).all()
+        want = oracle.extract(wf, ped, gain, c.W)
+        lo, hi = e0 * c.n_pixels, (e0 + 12) * c.n_pixels
+        got = tuple(o[lo:hi].cpu().numpy() for o in outs)
+        assert_parity(got, want, "%s events %d.." % (name, e0))
+        assert bit_identical(got, want)
+        check_invariants(wf, ped, gain, c.W, *got)
+    # whole-batch properties that hold at any size
+    s, t = outs[0], outs[1]
+    assert int(t.min()) >= 0 and int(t.max()) <= c.n_samples - c.W
+    assert bool(torch.isfinite(outs[3]).all()) and bool(torch.isfinite(outs[2]).all())
