@@ -1,0 +1,478 @@
+#!/usr/bin/env python
+"""bench.py — waveform GB/s extracted on B200 (BASELINE.json:metric).
+
+One "step" is one pass of the whole hot path (ingest,
+pedestal, window sums, arg-max, stores, charge, peak time) over one batch of
+synthetic camera waveforms, i.e. one rta_extract call through the C ABI.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C3|C4|C1]
+  python bench.py --impl reference ...      # the oracle on the host cores
+
+Prints ONE JSON line (rank 0). Keys beyond the driver's contract:
+  roofline      dominant kernel against the measured HBM peak
+  cpu_baseline  the oracle timed on this box's host cores (N=1, rank 0)
+  e2e           same metric through rta_extract_host (pinned host buffers in
+                and out, H2D/D2H inside the timed region)
+  sustained     BASELINE.json:configs[4] (C5): 29.68 GB of pinned host memory
+                fed through rta_extract_stream in 1 GiB chunks, against the
+                host-link bandwidth measured in the same run and the paper's
+                0.5-8 GB/s array data rate
+  configs       kernel-only numbers for the other single-GPU configs (C3, C4)
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "raw_waveform_GBps_extracted"
+UNIT = "GB/s"
+FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+PAPER_RATE_GBS = (0.5, 8.0)       # PAPER.md:27 / PAPER.md:67, whole-array data rate
+ALGO_BYTES_PER_TRACE_OUT = 16     # 2*S read + 16 written per trace
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C4"])
+    ap.add_argument("--no-extra", action="store_true", help="skip configs/e2e/sustained/cpu legs")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the 29.68 GB C5 leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--e2e-chunk-mb", type=int, default=64)
+    return ap.parse_args()
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json, burst copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(name):
+    """DRAM bytes per launch from the committed ncu --set full capture, if any."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(p)).get(name)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line)
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------- #
+def reference_arm(args):
+    """The oracle, as it stands, on the host cores: same metric and config.
+    Each step extracts a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import numpy as np
+    import dl0gen
+    import oracle
+    cfg = dl0gen.CONFIGS[args.workload]
+    cores = os.cpu_count() or 1
+    ped, gain = dl0gen.calib(cfg)
+    # ~0.3 GB/s per core: size the per-step sample for about 1 s of all-cores work
+    n_ev = max(cores, min(cfg.n_events, 200 * cores))
+    wf = dl0gen.events_cpu(cfg, 0, n_ev, threads=cores)
+    for _ in range(max(1, min(args.warmup, 2))):
+        oracle.extract_threads(wf, ped, gain, cfg.W, cores)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.extract_threads(wf, ped, gain, cfg.W, cores)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = wf.nbytes / dt / 1e9
+    sample = "first %d of %d events of %s per step, %d threads" % (n_ev, cfg.n_events, cfg.name, cores)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT,
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+        "config": {"workload": "%s: %s" % (cfg.name, cfg.label), "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+    return 0
+
+
+# --------------------------------------------------------------------------- #
+def time_steps(run, steps, stream):
+    """K back-to-back launches with an event between each: per-launch device
+    durations on the launching stream; their sum is the timed region."""
+    import torch
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    ev[0].record(stream)
+    for i in range(steps):
+        run()
+        ev[i + 1].record(stream)
+    torch.cuda.synchronize()
+    return [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
+
+
+def device_batch(cfg, torch, dl0gen):
+    d_wf = torch.empty((cfg.n_events, cfg.n_pixels, cfg.n_samples), dtype=torch.int16, device="cuda")
+    dl0gen.events_cuda(cfg, d_wf.data_ptr(), 0, cfg.n_events, torch.cuda.current_stream().cuda_stream)
+    ped, gain = dl0gen.calib(cfg)
+    d_ped, d_gain = torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda()
+    outs = [torch.empty(cfg.n_traces, dtype=dt, device="cuda")
+            for dt in (torch.int32, torch.int32, torch.float32, torch.float32)]
+    torch.cuda.synchronize()
+    return d_wf, d_ped, d_gain, outs, ped, gain
+
+
+def kernel_only(cfg, steps, warmup, torch, dl0gen, rta, barrier=None):
+    d_wf, d_ped, d_gain, outs, ped, gain = device_batch(cfg, torch, dl0gen)
+    stream = torch.cuda.current_stream()
+
+    def run():
+        rta.rta_extract(d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain,
+                        cfg.W, *outs, stream=stream)
+    for _ in range(max(3, warmup)):
+        run()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    before = rta.rta_launch_count()
+    per = time_steps(run, steps, stream)
+    launches = rta.rta_launch_count() - before
+    if barrier:
+        barrier()
+    checksum = int(d_wf.view(-1)[: min(d_wf.numel(), 1 << 26)].sum(dtype=torch.int64))
+    return {"per_launch_ms": per, "launches": launches, "checksum_first_64Mi_samples": checksum,
+            "keep": (d_wf, d_ped, d_gain, outs, ped, gain)}
+
+
+def summarise(cfg, per_ms, peak):
+    tot_ms = sum(per_ms)
+    avg = tot_ms / len(per_ms)
+    algo = cfg.input_bytes + cfg.output_bytes
+    return {
+        "workload": "%s: %s" % (cfg.name, cfg.label),
+        "ms_avg": avg, "ms_median": statistics.median(per_ms), "ms_best": min(per_ms),
+        "waveform_GBps": cfg.input_bytes / avg / 1e6,
+        "traces_per_s": cfg.n_traces / avg * 1e3,
+        "algorithmic_GBps": algo / avg / 1e6,
+        "frac_of_measured_hbm": algo / avg / 1e6 / peak,
+        "frac_of_nominal_8TBps": algo / avg / 1e6 / 8000.0,
+    }
+
+
+def host_link_bandwidth(torch, nbytes=1 << 30, reps=10):
+    """Pinned H2D cudaMemcpyAsync bandwidth, best of `reps` (the H2D-fed roofline)."""
+    h = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    d = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    best = None
+    for _ in range(reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        d.copy_(h, non_blocking=True)
+        b.record()
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b)
+        best = ms if best is None else min(best, ms)
+    del h, d
+    return nbytes / best / 1e6
+
+
+def e2e_leg(cfg, keep, steps, chunk_mb, torch, rta):
+    """Through the public host API: pinned host waveforms in, host results out."""
+    d_wf, d_ped, d_gain, outs, ped, gain = keep
+    h_wf = torch.empty(d_wf.shape, dtype=torch.int16, pin_memory=True)
+    h_wf.copy_(d_wf)
+    h_out = [torch.empty(cfg.n_traces, dtype=o.dtype, pin_memory=True) for o in outs]
+    torch.cuda.synchronize()
+    chunk = chunk_mb << 20
+
+    def run():
+        rta.rta_extract_host(h_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, ped, gain,
+                             cfg.W, *h_out, chunk_bytes=chunk)
+    for _ in range(2):
+        run()
+    # the host copy of the result equals the device-resident result
+    ok = all(bool((ho.cuda() == o).all()) for ho, o in zip(h_out[:2], outs[:2]))
+    torch.cuda.synchronize()
+    k = max(3, min(steps, 10))
+    before = rta.rta_launch_count()
+    t0 = time.perf_counter()
+    for _ in range(k):
+        run()                                    # synchronous by contract
+    dt = (time.perf_counter() - t0) / k
+    launches = (rta.rta_launch_count() - before) // k
+    del h_wf, h_out
+    return {"value": cfg.input_bytes / dt / 1e9, "unit": UNIT, "ms_per_step": dt * 1e3,
+            "h2d_bytes_per_step": cfg.input_bytes + 8 * cfg.n_pixels,
+            "d2h_bytes_per_step": cfg.output_bytes, "steps": k, "chunk_bytes": chunk,
+            "launches_per_step": launches, "matches_device_result": ok,
+            "api": "rta_extract_host (pinned host in/out, double-buffered H2D, D2H on a third stream)"}
+
+
+def sustained_leg(torch, dl0gen, rta, link_gbs):
+    """BASELINE.json:configs[4]: C5 in pinned host memory, 1 GiB chunks."""
+    cfg = dl0gen.CONFIGS["C5"]
+    try:
+        avail_kb = int([l for l in open("/proc/meminfo") if l.startswith("MemAvailable")][0].split()[1])
+    except Exception:
+        avail_kb = 0
+    if avail_kb < 44 * 1024 * 1024:
+        return {"skipped": "needs 29.68 GB of pinned host memory; MemAvailable=%d MB" % (avail_kb // 1024)}
+    t0 = time.perf_counter()
+    host = torch.empty((cfg.n_events, cfg.n_pixels, cfg.n_samples), dtype=torch.int16, pin_memory=True)
+    t_alloc = time.perf_counter() - t0
+    gen_ev = 10_000
+    stage = torch.empty((gen_ev, cfg.n_pixels, cfg.n_samples), dtype=torch.int16, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    for e0 in range(0, cfg.n_events, gen_ev):
+        dl0gen.events_cuda(cfg, stage.data_ptr(), e0, gen_ev, st)
+        host[e0:e0 + gen_ev].copy_(stage)
+    torch.cuda.synchronize()
+    del stage
+    ped, gain = dl0gen.calib(cfg)
+    d_ped, d_gain = torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda()
+    outs = [torch.empty(cfg.n_traces, dtype=dt, device="cuda")
+            for dt in (torch.int32, torch.int32, torch.float32, torch.float32)]
+    stream = torch.cuda.current_stream()
+
+    def run():
+        rta.rta_extract_stream(host, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain,
+                               cfg.W, *outs, chunk_bytes=1 << 30, stream=stream)
+    run()                                        # warm-up: allocates the workspace
+    torch.cuda.synchronize()
+    times = []
+    before = rta.rta_launch_count()
+    for _ in range(2):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()                 # first cudaMemcpyAsync issue ...
+        run()
+        torch.cuda.synchronize()                 # ... to completion of the last kernel
+        times.append(time.perf_counter() - t0)
+    launches = (rta.rta_launch_count() - before) // 2
+    dt = min(times)
+    val = cfg.input_bytes / dt / 1e9
+    res = {"workload": "%s: %s" % (cfg.name, cfg.label), "value": val, "unit": UNIT,
+           "seconds": dt, "traces_per_s": cfg.n_traces / dt, "chunk_bytes": 1 << 30,
+           "chunks": launches, "h2d_bytes": cfg.input_bytes,
+           "host_link_GBps_measured": link_gbs, "frac_of_host_link": val / link_gbs,
+           "paper_array_rate_GBps": list(PAPER_RATE_GBS),
+           "x_paper_max_rate": val / PAPER_RATE_GBS[1],
+           "pinned_alloc_s": t_alloc, "outputs": "stay on device (5.94 GB)"}
+    del host, outs
+    rta.rta_shutdown()
+    return res
+
+
+def cpu_baseline_leg(cfg, keep, dl0gen):
+    """The oracle, as it stands, on this box's host cores, on the same bytes."""
+    import numpy as np
+    import oracle
+    d_wf, _, _, outs, ped, gain = keep
+    cores = os.cpu_count() or 1
+    # bounded sample: ~0.28 GB/s per thread -> about 5 s single-threaded
+    n_ev = min(cfg.n_events, max(64, int(1.4e9 // (cfg.n_pixels * cfg.n_samples * 2))))
+    wf = d_wf[:n_ev].cpu().numpy().view(np.uint16)
+    t0 = time.perf_counter()
+    r1 = oracle.extract(wf, ped, gain, cfg.W)
+    t1 = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    oracle.extract_threads(wf, ped, gain, cfg.W, cores)
+    tn = time.perf_counter() - t0
+    n = n_ev * cfg.n_pixels
+    ints_equal = bool((outs[0][:n].cpu().numpy() == r1[0]).all()
+                      and (outs[1][:n].cpu().numpy() == r1[1]).all())
+    floats_equal = bool((outs[2][:n].cpu().numpy() == r1[2]).all()
+                        and (outs[3][:n].cpu().numpy() == r1[3]).all())
+    return {"value": wf.nbytes / tn / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "first %d of %d events of %s (%.2f GB), same bytes as the GPU run"
+                      % (n_ev, cfg.n_events, cfg.name, wf.nbytes / 1e9),
+            "single_thread_value": wf.nbytes / t1 / 1e9,
+            "traces_per_s": n / tn, "single_thread_traces_per_s": n / t1,
+            "gpu_matches_oracle_on_sample": {"ints_bit_exact": ints_equal,
+                                             "floats_bit_exact": floats_equal}}
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return reference_arm(args)
+
+    import torch
+    import dl0gen
+    import paper_1307_6489_b200 as rta
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    rta.lib()
+    cfg = dl0gen.CONFIGS[args.workload]
+    peak, peak_src = hbm_peak()
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    # Weak scaling: every rank extracts its own batch of the named workload
+    # (independent events; no data-path collective).
+    main_run = kernel_only(cfg, args.steps, args.warmup, torch, dl0gen, rta, barrier)
+    clocks = sampler.stop()
+    t_local = sum(main_run["per_launch_ms"])
+    t_max = t_local
+    if dist is not None:
+        t = torch.tensor([t_local], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_max = float(t.item())
+    ms_per_step = t_max / args.steps
+    value = world * cfg.input_bytes / ms_per_step / 1e6
+    summ = summarise(cfg, main_run["per_launch_ms"], peak)
+    algo_bytes = cfg.input_bytes + cfg.output_bytes
+    kname = rta.rta_kernel_name(cfg.n_samples, cfg.W, True)
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+        "config": {
+            "workload": "%s: %s" % (cfg.name, cfg.label),
+            "per_gpu": "%d events x %d pixels x %d samples uint16, W=%d" % (
+                cfg.n_events, cfg.n_pixels, cfg.n_samples, cfg.W),
+            "l2": "input %.2f GB per step exceeds the 126 MB L2 (no flush needed)" % (cfg.input_bytes / 1e9),
+            "parallelism": "independent events per GPU, no collective",
+            "seed": cfg.seed, "input_checksum": main_run["checksum_first_64Mi_samples"],
+        },
+        "traces_per_s": world * cfg.n_traces / ms_per_step * 1e3,
+        "pct_of_measured_hbm": 100.0 * summ["frac_of_measured_hbm"],
+        "gpu_launches": main_run["launches"],
+        "clocks": clocks,
+        "roofline": {
+            "bound": "hbm", "kernel": kname,
+            "achieved": summ["algorithmic_GBps"], "peak": peak, "unit": "GB/s",
+            "frac": summ["frac_of_measured_hbm"], "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": algo_bytes,
+            "bytes_per_trace": 2 * cfg.n_samples + ALGO_BYTES_PER_TRACE_OUT,
+            "avg_launch_ms": summ["ms_avg"],
+            "traffic": ncu_traffic(kname),
+            "frac_of_nominal_8TBps": summ["frac_of_nominal_8TBps"],
+        },
+    }
+
+    if not args.no_extra:
+        # host-fed leg on every rank (each GPU has its own host link); max over ranks
+        keep = main_run["keep"]
+        barrier()
+        e2e = e2e_leg(cfg, keep, args.steps, args.e2e_chunk_mb, torch, rta)
+        if dist is not None:
+            t = torch.tensor([e2e["ms_per_step"]], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e["ms_per_step"] = float(t.item())
+            e2e["value"] = world * cfg.input_bytes / e2e["ms_per_step"] / 1e6
+            e2e["h2d_bytes_per_step"] *= world
+            e2e["d2h_bytes_per_step"] *= world
+        out["e2e"] = e2e
+        if rank == 0 and world == 1:
+            if not args.no_cpu:
+                out["cpu_baseline"] = cpu_baseline_leg(cfg, keep, dl0gen)
+            main_run["keep"] = keep = None
+            torch.cuda.empty_cache()
+            others = {}
+            for name in ("C3", "C4"):
+                if name == cfg.name:
+                    continue
+                c = dl0gen.CONFIGS[name]
+                r = kernel_only(c, max(10, args.steps // 2), 3, torch, dl0gen, rta)
+                others[name] = summarise(c, r["per_launch_ms"], peak)
+                r = None
+                torch.cuda.empty_cache()
+            out["configs"] = others
+            link = host_link_bandwidth(torch)
+            out["e2e"]["host_link_GBps_measured"] = link
+            out["e2e"]["frac_of_host_link"] = out["e2e"]["value"] / link
+            if not args.no_sustained:
+                out["sustained"] = sustained_leg(torch, dl0gen, rta, link)
+    else:
+        out["e2e"] = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0,
+                      "d2h_bytes_per_step": 0, "note": "skipped by --no-extra"}
+    if rank == 0:
+        print(json.dumps(out))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
