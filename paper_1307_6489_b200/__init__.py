@@ -64,6 +64,8 @@ def lib() -> ctypes.CDLL:
             L.rta_launch_count.argtypes = []
             L.rta_shutdown.restype = None
             L.rta_shutdown.argtypes = []
+            L.rta_debug_static_schedule.restype = None
+            L.rta_debug_static_schedule.argtypes = [ctypes.c_int]
             _lib = L
     return _lib
 
@@ -147,6 +149,12 @@ def rta_launch_count() -> int:
 
 def rta_shutdown() -> None:
     lib().rta_shutdown()
+
+
+def rta_debug_static_schedule(on: bool) -> None:
+    """Test hook: force the static round-robin tile schedule of the staged
+    kernels (default is dynamic). Results are identical either way."""
+    lib().rta_debug_static_schedule(1 if on else 0)
 
 
 def shard_events(n_events: int, world_size: int, rank: int) -> tuple[int, int]:

@@ -405,6 +405,11 @@ void rta_shutdown(void) {
       cudaGetLastError();
     }
   }
+  rta_sched_release();
 }
+
+// Test hook (not in the public header): 1 = static round-robin tile schedule,
+// 0 = dynamic (default). Results are identical; only the tile->CTA map changes.
+void rta_debug_static_schedule(int on) { rta_set_static_schedule(on != 0); }
 
 }  // extern "C"

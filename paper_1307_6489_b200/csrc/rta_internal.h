@@ -21,4 +21,10 @@ const char* rta_pick_kernel_name(int32_t n_samples, int32_t W, bool aligned16);
 
 void rta_count_launch();
 
+// Tile scheduling of the staged kernels: dynamic (default) or the static
+// round-robin (tests compare the two). rta_sched_release frees the per-stream
+// scheduler words (rta_shutdown).
+void rta_set_static_schedule(bool on);
+void rta_sched_release();
+
 #endif

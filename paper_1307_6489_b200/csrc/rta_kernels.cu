@@ -30,6 +30,8 @@
 #include "rta_internal.h"
 
 #include <atomic>
+#include <mutex>
+#include <unordered_map>
 
 namespace {
 
@@ -244,6 +246,13 @@ __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, c
   }
 }
 
+// Tiles are handed out dynamically: SMs do not stream at the same rate (near /
+// far L2 die, DRAM channel load), and with a static round-robin the launch
+// ends when the slowest CTA has finished its fixed share (measured: 4-7 % of
+// SM-time idle). `sched` points at {next tile, CTAs done}, both zero on entry;
+// the last CTA to leave zeroes them again, so the pair is reusable by the next
+// launch on the same stream (and by CUDA-graph replays). sched == nullptr
+// selects the static round-robin (same code path, locally generated indices).
 template <class C>
 __global__ void __launch_bounds__(C::NT)
     extract_tile_kernel(const uint16_t* __restrict__ wf, const uint32_t n_traces,
@@ -251,19 +260,60 @@ __global__ void __launch_bounds__(C::NT)
                         const int* __restrict__ pedestal, const float* __restrict__ gain,
                         int* __restrict__ out_sum, int* __restrict__ out_start,
                         float* __restrict__ out_charge, float* __restrict__ out_time,
-                        const int vec_store) {
+                        const int vec_store, uint32_t* __restrict__ sched) {
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ __align__(8) uint64_t full_bar[C::STAGES];
+  constexpr int QN = C::STAGES + 1;  // queue of tile indices, one slot more than stages
+  __shared__ uint32_t tile_q[QN];
   const int tid = threadIdx.x;
   const uint32_t n_full = n_traces / C::TILE_TRACES;
   const uint32_t rem = n_traces - n_full * C::TILE_TRACES;
   const uint32_t smem_base = smem_u32(smem);
   const uint32_t bar_base = smem_u32(full_bar);
 
+  // The first STAGES tiles of every CTA are the static round-robin ones (no
+  // atomic round trip before the first load); the shared counter hands out
+  // the tiles after those, in runs of up to kMaxRun consecutive tiles per
+  // atomic: same-address atomics retire at only ~0.3 G/s on B200 (measured),
+  // which one atomic per 10-20 KB tile would saturate. Runs shrink to single
+  // tiles near the end so the CTAs still finish together.
+  constexpr uint32_t kMaxRun = 8;
+  const uint32_t dyn_base = (uint32_t)C::STAGES * gridDim.x;
+  // thread 0 only: static sequence, current run [cur, end), prefetched run [nxt, nxt + n_run)
+  uint32_t static_next = blockIdx.x, cur = 0, end = 0, nxt = 0, n_run = 0;
+  auto fetch_static = [&]() -> uint32_t {
+    const uint32_t t = static_next;
+    // saturate: indices past the end must stay past the end
+    static_next = (t > 0xFFFFFFFFu - gridDim.x) ? 0xFFFFFFFFu : t + gridDim.x;
+    return t;
+  };
+  auto run_length = [&](const uint32_t seen) -> uint32_t {
+    const uint32_t left = n_full > seen ? n_full - seen : 0u;
+    const uint32_t k = left / (8u * gridDim.x);
+    return k < 1u ? 1u : (k > kMaxRun ? kMaxRun : k);
+  };
+  auto fetch = [&]() -> uint32_t {
+    if (sched == nullptr) return fetch_static();
+    if (cur == end) {  // take the prefetched run, ask for the one after it
+      cur = nxt;
+      end = nxt + n_run;
+      n_run = run_length(cur);
+      nxt = dyn_base + atomicAdd(sched, n_run);
+    }
+    return cur++;
+  };
+
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < C::STAGES; ++s) mbar_init(bar_base + 8 * s, C::PAD ? C::NT : 1);
+    for (int s = 0; s < C::STAGES; ++s) {
+      mbar_init(bar_base + 8 * s, C::PAD ? C::NT : 1);
+      tile_q[s] = fetch_static();
+    }
     fence_mbar_init();
+    if (sched != nullptr) {
+      n_run = run_length(dyn_base);
+      nxt = dyn_base + atomicAdd(sched, n_run);
+    }
   }
   __syncthreads();
 
@@ -289,27 +339,38 @@ __global__ void __launch_bounds__(C::NT)
   // prologue: fill the ring
 #pragma unroll
   for (int s = 0; s < C::STAGES; ++s) {
-    const uint32_t tile = blockIdx.x + (uint32_t)s * gridDim.x;
+    const uint32_t tile = tile_q[s];
     if (tile < n_full) issue(tile, s);
   }
+  // thread 0 keeps one tile index in flight: fetched while a tile is being
+  // computed, published one iteration later (the atomic's latency is hidden)
+  uint32_t pre = 0;
+  if (tid == 0) pre = fetch();
 
-  uint32_t j = 0;
-  for (uint32_t tile = blockIdx.x; tile < n_full; tile += gridDim.x, ++j) {
+  uint32_t tile;
+  for (uint32_t j = 0;; ++j) {
+    tile = tile_q[j % QN];
+    if (tile >= n_full) break;  // indices grow per CTA: nothing later is valid either
     const int stage = (int)(j % C::STAGES);
     const uint32_t parity = (j / C::STAGES) & 1u;
+    if (tid == 0) {
+      // slot (j + STAGES) % QN == (j - 1) % QN was last read before the
+      // previous iteration's barrier
+      tile_q[(j + C::STAGES) % QN] = pre;
+      pre = fetch();
+    }
     mbar_wait(bar_base + 8 * stage, parity);
     const uint8_t* unit = smem + stage * C::STAGE_BYTES + tid * C::UNIT_STRIDE;
     const uint32_t g0 = tile * C::TILE_TRACES + (uint32_t)tid * C::TPT;
     compute_unit<C>(unit, g0, C::TPT, n_pixels, pix_inv, pedestal, gain, out_sum, out_start,
                     out_charge, out_time, vec_store != 0);
-    __syncthreads();  // every thread is done with this stage
-    const uint32_t next = tile + (uint32_t)C::STAGES * gridDim.x;
+    __syncthreads();  // every thread is done with this stage; tile_q slot is published
+    const uint32_t next = tile_q[(j + C::STAGES) % QN];
     if (next < n_full) issue(next, stage);
   }
 
-  // ragged tail (< one tile of traces): plain copies, one CTA
-  if (rem != 0 && blockIdx.x == n_full % gridDim.x) {
-    __syncthreads();
+  // ragged tail (< one tile of traces): plain copies, by the CTA that drew index n_full
+  if (rem != 0 && tile == n_full) {
     const uint16_t* src = wf + (size_t)n_full * C::TILE_TRACES * C::S;
     uint16_t* dst = reinterpret_cast<uint16_t*>(smem);
     const uint32_t n_hw = rem * C::S;
@@ -325,6 +386,16 @@ __global__ void __launch_bounds__(C::NT)
       const uint32_t g0 = n_full * C::TILE_TRACES + first;
       compute_unit<C>(unit, g0, rem - first, n_pixels, pix_inv, pedestal, gain, out_sum,
                       out_start, out_charge, out_time, vec_store != 0);
+    }
+  }
+
+  // hand the scheduler words back zeroed (all of this CTA's fetches precede this)
+  if (sched != nullptr && tid == 0) {
+    __threadfence();
+    if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) {
+      sched[0] = 0;
+      sched[1] = 0;
+      __threadfence();
     }
   }
 }
@@ -365,6 +436,7 @@ __global__ void __launch_bounds__(256)
 
 // ------------------------------------------------------------- dispatch ----
 constexpr int kMaxDevices = 32;
+std::atomic<bool> g_static_schedule{false};  // tests: force the static round-robin
 
 struct DeviceInfo {
   std::atomic<int> ready{0};
@@ -384,6 +456,51 @@ cudaError_t device_sms(int dev, int* sms) {
   }
   *sms = d.sms;
   return cudaSuccess;
+}
+
+// ---- scheduler words: one {next tile, CTAs done} pair per (device, stream) ----
+// Launches on one stream run one after the other, so a pair owned by a stream
+// is never shared by two running kernels; the kernel leaves it zeroed.
+constexpr int kSchedSlots = 1024;      // distinct streams per device before falling back
+constexpr int kSchedSlotWords = 32;    // 128 bytes apart: one L2 line per pair
+
+struct SchedPool {
+  std::mutex mu;
+  uint32_t* base[kMaxDevices] = {};
+  bool failed[kMaxDevices] = {};
+  std::unordered_map<uintptr_t, int> slot_of[kMaxDevices];
+};
+SchedPool g_sched;
+
+// nullptr = no pair available (static round-robin is used instead)
+uint32_t* sched_words(int dev, cudaStream_t stream) {
+  if (stream == cudaStreamPerThread) return nullptr;  // one handle, many streams
+  std::lock_guard<std::mutex> lock(g_sched.mu);
+  if (g_sched.failed[dev]) return nullptr;
+  if (g_sched.base[dev] == nullptr) {
+    const size_t bytes = (size_t)kSchedSlots * kSchedSlotWords * sizeof(uint32_t);
+    void* p = nullptr;
+    if (cudaMalloc(&p, bytes) != cudaSuccess || cudaMemset(p, 0, bytes) != cudaSuccess ||
+        cudaDeviceSynchronize() != cudaSuccess) {
+      cudaGetLastError();  // e.g. first call inside a stream capture: stay static on this device
+      if (p) cudaFree(p);
+      g_sched.failed[dev] = true;
+      return nullptr;
+    }
+    g_sched.base[dev] = static_cast<uint32_t*>(p);
+  }
+  auto& m = g_sched.slot_of[dev];
+  const uintptr_t key = (uintptr_t)stream;
+  auto it = m.find(key);
+  int slot;
+  if (it != m.end()) {
+    slot = it->second;
+  } else {
+    if ((int)m.size() >= kSchedSlots) return nullptr;
+    slot = (int)m.size();
+    m.emplace(key, slot);
+  }
+  return g_sched.base[dev] + (size_t)slot * kSchedSlotWords;
 }
 
 template <class C>
@@ -423,9 +540,10 @@ struct TileLauncher {
     const uintptr_t o = (uintptr_t)out_sum | (uintptr_t)out_start | (uintptr_t)out_charge |
                         (uintptr_t)out_time;
     const int vec_store = (o % 8 == 0) ? 1 : 0;
+    uint32_t* sched = g_static_schedule ? nullptr : sched_words(dev, stream);
     extract_tile_kernel<C><<<grid, C::NT, C::SMEM_BYTES, stream>>>(
         wf, n_traces, n_pixels, pix_inv, pedestal, gain, out_sum, out_start, out_charge, out_time,
-        vec_store);
+        vec_store, sched);
     rta_count_launch();
     return cudaGetLastError();
   }
@@ -437,12 +555,59 @@ int TileLauncher<C>::ctas_per_sm[kMaxDevices];
 
 // The four shapes of BASELINE.json:configs (NT, STAGES tuned on B200; see
 // DESIGN.md "Kernels" for the shared-memory budget of each).
-using CfgS30W7 = TileCfg<30, 7, 256, 3>;
-using CfgS40W7 = TileCfg<40, 7, 256, 3>;
-using CfgS25W4 = TileCfg<25, 4, 256, 3>;
-using CfgS128W8 = TileCfg<128, 8, 128, 2>;
+// Compile-time tunables, e.g. -DRTA_S40_NT=256 -DRTA_S40_ST=3 (threads per CTA, stages).
+#ifndef RTA_S30_NT
+#define RTA_S30_NT 256
+#endif
+#ifndef RTA_S30_ST
+#define RTA_S30_ST 3
+#endif
+#ifndef RTA_S40_NT
+#define RTA_S40_NT 256
+#endif
+#ifndef RTA_S40_ST
+#define RTA_S40_ST 3
+#endif
+#ifndef RTA_S25_NT
+#define RTA_S25_NT 256
+#endif
+#ifndef RTA_S25_ST
+#define RTA_S25_ST 2
+#endif
+#ifndef RTA_S128_NT
+#define RTA_S128_NT 64
+#endif
+#ifndef RTA_S128_ST
+#define RTA_S128_ST 2
+#endif
+using CfgS30W7 = TileCfg<30, 7, RTA_S30_NT, RTA_S30_ST>;
+using CfgS40W7 = TileCfg<40, 7, RTA_S40_NT, RTA_S40_ST>;
+using CfgS25W4 = TileCfg<25, 4, RTA_S25_NT, RTA_S25_ST>;
+using CfgS128W8 = TileCfg<128, 8, RTA_S128_NT, RTA_S128_ST>;
 
 }  // namespace
+
+void rta_set_static_schedule(bool on) { g_static_schedule.store(on); }
+
+// rta_shutdown: the caller has synchronised the device(s)
+void rta_sched_release() {
+  std::lock_guard<std::mutex> lock(g_sched.mu);
+  int cur = 0;
+  const bool have_cur = cudaGetDevice(&cur) == cudaSuccess;
+  for (int d = 0; d < kMaxDevices; ++d) {
+    if (g_sched.base[d]) {
+      if (cudaSetDevice(d) == cudaSuccess) {
+        cudaDeviceSynchronize();
+        cudaFree(g_sched.base[d]);
+      }
+      g_sched.base[d] = nullptr;
+    }
+    g_sched.failed[d] = false;
+    g_sched.slot_of[d].clear();
+  }
+  if (have_cur) cudaSetDevice(cur);
+  cudaGetLastError();
+}
 
 const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16) {
   if (aligned16) {

@@ -221,3 +221,95 @@ def test_full_size_configs_sampled_against_oracle(name):
     s, t = outs[0], outs[1]
     assert int(t.min()) >= 0 and int(t.max()) <= c.n_samples - c.W
     assert bool(torch.isfinite(outs[3]).all()) and bool(torch.isfinite(outs[2]).all())
+
+
+# ---- tile scheduler (dynamic by default) ---------------
+@pytest.mark.parametrize("name,n_ev", [("C1", 64), ("C2", 301), ("C3", 257), ("C4", 97)])
+def test_static_and_dynamic_tile_schedules_agree(name, n_ev):
+    """The tile->CTA map must not change any result: run the staged kernel with
+    the dynamic scheduler (default) and with the static round-robin."""
+    import paper_1307_6489_b200 as rta
+    c = dl0gen.CONFIGS[name]
+    ped, gain = dl0gen.calib(c)
+    wf = dl0gen.events_cpu(c, 5, n_ev, threads=4)
+    want = oracle.extract(wf, ped, gain, c.W)
+    try:
+        for static in (True, False, True, False):
+            rta.rta_debug_static_schedule(static)
+            got = run_gpu(wf, ped, gain, c.W)
+            assert bit_identical(got, want), "static=%s" % static
+    finally:
+        rta.rta_debug_static_schedule(False)
+
+
+def test_back_to_back_launches_reuse_the_scheduler_words():
+    """The dynamic scheduler's counters are left zeroed by each launch: many
+    launches in a row on one stream, alternating shapes and sizes."""
+    import torch
+    import paper_1307_6489_b200 as rta
+    cases = []
+    for name, n_ev in [("C2", 120), ("C4", 40), ("C3", 77), ("C2", 3), ("C1", 64), ("C2", 119)]:
+        c = dl0gen.CONFIGS[name]
+        ped, gain = dl0gen.calib(c)
+        wf = dl0gen.events_cpu(c, 11, n_ev, threads=4)
+        cases.append((c, n_ev, to_dev_u16(wf), torch.from_numpy(ped).cuda(),
+                      torch.from_numpy(gain).cuda(), alloc_outputs(n_ev * c.n_pixels),
+                      oracle.extract(wf, ped, gain, c.W)))
+    for _ in range(3):
+        for c, n_ev, d_wf, d_ped, d_gain, outs, want in cases:      # no sync in between
+            rta.rta_extract(d_wf, n_ev, c.n_pixels, c.n_samples, d_ped, d_gain, c.W, *outs)
+    torch.cuda.synchronize()
+    for c, n_ev, d_wf, d_ped, d_gain, outs, want in cases:
+        assert bit_identical(tuple(o.cpu().numpy() for o in outs), want)
+
+
+def test_concurrent_streams_have_their_own_scheduler_words():
+    import torch
+    import paper_1307_6489_b200 as rta
+    c = dl0gen.CONFIGS["C2"]
+    ped, gain = dl0gen.calib(c)
+    d_ped, d_gain = torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda()
+    streams = [torch.cuda.Stream() for _ in range(6)]
+    jobs = []
+    for i, st in enumerate(streams):
+        n_ev = 150 + 17 * i
+        wf = dl0gen.events_cpu(c, 1000 * i, n_ev, threads=4)
+        jobs.append((st, n_ev, to_dev_u16(wf), alloc_outputs(n_ev * c.n_pixels),
+                     oracle.extract(wf, ped, gain, c.W)))
+    torch.cuda.synchronize()
+    for _ in range(4):
+        for st, n_ev, d_wf, outs, want in jobs:
+            rta.rta_extract(d_wf, n_ev, c.n_pixels, c.n_samples, d_ped, d_gain, c.W, *outs,
+                            stream=st)
+    torch.cuda.synchronize()
+    for st, n_ev, d_wf, outs, want in jobs:
+        assert bit_identical(tuple(o.cpu().numpy() for o in outs), want)
+
+
+def test_cuda_graph_capture_and_replay():
+    """rta_extract is capturable: the scheduler words are reset by the kernel
+    itself, so a replayed graph sees them zeroed again."""
+    import torch
+    import paper_1307_6489_b200 as rta
+    c = dl0gen.CONFIGS["C2"]
+    n_ev = 200
+    ped, gain = dl0gen.calib(c)
+    d_ped, d_gain = torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda()
+    wfs = [dl0gen.events_cpu(c, 300 * i, n_ev, threads=4) for i in range(3)]
+    d_wf = to_dev_u16(wfs[0])
+    outs = alloc_outputs(n_ev * c.n_pixels)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):                         # warm-up on the capture stream
+        rta.rta_extract(d_wf, n_ev, c.n_pixels, c.n_samples, d_ped, d_gain, c.W, *outs)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        rta.rta_extract(d_wf, n_ev, c.n_pixels, c.n_samples, d_ped, d_gain, c.W, *outs)
+    for wf in wfs[::-1]:
+        d_wf.copy_(to_dev_u16(wf))
+        for o in outs:
+            o.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert bit_identical(tuple(o.cpu().numpy() for o in outs),
+                             oracle.extract(wf, ped, gain, c.W))
