@@ -43,7 +43,7 @@ ALGO_BYTES_PER_TRACE_OUT = 16     # 2*S read + 16 written per 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C4"])
@@ -72,32 +72,89 @@ def ncu_traffic(name):
 
 
 class ClockSampler:
-    """nvidia-smi clocks/throttle reasons sampled DURING the timed region."""
+    """SM clock and throttle reasons sampled DURING the timed region: an NVML
+    polling thread (about 1 kHz; the timed region of a default run lasts only a
+    few tens of ms), or `nvidia-smi -lms` when NVML cannot be loaded."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
-    def __init__(self, index):
+    def __init__(self, index, uuid=None):
         self.index = index
+        self.uuid = uuid
         self.proc = None
         self.lines = []
+        self.nvml = None
+        self.samples = []          # (sm_mhz, reasons bitmask)
+        self.sm_max = None
+        self.stop_flag = threading.Event()
+        self.thread = None
+
+    def _nvml_handle(self):
+        import pynvml
+        pynvml.nvmlInit()
+        if self.uuid:
+            try:
+                u = self.uuid if str(self.uuid).startswith("GPU-") else "GPU-" + str(self.uuid)
+                return pynvml, pynvml.nvmlDeviceGetHandleByUUID(u.encode())
+            except Exception:
+                pass
+        return pynvml, pynvml.nvmlDeviceGetHandleByIndex(self.index)
 
     def start(self):
         try:
+            self.nvml, self.handle = self._nvml_handle()
+            self.sm_max = float(self.nvml.nvmlDeviceGetMaxClockInfo(self.handle, self.nvml.NVML_CLOCK_SM))
+            self.thread = threading.Thread(target=self._poll, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.nvml = None
+        try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                 "--format=csv,noheader,nounits", "-lms", "50"],
+                 "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=self._read, daemon=True)
-            self.t.start()
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
         except Exception:
             self.proc = None
+
+    def _poll(self):
+        n = self.nvml
+        while not self.stop_flag.is_set():
+            try:
+                mhz = float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
+                mask = int(n.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle))
+                self.samples.append((mhz, mask))
+            except Exception:
+                pass
+            time.sleep(0.001)
 
     def _read(self):
         for line in self.proc.stdout:
             self.lines.append(line)
 
-    def stop(self):
+    def mark(self):
+        """Number of samples so far: bracket the timed region with two marks."""
+        return len(self.samples) if self.nvml else len(self.lines)
+
+    def stop(self, lo=0, hi=None):
+        if self.nvml:
+            self.stop_flag.set()
+            self.thread.join(timeout=2)
+            n = self.nvml
+            sel = self.samples[lo:hi] or self.samples
+            bits = {"hw_slowdown": n.nvmlClocksThrottleReasonHwSlowdown,
+                    "hw_thermal_slowdown": n.nvmlClocksThrottleReasonHwThermalSlowdown,
+                    "sw_thermal_slowdown": n.nvmlClocksThrottleReasonSwThermalSlowdown,
+                    "sw_power_cap": n.nvmlClocksThrottleReasonSwPowerCap}
+            reasons = sorted(k for k, b in bits.items() if any(m & b for _, m in sel))
+            sm = [x for x, _ in sel]
+            return {"sm_mhz": statistics.median(sm) if sm else None, "sm_min_mhz": min(sm) if sm else None,
+                    "sm_max_mhz": self.sm_max, "samples": len(sm), "source": "nvml, timed region only",
+                    "reasons": reasons}
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -106,8 +163,7 @@ class ClockSampler:
         except Exception:
             self.proc.kill()
         sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.lines:
+        for ln in (self.lines[lo:hi] or self.lines):
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 7:
                 continue
@@ -116,12 +172,12 @@ class ClockSampler:
                 mx.append(float(f[1]))
             except ValueError:
                 continue
-            for n, v in zip(names, f[3:7]):
+            for n, v in zip(self.NAMES, f[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(n)
         return {"sm_mhz": statistics.median(sm) if sm else None,
                 "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "samples": len(sm), "source": "nvidia-smi -lms 20", "reasons": sorted(reasons)}
 
 
 # --------------------------------------------------------------------------- #
@@ -187,7 +243,7 @@ def device_batch(cfg, torch, dl0gen):
     return d_wf, d_ped, d_gain, outs, ped, gain
 
 
-def kernel_only(cfg, steps, warmup, torch, dl0gen, rta, barrier=None):
+def kernel_only(cfg, steps, warmup, torch, dl0gen, rta, barrier=None, sampler=None):
     d_wf, d_ped, d_gain, outs, ped, gain = device_batch(cfg, torch, dl0gen)
     stream = torch.cuda.current_stream()
 
@@ -200,12 +256,15 @@ def kernel_only(cfg, steps, warmup, torch, dl0gen, rta, barrier=None):
     if barrier:
         barrier()
     before = rta.rta_launch_count()
+    m0 = sampler.mark() if sampler else 0
     per = time_steps(run, steps, stream)
+    m1 = sampler.mark() if sampler else 0
     launches = rta.rta_launch_count() - before
     if barrier:
         barrier()
     checksum = int(d_wf.view(-1)[: min(d_wf.numel(), 1 << 26)].sum(dtype=torch.int64))
     return {"per_launch_ms": per, "launches": launches, "checksum_first_64Mi_samples": checksum,
+            "marks": (m0, m1),
             "keep": (d_wf, d_ped, d_gain, outs, ped, gain)}
 
 
@@ -385,12 +444,16 @@ def main():
     cfg = dl0gen.CONFIGS[args.workload]
     peak, peak_src = hbm_peak()
 
-    sampler = ClockSampler(local)
+    try:
+        uuid = str(torch.cuda.get_device_properties(local).uuid)
+    except Exception:
+        uuid = None
+    sampler = ClockSampler(local, uuid)
     sampler.start()
     # Weak scaling: every rank extracts its own batch of the named workload
     # (independent events; no data-path collective).
-    main_run = kernel_only(cfg, args.steps, args.warmup, torch, dl0gen, rta, barrier)
-    clocks = sampler.stop()
+    main_run = kernel_only(cfg, args.steps, args.warmup, torch, dl0gen, rta, barrier, sampler)
+    clocks = sampler.stop(*main_run["marks"])
     t_local = sum(main_run["per_launch_ms"])
     t_max = t_local
     if dist is not None:
