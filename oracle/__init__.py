@@ -20,6 +20,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rta_oracle.cpp")
+_SRCS = [_SRC, os.path.join(_HERE, "rta_oracle_windows.cpp")]
 _LIB = os.path.join(_HERE, "librta_oracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -29,12 +30,12 @@ def build(force: bool = False) -> str:
     """Compile the oracle with g++ -O2 (single-threaded, no fast-math)."""
     with _lock:
         stale = (not os.path.exists(_LIB)
-                 or os.path.getmtime(_LIB) < os.path.getmtime(_SRC))
+                 or any(os.path.getmtime(_LIB) < os.path.getmtime(f) for f in _SRCS))
         if force or stale:
             tmp = _LIB + ".tmp%d" % os.getpid()
             subprocess.check_call(
                 ["g++", "-std=c++17", "-O2", "-fPIC", "-shared",
-                 "-ffp-contract=off", "-o", tmp, _SRC])
+                 "-ffp-contract=off", "-o", tmp] + _SRCS)
             os.replace(tmp, _LIB)
     return _LIB
 
@@ -48,8 +49,74 @@ def _load():
             ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32,
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32,
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        common = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32,
+                  ctypes.c_void_p, ctypes.c_void_p]
+        outs = [ctypes.c_void_p] * 4
+        lib.rta_oracle_extract_fixed.restype = ctypes.c_int
+        lib.rta_oracle_extract_fixed.argtypes = common + [ctypes.c_int32, ctypes.c_void_p] + outs
+        lib.rta_oracle_extract_local_peak.restype = ctypes.c_int
+        lib.rta_oracle_extract_local_peak.argtypes = common + [ctypes.c_int32, ctypes.c_int32] + outs
+        lib.rta_oracle_extract_fir.restype = ctypes.c_int
+        lib.rta_oracle_extract_fir.argtypes = common + [ctypes.c_void_p, ctypes.c_int32] + outs
         _lib = lib
     return _lib
+
+
+def _prep(wf, pedestal, gain):
+    wf = np.ascontiguousarray(wf, dtype=np.uint16)
+    if wf.ndim != 3:
+        raise ValueError("wf must be [n_events][n_pixels][n_samples]")
+    E, P, S = wf.shape
+    pedestal = np.ascontiguousarray(pedestal, dtype=np.int32)
+    gain = np.ascontiguousarray(gain, dtype=np.float32)
+    if pedestal.shape != (P,) or gain.shape != (P,):
+        raise ValueError("pedestal and gain must be [n_pixels]")
+    n = E * P
+    outs = (np.empty(n, np.int32), np.empty(n, np.int32), np.empty(n, np.float32),
+            np.empty(n, np.float32))
+    return wf, pedestal, gain, outs
+
+
+def extract_fixed(wf, pedestal, gain, W: int, window_start):
+    """Fixed-window extractor (rta_oracle_windows.cpp, reading R22)."""
+    wf, pedestal, gain, outs = _prep(wf, pedestal, gain)
+    E, P, S = wf.shape
+    ws = np.ascontiguousarray(window_start, dtype=np.int32)
+    if ws.shape != (P,):
+        raise ValueError("window_start must be [n_pixels]")
+    rc = _load().rta_oracle_extract_fixed(
+        wf.ctypes.data, E, P, S, pedestal.ctypes.data, gain.ctypes.data, int(W), ws.ctypes.data,
+        *[o.ctypes.data for o in outs])
+    if rc != 0:
+        raise ValueError("rta_oracle_extract_fixed: bad shape")
+    return outs
+
+
+def extract_local_peak(wf, pedestal, gain, W: int, shift: int):
+    """Local-peak extractor (rta_oracle_windows.cpp, reading R23)."""
+    wf, pedestal, gain, outs = _prep(wf, pedestal, gain)
+    E, P, S = wf.shape
+    rc = _load().rta_oracle_extract_local_peak(
+        wf.ctypes.data, E, P, S, pedestal.ctypes.data, gain.ctypes.data, int(W), int(shift),
+        *[o.ctypes.data for o in outs])
+    if rc != 0:
+        raise ValueError("rta_oracle_extract_local_peak: bad shape")
+    return outs
+
+
+def extract_fir(wf, pedestal, gain, taps):
+    """FIR / matched-filter extractor (rta_oracle_windows.cpp, reading R24)."""
+    wf, pedestal, gain, outs = _prep(wf, pedestal, gain)
+    E, P, S = wf.shape
+    taps = np.ascontiguousarray(taps, dtype=np.int32)
+    if taps.ndim != 1:
+        raise ValueError("taps must be 1-D")
+    rc = _load().rta_oracle_extract_fir(
+        wf.ctypes.data, E, P, S, pedestal.ctypes.data, gain.ctypes.data, taps.ctypes.data,
+        int(taps.size), *[o.ctypes.data for o in outs])
+    if rc != 0:
+        raise ValueError("rta_oracle_extract_fir: bad shape")
+    return outs
 
 
 def extract(wf: np.ndarray, pedestal: np.ndarray, gain: np.ndarray, W: int):

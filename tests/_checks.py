@@ -95,3 +95,47 @@ def check_invariants(wf, pedestal, gain, W, out_sum, out_start, out_charge,
     if big.any():
         assert (np.asarray(out_time, np.float32)[big]
                 == want_t[big].astype(np.float32)).all(), "time != RN32(exact)"
+
+
+# ---- window family (oracle/rta_oracle_windows.cpp): numpy restatements -------
+def np_window_outputs(x, start, gain_per_trace, weights):
+    """Outputs of every trace given its window start: x int64 [n][S], start
+    int64 [n], weights int64 [W] (ones for a plain window)."""
+    n, S = x.shape
+    W = len(weights)
+    idx = start[:, None] + np.arange(W)[None, :]
+    xs = np.take_along_axis(x, idx, 1) * weights[None, :]
+    s = xs.sum(1)
+    num = (idx * xs).sum(1)
+    charge = (s.astype(np.float64) * gain_per_trace).astype(np.float32)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        t_pos = num.astype(np.float64) / s.astype(np.float64)
+    time = np.where(s > 0, t_pos, start + 0.5 * (W - 1)).astype(np.float32)
+    return s.astype(np.int32), start.astype(np.int32), charge, time
+
+
+def _flat(wf, pedestal, gain):
+    wf = np.asarray(wf)
+    E, P, S = wf.shape
+    x = (wf.astype(np.int64) - np.asarray(pedestal, np.int64)[None, :, None]).reshape(E * P, S)
+    g = np.tile(np.asarray(gain, np.float32).astype(np.float64), E)
+    return E, P, S, x, g
+
+
+def np_fixed(wf, pedestal, gain, W, window_start):
+    E, P, S, x, g = _flat(wf, pedestal, gain)
+    start = np.tile(np.clip(np.asarray(window_start, np.int64), 0, S - W), E)
+    return np_window_outputs(x, start, g, np.ones(W, np.int64))
+
+
+def np_local_peak(wf, pedestal, gain, W, shift):
+    E, P, S, x, g = _flat(wf, pedestal, gain)
+    start = np.clip(x.argmax(1) - int(shift), 0, S - W)               # argmax: first maximum
+    return np_window_outputs(x, start, g, np.ones(W, np.int64))
+
+
+def np_fir(wf, pedestal, gain, taps):
+    E, P, S, x, g = _flat(wf, pedestal, gain)
+    c = np.asarray(taps, np.int64)
+    y = np.stack([np.correlate(row, c, mode="valid") for row in x])   # y[t] = sum_k c[k] x[t+k]
+    return np_window_outputs(x, y.argmax(1), g, c)
