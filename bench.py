@@ -283,6 +283,31 @@ def summarise(cfg, per_ms, peak):
     }
 
 
+def family_leg(cfg, steps, peak, torch, dl0gen, rta):
+    """Kernel-only throughput of the other extractors (NEXT-1) on the same
+    device-resident batch: fixed window, local peak, FIR (triangular taps)."""
+    import numpy as np
+    d_wf, d_ped, d_gain, outs, ped, gain = device_batch(cfg, torch, dl0gen)
+    stream = torch.cuda.current_stream()
+    start = torch.from_numpy(np.random.default_rng(cfg.seed).integers(
+        0, cfg.n_samples - cfg.W + 1, cfg.n_pixels).astype(np.int32)).cuda()
+    taps = [1, 2, 3, 4, 3, 2, 1, 1][:cfg.W]
+    base = (d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain)
+    runs = {
+        "fixed": lambda: rta.rta_extract_fixed(*base, cfg.W, start, *outs, stream=stream),
+        "local_peak": lambda: rta.rta_extract_local_peak(*base, cfg.W, cfg.W // 2, *outs, stream=stream),
+        "fir": lambda: rta.rta_extract_fir(*base, taps, *outs, stream=stream),
+    }
+    res = {}
+    for name, run in runs.items():
+        for _ in range(3):
+            run()
+        torch.cuda.synchronize()
+        res[name] = summarise(cfg, time_steps(run, steps, stream), peak)
+    res["fir"]["taps"] = taps
+    return res
+
+
 def host_link_bandwidth(torch, nbytes=1 << 30, reps=10):
     """Pinned H2D cudaMemcpyAsync bandwidth, best of `reps` (the H2D-fed roofline)."""
     h = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
@@ -521,6 +546,12 @@ def main():
                 r = None
                 torch.cuda.empty_cache()
             out["configs"] = others
+            fam = {}
+            for name in ("C2", "C3", "C4"):
+                fam[name] = family_leg(dl0gen.CONFIGS[name], max(10, args.steps // 4), peak,
+                                       torch, dl0gen, rta)
+                torch.cuda.empty_cache()
+            out["family"] = fam
             link = host_link_bandwidth(torch)
             out["e2e"]["host_link_GBps_measured"] = link
             out["e2e"]["frac_of_host_link"] = out["e2e"]["value"] / link

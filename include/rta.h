@@ -63,12 +63,57 @@ enum {
  *
  * Asynchronous: validates, enqueues on `stream`, returns without synchronising.
  * Outputs are valid once `stream` has been synchronised. n_events == 0 is
- * RTA_OK with nothing enqueued and the outputs untouched. Stateless and
- * thread-safe across streams. */
+ * RTA_OK with nothing enqueued and the outputs untouched. Thread-safe across
+ * streams; capturable into a CUDA graph after one warm-up call on the device
+ * (the first call allocates 128 KB of per-stream tile-scheduler words, owned by
+ * the library and released by rta_shutdown). */
 int rta_extract(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
                 int32_t n_samples, const int32_t* pedestal, const float* gain,
                 int32_t W, int32_t* out_sum, int32_t* out_start,
                 float* out_charge, float* out_time, void* stream);
+
+/* ---- Other members of the extractor family ----------
+ * The paper says "several signal extraction algorithms [13]" were being ported
+ * (§5) and names none; ref [13] is unavailable, so
+ * the three below are defined here (readings R22-R24). They share
+ * every argument, layout, output and error rule of rta_extract and differ only
+ * in how the window is chosen. With x[s] = wf[e][p][s] - pedestal[p]:
+ *
+ *   rta_extract_fixed       t* = clamp(window_start[p], 0, S-W)
+ *                           window_start: DEVICE int32 [n_pixels], 4-byte aligned.
+ *   rta_extract_local_peak  t* = clamp(peak - shift, 0, S-W), peak = smallest s
+ *                           with x[s] maximal; shift may be negative.
+ *   both:                   out_sum = sum_{k<W} x[t*+k], time numerator
+ *                           sum_{k<W} (t*+k) x[t*+k]
+ *   rta_extract_fir         y(t) = sum_{k<K} taps[k] x[t+k], t = 0..S-K;
+ *                           t* = smallest t with y(t) maximal; out_sum = y(t*);
+ *                           time numerator sum_{k<K} (t*+k) taps[k] x[t*+k]; W := K.
+ *                           taps: HOST int32 [n_taps], copied before returning;
+ *                           1 <= n_taps <= min(n_samples, 32) (more: RTA_ERR_UNSUPPORTED);
+ *                           n_samples * sum|taps| * 65535 >= 2^31: RTA_ERR_UNSUPPORTED.
+ *                           All-ones taps of length W give exactly rta_extract.
+ *   always                  out_start = t*, out_charge = RN32(out_sum * gain[p]),
+ *                           out_time = RN32(numerator / out_sum), or t* + (W-1)/2
+ *                           when out_sum <= 0.
+ *
+ * Asynchronous on `stream`, like rta_extract. */
+int rta_extract_fixed(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
+                      int32_t n_samples, const int32_t* pedestal, const float* gain,
+                      int32_t W, const int32_t* window_start, int32_t* out_sum,
+                      int32_t* out_start, float* out_charge, float* out_time,
+                      void* stream);
+
+int rta_extract_local_peak(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
+                           int32_t n_samples, const int32_t* pedestal,
+                           const float* gain, int32_t W, int32_t shift,
+                           int32_t* out_sum, int32_t* out_start, float* out_charge,
+                           float* out_time, void* stream);
+
+int rta_extract_fir(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
+                    int32_t n_samples, const int32_t* pedestal, const float* gain,
+                    const int32_t* taps, int32_t n_taps, int32_t* out_sum,
+                    int32_t* out_start, float* out_charge, float* out_time,
+                    void* stream);
 
 /* Host-fed path (step a8; BASELINE.json:configs[4]; page-locked transfer test
  * of PAPER.md:133/139 §5). Same operation, but `wf_host` is HOST memory

@@ -54,6 +54,14 @@ def lib() -> ctypes.CDLL:
             L.rta_extract_stream.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t, _VP]
             L.rta_extract_host.restype = ctypes.c_int
             L.rta_extract_host.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t]
+            L.rta_extract_fixed.restype = ctypes.c_int
+            L.rta_extract_fixed.argtypes = _EXTRACT_ARGS[:7] + [_VP] + [_VP] * 4 + [_VP]
+            L.rta_extract_local_peak.restype = ctypes.c_int
+            L.rta_extract_local_peak.argtypes = _EXTRACT_ARGS[:7] + [ctypes.c_int32] + [_VP] * 4 + [_VP]
+            L.rta_extract_fir.restype = ctypes.c_int
+            L.rta_extract_fir.argtypes = _EXTRACT_ARGS[:6] + [_VP, ctypes.c_int32] + [_VP] * 4 + [_VP]
+            L.rta_debug_force_generic.restype = None
+            L.rta_debug_force_generic.argtypes = [ctypes.c_int]
             L.rta_strerror.restype = ctypes.c_char_p
             L.rta_strerror.argtypes = [ctypes.c_int]
             L.rta_last_cuda_error.restype = ctypes.c_int
@@ -109,6 +117,36 @@ def rta_extract(wf, n_events, n_pixels, n_samples, pedestal, gain, W,
               _stream_handle(stream)))
 
 
+def rta_extract_fixed(wf, n_events, n_pixels, n_samples, pedestal, gain, W, window_start,
+                      out_sum, out_start, out_charge, out_time, stream=None) -> None:
+    """include/rta.h:rta_extract_fixed. ``window_start`` is a device int32 [n_pixels]."""
+    _check(lib().rta_extract_fixed(
+        _ptr(wf), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain), W,
+        _ptr(window_start), _ptr(out_sum), _ptr(out_start), _ptr(out_charge), _ptr(out_time),
+        _stream_handle(stream)))
+
+
+def rta_extract_local_peak(wf, n_events, n_pixels, n_samples, pedestal, gain, W, shift,
+                           out_sum, out_start, out_charge, out_time, stream=None) -> None:
+    """include/rta.h:rta_extract_local_peak."""
+    _check(lib().rta_extract_local_peak(
+        _ptr(wf), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain), W, int(shift),
+        _ptr(out_sum), _ptr(out_start), _ptr(out_charge), _ptr(out_time),
+        _stream_handle(stream)))
+
+
+def rta_extract_fir(wf, n_events, n_pixels, n_samples, pedestal, gain, taps,
+                    out_sum, out_start, out_charge, out_time, stream=None) -> None:
+    """include/rta.h:rta_extract_fir. ``taps`` is a host sequence of ints."""
+    taps = [int(t) for t in taps]
+    arr = (ctypes.c_int32 * max(1, len(taps)))(*taps)
+    _check(lib().rta_extract_fir(
+        _ptr(wf), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain),
+        ctypes.cast(arr, _VP) if taps else None, len(taps),
+        _ptr(out_sum), _ptr(out_start), _ptr(out_charge), _ptr(out_time),
+        _stream_handle(stream)))
+
+
 def rta_extract_stream(wf_host, n_events, n_pixels, n_samples, pedestal, gain, W,
                        out_sum, out_start, out_charge, out_time, chunk_bytes=0,
                        stream=None) -> None:
@@ -149,6 +187,11 @@ def rta_launch_count() -> int:
 
 def rta_shutdown() -> None:
     lib().rta_shutdown()
+
+
+def rta_debug_force_generic(on: bool) -> None:
+    """Test hook: route rta_extract_fixed/_local_peak/_fir to the generic kernel."""
+    lib().rta_debug_force_generic(1 if on else 0)
 
 
 def rta_debug_static_schedule(on: bool) -> None:

@@ -16,6 +16,7 @@
 namespace {
 
 thread_local int t_last_cuda = 0;
+std::atomic<bool> g_force_generic{false};  // tests: route the family entry points to the generic kernel
 std::atomic<uint64_t> g_launches{0};
 
 int fail_cuda(cudaError_t e) {
@@ -311,6 +312,69 @@ int rta_extract_generic(const uint16_t* wf, int64_t n_events, int32_t n_pixels, 
   return e == cudaSuccess ? RTA_OK : fail_cuda(e);
 }
 
+// ---- the other members of the extractor family (NEXT-1; readings R22-R24) ----
+int rta_extract_fixed(const uint16_t* wf, int64_t n_events, int32_t n_pixels, int32_t n_samples,
+                      const int32_t* pedestal, const float* gain, int32_t W,
+                      const int32_t* window_start, int32_t* out_sum, int32_t* out_start,
+                      float* out_charge, float* out_time, void* stream) {
+  const int v = validate(wf, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum, out_start,
+                         out_charge, out_time);
+  if (v != RTA_OK || n_events == 0) return v;
+  if (!window_start) return RTA_ERR_NULL;
+  if ((uintptr_t)window_start % 4 != 0) return RTA_ERR_ALIGN;
+  RtaMode m = {};
+  m.kind = RTA_MODE_FIXED;
+  m.window_start = window_start;
+  const cudaError_t e = rta_launch_extract(wf, n_events * (int64_t)n_pixels, n_pixels, n_samples,
+                                           pedestal, gain, W, out_sum, out_start, out_charge,
+                                           out_time, (cudaStream_t)stream, g_force_generic, &m);
+  return e == cudaSuccess ? RTA_OK : fail_cuda(e);
+}
+
+int rta_extract_local_peak(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
+                           int32_t n_samples, const int32_t* pedestal, const float* gain,
+                           int32_t W, int32_t shift, int32_t* out_sum, int32_t* out_start,
+                           float* out_charge, float* out_time, void* stream) {
+  const int v = validate(wf, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum, out_start,
+                         out_charge, out_time);
+  if (v != RTA_OK || n_events == 0) return v;
+  RtaMode m = {};
+  m.kind = RTA_MODE_LOCAL_PEAK;
+  // |shift| >= n_samples already pins the window to one end of the trace
+  m.shift = shift > n_samples ? n_samples : (shift < -n_samples ? -n_samples : shift);
+  const cudaError_t e = rta_launch_extract(wf, n_events * (int64_t)n_pixels, n_pixels, n_samples,
+                                           pedestal, gain, W, out_sum, out_start, out_charge,
+                                           out_time, (cudaStream_t)stream, g_force_generic, &m);
+  return e == cudaSuccess ? RTA_OK : fail_cuda(e);
+}
+
+int rta_extract_fir(const uint16_t* wf, int64_t n_events, int32_t n_pixels, int32_t n_samples,
+                    const int32_t* pedestal, const float* gain, const int32_t* taps,
+                    int32_t n_taps, int32_t* out_sum, int32_t* out_start, float* out_charge,
+                    float* out_time, void* stream) {
+  if (n_events < 0 || n_pixels < 1 || n_samples < 1 || n_taps < 1 || n_taps > n_samples)
+    return RTA_ERR_SHAPE;
+  if (n_taps > RTA_MAX_TAPS) return RTA_ERR_UNSUPPORTED;
+  if (!taps) return RTA_ERR_NULL;
+  int64_t abs_sum = 0;
+  for (int k = 0; k < n_taps; ++k) abs_sum += taps[k] < 0 ? -(int64_t)taps[k] : (int64_t)taps[k];
+  if (abs_sum < 1) abs_sum = 1;
+  if ((int64_t)n_samples * 65535ll >= (1ll << 31) / abs_sum) return RTA_ERR_UNSUPPORTED;
+  if (n_events * (int64_t)n_pixels >= (1ll << 31)) return RTA_ERR_UNSUPPORTED;
+  // the remaining checks are those of the plain window with W = 1 (pointers, alignment)
+  const int v = validate(wf, n_events, n_pixels, n_samples, pedestal, gain, 1, out_sum, out_start,
+                         out_charge, out_time);
+  if (v != RTA_OK || n_events == 0) return v;
+  RtaMode m = {};
+  m.kind = RTA_MODE_FIR;
+  m.n_taps = n_taps;
+  for (int k = 0; k < n_taps; ++k) m.taps[k] = taps[k];
+  const cudaError_t e = rta_launch_extract(wf, n_events * (int64_t)n_pixels, n_pixels, n_samples,
+                                           pedestal, gain, n_taps, out_sum, out_start, out_charge,
+                                           out_time, (cudaStream_t)stream, g_force_generic, &m);
+  return e == cudaSuccess ? RTA_OK : fail_cuda(e);
+}
+
 int rta_extract_stream(const uint16_t* wf_host, int64_t n_events, int32_t n_pixels,
                        int32_t n_samples, const int32_t* pedestal, const float* gain, int32_t W,
                        int32_t* out_sum, int32_t* out_start, float* out_charge, float* out_time,
@@ -407,6 +471,10 @@ void rta_shutdown(void) {
   }
   rta_sched_release();
 }
+
+// Test hook (not in the public header): 1 = rta_extract_fixed / _local_peak / _fir
+// take the generic kernel whatever the shape (two device paths must agree).
+void rta_debug_force_generic(int on) { g_force_generic.store(on != 0); }
 
 // Test hook (not in the public header): 1 = static round-robin tile schedule,
 // 0 = dynamic (default). Results are identical; only the tile->CTA map changes.

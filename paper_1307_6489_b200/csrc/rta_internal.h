@@ -6,15 +6,27 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// The extractor family (readings R22-R24): how the window is chosen.
+#define RTA_MAX_TAPS 32
+enum { RTA_MODE_SLIDING = 0, RTA_MODE_FIXED = 1, RTA_MODE_LOCAL_PEAK = 2, RTA_MODE_FIR = 3 };
+struct RtaMode {
+  int kind;
+  const int32_t* window_start;  // RTA_MODE_FIXED: DEVICE [n_pixels]
+  int32_t shift;                // RTA_MODE_LOCAL_PEAK
+  int32_t n_taps;               // RTA_MODE_FIR (== W passed to rta_launch_extract)
+  int32_t taps[RTA_MAX_TAPS];   // RTA_MODE_FIR
+};
+
 // Enqueue the extraction of `n_traces` traces starting at global trace index 0
 // of `wf` on `stream`. Arguments are already validated. Returns a cudaError_t.
 // `force_generic` routes every shape to the generic kernel (tests use it to
-// compare the two paths).
+// compare the two paths). `mode` == nullptr is the sliding-window extractor.
 cudaError_t rta_launch_extract(const uint16_t* wf, int64_t n_traces, int32_t n_pixels,
                                int32_t n_samples, const int32_t* pedestal,
                                const float* gain, int32_t W, int32_t* out_sum,
                                int32_t* out_start, float* out_charge, float* out_time,
-                               cudaStream_t stream, bool force_generic);
+                               cudaStream_t stream, bool force_generic,
+                               const RtaMode* mode = nullptr);
 
 // Name of the kernel the dispatcher picks (static string).
 const char* rta_pick_kernel_name(int32_t n_samples, int32_t W, bool aligned16);

@@ -96,17 +96,21 @@ struct Result {
   float charge, time;
 };
 
-// Steps a5-a7 from the raw (pedestal-deferred) quantities of one trace:
-//   rawsum = sum of raw samples in the winning window, tstar = its start,
-//   relnum = sum_k k * raw[tstar + k].
-__device__ __forceinline__ Result finish_trace(const int W, const uint32_t rawsum, const int tstar,
-                                               const uint32_t relnum, const int ped,
-                                               const float gain) {
+constexpr int kMaxTaps = RTA_MAX_TAPS;
+
+// Steps a5-a7 from the raw (pedestal-deferred) quantities of one trace. With
+// window weights c[k] (all ones except for the FIR extractor):
+//   rawsum = sum_k c[k] raw[tstar + k],  relnum = sum_k k c[k] raw[tstar + k],
+//   c0 = sum_k c[k],  c1 = sum_k k c[k],  W = number of weights.
+// The ABI guard n_samples * sum|c| * 65535 < 2^31 keeps tstar*rawsum + relnum
+// inside int32; everything touched by the pedestal is int64.
+__device__ __forceinline__ Result finish_trace(const int W, const int rawsum, const int tstar,
+                                               const int relnum, const int ped, const float gain,
+                                               const int c0, const int c1) {
   Result r;
-  const long long sum64 = (long long)rawsum - (long long)W * (long long)ped;
-  const int c = W * tstar + (W * (W - 1)) / 2;  // sum of the window's sample indices
-  const long long num64 =
-      (long long)((uint32_t)tstar * rawsum + relnum) - (long long)ped * (long long)c;
+  const long long sum64 = (long long)rawsum - (long long)c0 * (long long)ped;
+  const long long num64 = (long long)(tstar * rawsum + relnum) -
+                          (long long)ped * ((long long)tstar * (long long)c0 + (long long)c1);
   r.sum = (int)sum64;
   r.start = tstar;
   const long long lim = 1ll << 24;
@@ -126,6 +130,20 @@ __device__ __forceinline__ Result finish_trace(const int W, const uint32_t rawsu
                        : (float)((double)tstar + 0.5 * (double)(W - 1));
   }
   return r;
+}
+
+// ---- the extractor family (readings R22-R24): how t* is chosen ----
+enum : int { MODE_SLIDING = 0, MODE_FIXED = 1, MODE_LOCAL_PEAK = 2, MODE_FIR = 3 };
+
+struct ModeArgs {
+  const int32_t* window_start;  // MODE_FIXED: device, [n_pixels]
+  int32_t shift;                // MODE_LOCAL_PEAK
+  int32_t c0, c1;               // MODE_FIR: sum c[k], sum k c[k]
+  int32_t taps[kMaxTaps];       // MODE_FIR
+};
+
+__device__ __forceinline__ int clamp_start(const int t, const int S, const int W) {
+  return min(max(t, 0), S - W);
 }
 
 // ------------------------------------------------------- tile kernel cfg ----
@@ -149,6 +167,9 @@ struct TileCfg {
   static constexpr int NWIN = S - W + 1;
   static constexpr int KB = ilog2_ceil(NWIN);
   static constexpr uint32_t KM = (1u << KB) - 1u;
+  static constexpr int PB = ilog2_ceil(S);  // local-peak key: sample index bits
+  static constexpr uint32_t PM = (1u << PB) - 1u;
+  static_assert(16 + PB <= 32, "peak key must fit 32 bits");
   static_assert(W >= 1 && W <= S, "window must fit the trace");
   static_assert(NT % 32 == 0, "whole warps");
   static_assert(TILE_BYTES % 16 == 0, "TMA bulk copies move multiples of 16 bytes");
@@ -159,7 +180,7 @@ struct TileCfg {
 // raw sample h (halfword index inside the thread's unit), h known at compile time
 #define RTA_X(w, h) (((h)&1) ? ((w)[(h) >> 1] >> 16) : ((w)[(h) >> 1] & 0xFFFFu))
 
-template <class C>
+template <class C, int MODE>
 __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, const uint32_t g0,
                                              const uint32_t n_valid, const uint32_t n_pixels,
                                              const uint32_t pix_inv,
@@ -167,54 +188,104 @@ __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, c
                                              const float* __restrict__ gain,
                                              int* __restrict__ out_sum, int* __restrict__ out_start,
                                              float* __restrict__ out_charge,
-                                             float* __restrict__ out_time, const bool vec_store) {
+                                             float* __restrict__ out_time, const bool vec_store,
+                                             const ModeArgs& ma) {
   constexpr int S = C::S, W = C::W;
-  uint32_t w[C::NWORDS];
-  if constexpr (C::VEC == 16) {
+  // the fixed window touches W samples only: no register copy of the trace
+  constexpr bool NEED_W = (MODE != MODE_FIXED);
+  uint32_t w[NEED_W ? C::NWORDS : 1];
+  if constexpr (NEED_W) {
+    if constexpr (C::VEC == 16) {
 #pragma unroll
-    for (int i = 0; i < C::NVEC; ++i) {
-      const uint4 v = *reinterpret_cast<const uint4*>(unit + 16 * i);
-      w[4 * i] = v.x, w[4 * i + 1] = v.y, w[4 * i + 2] = v.z, w[4 * i + 3] = v.w;
+      for (int i = 0; i < C::NVEC; ++i) {
+        const uint4 v = *reinterpret_cast<const uint4*>(unit + 16 * i);
+        w[4 * i] = v.x, w[4 * i + 1] = v.y, w[4 * i + 2] = v.z, w[4 * i + 3] = v.w;
+      }
+    } else if constexpr (C::VEC == 8) {
+#pragma unroll
+      for (int i = 0; i < C::NVEC; ++i) {
+        const uint2 v = *reinterpret_cast<const uint2*>(unit + 8 * i);
+        w[2 * i] = v.x, w[2 * i + 1] = v.y;
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < C::NVEC; ++i) w[i] = *reinterpret_cast<const uint32_t*>(unit + 4 * i);
     }
-  } else if constexpr (C::VEC == 8) {
-#pragma unroll
-    for (int i = 0; i < C::NVEC; ++i) {
-      const uint2 v = *reinterpret_cast<const uint2*>(unit + 8 * i);
-      w[2 * i] = v.x, w[2 * i + 1] = v.y;
-    }
-  } else {
-#pragma unroll
-    for (int i = 0; i < C::NVEC; ++i) w[i] = *reinterpret_cast<const uint32_t*>(unit + 4 * i);
   }
 
   Result res[C::TPT];
   uint32_t p = fastmod(g0, n_pixels, pix_inv);
 #pragma unroll
   for (int j = 0; j < C::TPT; ++j) {
-    constexpr int dummy = 0;
-    (void)dummy;
     const int h0 = j * S;  // compile-time after unrolling
-    // a3 + a4 on raw samples: sliding sum, packed (sum, earliest) key
-    uint32_t sum = 0;
+    const uint16_t* tr0 = reinterpret_cast<const uint16_t*>(unit) + h0;
+    int tstar, rawsum, relnum = 0;
+    if constexpr (MODE == MODE_SLIDING) {
+      // a3 + a4 on raw samples: sliding sum, packed (sum, earliest) key
+      uint32_t sum = 0;
 #pragma unroll
-    for (int k = 0; k < W; ++k) sum += RTA_X(w, h0 + k);
-    uint32_t best = (sum << C::KB) | C::KM;
+      for (int k = 0; k < W; ++k) sum += RTA_X(w, h0 + k);
+      uint32_t best = (sum << C::KB) | C::KM;
 #pragma unroll
-    for (int t = 1; t < C::NWIN; ++t) {
-      sum = sum + RTA_X(w, h0 + t + W - 1) - RTA_X(w, h0 + t - 1);
-      const uint32_t key = (sum << C::KB) + (C::KM - (uint32_t)t);
-      best = max(best, key);
+      for (int t = 1; t < C::NWIN; ++t) {
+        sum = sum + RTA_X(w, h0 + t + W - 1) - RTA_X(w, h0 + t - 1);
+        const uint32_t key = (sum << C::KB) + (C::KM - (uint32_t)t);
+        best = max(best, key);
+      }
+      tstar = (int)(C::KM - (best & C::KM));
+      rawsum = (int)(best >> C::KB);
+      // a7 numerator: re-read the winning window (dynamic index -> shared memory)
+      const uint16_t* tr = tr0 + tstar;
+#pragma unroll
+      for (int k = 1; k < W; ++k) relnum += k * (int)tr[k];
+    } else if constexpr (MODE == MODE_FIR) {
+      // response on raw samples (the pedestal shifts every y(t) by the same
+      // c0*ped); signed compare, strict '>' scanning upwards = earliest on ties
+      int best = 0;
+#pragma unroll
+      for (int k = 0; k < W; ++k) best += ma.taps[k] * (int)RTA_X(w, h0 + k);
+      tstar = 0;
+#pragma unroll
+      for (int t = 1; t < C::NWIN; ++t) {
+        int y = 0;
+#pragma unroll
+        for (int k = 0; k < W; ++k) y += ma.taps[k] * (int)RTA_X(w, h0 + t + k);
+        if (y > best) {
+          best = y;
+          tstar = t;
+        }
+      }
+      rawsum = best;
+      const uint16_t* tr = tr0 + tstar;
+#pragma unroll
+      for (int k = 1; k < W; ++k) relnum += k * ma.taps[k] * (int)tr[k];
+    } else {
+      if constexpr (MODE == MODE_FIXED) {
+        tstar = clamp_start(__ldg(ma.window_start + p), S, W);
+      } else {  // MODE_LOCAL_PEAK: largest sample, earliest on ties, one max per sample
+        constexpr int PB = C::PB;
+        constexpr uint32_t PM = C::PM;
+        uint32_t best = (RTA_X(w, h0) << PB) | PM;
+#pragma unroll
+        for (int k = 1; k < S; ++k)
+          best = max(best, (RTA_X(w, h0 + k) << PB) + (PM - (uint32_t)k));
+        tstar = clamp_start((int)(PM - (best & PM)) - ma.shift, S, W);
+      }
+      const uint16_t* tr = tr0 + tstar;
+      rawsum = (int)tr[0];
+#pragma unroll
+      for (int k = 1; k < W; ++k) {
+        const int x = (int)tr[k];
+        rawsum += x;
+        relnum += k * x;
+      }
     }
-    const int tstar = (int)(C::KM - (best & C::KM));
-    const uint32_t rawsum = best >> C::KB;
-    // a7 numerator: re-read the winning window (dynamic index -> shared memory)
-    const uint16_t* tr = reinterpret_cast<const uint16_t*>(unit) + h0 + tstar;
-    uint32_t relnum = 0;
-#pragma unroll
-    for (int k = 1; k < W; ++k) relnum += (uint32_t)k * (uint32_t)tr[k];
     const int ped = __ldg(pedestal + p);
     const float gn = __ldg(gain + p);
-    res[j] = finish_trace(W, rawsum, tstar, relnum, ped, gn);
+    if constexpr (MODE == MODE_FIR)
+      res[j] = finish_trace(W, rawsum, tstar, relnum, ped, gn, ma.c0, ma.c1);
+    else
+      res[j] = finish_trace(W, rawsum, tstar, relnum, ped, gn, W, (W * (W - 1)) / 2);
     p = (p + 1 == n_pixels) ? 0u : p + 1;
   }
 
@@ -253,14 +324,15 @@ __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, c
 // the last CTA to leave zeroes them again, so the pair is reusable by the next
 // launch on the same stream (and by CUDA-graph replays). sched == nullptr
 // selects the static round-robin (same code path, locally generated indices).
-template <class C>
+template <class C, int MODE>
 __global__ void __launch_bounds__(C::NT)
     extract_tile_kernel(const uint16_t* __restrict__ wf, const uint32_t n_traces,
                         const uint32_t n_pixels, const uint32_t pix_inv,
                         const int* __restrict__ pedestal, const float* __restrict__ gain,
                         int* __restrict__ out_sum, int* __restrict__ out_start,
                         float* __restrict__ out_charge, float* __restrict__ out_time,
-                        const int vec_store, uint32_t* __restrict__ sched) {
+                        const int vec_store, uint32_t* __restrict__ sched,
+                        const __grid_constant__ ModeArgs ma) {
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ __align__(8) uint64_t full_bar[C::STAGES];
   constexpr int QN = C::STAGES + 1;  // queue of tile indices, one slot more than stages
@@ -362,8 +434,8 @@ __global__ void __launch_bounds__(C::NT)
     mbar_wait(bar_base + 8 * stage, parity);
     const uint8_t* unit = smem + stage * C::STAGE_BYTES + tid * C::UNIT_STRIDE;
     const uint32_t g0 = tile * C::TILE_TRACES + (uint32_t)tid * C::TPT;
-    compute_unit<C>(unit, g0, C::TPT, n_pixels, pix_inv, pedestal, gain, out_sum, out_start,
-                    out_charge, out_time, vec_store != 0);
+    compute_unit<C, MODE>(unit, g0, C::TPT, n_pixels, pix_inv, pedestal, gain, out_sum, out_start,
+                          out_charge, out_time, vec_store != 0, ma);
     __syncthreads();  // every thread is done with this stage; tile_q slot is published
     const uint32_t next = tile_q[(j + C::STAGES) % QN];
     if (next < n_full) issue(next, stage);
@@ -384,8 +456,8 @@ __global__ void __launch_bounds__(C::NT)
     if (first < rem) {
       const uint8_t* unit = smem + tid * C::UNIT_STRIDE;
       const uint32_t g0 = n_full * C::TILE_TRACES + first;
-      compute_unit<C>(unit, g0, rem - first, n_pixels, pix_inv, pedestal, gain, out_sum,
-                      out_start, out_charge, out_time, vec_store != 0);
+      compute_unit<C, MODE>(unit, g0, rem - first, n_pixels, pix_inv, pedestal, gain, out_sum,
+                            out_start, out_charge, out_time, vec_store != 0, ma);
     }
   }
 
@@ -403,30 +475,69 @@ __global__ void __launch_bounds__(C::NT)
 // -------------------------------------------------------- generic kernel ----
 // Any (S, W) inside the ABI guards, any 2-byte alignment: one thread per trace,
 // samples read straight from global memory (L1/L2 absorb the re-reads).
+template <int MODE>
 __global__ void __launch_bounds__(256)
     extract_generic_kernel(const uint16_t* __restrict__ wf, const uint32_t n_traces, const int S,
                            const int W, const uint32_t n_pixels, const uint32_t pix_inv,
                            const int* __restrict__ pedestal, const float* __restrict__ gain,
                            int* __restrict__ out_sum, int* __restrict__ out_start,
-                           float* __restrict__ out_charge, float* __restrict__ out_time) {
+                           float* __restrict__ out_charge, float* __restrict__ out_time,
+                           const __grid_constant__ ModeArgs ma) {
   for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < n_traces;
        g += gridDim.x * blockDim.x) {
     const uint16_t* tr = wf + (size_t)g * S;
-    uint32_t sum = 0;
-    for (int k = 0; k < W; ++k) sum += tr[k];
-    uint32_t best = sum;
-    int tstar = 0;
-    for (int t = 1; t + W <= S; ++t) {
-      sum = sum + tr[t + W - 1] - tr[t - 1];
-      if (sum > best) {  // strict: earliest on ties
-        best = sum;
-        tstar = t;
+    const uint32_t p = fastmod(g, n_pixels, pix_inv);
+    int tstar = 0, rawsum = 0, relnum = 0;
+    if constexpr (MODE == MODE_SLIDING) {
+      uint32_t sum = 0;
+      for (int k = 0; k < W; ++k) sum += tr[k];
+      uint32_t best = sum;
+      for (int t = 1; t + W <= S; ++t) {
+        sum = sum + tr[t + W - 1] - tr[t - 1];
+        if (sum > best) {  // strict: earliest on ties
+          best = sum;
+          tstar = t;
+        }
+      }
+      rawsum = (int)best;
+      for (int k = 1; k < W; ++k) relnum += k * (int)tr[tstar + k];
+    } else if constexpr (MODE == MODE_FIR) {
+      int best = 0;
+      for (int t = 0; t + W <= S; ++t) {
+        int y = 0;
+        for (int k = 0; k < W; ++k) y += ma.taps[k] * (int)tr[t + k];
+        if (t == 0 || y > best) {
+          best = y;
+          tstar = t;
+        }
+      }
+      rawsum = best;
+      for (int k = 1; k < W; ++k) relnum += k * ma.taps[k] * (int)tr[tstar + k];
+    } else {
+      if constexpr (MODE == MODE_FIXED) {
+        tstar = clamp_start(__ldg(ma.window_start + p), S, W);
+      } else {
+        int peak = 0;
+        uint32_t top = tr[0];
+        for (int k = 1; k < S; ++k) {
+          const uint32_t x = tr[k];
+          if (x > top) {
+            top = x;
+            peak = k;
+          }
+        }
+        tstar = clamp_start(peak - ma.shift, S, W);
+      }
+      for (int k = 0; k < W; ++k) {
+        const int x = (int)tr[tstar + k];
+        rawsum += x;
+        relnum += k * x;
       }
     }
-    uint32_t relnum = 0;
-    for (int k = 1; k < W; ++k) relnum += (uint32_t)k * (uint32_t)tr[tstar + k];
-    const uint32_t p = fastmod(g, n_pixels, pix_inv);
-    const Result r = finish_trace(W, best, tstar, relnum, __ldg(pedestal + p), __ldg(gain + p));
+    const int c0 = (MODE == MODE_FIR) ? ma.c0 : W;
+    const int c1 = (MODE == MODE_FIR) ? ma.c1 : (W * (W - 1)) / 2;
+    const Result r =
+        finish_trace(W, rawsum, tstar, relnum, __ldg(pedestal + p), __ldg(gain + p), c0, c1);
     out_sum[g] = r.sum;
     out_start[g] = r.start;
     out_charge[g] = r.charge;
@@ -503,19 +614,19 @@ uint32_t* sched_words(int dev, cudaStream_t stream) {
   return g_sched.base[dev] + (size_t)slot * kSchedSlotWords;
 }
 
-template <class C>
+template <class C, int MODE>
 struct TileLauncher {
   static std::atomic<int> ready[kMaxDevices];
   static int ctas_per_sm[kMaxDevices];
 
   static cudaError_t prepare(int dev) {
     if (ready[dev].load(std::memory_order_acquire)) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(extract_tile_kernel<C>,
+    cudaError_t e = cudaFuncSetAttribute(extract_tile_kernel<C, MODE>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          C::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     int occ = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, extract_tile_kernel<C>, C::NT,
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, extract_tile_kernel<C, MODE>, C::NT,
                                                       C::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     if (occ < 1) return cudaErrorLaunchOutOfResources;
@@ -527,7 +638,7 @@ struct TileLauncher {
   static cudaError_t launch(const uint16_t* wf, uint32_t n_traces, uint32_t n_pixels,
                             uint32_t pix_inv, const int32_t* pedestal, const float* gain,
                             int32_t* out_sum, int32_t* out_start, float* out_charge,
-                            float* out_time, cudaStream_t stream) {
+                            float* out_time, cudaStream_t stream, const ModeArgs& ma) {
     int dev = 0, sms = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
@@ -541,17 +652,17 @@ struct TileLauncher {
                         (uintptr_t)out_time;
     const int vec_store = (o % 8 == 0) ? 1 : 0;
     uint32_t* sched = g_static_schedule ? nullptr : sched_words(dev, stream);
-    extract_tile_kernel<C><<<grid, C::NT, C::SMEM_BYTES, stream>>>(
+    extract_tile_kernel<C, MODE><<<grid, C::NT, C::SMEM_BYTES, stream>>>(
         wf, n_traces, n_pixels, pix_inv, pedestal, gain, out_sum, out_start, out_charge, out_time,
-        vec_store, sched);
+        vec_store, sched, ma);
     rta_count_launch();
     return cudaGetLastError();
   }
 };
-template <class C>
-std::atomic<int> TileLauncher<C>::ready[kMaxDevices];
-template <class C>
-int TileLauncher<C>::ctas_per_sm[kMaxDevices];
+template <class C, int MODE>
+std::atomic<int> TileLauncher<C, MODE>::ready[kMaxDevices];
+template <class C, int MODE>
+int TileLauncher<C, MODE>::ctas_per_sm[kMaxDevices];
 
 // The four shapes of BASELINE.json:configs (NT, STAGES tuned on B200; see
 // DESIGN.md "Kernels" for the shared-memory budget of each).
@@ -619,39 +730,94 @@ const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16) {
   return "generic";
 }
 
-cudaError_t rta_launch_extract(const uint16_t* wf, int64_t n_traces64, int32_t n_pixels,
-                               int32_t S, const int32_t* pedestal, const float* gain, int32_t W,
-                               int32_t* out_sum, int32_t* out_start, float* out_charge,
-                               float* out_time, cudaStream_t stream, bool force_generic) {
-  if (n_traces64 <= 0) return cudaSuccess;
-  const uint32_t n_traces = (uint32_t)n_traces64;
-  const uint32_t P = (uint32_t)n_pixels;
-  const uint64_t inv64 = (1ull << 32) / P;
-  const uint32_t inv = inv64 > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)inv64;
-  const bool aligned16 = ((uintptr_t)wf % 16) == 0;
-  if (!force_generic && aligned16) {
-    if (S == 30 && W == 7)
-      return TileLauncher<CfgS30W7>::launch(wf, n_traces, P, inv, pedestal, gain, out_sum,
-                                            out_start, out_charge, out_time, stream);
-    if (S == 40 && W == 7)
-      return TileLauncher<CfgS40W7>::launch(wf, n_traces, P, inv, pedestal, gain, out_sum,
-                                            out_start, out_charge, out_time, stream);
-    if (S == 25 && W == 4)
-      return TileLauncher<CfgS25W4>::launch(wf, n_traces, P, inv, pedestal, gain, out_sum,
-                                            out_start, out_charge, out_time, stream);
-    if (S == 128 && W == 8)
-      return TileLauncher<CfgS128W8>::launch(wf, n_traces, P, inv, pedestal, gain, out_sum,
-                                             out_start, out_charge, out_time, stream);
+namespace {
+
+struct LaunchArgs {
+  const uint16_t* wf;
+  uint32_t n_traces, n_pixels, pix_inv;
+  int32_t S, W;
+  const int32_t* pedestal;
+  const float* gain;
+  int32_t *out_sum, *out_start;
+  float *out_charge, *out_time;
+  cudaStream_t stream;
+  bool staged;  // 16-byte aligned input and not forced to the generic kernel
+};
+
+template <int MODE>
+cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
+  if (a.staged) {
+#define RTA_TRY(CFG)                                                                          \
+  if (a.S == CFG::S && a.W == CFG::W)                                                         \
+    return TileLauncher<CFG, MODE>::launch(a.wf, a.n_traces, a.n_pixels, a.pix_inv,           \
+                                           a.pedestal, a.gain, a.out_sum, a.out_start,        \
+                                           a.out_charge, a.out_time, a.stream, ma);
+    RTA_TRY(CfgS30W7)
+    RTA_TRY(CfgS40W7)
+    RTA_TRY(CfgS25W4)
+    RTA_TRY(CfgS128W8)
+#undef RTA_TRY
   }
   int dev = 0, sms = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
-  uint32_t grid = (n_traces + 255u) / 256u;
+  uint32_t grid = (a.n_traces + 255u) / 256u;
   const uint32_t cap = (uint32_t)sms * 8u;
   if (grid > cap) grid = cap;
-  extract_generic_kernel<<<grid, 256, 0, stream>>>(wf, n_traces, S, W, P, inv, pedestal, gain,
-                                                   out_sum, out_start, out_charge, out_time);
+  extract_generic_kernel<MODE><<<grid, 256, 0, a.stream>>>(
+      a.wf, a.n_traces, a.S, a.W, a.n_pixels, a.pix_inv, a.pedestal, a.gain, a.out_sum,
+      a.out_start, a.out_charge, a.out_time, ma);
   rta_count_launch();
   return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t rta_launch_extract(const uint16_t* wf, int64_t n_traces64, int32_t n_pixels,
+                               int32_t S, const int32_t* pedestal, const float* gain, int32_t W,
+                               int32_t* out_sum, int32_t* out_start, float* out_charge,
+                               float* out_time, cudaStream_t stream, bool force_generic,
+                               const RtaMode* mode) {
+  if (n_traces64 <= 0) return cudaSuccess;
+  const uint32_t P = (uint32_t)n_pixels;
+  const uint64_t inv64 = (1ull << 32) / P;
+  LaunchArgs a;
+  a.wf = wf;
+  a.n_traces = (uint32_t)n_traces64;
+  a.n_pixels = P;
+  a.pix_inv = inv64 > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)inv64;
+  a.S = S;
+  a.W = W;
+  a.pedestal = pedestal;
+  a.gain = gain;
+  a.out_sum = out_sum;
+  a.out_start = out_start;
+  a.out_charge = out_charge;
+  a.out_time = out_time;
+  a.stream = stream;
+  a.staged = !force_generic && ((uintptr_t)wf % 16) == 0;
+  ModeArgs ma = {};
+  const int kind = mode ? mode->kind : RTA_MODE_SLIDING;
+  switch (kind) {
+    case RTA_MODE_SLIDING:
+      return launch_mode<MODE_SLIDING>(a, ma);
+    case RTA_MODE_FIXED:
+      ma.window_start = mode->window_start;
+      return launch_mode<MODE_FIXED>(a, ma);
+    case RTA_MODE_LOCAL_PEAK:
+      ma.shift = mode->shift;
+      return launch_mode<MODE_LOCAL_PEAK>(a, ma);
+    case RTA_MODE_FIR: {
+      // W == mode->n_taps (checked by the caller)
+      for (int k = 0; k < W; ++k) {
+        ma.taps[k] = mode->taps[k];
+        ma.c0 += mode->taps[k];
+        ma.c1 += k * mode->taps[k];
+      }
+      return launch_mode<MODE_FIR>(a, ma);
+    }
+    default:
+      return cudaErrorInvalidValue;
+  }
 }

@@ -124,3 +124,34 @@ def test_shard_events_partitions_exactly():
             for (a, ca), (b, _) in zip(parts, parts[1:]):
                 assert a + ca == b
             assert max(c for _, c in parts) - min(c for _, c in parts) <= 1
+
+
+# ---- extractor family (rta_extract_fixed / _local_peak / _fir) ---------------
+def _taps(vals):
+    return (ctypes.c_int32 * len(vals))(*vals)
+
+
+def test_family_entry_points_validate_before_any_cuda_call():
+    L = rta.lib()
+    o = (0x4000, 0x5000, 0x6000, 0x7000)
+    fixed = lambda **k: L.rta_extract_fixed(k.get("wf", 0x1000), k.get("E", 1), 4, 30, 0x2000, 0x3000,
+                                            k.get("W", 7), k.get("ws", 0x8000), *o, 0)
+    assert fixed(W=31) == rta.RTA_ERR_SHAPE
+    assert fixed(ws=None) == rta.RTA_ERR_NULL
+    assert fixed(ws=0x8002) == rta.RTA_ERR_ALIGN
+    assert fixed(wf=None) == rta.RTA_ERR_NULL
+    assert fixed(E=0, wf=None, ws=None) == rta.RTA_OK
+    peak = lambda **k: L.rta_extract_local_peak(k.get("wf", 0x1000), k.get("E", 1), 4, 30, 0x2000, 0x3000,
+                                                k.get("W", 7), k.get("shift", 3), *o, 0)
+    assert peak(W=0) == rta.RTA_ERR_SHAPE
+    assert peak(wf=0x1001) == rta.RTA_ERR_ALIGN
+    assert peak(E=0, wf=None) == rta.RTA_OK
+    fir = lambda taps, S=30, E=1, wf=0x1000: L.rta_extract_fir(
+        wf, E, 4, S, 0x2000, 0x3000, _taps(taps) if taps is not None else None,
+        len(taps) if taps is not None else 3, *o, 0)
+    assert fir([1] * 31) == rta.RTA_ERR_SHAPE              # more taps than samples
+    assert fir([1] * 33, S=64) == rta.RTA_ERR_UNSUPPORTED  # more than 32 taps
+    assert fir(None) == rta.RTA_ERR_NULL
+    assert fir([20000, -20000], S=30) == rta.RTA_ERR_UNSUPPORTED   # 30*40000*65535 >= 2^31
+    assert fir([1, 2, 1], wf=None) == rta.RTA_ERR_NULL
+    assert fir([1, 2, 1], E=0, wf=None) == rta.RTA_OK
