@@ -145,6 +145,8 @@ def _cpu_lib():
         lib.dl0gen_events_cpu.restype = None
         lib.dl0gen_events_cpu.argtypes = [ctypes.POINTER(Params), ctypes.c_int64,
                                           ctypes.c_int64, ctypes.c_void_p]
+        lib.dl0gen_pack12_cpu.restype = None
+        lib.dl0gen_pack12_cpu.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p]
         _cpu = lib
     return _cpu
 
@@ -156,6 +158,9 @@ def _cuda_lib():
         lib.dl0gen_events_cuda.restype = ctypes.c_int
         lib.dl0gen_events_cuda.argtypes = [ctypes.POINTER(Params), ctypes.c_longlong,
                                            ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
+        lib.dl0gen_pack12_cuda.restype = ctypes.c_int
+        lib.dl0gen_pack12_cuda.argtypes = [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p,
+                                           ctypes.c_void_p]
         _cuda = lib
     return _cuda
 
@@ -202,3 +207,25 @@ def events_cuda(cfg: Config, wf_dev_ptr: int, first_event: int, n_events: int,
                                         ctypes.c_void_p(wf_dev_ptr), ctypes.c_void_p(stream))
     if rc != 0:
         raise RuntimeError("dl0gen_events_cuda: cudaError %d" % rc)
+
+
+def packed12_nbytes(n_samples_total: int) -> int:
+    """Bytes of a P12 stream (12-bit little-endian packed) of that many samples."""
+    return (12 * int(n_samples_total) + 7) // 8
+
+
+def pack12_cpu(wf: np.ndarray) -> np.ndarray:
+    """Encode uint16 samples (any shape, flattened in C order, masked to 12 bits)
+    as a P12 byte stream. Input preparation only: decoding is the method's step."""
+    wf = np.ascontiguousarray(wf, dtype=np.uint16).ravel()
+    out = np.empty(packed12_nbytes(wf.size), np.uint8)
+    _cpu_lib().dl0gen_pack12_cpu(wf.ctypes.data, wf.size, out.ctypes.data)
+    return out
+
+
+def pack12_cuda(wf_dev_ptr: int, n_samples_total: int, out_dev_ptr: int, stream: int = 0) -> None:
+    """Device build of :func:`pack12_cpu` (raw device pointers; async on ``stream``)."""
+    rc = _cuda_lib().dl0gen_pack12_cuda(ctypes.c_void_p(wf_dev_ptr), int(n_samples_total),
+                                        ctypes.c_void_p(out_dev_ptr), ctypes.c_void_p(stream))
+    if rc != 0:
+        raise RuntimeError("dl0gen_pack12_cuda: cudaError %d" % rc)

@@ -29,3 +29,21 @@ void dl0gen_events_cpu(const dl0gen_params* q, int64_t first_event,
     }
   }
 }
+
+/* P12 encoder (input preparation for the packed-ingest path; the DECODER is
+ * the method's step and lives in oracle/ and in the CUDA library, not here).
+ * Samples are masked to 12 bits. out holds (12 n + 7) / 8 bytes. */
+void dl0gen_pack12_cpu(const uint16_t* in, int64_t n, uint8_t* out) {
+  int64_t k = 0;
+  for (; 2 * k + 1 < n; ++k) {
+    const unsigned a = in[2 * k] & 0xFFFu, b = in[2 * k + 1] & 0xFFFu;
+    out[3 * k] = (uint8_t)(a & 0xFFu);
+    out[3 * k + 1] = (uint8_t)((a >> 8) | ((b & 0xFu) << 4));
+    out[3 * k + 2] = (uint8_t)(b >> 4);
+  }
+  if (2 * k < n) {
+    const unsigned a = in[2 * k] & 0xFFFu;
+    out[3 * k] = (uint8_t)(a & 0xFFu);
+    out[3 * k + 1] = (uint8_t)(a >> 8);
+  }
+}

@@ -40,3 +40,32 @@ extern "C" int dl0gen_events_cuda(const dl0gen_params* q, long long first_event,
       *q, first_event, n_traces, wf_dev);
   return (int)cudaGetLastError();
 }
+
+// P12 encoder on the device (input preparation only; see dl0gen_cpu.c).
+// One thread packs 8 samples into 3 words; n is the sample count.
+__global__ void dl0gen_pack12_kernel(const unsigned short* __restrict__ in, long long n,
+                                     unsigned char* __restrict__ out) {
+  const long long npairs = (n + 1) / 2;
+  for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < npairs;
+       k += (long long)gridDim.x * blockDim.x) {
+    const unsigned a = in[2 * k] & 0xFFFu;
+    if (2 * k + 1 < n) {
+      const unsigned b = in[2 * k + 1] & 0xFFFu;
+      out[3 * k] = (unsigned char)(a & 0xFFu);
+      out[3 * k + 1] = (unsigned char)((a >> 8) | ((b & 0xFu) << 4));
+      out[3 * k + 2] = (unsigned char)(b >> 4);
+    } else {
+      out[3 * k] = (unsigned char)(a & 0xFFu);
+      out[3 * k + 1] = (unsigned char)(a >> 8);
+    }
+  }
+}
+
+extern "C" int dl0gen_pack12_cuda(const unsigned short* in_dev, long long n,
+                                  unsigned char* out_dev, void* stream) {
+  if (n <= 0) return 0;
+  long long blocks = ((n + 1) / 2 + 255) / 256;
+  if (blocks > 148LL * 64) blocks = 148LL * 64;
+  dl0gen_pack12_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(in_dev, n, out_dev);
+  return (int)cudaGetLastError();
+}

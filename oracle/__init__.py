@@ -20,7 +20,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rta_oracle.cpp")
-_SRCS = [_SRC, os.path.join(_HERE, "rta_oracle_windows.cpp")]
+_SRCS = [_SRC, os.path.join(_HERE, "rta_oracle_windows.cpp"),
+         os.path.join(_HERE, "rta_oracle_packed.cpp")]
 _LIB = os.path.join(_HERE, "librta_oracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -58,6 +59,10 @@ def _load():
         lib.rta_oracle_extract_local_peak.argtypes = common + [ctypes.c_int32, ctypes.c_int32] + outs
         lib.rta_oracle_extract_fir.restype = ctypes.c_int
         lib.rta_oracle_extract_fir.argtypes = common + [ctypes.c_void_p, ctypes.c_int32] + outs
+        lib.rta_oracle_unpack12.restype = ctypes.c_int
+        lib.rta_oracle_unpack12.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p]
+        lib.rta_oracle_extract_packed12.restype = ctypes.c_int
+        lib.rta_oracle_extract_packed12.argtypes = lib.rta_oracle_extract.argtypes
         _lib = lib
     return _lib
 
@@ -145,6 +150,41 @@ def extract(wf: np.ndarray, pedestal: np.ndarray, gain: np.ndarray, W: int):
     if rc != 0:
         raise ValueError("rta_oracle_extract: bad shape (S=%d, W=%d)" % (S, W))
     return out_sum, out_start, out_charge, out_time
+
+
+def packed12_nbytes(n_total: int) -> int:
+    """Bytes of a P12 stream holding ``n_total`` samples: ceil(12 n / 8)."""
+    return (12 * int(n_total) + 7) // 8
+
+
+def unpack12(packed, n_total: int) -> np.ndarray:
+    """Decode ``n_total`` samples of a P12 stream (rta_oracle_packed.cpp, readings R25-R27)."""
+    packed = np.ascontiguousarray(packed, dtype=np.uint8).ravel()
+    if packed.size < packed12_nbytes(n_total):
+        raise ValueError("P12 stream too short: %d bytes for %d samples" % (packed.size, n_total))
+    out = np.empty(int(n_total), np.uint16)
+    if _load().rta_oracle_unpack12(packed.ctypes.data, int(n_total), out.ctypes.data) != 0:
+        raise ValueError("rta_oracle_unpack12: bad size")
+    return out
+
+
+def extract_packed12(packed, n_events: int, pedestal, gain, n_samples: int, W: int):
+    """Sliding-window extraction of a P12 stream of ``n_events x len(pedestal) x n_samples``."""
+    pedestal = np.ascontiguousarray(pedestal, dtype=np.int32)
+    gain = np.ascontiguousarray(gain, dtype=np.float32)
+    P = pedestal.size
+    packed = np.ascontiguousarray(packed, dtype=np.uint8).ravel()
+    if packed.size < packed12_nbytes(n_events * P * n_samples):
+        raise ValueError("P12 stream too short")
+    n = int(n_events) * P
+    outs = (np.empty(n, np.int32), np.empty(n, np.int32), np.empty(n, np.float32),
+            np.empty(n, np.float32))
+    rc = _load().rta_oracle_extract_packed12(
+        packed.ctypes.data, int(n_events), P, int(n_samples), pedestal.ctypes.data,
+        gain.ctypes.data, int(W), *[o.ctypes.data for o in outs])
+    if rc != 0:
+        raise ValueError("rta_oracle_extract_packed12: bad shape")
+    return outs
 
 
 def extract_threads(wf, pedestal, gain, W, threads: int):
