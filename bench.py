@@ -18,6 +18,10 @@ Prints ONE JSON line (rank 0). Keys beyond the driver's contract:
                 host-link bandwidth measured in the same run and the paper's
                 0.5-8 GB/s array data rate
   configs       kernel-only numbers for the other single-GPU configs (C3, C4)
+  family        the other extractors (NEXT-1) on the same batches
+  packed12      NEXT-2: the same batches as P12 streams (12 bits per sample),
+                decoded inside the extraction kernel; sustained.packed12 is C5
+                fed as 22.26 GB of P12 through rta_extract_stream_packed12
 """
 from __future__ import annotations
 
@@ -308,6 +312,38 @@ def family_leg(cfg, steps, peak, torch, dl0gen, rta):
     return res
 
 
+def packed_leg(cfg, steps, peak, torch, dl0gen, rta):
+    """Kernel-only throughput of rta_extract_packed12 on the batch of `cfg`
+    stored as a P12 stream (1.5 bytes per sample instead of 2)."""
+    d_wf, d_ped, d_gain, outs, ped, gain = device_batch(cfg, torch, dl0gen)
+    stream = torch.cuda.current_stream()
+    n_total = cfg.n_traces * cfg.n_samples
+    nb = dl0gen.packed12_nbytes(n_total)
+    d_pk = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    dl0gen.pack12_cuda(d_wf.data_ptr(), n_total, d_pk.data_ptr(), stream.cuda_stream)
+    torch.cuda.synchronize()
+    del d_wf
+
+    def run():
+        rta.rta_extract_packed12(d_pk, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain,
+                                 cfg.W, *outs, stream=stream)
+    for _ in range(3):
+        run()
+    torch.cuda.synchronize()
+    per = time_steps(run, steps, stream)
+    avg = sum(per) / len(per)
+    algo = nb + cfg.output_bytes
+    return {"workload": "%s as P12: %s" % (cfg.name, cfg.label),
+            "kernel": rta.rta_kernel_name_packed12(cfg.n_samples, cfg.W, True),
+            "ms_avg": avg, "ms_median": statistics.median(per), "ms_best": min(per),
+            "packed_input_bytes": nb, "algorithmic_bytes_per_launch": algo,
+            "bytes_per_trace": 1.5 * cfg.n_samples + ALGO_BYTES_PER_TRACE_OUT,
+            "algorithmic_GBps": algo / avg / 1e6, "frac_of_measured_hbm": algo / avg / 1e6 / peak,
+            "packed_GBps": nb / avg / 1e6,
+            "waveform_equivalent_GBps": cfg.input_bytes / avg / 1e6,
+            "traces_per_s": cfg.n_traces / avg * 1e3}
+
+
 def host_link_bandwidth(torch, nbytes=1 << 30, reps=10):
     """Pinned H2D cudaMemcpyAsync bandwidth, best of `reps` (the H2D-fed roofline)."""
     h = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
@@ -406,6 +442,52 @@ def sustained_leg(torch, dl0gen, rta, link_gbs):
            "paper_array_rate_GBps": list(PAPER_RATE_GBS),
            "x_paper_max_rate": val / PAPER_RATE_GBS[1],
            "pinned_alloc_s": t_alloc, "outputs": "stay on device (5.94 GB)"}
+    # NEXT-2: the same 200 000 events as a P12 stream (22.26 GB) in the same pinned
+    # buffer, through rta_extract_stream_packed12 (chunks of 9644 events = 1.07 GB)
+    try:
+        ev_samples = cfg.n_pixels * cfg.n_samples
+        nb = dl0gen.packed12_nbytes(cfg.n_traces * cfg.n_samples)
+        hp = host.view(-1).view(torch.uint8)[:nb]
+        stage = torch.empty((gen_ev, cfg.n_pixels, cfg.n_samples), dtype=torch.int16, device="cuda")
+        stage_pk = torch.empty(gen_ev * ev_samples * 3 // 2, dtype=torch.uint8, device="cuda")
+        for e0 in range(0, cfg.n_events, gen_ev):
+            dl0gen.events_cuda(cfg, stage.data_ptr(), e0, gen_ev, st)
+            dl0gen.pack12_cuda(stage.data_ptr(), gen_ev * ev_samples, stage_pk.data_ptr(), st)
+            b0 = e0 * ev_samples * 3 // 2
+            hp[b0:b0 + stage_pk.numel()].copy_(stage_pk)
+        torch.cuda.synchronize()
+        del stage, stage_pk
+        want = [o[:64 * cfg.n_pixels].clone() for o in outs]     # uint16-path result, first events
+        for o in outs:
+            o.zero_()
+
+        def run12():
+            rta.rta_extract_stream_packed12(hp, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped,
+                                            d_gain, cfg.W, *outs, chunk_bytes=1 << 30, stream=stream)
+        run12()
+        torch.cuda.synchronize()
+        same = all(bool((o[:64 * cfg.n_pixels] == w).all()) for o, w in zip(outs, want))
+        times = []
+        before = rta.rta_launch_count()
+        for _ in range(2):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            run12()
+            torch.cuda.synchronize()
+            times.append(time.perf_counter() - t0)
+        dt12 = min(times)
+        res["packed12"] = {
+            "value": cfg.input_bytes / dt12 / 1e9, "unit": UNIT,
+            "meaning": "raw-waveform-equivalent GB/s (2 bytes per sample) of the same 200000 events",
+            "seconds": dt12, "h2d_bytes": nb, "link_GBps": nb / dt12 / 1e9,
+            "frac_of_host_link": nb / dt12 / 1e9 / link_gbs,
+            "chunks": (rta.rta_launch_count() - before) // 2,
+            "chunk_events": rta.rta_chunk_events(cfg.n_events, cfg.n_pixels, cfg.n_samples, 1 << 30, 12),
+            "traces_per_s": cfg.n_traces / dt12, "x_paper_max_rate": cfg.input_bytes / dt12 / 1e9 / PAPER_RATE_GBS[1],
+            "speedup_vs_uint16_feed": dt / dt12,
+            "first_64_events_equal_uint16_path": same}
+    except Exception as ex:  # the uint16 leg above stands on its own
+        res["packed12"] = {"error": repr(ex)}
     del host, outs
     rta.rta_shutdown()
     return res
@@ -552,6 +634,12 @@ def main():
                                        torch, dl0gen, rta)
                 torch.cuda.empty_cache()
             out["family"] = fam
+            pk = {}
+            for name in ("C2", "C3", "C4"):
+                pk[name] = packed_leg(dl0gen.CONFIGS[name], max(10, args.steps // 4), peak,
+                                      torch, dl0gen, rta)
+                torch.cuda.empty_cache()
+            out["packed12"] = pk
             link = host_link_bandwidth(torch)
             out["e2e"]["host_link_GBps_measured"] = link
             out["e2e"]["frac_of_host_link"] = out["e2e"]["value"] / link

@@ -43,7 +43,7 @@ enum {
   RTA_ERR_NULL = 1,        /* a required pointer is NULL while there is work to do */
   RTA_ERR_SHAPE = 2,       /* n_events < 0, n_pixels < 1, n_samples < 1, W < 1 or W > n_samples */
   RTA_ERR_UNSUPPORTED = 3, /* n_events*n_pixels >= 2^31, or n_samples*W*65535 >= 2^31 (int32 guard) */
-  RTA_ERR_ALIGN = 4,       /* wf is not 2-byte aligned / an output is not 4-byte aligned */
+  RTA_ERR_ALIGN = 4,       /* wf is not 2-byte aligned / an output is not 4-byte aligned (P12: any byte) */
   RTA_ERR_CUDA = 5,        /* CUDA runtime failure; see rta_last_cuda_error() */
   RTA_ERR_NOMEM = 6        /* workspace allocation failed (device or pinned host) */
 };
@@ -146,6 +146,52 @@ int rta_extract_host(const uint16_t* wf_host, int64_t n_events, int32_t n_pixels
                      int32_t* out_start_host, float* out_charge_host,
                      float* out_time_host, size_t chunk_bytes);
 
+/* ---- Packed 12-bit ingest -----------------------------
+ * The paper's Event-Builder simulator emits DL0 data as "a logical sequence of
+ * bits ... according with the definition of the satellite telemetry [12]"
+ * (§5); the format itself is not given and refs [11], [12] are
+ * unavailable, so the packed format is defined here (readings R25-R27).
+ *
+ * "P12": the dense sample stream wf[e][p][s] (flat sample index
+ * n = (e*n_pixels + p)*n_samples + s; no headers, no padding between traces or
+ * events) stored 12 bits per sample, little-endian in bits: sample n occupies
+ * bits [12 n, 12 n + 12) of the stream, bit b of the stream being bit (b % 8) of
+ * byte (b / 8). For a = sample 2k, b = sample 2k+1:
+ *     byte 3k = a & 0xFF;  byte 3k+1 = (a >> 8) | ((b & 0xF) << 4);  byte 3k+2 = b >> 4.
+ * The stream holds ceil(12 N / 8) bytes for N samples; with N odd the high
+ * nibble of the last byte is padding and is ignored. The library never reads a
+ * byte past ceil(12 N / 8).
+ *
+ * The three calls below decode the stream inside the extraction kernel (no
+ * unpacked copy ever exists in device memory) and then compute exactly what
+ * rta_extract / rta_extract_stream / rta_extract_host compute on the decoded
+ * samples; every other argument, output, error and ordering rule is theirs.
+ *
+ *   packed   uint8, ceil(12 * n_events*n_pixels*n_samples / 8) bytes, any byte
+ *            alignment (DEVICE for rta_extract_packed12, HOST for the other two).
+ *            A 16-byte-aligned device pointer takes the staged kernels.
+ *   chunk_bytes (host-fed calls): bytes of the PACKED stream per chunk; chunks
+ *            hold whole events and start on a 16-byte boundary of the stream, so
+ *            the event count per chunk is rounded down to a multiple of
+ *            m = 32 / gcd(n_pixels*n_samples, 32) (at least m events); 0 = 1 GiB. */
+int rta_extract_packed12(const uint8_t* packed, int64_t n_events, int32_t n_pixels,
+                         int32_t n_samples, const int32_t* pedestal, const float* gain,
+                         int32_t W, int32_t* out_sum, int32_t* out_start,
+                         float* out_charge, float* out_time, void* stream);
+
+int rta_extract_stream_packed12(const uint8_t* packed_host, int64_t n_events,
+                                int32_t n_pixels, int32_t n_samples,
+                                const int32_t* pedestal, const float* gain, int32_t W,
+                                int32_t* out_sum, int32_t* out_start, float* out_charge,
+                                float* out_time, size_t chunk_bytes, void* stream);
+
+int rta_extract_host_packed12(const uint8_t* packed_host, int64_t n_events,
+                              int32_t n_pixels, int32_t n_samples,
+                              const int32_t* pedestal_host, const float* gain_host,
+                              int32_t W, int32_t* out_sum_host, int32_t* out_start_host,
+                              float* out_charge_host, float* out_time_host,
+                              size_t chunk_bytes);
+
 /* Static, never-NULL description of a status code. */
 const char* rta_strerror(int status);
 
@@ -156,6 +202,16 @@ int rta_last_cuda_error(void);
 /* Which kernel a shape takes, for tests and profiles: writes a static string
  * such as "tile<S=40,W=7>" or "generic" for (n_samples, W, 16-byte-aligned?). */
 const char* rta_kernel_name(int32_t n_samples, int32_t W, int aligned16);
+/* Same for a P12 stream: "tile12<S=40,W=7>", "generic12", ... */
+const char* rta_kernel_name_packed12(int32_t n_samples, int32_t W, int aligned16);
+
+/* Events per chunk the host-fed calls use for this shape and `chunk_bytes`
+ * (sample_bits 16: rta_extract_stream / _host; 12: the _packed12 calls): whole
+ * events, rounded down, at least one (P12: a multiple of m, see above), never
+ * more than n_events (1 when n_events is 0). Pure host arithmetic; -1 on a bad
+ * shape or sample_bits. */
+int64_t rta_chunk_events(int64_t n_events, int32_t n_pixels, int32_t n_samples,
+                         size_t chunk_bytes, int32_t sample_bits);
 
 /* Number of kernels the library has launched in this process (all threads);
  * bench.py reports the difference over its timed region as gpu_launches. */

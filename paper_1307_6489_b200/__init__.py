@@ -54,6 +54,14 @@ def lib() -> ctypes.CDLL:
             L.rta_extract_stream.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t, _VP]
             L.rta_extract_host.restype = ctypes.c_int
             L.rta_extract_host.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t]
+            L.rta_extract_packed12.restype = ctypes.c_int
+            L.rta_extract_packed12.argtypes = _EXTRACT_ARGS + [_VP]
+            L.rta_extract_stream_packed12.restype = ctypes.c_int
+            L.rta_extract_stream_packed12.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t, _VP]
+            L.rta_extract_host_packed12.restype = ctypes.c_int
+            L.rta_extract_host_packed12.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t]
+            L.rta_kernel_name_packed12.restype = ctypes.c_char_p
+            L.rta_kernel_name_packed12.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int]
             L.rta_extract_fixed.restype = ctypes.c_int
             L.rta_extract_fixed.argtypes = _EXTRACT_ARGS[:7] + [_VP] + [_VP] * 4 + [_VP]
             L.rta_extract_local_peak.restype = ctypes.c_int
@@ -68,6 +76,9 @@ def lib() -> ctypes.CDLL:
             L.rta_last_cuda_error.argtypes = []
             L.rta_kernel_name.restype = ctypes.c_char_p
             L.rta_kernel_name.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int]
+            L.rta_chunk_events.restype = ctypes.c_int64
+            L.rta_chunk_events.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32,
+                                           ctypes.c_size_t, ctypes.c_int32]
             L.rta_launch_count.restype = ctypes.c_uint64
             L.rta_launch_count.argtypes = []
             L.rta_shutdown.restype = None
@@ -169,6 +180,36 @@ def rta_extract_host(wf_host, n_events, n_pixels, n_samples, pedestal_host, gain
         _ptr(out_charge_host), _ptr(out_time_host), int(chunk_bytes)))
 
 
+def rta_extract_packed12(packed, n_events, n_pixels, n_samples, pedestal, gain, W,
+                         out_sum, out_start, out_charge, out_time, stream=None) -> None:
+    """include/rta.h:rta_extract_packed12. ``packed`` is a device P12 byte stream."""
+    _check(lib().rta_extract_packed12(
+        _ptr(packed), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain), W,
+        _ptr(out_sum), _ptr(out_start), _ptr(out_charge), _ptr(out_time),
+        _stream_handle(stream)))
+
+
+def rta_extract_stream_packed12(packed_host, n_events, n_pixels, n_samples, pedestal, gain, W,
+                                out_sum, out_start, out_charge, out_time, chunk_bytes=0,
+                                stream=None) -> None:
+    """include/rta.h:rta_extract_stream_packed12. ``packed_host`` is a host P12
+    byte stream; calibration and outputs are device pointers."""
+    _check(lib().rta_extract_stream_packed12(
+        _ptr(packed_host), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain), W,
+        _ptr(out_sum), _ptr(out_start), _ptr(out_charge), _ptr(out_time),
+        int(chunk_bytes), _stream_handle(stream)))
+
+
+def rta_extract_host_packed12(packed_host, n_events, n_pixels, n_samples, pedestal_host,
+                              gain_host, W, out_sum_host, out_start_host, out_charge_host,
+                              out_time_host, chunk_bytes=0) -> None:
+    """include/rta.h:rta_extract_host_packed12. Every pointer is host memory; synchronous."""
+    _check(lib().rta_extract_host_packed12(
+        _ptr(packed_host), n_events, n_pixels, n_samples, _ptr(pedestal_host),
+        _ptr(gain_host), W, _ptr(out_sum_host), _ptr(out_start_host),
+        _ptr(out_charge_host), _ptr(out_time_host), int(chunk_bytes)))
+
+
 def rta_strerror(status: int) -> str:
     return lib().rta_strerror(status).decode()
 
@@ -181,6 +222,16 @@ def rta_kernel_name(n_samples: int, W: int, aligned16: bool = True) -> str:
     return lib().rta_kernel_name(n_samples, W, 1 if aligned16 else 0).decode()
 
 
+def rta_kernel_name_packed12(n_samples: int, W: int, aligned16: bool = True) -> str:
+    return lib().rta_kernel_name_packed12(n_samples, W, 1 if aligned16 else 0).decode()
+
+
+def rta_chunk_events(n_events: int, n_pixels: int, n_samples: int, chunk_bytes: int = 0,
+                     sample_bits: int = 16) -> int:
+    """include/rta.h:rta_chunk_events."""
+    return int(lib().rta_chunk_events(n_events, n_pixels, n_samples, int(chunk_bytes), sample_bits))
+
+
 def rta_launch_count() -> int:
     return int(lib().rta_launch_count())
 
@@ -190,7 +241,7 @@ def rta_shutdown() -> None:
 
 
 def rta_debug_force_generic(on: bool) -> None:
-    """Test hook: route rta_extract_fixed/_local_peak/_fir to the generic kernel."""
+    """Test hook: route rta_extract_fixed/_local_peak/_fir/_packed12 to the generic kernel."""
     lib().rta_debug_force_generic(1 if on else 0)
 
 

@@ -27,14 +27,14 @@ int fail_cuda(cudaError_t e) {
 
 int validate(const void* wf, int64_t n_events, int32_t n_pixels, int32_t n_samples,
              const void* pedestal, const void* gain, int32_t W, const void* o0, const void* o1,
-             const void* o2, const void* o3) {
+             const void* o2, const void* o3, int wf_align = 2) {
   if (n_events < 0 || n_pixels < 1 || n_samples < 1 || W < 1 || W > n_samples)
     return RTA_ERR_SHAPE;
   if (n_events * (int64_t)n_pixels >= (1ll << 31)) return RTA_ERR_UNSUPPORTED;
   if ((int64_t)n_samples * (int64_t)W * 65535ll >= (1ll << 31)) return RTA_ERR_UNSUPPORTED;
   if (n_events == 0) return RTA_OK;
   if (!wf || !pedestal || !gain || !o0 || !o1 || !o2 || !o3) return RTA_ERR_NULL;
-  if ((uintptr_t)wf % 2 != 0) return RTA_ERR_ALIGN;
+  if ((uintptr_t)wf % (uintptr_t)wf_align != 0) return RTA_ERR_ALIGN;
   if (((uintptr_t)o0 | (uintptr_t)o1 | (uintptr_t)o2 | (uintptr_t)o3 | (uintptr_t)pedestal |
        (uintptr_t)gain) % 4 != 0)
     return RTA_ERR_ALIGN;
@@ -153,14 +153,31 @@ bool is_pageable(const void* p) {
 struct ChunkPlan {
   int64_t chunk_events;
   int64_t n_chunks;
-  size_t event_bytes;
+  size_t event_bits;   // bits of one event in the source format
 };
-ChunkPlan plan_chunks(int64_t n_events, int32_t n_pixels, int32_t n_samples, size_t chunk_bytes) {
+int64_t gcd64(int64_t a, int64_t b) {
+  while (b) {
+    const int64_t t = a % b;
+    a = b;
+    b = t;
+  }
+  return a;
+}
+// Chunks of whole events of at most chunk_bytes (rounded down, at least one
+// event). A P12 chunk must also start on a 16-byte boundary of the stream
+// (whole bytes for the copy, 16 bytes for the staged kernels): its event count
+// is a multiple of m, the smallest count with m * n_pixels * n_samples % 32 == 0.
+ChunkPlan plan_chunks(int64_t n_events, int32_t n_pixels, int32_t n_samples, size_t chunk_bytes,
+                      int bits) {
   ChunkPlan p;
-  p.event_bytes = (size_t)n_pixels * (size_t)n_samples * 2u;
+  const int64_t ev_samples = (int64_t)n_pixels * (int64_t)n_samples;
+  p.event_bits = (size_t)ev_samples * (size_t)bits;
   if (chunk_bytes == 0) chunk_bytes = (size_t)1 << 30;
-  int64_t ce = (int64_t)(chunk_bytes / p.event_bytes);  // rounded down to whole events
-  if (ce < 1) ce = 1;
+  const int64_t m = bits == 12 ? 32 / gcd64(ev_samples, 32) : 1;
+  int64_t ce = (int64_t)((chunk_bytes / p.event_bits) * 8u +
+                         ((chunk_bytes % p.event_bits) * 8u) / p.event_bits);  // whole events
+  ce -= ce % m;
+  if (ce < m) ce = m;
   if (ce > n_events) ce = n_events > 0 ? n_events : 1;
   p.chunk_events = ce;
   p.n_chunks = (n_events + ce - 1) / ce;
@@ -176,13 +193,13 @@ struct HostOut {
   float* time;
 };
 
-int stream_impl(Workspace& w, const uint16_t* wf_host, int64_t n_events, int32_t n_pixels,
+int stream_impl(Workspace& w, const void* wf_host, int64_t n_events, int32_t n_pixels,
                 int32_t n_samples, const int32_t* pedestal, const float* gain, int32_t W,
                 int32_t* out_sum, int32_t* out_start, float* out_charge, float* out_time,
-                size_t chunk_bytes, cudaStream_t stream, const HostOut* host_out) {
+                size_t chunk_bytes, cudaStream_t stream, const HostOut* host_out, int bits = 16) {
   cudaError_t e;
-  const ChunkPlan plan = plan_chunks(n_events, n_pixels, n_samples, chunk_bytes);
-  const size_t buf_bytes = (size_t)plan.chunk_events * plan.event_bytes;
+  const ChunkPlan plan = plan_chunks(n_events, n_pixels, n_samples, chunk_bytes, bits);
+  const size_t buf_bytes = ((size_t)plan.chunk_events * plan.event_bits + 7u) / 8u;
   e = grow_pair(
       w.dev_buf, &w.dev_cap, buf_bytes, [](void** p, size_t n) { return cudaMalloc(p, n); },
       [](void* p) { cudaFree(p); });
@@ -207,8 +224,11 @@ int stream_impl(Workspace& w, const uint16_t* wf_host, int64_t n_events, int32_t
     const int b = (int)(k & 1);
     const int64_t ev0 = k * plan.chunk_events;
     const int64_t nev = (ev0 + plan.chunk_events <= n_events) ? plan.chunk_events : n_events - ev0;
-    const size_t bytes = (size_t)nev * plan.event_bytes;
-    const uint8_t* src = reinterpret_cast<const uint8_t*>(wf_host) + (size_t)ev0 * plan.event_bytes;
+    // ev0 * event_bits is a multiple of 128 (plan_chunks); only the last chunk
+    // of a P12 stream can end inside a byte
+    const size_t bytes = ((size_t)nev * plan.event_bits + 7u) / 8u;
+    const uint8_t* src =
+        reinterpret_cast<const uint8_t*>(wf_host) + ((size_t)ev0 * plan.event_bits) / 8u;
 
     // the device buffer is free once the kernel of chunk k-2 (or of an
     // earlier call) has finished with it
@@ -250,9 +270,8 @@ int stream_impl(Workspace& w, const uint16_t* wf_host, int64_t n_events, int32_t
       o_charge = out_charge + t0;
       o_time = out_time + t0;
     }
-    e = rta_launch_extract(reinterpret_cast<const uint16_t*>(w.dev_buf[b]), ntr, n_pixels,
-                           n_samples, pedestal, gain, W, o_sum, o_start, o_charge, o_time, stream,
-                           false);
+    e = rta_launch_extract(w.dev_buf[b], ntr, n_pixels, n_samples, pedestal, gain, W, o_sum,
+                           o_start, o_charge, o_time, stream, false, nullptr, bits);
     if (e != cudaSuccess) return fail_cuda(e);
     if ((e = cudaEventRecord(w.consumed[b], stream)) != cudaSuccess) return fail_cuda(e);
     w.consumed_valid[b] = true;
@@ -277,6 +296,54 @@ int stream_impl(Workspace& w, const uint16_t* wf_host, int64_t n_events, int32_t
       w.returned_valid[b] = true;
     }
   }
+  return RTA_OK;
+}
+
+// Host-to-host path (rta_extract_host, rta_extract_host_packed12): calibration
+// up, chunks through stream_impl, results back; synchronous.
+int host_impl(const void* wf_host, int64_t n_events, int32_t n_pixels, int32_t n_samples,
+              const int32_t* pedestal_host, const float* gain_host, int32_t W,
+              int32_t* out_sum_host, int32_t* out_start_host, float* out_charge_host,
+              float* out_time_host, size_t chunk_bytes, int bits) {
+  const int v = validate(wf_host, n_events, n_pixels, n_samples, pedestal_host, gain_host, W,
+                         out_sum_host, out_start_host, out_charge_host, out_time_host,
+                         bits == 12 ? 1 : 2);
+  if (v != RTA_OK || n_events == 0) return v;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  Workspace& w = g_ws;
+  cudaError_t e = ws_prepare(w);
+  if (e != cudaSuccess) return fail_cuda(e);
+  const size_t calib_bytes = (size_t)n_pixels * 8u;
+  if (w.calib_cap < calib_bytes) {
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail_cuda(e);
+    if (w.calib_buf) cudaFree(w.calib_buf);
+    w.calib_buf = nullptr;
+    w.calib_cap = 0;
+    if ((e = cudaMalloc(&w.calib_buf, calib_bytes)) != cudaSuccess) return fail_cuda(e);
+    w.calib_cap = calib_bytes;
+  }
+  int32_t* d_ped = reinterpret_cast<int32_t*>(w.calib_buf);
+  float* d_gain = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(w.calib_buf) +
+                                           (size_t)n_pixels * 4u);
+  // calibration constants may still be read by kernels of an earlier call
+  if ((e = cudaStreamSynchronize(w.host_stream)) != cudaSuccess) return fail_cuda(e);
+  if ((e = cudaMemcpyAsync(d_ped, pedestal_host, (size_t)n_pixels * 4u, cudaMemcpyHostToDevice,
+                           w.host_stream)) != cudaSuccess)
+    return fail_cuda(e);
+  if ((e = cudaMemcpyAsync(d_gain, gain_host, (size_t)n_pixels * 4u, cudaMemcpyHostToDevice,
+                           w.host_stream)) != cudaSuccess)
+    return fail_cuda(e);
+  const HostOut ho{out_sum_host, out_start_host, out_charge_host, out_time_host};
+  const int rc = stream_impl(w, wf_host, n_events, n_pixels, n_samples, d_ped, d_gain, W, nullptr,
+                             nullptr, nullptr, nullptr, chunk_bytes, w.host_stream, &ho, bits);
+  // synchronous by contract, also on the error path (nothing may outlive the call)
+  cudaError_t e1 = cudaStreamSynchronize(w.host_stream);
+  cudaError_t e2 = cudaStreamSynchronize(w.back_stream);
+  cudaError_t e3 = cudaStreamSynchronize(w.copy_stream);
+  if (rc != RTA_OK) return rc;
+  if (e1 != cudaSuccess) return fail_cuda(e1);
+  if (e2 != cudaSuccess) return fail_cuda(e2);
+  if (e3 != cudaSuccess) return fail_cuda(e3);
   return RTA_OK;
 }
 
@@ -393,45 +460,48 @@ int rta_extract_host(const uint16_t* wf_host, int64_t n_events, int32_t n_pixels
                      int32_t n_samples, const int32_t* pedestal_host, const float* gain_host,
                      int32_t W, int32_t* out_sum_host, int32_t* out_start_host,
                      float* out_charge_host, float* out_time_host, size_t chunk_bytes) {
-  const int v = validate(wf_host, n_events, n_pixels, n_samples, pedestal_host, gain_host, W,
-                         out_sum_host, out_start_host, out_charge_host, out_time_host);
+  return host_impl(wf_host, n_events, n_pixels, n_samples, pedestal_host, gain_host, W,
+                   out_sum_host, out_start_host, out_charge_host, out_time_host, chunk_bytes, 16);
+}
+
+// ---- packed 12-bit ingest (NEXT-2; readings R25-R27) -----------------
+int rta_extract_packed12(const uint8_t* packed, int64_t n_events, int32_t n_pixels,
+                         int32_t n_samples, const int32_t* pedestal, const float* gain,
+                         int32_t W, int32_t* out_sum, int32_t* out_start, float* out_charge,
+                         float* out_time, void* stream) {
+  const int v = validate(packed, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum,
+                         out_start, out_charge, out_time, 1);
+  if (v != RTA_OK || n_events == 0) return v;
+  const cudaError_t e = rta_launch_extract(packed, n_events * (int64_t)n_pixels, n_pixels,
+                                           n_samples, pedestal, gain, W, out_sum, out_start,
+                                           out_charge, out_time, (cudaStream_t)stream,
+                                           g_force_generic, nullptr, 12);
+  return e == cudaSuccess ? RTA_OK : fail_cuda(e);
+}
+
+int rta_extract_stream_packed12(const uint8_t* packed_host, int64_t n_events, int32_t n_pixels,
+                                int32_t n_samples, const int32_t* pedestal, const float* gain,
+                                int32_t W, int32_t* out_sum, int32_t* out_start,
+                                float* out_charge, float* out_time, size_t chunk_bytes,
+                                void* stream) {
+  const int v = validate(packed_host, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum,
+                         out_start, out_charge, out_time, 1);
   if (v != RTA_OK || n_events == 0) return v;
   std::lock_guard<std::mutex> lock(g_ws.mu);
-  Workspace& w = g_ws;
-  cudaError_t e = ws_prepare(w);
+  cudaError_t e = ws_prepare(g_ws);
   if (e != cudaSuccess) return fail_cuda(e);
-  const size_t calib_bytes = (size_t)n_pixels * 8u;
-  if (w.calib_cap < calib_bytes) {
-    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail_cuda(e);
-    if (w.calib_buf) cudaFree(w.calib_buf);
-    w.calib_buf = nullptr;
-    w.calib_cap = 0;
-    if ((e = cudaMalloc(&w.calib_buf, calib_bytes)) != cudaSuccess) return fail_cuda(e);
-    w.calib_cap = calib_bytes;
-  }
-  int32_t* d_ped = reinterpret_cast<int32_t*>(w.calib_buf);
-  float* d_gain = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(w.calib_buf) +
-                                           (size_t)n_pixels * 4u);
-  // calibration constants may still be read by kernels of an earlier call
-  if ((e = cudaStreamSynchronize(w.host_stream)) != cudaSuccess) return fail_cuda(e);
-  if ((e = cudaMemcpyAsync(d_ped, pedestal_host, (size_t)n_pixels * 4u, cudaMemcpyHostToDevice,
-                           w.host_stream)) != cudaSuccess)
-    return fail_cuda(e);
-  if ((e = cudaMemcpyAsync(d_gain, gain_host, (size_t)n_pixels * 4u, cudaMemcpyHostToDevice,
-                           w.host_stream)) != cudaSuccess)
-    return fail_cuda(e);
-  const HostOut ho{out_sum_host, out_start_host, out_charge_host, out_time_host};
-  const int rc = stream_impl(w, wf_host, n_events, n_pixels, n_samples, d_ped, d_gain, W, nullptr,
-                             nullptr, nullptr, nullptr, chunk_bytes, w.host_stream, &ho);
-  // synchronous by contract, also on the error path (nothing may outlive the call)
-  cudaError_t e1 = cudaStreamSynchronize(w.host_stream);
-  cudaError_t e2 = cudaStreamSynchronize(w.back_stream);
-  cudaError_t e3 = cudaStreamSynchronize(w.copy_stream);
-  if (rc != RTA_OK) return rc;
-  if (e1 != cudaSuccess) return fail_cuda(e1);
-  if (e2 != cudaSuccess) return fail_cuda(e2);
-  if (e3 != cudaSuccess) return fail_cuda(e3);
-  return RTA_OK;
+  return stream_impl(g_ws, packed_host, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum,
+                     out_start, out_charge, out_time, chunk_bytes, (cudaStream_t)stream, nullptr,
+                     12);
+}
+
+int rta_extract_host_packed12(const uint8_t* packed_host, int64_t n_events, int32_t n_pixels,
+                              int32_t n_samples, const int32_t* pedestal_host,
+                              const float* gain_host, int32_t W, int32_t* out_sum_host,
+                              int32_t* out_start_host, float* out_charge_host,
+                              float* out_time_host, size_t chunk_bytes) {
+  return host_impl(packed_host, n_events, n_pixels, n_samples, pedestal_host, gain_host, W,
+                   out_sum_host, out_start_host, out_charge_host, out_time_host, chunk_bytes, 12);
 }
 
 const char* rta_strerror(int status) {
@@ -454,6 +524,17 @@ const char* rta_kernel_name(int32_t n_samples, int32_t W, int aligned16) {
   return rta_pick_kernel_name(n_samples, W, aligned16 != 0);
 }
 
+const char* rta_kernel_name_packed12(int32_t n_samples, int32_t W, int aligned16) {
+  return rta_pick_kernel_name(n_samples, W, aligned16 != 0, 12);
+}
+
+int64_t rta_chunk_events(int64_t n_events, int32_t n_pixels, int32_t n_samples,
+                         size_t chunk_bytes, int32_t sample_bits) {
+  if (n_events < 0 || n_pixels < 1 || n_samples < 1 || (sample_bits != 16 && sample_bits != 12))
+    return -1;
+  return plan_chunks(n_events, n_pixels, n_samples, chunk_bytes, sample_bits).chunk_events;
+}
+
 uint64_t rta_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 void rta_shutdown(void) {
@@ -472,8 +553,8 @@ void rta_shutdown(void) {
   rta_sched_release();
 }
 
-// Test hook (not in the public header): 1 = rta_extract_fixed / _local_peak / _fir
-// take the generic kernel whatever the shape (two device paths must agree).
+// Test hook (not in the public header): 1 = rta_extract_fixed / _local_peak / _fir /
+// _packed12 take the generic kernel whatever the shape (two device paths must agree).
 void rta_debug_force_generic(int on) { g_force_generic.store(on != 0); }
 
 // Test hook (not in the public header): 1 = static round-robin tile schedule,

@@ -21,15 +21,16 @@ struct RtaMode {
 // of `wf` on `stream`. Arguments are already validated. Returns a cudaError_t.
 // `force_generic` routes every shape to the generic kernel (tests use it to
 // compare the two paths). `mode` == nullptr is the sliding-window extractor.
-cudaError_t rta_launch_extract(const uint16_t* wf, int64_t n_traces, int32_t n_pixels,
+// `sample_bits` is 16 (uint16 samples) or 12 (P12 stream, sliding extractor only).
+cudaError_t rta_launch_extract(const void* wf, int64_t n_traces, int32_t n_pixels,
                                int32_t n_samples, const int32_t* pedestal,
                                const float* gain, int32_t W, int32_t* out_sum,
                                int32_t* out_start, float* out_charge, float* out_time,
                                cudaStream_t stream, bool force_generic,
-                               const RtaMode* mode = nullptr);
+                               const RtaMode* mode = nullptr, int sample_bits = 16);
 
 // Name of the kernel the dispatcher picks (static string).
-const char* rta_pick_kernel_name(int32_t n_samples, int32_t W, bool aligned16);
+const char* rta_pick_kernel_name(int32_t n_samples, int32_t W, bool aligned16, int bits = 16);
 
 void rta_count_launch();
 

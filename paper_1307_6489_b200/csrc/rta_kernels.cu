@@ -147,38 +147,99 @@ __device__ __forceinline__ int clamp_start(const int t, const int S, const int W
 }
 
 // ------------------------------------------------------- tile kernel cfg ----
-template <int S_, int W_, int NT_, int STAGES_>
+// BITS = 16: uint16 samples (include/rta.h rta_extract). BITS = 12: the P12
+// stream of rta_extract_packed12 (readings R25-R27): sample n sits at
+// bits [12 n, 12 n + 12) of the byte stream, little-endian in bits.
+template <int S_, int W_, int NT_, int STAGES_, int BITS_ = 16>
 struct TileCfg {
-  static constexpr int S = S_, W = W_, NT = NT_, STAGES = STAGES_;
-  static constexpr int TRACE_BYTES = 2 * S;
-  static constexpr int TPT = (TRACE_BYTES % 4 == 0) ? 1 : 2;  // traces per thread
-  static constexpr int UNIT_BYTES = TRACE_BYTES * TPT;        // bytes one thread owns
-  static constexpr int VEC = (UNIT_BYTES % 16 == 0) ? 16 : (UNIT_BYTES % 8 == 0) ? 8 : 4;
-  static constexpr int NVEC = UNIT_BYTES / VEC;
+  static constexpr int S = S_, W = W_, NT = NT_, STAGES = STAGES_, BITS = BITS_;
+  static_assert(BITS == 16 || BITS == 12, "sample formats: uint16 or P12");
+  static constexpr int TRACE_BITS = BITS * S;
+  // traces per thread: the smallest count whose bytes a thread can own
+  // (uint16: a multiple of 4 bytes; P12: a whole number of bytes)
+  static constexpr int TPT = (BITS == 16) ? ((TRACE_BITS % 32 == 0) ? 1 : 2)
+                                          : ((TRACE_BITS % 8 == 0) ? 1 : 2);
+  static constexpr int UNIT_BYTES = TRACE_BITS * TPT / 8;     // bytes one thread owns
+  // P12 units of 45 or 75 bytes do not start on a word: the thread reads the
+  // aligned words around its unit and realigns them with one funnel shift each
+  static constexpr bool MISALIGNED = (UNIT_BYTES % 4 != 0);
+  static constexpr int VEC = MISALIGNED              ? 4
+                             : (UNIT_BYTES % 16 == 0) ? 16
+                             : (UNIT_BYTES % 8 == 0)  ? 8
+                                                      : 4;
+  static constexpr int NWORDS = (UNIT_BYTES + 3) / 4;          // words holding one unit
+  static constexpr int NVEC = MISALIGNED ? NWORDS + 1 : UNIT_BYTES / VEC;  // loads per thread
   // an even number of 16-byte chunks per unit puts the lanes of a quarter-warp
   // on the same banks: pad each unit by one chunk
   static constexpr bool PAD = (VEC == 16) && (NVEC % 2 == 0);
   static constexpr int UNIT_STRIDE = UNIT_BYTES + (PAD ? 16 : 0);
-  static constexpr int NWORDS = UNIT_BYTES / 4;
   static constexpr int TILE_TRACES = NT * TPT;
   static constexpr int TILE_BYTES = NT * UNIT_BYTES;
-  static constexpr int STAGE_BYTES = ((NT * UNIT_STRIDE + 127) / 128) * 128;
+  // misaligned units read up to 7 bytes past their end: keep the stage's tail inside the stage
+  static constexpr int STAGE_BYTES = ((NT * UNIT_STRIDE + (MISALIGNED ? 16 : 0) + 127) / 128) * 128;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES;
   static constexpr int NWIN = S - W + 1;
   static constexpr int KB = ilog2_ceil(NWIN);
   static constexpr uint32_t KM = (1u << KB) - 1u;
   static constexpr int PB = ilog2_ceil(S);  // local-peak key: sample index bits
-  static constexpr uint32_t PM = (1u << PB) - 1u;
+  static constexpr uint32_t XMAX = (BITS == 16) ? 65535u : 4095u;
   static_assert(16 + PB <= 32, "peak key must fit 32 bits");
   static_assert(W >= 1 && W <= S, "window must fit the trace");
   static_assert(NT % 32 == 0, "whole warps");
   static_assert(TILE_BYTES % 16 == 0, "TMA bulk copies move multiples of 16 bytes");
-  static_assert((unsigned long long)W * 65535ull * (1ull << KB) + KM < (1ull << 32),
-                "arg-max key must fit 32 bits for any uint16 data");
+  static_assert((unsigned long long)W * XMAX * (1ull << KB) + KM < (1ull << 32),
+                "arg-max key must fit 32 bits for any sample value");
 };
 
-// raw sample h (halfword index inside the thread's unit), h known at compile time
-#define RTA_X(w, h) (((h)&1) ? ((w)[(h) >> 1] >> 16) : ((w)[(h) >> 1] & 0xFFFFu))
+// raw sample h (sample index inside the thread's unit) from the register copy
+// w[] of the unit; h is a compile-time constant once the caller's loops are
+// unrolled, so every branch below folds away.
+template <class C>
+__device__ __forceinline__ uint32_t unit_sample(const uint32_t* w, const int h) {
+  if constexpr (C::BITS == 16) {
+    return (h & 1) ? (w[h >> 1] >> 16) : (w[h >> 1] & 0xFFFFu);
+  } else {
+    const int bit = 12 * h, i = bit >> 5, sh = bit & 31;
+    if (sh == 20) return w[i] >> 20;
+    if (sh < 20) return (w[i] >> sh) & 0xFFFu;
+    const int i1 = (i + 1 < C::NWORDS) ? i + 1 : i;  // a straddling sample always has a next word
+    return __funnelshift_r(w[i], w[i1], sh) & 0xFFFu;
+  }
+}
+#define RTA_X(w, h) unit_sample<C>(w, h)
+
+// Samples n0, n0+1, ... of a unit in shared memory at a data-dependent n0
+// (the winning window): read(k) returns sample n0 + k, k a compile-time
+// constant. uint16: one 16-bit load. P12: sample n occupies the two bytes at
+// floor(3 n / 2), shifted by 4 bits when n is odd; the byte address advances
+// by exactly 3 bytes per two samples, so one base per parity is enough.
+template <class C>
+struct WindowReader {
+  const uint8_t* be;   // bytes of sample n0 (even k)
+  const uint8_t* bo;   // bytes of sample n0 + 1 (odd k); P12 only
+  uint32_t she, sho;   // P12: 0 or 4
+  __device__ __forceinline__ WindowReader(const uint8_t* unit, const int n0) {
+    if constexpr (C::BITS == 16) {
+      be = unit + 2 * n0;
+      bo = be;
+      she = sho = 0;
+    } else {
+      be = unit + ((3 * n0) >> 1);
+      bo = unit + ((3 * n0 + 3) >> 1);
+      she = (uint32_t)(n0 & 1) << 2;
+      sho = she ^ 4u;
+    }
+  }
+  __device__ __forceinline__ int read(const int k) const {
+    if constexpr (C::BITS == 16) {
+      return (int)reinterpret_cast<const uint16_t*>(be)[k];
+    } else {
+      const uint8_t* b = (k & 1) ? bo + 3 * (k >> 1) : be + 3 * (k >> 1);
+      const uint32_t v = (uint32_t)b[0] | ((uint32_t)b[1] << 8);
+      return (int)((v >> ((k & 1) ? sho : she)) & 0xFFFu);
+    }
+  }
+};
 
 template <class C, int MODE>
 __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, const uint32_t g0,
@@ -195,7 +256,16 @@ __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, c
   constexpr bool NEED_W = (MODE != MODE_FIXED);
   uint32_t w[NEED_W ? C::NWORDS : 1];
   if constexpr (NEED_W) {
-    if constexpr (C::VEC == 16) {
+    if constexpr (C::MISALIGNED) {
+      // aligned words around the unit, then one funnel shift per word
+      const uint32_t ph = (uint32_t)(reinterpret_cast<uintptr_t>(unit) & 3u);
+      const uint32_t* src = reinterpret_cast<const uint32_t*>(unit - ph);
+      uint32_t raw[C::NWORDS + 1];
+#pragma unroll
+      for (int i = 0; i <= C::NWORDS; ++i) raw[i] = src[i];
+#pragma unroll
+      for (int i = 0; i < C::NWORDS; ++i) w[i] = __funnelshift_r(raw[i], raw[i + 1], 8u * ph);
+    } else if constexpr (C::VEC == 16) {
 #pragma unroll
       for (int i = 0; i < C::NVEC; ++i) {
         const uint4 v = *reinterpret_cast<const uint4*>(unit + 16 * i);
@@ -218,7 +288,6 @@ __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, c
 #pragma unroll
   for (int j = 0; j < C::TPT; ++j) {
     const int h0 = j * S;  // compile-time after unrolling
-    const uint16_t* tr0 = reinterpret_cast<const uint16_t*>(unit) + h0;
     int tstar, rawsum, relnum = 0;
     if constexpr (MODE == MODE_SLIDING) {
       // a3 + a4 on raw samples: sliding sum, packed (sum, earliest) key
@@ -235,9 +304,9 @@ __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, c
       tstar = (int)(C::KM - (best & C::KM));
       rawsum = (int)(best >> C::KB);
       // a7 numerator: re-read the winning window (dynamic index -> shared memory)
-      const uint16_t* tr = tr0 + tstar;
+      const WindowReader<C> tr(unit, h0 + tstar);
 #pragma unroll
-      for (int k = 1; k < W; ++k) relnum += k * (int)tr[k];
+      for (int k = 1; k < W; ++k) relnum += k * tr.read(k);
     } else if constexpr (MODE == MODE_FIR) {
       // response on raw samples (the pedestal shifts every y(t) by the same
       // c0*ped); signed compare, strict '>' scanning upwards = earliest on ties
@@ -256,26 +325,26 @@ __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, c
         }
       }
       rawsum = best;
-      const uint16_t* tr = tr0 + tstar;
+      const WindowReader<C> tr(unit, h0 + tstar);
 #pragma unroll
-      for (int k = 1; k < W; ++k) relnum += k * ma.taps[k] * (int)tr[k];
+      for (int k = 1; k < W; ++k) relnum += k * ma.taps[k] * tr.read(k);
     } else {
       if constexpr (MODE == MODE_FIXED) {
         tstar = clamp_start(__ldg(ma.window_start + p), S, W);
       } else {  // MODE_LOCAL_PEAK: largest sample, earliest on ties, one max per sample
         constexpr int PB = C::PB;
-        constexpr uint32_t PM = C::PM;
+        constexpr uint32_t PM = (1u << PB) - 1u;
         uint32_t best = (RTA_X(w, h0) << PB) | PM;
 #pragma unroll
         for (int k = 1; k < S; ++k)
           best = max(best, (RTA_X(w, h0 + k) << PB) + (PM - (uint32_t)k));
         tstar = clamp_start((int)(PM - (best & PM)) - ma.shift, S, W);
       }
-      const uint16_t* tr = tr0 + tstar;
-      rawsum = (int)tr[0];
+      const WindowReader<C> tr(unit, h0 + tstar);
+      rawsum = tr.read(0);
 #pragma unroll
       for (int k = 1; k < W; ++k) {
-        const int x = (int)tr[k];
+        const int x = tr.read(k);
         rawsum += x;
         relnum += k * x;
       }
@@ -326,7 +395,7 @@ __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, c
 // selects the static round-robin (same code path, locally generated indices).
 template <class C, int MODE>
 __global__ void __launch_bounds__(C::NT)
-    extract_tile_kernel(const uint16_t* __restrict__ wf, const uint32_t n_traces,
+    extract_tile_kernel(const uint8_t* __restrict__ wf, const uint32_t n_traces,
                         const uint32_t n_pixels, const uint32_t pix_inv,
                         const int* __restrict__ pedestal, const float* __restrict__ gain,
                         int* __restrict__ out_sum, int* __restrict__ out_start,
@@ -390,7 +459,7 @@ __global__ void __launch_bounds__(C::NT)
   __syncthreads();
 
   auto issue = [&](const uint32_t tile, const int stage) {
-    const uint8_t* src = reinterpret_cast<const uint8_t*>(wf) + (size_t)tile * C::TILE_BYTES;
+    const uint8_t* src = wf + (size_t)tile * C::TILE_BYTES;
     const uint32_t dst = smem_base + stage * C::STAGE_BYTES;
     const uint32_t bar = bar_base + 8 * stage;
     if constexpr (!C::PAD) {
@@ -443,13 +512,21 @@ __global__ void __launch_bounds__(C::NT)
 
   // ragged tail (< one tile of traces): plain copies, by the CTA that drew index n_full
   if (rem != 0 && tile == n_full) {
-    const uint16_t* src = wf + (size_t)n_full * C::TILE_TRACES * C::S;
-    uint16_t* dst = reinterpret_cast<uint16_t*>(smem);
-    const uint32_t n_hw = rem * C::S;
-    constexpr uint32_t UNIT_HW = C::UNIT_BYTES / 2, STRIDE_HW = C::UNIT_STRIDE / 2;
-    for (uint32_t i = tid; i < n_hw; i += C::NT) {
-      const uint32_t u = i / UNIT_HW;
-      dst[u * STRIDE_HW + (i - u * UNIT_HW)] = src[i];
+    const uint8_t* src = wf + (size_t)n_full * C::TILE_BYTES;  // 16-byte aligned
+    const uint32_t n_bytes = (rem * (uint32_t)C::TRACE_BITS + 7u) / 8u;
+    // byte b of the tail lives at (b / UNIT_BYTES) * UNIT_STRIDE + b % UNIT_BYTES;
+    // whole words first (a unit with padding is a multiple of 16 bytes), then
+    // the last 0-3 bytes one by one: nothing past the caller's buffer is read
+    const uint32_t n_w = n_bytes / 4u;
+    for (uint32_t i = tid; i < n_w; i += C::NT) {
+      uint32_t d = i;
+      if constexpr (C::PAD) d += (i / (C::UNIT_BYTES / 4)) * ((C::UNIT_STRIDE - C::UNIT_BYTES) / 4);
+      reinterpret_cast<uint32_t*>(smem)[d] = reinterpret_cast<const uint32_t*>(src)[i];
+    }
+    for (uint32_t b = 4u * n_w + tid; b < n_bytes; b += C::NT) {
+      uint32_t d = b;
+      if constexpr (C::PAD) d += (b / C::UNIT_BYTES) * (C::UNIT_STRIDE - C::UNIT_BYTES);
+      smem[d] = src[b];
     }
     __syncthreads();
     const uint32_t first = (uint32_t)tid * C::TPT;
@@ -473,11 +550,37 @@ __global__ void __launch_bounds__(C::NT)
 }
 
 // -------------------------------------------------------- generic kernel ----
-// Any (S, W) inside the ABI guards, any 2-byte alignment: one thread per trace,
-// samples read straight from global memory (L1/L2 absorb the re-reads).
-template <int MODE>
+// Any (S, W) inside the ABI guards, any alignment the format allows (uint16: 2
+// bytes; P12: 1 byte): one thread per trace, samples read straight from global
+// memory (L1/L2 absorb the re-reads).
+template <int BITS>
+struct GlobalTrace {
+  const uint8_t* base;  // uint16: first byte of the trace; P12: first byte of the stream
+  size_t n0;            // P12: flat index of the trace's first sample
+  __device__ __forceinline__ GlobalTrace(const uint8_t* wf, const uint32_t g, const int S) {
+    if constexpr (BITS == 16) {
+      base = wf + (size_t)g * (size_t)S * 2u;
+      n0 = 0;
+    } else {
+      base = wf;
+      n0 = (size_t)g * (size_t)S;
+    }
+  }
+  __device__ __forceinline__ uint32_t operator[](const int s) const {
+    if constexpr (BITS == 16) {
+      return reinterpret_cast<const uint16_t*>(base)[s];
+    } else {
+      const size_t n = n0 + (size_t)s;
+      const uint8_t* b = base + ((3u * n) >> 1);
+      const uint32_t v = (uint32_t)b[0] | ((uint32_t)b[1] << 8);
+      return (v >> ((uint32_t)(n & 1u) << 2)) & 0xFFFu;
+    }
+  }
+};
+
+template <int MODE, int BITS>
 __global__ void __launch_bounds__(256)
-    extract_generic_kernel(const uint16_t* __restrict__ wf, const uint32_t n_traces, const int S,
+    extract_generic_kernel(const uint8_t* __restrict__ wf, const uint32_t n_traces, const int S,
                            const int W, const uint32_t n_pixels, const uint32_t pix_inv,
                            const int* __restrict__ pedestal, const float* __restrict__ gain,
                            int* __restrict__ out_sum, int* __restrict__ out_start,
@@ -485,7 +588,7 @@ __global__ void __launch_bounds__(256)
                            const __grid_constant__ ModeArgs ma) {
   for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < n_traces;
        g += gridDim.x * blockDim.x) {
-    const uint16_t* tr = wf + (size_t)g * S;
+    const GlobalTrace<BITS> tr(wf, g, S);
     const uint32_t p = fastmod(g, n_pixels, pix_inv);
     int tstar = 0, rawsum = 0, relnum = 0;
     if constexpr (MODE == MODE_SLIDING) {
@@ -635,7 +738,7 @@ struct TileLauncher {
     return cudaSuccess;
   }
 
-  static cudaError_t launch(const uint16_t* wf, uint32_t n_traces, uint32_t n_pixels,
+  static cudaError_t launch(const uint8_t* wf, uint32_t n_traces, uint32_t n_pixels,
                             uint32_t pix_inv, const int32_t* pedestal, const float* gain,
                             int32_t* out_sum, int32_t* out_start, float* out_charge,
                             float* out_time, cudaStream_t stream, const ModeArgs& ma) {
@@ -695,6 +798,35 @@ using CfgS30W7 = TileCfg<30, 7, RTA_S30_NT, RTA_S30_ST>;
 using CfgS40W7 = TileCfg<40, 7, RTA_S40_NT, RTA_S40_ST>;
 using CfgS25W4 = TileCfg<25, 4, RTA_S25_NT, RTA_S25_ST>;
 using CfgS128W8 = TileCfg<128, 8, RTA_S128_NT, RTA_S128_ST>;
+// The same shapes fed by a P12 stream (rta_extract_packed12).
+#ifndef RTA_P30_NT
+#define RTA_P30_NT 256
+#endif
+#ifndef RTA_P30_ST
+#define RTA_P30_ST 3
+#endif
+#ifndef RTA_P40_NT
+#define RTA_P40_NT 256
+#endif
+#ifndef RTA_P40_ST
+#define RTA_P40_ST 3
+#endif
+#ifndef RTA_P25_NT
+#define RTA_P25_NT 256
+#endif
+#ifndef RTA_P25_ST
+#define RTA_P25_ST 3
+#endif
+#ifndef RTA_P128_NT
+#define RTA_P128_NT 64
+#endif
+#ifndef RTA_P128_ST
+#define RTA_P128_ST 2
+#endif
+using CfgP30W7 = TileCfg<30, 7, RTA_P30_NT, RTA_P30_ST, 12>;
+using CfgP40W7 = TileCfg<40, 7, RTA_P40_NT, RTA_P40_ST, 12>;
+using CfgP25W4 = TileCfg<25, 4, RTA_P25_NT, RTA_P25_ST, 12>;
+using CfgP128W8 = TileCfg<128, 8, RTA_P128_NT, RTA_P128_ST, 12>;
 
 }  // namespace
 
@@ -720,7 +852,16 @@ void rta_sched_release() {
   cudaGetLastError();
 }
 
-const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16) {
+const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16, int bits) {
+  if (bits == 12) {
+    if (aligned16) {
+      if (S == 30 && W == 7) return "tile12<S=30,W=7>";
+      if (S == 40 && W == 7) return "tile12<S=40,W=7>";
+      if (S == 25 && W == 4) return "tile12<S=25,W=4>";
+      if (S == 128 && W == 8) return "tile12<S=128,W=8>";
+    }
+    return "generic12";
+  }
   if (aligned16) {
     if (S == 30 && W == 7) return "tile<S=30,W=7>";
     if (S == 40 && W == 7) return "tile<S=40,W=7>";
@@ -733,7 +874,7 @@ const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16) {
 namespace {
 
 struct LaunchArgs {
-  const uint16_t* wf;
+  const uint8_t* wf;
   uint32_t n_traces, n_pixels, pix_inv;
   int32_t S, W;
   const int32_t* pedestal;
@@ -744,20 +885,8 @@ struct LaunchArgs {
   bool staged;  // 16-byte aligned input and not forced to the generic kernel
 };
 
-template <int MODE>
-cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
-  if (a.staged) {
-#define RTA_TRY(CFG)                                                                          \
-  if (a.S == CFG::S && a.W == CFG::W)                                                         \
-    return TileLauncher<CFG, MODE>::launch(a.wf, a.n_traces, a.n_pixels, a.pix_inv,           \
-                                           a.pedestal, a.gain, a.out_sum, a.out_start,        \
-                                           a.out_charge, a.out_time, a.stream, ma);
-    RTA_TRY(CfgS30W7)
-    RTA_TRY(CfgS40W7)
-    RTA_TRY(CfgS25W4)
-    RTA_TRY(CfgS128W8)
-#undef RTA_TRY
-  }
+template <int MODE, int BITS>
+cudaError_t launch_generic(const LaunchArgs& a, const ModeArgs& ma) {
   int dev = 0, sms = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
@@ -765,25 +894,54 @@ cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
   uint32_t grid = (a.n_traces + 255u) / 256u;
   const uint32_t cap = (uint32_t)sms * 8u;
   if (grid > cap) grid = cap;
-  extract_generic_kernel<MODE><<<grid, 256, 0, a.stream>>>(
+  extract_generic_kernel<MODE, BITS><<<grid, 256, 0, a.stream>>>(
       a.wf, a.n_traces, a.S, a.W, a.n_pixels, a.pix_inv, a.pedestal, a.gain, a.out_sum,
       a.out_start, a.out_charge, a.out_time, ma);
   rta_count_launch();
   return cudaGetLastError();
 }
 
+#define RTA_TRY(CFG)                                                                          \
+  if (a.S == CFG::S && a.W == CFG::W)                                                         \
+    return TileLauncher<CFG, MODE>::launch(a.wf, a.n_traces, a.n_pixels, a.pix_inv,           \
+                                           a.pedestal, a.gain, a.out_sum, a.out_start,        \
+                                           a.out_charge, a.out_time, a.stream, ma);
+template <int MODE>
+cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
+  if (a.staged) {
+    RTA_TRY(CfgS30W7)
+    RTA_TRY(CfgS40W7)
+    RTA_TRY(CfgS25W4)
+    RTA_TRY(CfgS128W8)
+  }
+  return launch_generic<MODE, 16>(a, ma);
+}
+
+// P12 input: the sliding-window extractor only (include/rta.h)
+cudaError_t launch_packed12(const LaunchArgs& a, const ModeArgs& ma) {
+  constexpr int MODE = MODE_SLIDING;
+  if (a.staged) {
+    RTA_TRY(CfgP30W7)
+    RTA_TRY(CfgP40W7)
+    RTA_TRY(CfgP25W4)
+    RTA_TRY(CfgP128W8)
+  }
+  return launch_generic<MODE, 12>(a, ma);
+}
+#undef RTA_TRY
+
 }  // namespace
 
-cudaError_t rta_launch_extract(const uint16_t* wf, int64_t n_traces64, int32_t n_pixels,
+cudaError_t rta_launch_extract(const void* wf, int64_t n_traces64, int32_t n_pixels,
                                int32_t S, const int32_t* pedestal, const float* gain, int32_t W,
                                int32_t* out_sum, int32_t* out_start, float* out_charge,
                                float* out_time, cudaStream_t stream, bool force_generic,
-                               const RtaMode* mode) {
+                               const RtaMode* mode, int sample_bits) {
   if (n_traces64 <= 0) return cudaSuccess;
   const uint32_t P = (uint32_t)n_pixels;
   const uint64_t inv64 = (1ull << 32) / P;
   LaunchArgs a;
-  a.wf = wf;
+  a.wf = static_cast<const uint8_t*>(wf);
   a.n_traces = (uint32_t)n_traces64;
   a.n_pixels = P;
   a.pix_inv = inv64 > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)inv64;
@@ -799,6 +957,9 @@ cudaError_t rta_launch_extract(const uint16_t* wf, int64_t n_traces64, int32_t n
   a.staged = !force_generic && ((uintptr_t)wf % 16) == 0;
   ModeArgs ma = {};
   const int kind = mode ? mode->kind : RTA_MODE_SLIDING;
+  if (sample_bits == 12)
+    return kind == RTA_MODE_SLIDING ? launch_packed12(a, ma) : cudaErrorInvalidValue;
+  if (sample_bits != 16) return cudaErrorInvalidValue;
   switch (kind) {
     case RTA_MODE_SLIDING:
       return launch_mode<MODE_SLIDING>(a, ma);

@@ -155,3 +155,71 @@ def test_family_entry_points_validate_before_any_cuda_call():
     assert fir([20000, -20000], S=30) == rta.RTA_ERR_UNSUPPORTED   # 30*40000*65535 >= 2^31
     assert fir([1, 2, 1], wf=None) == rta.RTA_ERR_NULL
     assert fir([1, 2, 1], E=0, wf=None) == rta.RTA_OK
+
+
+# ---- packed 12-bit ingest (rta_extract_packed12 and the host-fed variants) ----
+def test_packed12_entry_points_validate_before_any_cuda_call():
+    L = rta.lib()
+    o = (0x4000, 0x5000, 0x6000, 0x7000)
+    dev = lambda **k: L.rta_extract_packed12(k.get("wf", 0x1001), k.get("E", 1), k.get("P", 4),
+                                             k.get("S", 30), k.get("ped", 0x2000), 0x3000,
+                                             k.get("W", 7), *k.get("o", o), 0)
+    assert dev(W=31) == rta.RTA_ERR_SHAPE
+    assert dev(W=0) == rta.RTA_ERR_SHAPE
+    assert dev(P=0) == rta.RTA_ERR_SHAPE
+    assert dev(E=-1) == rta.RTA_ERR_SHAPE
+    assert dev(E=2 ** 31, P=1) == rta.RTA_ERR_UNSUPPORTED
+    assert dev(wf=None) == rta.RTA_ERR_NULL
+    assert dev(ped=None) == rta.RTA_ERR_NULL
+    assert dev(ped=0x2002) == rta.RTA_ERR_ALIGN
+    assert dev(o=(0x4001, 0x5000, 0x6000, 0x7000)) == rta.RTA_ERR_ALIGN
+    assert dev(E=0, wf=None, ped=None) == rta.RTA_OK
+    # a P12 stream may start on any byte: an odd address is not an alignment error
+    # (without a device the call then fails in CUDA, never in validation)
+    import torch
+    if not torch.cuda.is_available():
+        assert dev(wf=0x1001) in (rta.RTA_ERR_CUDA, rta.RTA_ERR_NOMEM)
+    assert L.rta_extract_stream_packed12(0x1001, 1, 4, 30, 0x2000, 0x3000, 31, *o, 0, 0) == rta.RTA_ERR_SHAPE
+    assert L.rta_extract_stream_packed12(None, 1, 4, 30, 0x2000, 0x3000, 7, *o, 0, 0) == rta.RTA_ERR_NULL
+    assert L.rta_extract_stream_packed12(None, 0, 4, 30, None, None, 7, None, None, None, None, 0, 0) == rta.RTA_OK
+    assert L.rta_extract_host_packed12(0x1001, 1, 4, 30, None, 0x3000, 7, *o, 0) == rta.RTA_ERR_NULL
+    assert L.rta_extract_host_packed12(None, 0, 4, 30, None, None, 7, None, None, None, None, 0) == rta.RTA_OK
+
+
+def test_packed12_kernel_names():
+    assert rta.rta_kernel_name_packed12(40, 7) == "tile12<S=40,W=7>"
+    assert rta.rta_kernel_name_packed12(30, 7) == "tile12<S=30,W=7>"
+    assert rta.rta_kernel_name_packed12(25, 4) == "tile12<S=25,W=4>"
+    assert rta.rta_kernel_name_packed12(128, 8) == "tile12<S=128,W=8>"
+    assert rta.rta_kernel_name_packed12(40, 7, aligned16=False) == "generic12"
+    assert rta.rta_kernel_name_packed12(41, 7) == "generic12"
+
+
+def test_chunk_events_planning():
+    """Host logic of the host-fed calls (R21, R27): whole events, rounded
+    down, at least one; P12 chunks start on a 16-byte boundary of the stream."""
+    ce = rta.rta_chunk_events
+    # BASELINE.json:configs[4]: 1 GiB chunks of 1855 x 40 uint16 events -> 7235 events, 28 chunks
+    assert ce(200_000, 1855, 40, 1 << 30, 16) == 7235
+    assert ce(200_000, 1855, 40, 0, 16) == 7235                       # 0 = 1 GiB
+    assert -(-200_000 // 7235) == 28
+    # the same events as P12: 111 300 B each -> 9647 fit; 1855*40 = 8 * 9275 -> multiples of 4
+    assert (1 << 30) // 111_300 == 9647
+    assert ce(200_000, 1855, 40, 1 << 30, 12) == 9644
+    for (P, S) in [(1855, 40), (1855, 30), (1764, 25), (2048, 128), (3, 5), (1, 1), (7, 32)]:
+        import math
+        m = 32 // math.gcd(P * S, 32)
+        for bits in (16, 12):
+            ev_bits = P * S * bits
+            for cb in (1, 100, ev_bits // 8, 10 * ev_bits // 8 + 5, 1 << 20, 1 << 30):
+                for E in (0, 1, 5, 1000, 200_000):
+                    got = ce(E, P, S, cb, bits)
+                    fit = (8 * cb) // ev_bits
+                    if bits == 12:
+                        fit -= fit % m
+                        fit = max(fit, m)
+                    want = max(1, min(max(fit, 1), E)) if E > 0 else 1
+                    assert got == want, (P, S, bits, cb, E, got, want)
+                    if bits == 12 and got < E:                       # every later chunk starts aligned
+                        assert (got * ev_bits) % 128 == 0
+    assert ce(-1, 4, 30, 0, 16) == -1 and ce(1, 4, 30, 0, 8) == -1 and ce(1, 0, 30, 0, 12) == -1
