@@ -51,6 +51,9 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C4"])
+    ap.add_argument("--input-format", default="u16", choices=["u16", "p12"],
+                    help="u16: BASELINE.json's uint16 waveforms (the headline); p12: the same batch as "
+                         "a packed 12-bit stream through rta_extract_packed12 (NEXT-2)")
     ap.add_argument("--no-extra", action="store_true", help="skip configs/e2e/sustained/cpu legs")
     ap.add_argument("--no-sustained", action="store_true", help="skip the 29.68 GB C5 leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
@@ -247,13 +250,22 @@ def device_batch(cfg, torch, dl0gen):
     return d_wf, d_ped, d_gain, outs, ped, gain
 
 
-def kernel_only(cfg, steps, warmup, torch, dl0gen, rta, barrier=None, sampler=None):
+def kernel_only(cfg, steps, warmup, torch, dl0gen, rta, barrier=None, sampler=None, fmt="u16"):
     d_wf, d_ped, d_gain, outs, ped, gain = device_batch(cfg, torch, dl0gen)
     stream = torch.cuda.current_stream()
+    if fmt == "p12":
+        n_total = cfg.n_traces * cfg.n_samples
+        d_pk = torch.empty(dl0gen.packed12_nbytes(n_total), dtype=torch.uint8, device="cuda")
+        dl0gen.pack12_cuda(d_wf.data_ptr(), n_total, d_pk.data_ptr(), stream.cuda_stream)
+        torch.cuda.synchronize()
 
-    def run():
-        rta.rta_extract(d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain,
-                        cfg.W, *outs, stream=stream)
+        def run():
+            rta.rta_extract_packed12(d_pk, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped,
+                                     d_gain, cfg.W, *outs, stream=stream)
+    else:
+        def run():
+            rta.rta_extract(d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain,
+                            cfg.W, *outs, stream=stream)
     for _ in range(max(3, warmup)):
         run()
     torch.cuda.synchronize()
@@ -559,7 +571,10 @@ def main():
     sampler.start()
     # Weak scaling: every rank extracts its own batch of the named workload
     # (independent events; no data-path collective).
-    main_run = kernel_only(cfg, args.steps, args.warmup, torch, dl0gen, rta, barrier, sampler)
+    fmt = args.input_format
+    if fmt == "p12":
+        args.no_extra = True     # the packed main leg is a profiling/diagnostic run
+    main_run = kernel_only(cfg, args.steps, args.warmup, torch, dl0gen, rta, barrier, sampler, fmt)
     clocks = sampler.stop(*main_run["marks"])
     t_local = sum(main_run["per_launch_ms"])
     t_max = t_local
@@ -572,12 +587,22 @@ def main():
     summ = summarise(cfg, main_run["per_launch_ms"], peak)
     algo_bytes = cfg.input_bytes + cfg.output_bytes
     kname = rta.rta_kernel_name(cfg.n_samples, cfg.W, True)
+    bytes_per_trace = 2 * cfg.n_samples + ALGO_BYTES_PER_TRACE_OUT
+    if fmt == "p12":
+        # same value definition (2 bytes per sample extracted); the roofline counts the packed bytes
+        algo_bytes = dl0gen.packed12_nbytes(cfg.n_traces * cfg.n_samples) + cfg.output_bytes
+        kname = rta.rta_kernel_name_packed12(cfg.n_samples, cfg.W, True)
+        bytes_per_trace = 1.5 * cfg.n_samples + ALGO_BYTES_PER_TRACE_OUT
+        avg = summ["ms_avg"]
+        summ["algorithmic_GBps"] = algo_bytes / avg / 1e6
+        summ["frac_of_measured_hbm"] = algo_bytes / avg / 1e6 / peak
+        summ["frac_of_nominal_8TBps"] = algo_bytes / avg / 1e6 / 8000.0
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
         "config": {
-            "workload": "%s: %s" % (cfg.name, cfg.label),
+            "workload": "%s: %s" % (cfg.name, cfg.label) + (" as a P12 stream" if fmt == "p12" else ""),
             "per_gpu": "%d events x %d pixels x %d samples uint16, W=%d" % (
                 cfg.n_events, cfg.n_pixels, cfg.n_samples, cfg.W),
             "l2": "input %.2f GB per step exceeds the 126 MB L2 (no flush needed)" % (cfg.input_bytes / 1e9),
@@ -593,7 +618,7 @@ def main():
             "achieved": summ["algorithmic_GBps"], "peak": peak, "unit": "GB/s",
             "frac": summ["frac_of_measured_hbm"], "peak_source": peak_src,
             "algorithmic_bytes_per_launch": algo_bytes,
-            "bytes_per_trace": 2 * cfg.n_samples + ALGO_BYTES_PER_TRACE_OUT,
+            "bytes_per_trace": bytes_per_trace,
             "avg_launch_ms": summ["ms_avg"],
             "traffic": ncu_traffic(kname),
             "frac_of_nominal_8TBps": summ["frac_of_nominal_8TBps"],
