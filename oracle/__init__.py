@@ -21,7 +21,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rta_oracle.cpp")
 _SRCS = [_SRC, os.path.join(_HERE, "rta_oracle_windows.cpp"),
-         os.path.join(_HERE, "rta_oracle_packed.cpp")]
+         os.path.join(_HERE, "rta_oracle_packed.cpp"),
+         os.path.join(_HERE, "rta_oracle_ragged.cpp")]
 _LIB = os.path.join(_HERE, "librta_oracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -63,6 +64,10 @@ def _load():
         lib.rta_oracle_unpack12.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p]
         lib.rta_oracle_extract_packed12.restype = ctypes.c_int
         lib.rta_oracle_extract_packed12.argtypes = lib.rta_oracle_extract.argtypes
+        lib.rta_oracle_extract_ragged.restype = ctypes.c_int
+        lib.rta_oracle_extract_ragged.argtypes = (
+            [ctypes.c_void_p, ctypes.c_int32] + [ctypes.c_void_p] * 4 + [ctypes.c_int64]
+            + [ctypes.c_void_p] * 3 + [ctypes.c_void_p] * 2 + [ctypes.c_void_p] * 4)
         _lib = lib
     return _lib
 
@@ -184,6 +189,46 @@ def extract_packed12(packed, n_events: int, pedestal, gain, n_samples: int, W: i
         gain.ctypes.data, int(W), *[o.ctypes.data for o in outs])
     if rc != 0:
         raise ValueError("rta_oracle_extract_packed12: bad shape")
+    return outs
+
+
+def extract_ragged(wf, tel_n_pixels, tel_n_samples, tel_W, tel_calib_offset, blk_tel,
+                   blk_wf_offset, blk_out_offset, pedestal, gain, n_out: int, fill=None):
+    """Mixed-camera batch (rta_oracle_ragged.cpp, readings R28-R30). ``wf`` is the
+    flat uint16 waveform buffer; the tables are sequences. Returns the four flat
+    output arrays of length ``n_out``; entries no block writes keep ``fill``
+    (default: -1 / -1 / NaN / NaN)."""
+    wf = np.ascontiguousarray(wf, dtype=np.uint16).ravel()
+    tp = np.ascontiguousarray(tel_n_pixels, dtype=np.int32)
+    ts = np.ascontiguousarray(tel_n_samples, dtype=np.int32)
+    tw = np.ascontiguousarray(tel_W, dtype=np.int32)
+    tc = np.ascontiguousarray(tel_calib_offset, dtype=np.int64)
+    bt = np.ascontiguousarray(blk_tel, dtype=np.int32)
+    bw = np.ascontiguousarray(blk_wf_offset, dtype=np.int64)
+    bo = np.ascontiguousarray(blk_out_offset, dtype=np.int64)
+    pedestal = np.ascontiguousarray(pedestal, dtype=np.int32)
+    gain = np.ascontiguousarray(gain, dtype=np.float32)
+    if not (tp.shape == ts.shape == tw.shape == tc.shape and bt.shape == bw.shape == bo.shape):
+        raise ValueError("table lengths differ")
+    for b in range(bt.size):                       # bounds (the C function trusts them)
+        k = int(bt[b])
+        if not 0 <= k < tp.size:
+            raise ValueError("block %d: telescope %d out of range" % (b, k))
+        if bw[b] < 0 or bw[b] + int(tp[k]) * int(ts[k]) > wf.size:
+            raise ValueError("block %d leaves the waveform buffer" % b)
+        if bo[b] < 0 or bo[b] + int(tp[k]) > n_out:
+            raise ValueError("block %d leaves the output arrays" % b)
+        if tc[k] < 0 or tc[k] + int(tp[k]) > pedestal.size or tc[k] + int(tp[k]) > gain.size:
+            raise ValueError("telescope %d leaves the calibration arrays" % k)
+    f = (-1, -1, np.nan, np.nan) if fill is None else fill
+    outs = (np.full(n_out, f[0], np.int32), np.full(n_out, f[1], np.int32),
+            np.full(n_out, f[2], np.float32), np.full(n_out, f[3], np.float32))
+    rc = _load().rta_oracle_extract_ragged(
+        wf.ctypes.data, int(tp.size), tp.ctypes.data, ts.ctypes.data, tw.ctypes.data,
+        tc.ctypes.data, int(bt.size), bt.ctypes.data, bw.ctypes.data, bo.ctypes.data,
+        pedestal.ctypes.data, gain.ctypes.data, *[o.ctypes.data for o in outs])
+    if rc != 0:
+        raise ValueError("rta_oracle_extract_ragged: bad table")
     return outs
 
 
