@@ -22,6 +22,7 @@ Prints ONE JSON line (rank 0). Keys beyond the driver's contract:
   packed12      NEXT-2: the same batches as P12 streams (12 bits per sample),
                 decoded inside the extraction kernel; sustained.packed12 is C5
                 fed as 22.26 GB of P12 through rta_extract_stream_packed12
+  ragged        NEXT-3: a mixed-camera array through rta_extract_ragged
 """
 from __future__ import annotations
 
@@ -356,6 +357,45 @@ def packed_leg(cfg, steps, peak, torch, dl0gen, rta):
             "traces_per_s": cfg.n_traces / avg * 1e3}
 
 
+def ragged_leg(steps, peak, torch, dl0gen, rta, n_events=1000):
+    """NEXT-3: a mixed-camera array (4 LST-, 10 MST-, 6 SST-like telescopes, the
+    cameras of C2/C3/C4), every event holding one block per telescope, through
+    one rta_extract_ragged call (one launch per camera shape)."""
+    m = dl0gen.MixedArray(n_events=n_events)
+    ped, gain = m.calib()
+    d_wf = torch.zeros(m.n_samples_total, dtype=torch.int16, device="cuda")
+    m.fill_cuda(torch, d_wf)
+    d_ped, d_gain = torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda()
+    outs = [torch.empty(m.n_traces, dtype=dt, device="cuda")
+            for dt in (torch.int32, torch.int32, torch.float32, torch.float32)]
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    plan = rta.rta_ragged_plan_create(*m.tables())
+    t_plan = time.perf_counter() - t0
+    stream = torch.cuda.current_stream()
+
+    def run():
+        rta.rta_extract_ragged(plan, d_wf, d_ped, d_gain, *outs, stream=stream)
+    for _ in range(3):
+        run()
+    torch.cuda.synchronize()
+    before = rta.rta_launch_count()
+    per = time_steps(run, steps, stream)
+    launches = (rta.rta_launch_count() - before) // steps
+    avg = sum(per) / len(per)
+    algo = m.wf_bytes + 16 * m.n_traces
+    res = {"workload": "mixed array: %d events x (4 x 1855x40 W7 + 10 x 1764x25 W4 + 6 x 2048x128 W8), "
+                       "%d blocks on 16-byte boundaries" % (m.n_events, len(m.blk_tel)),
+           "ms_avg": avg, "ms_median": statistics.median(per), "ms_best": min(per),
+           "launches_per_call": launches, "tiles": rta.rta_ragged_plan_info(plan, rta.RTA_RAGGED_N_TILES),
+           "waveform_bytes": m.wf_bytes, "algorithmic_bytes_per_call": algo,
+           "waveform_GBps": m.wf_bytes / avg / 1e6, "algorithmic_GBps": algo / avg / 1e6,
+           "frac_of_measured_hbm": algo / avg / 1e6 / peak, "traces_per_s": m.n_traces / avg * 1e3,
+           "plan_create_ms_host": t_plan * 1e3}
+    rta.rta_ragged_plan_destroy(plan)
+    return res
+
+
 def host_link_bandwidth(torch, nbytes=1 << 30, reps=10):
     """Pinned H2D cudaMemcpyAsync bandwidth, best of `reps` (the H2D-fed roofline)."""
     h = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
@@ -665,6 +705,8 @@ def main():
                                       torch, dl0gen, rta)
                 torch.cuda.empty_cache()
             out["packed12"] = pk
+            out["ragged"] = ragged_leg(max(10, args.steps // 4), peak, torch, dl0gen, rta)
+            torch.cuda.empty_cache()
             link = host_link_bandwidth(torch)
             out["e2e"]["host_link_GBps_measured"] = link
             out["e2e"]["frac_of_host_link"] = out["e2e"]["value"] / link

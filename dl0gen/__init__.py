@@ -229,3 +229,73 @@ def pack12_cuda(wf_dev_ptr: int, n_samples_total: int, out_dev_ptr: int, stream:
                                         ctypes.c_void_p(out_dev_ptr), ctypes.c_void_p(stream))
     if rc != 0:
         raise RuntimeError("dl0gen_pack12_cuda: cudaError %d" % rc)
+
+
+# --------------------------------------------------------------------------- #
+# Mixed-camera batches: layout arithmetic only.
+class MixedArray:
+    """A sub-array of telescopes with the cameras of C2/C3/C4 (LST-, MST-, SST-like;
+    PAPER.md:39 names the three sizes), every telescope triggered in every event.
+    Event e holds one block per telescope slot, in slot order, each block starting
+    on a multiple of ``align`` samples; event e of slot j is event ``j_c * n_events
+    + e`` of its camera's config, j_c being the slot's rank among slots of the same
+    camera — so any block can be regenerated on the host."""
+
+    def __init__(self, slots=(("C2", 4), ("C3", 10), ("C4", 6)), n_events=1000, align=8):
+        self.n_events = int(n_events)
+        self.slots = []                                   # (config, rank among its camera)
+        for name, count in slots:
+            for j in range(count):
+                self.slots.append((CONFIGS[name], j))
+        self.tel_n_pixels = [c.n_pixels for c, _ in self.slots]
+        self.tel_n_samples = [c.n_samples for c, _ in self.slots]
+        self.tel_W = [c.W for c, _ in self.slots]
+        self.tel_calib_offset, cal = [], 0
+        for c, _ in self.slots:
+            self.tel_calib_offset.append(cal)
+            cal += c.n_pixels
+        self.n_calib = cal
+        self.slot_offset, pos = [], 0                     # samples, inside one event
+        for c, _ in self.slots:
+            pos += -pos % align
+            self.slot_offset.append(pos)
+            pos += c.n_pixels * c.n_samples
+        pos += -pos % align
+        self.event_stride = pos                           # samples
+        self.traces_per_event = sum(self.tel_n_pixels)
+        self.slot_out = [sum(self.tel_n_pixels[:j]) for j in range(len(self.slots))]
+        self.blk_tel, self.blk_wf_offset, self.blk_out_offset = [], [], []
+        for e in range(self.n_events):
+            for j in range(len(self.slots)):
+                self.blk_tel.append(j)
+                self.blk_wf_offset.append(e * self.event_stride + self.slot_offset[j])
+                self.blk_out_offset.append(e * self.traces_per_event + self.slot_out[j])
+        self.n_samples_total = self.n_events * self.event_stride
+        self.n_traces = self.n_events * self.traces_per_event
+        self.wf_bytes = 2 * self.n_events * sum(p * s for p, s in zip(self.tel_n_pixels, self.tel_n_samples))
+
+    def tables(self):
+        return (self.tel_n_pixels, self.tel_n_samples, self.tel_W, self.tel_calib_offset,
+                self.blk_tel, self.blk_wf_offset, self.blk_out_offset)
+
+    def calib(self):
+        peds, gains = zip(*[calib(c) for c, _ in self.slots])
+        return np.concatenate(peds), np.concatenate(gains)
+
+    def block_cpu(self, event: int, slot: int) -> np.ndarray:
+        """uint16 [P][S] of one block, regenerated on the host."""
+        c, j = self.slots[slot]
+        return events_cpu(c, j * self.n_events + event, 1)[0]
+
+    def fill_cuda(self, torch, d_flat) -> None:
+        """Generate every block into ``d_flat`` (int16 device tensor of
+        n_samples_total elements); gaps keep their previous content."""
+        st = torch.cuda.current_stream().cuda_stream
+        for slot, (c, j) in enumerate(self.slots):
+            n = c.n_pixels * c.n_samples
+            tmp = torch.empty((self.n_events, n), dtype=torch.int16, device=d_flat.device)
+            events_cuda(c, tmp.data_ptr(), j * self.n_events, self.n_events, st)
+            view = torch.as_strided(d_flat, (self.n_events, n), (self.event_stride, 1),
+                                    self.slot_offset[slot])
+            view.copy_(tmp)
+            del tmp

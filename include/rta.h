@@ -192,6 +192,71 @@ int rta_extract_host_packed12(const uint8_t* packed_host, int64_t n_events,
                               float* out_charge_host, float* out_time_host,
                               size_t chunk_bytes);
 
+/* ---- Mixed-camera (ragged) batches ---------------------
+ * The array has three telescope sizes (§1), runs as "multiple
+ * sub-array" configurations (§2.2), and the Central Event Builder
+ * merges the telescopes triggered by one event (§4.1). The paper
+ * gives no layout for a merged event; this one is defined here (DESIGN.md
+ * readings R28-R30):
+ *
+ *   telescope k = 0..n_tel-1:  camera of tel_n_pixels[k] pixels, tel_n_samples[k]
+ *       samples per trace, window tel_W[k]; calibration pedestal[c + p], gain[c + p]
+ *       with c = tel_calib_offset[k], p = 0..tel_n_pixels[k]-1 (flat DEVICE arrays
+ *       shared by all telescopes).
+ *   block b = 0..n_blocks-1:  one event of telescope blk_tel[b]: a dense uint16
+ *       [n_pixels][n_samples] array at SAMPLE index blk_wf_offset[b] of `wf`; its
+ *       results go to flat output index blk_out_offset[b] + p. Any order; gaps
+ *       allowed; output ranges of different blocks must not overlap.
+ *
+ * Every trace gets exactly rta_extract's result for its telescope's (S, W) and
+ * calibration. The tables are HOST arrays, read only by rta_ragged_plan_create,
+ * which validates them, cuts each block into tiles, uploads the tile tables to
+ * the current device (synchronously) and returns an opaque plan. A plan depends
+ * on the tables only — not on wf, calibration or outputs — and can be reused for
+ * any number of rta_extract_ragged calls, from any stream, until destroyed.
+ *
+ * rta_extract_ragged is asynchronous on `stream`: one launch per distinct
+ * (n_samples, W) among the blocks (rta_ragged_plan_info(RTA_RAGGED_N_LAUNCHES)).
+ * Shapes (30,7), (40,7), (25,4), (128,8) take the staged kernels; others a
+ * generic kernel. Blocks starting on a 16-byte boundary of `wf` are fastest
+ * (TMA bulk copies); 4-byte-aligned ones use 4-byte cp.async; others plain loads.
+ *
+ * Errors (plan_create, before any CUDA call): NULL table with entries, or
+ * plan == NULL -> RTA_ERR_NULL; a telescope with n_pixels < 1, n_samples < 1,
+ * W < 1, W > n_samples or a negative offset, or a block with a telescope index
+ * out of range or a negative offset -> RTA_ERR_SHAPE; n_samples*W*65535 >= 2^31,
+ * an output index >= 2^31, a calibration index >= 2^32 or a byte offset >= 2^48
+ * -> RTA_ERR_UNSUPPORTED. n_blocks == 0 gives a valid empty plan (no device
+ * needed) whose extraction is RTA_OK with nothing enqueued. */
+typedef struct rta_ragged_plan rta_ragged_plan;
+
+int rta_ragged_plan_create(int32_t n_tel, const int32_t* tel_n_pixels,
+                           const int32_t* tel_n_samples, const int32_t* tel_W,
+                           const int64_t* tel_calib_offset, int64_t n_blocks,
+                           const int32_t* blk_tel, const int64_t* blk_wf_offset,
+                           const int64_t* blk_out_offset, rta_ragged_plan** plan);
+
+/* wf, pedestal, gain, out_*: DEVICE. The caller guarantees that the buffers
+ * cover every offset in the plan (RTA_RAGGED_WF_END_BYTES, RTA_RAGGED_OUT_END). */
+int rta_extract_ragged(const rta_ragged_plan* plan, const uint16_t* wf,
+                       const int32_t* pedestal, const float* gain, int32_t* out_sum,
+                       int32_t* out_start, float* out_charge, float* out_time,
+                       void* stream);
+
+enum {
+  RTA_RAGGED_N_LAUNCHES = 0,   /* kernels per rta_extract_ragged call */
+  RTA_RAGGED_N_TILES = 1,
+  RTA_RAGGED_N_TRACES = 2,     /* sum of n_pixels over the blocks */
+  RTA_RAGGED_WF_BYTES = 3,     /* waveform bytes the blocks hold (gaps excluded) */
+  RTA_RAGGED_WF_END_BYTES = 4, /* one past the last waveform byte any block reads */
+  RTA_RAGGED_OUT_END = 5       /* one past the last output index any block writes */
+};
+int64_t rta_ragged_plan_info(const rta_ragged_plan* plan, int32_t what);  /* -1: bad argument */
+
+/* Synchronises the plan's device (kernels may still be reading the tables),
+ * frees the tables and the plan. NULL is ignored. */
+void rta_ragged_plan_destroy(rta_ragged_plan* plan);
+
 /* Static, never-NULL description of a status code. */
 const char* rta_strerror(int status);
 

@@ -76,6 +76,15 @@ def lib() -> ctypes.CDLL:
             L.rta_last_cuda_error.argtypes = []
             L.rta_kernel_name.restype = ctypes.c_char_p
             L.rta_kernel_name.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int]
+            L.rta_ragged_plan_create.restype = ctypes.c_int
+            L.rta_ragged_plan_create.argtypes = ([ctypes.c_int32] + [_VP] * 4 + [ctypes.c_int64]
+                                                 + [_VP] * 3 + [ctypes.POINTER(_VP)])
+            L.rta_extract_ragged.restype = ctypes.c_int
+            L.rta_extract_ragged.argtypes = [_VP] * 9
+            L.rta_ragged_plan_info.restype = ctypes.c_int64
+            L.rta_ragged_plan_info.argtypes = [_VP, ctypes.c_int32]
+            L.rta_ragged_plan_destroy.restype = None
+            L.rta_ragged_plan_destroy.argtypes = [_VP]
             L.rta_chunk_events.restype = ctypes.c_int64
             L.rta_chunk_events.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32,
                                            ctypes.c_size_t, ctypes.c_int32]
@@ -208,6 +217,56 @@ def rta_extract_host_packed12(packed_host, n_events, n_pixels, n_samples, pedest
         _ptr(packed_host), n_events, n_pixels, n_samples, _ptr(pedestal_host),
         _ptr(gain_host), W, _ptr(out_sum_host), _ptr(out_start_host),
         _ptr(out_charge_host), _ptr(out_time_host), int(chunk_bytes)))
+
+
+RTA_RAGGED_N_LAUNCHES = 0
+RTA_RAGGED_N_TILES = 1
+RTA_RAGGED_N_TRACES = 2
+RTA_RAGGED_WF_BYTES = 3
+RTA_RAGGED_WF_END_BYTES = 4
+RTA_RAGGED_OUT_END = 5
+
+
+def _host_array(seq, ctype):
+    seq = [int(v) for v in seq]
+    return (ctype * max(1, len(seq)))(*seq), len(seq)
+
+
+def rta_ragged_plan_create(tel_n_pixels, tel_n_samples, tel_W, tel_calib_offset,
+                           blk_tel, blk_wf_offset, blk_out_offset) -> int:
+    """include/rta.h:rta_ragged_plan_create. The tables are host sequences of
+    ints; returns the opaque plan handle (an address)."""
+    tp, n_tel = _host_array(tel_n_pixels, ctypes.c_int32)
+    ts, n1 = _host_array(tel_n_samples, ctypes.c_int32)
+    tw, n2 = _host_array(tel_W, ctypes.c_int32)
+    tc, n3 = _host_array(tel_calib_offset, ctypes.c_int64)
+    bt, n_blk = _host_array(blk_tel, ctypes.c_int32)
+    bw, m1 = _host_array(blk_wf_offset, ctypes.c_int64)
+    bo, m2 = _host_array(blk_out_offset, ctypes.c_int64)
+    if not (n_tel == n1 == n2 == n3 and n_blk == m1 == m2):
+        raise ValueError("table lengths differ")
+    plan = _VP()
+    _check(lib().rta_ragged_plan_create(
+        n_tel, ctypes.cast(tp, _VP), ctypes.cast(ts, _VP), ctypes.cast(tw, _VP),
+        ctypes.cast(tc, _VP), n_blk, ctypes.cast(bt, _VP), ctypes.cast(bw, _VP),
+        ctypes.cast(bo, _VP), ctypes.byref(plan)))
+    return plan.value
+
+
+def rta_extract_ragged(plan, wf, pedestal, gain, out_sum, out_start, out_charge, out_time,
+                       stream=None) -> None:
+    """include/rta.h:rta_extract_ragged. Device pointers; asynchronous on ``stream``."""
+    _check(lib().rta_extract_ragged(
+        plan, _ptr(wf), _ptr(pedestal), _ptr(gain), _ptr(out_sum), _ptr(out_start),
+        _ptr(out_charge), _ptr(out_time), _stream_handle(stream)))
+
+
+def rta_ragged_plan_info(plan, what: int) -> int:
+    return int(lib().rta_ragged_plan_info(plan, int(what)))
+
+
+def rta_ragged_plan_destroy(plan) -> None:
+    lib().rta_ragged_plan_destroy(plan)
 
 
 def rta_strerror(status: int) -> str:

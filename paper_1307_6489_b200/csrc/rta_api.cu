@@ -9,7 +9,11 @@
 
 #include <atomic>
 #include <cstring>
+#include <map>
 #include <mutex>
+#include <new>
+#include <utility>
+#include <vector>
 
 #include "rta_internal.h"
 
@@ -502,6 +506,149 @@ int rta_extract_host_packed12(const uint8_t* packed_host, int64_t n_events, int3
                               float* out_time_host, size_t chunk_bytes) {
   return host_impl(packed_host, n_events, n_pixels, n_samples, pedestal_host, gain_host, W,
                    out_sum_host, out_start_host, out_charge_host, out_time_host, chunk_bytes, 12);
+}
+
+// ---- mixed-camera batches (NEXT-3; readings R28-R30) ----------------
+struct rta_ragged_plan {
+  int device = -1;
+  RtaRaggedTile* tiles_dev = nullptr;  // all classes, one after the other
+  struct Class {
+    int32_t S, W;
+    uint32_t first, count;  // range in tiles_dev
+  };
+  std::vector<Class> classes;
+  int64_t n_blocks = 0, n_traces = 0, n_tiles = 0, wf_bytes = 0, wf_end = 0, out_end = 0;
+};
+
+int rta_ragged_plan_create(int32_t n_tel, const int32_t* tel_n_pixels,
+                           const int32_t* tel_n_samples, const int32_t* tel_W,
+                           const int64_t* tel_calib_offset, int64_t n_blocks,
+                           const int32_t* blk_tel, const int64_t* blk_wf_offset,
+                           const int64_t* blk_out_offset, rta_ragged_plan** plan) {
+  if (!plan) return RTA_ERR_NULL;
+  *plan = nullptr;
+  if (n_tel < 0 || n_blocks < 0) return RTA_ERR_SHAPE;
+  if (n_tel > 0 && (!tel_n_pixels || !tel_n_samples || !tel_W || !tel_calib_offset))
+    return RTA_ERR_NULL;
+  if (n_blocks > 0 && (!blk_tel || !blk_wf_offset || !blk_out_offset)) return RTA_ERR_NULL;
+  for (int32_t k = 0; k < n_tel; ++k) {
+    const int64_t P = tel_n_pixels[k], S = tel_n_samples[k], W = tel_W[k];
+    if (P < 1 || S < 1 || W < 1 || W > S || tel_calib_offset[k] < 0) return RTA_ERR_SHAPE;
+    if (S * W * 65535ll >= (1ll << 31)) return RTA_ERR_UNSUPPORTED;
+    if (tel_calib_offset[k] + P >= (1ll << 32)) return RTA_ERR_UNSUPPORTED;
+  }
+  rta_ragged_plan* pl = new (std::nothrow) rta_ragged_plan;
+  if (!pl) return RTA_ERR_NOMEM;
+  // tiles grouped by shape class, blocks in table order inside a class
+  std::map<std::pair<int32_t, int32_t>, std::vector<RtaRaggedTile>> by_shape;
+  for (int64_t b = 0; b < n_blocks; ++b) {
+    const int32_t k = blk_tel[b];
+    if (k < 0 || k >= n_tel || blk_wf_offset[b] < 0 || blk_out_offset[b] < 0) {
+      delete pl;
+      return RTA_ERR_SHAPE;
+    }
+    const int64_t P = tel_n_pixels[k], S = tel_n_samples[k];
+    const int64_t end_bytes = (blk_wf_offset[b] + P * S) * 2;
+    if (blk_out_offset[b] + P >= (1ll << 31) || end_bytes >= (1ll << 48)) {
+      delete pl;
+      return RTA_ERR_UNSUPPORTED;
+    }
+    const int64_t tt = rta_ragged_tile_traces((int32_t)S, tel_W[k]);
+    std::vector<RtaRaggedTile>& v = by_shape[std::make_pair((int32_t)S, tel_W[k])];
+    for (int64_t t0 = 0; t0 < P; t0 += tt) {
+      const int64_t n = (P - t0 < tt) ? P - t0 : tt;
+      RtaRaggedTile t;
+      t.src = (unsigned long long)((blk_wf_offset[b] + t0 * S) * 2) | ((unsigned long long)n << 48);
+      t.out_base = (uint32_t)(blk_out_offset[b] + t0);
+      t.cal0 = (uint32_t)(tel_calib_offset[k] + t0);
+      v.push_back(t);
+    }
+    pl->n_traces += P;
+    pl->wf_bytes += P * S * 2;
+    if (end_bytes > pl->wf_end) pl->wf_end = end_bytes;
+    if (blk_out_offset[b] + P > pl->out_end) pl->out_end = blk_out_offset[b] + P;
+  }
+  pl->n_blocks = n_blocks;
+  std::vector<RtaRaggedTile> all;
+  for (auto& kv : by_shape) {
+    if (kv.second.size() >= (1ull << 32) || all.size() + kv.second.size() >= (1ull << 32)) {
+      delete pl;
+      return RTA_ERR_UNSUPPORTED;
+    }
+    rta_ragged_plan::Class c;
+    c.S = kv.first.first;
+    c.W = kv.first.second;
+    c.first = (uint32_t)all.size();
+    c.count = (uint32_t)kv.second.size();
+    pl->classes.push_back(c);
+    all.insert(all.end(), kv.second.begin(), kv.second.end());
+  }
+  pl->n_tiles = (int64_t)all.size();
+  if (!all.empty()) {
+    cudaError_t e = cudaGetDevice(&pl->device);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&pl->tiles_dev, all.size() * sizeof(RtaRaggedTile));
+    if (e == cudaSuccess)
+      e = cudaMemcpy(pl->tiles_dev, all.data(), all.size() * sizeof(RtaRaggedTile),
+                     cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+      if (pl->tiles_dev) cudaFree(pl->tiles_dev);
+      delete pl;
+      return fail_cuda(e);
+    }
+  }
+  *plan = pl;
+  return RTA_OK;
+}
+
+int rta_extract_ragged(const rta_ragged_plan* plan, const uint16_t* wf, const int32_t* pedestal,
+                       const float* gain, int32_t* out_sum, int32_t* out_start,
+                       float* out_charge, float* out_time, void* stream) {
+  if (!plan) return RTA_ERR_NULL;
+  if (plan->n_tiles == 0) return RTA_OK;
+  if (!wf || !pedestal || !gain || !out_sum || !out_start || !out_charge || !out_time)
+    return RTA_ERR_NULL;
+  if ((uintptr_t)wf % 2 != 0) return RTA_ERR_ALIGN;
+  if (((uintptr_t)out_sum | (uintptr_t)out_start | (uintptr_t)out_charge | (uintptr_t)out_time |
+       (uintptr_t)pedestal | (uintptr_t)gain) % 4 != 0)
+    return RTA_ERR_ALIGN;
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail_cuda(e);
+  if (dev != plan->device) return fail_cuda(cudaErrorInvalidDevice);
+  for (const rta_ragged_plan::Class& c : plan->classes) {
+    e = rta_launch_ragged(wf, plan->tiles_dev + c.first, c.count, c.S, c.W, pedestal, gain,
+                          out_sum, out_start, out_charge, out_time, (cudaStream_t)stream);
+    if (e != cudaSuccess) return fail_cuda(e);
+  }
+  return RTA_OK;
+}
+
+int64_t rta_ragged_plan_info(const rta_ragged_plan* plan, int32_t what) {
+  if (!plan) return -1;
+  switch (what) {
+    case RTA_RAGGED_N_LAUNCHES: return (int64_t)plan->classes.size();
+    case RTA_RAGGED_N_TILES: return plan->n_tiles;
+    case RTA_RAGGED_N_TRACES: return plan->n_traces;
+    case RTA_RAGGED_WF_BYTES: return plan->wf_bytes;
+    case RTA_RAGGED_WF_END_BYTES: return plan->wf_end;
+    case RTA_RAGGED_OUT_END: return plan->out_end;
+    default: return -1;
+  }
+}
+
+void rta_ragged_plan_destroy(rta_ragged_plan* plan) {
+  if (!plan) return;
+  if (plan->tiles_dev) {
+    int cur = 0;
+    if (cudaGetDevice(&cur) == cudaSuccess) {
+      cudaSetDevice(plan->device);
+      cudaDeviceSynchronize();  // kernels of earlier calls may still read the table
+      cudaFree(plan->tiles_dev);
+      cudaSetDevice(cur);
+    }
+    cudaGetLastError();
+  }
+  delete plan;
 }
 
 const char* rta_strerror(int status) {

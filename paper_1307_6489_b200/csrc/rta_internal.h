@@ -32,6 +32,20 @@ cudaError_t rta_launch_extract(const void* wf, int64_t n_traces, int32_t n_pixel
 // Name of the kernel the dispatcher picks (static string).
 const char* rta_pick_kernel_name(int32_t n_samples, int32_t W, bool aligned16, int bits = 16);
 
+// Mixed-camera batches (include/rta.h rta_ragged_plan_*): one entry per tile of
+// at most rta_ragged_tile_traces(S, W) traces of one block.
+struct alignas(16) RtaRaggedTile {
+  unsigned long long src;  // byte offset of the tile's first trace in wf | n_traces << 48
+  uint32_t out_base;       // flat output index of the first trace
+  uint32_t cal0;           // calibration index of the first trace
+};
+int rta_ragged_tile_traces(int32_t n_samples, int32_t W);
+// One launch over a device-resident tile table whose tiles all have shape (S, W).
+cudaError_t rta_launch_ragged(const void* wf, const RtaRaggedTile* tiles_dev, uint32_t n_tiles,
+                              int32_t n_samples, int32_t W, const int32_t* pedestal,
+                              const float* gain, int32_t* out_sum, int32_t* out_start,
+                              float* out_charge, float* out_time, cudaStream_t stream);
+
 void rta_count_launch();
 
 // Tile scheduling of the staged kernels: dynamic (default) or the static

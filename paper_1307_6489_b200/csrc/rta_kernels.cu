@@ -243,8 +243,8 @@ struct WindowReader {
 
 template <class C, int MODE>
 __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, const uint32_t g0,
-                                             const uint32_t n_valid, const uint32_t n_pixels,
-                                             const uint32_t pix_inv,
+                                             const uint32_t n_valid, const uint32_t p0,
+                                             const uint32_t n_pixels,
                                              const int* __restrict__ pedestal,
                                              const float* __restrict__ gain,
                                              int* __restrict__ out_sum, int* __restrict__ out_start,
@@ -284,7 +284,9 @@ __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, c
   }
 
   Result res[C::TPT];
-  uint32_t p = fastmod(g0, n_pixels, pix_inv);
+  // p: calibration index of trace j; wraps to 0 after n_pixels - 1 (a uniform
+  // batch runs through the camera again; the ragged path passes n_pixels = 0)
+  uint32_t p = p0;
 #pragma unroll
   for (int j = 0; j < C::TPT; ++j) {
     const int h0 = j * S;  // compile-time after unrolling
@@ -503,8 +505,8 @@ __global__ void __launch_bounds__(C::NT)
     mbar_wait(bar_base + 8 * stage, parity);
     const uint8_t* unit = smem + stage * C::STAGE_BYTES + tid * C::UNIT_STRIDE;
     const uint32_t g0 = tile * C::TILE_TRACES + (uint32_t)tid * C::TPT;
-    compute_unit<C, MODE>(unit, g0, C::TPT, n_pixels, pix_inv, pedestal, gain, out_sum, out_start,
-                          out_charge, out_time, vec_store != 0, ma);
+    compute_unit<C, MODE>(unit, g0, C::TPT, fastmod(g0, n_pixels, pix_inv), n_pixels, pedestal,
+                          gain, out_sum, out_start, out_charge, out_time, vec_store != 0, ma);
     __syncthreads();  // every thread is done with this stage; tile_q slot is published
     const uint32_t next = tile_q[(j + C::STAGES) % QN];
     if (next < n_full) issue(next, stage);
@@ -533,8 +535,9 @@ __global__ void __launch_bounds__(C::NT)
     if (first < rem) {
       const uint8_t* unit = smem + tid * C::UNIT_STRIDE;
       const uint32_t g0 = n_full * C::TILE_TRACES + first;
-      compute_unit<C, MODE>(unit, g0, rem - first, n_pixels, pix_inv, pedestal, gain, out_sum,
-                            out_start, out_charge, out_time, vec_store != 0, ma);
+      compute_unit<C, MODE>(unit, g0, rem - first, fastmod(g0, n_pixels, pix_inv), n_pixels,
+                            pedestal, gain, out_sum, out_start, out_charge, out_time,
+                            vec_store != 0, ma);
     }
   }
 
@@ -578,6 +581,65 @@ struct GlobalTrace {
   }
 };
 
+// One trace through the definition with runtime (S, W): p = calibration index.
+template <int MODE, int BITS>
+__device__ __forceinline__ Result generic_trace(const GlobalTrace<BITS>& tr, const int S,
+                                                const int W, const uint32_t p,
+                                                const int* __restrict__ pedestal,
+                                                const float* __restrict__ gain,
+                                                const ModeArgs& ma) {
+  int tstar = 0, rawsum = 0, relnum = 0;
+  if constexpr (MODE == MODE_SLIDING) {
+    uint32_t sum = 0;
+    for (int k = 0; k < W; ++k) sum += tr[k];
+    uint32_t best = sum;
+    for (int t = 1; t + W <= S; ++t) {
+      sum = sum + tr[t + W - 1] - tr[t - 1];
+      if (sum > best) {  // strict: earliest on ties
+        best = sum;
+        tstar = t;
+      }
+    }
+    rawsum = (int)best;
+    for (int k = 1; k < W; ++k) relnum += k * (int)tr[tstar + k];
+  } else if constexpr (MODE == MODE_FIR) {
+    int best = 0;
+    for (int t = 0; t + W <= S; ++t) {
+      int y = 0;
+      for (int k = 0; k < W; ++k) y += ma.taps[k] * (int)tr[t + k];
+      if (t == 0 || y > best) {
+        best = y;
+        tstar = t;
+      }
+    }
+    rawsum = best;
+    for (int k = 1; k < W; ++k) relnum += k * ma.taps[k] * (int)tr[tstar + k];
+  } else {
+    if constexpr (MODE == MODE_FIXED) {
+      tstar = clamp_start(__ldg(ma.window_start + p), S, W);
+    } else {
+      int peak = 0;
+      uint32_t top = tr[0];
+      for (int k = 1; k < S; ++k) {
+        const uint32_t x = tr[k];
+        if (x > top) {
+          top = x;
+          peak = k;
+        }
+      }
+      tstar = clamp_start(peak - ma.shift, S, W);
+    }
+    for (int k = 0; k < W; ++k) {
+      const int x = (int)tr[tstar + k];
+      rawsum += x;
+      relnum += k * x;
+    }
+  }
+  const int c0 = (MODE == MODE_FIR) ? ma.c0 : W;
+  const int c1 = (MODE == MODE_FIR) ? ma.c1 : (W * (W - 1)) / 2;
+  return finish_trace(W, rawsum, tstar, relnum, __ldg(pedestal + p), __ldg(gain + p), c0, c1);
+}
+
 template <int MODE, int BITS>
 __global__ void __launch_bounds__(256)
     extract_generic_kernel(const uint8_t* __restrict__ wf, const uint32_t n_traces, const int S,
@@ -589,62 +651,198 @@ __global__ void __launch_bounds__(256)
   for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < n_traces;
        g += gridDim.x * blockDim.x) {
     const GlobalTrace<BITS> tr(wf, g, S);
-    const uint32_t p = fastmod(g, n_pixels, pix_inv);
-    int tstar = 0, rawsum = 0, relnum = 0;
-    if constexpr (MODE == MODE_SLIDING) {
-      uint32_t sum = 0;
-      for (int k = 0; k < W; ++k) sum += tr[k];
-      uint32_t best = sum;
-      for (int t = 1; t + W <= S; ++t) {
-        sum = sum + tr[t + W - 1] - tr[t - 1];
-        if (sum > best) {  // strict: earliest on ties
-          best = sum;
-          tstar = t;
-        }
-      }
-      rawsum = (int)best;
-      for (int k = 1; k < W; ++k) relnum += k * (int)tr[tstar + k];
-    } else if constexpr (MODE == MODE_FIR) {
-      int best = 0;
-      for (int t = 0; t + W <= S; ++t) {
-        int y = 0;
-        for (int k = 0; k < W; ++k) y += ma.taps[k] * (int)tr[t + k];
-        if (t == 0 || y > best) {
-          best = y;
-          tstar = t;
-        }
-      }
-      rawsum = best;
-      for (int k = 1; k < W; ++k) relnum += k * ma.taps[k] * (int)tr[tstar + k];
-    } else {
-      if constexpr (MODE == MODE_FIXED) {
-        tstar = clamp_start(__ldg(ma.window_start + p), S, W);
-      } else {
-        int peak = 0;
-        uint32_t top = tr[0];
-        for (int k = 1; k < S; ++k) {
-          const uint32_t x = tr[k];
-          if (x > top) {
-            top = x;
-            peak = k;
-          }
-        }
-        tstar = clamp_start(peak - ma.shift, S, W);
-      }
-      for (int k = 0; k < W; ++k) {
-        const int x = (int)tr[tstar + k];
-        rawsum += x;
-        relnum += k * x;
-      }
-    }
-    const int c0 = (MODE == MODE_FIR) ? ma.c0 : W;
-    const int c1 = (MODE == MODE_FIR) ? ma.c1 : (W * (W - 1)) / 2;
-    const Result r =
-        finish_trace(W, rawsum, tstar, relnum, __ldg(pedestal + p), __ldg(gain + p), c0, c1);
+    const Result r = generic_trace<MODE, BITS>(tr, S, W, fastmod(g, n_pixels, pix_inv), pedestal,
+                                               gain, ma);
     out_sum[g] = r.sum;
     out_start[g] = r.start;
     out_charge[g] = r.charge;
     out_time[g] = r.time;
+  }
+}
+
+// ------------------------------------------------- mixed-camera batches ----
+// SURVEY.md §8(f) NEXT-3 (readings R28-R30). The host plan cuts every
+// block (one telescope, one event) into tiles of at most TILE_TRACES traces of
+// one shape; one launch per shape class walks its tile table with the same
+// stage ring and dynamic scheduler as the uniform kernel. A tile whose source
+// is 16-byte aligned arrives by TMA bulk copy (cp.async 16 for the padded
+// S = 128 layout); a 4-byte-aligned one by 4-byte cp.async; anything else by
+// plain halfword copies. Every thread arrives on the stage's mbarrier through
+// cp.async.mbarrier.arrive, so the three ways share one completion mechanism.
+using RaggedTile = RtaRaggedTile;  // rta_internal.h: {src offset | n << 48, out_base, cal0}
+constexpr unsigned long long kRaggedOffMask = (1ull << 48) - 1ull;
+
+__device__ __forceinline__ void mbar_expect_tx_only(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async4(uint32_t dst, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+}
+
+template <class C>
+__global__ void __launch_bounds__(C::NT)
+    extract_ragged_kernel(const uint8_t* __restrict__ wf, const RaggedTile* __restrict__ tiles,
+                          const uint32_t n_tiles, const int* __restrict__ pedestal,
+                          const float* __restrict__ gain, int* __restrict__ out_sum,
+                          int* __restrict__ out_start, float* __restrict__ out_charge,
+                          float* __restrict__ out_time, const int vec_store,
+                          uint32_t* __restrict__ sched) {
+  static_assert(C::BITS == 16 && C::STAGES >= 2, "uint16 blocks, at least two stages");
+  extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t full_bar[C::STAGES];
+  constexpr int QN = C::STAGES + 1;
+  __shared__ uint32_t tile_q[QN];
+  const int tid = threadIdx.x;
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t bar_base = smem_u32(full_bar);
+  const ModeArgs ma = {};
+
+  // tile indices: the first STAGES of a CTA are static (blockIdx.x + k * gridDim.x),
+  // the rest come from the shared counter, one run of tiles per atomic
+  constexpr uint32_t kMaxRun = 8;
+  const uint32_t dyn_base = (uint32_t)C::STAGES * gridDim.x;
+  uint32_t static_next = blockIdx.x, cur = 0, end = 0, nxt = 0, n_run = 0;
+  auto fetch_static = [&]() -> uint32_t {
+    const uint32_t t = static_next;
+    static_next = (t > 0xFFFFFFFFu - gridDim.x) ? 0xFFFFFFFFu : t + gridDim.x;
+    return t;
+  };
+  auto run_length = [&](const uint32_t seen) -> uint32_t {
+    const uint32_t left = n_tiles > seen ? n_tiles - seen : 0u;
+    const uint32_t k = left / (8u * gridDim.x);
+    return k < 1u ? 1u : (k > kMaxRun ? kMaxRun : k);
+  };
+  auto fetch = [&]() -> uint32_t {
+    if (sched == nullptr) return fetch_static();
+    if (cur == end) {
+      cur = nxt;
+      end = nxt + n_run;
+      n_run = run_length(cur);
+      nxt = dyn_base + atomicAdd(sched, n_run);
+    }
+    return cur++;
+  };
+
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < C::STAGES; ++s) {
+      mbar_init(bar_base + 8 * s, C::NT);
+      tile_q[s] = fetch_static();
+    }
+    fence_mbar_init();
+    if (sched != nullptr) {
+      n_run = run_length(dyn_base);
+      nxt = dyn_base + atomicAdd(sched, n_run);
+    }
+  }
+  __syncthreads();
+
+  constexpr uint32_t UB = C::UNIT_BYTES, PADB = C::UNIT_STRIDE - C::UNIT_BYTES;
+  constexpr uint32_t TRACE_BYTES = C::TRACE_BITS / 8;
+  auto issue = [&](const uint32_t ti, const int stage) {
+    const RaggedTile t = tiles[ti];
+    const uint8_t* src = wf + (size_t)(t.src & kRaggedOffMask);
+    const uint32_t bytes = (uint32_t)(t.src >> 48) * TRACE_BYTES;
+    uint8_t* dstp = smem + stage * C::STAGE_BYTES;
+    const uint32_t dst = smem_base + stage * C::STAGE_BYTES;
+    const uint32_t bar = bar_base + 8 * stage;
+    const uint32_t mis = (uint32_t)(reinterpret_cast<uintptr_t>(src) & 15u);
+    uint32_t done;  // bytes moved by the wide path; the rest goes halfword by halfword
+    if (mis == 0) {
+      if constexpr (!C::PAD) {
+        done = bytes & ~15u;
+        if (tid == 0 && done != 0) {
+          mbar_expect_tx_only(bar, done);
+          tma_bulk_g2s(dst, src, done, bar);
+        }
+      } else {
+        done = bytes;  // a padded unit is a whole number of 16-byte chunks
+        for (uint32_t c = tid; c < bytes / 16u; c += C::NT)
+          cp_async16(dst + (c + c / (UB / 16u)) * 16u, src + (size_t)c * 16u);
+      }
+    } else if ((mis & 3u) == 0) {
+      done = bytes & ~3u;
+      for (uint32_t c = tid; c < done / 4u; c += C::NT) {
+        uint32_t d = c * 4u;
+        if constexpr (C::PAD) d += (d / UB) * PADB;
+        cp_async4(dst + d, src + (size_t)c * 4u);
+      }
+    } else {
+      done = 0;
+    }
+    for (uint32_t b = done + 2u * tid; b < bytes; b += 2u * C::NT) {
+      uint32_t d = b;
+      if constexpr (C::PAD) d += (b / UB) * PADB;
+      *reinterpret_cast<uint16_t*>(dstp + d) = *reinterpret_cast<const uint16_t*>(src + b);
+    }
+    cp_async_mbar_arrive(bar);  // counts once this thread's cp.async copies have landed
+  };
+
+#pragma unroll
+  for (int s = 0; s < C::STAGES; ++s) {
+    const uint32_t tile = tile_q[s];
+    if (tile < n_tiles) issue(tile, s);
+  }
+  uint32_t pre = 0;
+  if (tid == 0) pre = fetch();
+
+  for (uint32_t j = 0;; ++j) {
+    const uint32_t tile = tile_q[j % QN];
+    if (tile >= n_tiles) break;
+    const int stage = (int)(j % C::STAGES);
+    const uint32_t parity = (j / C::STAGES) & 1u;
+    if (tid == 0) {
+      tile_q[(j + C::STAGES) % QN] = pre;
+      pre = fetch();
+    }
+    const RaggedTile t = tiles[tile];
+    const uint32_t n = (uint32_t)(t.src >> 48);
+    mbar_wait(bar_base + 8 * stage, parity);
+    const uint32_t first = (uint32_t)tid * C::TPT;
+    if (first < n) {
+      const uint8_t* unit = smem + stage * C::STAGE_BYTES + tid * C::UNIT_STRIDE;
+      compute_unit<C, MODE_SLIDING>(unit, t.out_base + first, n - first, t.cal0 + first, 0u,
+                                    pedestal, gain, out_sum, out_start, out_charge, out_time,
+                                    vec_store != 0 && (t.out_base & 1u) == 0, ma);
+    }
+    __syncthreads();
+    const uint32_t next = tile_q[(j + C::STAGES) % QN];
+    if (next < n_tiles) issue(next, stage);
+  }
+
+  if (sched != nullptr && tid == 0) {
+    __threadfence();
+    if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) {
+      sched[0] = 0;
+      sched[1] = 0;
+      __threadfence();
+    }
+  }
+}
+
+// Shapes without a specialisation: one thread per trace, one tile (<= 256 traces) per CTA pass.
+__global__ void __launch_bounds__(256)
+    extract_ragged_generic_kernel(const uint8_t* __restrict__ wf,
+                                  const RaggedTile* __restrict__ tiles, const uint32_t n_tiles,
+                                  const int S, const int W, const int* __restrict__ pedestal,
+                                  const float* __restrict__ gain, int* __restrict__ out_sum,
+                                  int* __restrict__ out_start, float* __restrict__ out_charge,
+                                  float* __restrict__ out_time) {
+  const ModeArgs ma = {};
+  for (uint32_t ti = blockIdx.x; ti < n_tiles; ti += gridDim.x) {
+    const RaggedTile t = tiles[ti];
+    const uint32_t n = (uint32_t)(t.src >> 48);
+    if (threadIdx.x < n) {
+      const GlobalTrace<16> tr(wf + (size_t)(t.src & kRaggedOffMask), threadIdx.x, S);
+      const Result r =
+          generic_trace<MODE_SLIDING, 16>(tr, S, W, t.cal0 + threadIdx.x, pedestal, gain, ma);
+      const uint32_t g = t.out_base + threadIdx.x;
+      out_sum[g] = r.sum;
+      out_start[g] = r.start;
+      out_charge[g] = r.charge;
+      out_time[g] = r.time;
+    }
   }
 }
 
@@ -930,7 +1128,85 @@ cudaError_t launch_packed12(const LaunchArgs& a, const ModeArgs& ma) {
 }
 #undef RTA_TRY
 
+template <class C>
+struct RaggedLauncher {
+  static std::atomic<int> ready[kMaxDevices];
+  static int ctas_per_sm[kMaxDevices];
+  static cudaError_t launch(const uint8_t* wf, const RaggedTile* tiles, uint32_t n_tiles,
+                            const int32_t* pedestal, const float* gain, int32_t* out_sum,
+                            int32_t* out_start, float* out_charge, float* out_time,
+                            cudaStream_t stream) {
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
+    if (!ready[dev].load(std::memory_order_acquire)) {
+      e = cudaFuncSetAttribute(extract_ragged_kernel<C>,
+                               cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+      if (e != cudaSuccess) return e;
+      int occ = 0;
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, extract_ragged_kernel<C>, C::NT,
+                                                        C::SMEM_BYTES);
+      if (e != cudaSuccess) return e;
+      if (occ < 1) return cudaErrorLaunchOutOfResources;
+      ctas_per_sm[dev] = occ;
+      ready[dev].store(1, std::memory_order_release);
+    }
+    uint32_t grid = (uint32_t)(sms * ctas_per_sm[dev]);
+    if (grid > n_tiles) grid = n_tiles;
+    const uintptr_t o = (uintptr_t)out_sum | (uintptr_t)out_start | (uintptr_t)out_charge |
+                        (uintptr_t)out_time;
+    uint32_t* sched = g_static_schedule ? nullptr : sched_words(dev, stream);
+    extract_ragged_kernel<C><<<grid, C::NT, C::SMEM_BYTES, stream>>>(
+        wf, tiles, n_tiles, pedestal, gain, out_sum, out_start, out_charge, out_time,
+        (o % 8 == 0) ? 1 : 0, sched);
+    rta_count_launch();
+    return cudaGetLastError();
+  }
+};
+template <class C>
+std::atomic<int> RaggedLauncher<C>::ready[kMaxDevices];
+template <class C>
+int RaggedLauncher<C>::ctas_per_sm[kMaxDevices];
+
 }  // namespace
+
+int rta_ragged_tile_traces(int32_t S, int32_t W) {
+  if (S == CfgS30W7::S && W == CfgS30W7::W) return CfgS30W7::TILE_TRACES;
+  if (S == CfgS40W7::S && W == CfgS40W7::W) return CfgS40W7::TILE_TRACES;
+  if (S == CfgS25W4::S && W == CfgS25W4::W) return CfgS25W4::TILE_TRACES;
+  if (S == CfgS128W8::S && W == CfgS128W8::W) return CfgS128W8::TILE_TRACES;
+  return 256;  // extract_ragged_generic_kernel: one thread per trace, 256 threads
+}
+
+cudaError_t rta_launch_ragged(const void* wf, const RtaRaggedTile* tiles_dev, uint32_t n_tiles,
+                              int32_t S, int32_t W, const int32_t* pedestal, const float* gain,
+                              int32_t* out_sum, int32_t* out_start, float* out_charge,
+                              float* out_time, cudaStream_t stream) {
+  if (n_tiles == 0) return cudaSuccess;
+  const uint8_t* w = static_cast<const uint8_t*>(wf);
+#define RTA_TRY(CFG)                                                                        \
+  if (S == CFG::S && W == CFG::W)                                                           \
+    return RaggedLauncher<CFG>::launch(w, tiles_dev, n_tiles, pedestal, gain, out_sum,      \
+                                       out_start, out_charge, out_time, stream);
+  RTA_TRY(CfgS30W7)
+  RTA_TRY(CfgS40W7)
+  RTA_TRY(CfgS25W4)
+  RTA_TRY(CfgS128W8)
+#undef RTA_TRY
+  int dev = 0, sms = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
+  uint32_t grid = n_tiles;
+  const uint32_t cap = (uint32_t)sms * 8u;
+  if (grid > cap) grid = cap;
+  extract_ragged_generic_kernel<<<grid, 256, 0, stream>>>(w, tiles_dev, n_tiles, S, W, pedestal,
+                                                          gain, out_sum, out_start, out_charge,
+                                                          out_time);
+  rta_count_launch();
+  return cudaGetLastError();
+}
 
 cudaError_t rta_launch_extract(const void* wf, int64_t n_traces64, int32_t n_pixels,
                                int32_t S, const int32_t* pedestal, const float* gain, int32_t W,

@@ -223,3 +223,50 @@ def test_chunk_events_planning():
                     if bits == 12 and got < E:                       # every later chunk starts aligned
                         assert (got * ev_bits) % 128 == 0
     assert ce(-1, 4, 30, 0, 16) == -1 and ce(1, 4, 30, 0, 8) == -1 and ce(1, 0, 30, 0, 12) == -1
+
+
+# ---- mixed-camera (ragged) plans: validation is pure host logic ----------------
+def _plan_status(tp, ts, tw, tc, bt, bw, bo):
+    L = rta.lib()
+    a32 = lambda v: (ctypes.c_int32 * max(1, len(v)))(*v)
+    a64 = lambda v: (ctypes.c_int64 * max(1, len(v)))(*v)
+    plan = ctypes.c_void_p()
+    rc = L.rta_ragged_plan_create(len(tp), ctypes.cast(a32(tp), ctypes.c_void_p), ctypes.cast(a32(ts), ctypes.c_void_p),
+                                  ctypes.cast(a32(tw), ctypes.c_void_p), ctypes.cast(a64(tc), ctypes.c_void_p),
+                                  len(bt), ctypes.cast(a32(bt), ctypes.c_void_p), ctypes.cast(a64(bw), ctypes.c_void_p),
+                                  ctypes.cast(a64(bo), ctypes.c_void_p), ctypes.byref(plan))
+    if rc == rta.RTA_OK:
+        L.rta_ragged_plan_destroy(plan)
+    else:
+        assert plan.value is None
+    return rc
+
+
+def test_ragged_plan_validation_before_any_cuda_call():
+    ok = ([4], [30], [7], [0])
+    assert _plan_status(*ok, [], [], []) == rta.RTA_OK                       # empty plan, no device needed
+    assert _plan_status([0], [30], [7], [0], [], [], []) == rta.RTA_ERR_SHAPE
+    assert _plan_status([4], [30], [31], [0], [], [], []) == rta.RTA_ERR_SHAPE   # W > S
+    assert _plan_status([4], [30], [0], [0], [], [], []) == rta.RTA_ERR_SHAPE
+    assert _plan_status([4], [30], [7], [-1], [], [], []) == rta.RTA_ERR_SHAPE
+    assert _plan_status([4], [2048], [17], [0], [], [], []) == rta.RTA_ERR_UNSUPPORTED
+    assert _plan_status(*ok, [1], [0], [0]) == rta.RTA_ERR_SHAPE              # telescope index out of range
+    assert _plan_status(*ok, [-1], [0], [0]) == rta.RTA_ERR_SHAPE
+    assert _plan_status(*ok, [0], [-2], [0]) == rta.RTA_ERR_SHAPE
+    assert _plan_status(*ok, [0], [0], [-2]) == rta.RTA_ERR_SHAPE
+    assert _plan_status(*ok, [0], [0], [2 ** 31 - 2]) == rta.RTA_ERR_UNSUPPORTED
+    assert _plan_status(*ok, [0], [2 ** 47], [0]) == rta.RTA_ERR_UNSUPPORTED
+    L = rta.lib()
+    assert L.rta_ragged_plan_create(0, None, None, None, None, 0, None, None, None, None) == rta.RTA_ERR_NULL
+    assert L.rta_extract_ragged(None, 0x1000, 0x2000, 0x3000, 0x4000, 0x5000, 0x6000, 0x7000, 0) == rta.RTA_ERR_NULL
+    assert L.rta_ragged_plan_info(None, 0) == -1
+    L.rta_ragged_plan_destroy(None)
+    # an empty plan extracts to RTA_OK with null pointers and launches nothing
+    plan = rta.rta_ragged_plan_create([4], [30], [7], [0], [], [], [])
+    before = rta.rta_launch_count()
+    assert L.rta_extract_ragged(plan, None, None, None, None, None, None, None, 0) == rta.RTA_OK
+    assert rta.rta_launch_count() == before
+    assert rta.rta_ragged_plan_info(plan, rta.RTA_RAGGED_N_TILES) == 0
+    assert rta.rta_ragged_plan_info(plan, rta.RTA_RAGGED_N_LAUNCHES) == 0
+    assert rta.rta_ragged_plan_info(plan, 99) == -1
+    rta.rta_ragged_plan_destroy(plan)
