@@ -299,3 +299,30 @@ class MixedArray:
                                     self.slot_offset[slot])
             view.copy_(tmp)
             del tmp
+
+
+# --------------------------------------------------------------------------- #
+# Synthetic camera geometry (the real pixel tables are
+# not available). Geometry only: no cleaning, no moments.
+def hex_camera(n_pixels: int, pitch: float = 0.05):
+    """The ``n_pixels`` hexagonal-lattice points nearest the origin (ties broken
+    by the integer axial coordinates, so the result is platform-independent).
+    Returns (x float32[P], y float32[P], neighbors int32[P][6], -1 = none).
+    Axial (a, b): x = pitch (a + b/2), y = pitch (sqrt(3)/2) b; neighbours are the
+    six lattice neighbours (+-1,0), (0,+-1), (1,-1), (-1,1) present in the set."""
+    n_pixels = int(n_pixels)
+    r = 2
+    while 3 * r * (r + 1) + 1 < n_pixels:
+        r += 1
+    r += 2
+    pts = [(a * a + a * b + b * b, a, b) for a in range(-r, r + 1) for b in range(-r, r + 1)]
+    pts.sort()
+    pts = pts[:n_pixels]
+    index = {(a, b): i for i, (_, a, b) in enumerate(pts)}
+    x = np.array([pitch * (a + 0.5 * b) for _, a, b in pts], np.float64).astype(np.float32)
+    y = np.array([pitch * (np.sqrt(3.0) / 2.0) * b for _, a, b in pts], np.float64).astype(np.float32)
+    nbr = np.full((n_pixels, 6), -1, np.int32)
+    for i, (_, a, b) in enumerate(pts):
+        for j, (da, db) in enumerate(((1, 0), (-1, 0), (0, 1), (0, -1), (1, -1), (-1, 1))):
+            nbr[i, j] = index.get((a + da, b + db), -1)
+    return x, y, nbr

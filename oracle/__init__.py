@@ -22,7 +22,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rta_oracle.cpp")
 _SRCS = [_SRC, os.path.join(_HERE, "rta_oracle_windows.cpp"),
          os.path.join(_HERE, "rta_oracle_packed.cpp"),
-         os.path.join(_HERE, "rta_oracle_ragged.cpp")]
+         os.path.join(_HERE, "rta_oracle_ragged.cpp"),
+         os.path.join(_HERE, "rta_oracle_image.cpp")]
 _LIB = os.path.join(_HERE, "librta_oracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -68,6 +69,10 @@ def _load():
         lib.rta_oracle_extract_ragged.argtypes = (
             [ctypes.c_void_p, ctypes.c_int32] + [ctypes.c_void_p] * 4 + [ctypes.c_int64]
             + [ctypes.c_void_p] * 3 + [ctypes.c_void_p] * 2 + [ctypes.c_void_p] * 4)
+        lib.rta_oracle_image_moments.restype = ctypes.c_int
+        lib.rta_oracle_image_moments.argtypes = (
+            [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32] + [ctypes.c_void_p] * 3
+            + [ctypes.c_float, ctypes.c_float] + [ctypes.c_void_p] * 3)
         _lib = lib
     return _lib
 
@@ -230,6 +235,32 @@ def extract_ragged(wf, tel_n_pixels, tel_n_samples, tel_W, tel_calib_offset, blk
     if rc != 0:
         raise ValueError("rta_oracle_extract_ragged: bad table")
     return outs
+
+
+def image_moments(charge, time, pix_x, pix_y, neighbors, thr_picture: float, thr_boundary: float):
+    """Cleaning + image moments per event (rta_oracle_image.cpp, readings R31-R35).
+    ``charge``/``time``: float32 [E][P]. Returns (n_pix int32[E], params float32[E][8],
+    mask uint8[E][P]); params = size, cog_x, cog_y, length, width, psi, t_mean, q_max."""
+    charge = np.ascontiguousarray(charge, dtype=np.float32)
+    time = np.ascontiguousarray(time, dtype=np.float32)
+    if charge.ndim != 2 or time.shape != charge.shape:
+        raise ValueError("charge and time must be [n_events][n_pixels]")
+    E, P = charge.shape
+    pix_x = np.ascontiguousarray(pix_x, dtype=np.float32)
+    pix_y = np.ascontiguousarray(pix_y, dtype=np.float32)
+    neighbors = np.ascontiguousarray(neighbors, dtype=np.int32)
+    if pix_x.shape != (P,) or pix_y.shape != (P,) or neighbors.shape != (P, 6):
+        raise ValueError("geometry must be x[P], y[P], neighbors[P][6]")
+    npix = np.empty(E, np.int32)
+    params = np.empty((E, 8), np.float32)
+    mask = np.empty((E, P), np.uint8)
+    rc = _load().rta_oracle_image_moments(
+        charge.ctypes.data, time.ctypes.data, E, P, pix_x.ctypes.data, pix_y.ctypes.data,
+        neighbors.ctypes.data, float(thr_picture), float(thr_boundary), npix.ctypes.data,
+        params.ctypes.data, mask.ctypes.data)
+    if rc != 0:
+        raise ValueError("rta_oracle_image_moments: bad shape")
+    return npix, params, mask
 
 
 def extract_threads(wf, pedestal, gain, W, threads: int):
