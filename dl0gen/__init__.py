@@ -304,6 +304,13 @@ class MixedArray:
 # --------------------------------------------------------------------------- #
 # Synthetic camera geometry (the real pixel tables are
 # not available). Geometry only: no cleaning, no moments.
+# Cleaning thresholds (picture, boundary) used with each config's charges by the
+# tests and bench.py (inputs of the call, chosen so that most events keep a few
+# dozen pixels and a few keep none; charge unit = ADC counts summed over W).
+IMAGE_THRESHOLDS = {"C1": (60.0, 30.0), "C2": (60.0, 30.0), "C3": (40.0, 20.0), "C4": (60.0, 30.0),
+                    "C5": (60.0, 30.0)}
+
+
 def hex_camera(n_pixels: int, pitch: float = 0.05):
     """The ``n_pixels`` hexagonal-lattice points nearest the origin (ties broken
     by the integer axial coordinates, so the result is platform-independent).

@@ -257,6 +257,92 @@ int64_t rta_ragged_plan_info(const rta_ragged_plan* plan, int32_t what);  /* -1:
  * frees the tables and the plan. NULL is ignored. */
 void rta_ragged_plan_destroy(rta_ragged_plan* plan);
 
+/* ---- Image cleaning + image moments ---------------------
+ * The first step downstream of the extraction, so that "event-level
+ * reconstruction parameters (but not the raw data)" (§2.2) are what
+ * leaves the GPU. The paper names the chain only ("calibration, the
+ * gamma/hadron separation, and the energy and direction reconstruction",
+ * PAPER.md:101 §4.1; RT-RECO is a reduced, fast version, §4.2) and
+ * defines none of it; the operation is defined here (readings R31-R35).
+ * Per event, with q[p] the pixel charges, t[p] the peak times, (x[p], y[p]) the
+ * pixel centres and up to six neighbours per pixel:
+ *
+ *   core[p] = q[p] >= thr_picture                      (fp32 compare; NaN fails)
+ *   keep[p] = core[p] and some neighbour n of p has core[n]
+ *   edge[p] = q[p] >= thr_boundary and some neighbour n of p has keep[n]
+ *   mask[p] = keep[p] or edge[p]
+ *   n_pix   = pixels in the mask;   size = sum q over the mask
+ *   cog_x   = sum q x / size,  cog_y = sum q y / size
+ *   sxx     = sum q (x - cog_x)^2 / size,  syy likewise,  sxy = sum q (x - cog_x)(y - cog_y) / size
+ *   z       = sqrt((sxx - syy)^2 + 4 sxy^2)
+ *   length  = sqrt((sxx + syy + z) / 2),   width = sqrt(max(0, (sxx + syy - z) / 2))
+ *   psi     = atan2(2 sxy, sxx - syy) / 2            (major-axis angle, (-pi/2, pi/2])
+ *   t_mean  = sum q t / size;   q_max = largest q in the mask
+ *   out_params[e][0..7] = size, cog_x, cog_y, length, width, psi, t_mean, q_max
+ *   n_pix == 0, or size <= 0 or NaN  ->  all eight parameters are 0 (n_pix is still the count).
+ *
+ * Sums are accumulated in fp64 and rounded once to fp32; n_pix, the mask and
+ * q_max are exact. Results do not depend on the launch (no atomics).
+ *
+ *   pix_x, pix_y  DEVICE float [n_pixels]      pixel centres, any unit
+ *   neighbors     DEVICE int32 [n_pixels][6]   neighbour pixel indices; any value outside
+ *                                              [0, n_pixels) means "no neighbour". The table is
+ *                                              used as given (it need not be symmetric).
+ *   out_n_pix     DEVICE int32 [n_events]
+ *   out_params    DEVICE float [n_events][8]
+ *   out_mask      DEVICE uint8 [n_events][n_pixels] (0/1), or NULL when not wanted
+ *
+ * rta_image_moments: cleaning + moments of charge / time arrays already on the
+ * device (float [n_events][n_pixels], e.g. rta_extract's out_charge / out_time).
+ * rta_extract_image: rta_extract's sliding-window extraction and the step above
+ * in ONE kernel; charge and peak time stay in shared memory and only the event
+ * parameters (36 bytes per event, + the mask if asked for) are written. Shapes
+ * (30,7), (40,7), (25,4), (128,8) with a 16-byte-aligned wf and every event
+ * starting on a boundary the staged loads accept take the staged kernels; any
+ * other shape or alignment a generic kernel. Same results either way
+ * (rta_image_kernel_name says which). rta_extract_image(...) equals
+ * rta_extract(...) followed by rta_image_moments(out_charge, out_time, ...).
+ * rta_extract_image_stream / _host: the host-fed variants, chunked and double
+ * buffered exactly like rta_extract_stream / rta_extract_host (same chunk rule,
+ * same workspace and mutex); _host brings 36 bytes per event (+ mask) back.
+ *
+ * All asynchronous on `stream` except _host. Errors: the shape/NULL/alignment
+ * rules of rta_extract for the waveform side; n_pixels above
+ * rta_image_max_pixels() (one event's charges, times and flags must fit one
+ * CTA's shared memory: 23 136 pixels) -> RTA_ERR_UNSUPPORTED; NULL geometry or
+ * output (out_mask excepted) -> RTA_ERR_NULL; 4-byte alignment of every float /
+ * int32 array. NaN thresholds give empty masks. n_events == 0 -> RTA_OK. */
+int rta_image_moments(const float* charge, const float* time, int64_t n_events,
+                      int32_t n_pixels, const float* pix_x, const float* pix_y,
+                      const int32_t* neighbors, float thr_picture, float thr_boundary,
+                      int32_t* out_n_pix, float* out_params, uint8_t* out_mask, void* stream);
+
+int rta_extract_image(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
+                      int32_t n_samples, const int32_t* pedestal, const float* gain, int32_t W,
+                      const float* pix_x, const float* pix_y, const int32_t* neighbors,
+                      float thr_picture, float thr_boundary, int32_t* out_n_pix,
+                      float* out_params, uint8_t* out_mask, void* stream);
+
+/* wf_host: HOST (pinned or pageable); everything else DEVICE. */
+int rta_extract_image_stream(const uint16_t* wf_host, int64_t n_events, int32_t n_pixels,
+                             int32_t n_samples, const int32_t* pedestal, const float* gain,
+                             int32_t W, const float* pix_x, const float* pix_y,
+                             const int32_t* neighbors, float thr_picture, float thr_boundary,
+                             int32_t* out_n_pix, float* out_params, uint8_t* out_mask,
+                             size_t chunk_bytes, void* stream);
+
+/* Every pointer HOST; synchronous. */
+int rta_extract_image_host(const uint16_t* wf_host, int64_t n_events, int32_t n_pixels,
+                           int32_t n_samples, const int32_t* pedestal_host,
+                           const float* gain_host, int32_t W, const float* pix_x_host,
+                           const float* pix_y_host, const int32_t* neighbors_host,
+                           float thr_picture, float thr_boundary, int32_t* out_n_pix_host,
+                           float* out_params_host, uint8_t* out_mask_host, size_t chunk_bytes);
+
+/* "image_tile<S=40,W=7>", ..., or "image_generic". */
+const char* rta_image_kernel_name(int32_t n_pixels, int32_t n_samples, int32_t W, int aligned16);
+int32_t rta_image_max_pixels(void);
+
 /* Static, never-NULL description of a status code. */
 const char* rta_strerror(int status);
 

@@ -85,6 +85,26 @@ def lib() -> ctypes.CDLL:
             L.rta_ragged_plan_info.argtypes = [_VP, ctypes.c_int32]
             L.rta_ragged_plan_destroy.restype = None
             L.rta_ragged_plan_destroy.argtypes = [_VP]
+            _CAM = [_VP, _VP, _VP, ctypes.c_float, ctypes.c_float]
+            _IMG_OUT = [_VP, _VP, _VP]
+            L.rta_image_moments.restype = ctypes.c_int
+            L.rta_image_moments.argtypes = ([_VP, _VP, ctypes.c_int64, ctypes.c_int32] + _CAM
+                                            + _IMG_OUT + [_VP])
+            for name in ("rta_extract_image", "rta_extract_image_generic"):
+                fn = getattr(L, name)
+                fn.restype = ctypes.c_int
+                fn.argtypes = _EXTRACT_ARGS[:7] + _CAM + _IMG_OUT + [_VP]
+            L.rta_extract_image_stream.restype = ctypes.c_int
+            L.rta_extract_image_stream.argtypes = (_EXTRACT_ARGS[:7] + _CAM + _IMG_OUT
+                                                   + [ctypes.c_size_t, _VP])
+            L.rta_extract_image_host.restype = ctypes.c_int
+            L.rta_extract_image_host.argtypes = (_EXTRACT_ARGS[:7] + _CAM + _IMG_OUT
+                                                 + [ctypes.c_size_t])
+            L.rta_image_kernel_name.restype = ctypes.c_char_p
+            L.rta_image_kernel_name.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                                ctypes.c_int]
+            L.rta_image_max_pixels.restype = ctypes.c_int32
+            L.rta_image_max_pixels.argtypes = []
             L.rta_chunk_events.restype = ctypes.c_int64
             L.rta_chunk_events.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32,
                                            ctypes.c_size_t, ctypes.c_int32]
@@ -267,6 +287,58 @@ def rta_ragged_plan_info(plan, what: int) -> int:
 
 def rta_ragged_plan_destroy(plan) -> None:
     lib().rta_ragged_plan_destroy(plan)
+
+
+def rta_image_moments(charge, time, n_events, n_pixels, pix_x, pix_y, neighbors, thr_picture,
+                      thr_boundary, out_n_pix, out_params, out_mask=None, stream=None) -> None:
+    """include/rta.h:rta_image_moments. Device pointers; asynchronous on ``stream``."""
+    _check(lib().rta_image_moments(
+        _ptr(charge), _ptr(time), n_events, n_pixels, _ptr(pix_x), _ptr(pix_y), _ptr(neighbors),
+        float(thr_picture), float(thr_boundary), _ptr(out_n_pix), _ptr(out_params),
+        _ptr(out_mask), _stream_handle(stream)))
+
+
+def rta_extract_image(wf, n_events, n_pixels, n_samples, pedestal, gain, W, pix_x, pix_y,
+                      neighbors, thr_picture, thr_boundary, out_n_pix, out_params,
+                      out_mask=None, stream=None, *, generic: bool = False) -> None:
+    """include/rta.h:rta_extract_image. Device pointers; asynchronous on ``stream``."""
+    fn = lib().rta_extract_image_generic if generic else lib().rta_extract_image
+    _check(fn(_ptr(wf), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain), W,
+              _ptr(pix_x), _ptr(pix_y), _ptr(neighbors), float(thr_picture),
+              float(thr_boundary), _ptr(out_n_pix), _ptr(out_params), _ptr(out_mask),
+              _stream_handle(stream)))
+
+
+def rta_extract_image_stream(wf_host, n_events, n_pixels, n_samples, pedestal, gain, W, pix_x,
+                             pix_y, neighbors, thr_picture, thr_boundary, out_n_pix, out_params,
+                             out_mask=None, chunk_bytes=0, stream=None) -> None:
+    """include/rta.h:rta_extract_image_stream. ``wf_host`` is host memory; the
+    rest are device pointers."""
+    _check(lib().rta_extract_image_stream(
+        _ptr(wf_host), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain), W,
+        _ptr(pix_x), _ptr(pix_y), _ptr(neighbors), float(thr_picture), float(thr_boundary),
+        _ptr(out_n_pix), _ptr(out_params), _ptr(out_mask), int(chunk_bytes),
+        _stream_handle(stream)))
+
+
+def rta_extract_image_host(wf_host, n_events, n_pixels, n_samples, pedestal_host, gain_host, W,
+                           pix_x_host, pix_y_host, neighbors_host, thr_picture, thr_boundary,
+                           out_n_pix_host, out_params_host, out_mask_host=None,
+                           chunk_bytes=0) -> None:
+    """include/rta.h:rta_extract_image_host. Every pointer is host memory; synchronous."""
+    _check(lib().rta_extract_image_host(
+        _ptr(wf_host), n_events, n_pixels, n_samples, _ptr(pedestal_host), _ptr(gain_host), W,
+        _ptr(pix_x_host), _ptr(pix_y_host), _ptr(neighbors_host), float(thr_picture),
+        float(thr_boundary), _ptr(out_n_pix_host), _ptr(out_params_host), _ptr(out_mask_host),
+        int(chunk_bytes)))
+
+
+def rta_image_kernel_name(n_pixels: int, n_samples: int, W: int, aligned16: bool = True) -> str:
+    return lib().rta_image_kernel_name(n_pixels, n_samples, W, 1 if aligned16 else 0).decode()
+
+
+def rta_image_max_pixels() -> int:
+    return int(lib().rta_image_max_pixels())
 
 
 def rta_strerror(status: int) -> str:

@@ -3,6 +3,7 @@ sm_100a. ``python -m paper_1307_6489_b200.build`` or ``build()``."""
 from __future__ import annotations
 
 import os
+import shlex
 import subprocess
 import sys
 
@@ -10,12 +11,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librta.so")
-SOURCES = [os.path.join(CSRC, "rta_kernels.cu"), os.path.join(CSRC, "rta_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "rta_internal.h"), os.path.join(ROOT, "include", "rta.h")]
+SOURCES = [os.path.join(CSRC, n) for n in ("rta_kernels.cu", "rta_image.cu", "rta_api.cu")]
+DEPS = SOURCES + [os.path.join(CSRC, "rta_internal.h"), os.path.join(CSRC, "rta_device.cuh"),
+                  os.path.join(ROOT, "include", "rta.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-    "-Xcompiler", "-fPIC", "-shared",
+    "-Xcompiler", "-fPIC",
 ]
 
 
@@ -26,10 +28,23 @@ def stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
-        tmp = LIB + ".tmp%d" % os.getpid()
-        cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
-        subprocess.check_call(cmd)
-        os.replace(tmp, LIB)
+        # one nvcc per translation unit, side by side, then one link
+        tag = ".tmp%d" % os.getpid()
+        extra = (["-Xptxas", "-v"] if verbose else []) + shlex.split(os.environ.get("RTA_NVCC_EXTRA", ""))
+        objs = [os.path.join(HERE, os.path.basename(s)[:-3] + tag + ".o") for s in SOURCES]
+        procs = [subprocess.Popen(["nvcc"] + NVCC_FLAGS + extra + ["-c", "-o", o, s])
+                 for s, o in zip(SOURCES, objs)]
+        try:
+            codes = [p.wait() for p in procs]
+            if any(codes):
+                raise subprocess.CalledProcessError(max(codes), "nvcc -c")
+            tmp = LIB + tag
+            subprocess.check_call(["nvcc"] + NVCC_FLAGS + ["-shared", "-o", tmp] + objs)
+            os.replace(tmp, LIB)
+        finally:
+            for o in objs:
+                if os.path.exists(o):
+                    os.remove(o)
     return LIB
 
 

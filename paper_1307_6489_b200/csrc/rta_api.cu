@@ -188,19 +188,15 @@ ChunkPlan plan_chunks(int64_t n_events, int32_t n_pixels, int32_t n_samples, siz
   return p;
 }
 
-// Core of the host-fed path. When `host_out` is set, per-chunk results are
-// written to library-owned device slots and copied back to the host arrays.
-struct HostOut {
-  int32_t* sum;
-  int32_t* start;
-  float* charge;
-  float* time;
-};
-
-int stream_impl(Workspace& w, const void* wf_host, int64_t n_events, int32_t n_pixels,
-                int32_t n_samples, const int32_t* pedestal, const float* gain, int32_t W,
-                int32_t* out_sum, int32_t* out_start, float* out_charge, float* out_time,
-                size_t chunk_bytes, cudaStream_t stream, const HostOut* host_out, int bits = 16) {
+// Core of the host-fed path: chunks of whole events go through the device
+// double buffer; `launch(dev_chunk, ev0, nev, slot)` enqueues the kernel(s) of
+// one chunk on `stream`. With out_slot_bytes != 0 the kernels write to one of
+// two library-owned device slots (`slot`, else nullptr) and
+// `back(ev0, nev, slot, back_stream)` enqueues the D2H copies of that chunk.
+template <class Launch, class Back>
+int stream_core(Workspace& w, const void* wf_host, int64_t n_events, int32_t n_pixels,
+                int32_t n_samples, size_t chunk_bytes, cudaStream_t stream, int bits,
+                size_t out_slot_bytes, Launch launch, Back back) {
   cudaError_t e;
   const ChunkPlan plan = plan_chunks(n_events, n_pixels, n_samples, chunk_bytes, bits);
   const size_t buf_bytes = ((size_t)plan.chunk_events * plan.event_bits + 7u) / 8u;
@@ -216,10 +212,10 @@ int stream_impl(Workspace& w, const void* wf_host, int64_t n_events, int32_t n_p
         [](void* p) { cudaFreeHost(p); });
     if (e != cudaSuccess) return fail_cuda(e);
   }
-  const size_t chunk_traces = (size_t)plan.chunk_events * (size_t)n_pixels;
-  if (host_out) {
+  const bool to_host = out_slot_bytes != 0;
+  if (to_host) {
     e = grow_pair(
-        w.out_buf, &w.out_cap, chunk_traces * 16u,
+        w.out_buf, &w.out_cap, out_slot_bytes,
         [](void** p, size_t n) { return cudaMalloc(p, n); }, [](void* p) { cudaFree(p); });
     if (e != cudaSuccess) return fail_cuda(e);
   }
@@ -253,54 +249,69 @@ int stream_impl(Workspace& w, const void* wf_host, int64_t n_events, int32_t n_p
     if ((e = cudaEventRecord(w.copied[b], w.copy_stream)) != cudaSuccess) return fail_cuda(e);
     if ((e = cudaStreamWaitEvent(stream, w.copied[b], 0)) != cudaSuccess) return fail_cuda(e);
 
-    const size_t t0 = (size_t)ev0 * (size_t)n_pixels;
-    const int64_t ntr = nev * (int64_t)n_pixels;
-    int32_t *o_sum, *o_start;
-    float *o_charge, *o_time;
-    if (host_out) {
-      // output slot b is free once its previous D2H has finished
-      if (w.returned_valid[b]) {
-        if ((e = cudaStreamWaitEvent(stream, w.returned[b], 0)) != cudaSuccess)
-          return fail_cuda(e);
-      }
-      uint8_t* ob = reinterpret_cast<uint8_t*>(w.out_buf[b]);
-      o_sum = reinterpret_cast<int32_t*>(ob);
-      o_start = reinterpret_cast<int32_t*>(ob + chunk_traces * 4u);
-      o_charge = reinterpret_cast<float*>(ob + chunk_traces * 8u);
-      o_time = reinterpret_cast<float*>(ob + chunk_traces * 12u);
-    } else {
-      o_sum = out_sum + t0;
-      o_start = out_start + t0;
-      o_charge = out_charge + t0;
-      o_time = out_time + t0;
+    // output slot b is free once its previous D2H has finished
+    if (to_host && w.returned_valid[b]) {
+      if ((e = cudaStreamWaitEvent(stream, w.returned[b], 0)) != cudaSuccess) return fail_cuda(e);
     }
-    e = rta_launch_extract(w.dev_buf[b], ntr, n_pixels, n_samples, pedestal, gain, W, o_sum,
-                           o_start, o_charge, o_time, stream, false, nullptr, bits);
-    if (e != cudaSuccess) return fail_cuda(e);
+    uint8_t* slot = to_host ? reinterpret_cast<uint8_t*>(w.out_buf[b]) : nullptr;
+    if ((e = launch(w.dev_buf[b], ev0, nev, slot)) != cudaSuccess) return fail_cuda(e);
     if ((e = cudaEventRecord(w.consumed[b], stream)) != cudaSuccess) return fail_cuda(e);
     w.consumed_valid[b] = true;
 
-    if (host_out) {
+    if (to_host) {
       if ((e = cudaStreamWaitEvent(w.back_stream, w.consumed[b], 0)) != cudaSuccess)
         return fail_cuda(e);
-      const size_t nb = (size_t)ntr * 4u;
-      if ((e = cudaMemcpyAsync(host_out->sum + t0, o_sum, nb, cudaMemcpyDeviceToHost,
-                               w.back_stream)) != cudaSuccess)
-        return fail_cuda(e);
-      if ((e = cudaMemcpyAsync(host_out->start + t0, o_start, nb, cudaMemcpyDeviceToHost,
-                               w.back_stream)) != cudaSuccess)
-        return fail_cuda(e);
-      if ((e = cudaMemcpyAsync(host_out->charge + t0, o_charge, nb, cudaMemcpyDeviceToHost,
-                               w.back_stream)) != cudaSuccess)
-        return fail_cuda(e);
-      if ((e = cudaMemcpyAsync(host_out->time + t0, o_time, nb, cudaMemcpyDeviceToHost,
-                               w.back_stream)) != cudaSuccess)
-        return fail_cuda(e);
+      if ((e = back(ev0, nev, slot, w.back_stream)) != cudaSuccess) return fail_cuda(e);
       if ((e = cudaEventRecord(w.returned[b], w.back_stream)) != cudaSuccess) return fail_cuda(e);
       w.returned_valid[b] = true;
     }
   }
   return RTA_OK;
+}
+
+// Per-trace extraction through stream_core. When `host_out` is set, per-chunk
+// results are written to the device slots and copied back to the host arrays.
+struct HostOut {
+  int32_t* sum;
+  int32_t* start;
+  float* charge;
+  float* time;
+};
+
+int stream_impl(Workspace& w, const void* wf_host, int64_t n_events, int32_t n_pixels,
+                int32_t n_samples, const int32_t* pedestal, const float* gain, int32_t W,
+                int32_t* out_sum, int32_t* out_start, float* out_charge, float* out_time,
+                size_t chunk_bytes, cudaStream_t stream, const HostOut* host_out, int bits = 16) {
+  const ChunkPlan plan = plan_chunks(n_events, n_pixels, n_samples, chunk_bytes, bits);
+  const size_t chunk_traces = (size_t)plan.chunk_events * (size_t)n_pixels;
+  auto launch = [&](const void* dev_chunk, int64_t ev0, int64_t nev, uint8_t* slot) {
+    const size_t t0 = (size_t)ev0 * (size_t)n_pixels;
+    int32_t *o_sum = out_sum + t0, *o_start = out_start + t0;
+    float *o_charge = out_charge + t0, *o_time = out_time + t0;
+    if (slot) {
+      o_sum = reinterpret_cast<int32_t*>(slot);
+      o_start = reinterpret_cast<int32_t*>(slot + chunk_traces * 4u);
+      o_charge = reinterpret_cast<float*>(slot + chunk_traces * 8u);
+      o_time = reinterpret_cast<float*>(slot + chunk_traces * 12u);
+    }
+    return rta_launch_extract(dev_chunk, nev * (int64_t)n_pixels, n_pixels, n_samples, pedestal,
+                              gain, W, o_sum, o_start, o_charge, o_time, stream, false, nullptr,
+                              bits);
+  };
+  auto back = [&](int64_t ev0, int64_t nev, uint8_t* slot, cudaStream_t bs) {
+    const size_t t0 = (size_t)ev0 * (size_t)n_pixels;
+    const size_t nb = (size_t)nev * (size_t)n_pixels * 4u;
+    void* dst[4] = {host_out->sum + t0, host_out->start + t0, host_out->charge + t0,
+                    host_out->time + t0};
+    for (int i = 0; i < 4; ++i) {
+      const cudaError_t e = cudaMemcpyAsync(dst[i], slot + chunk_traces * 4u * (size_t)i, nb,
+                                            cudaMemcpyDeviceToHost, bs);
+      if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+  };
+  return stream_core(w, wf_host, n_events, n_pixels, n_samples, chunk_bytes, stream, bits,
+                     host_out ? chunk_traces * 16u : 0u, launch, back);
 }
 
 // Host-to-host path (rta_extract_host, rta_extract_host_packed12): calibration
@@ -349,6 +360,83 @@ int host_impl(const void* wf_host, int64_t n_events, int32_t n_pixels, int32_t n
   if (e2 != cudaSuccess) return fail_cuda(e2);
   if (e3 != cudaSuccess) return fail_cuda(e3);
   return RTA_OK;
+}
+
+// ---- image cleaning + moments (NEXT-4; readings R31-R35) ----------
+int validate_image(int64_t n_events, int32_t n_pixels, const void* pix_x, const void* pix_y,
+                   const void* neighbors, const void* out_n_pix, const void* out_params,
+                   const void* out_mask) {
+  (void)out_mask;  // optional, bytes: no alignment requirement
+  if (n_events < 0 || n_pixels < 1) return RTA_ERR_SHAPE;
+  if (n_events * (int64_t)n_pixels >= (1ll << 31)) return RTA_ERR_UNSUPPORTED;
+  if (n_pixels > rta_image_pixel_limit()) return RTA_ERR_UNSUPPORTED;
+  if (n_events == 0) return RTA_OK;
+  if (!pix_x || !pix_y || !neighbors || !out_n_pix || !out_params) return RTA_ERR_NULL;
+  if (((uintptr_t)pix_x | (uintptr_t)pix_y | (uintptr_t)neighbors | (uintptr_t)out_n_pix |
+       (uintptr_t)out_params) % 4 != 0)
+    return RTA_ERR_ALIGN;
+  return RTA_OK;
+}
+
+// extraction-side checks of the fused calls (no per-trace outputs to check)
+int validate_fused(const void* wf, int64_t n_events, int32_t n_pixels, int32_t n_samples,
+                   const void* pedestal, const void* gain, int32_t W) {
+  if (n_events < 0 || n_pixels < 1 || n_samples < 1 || W < 1 || W > n_samples)
+    return RTA_ERR_SHAPE;
+  if (n_events * (int64_t)n_pixels >= (1ll << 31)) return RTA_ERR_UNSUPPORTED;
+  if ((int64_t)n_samples * (int64_t)W * 65535ll >= (1ll << 31)) return RTA_ERR_UNSUPPORTED;
+  if (n_events == 0) return RTA_OK;
+  if (!wf || !pedestal || !gain) return RTA_ERR_NULL;
+  if ((uintptr_t)wf % 2 != 0) return RTA_ERR_ALIGN;
+  if (((uintptr_t)pedestal | (uintptr_t)gain) % 4 != 0) return RTA_ERR_ALIGN;
+  return RTA_OK;
+}
+
+// Host-fed fused path: waveform chunks in, event parameters out. `host_out`
+// set: results go through the device slots back to host arrays.
+struct ImageHostOut {
+  int32_t* n_pix;
+  float* params;
+  uint8_t* mask;
+};
+
+int image_stream_impl(Workspace& w, const void* wf_host, int64_t n_events, int32_t n_pixels,
+                      int32_t n_samples, const int32_t* pedestal, const float* gain, int32_t W,
+                      const RtaCamera& cam, const RtaImageOut& out, size_t chunk_bytes,
+                      cudaStream_t stream, const ImageHostOut* host_out) {
+  const ChunkPlan plan = plan_chunks(n_events, n_pixels, n_samples, chunk_bytes, 16);
+  const size_t ce = (size_t)plan.chunk_events;
+  const bool want_mask = host_out ? host_out->mask != nullptr : out.mask != nullptr;
+  // slot layout: params [ce][8] float, n_pix [ce] int32, mask [ce][P] bytes
+  const size_t slot_bytes = ce * 36u + (want_mask ? ce * (size_t)n_pixels : 0u);
+  auto launch = [&](const void* dev_chunk, int64_t ev0, int64_t nev, uint8_t* slot) {
+    RtaImageOut o;
+    if (slot) {
+      o.params = reinterpret_cast<float*>(slot);
+      o.n_pix = reinterpret_cast<int32_t*>(slot + ce * 32u);
+      o.mask = want_mask ? slot + ce * 36u : nullptr;
+    } else {
+      o.n_pix = out.n_pix + ev0;
+      o.params = out.params + (size_t)ev0 * 8u;
+      o.mask = out.mask ? out.mask + (size_t)ev0 * (size_t)n_pixels : nullptr;
+    }
+    return rta_launch_extract_image(dev_chunk, nev, n_pixels, n_samples, pedestal, gain, W, cam,
+                                    o, stream, false);
+  };
+  auto back = [&](int64_t ev0, int64_t nev, uint8_t* slot, cudaStream_t bs) {
+    cudaError_t e = cudaMemcpyAsync(host_out->params + (size_t)ev0 * 8u, slot,
+                                    (size_t)nev * 32u, cudaMemcpyDeviceToHost, bs);
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpyAsync(host_out->n_pix + ev0, slot + ce * 32u, (size_t)nev * 4u,
+                        cudaMemcpyDeviceToHost, bs);
+    if (e != cudaSuccess) return e;
+    if (want_mask)
+      e = cudaMemcpyAsync(host_out->mask + (size_t)ev0 * (size_t)n_pixels, slot + ce * 36u,
+                          (size_t)nev * (size_t)n_pixels, cudaMemcpyDeviceToHost, bs);
+    return e;
+  };
+  return stream_core(w, wf_host, n_events, n_pixels, n_samples, chunk_bytes, stream, 16,
+                     host_out ? slot_bytes : 0u, launch, back);
 }
 
 }  // namespace
@@ -649,6 +737,143 @@ void rta_ragged_plan_destroy(rta_ragged_plan* plan) {
     cudaGetLastError();
   }
   delete plan;
+}
+
+// ---- image cleaning + moments (NEXT-4) ----------------------------------------
+int rta_image_moments(const float* charge, const float* time, int64_t n_events,
+                      int32_t n_pixels, const float* pix_x, const float* pix_y,
+                      const int32_t* neighbors, float thr_picture, float thr_boundary,
+                      int32_t* out_n_pix, float* out_params, uint8_t* out_mask, void* stream) {
+  const int v = validate_image(n_events, n_pixels, pix_x, pix_y, neighbors, out_n_pix, out_params,
+                               out_mask);
+  if (v != RTA_OK || n_events == 0) return v;
+  if (!charge || !time) return RTA_ERR_NULL;
+  if (((uintptr_t)charge | (uintptr_t)time) % 4 != 0) return RTA_ERR_ALIGN;
+  const RtaCamera cam{pix_x, pix_y, neighbors, thr_picture, thr_boundary};
+  const RtaImageOut out{out_n_pix, out_params, out_mask};
+  const cudaError_t e = rta_launch_image_moments(charge, time, n_events, n_pixels, cam, out,
+                                                 (cudaStream_t)stream);
+  return e == cudaSuccess ? RTA_OK : fail_cuda(e);
+}
+
+static int extract_image_common(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
+                                int32_t n_samples, const int32_t* pedestal, const float* gain,
+                                int32_t W, const float* pix_x, const float* pix_y,
+                                const int32_t* neighbors, float thr_picture, float thr_boundary,
+                                int32_t* out_n_pix, float* out_params, uint8_t* out_mask,
+                                void* stream, bool force_generic) {
+  int v = validate_fused(wf, n_events, n_pixels, n_samples, pedestal, gain, W);
+  if (v != RTA_OK) return v;
+  v = validate_image(n_events, n_pixels, pix_x, pix_y, neighbors, out_n_pix, out_params, out_mask);
+  if (v != RTA_OK || n_events == 0) return v;
+  const RtaCamera cam{pix_x, pix_y, neighbors, thr_picture, thr_boundary};
+  const RtaImageOut out{out_n_pix, out_params, out_mask};
+  const cudaError_t e = rta_launch_extract_image(wf, n_events, n_pixels, n_samples, pedestal, gain,
+                                                 W, cam, out, (cudaStream_t)stream, force_generic);
+  return e == cudaSuccess ? RTA_OK : fail_cuda(e);
+}
+
+int rta_extract_image(const uint16_t* wf, int64_t n_events, int32_t n_pixels, int32_t n_samples,
+                      const int32_t* pedestal, const float* gain, int32_t W, const float* pix_x,
+                      const float* pix_y, const int32_t* neighbors, float thr_picture,
+                      float thr_boundary, int32_t* out_n_pix, float* out_params,
+                      uint8_t* out_mask, void* stream) {
+  return extract_image_common(wf, n_events, n_pixels, n_samples, pedestal, gain, W, pix_x, pix_y,
+                              neighbors, thr_picture, thr_boundary, out_n_pix, out_params,
+                              out_mask, stream, false);
+}
+
+// Same through the generic fused kernel. Exported for the tests; not in the public header.
+int rta_extract_image_generic(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
+                              int32_t n_samples, const int32_t* pedestal, const float* gain,
+                              int32_t W, const float* pix_x, const float* pix_y,
+                              const int32_t* neighbors, float thr_picture, float thr_boundary,
+                              int32_t* out_n_pix, float* out_params, uint8_t* out_mask,
+                              void* stream) {
+  return extract_image_common(wf, n_events, n_pixels, n_samples, pedestal, gain, W, pix_x, pix_y,
+                              neighbors, thr_picture, thr_boundary, out_n_pix, out_params,
+                              out_mask, stream, true);
+}
+
+int rta_extract_image_stream(const uint16_t* wf_host, int64_t n_events, int32_t n_pixels,
+                             int32_t n_samples, const int32_t* pedestal, const float* gain,
+                             int32_t W, const float* pix_x, const float* pix_y,
+                             const int32_t* neighbors, float thr_picture, float thr_boundary,
+                             int32_t* out_n_pix, float* out_params, uint8_t* out_mask,
+                             size_t chunk_bytes, void* stream) {
+  int v = validate_fused(wf_host, n_events, n_pixels, n_samples, pedestal, gain, W);
+  if (v != RTA_OK) return v;
+  v = validate_image(n_events, n_pixels, pix_x, pix_y, neighbors, out_n_pix, out_params, out_mask);
+  if (v != RTA_OK || n_events == 0) return v;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  cudaError_t e = ws_prepare(g_ws);
+  if (e != cudaSuccess) return fail_cuda(e);
+  const RtaCamera cam{pix_x, pix_y, neighbors, thr_picture, thr_boundary};
+  const RtaImageOut out{out_n_pix, out_params, out_mask};
+  return image_stream_impl(g_ws, wf_host, n_events, n_pixels, n_samples, pedestal, gain, W, cam,
+                           out, chunk_bytes, (cudaStream_t)stream, nullptr);
+}
+
+int rta_extract_image_host(const uint16_t* wf_host, int64_t n_events, int32_t n_pixels,
+                           int32_t n_samples, const int32_t* pedestal_host,
+                           const float* gain_host, int32_t W, const float* pix_x_host,
+                           const float* pix_y_host, const int32_t* neighbors_host,
+                           float thr_picture, float thr_boundary, int32_t* out_n_pix_host,
+                           float* out_params_host, uint8_t* out_mask_host, size_t chunk_bytes) {
+  int v = validate_fused(wf_host, n_events, n_pixels, n_samples, pedestal_host, gain_host, W);
+  if (v != RTA_OK) return v;
+  v = validate_image(n_events, n_pixels, pix_x_host, pix_y_host, neighbors_host, out_n_pix_host,
+                     out_params_host, out_mask_host);
+  if (v != RTA_OK || n_events == 0) return v;
+  std::lock_guard<std::mutex> lock(g_ws.mu);
+  Workspace& w = g_ws;
+  cudaError_t e = ws_prepare(w);
+  if (e != cudaSuccess) return fail_cuda(e);
+  // pedestal, gain, pix_x, pix_y: 4 bytes per pixel each; neighbours: 24
+  const size_t P = (size_t)n_pixels, calib_bytes = P * 40u;
+  if (w.calib_cap < calib_bytes) {
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail_cuda(e);
+    if (w.calib_buf) cudaFree(w.calib_buf);
+    w.calib_buf = nullptr;
+    w.calib_cap = 0;
+    if ((e = cudaMalloc(&w.calib_buf, calib_bytes)) != cudaSuccess) return fail_cuda(e);
+    w.calib_cap = calib_bytes;
+  }
+  uint8_t* cb = reinterpret_cast<uint8_t*>(w.calib_buf);
+  const void* src[5] = {pedestal_host, gain_host, pix_x_host, pix_y_host, neighbors_host};
+  const size_t off[5] = {0, P * 4u, P * 8u, P * 12u, P * 16u};
+  const size_t len[5] = {P * 4u, P * 4u, P * 4u, P * 4u, P * 24u};
+  // the tables may still be read by kernels of an earlier call
+  if ((e = cudaStreamSynchronize(w.host_stream)) != cudaSuccess) return fail_cuda(e);
+  for (int i = 0; i < 5; ++i) {
+    if ((e = cudaMemcpyAsync(cb + off[i], src[i], len[i], cudaMemcpyHostToDevice,
+                             w.host_stream)) != cudaSuccess)
+      return fail_cuda(e);
+  }
+  const RtaCamera cam{reinterpret_cast<const float*>(cb + off[2]),
+                      reinterpret_cast<const float*>(cb + off[3]),
+                      reinterpret_cast<const int32_t*>(cb + off[4]), thr_picture, thr_boundary};
+  const RtaImageOut none{nullptr, nullptr, nullptr};
+  const ImageHostOut ho{out_n_pix_host, out_params_host, out_mask_host};
+  const int rc = image_stream_impl(w, wf_host, n_events, n_pixels, n_samples,
+                                   reinterpret_cast<const int32_t*>(cb + off[0]),
+                                   reinterpret_cast<const float*>(cb + off[1]), W, cam, none,
+                                   chunk_bytes, w.host_stream, &ho);
+  // synchronous by contract, also on the error path (nothing may outlive the call)
+  cudaError_t e1 = cudaStreamSynchronize(w.host_stream);
+  cudaError_t e2 = cudaStreamSynchronize(w.back_stream);
+  cudaError_t e3 = cudaStreamSynchronize(w.copy_stream);
+  if (rc != RTA_OK) return rc;
+  if (e1 != cudaSuccess) return fail_cuda(e1);
+  if (e2 != cudaSuccess) return fail_cuda(e2);
+  if (e3 != cudaSuccess) return fail_cuda(e3);
+  return RTA_OK;
+}
+
+int32_t rta_image_max_pixels(void) { return rta_image_pixel_limit(); }
+
+const char* rta_image_kernel_name(int32_t n_pixels, int32_t n_samples, int32_t W, int aligned16) {
+  return rta_pick_image_kernel_name(n_pixels, n_samples, W, aligned16 != 0);
 }
 
 const char* rta_strerror(int status) {

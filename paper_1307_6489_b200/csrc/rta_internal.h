@@ -52,6 +52,37 @@ void rta_count_launch();
 // round-robin (tests compare the two). rta_sched_release frees the per-stream
 // scheduler words (rta_shutdown).
 void rta_set_static_schedule(bool on);
+bool rta_static_schedule();
 void rta_sched_release();
+// {next work item, CTAs done} pair owned by (device, stream), zero between
+// launches; nullptr = none available (use the static round-robin).
+uint32_t* rta_sched_words(int dev, cudaStream_t stream);
+cudaError_t rta_device_sms(int dev, int* sms);
+
+// Image cleaning + moments (include/rta.h rta_image_moments, rta_extract_image;
+// DESIGN.md readings R31-R35). Device pointers, already validated.
+struct RtaCamera {
+  const float* pix_x;        // [n_pixels]
+  const float* pix_y;        // [n_pixels]
+  const int32_t* neighbors;  // [n_pixels][6], -1 (or any index outside [0, n_pixels)) = none
+  float thr_picture, thr_boundary;
+};
+struct RtaImageOut {
+  int32_t* n_pix;   // [n_events]
+  float* params;    // [n_events][8]
+  uint8_t* mask;    // [n_events][n_pixels] or nullptr
+};
+cudaError_t rta_launch_image_moments(const float* charge, const float* time, int64_t n_events,
+                                     int32_t n_pixels, const RtaCamera& cam,
+                                     const RtaImageOut& out, cudaStream_t stream);
+// Extraction fused with cleaning + moments: per-trace results stay in shared memory.
+cudaError_t rta_launch_extract_image(const void* wf, int64_t n_events, int32_t n_pixels,
+                                     int32_t n_samples, const int32_t* pedestal,
+                                     const float* gain, int32_t W, const RtaCamera& cam,
+                                     const RtaImageOut& out, cudaStream_t stream,
+                                     bool force_generic);
+int32_t rta_image_pixel_limit();  // charge, time and flags of one event must fit one CTA
+const char* rta_pick_image_kernel_name(int32_t n_pixels, int32_t n_samples, int32_t W,
+                                       bool aligned16);
 
 #endif

@@ -1,0 +1,386 @@
+"""GPU parity of image cleaning + moments (DESIGN.md
+readings R31-R35) against oracle/rta_oracle_image.cpp, through the C ABI:
+rta_image_moments on device charge / time arrays, and rta_extract_image (the
+extraction and the cleaning in one kernel) against oracle.extract followed by
+oracle.image_moments. n_pix, mask and q_max bit-exact; the fp32 parameters
+within the tolerances of tests/_image.py::assert_image_parity."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import dl0gen
+import oracle
+from tests._image import F32, assert_image_parity, blob_images
+
+pytestmark = pytest.mark.gpu
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "image7.json")
+
+
+def dev(a, dtype=None):
+    import torch
+    a = np.ascontiguousarray(a, dtype)
+    if a.dtype == np.uint16:
+        a = a.view(np.int16)
+    return torch.from_numpy(a).cuda()
+
+
+def image_outputs(E, P, mask=True):
+    import torch
+    return (torch.full((E,), -7, dtype=torch.int32, device="cuda"),
+            torch.full((E, 8), -7.0, dtype=torch.float32, device="cuda"),
+            torch.full((E, P), 9, dtype=torch.uint8, device="cuda") if mask else None)
+
+
+def host(outs):
+    import torch
+    torch.cuda.synchronize()
+    return tuple(None if o is None else o.cpu().numpy() for o in outs)
+
+
+def gpu_moments(q, t, x, y, nbr, tp, tb, mask=True):
+    import paper_1307_6489_b200 as rta
+    E, P = q.shape
+    outs = image_outputs(E, P, mask)
+    rta.rta_image_moments(dev(q, F32), dev(t, F32), E, P, dev(x, F32), dev(y, F32),
+                          dev(nbr, np.int32), tp, tb, *outs)
+    return host(outs)
+
+
+def gpu_extract_image(wf, ped, gain, W, x, y, nbr, tp, tb, mask=True, generic=False, d_wf=None):
+    import paper_1307_6489_b200 as rta
+    E, P, S = wf.shape
+    outs = image_outputs(E, P, mask)
+    rta.rta_extract_image(dev(wf) if d_wf is None else d_wf, E, P, S, dev(ped, np.int32),
+                          dev(gain, F32), W, dev(x, F32), dev(y, F32), dev(nbr, np.int32),
+                          tp, tb, *outs, generic=generic)
+    return host(outs)
+
+
+def oracle_extract_image(wf, ped, gain, W, x, y, nbr, tp, tb):
+    E, P, _ = wf.shape
+    _, _, q, t = oracle.extract(wf, ped, gain, W)
+    return oracle.image_moments(q.reshape(E, P), t.reshape(E, P), x, y, nbr, tp, tb)
+
+
+# ---------------------------------------------------------------- rta_image_moments
+def test_hand_worked_camera_on_the_device():
+    g = json.load(open(GOLD))
+    q = np.array([[float(v) for v in ev["charge"]] for ev in g["events"]], F32)
+    t = np.array([ev["time"] for ev in g["events"]], F32)
+    x, y, nbr = np.array(g["pix_x"], F32), np.array(g["pix_y"], F32), np.array(g["neighbors"], np.int32)
+    got = gpu_moments(q, t, x, y, nbr, g["thr_picture"], g["thr_boundary"])
+    for i, ev in enumerate(g["events"]):
+        assert got[2][i].tolist() == ev["mask"], ev["name"]
+        assert got[0][i] == ev["n_pix"]
+    assert_image_parity(got, oracle.image_moments(q, t, x, y, nbr, g["thr_picture"], g["thr_boundary"]),
+                        x, y, "image7")
+
+
+@pytest.mark.parametrize("P,E,seed", [(1855, 70, 0), (1764, 33, 1), (2048, 40, 3), (37, 300, 2),
+                                      (7, 50, 4), (1, 5, 5), (255, 64, 6), (257, 64, 7),
+                                      (5000, 12, 8), (11328, 6, 9)])
+def test_blob_images(P, E, seed):
+    q, t, x, y, nbr = blob_images(E, P, seed)
+    got = gpu_moments(q, t, x, y, nbr, 8.0, 4.0)
+    want = oracle.image_moments(q, t, x, y, nbr, 8.0, 4.0)
+    n_axis = assert_image_parity(got, want, x, y, "blobs P=%d" % P)
+    if P >= 37:
+        assert want[0].max() > 5 and n_axis > 0
+    # without the mask output: same parameters, bit for bit
+    got2 = gpu_moments(q, t, x, y, nbr, 8.0, 4.0, mask=False)
+    assert np.array_equal(got2[0], got[0]) and np.array_equal(got2[1].view(np.int32), got[1].view(np.int32))
+
+
+def test_thresholds_and_special_values():
+    q, t, x, y, nbr = blob_images(24, 469, 11)
+    q[3, :] = np.nan                       # NaN never passes a threshold
+    q[4, 10:40] = np.nan
+    q[5, :] = -3.0                         # everything passes negative thresholds, size < 0 -> zeros
+    q[6, :] = 20.0                         # every pixel is core
+    q[7, :] = 0.0
+    q[8, 100] = np.inf                     # an isolated infinite pixel is dropped
+    for tp, tb in ((8.0, 4.0), (4.0, 8.0), (-5.0, -5.0), (1e9, 1.0), (8.0, -1e9),
+                   (float("nan"), 1.0), (8.0, float("nan")), (8.0, 8.0)):
+        got = gpu_moments(q, t, x, y, nbr, tp, tb)
+        want = oracle.image_moments(q, t, x, y, nbr, tp, tb)
+        assert_image_parity(got, want, x, y, "thr %r %r" % (tp, tb))
+    assert want[0][6] == 469
+
+
+def test_neighbour_table_is_used_as_given():
+    """Out-of-range entries mean 'none'; self references, duplicates and a
+    one-directional table follow the definition, not a symmetrised version."""
+    rng = np.random.default_rng(5)
+    P = 300
+    q, t, x, y, _ = blob_images(40, P, 12)
+    nbr = rng.integers(-50, P + 50, (P, 6)).astype(np.int32)
+    nbr[::7, 0] = np.arange(P)[::7]        # self neighbours
+    nbr[5] = [2**31 - 1, -2**31, P, -1, 6, 6]
+    got = gpu_moments(q, t, x, y, nbr, 3.0, 1.0)
+    want = oracle.image_moments(q, t, x, y, nbr, 3.0, 1.0)
+    assert want[0].max() > 3
+    assert_image_parity(got, want, x, y, "random table")
+
+
+def test_unaligned_rows_and_outputs():
+    """P % 4 != 0 makes most event rows 4-byte aligned only; odd output addresses."""
+    import torch
+    import paper_1307_6489_b200 as rta
+    q, t, x, y, nbr = blob_images(9, 1855, 13)
+    E, P = q.shape
+    dq = torch.empty(E * P + 1, dtype=torch.float32, device="cuda")[1:]
+    dt = torch.empty(E * P + 3, dtype=torch.float32, device="cuda")[3:]
+    dq.copy_(torch.from_numpy(q).reshape(-1))
+    dt.copy_(torch.from_numpy(t).reshape(-1))
+    n = torch.empty(E + 1, dtype=torch.int32, device="cuda")[1:]
+    par = torch.empty(E * 8 + 1, dtype=torch.float32, device="cuda")[1:]
+    m = torch.empty(E * P + 1, dtype=torch.uint8, device="cuda")[1:]
+    rta.rta_image_moments(dq, dt, E, P, dev(x), dev(y), dev(nbr), 8.0, 4.0, n, par, m)
+    got = host((n, par.reshape(E, 8), m.reshape(E, P)))
+    assert_image_parity(got, oracle.image_moments(q, t, x, y, nbr, 8.0, 4.0), x, y, "unaligned")
+
+
+def test_image_moments_errors():
+    import torch
+    import paper_1307_6489_b200 as rta
+    q, t, x, y, nbr = blob_images(2, 37, 1)
+    a = dict(charge=dev(q), time=dev(t), x=dev(x), y=dev(y), nbr=dev(nbr))
+    n, par, m = image_outputs(2, 37)
+
+    def call(**kw):
+        args = dict(charge=a["charge"], time=a["time"], E=2, P=37, x=a["x"], y=a["y"], nbr=a["nbr"],
+                    n=n, par=par, m=m)
+        args.update(kw)
+        rta.rta_image_moments(args["charge"], args["time"], args["E"], args["P"], args["x"], args["y"],
+                              args["nbr"], 8.0, 4.0, args["n"], args["par"], args["m"])
+    for kw, status in ((dict(charge=None), rta.RTA_ERR_NULL), (dict(x=None), rta.RTA_ERR_NULL),
+                       (dict(nbr=None), rta.RTA_ERR_NULL), (dict(n=None), rta.RTA_ERR_NULL),
+                       (dict(par=None), rta.RTA_ERR_NULL), (dict(E=-1), rta.RTA_ERR_SHAPE),
+                       (dict(P=0), rta.RTA_ERR_SHAPE),
+                       (dict(P=rta.rta_image_max_pixels() + 1), rta.RTA_ERR_UNSUPPORTED),
+                       (dict(charge=a["charge"].data_ptr() + 2), rta.RTA_ERR_ALIGN)):
+        with pytest.raises(rta.RtaError) as ei:
+            call(**kw)
+        assert ei.value.status == status, kw
+    torch.cuda.synchronize()
+    assert (n.cpu() == -7).all() and (par.cpu() == -7).all()    # nothing was enqueued
+    call(E=0, charge=None, x=None, n=None, par=None)             # empty input: ok, nothing touched
+    call(m=None)
+    torch.cuda.synchronize()
+    assert (m.cpu() == 9).all()
+
+
+def test_largest_camera():
+    import paper_1307_6489_b200 as rta
+    P = rta.rta_image_max_pixels()
+    q, t, x, y, nbr = blob_images(3, P, 21)
+    assert_image_parity(gpu_moments(q, t, x, y, nbr, 8.0, 4.0),
+                        oracle.image_moments(q, t, x, y, nbr, 8.0, 4.0), x, y, "P max")
+
+
+# ---------------------------------------------------------------- rta_extract_image
+def config_batch(name, n_events, first=0):
+    cfg = dl0gen.CONFIGS[name]
+    ped, gain = dl0gen.calib(cfg)
+    wf = dl0gen.events_cpu(cfg, first, n_events, threads=8)
+    x, y, nbr = dl0gen.hex_camera(cfg.n_pixels)
+    tp, tb = dl0gen.IMAGE_THRESHOLDS[name]
+    return cfg, wf, ped, gain, x, y, nbr, tp, tb
+
+
+@pytest.mark.parametrize("name,n_events", [("C1", 64), ("C2", 150), ("C3", 201), ("C4", 37)])
+def test_fused_on_the_config_shapes(name, n_events):
+    import paper_1307_6489_b200 as rta
+    cfg, wf, ped, gain, x, y, nbr, tp, tb = config_batch(name, n_events)
+    assert rta.rta_image_kernel_name(cfg.n_pixels, cfg.n_samples, cfg.W).startswith("image_tile")
+    want = oracle_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb)
+    assert (want[0] > 0).sum() > n_events // 2
+    got = gpu_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb)
+    assert_image_parity(got, want, x, y, name + " staged")
+    gen = gpu_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb, generic=True)
+    assert_image_parity(gen, want, x, y, name + " generic")
+    # the two device paths run the same cleaning code on the same charges: bit-identical
+    for a, b in zip(got, gen):
+        assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
+    rta.rta_debug_static_schedule(True)
+    try:
+        st = gpu_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb)
+    finally:
+        rta.rta_debug_static_schedule(False)
+    for a, b in zip(got, st):
+        assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4"])
+def test_fused_equals_extract_then_moments(name):
+    """rta_extract_image == rta_extract followed by rta_image_moments, bit for bit."""
+    import paper_1307_6489_b200 as rta
+    from tests._gpu import alloc_outputs
+    cfg, wf, ped, gain, x, y, nbr, tp, tb = config_batch(name, 48, first=100)
+    E, P, S = wf.shape
+    d_wf, d_ped, d_gain = dev(wf), dev(ped, np.int32), dev(gain, F32)
+    outs = alloc_outputs(E * P)
+    rta.rta_extract(d_wf, E, P, S, d_ped, d_gain, cfg.W, *outs)
+    two = image_outputs(E, P)
+    rta.rta_image_moments(outs[2], outs[3], E, P, dev(x), dev(y), dev(nbr), tp, tb, *two)
+    one = gpu_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb)
+    for a, b in zip(one, host(two)):
+        assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
+
+
+@pytest.mark.parametrize("S,W,P,E", [
+    (40, 7, 1, 50), (40, 7, 255, 40), (40, 7, 256, 40), (40, 7, 257, 40), (40, 7, 512, 20),
+    (40, 7, 3000, 9),                       # staged, tiles per event 1 .. 12
+    (30, 7, 333, 31), (30, 7, 2, 100),      # 60-byte traces: events 4-byte aligned only
+    (25, 4, 1764, 21), (25, 4, 510, 33), (25, 4, 2, 64),   # two traces per thread, 8-byte phases
+    (25, 4, 1765, 11),                      # odd camera -> generic
+    (128, 8, 2048, 9), (128, 8, 63, 40), (128, 8, 65, 40),
+    (33, 5, 400, 20), (16, 16, 100, 20), (7, 1, 1855, 10),  # no specialisation -> generic
+])
+def test_fused_shapes_and_event_phases(S, W, P, E):
+    rng = np.random.default_rng(S * 1000 + P)
+    x, y, nbr = dl0gen.hex_camera(P)
+    ped = rng.integers(380, 421, P).astype(np.int32)
+    gain = rng.uniform(0.9, 1.1, P).astype(F32)
+    wf = (400 + rng.normal(0, 4, (E, P, S))).round().clip(0, 4095).astype(np.uint16)
+    # pulses on clusters of neighbouring pixels so that the cleaning keeps something
+    for e in range(E):
+        p = int(rng.integers(0, P))
+        for n in [p] + [int(v) for v in nbr[p] if v >= 0]:
+            wf[e, n, S // 2: S // 2 + max(1, W // 2)] += np.uint16(rng.integers(20, 200))
+    want = oracle_extract_image(wf, ped, gain, W, x, y, nbr, 60.0, 30.0)
+    if P > 1:
+        assert (want[0] > 0).any()
+    got = gpu_extract_image(wf, ped, gain, W, x, y, nbr, 60.0, 30.0)
+    assert_image_parity(got, want, x, y, "S=%d P=%d" % (S, P))
+
+
+def test_fused_unaligned_waveforms_take_the_generic_kernel():
+    import torch
+    cfg, wf, ped, gain, x, y, nbr, tp, tb = config_batch("C2", 20)
+    want = oracle_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb)
+    for off in (1, 3, 4):   # halfwords
+        buf = torch.empty(wf.size + 8, dtype=torch.int16, device="cuda")
+        d_wf = buf[off: off + wf.size]
+        d_wf.copy_(torch.from_numpy(wf.view(np.int16)).reshape(-1))
+        got = gpu_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb, d_wf=d_wf)
+        assert_image_parity(got, want, x, y, "offset %d" % off)
+
+
+def test_fused_last_event_tail_is_not_overread():
+    """C1: 111 300 bytes per event, so the last tile of the last event ends 12
+    bytes past a 16-byte boundary; the buffer ends exactly there, followed by a
+    guard the kernel must not need (values differ, results must not)."""
+    import torch
+    cfg, wf, ped, gain, x, y, nbr, tp, tb = config_batch("C1", 5)
+    want = oracle_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb)
+    n = wf.size
+    for guard in (0, -1):
+        buf = torch.full((n + 64,), guard, dtype=torch.int16, device="cuda")
+        buf[:n].copy_(torch.from_numpy(wf.view(np.int16)).reshape(-1))
+        got = gpu_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb, d_wf=buf[:n])
+        assert_image_parity(got, want, x, y, "tail")
+
+
+def test_fused_full_uint16_range_and_extreme_calibration():
+    rng = np.random.default_rng(77)
+    E, P, S, W = 12, 700, 40, 7
+    x, y, nbr = dl0gen.hex_camera(P)
+    wf = rng.integers(0, 65536, (E, P, S)).astype(np.uint16)
+    ped = rng.integers(-2**20, 2**20, P).astype(np.int32)
+    gain = rng.uniform(-2, 2, P).astype(F32)
+    gain[::50] = np.nan
+    gain[1::50] = np.inf
+    want = oracle_extract_image(wf, ped, gain, W, x, y, nbr, 1e5, 1e4)
+    got = gpu_extract_image(wf, ped, gain, W, x, y, nbr, 1e5, 1e4)
+    # (+inf charges make size infinite and the ratios NaN on both sides: assert_image_parity)
+    assert_image_parity(got, want, x, y, "extreme")
+
+
+def test_fused_errors():
+    import paper_1307_6489_b200 as rta
+    cfg, wf, ped, gain, x, y, nbr, tp, tb = config_batch("C1", 2)
+    E, P, S = wf.shape
+    d = dict(wf=dev(wf), ped=dev(ped, np.int32), gain=dev(gain, F32), x=dev(x), y=dev(y), nbr=dev(nbr))
+    n, par, m = image_outputs(E, P)
+
+    def call(**kw):
+        a = dict(d, E=E, P=P, S=S, W=cfg.W, n=n, par=par, m=m)
+        a.update(kw)
+        rta.rta_extract_image(a["wf"], a["E"], a["P"], a["S"], a["ped"], a["gain"], a["W"], a["x"],
+                              a["y"], a["nbr"], tp, tb, a["n"], a["par"], a["m"])
+    for kw, status in ((dict(wf=None), rta.RTA_ERR_NULL), (dict(ped=None), rta.RTA_ERR_NULL),
+                       (dict(nbr=None), rta.RTA_ERR_NULL), (dict(par=None), rta.RTA_ERR_NULL),
+                       (dict(W=0), rta.RTA_ERR_SHAPE), (dict(W=S + 1), rta.RTA_ERR_SHAPE),
+                       (dict(E=-2), rta.RTA_ERR_SHAPE), (dict(S=40000, W=1), rta.RTA_ERR_UNSUPPORTED),
+                       (dict(P=rta.rta_image_max_pixels() + 1), rta.RTA_ERR_UNSUPPORTED),
+                       (dict(wf=d["wf"].data_ptr() + 1), rta.RTA_ERR_ALIGN)):
+        with pytest.raises(rta.RtaError) as ei:
+            call(**kw)
+        assert ei.value.status == status, kw
+    call(E=0, wf=None)
+
+
+# ------------------------------------------------------------ host-fed variants
+def test_stream_and_host_variants_match_the_device_call():
+    import torch
+    import paper_1307_6489_b200 as rta
+    cfg, wf, ped, gain, x, y, nbr, tp, tb = config_batch("C2", 100)
+    E, P, S = wf.shape
+    ref = gpu_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb)
+    ev_bytes = P * S * 2
+    pinned = torch.from_numpy(wf.view(np.int16)).pin_memory()
+    for src in (pinned, wf):                                    # pinned and pageable sources
+        for chunk in (0, 7 * ev_bytes + 5, ev_bytes, 64 * ev_bytes):
+            for want_mask in (True, False):
+                outs = image_outputs(E, P, want_mask)
+                rta.rta_extract_image_stream(src, E, P, S, dev(ped, np.int32), dev(gain, F32), cfg.W,
+                                             dev(x), dev(y), dev(nbr), tp, tb, *outs, chunk_bytes=chunk)
+                got = host(outs)
+                for a, b in zip(got, ref):
+                    if a is not None:
+                        assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
+    for chunk in (0, 9 * ev_bytes):
+        for want_mask in (True, False):
+            n = np.full(E, -7, np.int32)
+            par = np.full((E, 8), -7, F32)
+            m = np.full((E, P), 9, np.uint8) if want_mask else None
+            rta.rta_extract_image_host(wf, E, P, S, ped, gain, cfg.W, x, y, nbr, tp, tb, n, par, m,
+                                       chunk_bytes=chunk)
+            assert np.array_equal(n, ref[0]) and np.array_equal(par.view(np.int32), ref[1].view(np.int32))
+            if want_mask:
+                assert np.array_equal(m, ref[2])
+    rta.rta_shutdown()
+
+
+# ------------------------------------------------------ bench-sized, sampled events
+@pytest.mark.parametrize("name", ["C2", "C3", "C4"])
+def test_fused_at_full_size_sampled_events(name):
+    """BASELINE.json configs at full size, generated on the device; the oracle
+    checks event blocks regenerated on the host (same bytes: tests/test_dl0gen.py)."""
+    import torch
+    import paper_1307_6489_b200 as rta
+    cfg = dl0gen.CONFIGS[name]
+    ped, gain = dl0gen.calib(cfg)
+    x, y, nbr = dl0gen.hex_camera(cfg.n_pixels)
+    tp, tb = dl0gen.IMAGE_THRESHOLDS[name]
+    E, P, S = cfg.n_events, cfg.n_pixels, cfg.n_samples
+    d_wf = torch.empty((E, P, S), dtype=torch.int16, device="cuda")
+    dl0gen.events_cuda(cfg, d_wf.data_ptr(), 0, E, torch.cuda.current_stream().cuda_stream)
+    outs = image_outputs(E, P, mask=False)
+    before = rta.rta_launch_count()
+    rta.rta_extract_image(d_wf, E, P, S, dev(ped, np.int32), dev(gain, F32), cfg.W, dev(x), dev(y),
+                          dev(nbr), tp, tb, *outs)
+    n, par, _ = host(outs)
+    assert rta.rta_launch_count() == before + 1
+    del d_wf
+    assert (n >= 0).all() and (n <= P).all() and np.isfinite(par).all()
+    assert ((par == 0).all(1) == (n == 0)).all()              # positive thresholds: empty <=> zero
+    nb = 6 if name != "C4" else 3
+    for first in [0, E - 8] + [int(v) for v in np.random.default_rng(1).integers(8, E - 16, nb)]:
+        wf = dl0gen.events_cpu(cfg, first, 8, threads=8)
+        want = oracle_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb)
+        assert_image_parity((n[first:first + 8], par[first:first + 8], None), want, x, y,
+                            "%s events %d.." % (name, first))

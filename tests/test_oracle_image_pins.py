@@ -14,6 +14,7 @@ import pytest
 
 import dl0gen
 import oracle
+from tests._image import blob_images
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden", "image7.json")
 F32 = np.float32
@@ -76,23 +77,6 @@ def np_moments(q, t, x, y, mask):
                   math.sqrt(max(ev[1], 0)), math.sqrt(max(ev[0], 0)), psi,
                   np.average(t[e][m].astype(np.float64), weights=w), q[e][m].max()]
     return out
-
-
-def blob_images(E, P, seed, pitch=0.05):
-    """Elliptical Gaussian blobs on a hex camera plus noise: shower-like test images."""
-    rng = np.random.default_rng(seed)
-    x, y, nbr = dl0gen.hex_camera(P, pitch)
-    R = float(np.hypot(x, y).max())
-    q = rng.normal(0, 1.5, (E, P))
-    t = rng.normal(15, 3, (E, P))
-    for e in range(E):
-        cx, cy = rng.uniform(-0.5 * R, 0.5 * R, 2)
-        L, Wd = rng.uniform(2, 6) * pitch, rng.uniform(0.7, 2) * pitch
-        a = rng.uniform(-np.pi / 2, np.pi / 2)
-        u = (x - cx) * np.cos(a) + (y - cy) * np.sin(a)
-        v = -(x - cx) * np.sin(a) + (y - cy) * np.cos(a)
-        q[e] += rng.uniform(30, 300) * np.exp(-0.5 * ((u / L) ** 2 + (v / Wd) ** 2))
-    return q.astype(F32), t.astype(F32), x, y, nbr
 
 
 @pytest.mark.parametrize("P,seed", [(1855, 0), (1764, 1), (37, 2), (2048, 3)])
