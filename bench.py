@@ -55,6 +55,10 @@ def parse_args():
     ap.add_argument("--input-format", default="u16", choices=["u16", "p12"],
                     help="u16: BASELINE.json's uint16 waveforms (the headline); p12: the same batch as "
                          "a packed 12-bit stream through rta_extract_packed12 (NEXT-2)")
+    ap.add_argument("--path", default="extract", choices=["extract", "image", "moments"],
+                    help="main leg: rta_extract (default, the BASELINE metric); 'image' = "
+                         "rta_extract_image, 'moments' = rta_image_moments (diagnostic runs "
+                         "for profiling, imply --no-extra)")
     ap.add_argument("--no-extra", action="store_true", help="skip configs/e2e/sustained/cpu legs")
     ap.add_argument("--no-sustained", action="store_true", help="skip the 29.68 GB C5 leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
@@ -251,10 +255,36 @@ def device_batch(cfg, torch, dl0gen):
     return d_wf, d_ped, d_gain, outs, ped, gain
 
 
-def kernel_only(cfg, steps, warmup, torch, dl0gen, rta, barrier=None, sampler=None, fmt="u16"):
+def camera_on_device(cfg, torch, dl0gen):
+    x, y, nbr = dl0gen.hex_camera(cfg.n_pixels)
+    tp, tb = dl0gen.IMAGE_THRESHOLDS[cfg.name]
+    return torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda(), torch.from_numpy(nbr).cuda(), tp, tb
+
+
+def image_outputs(cfg, torch):
+    return (torch.empty(cfg.n_events, dtype=torch.int32, device="cuda"),
+            torch.empty((cfg.n_events, 8), dtype=torch.float32, device="cuda"))
+
+
+def kernel_only(cfg, steps, warmup, torch, dl0gen, rta, barrier=None, sampler=None, fmt="u16",
+                path="extract"):
     d_wf, d_ped, d_gain, outs, ped, gain = device_batch(cfg, torch, dl0gen)
     stream = torch.cuda.current_stream()
-    if fmt == "p12":
+    if path in ("image", "moments"):
+        cam = camera_on_device(cfg, torch, dl0gen)
+        ev_out = image_outputs(cfg, torch)
+        if path == "image":
+            def run():
+                rta.rta_extract_image(d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped,
+                                      d_gain, cfg.W, *cam, *ev_out, None, stream=stream)
+        else:
+            rta.rta_extract(d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain,
+                            cfg.W, *outs, stream=stream)
+
+            def run():
+                rta.rta_image_moments(outs[2], outs[3], cfg.n_events, cfg.n_pixels, *cam,
+                                      *ev_out, None, stream=stream)
+    elif fmt == "p12":
         n_total = cfg.n_traces * cfg.n_samples
         d_pk = torch.empty(dl0gen.packed12_nbytes(n_total), dtype=torch.uint8, device="cuda")
         dl0gen.pack12_cuda(d_wf.data_ptr(), n_total, d_pk.data_ptr(), stream.cuda_stream)
@@ -393,6 +423,55 @@ def ragged_leg(steps, peak, torch, dl0gen, rta, n_events=1000):
            "frac_of_measured_hbm": algo / avg / 1e6 / peak, "traces_per_s": m.n_traces / avg * 1e3,
            "plan_create_ms_host": t_plan * 1e3}
     rta.rta_ragged_plan_destroy(plan)
+    return res
+
+
+EVENT_OUT_BYTES = 36   # n_pix int32 + 8 fp32 parameters per event
+
+
+def image_leg(cfg, steps, peak, torch, dl0gen, rta):
+    """NEXT-4: extraction + cleaning + moments. `fused` = rta_extract_image (one
+    kernel, 36 bytes per event written); `two_calls` = rta_extract followed by
+    rta_image_moments (charge / time cross HBM twice); `moments` = the second
+    call alone. GB/s are algorithmic bytes of each leg over its device time."""
+    d_wf, d_ped, d_gain, outs, ped, gain = device_batch(cfg, torch, dl0gen)
+    cam = camera_on_device(cfg, torch, dl0gen)
+    ev_out = image_outputs(cfg, torch)
+    stream = torch.cuda.current_stream()
+    base = (d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain, cfg.W)
+
+    def fused():
+        rta.rta_extract_image(*base, *cam, *ev_out, None, stream=stream)
+
+    def moments():
+        rta.rta_image_moments(outs[2], outs[3], cfg.n_events, cfg.n_pixels, *cam, *ev_out, None,
+                              stream=stream)
+
+    def two_calls():
+        rta.rta_extract(*base, *outs, stream=stream)
+        moments()
+    ev_bytes = EVENT_OUT_BYTES * cfg.n_events
+    algo = {"fused": cfg.input_bytes + ev_bytes,
+            "two_calls": cfg.input_bytes + cfg.output_bytes + 8 * cfg.n_traces + ev_bytes,
+            "moments": 8 * cfg.n_traces + ev_bytes}
+    res = {"workload": "%s: %s; hex camera, thresholds %g / %g" % (
+        cfg.name, cfg.label, cam[3], cam[4]),
+        "kernel": rta.rta_image_kernel_name(cfg.n_pixels, cfg.n_samples, cfg.W, True)}
+    for name, run in (("fused", fused), ("two_calls", two_calls), ("moments", moments)):
+        for _ in range(3):
+            run()
+        torch.cuda.synchronize()
+        per = time_steps(run, steps, stream)
+        avg = sum(per) / len(per)
+        res[name] = {"ms_avg": avg, "ms_median": statistics.median(per), "ms_best": min(per),
+                     "algorithmic_bytes": algo[name], "algorithmic_GBps": algo[name] / avg / 1e6,
+                     "frac_of_measured_hbm": algo[name] / avg / 1e6 / peak,
+                     "waveform_GBps": cfg.input_bytes / avg / 1e6,
+                     "events_per_s": cfg.n_events / avg * 1e3}
+    n = ev_out[0].cpu()
+    res["mean_pixels_in_image"] = float(n.float().mean())
+    res["empty_events_frac"] = float((n == 0).float().mean())
+    res["fused_speedup_vs_two_calls"] = res["two_calls"]["ms_avg"] / res["fused"]["ms_avg"]
     return res
 
 
@@ -612,9 +691,10 @@ def main():
     # Weak scaling: every rank extracts its own batch of the named workload
     # (independent events; no data-path collective).
     fmt = args.input_format
-    if fmt == "p12":
-        args.no_extra = True     # the packed main leg is a profiling/diagnostic run
-    main_run = kernel_only(cfg, args.steps, args.warmup, torch, dl0gen, rta, barrier, sampler, fmt)
+    if fmt == "p12" or args.path != "extract":
+        args.no_extra = True     # the packed / image main legs are profiling/diagnostic runs
+    main_run = kernel_only(cfg, args.steps, args.warmup, torch, dl0gen, rta, barrier, sampler, fmt,
+                           args.path)
     clocks = sampler.stop(*main_run["marks"])
     t_local = sum(main_run["per_launch_ms"])
     t_max = t_local
@@ -637,12 +717,28 @@ def main():
         summ["algorithmic_GBps"] = algo_bytes / avg / 1e6
         summ["frac_of_measured_hbm"] = algo_bytes / avg / 1e6 / peak
         summ["frac_of_nominal_8TBps"] = algo_bytes / avg / 1e6 / 8000.0
+    if args.path != "extract":
+        ev_bytes = EVENT_OUT_BYTES * cfg.n_events
+        if args.path == "image":
+            algo_bytes = cfg.input_bytes + ev_bytes
+            kname = rta.rta_image_kernel_name(cfg.n_pixels, cfg.n_samples, cfg.W, True)
+            bytes_per_trace = 2 * cfg.n_samples + EVENT_OUT_BYTES / cfg.n_pixels
+        else:
+            algo_bytes = 8 * cfg.n_traces + ev_bytes
+            kname = "image_moments"
+            bytes_per_trace = 8 + EVENT_OUT_BYTES / cfg.n_pixels
+        avg = summ["ms_avg"]
+        summ["algorithmic_GBps"] = algo_bytes / avg / 1e6
+        summ["frac_of_measured_hbm"] = algo_bytes / avg / 1e6 / peak
+        summ["frac_of_nominal_8TBps"] = algo_bytes / avg / 1e6 / 8000.0
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
         "config": {
-            "workload": "%s: %s" % (cfg.name, cfg.label) + (" as a P12 stream" if fmt == "p12" else ""),
+            "workload": "%s: %s" % (cfg.name, cfg.label) + (" as a P12 stream" if fmt == "p12" else "")
+                        + {"extract": "", "image": " through rta_extract_image",
+                           "moments": " charges through rta_image_moments"}[args.path],
             "per_gpu": "%d events x %d pixels x %d samples uint16, W=%d" % (
                 cfg.n_events, cfg.n_pixels, cfg.n_samples, cfg.W),
             "l2": "input %.2f GB per step exceeds the 126 MB L2 (no flush needed)" % (cfg.input_bytes / 1e9),
@@ -707,6 +803,12 @@ def main():
             out["packed12"] = pk
             out["ragged"] = ragged_leg(max(10, args.steps // 4), peak, torch, dl0gen, rta)
             torch.cuda.empty_cache()
+            img = {}
+            for name in ("C2", "C3", "C4"):
+                img[name] = image_leg(dl0gen.CONFIGS[name], max(10, args.steps // 4), peak,
+                                      torch, dl0gen, rta)
+                torch.cuda.empty_cache()
+            out["image"] = img
             link = host_link_bandwidth(torch)
             out["e2e"]["host_link_GBps_measured"] = link
             out["e2e"]["frac_of_host_link"] = out["e2e"]["value"] / link

@@ -308,8 +308,8 @@ void rta_ragged_plan_destroy(rta_ragged_plan* plan);
  *
  * All asynchronous on `stream` except _host. Errors: the shape/NULL/alignment
  * rules of rta_extract for the waveform side; n_pixels above
- * rta_image_max_pixels() (one event's charges, times and flags must fit one
- * CTA's shared memory: 23 136 pixels) -> RTA_ERR_UNSUPPORTED; NULL geometry or
+ * rta_image_max_pixels() (two events' charges, times and bit masks must fit one
+ * CTA's shared memory: 12 288 pixels) -> RTA_ERR_UNSUPPORTED; NULL geometry or
  * output (out_mask excepted) -> RTA_ERR_NULL; 4-byte alignment of every float /
  * int32 array. NaN thresholds give empty masks. n_events == 0 -> RTA_OK. */
 int rta_image_moments(const float* charge, const float* time, int64_t n_events,

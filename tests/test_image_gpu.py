@@ -233,6 +233,7 @@ def test_fused_equals_extract_then_moments(name):
 @pytest.mark.parametrize("S,W,P,E", [
     (40, 7, 1, 50), (40, 7, 255, 40), (40, 7, 256, 40), (40, 7, 257, 40), (40, 7, 512, 20),
     (40, 7, 3000, 9),                       # staged, tiles per event 1 .. 12
+    (40, 7, 12288, 3),                      # the largest camera (generic: the buffers fill the SM)
     (30, 7, 333, 31), (30, 7, 2, 100),      # 60-byte traces: events 4-byte aligned only
     (25, 4, 1764, 21), (25, 4, 510, 33), (25, 4, 2, 64),   # two traces per thread, 8-byte phases
     (25, 4, 1765, 11),                      # odd camera -> generic
