@@ -92,101 +92,149 @@ struct CleanScratch {
 };
 
 // Pixel indices of the set bits of word(w), w = 0 .. NW-1, in ascending order
-// into list[]; returns their number (same value in every lane). One warp.
+// into list[]; returns their number (same value in every lane). One warp: lane
+// l owns the K = ceil(NW / 32) consecutive words l K .. l K + K - 1, so one
+// prefix sum over the lanes' bit counts places every lane's run.
 template <class F>
 __device__ __forceinline__ int compact_bits(const int NW, uint16_t* __restrict__ list, F word) {
   const int lane = threadIdx.x & 31;
-  int base = 0;
-  for (int w0 = 0; w0 < NW; w0 += 32) {
-    const int w = w0 + lane;
-    uint32_t bits = w < NW ? word(w) : 0u;
-    const int c = __popc(bits);
-    int incl = c;
+  const int K = (NW + 31) >> 5;
+  const int w_lo = lane * K, w_hi = min(w_lo + K, NW);
+  int c = 0;
+  for (int w = w_lo; w < w_hi; ++w) c += __popc(word(w));
+  int incl = c;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
-      if (lane >= o) incl += v;
-    }
-    int off = base + incl - c;
+  for (int o = 1; o < 32; o <<= 1) {
+    const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  int off = incl - c;
+  for (int w = w_lo; w < w_hi; ++w) {
+    uint32_t bits = word(w);
     while (bits) {
       const int b = __ffs((int)bits) - 1;
       bits &= bits - 1u;
       list[off++] = (uint16_t)(32 * w + b);
     }
-    base += __shfl_sync(0xFFFFFFFFu, incl, 31);
   }
+  const int total = __shfl_sync(0xFFFFFFFFu, incl, 31);
   __syncwarp();
-  return base;
+  return total;
 }
 
 __device__ __forceinline__ bool test_bit(const uint32_t* w, const int n) {
   return (w[n >> 5] >> (n & 31)) & 1u;
 }
 
+// For the n listed pixels: hit = some neighbour's bit is set in in_w; hits set
+// the pixel's bit in out_w. Four list entries per lane are in flight at once
+// (their neighbour rows are loaded before any is used). Returns "any hit" per
+// lane. nb8: the table is 8-byte aligned, so a 24-byte row is three 8-byte loads.
+__device__ __forceinline__ int neighbour_pass(const int n, const uint16_t* __restrict__ list,
+                                              const int32_t* __restrict__ nbr, const bool nb8,
+                                              const int P, const uint32_t* in_w,
+                                              uint32_t* out_w) {
+  const int lane = threadIdx.x & 31;
+  constexpr int U = 2;
+  int any = 0;
+  for (int i0 = 0; i0 < n; i0 += 32 * U) {
+    int p[U], nb[U][6];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int i = i0 + 32 * u + lane;
+      p[u] = i < n ? (int)list[i] : -1;
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (p[u] >= 0) {
+        const int32_t* row = nbr + 6u * (size_t)p[u];
+        if (nb8) {
+#pragma unroll
+          for (int j = 0; j < 3; ++j) {
+            const int2 v = __ldg(reinterpret_cast<const int2*>(row) + j);
+            nb[u][2 * j] = v.x, nb[u][2 * j + 1] = v.y;
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 6; ++j) nb[u][j] = __ldg(row + j);
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (p[u] >= 0) {
+        bool hit = false;
+#pragma unroll
+        for (int j = 0; j < 6; ++j)
+          if ((unsigned)nb[u][j] < (unsigned)P && test_bit(in_w, nb[u][j])) hit = true;
+        if (hit) {
+          atomicOr(&out_w[p[u] >> 5], 1u << (p[u] & 31));
+          any = 1;
+        }
+      }
+    }
+  }
+  __syncwarp();
+  return any;
+}
+
+__device__ __forceinline__ double bcast(const double v, const int src) {
+  return __shfl_sync(0xFFFFFFFFu, v, src);
+}
+
 // Cleaning and moments of event e (readings R31-R35), executed by one whole
-// warp. buf.q / core_w / low_w are in shared memory and complete; t points at
-// the event's peak times (shared or global memory).
+// warp. q / core_w / low_w are in shared memory and complete; t points at the
+// event's peak times (shared or global memory).
 __device__ __forceinline__ void clean_warp(const uint32_t e, const int P, const float* q,
                                            const float* t, const uint32_t* core_w,
                                            const uint32_t* low_w, const CleanScratch& sc,
                                            const RtaCamera& cam, const RtaImageOut& out) {
   const int lane = threadIdx.x & 31;
   const int NW = (int)mask_words(P);
+  const bool nb8 = (reinterpret_cast<uintptr_t>(cam.neighbors) & 7u) == 0;
   uint8_t* mrow = out.mask ? out.mask + (size_t)e * (size_t)P : nullptr;
 
   // keep[p] = core[p] and some neighbour is core (isolated core pixels drop)
-  const int n_core = compact_bits(NW, sc.list, [&](int w) { return core_w[w]; });
   for (int w = lane; w < NW; w += 32) sc.keep_w[w] = 0u;
-  __syncwarp();
-  int kept = 0;
-  for (int i = lane; i < n_core; i += 32) {
-    const int p = sc.list[i];
-    const int32_t* nb = cam.neighbors + 6u * (size_t)p;
-    bool k = false;
-#pragma unroll
-    for (int j = 0; j < 6; ++j) {
-      const int n = __ldg(nb + j);
-      if ((unsigned)n < (unsigned)P && test_bit(core_w, n)) k = true;
-    }
-    if (k) {
-      atomicOr(&sc.keep_w[p >> 5], 1u << (p & 31));
-      kept = 1;
-    }
-  }
-  __syncwarp();
+  const int n_core = compact_bits(NW, sc.list, [&](int w) { return core_w[w]; });
+  const int kept = neighbour_pass(n_core, sc.list, cam.neighbors, nb8, P, core_w, sc.keep_w);
   if (!__any_sync(0xFFFFFFFFu, kept)) {  // no surviving core pixel: the mask is empty
     if (mrow)
       for (int p = lane; p < P; p += 32) mrow[p] = 0;
-    if (lane == 0) out.n_pix[e] = 0;
+    if (lane == 8) out.n_pix[e] = 0;
     if (lane < 8) out.params[(size_t)e * 8u + lane] = 0.0f;
     return;
   }
 
   // mask[p] = keep[p] or (q[p] >= thr_boundary and some neighbour is kept)
+  for (int w = lane; w < NW; w += 32) sc.mask_w[w] = sc.keep_w[w];
   const int n_cand =
       compact_bits(NW, sc.list, [&](int w) { return low_w[w] & ~sc.keep_w[w]; });
-  for (int w = lane; w < NW; w += 32) sc.mask_w[w] = sc.keep_w[w];
-  __syncwarp();
-  for (int i = lane; i < n_cand; i += 32) {
-    const int p = sc.list[i];
-    const int32_t* nb = cam.neighbors + 6u * (size_t)p;
-    bool m = false;
-#pragma unroll
-    for (int j = 0; j < 6; ++j) {
-      const int n = __ldg(nb + j);
-      if ((unsigned)n < (unsigned)P && test_bit(sc.keep_w, n)) m = true;
-    }
-    if (m) atomicOr(&sc.mask_w[p >> 5], 1u << (p & 31));
-  }
-  __syncwarp();
+  neighbour_pass(n_cand, sc.list, cam.neighbors, nb8, P, sc.keep_w, sc.mask_w);
   if (mrow)
     for (int p = lane; p < P; p += 32) mrow[p] = test_bit(sc.mask_w, p) ? 1 : 0;
 
-  // pass 1 over the mask pixels (ascending pixel order, lane i takes entries i, i + 32, ...)
+  // pass 1 over the mask pixels in ascending pixel order: lane i takes entries
+  // i, i + 32, ...; the first two per lane stay in registers for pass 2
   const int n_pix = compact_bits(NW, sc.list, [&](int w) { return sc.mask_w[w]; });
-  double s0 = 0.0, sx = 0.0, sy = 0.0, st = 0.0;
+  double rw[2] = {0.0, 0.0}, rx[2] = {0.0, 0.0}, ry[2] = {0.0, 0.0}, rt[2] = {0.0, 0.0};
   float qm = -INFINITY;
-  for (int i = lane; i < n_pix; i += 32) {
+#pragma unroll
+  for (int u = 0; u < 2; ++u) {
+    const int i = lane + 32 * u;
+    if (i < n_pix) {
+      const int p = sc.list[i];
+      const float qp = q[p];
+      rw[u] = (double)qp;
+      rx[u] = (double)__ldg(cam.pix_x + p);
+      ry[u] = (double)__ldg(cam.pix_y + p);
+      rt[u] = (double)t[p];
+      qm = fmaxf(qm, qp);
+    }
+  }
+  double s0 = rw[0], sx = rw[0] * rx[0], sy = rw[0] * ry[0], st = rw[0] * rt[0];
+  s0 += rw[1], sx += rw[1] * rx[1], sy += rw[1] * ry[1], st += rw[1] * rt[1];
+  for (int i = lane + 64; i < n_pix; i += 32) {
     const int p = sc.list[i];
     const float qp = q[p];
     const double w = (double)qp;
@@ -200,15 +248,24 @@ __device__ __forceinline__ void clean_warp(const uint32_t e, const int P, const 
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) qm = fmaxf(qm, __shfl_xor_sync(0xFFFFFFFFu, qm, o));
   if (!(s0 > 0.0)) {  // non-positive (or NaN) total charge: parameters are zero, the count stands
-    if (lane == 0) out.n_pix[e] = n_pix;
+    if (lane == 8) out.n_pix[e] = n_pix;
     if (lane < 8) out.params[(size_t)e * 8u + lane] = 0.0f;
     return;
   }
-  const double cx = sx / s0, cy = sy / s0;
+  // one division for three quotients: lane 0, 1, 2 divide sx, sy, st by s0
+  const double r1 = (lane == 0 ? sx : lane == 1 ? sy : st) / s0;
+  const double cx = bcast(r1, 0), cy = bcast(r1, 1), tm = bcast(r1, 2);
 
   // pass 2: centred second moments
   double sxx = 0.0, syy = 0.0, sxy = 0.0;
-  for (int i = lane; i < n_pix; i += 32) {
+#pragma unroll
+  for (int u = 0; u < 2; ++u) {  // entries past n_pix carry zero weight
+    const double dx = rx[u] - cx, dy = ry[u] - cy;
+    sxx += rw[u] * dx * dx;
+    syy += rw[u] * dy * dy;
+    sxy += rw[u] * dx * dy;
+  }
+  for (int i = lane + 64; i < n_pix; i += 32) {
     const int p = sc.list[i];
     const double w = (double)q[p];
     const double dx = (double)__ldg(cam.pix_x + p) - cx, dy = (double)__ldg(cam.pix_y + p) - cy;
@@ -216,28 +273,37 @@ __device__ __forceinline__ void clean_warp(const uint32_t e, const int P, const 
     syy += w * dy * dy;
     sxy += w * dx * dy;
   }
-  sxx = warp_sum(sxx) / s0, syy = warp_sum(syy) / s0, sxy = warp_sum(sxy) / s0;
-  // every lane holds the same sums; lane i computes and stores parameter i
+  sxx = warp_sum(sxx), syy = warp_sum(syy), sxy = warp_sum(sxy);
+  const double r2 = (lane == 0 ? sxx : lane == 1 ? syy : sxy) / s0;
+  sxx = bcast(r2, 0), syy = bcast(r2, 1), sxy = bcast(r2, 2);
   const double d = sxx - syy;
   const double z = sqrt(d * d + 4.0 * sxy * sxy);
-  float v;
-  switch (lane) {
-    case 0: v = (float)s0; break;
-    case 1: v = (float)cx; break;
-    case 2: v = (float)cy; break;
-    case 3: v = (float)sqrt(0.5 * (sxx + syy + z)); break;
-    case 4: v = (float)sqrt(fmax(0.5 * (sxx + syy - z), 0.0)); break;
-    case 5: v = (float)(0.5 * atan2(2.0 * sxy, d)); break;
-    case 6: v = (float)(st / s0); break;
-    default: v = qm; break;
-  }
-  if (lane < 8) out.params[(size_t)e * 8u + lane] = v;
+  // one square root for length (lane 3) and width (lane 4)
+  const double r3 = sqrt(lane == 3 ? 0.5 * (sxx + syy + z) : fmax(0.5 * (sxx + syy - z), 0.0));
+  const double psi = 0.5 * atan2(2.0 * sxy, d);
+  const double v = lane == 0 ? s0 : lane == 1 ? cx : lane == 2 ? cy : lane == 5 ? psi
+                 : lane == 6 ? tm : r3;
+  if (lane < 7) out.params[(size_t)e * 8u + lane] = (float)v;
+  if (lane == 7) out.params[(size_t)e * 8u + 7u] = qm;
   if (lane == 8) out.n_pix[e] = n_pix;
 }
 
 // ------------------------------------------------ cleaning on HBM arrays ----
-// One warp per event: the charge row goes through shared memory (its
-// threshold bits by ballot on the way), peak times stay in HBM.
+// One warp per event: the charge row comes in by cp.async into one of two
+// per-warp buffers (the next event's row is in flight while this one is
+// cleaned); peak times stay in HBM and are gathered for the mask pixels only.
+__device__ __forceinline__ void row_async(float* dst, const float* src, const int P) {
+  const int lane = threadIdx.x & 31;
+  int p = 0;
+  if ((reinterpret_cast<uintptr_t>(src) & 15u) == 0) {
+    const int n4 = P >> 2;
+    for (int i = lane; i < n4; i += 32) cp_async16(smem_u32(dst + 4 * i), src + 4 * i);
+    p = 4 * n4;
+  }
+  for (int i = p + lane; i < P; i += 32) cp_async4(smem_u32(dst + i), src + i);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+}
+
 template <int WARPS>
 __global__ void __launch_bounds__(32 * WARPS)
     image_moments_kernel(const float* __restrict__ charge, const float* __restrict__ time,
@@ -246,25 +312,36 @@ __global__ void __launch_bounds__(32 * WARPS)
                          const __grid_constant__ RtaImageOut out) {
   extern __shared__ __align__(128) uint8_t smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const size_t per_warp = EventBuf::bytes(P, false) + CleanScratch::bytes(P);
+  const size_t row_bytes = r16(4u * (size_t)P);
+  const size_t per_warp = row_bytes + EventBuf::bytes(P, false) + CleanScratch::bytes(P);
   uint8_t* mine = smem + (size_t)warp * per_warp;
-  const EventBuf buf(mine, P, false);
-  const CleanScratch sc(mine + EventBuf::bytes(P, false), P);
+  float* rows[2] = {reinterpret_cast<float*>(mine), reinterpret_cast<float*>(mine + row_bytes)};
+  const EventBuf buf(mine + row_bytes, P, false);  // buf.q == rows[1]; only the bit words are used
+  const CleanScratch sc(mine + row_bytes + EventBuf::bytes(P, false), P);
   const float thr_p = cam.thr_picture, thr_b = cam.thr_boundary;
-  for (uint32_t e = blockIdx.x * WARPS + warp; e < n_events; e += gridDim.x * WARPS) {
-    const float* q = charge + (size_t)e * (size_t)P;
+  const uint32_t stride = gridDim.x * WARPS;
+  uint32_t e = blockIdx.x * WARPS + warp;
+  if (e < n_events) row_async(rows[0], charge + (size_t)e * (size_t)P, P);
+  for (int b = 0; e < n_events; e += stride, b ^= 1) {
+    if (e + stride < n_events) {
+      row_async(rows[b ^ 1], charge + (size_t)(e + stride) * (size_t)P, P);
+      asm volatile("cp.async.wait_group 1;" ::: "memory");
+    } else {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
+    __syncwarp();
+    const float* q = rows[b];
 #pragma unroll 4
     for (int p0 = 0; p0 < P; p0 += 32) {
       const int p = p0 + lane;
       const bool in = p < P;
-      const float v = in ? __ldcs(q + p) : 0.0f;
-      if (in) buf.q[p] = v;
+      const float v = in ? q[p] : 0.0f;
       const uint32_t c = __ballot_sync(0xFFFFFFFFu, in && v >= thr_p);
       const uint32_t l = __ballot_sync(0xFFFFFFFFu, in && v >= thr_b);
       if (lane == 0) buf.core_w[p0 >> 5] = c, buf.low_w[p0 >> 5] = l;
     }
     __syncwarp();
-    clean_warp(e, P, buf.q, time + (size_t)e * (size_t)P, buf.core_w, buf.low_w, sc, cam, out);
+    clean_warp(e, P, q, time + (size_t)e * (size_t)P, buf.core_w, buf.low_w, sc, cam, out);
     __syncwarp();
   }
 }
@@ -374,7 +451,7 @@ __device__ __forceinline__ uint32_t spread16(uint32_t x) {
 // the next event drawn from the shared counter. The producer side runs STAGES
 // items ahead of the consumer through item_q, across event boundaries.
 template <class C>
-__global__ void __launch_bounds__(C::NT + 32)
+__global__ void __launch_bounds__(C::NT + 32, C::NT >= 256 ? 3 : 1)
     extract_image_kernel(const uint8_t* __restrict__ wf, const uint32_t n_events, const int P,
                          const int* __restrict__ pedestal, const float* __restrict__ gain,
                          const __grid_constant__ RtaCamera cam,
@@ -583,6 +660,11 @@ using ImgS40W7 = TileCfg<40, 7, RTA_I40_NT, RTA_I40_ST>;
 using ImgS25W4 = TileCfg<25, 4, RTA_I25_NT, RTA_I25_ST>;
 using ImgS128W8 = TileCfg<128, 8, RTA_I128_NT, RTA_I128_ST>;
 
+// shared memory of one warp of image_moments_kernel: two charge rows, bit words, scratch
+size_t moments_warp_bytes(int32_t P) {
+  return r16(4u * (size_t)P) + EventBuf::bytes(P, false) + CleanScratch::bytes(P);
+}
+
 // shared memory of the fused kernels behind the stage ring: two event buffers
 // and the cleaning warp's scratch
 size_t fused_image_bytes(int32_t P) {
@@ -654,7 +736,7 @@ cudaError_t resident_grid(K kernel, int threads, size_t smem, uint32_t n_events,
 template <int WARPS>
 cudaError_t launch_moments(const float* charge, const float* time, uint32_t n_events, int32_t P,
                            const RtaCamera& cam, const RtaImageOut& out, cudaStream_t stream) {
-  const size_t smem = WARPS * (EventBuf::bytes(P, false) + CleanScratch::bytes(P));
+  const size_t smem = WARPS * moments_warp_bytes(P);
   uint32_t grid = 0;
   cudaError_t e =
       resident_grid(image_moments_kernel<WARPS>, 32 * WARPS, smem, n_events, WARPS, &grid);
@@ -689,7 +771,7 @@ cudaError_t rta_launch_image_moments(const float* charge, const float* time, int
                                      const RtaImageOut& out, cudaStream_t stream) {
   if (n_events <= 0) return cudaSuccess;
   // as many warps per CTA as keep two CTAs per SM resident
-  const size_t per_warp = EventBuf::bytes(n_pixels, false) + CleanScratch::bytes(n_pixels);
+  const size_t per_warp = moments_warp_bytes(n_pixels);
   const size_t half = (kSmemLimit - 2048u) / 2u;
   const uint32_t E = (uint32_t)n_events;
   if (8u * per_warp <= half) return launch_moments<8>(charge, time, E, n_pixels, cam, out, stream);
