@@ -114,6 +114,8 @@ def lib() -> ctypes.CDLL:
             L.rta_shutdown.argtypes = []
             L.rta_debug_static_schedule.restype = None
             L.rta_debug_static_schedule.argtypes = [ctypes.c_int]
+            L.rta_debug_general_cleaning.restype = None
+            L.rta_debug_general_cleaning.argtypes = [ctypes.c_int]
             _lib = L
     return _lib
 
@@ -380,6 +382,12 @@ def rta_debug_static_schedule(on: bool) -> None:
     """Test hook: force the static round-robin tile schedule of the staged
     kernels (default is dynamic). Results are identical either way."""
     lib().rta_debug_static_schedule(1 if on else 0)
+
+
+def rta_debug_general_cleaning(on: bool) -> None:
+    """Test hook: the image cleaning runs the two steps of its definition even
+    when the neighbour table is symmetric (same masks either way)."""
+    lib().rta_debug_general_cleaning(1 if on else 0)
 
 
 def shard_events(n_events: int, world_size: int, rank: int) -> tuple[int, int]:

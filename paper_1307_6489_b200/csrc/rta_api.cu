@@ -933,4 +933,8 @@ void rta_debug_force_generic(int on) { g_force_generic.store(on != 0); }
 // 0 = dynamic (default). Results are identical; only the tile->CTA map changes.
 void rta_debug_static_schedule(int on) { rta_set_static_schedule(on != 0); }
 
+// Test hook (not in the public header): 1 = the image cleaning runs the two
+// steps of its definition even when the neighbour table is symmetric.
+void rta_debug_general_cleaning(int on) { rta_set_general_cleaning(on != 0); }
+
 }  // extern "C"

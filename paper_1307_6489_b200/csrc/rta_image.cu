@@ -10,67 +10,70 @@
 // of the surviving pixels (size, centre of gravity, length, width, psi), the
 // charge-weighted mean peak time, the largest charge and the pixel count.
 //
-// How:
-//  * clean_warp: ONE WARP cleans one event. The image is sparse (a few per
+// How (DESIGN.md section 5e):
+//  * clean_event: ONE WARP cleans one event. The image is sparse (a few per
 //    cent of the pixels pass a threshold), so the work is organised around bit
-//    masks of the camera (one bit per pixel: core, low, keep, mask) and
-//    compacted pixel lists: only core pixels look at their neighbours' core
-//    bits, only pixels above the boundary threshold that are not kept look at
-//    their neighbours' keep bits, and the moments run over the list of mask
-//    pixels. Sums are fp64 (per-lane partial sums over the list in pixel order,
-//    xor butterfly over the lanes: no atomics on floating point, run-to-run
-//    deterministic), centred second moments in a second pass like the definition.
-//  * extract_image_kernel<C> (fused, staged): a CTA owns one event at a time.
-//    NT extraction threads stream the event's traces through the same
-//    shared-memory stage ring as extract_tile_kernel (TMA bulk copies, or
-//    16-byte cp.async for the padded S = 128 layout; tiles cut per event) and
-//    write charge / peak time / threshold bits into one of two per-event
-//    buffers in shared memory instead of HBM. One extra warp — the cleaning
-//    warp — takes a finished buffer and runs clean_warp on it while the
-//    extraction threads are already on the next event (named-barrier hand-off:
-//    ready / free per buffer). Events are handed out dynamically (one atomic
-//    per event). HBM traffic: the waveform bytes once in, 36 bytes per event
-//    out (+ 1 byte per pixel if the mask is asked for).
-//  * extract_image_generic_kernel: the same hand-off for any (S, W) and any
-//    2-byte alignment; traces are read straight from global memory.
+//    masks of the camera (one bit per pixel) and compacted pixel lists. When
+//    the neighbour table is symmetric (checked by every CTA when it starts,
+//    6 P look-ups spread over its threads) one pass over the core pixels does
+//    both cleaning steps: a core pixel with a core neighbour is kept and marks
+//    those of its neighbours that pass the boundary threshold; otherwise the
+//    two steps of the definition are run as written (pull, two lists). The
+//    moments are ONE pass over the list of mask pixels, about the first mask
+//    pixel as origin (fp64, per-lane partial sums in list order, xor butterfly:
+//    no floating-point atomics, run-to-run deterministic). The scalar tail
+//    (divisions, square roots, atan2) is not run per event: each event's sums
+//    are parked in the registers of one lane and 32 events are finished at
+//    once, one event per lane.
+//  * extract_image_kernel<C, G> (fused, staged): ONE persistent CTA per SM.
+//    G groups of NT extraction threads each stream tiles of the CTA's current
+//    events through their own TMA / cp.async stage ring and write charge, peak
+//    time and threshold bits into one of NB per-event buffers in shared memory
+//    instead of HBM; NC cleaning warps take finished buffers (mbarrier
+//    hand-off: ready[b] counts one arrival per warp and tile, free[b] one per
+//    cleaned event). HBM traffic: the waveform bytes once in, 36 bytes per
+//    event out (+ 1 byte per pixel if the mask is asked for).
+//  * extract_image_generic_kernel: one cleaning warp beside 256 extraction
+//    threads (named barriers) for any (S, W), camera size and 2-byte alignment;
+//    traces are read straight from global memory.
 //  * image_moments_kernel: charge / time arrays already in HBM (rta_extract's
-//    outputs); one warp per event, the charge row staged in shared memory, peak
-//    times gathered from HBM for the mask pixels only.
+//    outputs); one warp per event builds the threshold bits from one coalesced
+//    sweep over the charge row and gathers charge and peak time of the mask
+//    pixels from L2.
 #include "rta_device.cuh"
+
+#include <atomic>
 
 namespace {
 
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
-  return v;
-}
 __device__ __forceinline__ void named_sync(const int id, const int n) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory");
 }
 __device__ __forceinline__ void named_arrive(const int id, const int n) {
   asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 
 __host__ __device__ constexpr size_t r16(size_t n) { return (n + 15u) & ~(size_t)15u; }
 __host__ __device__ constexpr size_t mask_words(int P) { return ((size_t)P + 31u) >> 5; }
 
-// What the producer of an event (extraction threads, or the loading warp
-// itself) hands to clean_warp: charges, peak times (shared or global memory)
-// and the two threshold bit masks, bit p & 31 of word p >> 5.
+// What the producer of an event hands to clean_event: charges, peak times and
+// the two threshold bit masks, bit p & 31 of word p >> 5 (bits past P are 0).
 struct EventBuf {
   float* q;          // [P]
-  float* t;          // [P] (fused kernels only)
+  float* t;          // [P]
   uint32_t* core_w;  // q >= thr_picture
   uint32_t* low_w;   // q >= thr_boundary
-  static __host__ __device__ size_t bytes(int P, bool with_t) {
-    return (with_t ? 2u : 1u) * r16(4u * (size_t)P) + 2u * r16(4u * mask_words(P));
+  static __host__ __device__ size_t bytes(int P) {
+    return 2u * r16(4u * (size_t)P) + 2u * r16(4u * mask_words(P));
   }
-  __device__ __forceinline__ EventBuf(uint8_t* base, const int P, const bool with_t) {
+  __device__ __forceinline__ EventBuf(uint8_t* base, const int P) {
     q = reinterpret_cast<float*>(base);
     base += r16(4u * (size_t)P);
     t = reinterpret_cast<float*>(base);
-    if (with_t) base += r16(4u * (size_t)P);
+    base += r16(4u * (size_t)P);
     core_w = reinterpret_cast<uint32_t*>(base);
     low_w = reinterpret_cast<uint32_t*>(base + r16(4u * mask_words(P)));
   }
@@ -126,10 +129,25 @@ __device__ __forceinline__ bool test_bit(const uint32_t* w, const int n) {
   return (w[n >> 5] >> (n & 31)) & 1u;
 }
 
+// nb8: the table is 8-byte aligned, so a 24-byte row is three 8-byte loads
+__device__ __forceinline__ void load_row(const int32_t* __restrict__ nbr, const bool nb8,
+                                         const int p, int (&nb)[6]) {
+  const int32_t* row = nbr + 6u * (size_t)p;
+  if (nb8) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      const int2 v = __ldg(reinterpret_cast<const int2*>(row) + j);
+      nb[2 * j] = v.x, nb[2 * j + 1] = v.y;
+    }
+  } else {
+#pragma unroll
+    for (int j = 0; j < 6; ++j) nb[j] = __ldg(row + j);
+  }
+}
+
 // For the n listed pixels: hit = some neighbour's bit is set in in_w; hits set
-// the pixel's bit in out_w. Four list entries per lane are in flight at once
-// (their neighbour rows are loaded before any is used). Returns "any hit" per
-// lane. nb8: the table is 8-byte aligned, so a 24-byte row is three 8-byte loads.
+// the pixel's bit in out_w. Two list entries per lane are in flight at once
+// (their neighbour rows are loaded before any is used). Returns "any hit" per lane.
 __device__ __forceinline__ int neighbour_pass(const int n, const uint16_t* __restrict__ list,
                                               const int32_t* __restrict__ nbr, const bool nb8,
                                               const int P, const uint32_t* in_w,
@@ -145,21 +163,8 @@ __device__ __forceinline__ int neighbour_pass(const int n, const uint16_t* __res
       p[u] = i < n ? (int)list[i] : -1;
     }
 #pragma unroll
-    for (int u = 0; u < U; ++u) {
-      if (p[u] >= 0) {
-        const int32_t* row = nbr + 6u * (size_t)p[u];
-        if (nb8) {
-#pragma unroll
-          for (int j = 0; j < 3; ++j) {
-            const int2 v = __ldg(reinterpret_cast<const int2*>(row) + j);
-            nb[u][2 * j] = v.x, nb[u][2 * j + 1] = v.y;
-          }
-        } else {
-#pragma unroll
-          for (int j = 0; j < 6; ++j) nb[u][j] = __ldg(row + j);
-        }
-      }
-    }
+    for (int u = 0; u < U; ++u)
+      if (p[u] >= 0) load_row(nbr, nb8, p[u], nb[u]);
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       if (p[u] >= 0) {
@@ -178,183 +183,297 @@ __device__ __forceinline__ int neighbour_pass(const int n, const uint16_t* __res
   return any;
 }
 
-__device__ __forceinline__ double bcast(const double v, const int src) {
-  return __shfl_sync(0xFFFFFFFFu, v, src);
+// Symmetric neighbour table (p in nbr[n] whenever n in nbr[p]): "n has a kept
+// neighbour" is the same as "a kept pixel lists n", so one pass over the core
+// pixels does both steps of the cleaning. A core pixel with a core neighbour is
+// kept: its own bit goes into mask_w, and so does every neighbour that passes
+// the boundary threshold. Returns "any pixel kept" per lane.
+__device__ __forceinline__ int symmetric_pass(const int n, const uint16_t* __restrict__ list,
+                                              const int32_t* __restrict__ nbr, const bool nb8,
+                                              const int P, const uint32_t* core_w,
+                                              const uint32_t* low_w, uint32_t* mask_w) {
+  const int lane = threadIdx.x & 31;
+  constexpr int U = 2;
+  int any = 0;
+  for (int i0 = 0; i0 < n; i0 += 32 * U) {
+    int p[U], nb[U][6];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int i = i0 + 32 * u + lane;
+      p[u] = i < n ? (int)list[i] : -1;
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+      if (p[u] >= 0) load_row(nbr, nb8, p[u], nb[u]);
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (p[u] >= 0) {
+        bool hit = false;
+        uint32_t lw[6];
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+          const bool ok = (unsigned)nb[u][j] < (unsigned)P;
+          const int w = ok ? (nb[u][j] >> 5) : 0;
+          const uint32_t bit = ok ? (1u << (nb[u][j] & 31)) : 0u;
+          if (core_w[w] & bit) hit = true;
+          lw[j] = low_w[w] & bit;
+        }
+        if (hit) {
+          atomicOr(&mask_w[p[u] >> 5], 1u << (p[u] & 31));
+#pragma unroll
+          for (int j = 0; j < 6; ++j)
+            if (lw[j]) atomicOr(&mask_w[nb[u][j] >> 5], lw[j]);
+          any = 1;
+        }
+      }
+    }
+  }
+  __syncwarp();
+  return any;
 }
 
-// Cleaning and moments of event e (readings R31-R35), executed by one whole
-// warp. q / core_w / low_w are in shared memory and complete; t points at the
-// event's peak times (shared or global memory).
-__device__ __forceinline__ void clean_warp(const uint32_t e, const int P, const float* q,
-                                           const float* t, const uint32_t* core_w,
-                                           const uint32_t* low_w, const CleanScratch& sc,
-                                           const RtaCamera& cam, const RtaImageOut& out) {
+// Every thread of the CTA: is the neighbour table symmetric? One (pixel, slot)
+// entry per thread and step; the answer is the same in every thread. Contains
+// __syncthreads.
+__device__ __forceinline__ int table_is_symmetric(const int32_t* __restrict__ nbr, const int P) {
+  int ok = 1;
+  const int n_entries = 6 * P;
+  for (int i = threadIdx.x; i < n_entries; i += blockDim.x) {
+    const int n = __ldg(nbr + i);
+    if ((unsigned)n < (unsigned)P) {
+      const int p = i / 6;
+      const int32_t* r = nbr + 6u * (size_t)n;
+      bool back = false;
+#pragma unroll
+      for (int j = 0; j < 6; ++j) back |= (__ldg(r + j) == p);
+      if (!back) ok = 0;
+    }
+  }
+  return __syncthreads_and(ok);
+}
+
+// The sums of one event, parked in one lane until 32 events are finished together.
+struct Pending {
+  double s0, sx, sy, st, sxx, syy, sxy;  // about the origin (x0, y0)
+  float x0, y0, qm;
+  int n_pix;
+  uint32_t e;
+};
+
+// One lane, one event: the scalar tail of readings R33 / R34.
+__device__ __forceinline__ void finish_event(const Pending& pd, const RtaImageOut& out) {
+  float o[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) o[i] = 0.0f;
+  if (pd.n_pix > 0 && pd.s0 > 0.0) {  // else: non-positive (or NaN) total charge, parameters are zero
+    const double mx = __ddiv_rn(pd.sx, pd.s0), my = __ddiv_rn(pd.sy, pd.s0);
+    // centred second moments from the ones about the origin: E[d^2] - E[d]^2
+    const double sxx = __fma_rn(-mx, mx, __ddiv_rn(pd.sxx, pd.s0));
+    const double syy = __fma_rn(-my, my, __ddiv_rn(pd.syy, pd.s0));
+    const double sxy = __fma_rn(-mx, my, __ddiv_rn(pd.sxy, pd.s0));
+    const double d = __dsub_rn(sxx, syy);
+    const double z = sqrt(__fma_rn(d, d, __dmul_rn(4.0, __dmul_rn(sxy, sxy))));
+    const double tr = __dadd_rn(sxx, syy);
+    o[0] = (float)pd.s0;
+    o[1] = (float)__dadd_rn((double)pd.x0, mx);
+    o[2] = (float)__dadd_rn((double)pd.y0, my);
+    o[3] = (float)sqrt(__dmul_rn(0.5, __dadd_rn(tr, z)));
+    o[4] = (float)sqrt(fmax(__dmul_rn(0.5, __dsub_rn(tr, z)), 0.0));
+    o[5] = (float)__dmul_rn(0.5, atan2(__dmul_rn(2.0, sxy), d));
+    o[6] = (float)__ddiv_rn(pd.st, pd.s0);
+    o[7] = pd.qm;
+  }
+  float* dst = out.params + (size_t)pd.e * 8u;
+  if ((reinterpret_cast<uintptr_t>(dst) & 15u) == 0) {
+    reinterpret_cast<float4*>(dst)[0] = make_float4(o[0], o[1], o[2], o[3]);
+    reinterpret_cast<float4*>(dst)[1] = make_float4(o[4], o[5], o[6], o[7]);
+  } else {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) dst[i] = o[i];
+  }
+  out.n_pix[pd.e] = pd.n_pix;
+}
+
+__device__ __forceinline__ void flush_pending(const Pending& pd, int& n_pend,
+                                              const RtaImageOut& out) {
+  if ((int)(threadIdx.x & 31) < n_pend) finish_event(pd, out);
+  n_pend = 0;
+  __syncwarp();
+}
+
+__device__ __forceinline__ double shfl_xor_f64(const double v, const int o) {
+  return __shfl_xor_sync(0xFFFFFFFFu, v, o);
+}
+
+// Cleaning and moment sums of event e (readings R31-R35), executed by one whole
+// warp. core_w / low_w are in shared memory and complete; q and t point at the
+// event's charges and peak times (shared or global memory). The event's sums go
+// into lane n_pend's `pd`; after 32 events the warp finishes them together.
+__device__ __forceinline__ void clean_event(const uint32_t e, const int P, const float* q,
+                                            const float* t, const uint32_t* core_w,
+                                            const uint32_t* low_w, const CleanScratch& sc,
+                                            const RtaCamera& cam, const RtaImageOut& out,
+                                            const bool symmetric, Pending& pd, int& n_pend) {
   const int lane = threadIdx.x & 31;
   const int NW = (int)mask_words(P);
   const bool nb8 = (reinterpret_cast<uintptr_t>(cam.neighbors) & 7u) == 0;
   uint8_t* mrow = out.mask ? out.mask + (size_t)e * (size_t)P : nullptr;
 
-  // keep[p] = core[p] and some neighbour is core (isolated core pixels drop)
-  for (int w = lane; w < NW; w += 32) sc.keep_w[w] = 0u;
+  Pending cur;
+  cur.s0 = cur.sx = cur.sy = cur.st = cur.sxx = cur.syy = cur.sxy = 0.0;
+  cur.x0 = cur.y0 = cur.qm = 0.0f;
+  cur.n_pix = 0;
+  cur.e = e;
+
   const int n_core = compact_bits(NW, sc.list, [&](int w) { return core_w[w]; });
-  const int kept = neighbour_pass(n_core, sc.list, cam.neighbors, nb8, P, core_w, sc.keep_w);
-  if (!__any_sync(0xFFFFFFFFu, kept)) {  // no surviving core pixel: the mask is empty
-    if (mrow)
-      for (int p = lane; p < P; p += 32) mrow[p] = 0;
-    if (lane == 8) out.n_pix[e] = 0;
-    if (lane < 8) out.params[(size_t)e * 8u + lane] = 0.0f;
-    return;
+  int kept;
+  if (symmetric) {
+    for (int w = lane; w < NW; w += 32) sc.mask_w[w] = 0u;
+    __syncwarp();
+    kept = symmetric_pass(n_core, sc.list, cam.neighbors, nb8, P, core_w, low_w, sc.mask_w);
+  } else {
+    // keep[p] = core[p] and some neighbour is core (isolated core pixels drop)
+    for (int w = lane; w < NW; w += 32) sc.keep_w[w] = 0u;
+    __syncwarp();
+    kept = neighbour_pass(n_core, sc.list, cam.neighbors, nb8, P, core_w, sc.keep_w);
   }
+  if (__any_sync(0xFFFFFFFFu, kept)) {
+    if (!symmetric) {
+      // mask[p] = keep[p] or (q[p] >= thr_boundary and some neighbour is kept)
+      for (int w = lane; w < NW; w += 32) sc.mask_w[w] = sc.keep_w[w];
+      const int n_cand =
+          compact_bits(NW, sc.list, [&](int w) { return low_w[w] & ~sc.keep_w[w]; });
+      neighbour_pass(n_cand, sc.list, cam.neighbors, nb8, P, sc.keep_w, sc.mask_w);
+    }
+    if (mrow)
+      for (int p = lane; p < P; p += 32) mrow[p] = test_bit(sc.mask_w, p) ? 1 : 0;
 
-  // mask[p] = keep[p] or (q[p] >= thr_boundary and some neighbour is kept)
-  for (int w = lane; w < NW; w += 32) sc.mask_w[w] = sc.keep_w[w];
-  const int n_cand =
-      compact_bits(NW, sc.list, [&](int w) { return low_w[w] & ~sc.keep_w[w]; });
-  neighbour_pass(n_cand, sc.list, cam.neighbors, nb8, P, sc.keep_w, sc.mask_w);
-  if (mrow)
-    for (int p = lane; p < P; p += 32) mrow[p] = test_bit(sc.mask_w, p) ? 1 : 0;
-
-  // pass 1 over the mask pixels in ascending pixel order: lane i takes entries
-  // i, i + 32, ...; the first two per lane stay in registers for pass 2
-  const int n_pix = compact_bits(NW, sc.list, [&](int w) { return sc.mask_w[w]; });
-  double rw[2] = {0.0, 0.0}, rx[2] = {0.0, 0.0}, ry[2] = {0.0, 0.0}, rt[2] = {0.0, 0.0};
-  float qm = -INFINITY;
-#pragma unroll
-  for (int u = 0; u < 2; ++u) {
-    const int i = lane + 32 * u;
-    if (i < n_pix) {
+    // one pass over the mask pixels in ascending pixel order: lane i takes
+    // entries i, i + 32, ...; origin = the first mask pixel (lane 0's first entry)
+    const int n_pix = compact_bits(NW, sc.list, [&](int w) { return sc.mask_w[w]; });
+    float qm = -INFINITY;
+    float fx = 0.0f, fy = 0.0f, fq = 0.0f, ft = 0.0f;
+    if (lane < n_pix) {
+      const int p = sc.list[lane];
+      fq = q[p];
+      ft = t[p];
+      fx = __ldg(cam.pix_x + p);
+      fy = __ldg(cam.pix_y + p);
+      qm = fq;
+    }
+    const float x0 = __shfl_sync(0xFFFFFFFFu, fx, 0), y0 = __shfl_sync(0xFFFFFFFFu, fy, 0);
+    const double X0 = (double)x0, Y0 = (double)y0;
+    double s0, sx, sy, st, sxx, syy, sxy;
+    {
+      const double w = (double)fq;  // 0 for lanes past the list
+      const double dx = __dsub_rn((double)fx, X0), dy = __dsub_rn((double)fy, Y0);
+      const double wx = __dmul_rn(w, dx), wy = __dmul_rn(w, dy);
+      s0 = lane < n_pix ? w : 0.0;
+      sx = lane < n_pix ? wx : 0.0;
+      sy = lane < n_pix ? wy : 0.0;
+      st = lane < n_pix ? __dmul_rn(w, (double)ft) : 0.0;
+      sxx = lane < n_pix ? __dmul_rn(wx, dx) : 0.0;
+      syy = lane < n_pix ? __dmul_rn(wy, dy) : 0.0;
+      sxy = lane < n_pix ? __dmul_rn(wx, dy) : 0.0;
+    }
+    for (int i = lane + 32; i < n_pix; i += 32) {
       const int p = sc.list[i];
       const float qp = q[p];
-      rw[u] = (double)qp;
-      rx[u] = (double)__ldg(cam.pix_x + p);
-      ry[u] = (double)__ldg(cam.pix_y + p);
-      rt[u] = (double)t[p];
+      const double w = (double)qp;
+      const double dx = __dsub_rn((double)__ldg(cam.pix_x + p), X0);
+      const double dy = __dsub_rn((double)__ldg(cam.pix_y + p), Y0);
+      const double wx = __dmul_rn(w, dx), wy = __dmul_rn(w, dy);
+      s0 = __dadd_rn(s0, w);
+      sx = __dadd_rn(sx, wx);
+      sy = __dadd_rn(sy, wy);
+      st = __fma_rn(w, (double)t[p], st);
+      sxx = __fma_rn(wx, dx, sxx);
+      syy = __fma_rn(wy, dy, syy);
+      sxy = __fma_rn(wx, dy, sxy);
       qm = fmaxf(qm, qp);
     }
-  }
-  double s0 = rw[0], sx = rw[0] * rx[0], sy = rw[0] * ry[0], st = rw[0] * rt[0];
-  s0 += rw[1], sx += rw[1] * rx[1], sy += rw[1] * ry[1], st += rw[1] * rt[1];
-  for (int i = lane + 64; i < n_pix; i += 32) {
-    const int p = sc.list[i];
-    const float qp = q[p];
-    const double w = (double)qp;
-    s0 += w;
-    sx += w * (double)__ldg(cam.pix_x + p);
-    sy += w * (double)__ldg(cam.pix_y + p);
-    st += w * (double)t[p];
-    qm = fmaxf(qm, qp);
-  }
-  s0 = warp_sum(s0), sx = warp_sum(sx), sy = warp_sum(sy), st = warp_sum(st);
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) qm = fmaxf(qm, __shfl_xor_sync(0xFFFFFFFFu, qm, o));
-  if (!(s0 > 0.0)) {  // non-positive (or NaN) total charge: parameters are zero, the count stands
-    if (lane == 8) out.n_pix[e] = n_pix;
-    if (lane < 8) out.params[(size_t)e * 8u + lane] = 0.0f;
-    return;
+    for (int o = 16; o > 0; o >>= 1) {
+      s0 = __dadd_rn(s0, shfl_xor_f64(s0, o));
+      sx = __dadd_rn(sx, shfl_xor_f64(sx, o));
+      sy = __dadd_rn(sy, shfl_xor_f64(sy, o));
+      st = __dadd_rn(st, shfl_xor_f64(st, o));
+      sxx = __dadd_rn(sxx, shfl_xor_f64(sxx, o));
+      syy = __dadd_rn(syy, shfl_xor_f64(syy, o));
+      sxy = __dadd_rn(sxy, shfl_xor_f64(sxy, o));
+      qm = fmaxf(qm, __shfl_xor_sync(0xFFFFFFFFu, qm, o));
+    }
+    cur.s0 = s0, cur.sx = sx, cur.sy = sy, cur.st = st;
+    cur.sxx = sxx, cur.syy = syy, cur.sxy = sxy;
+    cur.x0 = x0, cur.y0 = y0, cur.qm = qm;
+    cur.n_pix = n_pix;
+  } else if (mrow) {  // no surviving core pixel: the mask is empty
+    for (int p = lane; p < P; p += 32) mrow[p] = 0;
   }
-  // one division for three quotients: lane 0, 1, 2 divide sx, sy, st by s0
-  const double r1 = (lane == 0 ? sx : lane == 1 ? sy : st) / s0;
-  const double cx = bcast(r1, 0), cy = bcast(r1, 1), tm = bcast(r1, 2);
-
-  // pass 2: centred second moments
-  double sxx = 0.0, syy = 0.0, sxy = 0.0;
-#pragma unroll
-  for (int u = 0; u < 2; ++u) {  // entries past n_pix carry zero weight
-    const double dx = rx[u] - cx, dy = ry[u] - cy;
-    sxx += rw[u] * dx * dx;
-    syy += rw[u] * dy * dy;
-    sxy += rw[u] * dx * dy;
-  }
-  for (int i = lane + 64; i < n_pix; i += 32) {
-    const int p = sc.list[i];
-    const double w = (double)q[p];
-    const double dx = (double)__ldg(cam.pix_x + p) - cx, dy = (double)__ldg(cam.pix_y + p) - cy;
-    sxx += w * dx * dx;
-    syy += w * dy * dy;
-    sxy += w * dx * dy;
-  }
-  sxx = warp_sum(sxx), syy = warp_sum(syy), sxy = warp_sum(sxy);
-  const double r2 = (lane == 0 ? sxx : lane == 1 ? syy : sxy) / s0;
-  sxx = bcast(r2, 0), syy = bcast(r2, 1), sxy = bcast(r2, 2);
-  const double d = sxx - syy;
-  const double z = sqrt(d * d + 4.0 * sxy * sxy);
-  // one square root for length (lane 3) and width (lane 4)
-  const double r3 = sqrt(lane == 3 ? 0.5 * (sxx + syy + z) : fmax(0.5 * (sxx + syy - z), 0.0));
-  const double psi = 0.5 * atan2(2.0 * sxy, d);
-  const double v = lane == 0 ? s0 : lane == 1 ? cx : lane == 2 ? cy : lane == 5 ? psi
-                 : lane == 6 ? tm : r3;
-  if (lane < 7) out.params[(size_t)e * 8u + lane] = (float)v;
-  if (lane == 7) out.params[(size_t)e * 8u + 7u] = qm;
-  if (lane == 8) out.n_pix[e] = n_pix;
+  if (lane == n_pend) pd = cur;
+  if (++n_pend == 32) flush_pending(pd, n_pend, out);
 }
 
 // ------------------------------------------------ cleaning on HBM arrays ----
-// One warp per event: the charge row comes in by cp.async into one of two
-// per-warp buffers (the next event's row is in flight while this one is
-// cleaned); peak times stay in HBM and are gathered for the mask pixels only.
-__device__ __forceinline__ void row_async(float* dst, const float* src, const int P) {
-  const int lane = threadIdx.x & 31;
-  int p = 0;
-  if ((reinterpret_cast<uintptr_t>(src) & 15u) == 0) {
-    const int n4 = P >> 2;
-    for (int i = lane; i < n4; i += 32) cp_async16(smem_u32(dst + 4 * i), src + 4 * i);
-    p = 4 * n4;
-  }
-  for (int i = p + lane; i < P; i += 32) cp_async4(smem_u32(dst + i), src + i);
-  asm volatile("cp.async.commit_group;" ::: "memory");
-}
+// One warp per event. The warp sweeps the charge row once with coalesced loads
+// (lane = pixel mod 32, so a ballot is a word of the bit mask) and then cleans
+// with charge / peak time of the few mask pixels gathered from L2. Shared
+// memory per warp: two threshold bit masks and the cleaning scratch only.
+size_t moments_warp_bytes(int32_t P) { return 2u * r16(4u * mask_words(P)) + CleanScratch::bytes(P); }
 
 template <int WARPS>
-__global__ void __launch_bounds__(32 * WARPS)
+__global__ void __launch_bounds__(32 * WARPS, 1)
     image_moments_kernel(const float* __restrict__ charge, const float* __restrict__ time,
                          const uint32_t n_events, const int P,
                          const __grid_constant__ RtaCamera cam,
-                         const __grid_constant__ RtaImageOut out) {
+                         const __grid_constant__ RtaImageOut out, const int force_general) {
   extern __shared__ __align__(128) uint8_t smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const size_t row_bytes = r16(4u * (size_t)P);
-  const size_t per_warp = row_bytes + EventBuf::bytes(P, false) + CleanScratch::bytes(P);
-  uint8_t* mine = smem + (size_t)warp * per_warp;
-  float* rows[2] = {reinterpret_cast<float*>(mine), reinterpret_cast<float*>(mine + row_bytes)};
-  const EventBuf buf(mine + row_bytes, P, false);  // buf.q == rows[1]; only the bit words are used
-  const CleanScratch sc(mine + row_bytes + EventBuf::bytes(P, false), P);
+  const size_t wb = r16(4u * mask_words(P));
+  uint8_t* mine = smem + (size_t)warp * (2u * wb + CleanScratch::bytes(P));
+  uint32_t* core_w = reinterpret_cast<uint32_t*>(mine);
+  uint32_t* low_w = reinterpret_cast<uint32_t*>(mine + wb);
+  const CleanScratch sc(mine + 2u * wb, P);
+  const bool symmetric = table_is_symmetric(cam.neighbors, P) && !force_general;
   const float thr_p = cam.thr_picture, thr_b = cam.thr_boundary;
   const uint32_t stride = gridDim.x * WARPS;
-  uint32_t e = blockIdx.x * WARPS + warp;
-  if (e < n_events) row_async(rows[0], charge + (size_t)e * (size_t)P, P);
-  for (int b = 0; e < n_events; e += stride, b ^= 1) {
-    if (e + stride < n_events) {
-      row_async(rows[b ^ 1], charge + (size_t)(e + stride) * (size_t)P, P);
-      asm volatile("cp.async.wait_group 1;" ::: "memory");
-    } else {
-      asm volatile("cp.async.wait_group 0;" ::: "memory");
+  Pending pd = {};
+  int n_pend = 0;
+  for (uint32_t e = blockIdx.x * WARPS + warp; e < n_events; e += stride) {
+    const float* q = charge + (size_t)e * (size_t)P;
+    constexpr int U = 4;
+    for (int p0 = 0; p0 < P; p0 += 32 * U) {
+      float v[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int p = p0 + 32 * u + lane;
+        v[u] = p < P ? __ldg(q + p) : 0.0f;
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const bool in = p0 + 32 * u + lane < P;
+        const uint32_t c = __ballot_sync(0xFFFFFFFFu, in && v[u] >= thr_p);
+        const uint32_t l = __ballot_sync(0xFFFFFFFFu, in && v[u] >= thr_b);
+        if (lane == 0 && p0 + 32 * u < P) core_w[(p0 >> 5) + u] = c, low_w[(p0 >> 5) + u] = l;
+      }
     }
     __syncwarp();
-    const float* q = rows[b];
-#pragma unroll 4
-    for (int p0 = 0; p0 < P; p0 += 32) {
-      const int p = p0 + lane;
-      const bool in = p < P;
-      const float v = in ? q[p] : 0.0f;
-      const uint32_t c = __ballot_sync(0xFFFFFFFFu, in && v >= thr_p);
-      const uint32_t l = __ballot_sync(0xFFFFFFFFu, in && v >= thr_b);
-      if (lane == 0) buf.core_w[p0 >> 5] = c, buf.low_w[p0 >> 5] = l;
-    }
-    __syncwarp();
-    clean_warp(e, P, q, time + (size_t)e * (size_t)P, buf.core_w, buf.low_w, sc, cam, out);
+    clean_event(e, P, q, time + (size_t)e * (size_t)P, core_w, low_w, sc, cam, out, symmetric, pd,
+                n_pend);
     __syncwarp();
   }
+  flush_pending(pd, n_pend, out);
 }
 
 // ------------------------------------------------- producer / cleaner hand-off ----
-// The fused kernels run NT extraction threads and one cleaning warp (threads
-// NT .. NT+31). Event number k of the CTA uses buffer k & 1. Named barriers
-// (all with NT + 32 participants): READY + b — the extraction threads arrive
-// when the buffer is complete, the cleaning warp waits; FREE + b — the
+// The generic fused kernel runs NT extraction threads and one cleaning warp
+// (threads NT .. NT+31). Event number k of the CTA uses buffer k & 1. Named
+// barriers (all with NT + 32 participants): READY + b — the extraction threads
+// arrive when the buffer is complete, the cleaning warp waits; FREE + b — the
 // cleaning warp arrives when it is done with the buffer, the extraction
 // threads wait before writing event k + 2 into it. ev_id[b] carries the event
 // index (kNoEvent = no more events).
-enum : int { BAR_READY = 1, BAR_FREE = 3, BAR_EXTRACT = 5 };
+enum : int { BAR_READY = 1, BAR_FREE = 3 };
 constexpr uint32_t kNoEvent = 0xFFFFFFFFu;
 
 struct FusedShared {
@@ -364,19 +483,22 @@ struct FusedShared {
 template <int NT>
 __device__ __forceinline__ void cleaner_loop(const int P, uint8_t* ev_base, uint8_t* sc_base,
                                              volatile FusedShared& fs, const RtaCamera& cam,
-                                             const RtaImageOut& out) {
-  const size_t eb = EventBuf::bytes(P, true);
+                                             const RtaImageOut& out, const bool symmetric) {
+  const size_t eb = EventBuf::bytes(P);
   const CleanScratch sc(sc_base, P);
+  Pending pd = {};
+  int n_pend = 0;
   for (uint32_t k = 0;; ++k) {
     const int b = (int)(k & 1u);
     named_sync(BAR_READY + b, NT + 32);
     const uint32_t e = fs.ev_id[b];
     if (e == kNoEvent) break;
-    const EventBuf buf(ev_base + (size_t)b * eb, P, true);
-    clean_warp(e, P, buf.q, buf.t, buf.core_w, buf.low_w, sc, cam, out);
+    const EventBuf buf(ev_base + (size_t)b * eb, P);
+    clean_event(e, P, buf.q, buf.t, buf.core_w, buf.low_w, sc, cam, out, symmetric, pd, n_pend);
     __syncwarp();
     named_arrive(BAR_FREE + b, NT + 32);
   }
+  flush_pending(pd, n_pend, out);
 }
 
 // extraction side: before the first write of the CTA's event number k
@@ -400,13 +522,14 @@ __global__ void __launch_bounds__(NT + 32)
                                  const int P, const int S, const int W,
                                  const int* __restrict__ pedestal, const float* __restrict__ gain,
                                  const __grid_constant__ RtaCamera cam,
-                                 const __grid_constant__ RtaImageOut out) {
+                                 const __grid_constant__ RtaImageOut out, const int force_general) {
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ FusedShared fs;
   const int tid = threadIdx.x, lane = tid & 31;
-  const size_t eb = EventBuf::bytes(P, true);
+  const size_t eb = EventBuf::bytes(P);
+  const bool symmetric = table_is_symmetric(cam.neighbors, P) && !force_general;
   if (tid >= NT) {
-    cleaner_loop<NT>(P, smem, smem + 2u * eb, fs, cam, out);
+    cleaner_loop<NT>(P, smem, smem + 2u * eb, fs, cam, out, symmetric);
     return;
   }
   const ModeArgs ma = {};
@@ -414,7 +537,7 @@ __global__ void __launch_bounds__(NT + 32)
   uint32_t k = 0;
   for (uint32_t e = blockIdx.x; e < n_events; e += gridDim.x, ++k) {
     producer_acquire<NT>(k);
-    const EventBuf buf(smem + (size_t)(k & 1u) * eb, P, true);
+    const EventBuf buf(smem + (size_t)(k & 1u) * eb, P);
     const uint8_t* base = wf + (size_t)e * (size_t)P * (size_t)S * 2u;
     for (int p0 = tid - lane; p0 < P; p0 += NT) {  // whole warps: the ballots need every lane
       const int p = p0 + lane;
@@ -447,84 +570,109 @@ __device__ __forceinline__ uint32_t spread16(uint32_t x) {
 }
 
 // ------------------------------------------- extraction + cleaning, staged ----
-// Work items of a CTA: (event, tile) pairs, tiles 0 .. nt-1 of one event, then
-// the next event drawn from the shared counter. The producer side runs STAGES
-// items ahead of the consumer through item_q, across event boundaries.
-template <class C>
-__global__ void __launch_bounds__(C::NT + 32, C::NT >= 256 ? 3 : 1)
+// One persistent CTA per SM: G extraction groups of NT threads (thread t of
+// group g = thread g NT + t) and up to NCMAX cleaning warps behind them. The
+// CTA's events are e_k = blockIdx.x + k gridDim.x, k = 0, 1, ...; event k is
+// written into buffer k mod NB and cleaned by warp k mod NC. The (event, tile)
+// items of the CTA, in order, are dealt round-robin to the groups: group g
+// takes items g, g + G, ...; every thread derives its group's item sequence
+// arithmetically, so there is no queue. Each group has its own ring of STAGES
+// stages filled by TMA bulk copies (16-byte cp.async for the padded S = 128
+// layout) and its own named barrier.
+//   full[g][s]  the stage's bytes have landed (TMA complete_tx / cp.async arrive)
+//   ready[b]    one arrival per extraction warp and tile of the event in buffer b:
+//               nt * NT / 32 arrivals per phase; the cleaning warp waits
+//   freeb[b]    one arrival by the cleaning warp per cleaned event; the extraction
+//               threads wait before the first write of event k >= NB
+constexpr int kMaxBuf = 8;
+
+template <class C, int G, int NCMAX>
+__global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
     extract_image_kernel(const uint8_t* __restrict__ wf, const uint32_t n_events, const int P,
                          const int* __restrict__ pedestal, const float* __restrict__ gain,
                          const __grid_constant__ RtaCamera cam,
-                         const __grid_constant__ RtaImageOut out, uint32_t* __restrict__ sched) {
+                         const __grid_constant__ RtaImageOut out, const int NB, const int NC,
+                         const int force_general) {
   static_assert(C::BITS == 16 && C::STAGES >= 2, "uint16 samples, at least two stages");
   static_assert(C::TPT == 1 || C::TPT == 2, "one or two traces per thread");
+  static_assert(G >= 1 && G <= 14, "named barriers 1 .. G");
   // an event may start at any multiple of VEC bytes: the copy starts at the
   // 16-byte boundary below it, so a stage holds up to 16 bytes more than a tile
   constexpr int STG = C::STAGE_BYTES + 16;
-  constexpr int NT = C::NT;
+  constexpr int NT = C::NT, NX = G * NT;
   constexpr uint32_t TRACE_BYTES = C::TRACE_BITS / 8;
   extern __shared__ __align__(128) uint8_t smem[];
-  __shared__ __align__(8) uint64_t full_bar[C::STAGES];
-  constexpr int QN = C::STAGES + 1;
-  __shared__ uint2 item_q[QN];  // {event, tile}
-  __shared__ FusedShared fs;
+  __shared__ __align__(8) uint64_t full_bar[G * C::STAGES];
+  __shared__ __align__(8) uint64_t ready_bar[kMaxBuf];
+  __shared__ __align__(8) uint64_t free_bar[kMaxBuf];
   const int tid = threadIdx.x, lane = tid & 31;
-  const uint32_t smem_base = smem_u32(smem);
-  const uint32_t bar_base = smem_u32(full_bar);
-  uint8_t* ev_base = smem + C::STAGES * STG;
-  const size_t eb = EventBuf::bytes(P, true);
-  const ModeArgs ma = {};
   const uint32_t nt = ((uint32_t)P + C::TILE_TRACES - 1u) / C::TILE_TRACES;  // tiles per event
-  const unsigned long long EB = (unsigned long long)P * TRACE_BYTES;         // bytes per event
-  const unsigned long long total = (unsigned long long)n_events * EB;
-  const float thr_p = cam.thr_picture, thr_b = cam.thr_boundary;
-
-  // thread 0: the producer cursor (pev, pt) and one prefetched event index
-  uint32_t pev = blockIdx.x, pt = 0, pre_ev = kNoEvent;
-  auto fetch_event = [&]() -> uint32_t {
-    if (sched == nullptr) return (pev > kNoEvent - gridDim.x) ? kNoEvent : pev + gridDim.x;
-    const uint32_t got = pre_ev;
-    const uint32_t k = atomicAdd(sched, 1u);
-    pre_ev = (k > kNoEvent - gridDim.x) ? kNoEvent : gridDim.x + k;
-    return got;
-  };
-  auto next_item = [&]() -> uint2 {
-    const uint2 it = make_uint2(pev, pt);
-    if (pev < n_events && ++pt == nt) {
-      pt = 0;
-      pev = fetch_event();
-    }
-    return it;
-  };
+  uint8_t* ev_base = smem + (size_t)G * C::STAGES * STG;
+  const size_t eb = EventBuf::bytes(P);
+  const uint32_t ready0 = smem_u32(ready_bar), free0 = smem_u32(free_bar);
 
   if (tid == 0) {
-    if (sched != nullptr) {
-      const uint32_t k = atomicAdd(sched, 1u);
-      pre_ev = (k > kNoEvent - gridDim.x) ? kNoEvent : gridDim.x + k;
-    }
 #pragma unroll
-    for (int s = 0; s < C::STAGES; ++s) {
-      mbar_init(bar_base + 8 * s, C::PAD ? NT : 1);
-      item_q[s] = next_item();
+    for (int s = 0; s < G * C::STAGES; ++s) mbar_init(smem_u32(full_bar) + 8 * s, C::PAD ? NT : 1);
+    for (int b = 0; b < NB; ++b) {
+      mbar_init(ready0 + 8 * b, nt * (NT / 32));
+      mbar_init(free0 + 8 * b, 1);
     }
     fence_mbar_init();
   }
   __syncthreads();
-  if (tid >= NT) {  // the cleaning warp
-    cleaner_loop<NT>(P, ev_base, ev_base + 2u * eb, fs, cam, out);
+  const auto event_of = [&](const uint32_t k) -> unsigned long long {
+    return (unsigned long long)blockIdx.x + (unsigned long long)k * gridDim.x;
+  };
+
+  if (tid >= NX) {  // ------------------------------------------------ cleaning warps
+    const bool symmetric = table_is_symmetric(cam.neighbors, P) && !force_general;
+    const int c = (tid - NX) >> 5;
+    if (c >= NC) return;
+    const CleanScratch sc(ev_base + (size_t)NB * eb + (size_t)c * CleanScratch::bytes(P), P);
+    Pending pd = {};
+    int n_pend = 0;
+    for (uint32_t k = (uint32_t)c; event_of(k) < n_events; k += (uint32_t)NC) {
+      const uint32_t b = k % (uint32_t)NB, use = k / (uint32_t)NB;
+      mbar_wait(ready0 + 8 * b, use & 1u);
+      const EventBuf buf(ev_base + (size_t)b * eb, P);
+      clean_event((uint32_t)event_of(k), P, buf.q, buf.t, buf.core_w, buf.low_w, sc, cam, out,
+                  symmetric, pd, n_pend);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(free0 + 8 * b);
+    }
+    flush_pending(pd, n_pend, out);
     return;
   }
 
-  auto issue = [&](const uint2 it, const int stage) {
-    const unsigned long long start = (unsigned long long)it.x * EB +
-                                     (unsigned long long)it.y * C::TILE_BYTES;
-    const uint32_t left = (uint32_t)P - it.y * C::TILE_TRACES;
+  // ---------------------------------------------------------------- extraction groups
+  const int g = tid / NT, gt = tid - g * NT;
+  const uint32_t ring = smem_u32(smem) + (uint32_t)(g * C::STAGES * STG);
+  uint8_t* ringp = smem + (size_t)g * C::STAGES * STG;
+  const uint32_t bar_base = smem_u32(full_bar) + 8u * (uint32_t)(g * C::STAGES);
+  const ModeArgs ma = {};
+  const unsigned long long EB = (unsigned long long)P * TRACE_BYTES;  // bytes per event
+  const unsigned long long total = (unsigned long long)n_events * EB;
+  const float thr_p = cam.thr_picture, thr_b = cam.thr_boundary;
+
+  // item cursor (k, tile): advance by G items
+  const auto advance = [&](uint32_t& k, uint32_t& tile) {
+    tile += (uint32_t)G;
+    while (tile >= nt) {
+      tile -= nt;
+      ++k;
+    }
+  };
+  const auto issue = [&](const uint32_t ev, const uint32_t tile, const int stage) {
+    const unsigned long long start = (unsigned long long)ev * EB +
+                                     (unsigned long long)tile * C::TILE_BYTES;
+    const uint32_t left = (uint32_t)P - tile * C::TILE_TRACES;
     const uint32_t n = left < (uint32_t)C::TILE_TRACES ? left : (uint32_t)C::TILE_TRACES;
     const uint32_t bytes = n * TRACE_BYTES;
-    const uint32_t dst = smem_base + stage * STG;
+    const uint32_t dst = ring + stage * STG;
     const uint32_t bar = bar_base + 8 * stage;
     if constexpr (!C::PAD) {
-      if (tid == 0) {
+      if (gt == 0) {
         const uint32_t mis = (uint32_t)(start & 15u);
         const unsigned long long lo = start - mis;
         uint32_t len = (mis + bytes + 15u) & ~15u;
@@ -532,7 +680,7 @@ __global__ void __launch_bounds__(C::NT + 32, C::NT >= 256 ? 3 : 1)
           // the last tile of the last event: nothing past the caller's buffer
           // is read; the final < 16 bytes go halfword by halfword
           len = (uint32_t)((total - lo) & ~15ull);
-          uint8_t* d = smem + stage * STG;
+          uint8_t* d = ringp + stage * STG;
           for (uint32_t b = len; b < mis + bytes; b += 2u)
             *reinterpret_cast<uint16_t*>(d + b) = *reinterpret_cast<const uint16_t*>(wf + lo + b);
         }
@@ -543,7 +691,7 @@ __global__ void __launch_bounds__(C::NT + 32, C::NT >= 256 ? 3 : 1)
       // S = 128: events start on 16-byte boundaries (256-byte traces)
       const uint8_t* src = wf + start;
 #pragma unroll 4
-      for (uint32_t c = tid; c < bytes / 16u; c += NT) {
+      for (uint32_t c = gt; c < bytes / 16u; c += NT) {
         const uint32_t u = c / C::NVEC;  // one extra chunk of padding per unit
         cp_async16(dst + (c + u) * 16u, src + (size_t)c * 16u);
       }
@@ -551,31 +699,50 @@ __global__ void __launch_bounds__(C::NT + 32, C::NT >= 256 ? 3 : 1)
     }
   };
 
+  // consumer cursor = item g; the producer cursor runs STAGES items ahead
+  uint32_t k = 0, tile = 0;
+  {
+    uint32_t first = (uint32_t)g;
+    while (first >= nt) {
+      first -= nt;
+      ++k;
+    }
+    tile = first;
+  }
+  uint32_t pk = k, ptile = tile;
 #pragma unroll
   for (int s = 0; s < C::STAGES; ++s) {
-    const uint2 it = item_q[s];
-    if (it.x < n_events) issue(it, s);
+    if (event_of(pk) < n_events) issue((uint32_t)event_of(pk), ptile, s);
+    advance(pk, ptile);
   }
+  // the table check overlaps the first loads (its __syncthreads pairs with the cleaning warps')
+  table_is_symmetric(cam.neighbors, P);
 
-  uint32_t k = 0;  // events of this CTA so far
+  uint32_t cur_k = 0xFFFFFFFFu, b = 0;
+  uint8_t* bufp = ev_base;
   for (uint32_t j = 0;; ++j) {
-    const uint2 it = item_q[j % QN];
-    if (it.x >= n_events) break;  // event indices grow per CTA: nothing later is valid either
+    const unsigned long long ev = event_of(k);
+    if (ev >= n_events) break;
     const int stage = (int)(j % C::STAGES);
     const uint32_t parity = (j / C::STAGES) & 1u;
-    if (tid == 0) item_q[(j + C::STAGES) % QN] = next_item();
-    if (it.y == 0) producer_acquire<NT>(k);
-    const EventBuf buf(ev_base + (size_t)(k & 1u) * eb, P, true);
+    if (k != cur_k) {  // first tile of this group in event k: the buffer must be free
+      cur_k = k;
+      b = k % (uint32_t)NB;
+      bufp = ev_base + (size_t)b * eb;
+      if (k >= (uint32_t)NB) mbar_wait(free0 + 8 * b, (k / (uint32_t)NB - 1u) & 1u);
+    }
+    const EventBuf buf(bufp, P);
     mbar_wait(bar_base + 8 * stage, parity);
-    const uint32_t p0 = it.y * C::TILE_TRACES + (uint32_t)tid * C::TPT;
+    const uint32_t p0 = tile * C::TILE_TRACES + (uint32_t)gt * C::TPT;
     float qv[C::TPT];
 #pragma unroll
     for (int i = 0; i < C::TPT; ++i) qv[i] = 0.0f;
-    if (p0 < (uint32_t)P) {
+    const bool in = p0 < (uint32_t)P;
+    if (in) {
       uint32_t mis = 0;
       if constexpr (!C::PAD)
-        mis = (uint32_t)(((unsigned long long)it.x * EB + (unsigned long long)it.y * C::TILE_BYTES) & 15u);
-      const uint8_t* unit = smem + stage * STG + mis + tid * C::UNIT_STRIDE;
+        mis = (uint32_t)((ev * EB + (unsigned long long)tile * C::TILE_BYTES) & 15u);
+      const uint8_t* unit = ringp + stage * STG + mis + gt * C::UNIT_STRIDE;
       Result res[C::TPT];
       compute_results<C, MODE_SLIDING>(unit, p0, 0u, pedestal, gain, ma, res);
 #pragma unroll
@@ -585,8 +752,7 @@ __global__ void __launch_bounds__(C::NT + 32, C::NT >= 256 ? 3 : 1)
       }
     }
     // threshold bits of this warp's 32 * TPT pixels (warps past the camera's end write nothing)
-    const uint32_t w0 = (it.y * C::TILE_TRACES + (uint32_t)(tid - lane) * C::TPT) >> 5;
-    const bool in = p0 < (uint32_t)P;
+    const uint32_t w0 = (tile * C::TILE_TRACES + (uint32_t)(gt - lane) * C::TPT) >> 5;
     if constexpr (C::TPT == 1) {
       const uint32_t c = __ballot_sync(0xFFFFFFFFu, in && qv[0] >= thr_p);
       const uint32_t l = __ballot_sync(0xFFFFFFFFu, in && qv[0] >= thr_b);
@@ -606,148 +772,143 @@ __global__ void __launch_bounds__(C::NT + 32, C::NT >= 256 ? 3 : 1)
         }
       }
     }
-    named_sync(BAR_EXTRACT, NT);  // the stage is free, the item slot is published
-    const uint2 nxt = item_q[(j + C::STAGES) % QN];
-    if (nxt.x < n_events) issue(nxt, stage);
-    if (it.y + 1u == nt) {
-      producer_release<NT>(k, it.x, fs, tid == 0);
-      ++k;
-    }
-  }
-  producer_acquire<NT>(k);
-  producer_release<NT>(k, kNoEvent, fs, tid == 0);
-
-  if (sched != nullptr && tid == 0) {
-    __threadfence();
-    if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) {
-      sched[0] = 0;
-      sched[1] = 0;
-      __threadfence();
-    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(ready0 + 8 * b);  // release: this warp's share of the tile is in the buffer
+    named_sync(1 + g, NT);                       // every thread of the group is done with the stage
+    if (event_of(pk) < n_events) issue((uint32_t)event_of(pk), ptile, stage);
+    advance(pk, ptile);
+    advance(k, tile);
   }
 }
 
 // ------------------------------------------------------------- dispatch ----
 constexpr int kGenericNT = 256;
 constexpr size_t kSmemLimit = 227u * 1024u;
+std::atomic<bool> g_general_cleaning{false};  // tests: never take the symmetric-table shortcut
 
+// Staged fused kernels of the four config shapes: threads per group, stages
+// per group (TileCfg), groups, cleaning warps (tuned on B200).
 #ifndef RTA_I30_NT
-#define RTA_I30_NT 256
+#define RTA_I30_NT 128
 #endif
-#ifndef RTA_I30_ST
-#define RTA_I30_ST 2
+#ifndef RTA_I30_G
+#define RTA_I30_G 5
 #endif
 #ifndef RTA_I40_NT
-#define RTA_I40_NT 256
+#define RTA_I40_NT 128
 #endif
-#ifndef RTA_I40_ST
-#define RTA_I40_ST 2
+#ifndef RTA_I40_G
+#define RTA_I40_G 5
 #endif
 #ifndef RTA_I25_NT
-#define RTA_I25_NT 256
+#define RTA_I25_NT 128
 #endif
-#ifndef RTA_I25_ST
-#define RTA_I25_ST 2
+#ifndef RTA_I25_G
+#define RTA_I25_G 5
 #endif
 #ifndef RTA_I128_NT
 #define RTA_I128_NT 64
 #endif
-#ifndef RTA_I128_ST
-#define RTA_I128_ST 2
+#ifndef RTA_I128_G
+#define RTA_I128_G 5
 #endif
-using ImgS30W7 = TileCfg<30, 7, RTA_I30_NT, RTA_I30_ST>;
-using ImgS40W7 = TileCfg<40, 7, RTA_I40_NT, RTA_I40_ST>;
-using ImgS25W4 = TileCfg<25, 4, RTA_I25_NT, RTA_I25_ST>;
-using ImgS128W8 = TileCfg<128, 8, RTA_I128_NT, RTA_I128_ST>;
+#ifndef RTA_IMG_NC
+#define RTA_IMG_NC 3
+#endif
+#ifndef RTA_I128_NC
+#define RTA_I128_NC 2
+#endif
+template <class C_, int G_, int NCMAX_>
+struct ImgCfg {
+  using C = C_;
+  static constexpr int G = G_, NCMAX = NCMAX_;
+  static constexpr int THREADS = G * C::NT + 32 * NCMAX;
+  static constexpr size_t RING = (size_t)G * C::STAGES * (C::STAGE_BYTES + 16);
+  static_assert(THREADS <= 1024, "one CTA");
+};
+using ImgS30W7 = ImgCfg<TileCfg<30, 7, RTA_I30_NT, 2>, RTA_I30_G, RTA_IMG_NC>;
+using ImgS40W7 = ImgCfg<TileCfg<40, 7, RTA_I40_NT, 2>, RTA_I40_G, RTA_IMG_NC>;
+using ImgS25W4 = ImgCfg<TileCfg<25, 4, RTA_I25_NT, 2>, RTA_I25_G, RTA_IMG_NC>;
+using ImgS128W8 = ImgCfg<TileCfg<128, 8, RTA_I128_NT, 2>, RTA_I128_G, RTA_I128_NC>;
 
-// shared memory of one warp of image_moments_kernel: two charge rows, bit words, scratch
-size_t moments_warp_bytes(int32_t P) {
-  return r16(4u * (size_t)P) + EventBuf::bytes(P, false) + CleanScratch::bytes(P);
-}
-
-// shared memory of the fused kernels behind the stage ring: two event buffers
-// and the cleaning warp's scratch
-size_t fused_image_bytes(int32_t P) {
-  return 2u * EventBuf::bytes(P, true) + CleanScratch::bytes(P);
+// Cleaning warps NC and event buffers NB = NC + 1 that fit behind the ring
+// (0 = not even one warp and two buffers fit).
+template <class I>
+int fused_cleaners(int32_t P) {
+  for (int nc = I::NCMAX; nc >= 1; --nc) {
+    const size_t need = I::RING + (size_t)(nc + 1) * EventBuf::bytes(P) +
+                        (size_t)nc * CleanScratch::bytes(P) + 1024u;
+    if (need <= kSmemLimit) return nc;
+  }
+  return 0;
 }
 
 // The staged kernel takes a shape when every event starts on a boundary its
 // units can be read from (VEC bytes; whole units per event) and the per-event
 // buffers fit behind the ring.
-template <class C>
+template <class I>
 bool staged_ok(int32_t P) {
+  using C = typename I::C;
   const size_t eb = (size_t)P * (C::TRACE_BITS / 8);
   if (P % C::TPT != 0 || eb % C::VEC != 0) return false;
   if (C::PAD && eb % 16 != 0) return false;
-  return C::STAGES * (size_t)(C::STAGE_BYTES + 16) + fused_image_bytes(P) + 1024u <= kSmemLimit;
+  return fused_cleaners<I>(P) >= 1;
 }
 
-template <class C>
+template <class I>
 struct FusedLauncher {
   static cudaError_t launch(const uint8_t* wf, uint32_t n_events, int32_t P,
                             const int32_t* pedestal, const float* gain, const RtaCamera& cam,
                             const RtaImageOut& out, cudaStream_t stream) {
+    using C = typename I::C;
     int dev = 0, sms = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if ((e = rta_device_sms(dev, &sms)) != cudaSuccess) return e;
-    const size_t smem = C::STAGES * (size_t)(C::STAGE_BYTES + 16) + fused_image_bytes(P);
+    const int nc = fused_cleaners<I>(P);
+    int nb = nc + 1;
+    size_t smem = I::RING + (size_t)nb * EventBuf::bytes(P) + (size_t)nc * CleanScratch::bytes(P);
+    // one more buffer when there is room: the extraction groups run further ahead
+    if (nb + 1 <= kMaxBuf && smem + EventBuf::bytes(P) + 1024u <= kSmemLimit) {
+      ++nb;
+      smem += EventBuf::bytes(P);
+    }
+    auto kernel = extract_image_kernel<C, I::G, I::NCMAX>;
     // the dynamic shared-memory size depends on n_pixels: set per launch (cheap)
-    e = cudaFuncSetAttribute(extract_image_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)smem);
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    int occ = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, extract_image_kernel<C>, C::NT + 32,
-                                                      smem);
-    if (e != cudaSuccess) return e;
-    if (occ < 1) return cudaErrorLaunchOutOfResources;
-    uint32_t grid = (uint32_t)(sms * occ);
+    uint32_t grid = (uint32_t)sms;
     if (grid > n_events) grid = n_events;
-    uint32_t* sched = rta_static_schedule() ? nullptr : rta_sched_words(dev, stream);
-    extract_image_kernel<C><<<grid, C::NT + 32, smem, stream>>>(wf, n_events, P, pedestal, gain,
-                                                                cam, out, sched);
+    kernel<<<grid, I::THREADS, smem, stream>>>(wf, n_events, P, pedestal, gain, cam, out, nb, nc,
+                                               g_general_cleaning.load() ? 1 : 0);
     rta_count_launch();
     return cudaGetLastError();
   }
 };
 
-// grid = every CTA the device holds at once (or one per `per_cta` events)
-template <class K>
-cudaError_t resident_grid(K kernel, int threads, size_t smem, uint32_t n_events, uint32_t per_cta,
-                          uint32_t* grid_out) {
+template <int WARPS>
+cudaError_t launch_moments(const float* charge, const float* time, uint32_t n_events, int32_t P,
+                           const RtaCamera& cam, const RtaImageOut& out, cudaStream_t stream) {
   int dev = 0, sms = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if ((e = rta_device_sms(dev, &sms)) != cudaSuccess) return e;
-  if (smem + 1024u > kSmemLimit) return cudaErrorInvalidValue;
-  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  int occ = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem);
-  if (e != cudaSuccess) return e;
-  if (occ < 1) return cudaErrorLaunchOutOfResources;
-  uint32_t grid = (uint32_t)(sms * occ);
-  const uint32_t need = (n_events + per_cta - 1u) / per_cta;
-  if (grid > need) grid = need;
-  *grid_out = grid;
-  return cudaSuccess;
-}
-
-template <int WARPS>
-cudaError_t launch_moments(const float* charge, const float* time, uint32_t n_events, int32_t P,
-                           const RtaCamera& cam, const RtaImageOut& out, cudaStream_t stream) {
   const size_t smem = WARPS * moments_warp_bytes(P);
-  uint32_t grid = 0;
-  cudaError_t e =
-      resident_grid(image_moments_kernel<WARPS>, 32 * WARPS, smem, n_events, WARPS, &grid);
+  e = cudaFuncSetAttribute(image_moments_kernel<WARPS>,
+                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  image_moments_kernel<WARPS><<<grid, 32 * WARPS, smem, stream>>>(charge, time, n_events, P, cam,
-                                                                 out);
+  uint32_t grid = (uint32_t)sms;  // one CTA per SM (launch bounds)
+  const uint32_t need = (n_events + WARPS - 1u) / WARPS;
+  if (grid > need) grid = need;
+  image_moments_kernel<WARPS><<<grid, 32 * WARPS, smem, stream>>>(
+      charge, time, n_events, P, cam, out, g_general_cleaning.load() ? 1 : 0);
   rta_count_launch();
   return cudaGetLastError();
 }
 
 }  // namespace
+
+void rta_set_general_cleaning(bool on) { g_general_cleaning.store(on); }
 
 int32_t rta_image_pixel_limit() {
   // two event buffers (charge, time, two bit masks) and the cleaning warp's
@@ -770,14 +931,14 @@ cudaError_t rta_launch_image_moments(const float* charge, const float* time, int
                                      int32_t n_pixels, const RtaCamera& cam,
                                      const RtaImageOut& out, cudaStream_t stream) {
   if (n_events <= 0) return cudaSuccess;
-  // as many warps per CTA as keep two CTAs per SM resident
+  // as many warps as one CTA's shared memory holds, up to 24 (85 registers per thread)
   const size_t per_warp = moments_warp_bytes(n_pixels);
-  const size_t half = (kSmemLimit - 2048u) / 2u;
+  const size_t room = kSmemLimit - 2048u;
   const uint32_t E = (uint32_t)n_events;
-  if (8u * per_warp <= half) return launch_moments<8>(charge, time, E, n_pixels, cam, out, stream);
-  if (4u * per_warp <= half) return launch_moments<4>(charge, time, E, n_pixels, cam, out, stream);
-  if (2u * per_warp <= half) return launch_moments<2>(charge, time, E, n_pixels, cam, out, stream);
-  return launch_moments<1>(charge, time, E, n_pixels, cam, out, stream);
+  if (24u * per_warp <= room) return launch_moments<24>(charge, time, E, n_pixels, cam, out, stream);
+  if (16u * per_warp <= room) return launch_moments<16>(charge, time, E, n_pixels, cam, out, stream);
+  if (8u * per_warp <= room) return launch_moments<8>(charge, time, E, n_pixels, cam, out, stream);
+  return launch_moments<4>(charge, time, E, n_pixels, cam, out, stream);
 }
 
 cudaError_t rta_launch_extract_image(const void* wf, int64_t n_events, int32_t n_pixels,
@@ -788,7 +949,7 @@ cudaError_t rta_launch_extract_image(const void* wf, int64_t n_events, int32_t n
   const uint8_t* w = static_cast<const uint8_t*>(wf);
   if (!force_generic && ((uintptr_t)wf % 16) == 0) {
 #define RTA_TRY(CFG)                                                                     \
-  if (S == CFG::S && W == CFG::W && staged_ok<CFG>(n_pixels))                            \
+  if (S == CFG::C::S && W == CFG::C::W && staged_ok<CFG>(n_pixels))                      \
     return FusedLauncher<CFG>::launch(w, (uint32_t)n_events, n_pixels, pedestal, gain,   \
                                       cam, out, stream);
     RTA_TRY(ImgS30W7)
@@ -797,13 +958,24 @@ cudaError_t rta_launch_extract_image(const void* wf, int64_t n_events, int32_t n
     RTA_TRY(ImgS128W8)
 #undef RTA_TRY
   }
-  const size_t smem = fused_image_bytes(n_pixels);
-  uint32_t grid = 0;
-  cudaError_t e = resident_grid(extract_image_generic_kernel<kGenericNT>, kGenericNT + 32, smem,
-                                (uint32_t)n_events, 1u, &grid);
+  const size_t smem = 2u * EventBuf::bytes(n_pixels) + CleanScratch::bytes(n_pixels);
+  if (smem + 1024u > kSmemLimit) return cudaErrorInvalidValue;
+  int dev = 0, sms = 0;
+  cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
-  extract_image_generic_kernel<kGenericNT><<<grid, kGenericNT + 32, smem, stream>>>(
-      w, (uint32_t)n_events, n_pixels, S, W, pedestal, gain, cam, out);
+  if ((e = rta_device_sms(dev, &sms)) != cudaSuccess) return e;
+  auto kernel = extract_image_generic_kernel<kGenericNT>;
+  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  int occ = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, kGenericNT + 32, smem);
+  if (e != cudaSuccess) return e;
+  if (occ < 1) return cudaErrorLaunchOutOfResources;
+  uint32_t grid = (uint32_t)(sms * occ);
+  if (grid > (uint32_t)n_events) grid = (uint32_t)n_events;
+  kernel<<<grid, kGenericNT + 32, smem, stream>>>(w, (uint32_t)n_events, n_pixels, S, W, pedestal,
+                                                  gain, cam, out,
+                                                  g_general_cleaning.load() ? 1 : 0);
   rta_count_launch();
   return cudaGetLastError();
 }

@@ -81,6 +81,9 @@ cudaError_t rta_launch_extract_image(const void* wf, int64_t n_events, int32_t n
                                      const float* gain, int32_t W, const RtaCamera& cam,
                                      const RtaImageOut& out, cudaStream_t stream,
                                      bool force_generic);
+// Tests: never take the symmetric-neighbour-table shortcut of the cleaning (both
+// ways give the same mask on a symmetric table).
+void rta_set_general_cleaning(bool on);
 int32_t rta_image_pixel_limit();  // charge, time and flags of one event must fit one CTA
 const char* rta_pick_image_kernel_name(int32_t n_pixels, int32_t n_samples, int32_t W,
                                        bool aligned16);
