@@ -56,6 +56,23 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 
+// wait with back-off: for warps that are idle most of the time (the spin of
+// mbar_wait would take issue slots from the extraction warps)
+__device__ __forceinline__ void mbar_wait_idle(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  for (;;) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (ok) break;
+    __nanosleep(256);
+  }
+}
+
 __host__ __device__ constexpr size_t r16(size_t n) { return (n + 15u) & ~(size_t)15u; }
 __host__ __device__ constexpr size_t mask_words(int P) { return ((size_t)P + 31u) >> 5; }
 
@@ -559,16 +576,6 @@ __global__ void __launch_bounds__(NT + 32)
   producer_release<NT>(k, kNoEvent, fs, tid == 0);
 }
 
-// 16 bits -> the even bit positions of 32 bits
-__device__ __forceinline__ uint32_t spread16(uint32_t x) {
-  x &= 0xFFFFu;
-  x = (x | (x << 8)) & 0x00FF00FFu;
-  x = (x | (x << 4)) & 0x0F0F0F0Fu;
-  x = (x | (x << 2)) & 0x33333333u;
-  x = (x | (x << 1)) & 0x55555555u;
-  return x;
-}
-
 // ------------------------------------------- extraction + cleaning, staged ----
 // One persistent CTA per SM: G extraction groups of NT threads (thread t of
 // group g = thread g NT + t) and up to NCMAX cleaning warps behind them. The
@@ -585,6 +592,7 @@ __device__ __forceinline__ uint32_t spread16(uint32_t x) {
 //   freeb[b]    one arrival by the cleaning warp per cleaned event; the extraction
 //               threads wait before the first write of event k >= NB
 constexpr int kMaxBuf = 8;
+constexpr int kCleanRegs = 152, kExtractRegs = 56;  // after the register split (multiples of 8)
 
 template <class C, int G, int NCMAX>
 __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
@@ -621,11 +629,16 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
     fence_mbar_init();
   }
   __syncthreads();
-  const auto event_of = [&](const uint32_t k) -> unsigned long long {
-    return (unsigned long long)blockIdx.x + (unsigned long long)k * gridDim.x;
-  };
+  // event number k of this CTA. n_events < 2^31 and the walks stop a few items
+  // past the end, so 32 bits hold every index that is formed
+  const auto event_of = [&](const uint32_t k) -> uint32_t { return blockIdx.x + k * gridDim.x; };
+  // Register split (whole warpgroups only): the extraction code needs about 48
+  // registers, the cleaning code about 130; the CTA is launched with the same
+  // number for everyone and the warpgroups trade them here.
+  constexpr bool REGSPLIT = (NX % 128 == 0) && (NCMAX == 4);
 
   if (tid >= NX) {  // ------------------------------------------------ cleaning warps
+    if constexpr (REGSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kCleanRegs));
     const bool symmetric = table_is_symmetric(cam.neighbors, P) && !force_general;
     const int c = (tid - NX) >> 5;
     if (c >= NC) return;
@@ -634,10 +647,10 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
     int n_pend = 0;
     for (uint32_t k = (uint32_t)c; event_of(k) < n_events; k += (uint32_t)NC) {
       const uint32_t b = k % (uint32_t)NB, use = k / (uint32_t)NB;
-      mbar_wait(ready0 + 8 * b, use & 1u);
+      mbar_wait_idle(ready0 + 8 * b, use & 1u);
       const EventBuf buf(ev_base + (size_t)b * eb, P);
-      clean_event((uint32_t)event_of(k), P, buf.q, buf.t, buf.core_w, buf.low_w, sc, cam, out,
-                  symmetric, pd, n_pend);
+      clean_event(event_of(k), P, buf.q, buf.t, buf.core_w, buf.low_w, sc, cam, out, symmetric,
+                  pd, n_pend);
       __syncwarp();
       if (lane == 0) mbar_arrive(free0 + 8 * b);
     }
@@ -646,6 +659,7 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
   }
 
   // ---------------------------------------------------------------- extraction groups
+  if constexpr (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kExtractRegs));
   const int g = tid / NT, gt = tid - g * NT;
   const uint32_t ring = smem_u32(smem) + (uint32_t)(g * C::STAGES * STG);
   uint8_t* ringp = smem + (size_t)g * C::STAGES * STG;
@@ -655,12 +669,17 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
   const unsigned long long total = (unsigned long long)n_events * EB;
   const float thr_p = cam.thr_picture, thr_b = cam.thr_boundary;
 
-  // item cursor (k, tile): advance by G items
-  const auto advance = [&](uint32_t& k, uint32_t& tile) {
-    tile += (uint32_t)G;
-    while (tile >= nt) {
-      tile -= nt;
-      ++k;
+  // item cursor: event number k (kept as its event index ev and its buffer
+  // b = k mod NB, use = k div NB) and tile; advance by G items
+  struct Cursor {
+    uint32_t ev, tile, b, use;
+  };
+  const auto advance = [&](Cursor& c) {
+    c.tile += (uint32_t)G;
+    while (c.tile >= nt) {
+      c.tile -= nt;
+      c.ev += gridDim.x;
+      if (++c.b == (uint32_t)NB) c.b = 0, ++c.use;
     }
   };
   const auto issue = [&](const uint32_t ev, const uint32_t tile, const int stage) {
@@ -700,38 +719,33 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
   };
 
   // consumer cursor = item g; the producer cursor runs STAGES items ahead
-  uint32_t k = 0, tile = 0;
-  {
-    uint32_t first = (uint32_t)g;
-    while (first >= nt) {
-      first -= nt;
-      ++k;
-    }
-    tile = first;
+  Cursor cc = {blockIdx.x, 0u, 0u, 0u};
+  if (g != 0) {  // items 0 .. g-1 belong to the groups before this one
+    cc.tile = (uint32_t)g - (uint32_t)G;
+    advance(cc);
   }
-  uint32_t pk = k, ptile = tile;
+  Cursor pc = cc;
 #pragma unroll
   for (int s = 0; s < C::STAGES; ++s) {
-    if (event_of(pk) < n_events) issue((uint32_t)event_of(pk), ptile, s);
-    advance(pk, ptile);
+    if (pc.ev < n_events) issue(pc.ev, pc.tile, s);
+    advance(pc);
   }
   // the table check overlaps the first loads (its __syncthreads pairs with the cleaning warps')
   table_is_symmetric(cam.neighbors, P);
 
-  uint32_t cur_k = 0xFFFFFFFFu, b = 0;
-  uint8_t* bufp = ev_base;
+  uint32_t cur_ev = 0xFFFFFFFFu;
+  const uint32_t EB32 = (uint32_t)EB;  // low bits are all that the 16-byte phase needs
+  const uint32_t NW = (uint32_t)mask_words(P);
   for (uint32_t j = 0;; ++j) {
-    const unsigned long long ev = event_of(k);
+    const uint32_t ev = cc.ev, tile = cc.tile, b = cc.b;
     if (ev >= n_events) break;
     const int stage = (int)(j % C::STAGES);
     const uint32_t parity = (j / C::STAGES) & 1u;
-    if (k != cur_k) {  // first tile of this group in event k: the buffer must be free
-      cur_k = k;
-      b = k % (uint32_t)NB;
-      bufp = ev_base + (size_t)b * eb;
-      if (k >= (uint32_t)NB) mbar_wait(free0 + 8 * b, (k / (uint32_t)NB - 1u) & 1u);
+    if (ev != cur_ev) {  // first tile of this group in this event: the buffer must be free
+      cur_ev = ev;
+      if (cc.use != 0) mbar_wait(free0 + 8 * b, (cc.use - 1u) & 1u);
     }
-    const EventBuf buf(bufp, P);
+    const EventBuf buf(ev_base + (size_t)b * eb, P);
     mbar_wait(bar_base + 8 * stage, parity);
     const uint32_t p0 = tile * C::TILE_TRACES + (uint32_t)gt * C::TPT;
     float qv[C::TPT];
@@ -740,8 +754,7 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
     const bool in = p0 < (uint32_t)P;
     if (in) {
       uint32_t mis = 0;
-      if constexpr (!C::PAD)
-        mis = (uint32_t)((ev * EB + (unsigned long long)tile * C::TILE_BYTES) & 15u);
+      if constexpr (!C::PAD) mis = (ev * EB32) & 15u;  // TILE_BYTES is a multiple of 16
       const uint8_t* unit = ringp + stage * STG + mis + gt * C::UNIT_STRIDE;
       Result res[C::TPT];
       compute_results<C, MODE_SLIDING>(unit, p0, 0u, pedestal, gain, ma, res);
@@ -756,28 +769,32 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
     if constexpr (C::TPT == 1) {
       const uint32_t c = __ballot_sync(0xFFFFFFFFu, in && qv[0] >= thr_p);
       const uint32_t l = __ballot_sync(0xFFFFFFFFu, in && qv[0] >= thr_b);
-      if (lane == 0 && w0 < mask_words(P)) buf.core_w[w0] = c, buf.low_w[w0] = l;
+      if (lane == 0 && w0 < NW) buf.core_w[w0] = c, buf.low_w[w0] = l;
     } else {
-      const uint32_t c0 = __ballot_sync(0xFFFFFFFFu, in && qv[0] >= thr_p);
-      const uint32_t c1 = __ballot_sync(0xFFFFFFFFu, in && qv[1] >= thr_p);
-      const uint32_t l0 = __ballot_sync(0xFFFFFFFFu, in && qv[0] >= thr_b);
-      const uint32_t l1 = __ballot_sync(0xFFFFFFFFu, in && qv[1] >= thr_b);
-      // lane l holds pixels 2 l and 2 l + 1 of the warp's 64: lanes 0-15 fill word w0, 16-31 word w0 + 1
-      if ((lane & 15) == 0) {
-        const int sh = lane;  // 0 or 16
-        const uint32_t w = w0 + (uint32_t)(lane >> 4);
-        if (w < mask_words(P)) {
-          buf.core_w[w] = spread16(c0 >> sh) | (spread16(c1 >> sh) << 1);
-          buf.low_w[w] = spread16(l0 >> sh) | (spread16(l1 >> sh) << 1);
-        }
+      // lane l holds pixels 2 l and 2 l + 1 of the warp's 64: each half-warp ORs
+      // its lanes' bit pairs into one word (lanes 0-15: word w0, 16-31: w0 + 1)
+      const uint32_t sh = 2u * (uint32_t)(lane & 15);
+      uint32_t cb = 0, lb = 0;
+      if (in) {
+        cb = ((qv[0] >= thr_p ? 1u : 0u) | (qv[1] >= thr_p ? 2u : 0u)) << sh;
+        lb = ((qv[0] >= thr_b ? 1u : 0u) | (qv[1] >= thr_b ? 2u : 0u)) << sh;
+      }
+      const bool hi = (lane & 16) != 0;
+      const uint32_t c_lo = __reduce_or_sync(0xFFFFFFFFu, hi ? 0u : cb);
+      const uint32_t c_hi = __reduce_or_sync(0xFFFFFFFFu, hi ? cb : 0u);
+      const uint32_t l_lo = __reduce_or_sync(0xFFFFFFFFu, hi ? 0u : lb);
+      const uint32_t l_hi = __reduce_or_sync(0xFFFFFFFFu, hi ? lb : 0u);
+      if (lane == 0) {
+        if (w0 < NW) buf.core_w[w0] = c_lo, buf.low_w[w0] = l_lo;
+        if (w0 + 1u < NW) buf.core_w[w0 + 1u] = c_hi, buf.low_w[w0 + 1u] = l_hi;
       }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(ready0 + 8 * b);  // release: this warp's share of the tile is in the buffer
     named_sync(1 + g, NT);                       // every thread of the group is done with the stage
-    if (event_of(pk) < n_events) issue((uint32_t)event_of(pk), ptile, stage);
-    advance(pk, ptile);
-    advance(k, tile);
+    if (pc.ev < n_events) issue(pc.ev, pc.tile, stage);
+    advance(pc);
+    advance(cc);
   }
 }
 
@@ -813,7 +830,7 @@ std::atomic<bool> g_general_cleaning{false};  // tests: never take the symmetric
 #define RTA_I128_G 5
 #endif
 #ifndef RTA_IMG_NC
-#define RTA_IMG_NC 3
+#define RTA_IMG_NC 4
 #endif
 #ifndef RTA_I128_NC
 #define RTA_I128_NC 2
