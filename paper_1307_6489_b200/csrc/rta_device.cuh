@@ -119,7 +119,23 @@ struct ModeArgs {
   int32_t shift;                // MODE_LOCAL_PEAK
   int32_t c0, c1;               // MODE_FIR: sum c[k], sum k c[k]
   int32_t taps[kMaxTaps];       // MODE_FIR
+  // MODE_FIR, every tap in [-128, 127]: tap pair m = (c[2m], c[2m+1]) as two
+  // signed bytes in half (m & 1) of word m >> 1 (a missing last tap is 0), for
+  // one dp2a per two samples on the packed uint16 pairs; fir_packed = 1 selects it
+  uint32_t taps2[kMaxTaps / 4];
+  int32_t fir_packed;
 };
+
+// d = c + a.u16[0] * b.s8[2 hi] + a.u16[1] * b.s8[2 hi + 1]  (SASS IDP.2A)
+template <int HI>
+__device__ __forceinline__ int dp2a_u16_s8(const uint32_t a, const uint32_t b, const int c) {
+  int d;
+  if constexpr (HI)
+    asm("dp2a.hi.u32.s32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  else
+    asm("dp2a.lo.u32.s32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  return d;
+}
 
 __device__ __forceinline__ int clamp_start(const int t, const int S, const int W) {
   return min(max(t, 0), S - W);
@@ -288,17 +304,48 @@ __device__ __forceinline__ void compute_results(const uint8_t* __restrict__ unit
       // response on raw samples (the pedestal shifts every y(t) by the same
       // c0*ped); signed compare, strict '>' scanning upwards = earliest on ties
       int best = 0;
-#pragma unroll
-      for (int k = 0; k < W; ++k) best += ma.taps[k] * (int)RTA_X(w, h0 + k);
       tstar = 0;
+      bool done = false;
+      if constexpr (C::BITS == 16) {
+        if (ma.fir_packed) {
+          // small taps: the register copy already holds sample pairs (x[2i], x[2i+1]);
+          // windows at odd samples use the pairs (x[2i+1], x[2i+2]); one IDP.2A per pair
+          constexpr int KP = (W + 1) / 2, NWD = C::NWORDS;
+          uint32_t wo[NWD];
 #pragma unroll
-      for (int t = 1; t < C::NWIN; ++t) {
-        int y = 0;
+          for (int i = 0; i < NWD; ++i)
+            wo[i] = __funnelshift_r(w[i], i + 1 < NWD ? w[i + 1] : 0u, 16);
 #pragma unroll
-        for (int k = 0; k < W; ++k) y += ma.taps[k] * (int)RTA_X(w, h0 + t + k);
-        if (y > best) {
-          best = y;
-          tstar = t;
+          for (int t = 0; t < C::NWIN; ++t) {
+            int y = 0;
+#pragma unroll
+            for (int m = 0; m < KP; ++m) {
+              const int n = h0 + t + 2 * m;  // first sample of the pair (compile time)
+              const int i = n >> 1;
+              const uint32_t a = i < NWD ? ((n & 1) ? wo[i] : w[i]) : 0u;
+              y = (m & 1) ? dp2a_u16_s8<1>(a, ma.taps2[m >> 1], y)
+                          : dp2a_u16_s8<0>(a, ma.taps2[m >> 1], y);
+            }
+            if (t == 0 || y > best) {
+              best = y;
+              tstar = t;
+            }
+          }
+          done = true;
+        }
+      }
+      if (!done) {
+#pragma unroll
+        for (int k = 0; k < W; ++k) best += ma.taps[k] * (int)RTA_X(w, h0 + k);
+#pragma unroll
+        for (int t = 1; t < C::NWIN; ++t) {
+          int y = 0;
+#pragma unroll
+          for (int k = 0; k < W; ++k) y += ma.taps[k] * (int)RTA_X(w, h0 + t + k);
+          if (y > best) {
+            best = y;
+            tstar = t;
+          }
         }
       }
       rawsum = best;

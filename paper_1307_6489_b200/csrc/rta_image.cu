@@ -809,13 +809,13 @@ std::atomic<bool> g_general_cleaning{false};  // tests: never take the symmetric
 #define RTA_I30_NT 128
 #endif
 #ifndef RTA_I30_G
-#define RTA_I30_G 5
+#define RTA_I30_G 6
 #endif
 #ifndef RTA_I40_NT
 #define RTA_I40_NT 128
 #endif
 #ifndef RTA_I40_G
-#define RTA_I40_G 5
+#define RTA_I40_G 6
 #endif
 #ifndef RTA_I25_NT
 #define RTA_I25_NT 128

@@ -747,10 +747,15 @@ cudaError_t rta_launch_extract(const void* wf, int64_t n_traces64, int32_t n_pix
       return launch_mode<MODE_LOCAL_PEAK>(a, ma);
     case RTA_MODE_FIR: {
       // W == mode->n_taps (checked by the caller)
+      ma.fir_packed = 1;
       for (int k = 0; k < W; ++k) {
-        ma.taps[k] = mode->taps[k];
-        ma.c0 += mode->taps[k];
-        ma.c1 += k * mode->taps[k];
+        const int32_t c = mode->taps[k];
+        ma.taps[k] = c;
+        ma.c0 += c;
+        ma.c1 += k * c;
+        if (c < -128 || c > 127) ma.fir_packed = 0;
+        const int m = k >> 1;  // pair m: byte (k & 1) of half (m & 1) of word m >> 1
+        ma.taps2[m >> 1] |= ((uint32_t)c & 0xFFu) << (16 * (m & 1) + 8 * (k & 1));
       }
       return launch_mode<MODE_FIR>(a, ma);
     }

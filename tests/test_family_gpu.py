@@ -114,6 +114,23 @@ def test_fir_random(S, K, E, P):
         both("fir", wf, ped, gain, taps=taps.astype(np.int32))
 
 
+@pytest.mark.parametrize("S,K", SHAPES)
+@pytest.mark.parametrize("edge", [127, -128, 128, -129, 200])
+def test_fir_tap_range_paths(S, K, edge):
+    """Taps inside [-128, 127] take the packed IDP.2A path of the staged kernels,
+    anything else the int32 multiply-add path; both must match the oracle at the
+    boundary values (few non-zero taps keep S * sum|c| * 65535 < 2^31)."""
+    full = edge > 0
+    rng, wf, ped, gain = _random_case(S, 4, 300, S * 3 + K + abs(edge), full)
+    taps = np.zeros(K, np.int32)
+    taps[0] = edge
+    taps[K - 1] = -3 if edge > 0 else 2
+    if K > 2:
+        taps[K // 2] = 1
+    assert S * 65535 * int(np.abs(taps).sum()) < 2 ** 31
+    both("fir", wf, ped, gain, taps=taps)
+
+
 @pytest.mark.parametrize("S,W", SHAPES)
 def test_fir_all_ones_equals_rta_extract_on_device(S, W):
     import torch
