@@ -452,8 +452,8 @@ def image_leg(cfg, steps, peak, torch, dl0gen, rta):
         moments()
     ev_bytes = EVENT_OUT_BYTES * cfg.n_events
     algo = {"fused": cfg.input_bytes + ev_bytes,
-            "two_calls": cfg.input_bytes + cfg.output_bytes + 8 * cfg.n_traces + ev_bytes,
-            "moments": 8 * cfg.n_traces + ev_bytes}
+            "two_calls": cfg.input_bytes + cfg.output_bytes + 4 * cfg.n_traces + ev_bytes,
+            "moments": 4 * cfg.n_traces + ev_bytes}
     res = {"workload": "%s: %s; hex camera, thresholds %g / %g" % (
         cfg.name, cfg.label, cam[3], cam[4]),
         "kernel": rta.rta_image_kernel_name(cfg.n_pixels, cfg.n_samples, cfg.W, True)}
@@ -724,9 +724,10 @@ def main():
             kname = rta.rta_image_kernel_name(cfg.n_pixels, cfg.n_samples, cfg.W, True)
             bytes_per_trace = 2 * cfg.n_samples + EVENT_OUT_BYTES / cfg.n_pixels
         else:
-            algo_bytes = 8 * cfg.n_traces + ev_bytes
+            # the charge row is read once; peak times are gathered for the mask pixels only
+            algo_bytes = 4 * cfg.n_traces + ev_bytes
             kname = "image_moments"
-            bytes_per_trace = 8 + EVENT_OUT_BYTES / cfg.n_pixels
+            bytes_per_trace = 4 + EVENT_OUT_BYTES / cfg.n_pixels
         avg = summ["ms_avg"]
         summ["algorithmic_GBps"] = algo_bytes / avg / 1e6
         summ["frac_of_measured_hbm"] = algo_bytes / avg / 1e6 / peak

@@ -124,6 +124,10 @@ struct ModeArgs {
   // one dp2a per two samples on the packed uint16 pairs; fir_packed = 1 selects it
   uint32_t taps2[kMaxTaps / 4];
   int32_t fir_packed;
+  // 2^KB of the launched TileCfg, read from the constant bank: the arg-max key
+  // sum * 2^KB + (2^KB - 1 - t) then compiles to one IMAD (fma pipe) instead of
+  // one LEA (alu pipe), which is the pipe these kernels fill first
+  uint32_t key_mul;
 };
 
 // d = c + a.u16[0] * b.s8[2 hi] + a.u16[1] * b.s8[2 hi + 1]  (SASS IDP.2A)
@@ -141,6 +145,15 @@ __device__ __forceinline__ int clamp_start(const int t, const int S, const int W
   return min(max(t, 0), S - W);
 }
 
+#ifndef RTA_KEYMODE_P12
+#define RTA_KEYMODE_P12 1
+#endif
+#ifndef RTA_KEYMODE_P40
+#define RTA_KEYMODE_P40 1
+#endif
+#ifndef RTA_KEYMODE_U16
+#define RTA_KEYMODE_U16 1
+#endif
 // ------------------------------------------------------- tile kernel cfg ----
 // BITS = 16: uint16 samples (include/rta.h rta_extract). BITS = 12: the P12
 // stream of rta_extract_packed12 (readings R25-R27): sample n sits at
@@ -177,6 +190,9 @@ struct TileCfg {
   static constexpr int KB = ilog2_ceil(NWIN);
   static constexpr uint32_t KM = (1u << KB) - 1u;
   static constexpr int PB = ilog2_ceil(S);  // local-peak key: sample index bits
+  // how the arg-max keys are formed (compute_results KEYMUL): tuned per shape on B200
+  static constexpr int KEYMODE = (BITS == 12) ? ((S == 40 || S == 30) ? RTA_KEYMODE_P40 : RTA_KEYMODE_P12)
+                                              : RTA_KEYMODE_U16;
   static constexpr uint32_t XMAX = (BITS == 16) ? 65535u : 4095u;
   static_assert(16 + PB <= 32, "peak key must fit 32 bits");
   static_assert(W >= 1 && W <= S, "window must fit the trace");
@@ -239,7 +255,7 @@ struct WindowReader {
 // Steps a2-a7 for the C::TPT traces of one thread's unit in shared memory.
 // p0: calibration index of the first trace; it wraps to 0 after n_pixels - 1
 // (a uniform batch runs through the camera again; n_pixels = 0 never wraps).
-template <class C, int MODE>
+template <class C, int MODE, int KEYMUL = 0>
 __device__ __forceinline__ void compute_results(const uint8_t* __restrict__ unit,
                                                 const uint32_t p0, const uint32_t n_pixels,
                                                 const int* __restrict__ pedestal,
@@ -287,12 +303,19 @@ __device__ __forceinline__ void compute_results(const uint8_t* __restrict__ unit
       uint32_t sum = 0;
 #pragma unroll
       for (int k = 0; k < W; ++k) sum += RTA_X(w, h0 + k);
-      uint32_t best = (sum << C::KB) | C::KM;
+      // KEYMUL 1: every key by IMAD with the constant-bank multiplier; 2: every other one
+      const auto make_key = [&](const uint32_t s, const int t) -> uint32_t {
+        const uint32_t low = C::KM - (uint32_t)t;
+        if (KEYMUL == 1 || (KEYMUL == 2 && (t & 1)))
+          return s * ma.key_mul + low;
+        else
+          return (s << C::KB) + low;
+      };
+      uint32_t best = make_key(sum, 0);
 #pragma unroll
       for (int t = 1; t < C::NWIN; ++t) {
         sum = sum + RTA_X(w, h0 + t + W - 1) - RTA_X(w, h0 + t - 1);
-        const uint32_t key = (sum << C::KB) + (C::KM - (uint32_t)t);
-        best = max(best, key);
+        best = max(best, make_key(sum, t));
       }
       tstar = (int)(C::KM - (best & C::KM));
       rawsum = (int)(best >> C::KB);
@@ -420,7 +443,7 @@ __device__ __forceinline__ void store_results(const Result (&res)[C::TPT], const
   }
 }
 
-template <class C, int MODE>
+template <class C, int MODE, int KEYMUL = 0>
 __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, const uint32_t g0,
                                              const uint32_t n_valid, const uint32_t p0,
                                              const uint32_t n_pixels,
@@ -431,7 +454,7 @@ __device__ __forceinline__ void compute_unit(const uint8_t* __restrict__ unit, c
                                              float* __restrict__ out_time, const bool vec_store,
                                              const ModeArgs& ma) {
   Result res[C::TPT];
-  compute_results<C, MODE>(unit, p0, n_pixels, pedestal, gain, ma, res);
+  compute_results<C, MODE, KEYMUL>(unit, p0, n_pixels, pedestal, gain, ma, res);
   store_results<C>(res, g0, n_valid, out_sum, out_start, out_charge, out_time, vec_store);
 }
 

@@ -152,8 +152,9 @@ __global__ void __launch_bounds__(C::NT)
     mbar_wait(bar_base + 8 * stage, parity);
     const uint8_t* unit = smem + stage * C::STAGE_BYTES + tid * C::UNIT_STRIDE;
     const uint32_t g0 = tile * C::TILE_TRACES + (uint32_t)tid * C::TPT;
-    compute_unit<C, MODE>(unit, g0, C::TPT, fastmod(g0, n_pixels, pix_inv), n_pixels, pedestal,
-                          gain, out_sum, out_start, out_charge, out_time, vec_store != 0, ma);
+    compute_unit<C, MODE, C::KEYMODE>(unit, g0, C::TPT, fastmod(g0, n_pixels, pix_inv), n_pixels,
+                                pedestal, gain, out_sum, out_start, out_charge, out_time,
+                                vec_store != 0, ma);
     __syncthreads();  // every thread is done with this stage; tile_q slot is published
     const uint32_t next = tile_q[(j + C::STAGES) % QN];
     if (next < n_full) issue(next, stage);
@@ -182,9 +183,9 @@ __global__ void __launch_bounds__(C::NT)
     if (first < rem) {
       const uint8_t* unit = smem + tid * C::UNIT_STRIDE;
       const uint32_t g0 = n_full * C::TILE_TRACES + first;
-      compute_unit<C, MODE>(unit, g0, rem - first, fastmod(g0, n_pixels, pix_inv), n_pixels,
-                            pedestal, gain, out_sum, out_start, out_charge, out_time,
-                            vec_store != 0, ma);
+      compute_unit<C, MODE, C::KEYMODE>(unit, g0, rem - first, fastmod(g0, n_pixels, pix_inv), n_pixels,
+                                  pedestal, gain, out_sum, out_start, out_charge, out_time,
+                                  vec_store != 0, ma);
     }
   }
 
@@ -510,9 +511,11 @@ struct TileLauncher {
                         (uintptr_t)out_time;
     const int vec_store = (o % 8 == 0) ? 1 : 0;
     uint32_t* sched = g_static_schedule ? nullptr : sched_words(dev, stream);
+    ModeArgs m = ma;
+    m.key_mul = 1u << C::KB;
     extract_tile_kernel<C, MODE><<<grid, C::NT, C::SMEM_BYTES, stream>>>(
         wf, n_traces, n_pixels, pix_inv, pedestal, gain, out_sum, out_start, out_charge, out_time,
-        vec_store, sched, ma);
+        vec_store, sched, m);
     rta_count_launch();
     return cudaGetLastError();
   }
