@@ -128,6 +128,7 @@ struct ModeArgs {
   // sum * 2^KB + (2^KB - 1 - t) then compiles to one IMAD (fma pipe) instead of
   // one LEA (alu pipe), which is the pipe these kernels fill first
   uint32_t key_mul;
+  uint32_t one, minus_one;  // 1 and 2^32 - 1, for the same reason (TileCfg::SLIDEMODE)
 };
 
 // d = c + a.u16[0] * b.s8[2 hi] + a.u16[1] * b.s8[2 hi + 1]  (SASS IDP.2A)
@@ -145,6 +146,12 @@ __device__ __forceinline__ int clamp_start(const int t, const int S, const int W
   return min(max(t, 0), S - W);
 }
 
+#ifndef RTA_SLIDEMODE_P12
+#define RTA_SLIDEMODE_P12 2
+#endif
+#ifndef RTA_SLIDEMODE_U16
+#define RTA_SLIDEMODE_U16 0
+#endif
 #ifndef RTA_KEYMODE_P12
 #define RTA_KEYMODE_P12 1
 #endif
@@ -191,6 +198,7 @@ struct TileCfg {
   static constexpr uint32_t KM = (1u << KB) - 1u;
   static constexpr int PB = ilog2_ceil(S);  // local-peak key: sample index bits
   // how the arg-max keys are formed (compute_results KEYMUL): tuned per shape on B200
+  static constexpr int SLIDEMODE = (BITS == 12) ? RTA_SLIDEMODE_P12 : RTA_SLIDEMODE_U16;
   static constexpr int KEYMODE = (BITS == 12) ? ((S == 40 || S == 30) ? RTA_KEYMODE_P40 : RTA_KEYMODE_P12)
                                               : RTA_KEYMODE_U16;
   static constexpr uint32_t XMAX = (BITS == 16) ? 65535u : 4095u;
@@ -255,6 +263,8 @@ struct WindowReader {
 // Steps a2-a7 for the C::TPT traces of one thread's unit in shared memory.
 // p0: calibration index of the first trace; it wraps to 0 after n_pixels - 1
 // (a uniform batch runs through the camera again; n_pixels = 0 never wraps).
+// KEYMUL != 0: `ma` comes from the launch (constant bank) and carries key_mul /
+// one / minus_one, which lets part of the integer work run on the fma pipe.
 template <class C, int MODE, int KEYMUL = 0>
 __device__ __forceinline__ void compute_results(const uint8_t* __restrict__ unit,
                                                 const uint32_t p0, const uint32_t n_pixels,
@@ -314,7 +324,13 @@ __device__ __forceinline__ void compute_results(const uint8_t* __restrict__ unit
       uint32_t best = make_key(sum, 0);
 #pragma unroll
       for (int t = 1; t < C::NWIN; ++t) {
-        sum = sum + RTA_X(w, h0 + t + W - 1) - RTA_X(w, h0 + t - 1);
+        if (KEYMUL != 0 && (C::SLIDEMODE == 1 || (C::SLIDEMODE == 2 && (t & 1)))) {
+          // the same update as two IMADs with constant-bank multipliers 1 and -1 (fma pipe)
+          sum = RTA_X(w, h0 + t + W - 1) * ma.one + sum;
+          sum = RTA_X(w, h0 + t - 1) * ma.minus_one + sum;
+        } else {
+          sum = sum + RTA_X(w, h0 + t + W - 1) - RTA_X(w, h0 + t - 1);
+        }
         best = max(best, make_key(sum, t));
       }
       tstar = (int)(C::KM - (best & C::KM));

@@ -513,6 +513,8 @@ struct TileLauncher {
     uint32_t* sched = g_static_schedule ? nullptr : sched_words(dev, stream);
     ModeArgs m = ma;
     m.key_mul = 1u << C::KB;
+    m.one = 1u;
+    m.minus_one = 0xFFFFFFFFu;
     extract_tile_kernel<C, MODE><<<grid, C::NT, C::SMEM_BYTES, stream>>>(
         wf, n_traces, n_pixels, pix_inv, pedestal, gain, out_sum, out_start, out_charge, out_time,
         vec_store, sched, m);
