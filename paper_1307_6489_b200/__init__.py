@@ -114,6 +114,8 @@ def lib() -> ctypes.CDLL:
             L.rta_shutdown.argtypes = []
             L.rta_debug_static_schedule.restype = None
             L.rta_debug_static_schedule.argtypes = [ctypes.c_int]
+            L.rta_debug_serial_ragged.restype = None
+            L.rta_debug_serial_ragged.argtypes = [ctypes.c_int]
             L.rta_debug_general_cleaning.restype = None
             L.rta_debug_general_cleaning.argtypes = [ctypes.c_int]
             _lib = L
@@ -382,6 +384,12 @@ def rta_debug_static_schedule(on: bool) -> None:
     """Test hook: force the static round-robin tile schedule of the staged
     kernels (default is dynamic). Results are identical either way."""
     lib().rta_debug_static_schedule(1 if on else 0)
+
+
+def rta_debug_serial_ragged(on: bool) -> None:
+    """Test hook: rta_extract_ragged issues its launches one after the other on
+    the caller's stream instead of forking side streams. Same results."""
+    lib().rta_debug_serial_ragged(1 if on else 0)
 
 
 def rta_debug_general_cleaning(on: bool) -> None:

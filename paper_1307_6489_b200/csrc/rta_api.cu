@@ -20,6 +20,7 @@
 namespace {
 
 thread_local int t_last_cuda = 0;
+std::atomic<bool> g_serial_ragged{false};  // tests: rta_extract_ragged without side streams
 std::atomic<bool> g_force_generic{false};  // tests: route the family entry points to the generic kernel
 std::atomic<uint64_t> g_launches{0};
 
@@ -688,6 +689,63 @@ int rta_ragged_plan_create(int32_t n_tel, const int32_t* tel_n_pixels,
   return RTA_OK;
 }
 
+// Side streams for rta_extract_ragged: the launches of one call (one per camera
+// shape) are independent, so all but the first run on library-owned streams
+// forked from and joined back into the caller's stream. Every launch is a
+// persistent grid sized for the whole GPU: the CTAs of the next shape become
+// resident as those of the previous one drain, which hides the launch tails.
+namespace {
+constexpr int kSideStreams = 2;
+constexpr int kMaxDev = 32;
+struct SideStreams {
+  std::mutex mu;
+  bool ready[kMaxDev] = {};
+  bool failed[kMaxDev] = {};
+  cudaStream_t s[kMaxDev][kSideStreams] = {};
+  cudaEvent_t fork[kMaxDev] = {};
+  cudaEvent_t join[kMaxDev][kSideStreams] = {};
+};
+SideStreams g_side;
+
+// caller holds g_side.mu
+bool side_streams_ready(int dev) {
+  if (dev < 0 || dev >= kMaxDev || g_side.failed[dev]) return false;
+  if (g_side.ready[dev]) return true;
+  bool ok = cudaEventCreateWithFlags(&g_side.fork[dev], cudaEventDisableTiming) == cudaSuccess;
+  for (int i = 0; i < kSideStreams && ok; ++i)
+    ok = cudaStreamCreateWithFlags(&g_side.s[dev][i], cudaStreamNonBlocking) == cudaSuccess &&
+         cudaEventCreateWithFlags(&g_side.join[dev][i], cudaEventDisableTiming) == cudaSuccess;
+  if (!ok) {
+    cudaGetLastError();
+    g_side.failed[dev] = true;  // stay on the caller's stream (what is half-built is leaked once)
+    return false;
+  }
+  g_side.ready[dev] = true;
+  return true;
+}
+
+// rta_shutdown: the caller has synchronised the devices in use
+void side_streams_release() {
+  std::lock_guard<std::mutex> lock(g_side.mu);
+  int cur = 0;
+  const bool have_cur = cudaGetDevice(&cur) == cudaSuccess;
+  for (int d = 0; d < kMaxDev; ++d) {
+    if (g_side.ready[d] && cudaSetDevice(d) == cudaSuccess) {
+      for (int i = 0; i < kSideStreams; ++i) {
+        cudaStreamSynchronize(g_side.s[d][i]);
+        cudaStreamDestroy(g_side.s[d][i]);
+        cudaEventDestroy(g_side.join[d][i]);
+      }
+      cudaEventDestroy(g_side.fork[d]);
+    }
+    g_side.ready[d] = false;
+    g_side.failed[d] = false;
+  }
+  if (have_cur) cudaSetDevice(cur);
+  cudaGetLastError();
+}
+}  // namespace
+
 int rta_extract_ragged(const rta_ragged_plan* plan, const uint16_t* wf, const int32_t* pedestal,
                        const float* gain, int32_t* out_sum, int32_t* out_start,
                        float* out_charge, float* out_time, void* stream) {
@@ -703,11 +761,44 @@ int rta_extract_ragged(const rta_ragged_plan* plan, const uint16_t* wf, const in
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return fail_cuda(e);
   if (dev != plan->device) return fail_cuda(cudaErrorInvalidDevice);
-  for (const rta_ragged_plan::Class& c : plan->classes) {
-    e = rta_launch_ragged(wf, plan->tiles_dev + c.first, c.count, c.S, c.W, pedestal, gain,
-                          out_sum, out_start, out_charge, out_time, (cudaStream_t)stream);
-    if (e != cudaSuccess) return fail_cuda(e);
+  const cudaStream_t user = (cudaStream_t)stream;
+  const size_t n_classes = plan->classes.size();
+  std::unique_lock<std::mutex> lock(g_side.mu, std::defer_lock);
+  bool forked = false;
+  if (n_classes > 1 && !g_serial_ragged.load()) {
+    lock.lock();
+    forked = side_streams_ready(dev) &&
+             cudaEventRecord(g_side.fork[dev], user) == cudaSuccess;
+    if (!forked) {
+      cudaGetLastError();
+      lock.unlock();
+    }
   }
+  int used = 0;  // side streams that got work
+  cudaError_t first_err = cudaSuccess;
+  for (size_t i = 0; i < n_classes; ++i) {
+    const rta_ragged_plan::Class& c = plan->classes[i];
+    cudaStream_t st = user;
+    if (forked && i > 0) {
+      const int k = (int)((i - 1) % kSideStreams);
+      st = g_side.s[dev][k];
+      if (k >= used) {  // first work on this side stream: order it after the caller's stream
+        e = cudaStreamWaitEvent(st, g_side.fork[dev], 0);
+        if (e != cudaSuccess && first_err == cudaSuccess) first_err = e;
+        used = k + 1;
+      }
+    }
+    e = rta_launch_ragged(wf, plan->tiles_dev + c.first, c.count, c.S, c.W, pedestal, gain,
+                          out_sum, out_start, out_charge, out_time, st);
+    if (e != cudaSuccess && first_err == cudaSuccess) first_err = e;
+  }
+  // join, also after an error: the caller's stream must not run ahead of what was enqueued
+  for (int k = 0; k < used; ++k) {
+    e = cudaEventRecord(g_side.join[dev][k], g_side.s[dev][k]);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(user, g_side.join[dev][k], 0);
+    if (e != cudaSuccess && first_err == cudaSuccess) first_err = e;
+  }
+  if (first_err != cudaSuccess) return fail_cuda(first_err);
   return RTA_OK;
 }
 
@@ -922,8 +1013,13 @@ void rta_shutdown(void) {
       cudaGetLastError();
     }
   }
+  side_streams_release();
   rta_sched_release();
 }
+
+// Test hook (not in the public header): 1 = rta_extract_ragged issues every
+// launch on the caller's stream, one after the other.
+void rta_debug_serial_ragged(int on) { g_serial_ragged.store(on != 0); }
 
 // Test hook (not in the public header): 1 = rta_extract_fixed / _local_peak / _fir /
 // _packed12 take the generic kernel whatever the shape (two device paths must agree).

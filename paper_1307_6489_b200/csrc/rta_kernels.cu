@@ -251,6 +251,9 @@ __global__ void __launch_bounds__(C::NT)
   __shared__ __align__(8) uint64_t full_bar[C::STAGES];
   constexpr int QN = C::STAGES + 1;
   __shared__ uint32_t tile_q[QN];
+  // the table entry of every queued tile, fetched by thread 0 one iteration
+  // ahead together with the index: no thread waits on a dependent global load
+  __shared__ RaggedTile desc_q[QN];
   const int tid = threadIdx.x;
   const uint32_t smem_base = smem_u32(smem);
   const uint32_t bar_base = smem_u32(full_bar);
@@ -282,11 +285,16 @@ __global__ void __launch_bounds__(C::NT)
     return cur++;
   };
 
+  const auto entry = [&](const uint32_t ti) -> RaggedTile {
+    if (ti < n_tiles) return tiles[ti];
+    return RaggedTile{0ull, 0u, 0u};
+  };
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < C::STAGES; ++s) {
       mbar_init(bar_base + 8 * s, C::NT);
       tile_q[s] = fetch_static();
+      desc_q[s] = entry(tile_q[s]);
     }
     fence_mbar_init();
     if (sched != nullptr) {
@@ -298,8 +306,8 @@ __global__ void __launch_bounds__(C::NT)
 
   constexpr uint32_t UB = C::UNIT_BYTES, PADB = C::UNIT_STRIDE - C::UNIT_BYTES;
   constexpr uint32_t TRACE_BYTES = C::TRACE_BITS / 8;
-  auto issue = [&](const uint32_t ti, const int stage) {
-    const RaggedTile t = tiles[ti];
+  auto issue = [&](const int slot, const int stage) {
+    const RaggedTile t = desc_q[slot];
     const uint8_t* src = wf + (size_t)(t.src & kRaggedOffMask);
     const uint32_t bytes = (uint32_t)(t.src >> 48) * TRACE_BYTES;
     uint8_t* dstp = smem + stage * C::STAGE_BYTES;
@@ -316,8 +324,16 @@ __global__ void __launch_bounds__(C::NT)
         }
       } else {
         done = bytes;  // a padded unit is a whole number of 16-byte chunks
-        for (uint32_t c = tid; c < bytes / 16u; c += C::NT)
-          cp_async16(dst + (c + c / (UB / 16u)) * 16u, src + (size_t)c * 16u);
+        if (bytes == (uint32_t)C::TILE_BYTES) {  // full tile: compile-time trip count, as the uniform kernel
+#pragma unroll 4
+          for (int c = tid; c < C::TILE_BYTES / 16; c += C::NT) {
+            const int u = c / C::NVEC;
+            cp_async16(dst + (uint32_t)(c + u) * 16u, src + (size_t)c * 16);
+          }
+        } else {
+          for (uint32_t c = tid; c < bytes / 16u; c += C::NT)
+            cp_async16(dst + (c + c / (UB / 16u)) * 16u, src + (size_t)c * 16u);
+        }
       }
     } else if ((mis & 3u) == 0) {
       done = bytes & ~3u;
@@ -340,10 +356,14 @@ __global__ void __launch_bounds__(C::NT)
 #pragma unroll
   for (int s = 0; s < C::STAGES; ++s) {
     const uint32_t tile = tile_q[s];
-    if (tile < n_tiles) issue(tile, s);
+    if (tile < n_tiles) issue(s, s);
   }
   uint32_t pre = 0;
-  if (tid == 0) pre = fetch();
+  RaggedTile pre_d = {0ull, 0u, 0u};
+  if (tid == 0) {
+    pre = fetch();
+    pre_d = entry(pre);
+  }
 
   for (uint32_t j = 0;; ++j) {
     const uint32_t tile = tile_q[j % QN];
@@ -352,9 +372,11 @@ __global__ void __launch_bounds__(C::NT)
     const uint32_t parity = (j / C::STAGES) & 1u;
     if (tid == 0) {
       tile_q[(j + C::STAGES) % QN] = pre;
+      desc_q[(j + C::STAGES) % QN] = pre_d;
       pre = fetch();
+      pre_d = entry(pre);
     }
-    const RaggedTile t = tiles[tile];
+    const RaggedTile t = desc_q[j % QN];
     const uint32_t n = (uint32_t)(t.src >> 48);
     mbar_wait(bar_base + 8 * stage, parity);
     const uint32_t first = (uint32_t)tid * C::TPT;
@@ -366,7 +388,7 @@ __global__ void __launch_bounds__(C::NT)
     }
     __syncthreads();
     const uint32_t next = tile_q[(j + C::STAGES) % QN];
-    if (next < n_tiles) issue(next, stage);
+    if (next < n_tiles) issue((int)((j + C::STAGES) % QN), stage);
   }
 
   if (sched != nullptr && tid == 0) {

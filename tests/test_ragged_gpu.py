@@ -18,7 +18,7 @@ GOLD = os.path.join(os.path.dirname(__file__), "golden", "ragged.json")
 FILL = (-7, -7, -7.0, -7.0)
 
 
-def run_gpu(b, wf=None, wf_shift=0, streams=1, static=False):
+def run_gpu(b, wf=None, wf_shift=0, streams=1, static=False, serial=False):
     """wf_shift: place the waveform buffer that many samples into a 256-byte-aligned
     allocation (so block alignments change without touching the tables)."""
     import torch
@@ -35,6 +35,7 @@ def run_gpu(b, wf=None, wf_shift=0, streams=1, static=False):
     plan = rta.rta_ragged_plan_create(*b.tables())
     try:
         rta.rta_debug_static_schedule(static)
+        rta.rta_debug_serial_ragged(serial)
         before = rta.rta_launch_count()
         rta.rta_extract_ragged(plan, d_wf, d_ped, d_gain, *outs)
         torch.cuda.synchronize()
@@ -43,6 +44,7 @@ def run_gpu(b, wf=None, wf_shift=0, streams=1, static=False):
             b.tel_n_pixels[k] for k in b.blk_tel)
     finally:
         rta.rta_debug_static_schedule(False)
+        rta.rta_debug_serial_ragged(False)
         rta.rta_ragged_plan_destroy(plan)
     return tuple(o.cpu().numpy() for o in outs)
 
@@ -103,6 +105,21 @@ def test_static_and_dynamic_tile_schedules_agree():
     b = make_batch(SPECIAL, n_events=6, seed=9, gap=3)
     check(b, static=True)
     check(b, static=False)
+
+
+def test_side_streams_and_serial_launches_agree():
+    """One launch per camera shape: forked onto library-owned side streams
+    (default) or one after the other on the caller's stream; also on a
+    non-default caller stream followed by dependent work on that stream."""
+    import torch
+    b = make_batch(SPECIAL, n_events=6, seed=21, gap=3)
+    assert len({(b.tel_n_samples[k], b.tel_W[k]) for k in b.blk_tel}) > 1
+    check(b, serial=True)
+    check(b, serial=False)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        for _ in range(3):
+            check(b)
 
 
 def test_config_cameras_full_blocks():
