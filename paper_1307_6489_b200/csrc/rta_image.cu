@@ -44,6 +44,12 @@
 
 #include <atomic>
 
+// how the fused kernels form the arg-max keys (compute_results KEYMUL): 1 = IMAD
+// with a constant-bank multiplier (fma pipe); these kernels are alu-pipe-bound
+#ifndef RTA_IMG_KEYMODE
+#define RTA_IMG_KEYMODE 1
+#endif
+
 namespace {
 
 __device__ __forceinline__ void named_sync(const int id, const int n) {
@@ -600,7 +606,7 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
                          const int* __restrict__ pedestal, const float* __restrict__ gain,
                          const __grid_constant__ RtaCamera cam,
                          const __grid_constant__ RtaImageOut out, const int NB, const int NC,
-                         const int force_general) {
+                         const int force_general, const __grid_constant__ ModeArgs ma) {
   static_assert(C::BITS == 16 && C::STAGES >= 2, "uint16 samples, at least two stages");
   static_assert(C::TPT == 1 || C::TPT == 2, "one or two traces per thread");
   static_assert(G >= 1 && G <= 14, "named barriers 1 .. G");
@@ -664,7 +670,6 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
   const uint32_t ring = smem_u32(smem) + (uint32_t)(g * C::STAGES * STG);
   uint8_t* ringp = smem + (size_t)g * C::STAGES * STG;
   const uint32_t bar_base = smem_u32(full_bar) + 8u * (uint32_t)(g * C::STAGES);
-  const ModeArgs ma = {};
   const unsigned long long EB = (unsigned long long)P * TRACE_BYTES;  // bytes per event
   const unsigned long long total = (unsigned long long)n_events * EB;
   const float thr_p = cam.thr_picture, thr_b = cam.thr_boundary;
@@ -757,7 +762,7 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
       if constexpr (!C::PAD) mis = (ev * EB32) & 15u;  // TILE_BYTES is a multiple of 16
       const uint8_t* unit = ringp + stage * STG + mis + gt * C::UNIT_STRIDE;
       Result res[C::TPT];
-      compute_results<C, MODE_SLIDING>(unit, p0, 0u, pedestal, gain, ma, res);
+      compute_results<C, MODE_SLIDING, RTA_IMG_KEYMODE>(unit, p0, 0u, pedestal, gain, ma, res);
 #pragma unroll
       for (int i = 0; i < C::TPT; ++i) {  // P is a multiple of TPT: the unit is whole
         buf.q[p0 + i] = qv[i] = res[i].charge;
@@ -896,8 +901,12 @@ struct FusedLauncher {
     if (e != cudaSuccess) return e;
     uint32_t grid = (uint32_t)sms;
     if (grid > n_events) grid = n_events;
+    ModeArgs ma = {};  // constant-bank operands of compute_results (KEYMUL)
+    ma.key_mul = 1u << C::KB;
+    ma.one = 1u;
+    ma.minus_one = 0xFFFFFFFFu;
     kernel<<<grid, I::THREADS, smem, stream>>>(wf, n_events, P, pedestal, gain, cam, out, nb, nc,
-                                               g_general_cleaning.load() ? 1 : 0);
+                                               g_general_cleaning.load() ? 1 : 0, ma);
     rta_count_launch();
     return cudaGetLastError();
   }
