@@ -46,6 +46,11 @@
 
 // how the fused kernels form the arg-max keys (compute_results KEYMUL): 1 = IMAD
 // with a constant-bank multiplier (fma pipe); these kernels are alu-pipe-bound
+// most warps per CTA of image_moments_kernel: 16 leaves the cleaning code its 128
+// registers (24 would spill)
+#ifndef RTA_MOM_WARPS
+#define RTA_MOM_WARPS 16
+#endif
 #ifndef RTA_IMG_KEYMODE
 #define RTA_IMG_KEYMODE 1
 #endif
@@ -464,7 +469,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   int n_pend = 0;
   for (uint32_t e = blockIdx.x * WARPS + warp; e < n_events; e += stride) {
     const float* q = charge + (size_t)e * (size_t)P;
-    constexpr int U = 4;
+    constexpr int U = 16;  // loads in flight per lane: the sweep is one DRAM latency per 512 pixels
     for (int p0 = 0; p0 < P; p0 += 32 * U) {
       float v[U];
 #pragma unroll
@@ -957,11 +962,13 @@ cudaError_t rta_launch_image_moments(const float* charge, const float* time, int
                                      int32_t n_pixels, const RtaCamera& cam,
                                      const RtaImageOut& out, cudaStream_t stream) {
   if (n_events <= 0) return cudaSuccess;
-  // as many warps as one CTA's shared memory holds, up to 24 (85 registers per thread)
+  // as many warps as one CTA's shared memory holds, up to RTA_MOM_WARPS
   const size_t per_warp = moments_warp_bytes(n_pixels);
   const size_t room = kSmemLimit - 2048u;
   const uint32_t E = (uint32_t)n_events;
+#if RTA_MOM_WARPS >= 24
   if (24u * per_warp <= room) return launch_moments<24>(charge, time, E, n_pixels, cam, out, stream);
+#endif
   if (16u * per_warp <= room) return launch_moments<16>(charge, time, E, n_pixels, cam, out, stream);
   if (8u * per_warp <= room) return launch_moments<8>(charge, time, E, n_pixels, cam, out, stream);
   return launch_moments<4>(charge, time, E, n_pixels, cam, out, stream);
