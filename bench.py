@@ -573,6 +573,43 @@ def sustained_leg(torch, dl0gen, rta, link_gbs):
            "paper_array_rate_GBps": list(PAPER_RATE_GBS),
            "x_paper_max_rate": val / PAPER_RATE_GBS[1],
            "pinned_alloc_s": t_alloc, "outputs": "stay on device (5.94 GB)"}
+    # NEXT-4: the same pinned buffer through rta_extract_image_stream: waveforms in at
+    # link speed, 36 bytes of event parameters per event out (they stay on the device)
+    try:
+        cam = camera_on_device(cfg, torch, dl0gen)
+        n_pix = torch.empty(cfg.n_events, dtype=torch.int32, device="cuda")
+        par = torch.empty((cfg.n_events, 8), dtype=torch.float32, device="cuda")
+
+        def run_img():
+            rta.rta_extract_image_stream(host, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped,
+                                         d_gain, cfg.W, *cam, n_pix, par, None,
+                                         chunk_bytes=1 << 30, stream=stream)
+        run_img()
+        torch.cuda.synchronize()
+        # the first events again from the per-trace outputs of the uint16 leg above
+        n64, p64 = image_outputs(dl0gen.CONFIGS["C1"], torch)            # 64 events
+        rta.rta_image_moments(outs[2], outs[3], 64, cfg.n_pixels, *cam, n64, p64, None, stream=stream)
+        torch.cuda.synchronize()
+        same_img = bool((n_pix[:64] == n64).all()) and bool(
+            (par[:64].view(torch.int32) == p64.view(torch.int32)).all())
+        times = []
+        for _ in range(2):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            run_img()
+            torch.cuda.synchronize()
+            times.append(time.perf_counter() - t0)
+        dti = min(times)
+        res["image"] = {
+            "value": cfg.input_bytes / dti / 1e9, "unit": UNIT, "seconds": dti,
+            "api": "rta_extract_image_stream (extraction + cleaning + moments in one kernel per chunk)",
+            "events_per_s": cfg.n_events / dti, "frac_of_host_link": cfg.input_bytes / dti / 1e9 / link_gbs,
+            "result_bytes": EVENT_OUT_BYTES * cfg.n_events,
+            "mean_pixels_in_image": float(n_pix.float().mean()),
+            "first_64_events_equal_extract_then_moments": same_img}
+        del n_pix, par
+    except Exception as ex:
+        res["image"] = {"error": repr(ex)}
     # NEXT-2: the same 200 000 events as a P12 stream (22.26 GB) in the same pinned
     # buffer, through rta_extract_stream_packed12 (chunks of 9644 events = 1.07 GB)
     try:
