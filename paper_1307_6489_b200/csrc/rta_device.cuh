@@ -87,22 +87,43 @@ __device__ __forceinline__ Result finish_trace(const int W, const int rawsum, co
                                                const int relnum, const int ped, const float gain,
                                                const int c0, const int c1) {
   Result r;
-  const long long sum64 = (long long)rawsum - (long long)c0 * (long long)ped;
-  const long long num64 = (long long)(tstar * rawsum + relnum) -
-                          (long long)ped * ((long long)tstar * (long long)c0 + (long long)c1);
-  r.sum = (int)sum64;
   r.start = tstar;
-  const long long lim = 1ll << 24;
-  if (sum64 > -lim && sum64 < lim && num64 > -lim && num64 < lim) {
-    // every operand is an exactly representable integer: one IEEE operation
-    // each, bit-identical to rounding the double-precision result
-    int n = (int)num64, d = (int)sum64;
+  constexpr int lim = 1 << 24;
+  // every operand below 2^24 in magnitude is an exactly representable integer:
+  // one IEEE operation each, bit-identical to rounding the double-precision result
+  const auto small_floats = [&](const int sum, const int num) {
+    int n = num, d = sum;
     if (d <= 0) {  // degenerate mean -> window centre = (2 t* + W - 1) / 2
       n = 2 * tstar + W - 1;
       d = 2;
     }
-    r.charge = __fmul_rn((float)(int)sum64, gain);
+    r.charge = __fmul_rn((float)sum, gain);
     r.time = __fdiv_rn((float)n, (float)d);
+  };
+  const auto in24 = [](const int x) { return (unsigned)(x + (lim - 1)) < (unsigned)(2 * lim - 1); };
+  if ((unsigned)ped <= 65535u) {
+    // A pedestal inside the sample range (every config): x = raw - ped lies in
+    // [-65535, 65535], so Sum and the numerator are bounded by the ABI guard
+    // n_samples * sum|c| * 65535 < 2^31 and 32-bit arithmetic (exact modulo 2^32
+    // in the intermediate products) gives them exactly.
+    const int sum = rawsum - c0 * ped;
+    const int num = tstar * rawsum + relnum - ped * (tstar * c0 + c1);
+    r.sum = sum;
+    if (in24(sum) && in24(num)) {
+      small_floats(sum, num);
+    } else {
+      r.charge = (float)((double)sum * (double)gain);
+      r.time = sum > 0 ? (float)((double)num / (double)sum)
+                       : (float)((double)tstar + 0.5 * (double)(W - 1));
+    }
+    return r;
+  }
+  const long long sum64 = (long long)rawsum - (long long)c0 * (long long)ped;
+  const long long num64 = (long long)(tstar * rawsum + relnum) -
+                          (long long)ped * ((long long)tstar * (long long)c0 + (long long)c1);
+  r.sum = (int)sum64;
+  if (sum64 > -lim && sum64 < lim && num64 > -lim && num64 < lim) {
+    small_floats((int)sum64, (int)num64);
   } else {
     r.charge = (float)((double)sum64 * (double)gain);
     r.time = sum64 > 0 ? (float)((double)num64 / (double)sum64)

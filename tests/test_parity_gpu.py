@@ -128,6 +128,29 @@ def test_extreme_pedestals_take_the_wide_path(S, W):
     assert bit_identical(got, want)
 
 
+@pytest.mark.parametrize("S,W", SHAPES + [(33, 5)])
+def test_pedestals_at_the_edges_of_the_sample_range(S, W):
+    """finish_trace computes in 32 bits when 0 <= pedestal <= 65535 and in 64 bits
+    otherwise: both sides of both edges, on full-range samples (largest sums and
+    numerators the ABI guard allows) and on all-0 / all-65535 traces."""
+    rng = np.random.default_rng(S + 1000)
+    E = 4
+    edge = np.array([0, 1, 65534, 65535, 65536, 65537, -1, -2, 32767, 32768, 40000, 2 ** 31 - 1,
+                     -2 ** 31, 70000, -65535], np.int32)
+    P = len(edge) * 8
+    ped = np.tile(edge, 8)
+    wf = rng.integers(0, 65536, size=(E, P, S)).astype(np.uint16)
+    wf[0, :, :] = 65535
+    wf[1, :, :] = 0
+    wf[2, :, S // 2:] = 65535                             # late plateau: largest time numerators
+    gain = rng.uniform(0.5, 2, P).astype(np.float32)
+    want = oracle.extract(wf, ped, gain, W)
+    for generic in (False, True):
+        got = run_gpu(wf, ped, gain, W, generic=generic)
+        assert (got[0] == want[0]).all() and (got[1] == want[1]).all()
+        assert bit_identical(got, want)
+
+
 def test_unaligned_input_takes_generic_kernel_and_agrees():
     import torch
     import paper_1307_6489_b200 as rta
