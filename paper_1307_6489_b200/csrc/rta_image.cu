@@ -44,13 +44,13 @@
 
 #include <atomic>
 
-// how the fused kernels form the arg-max keys (compute_results KEYMUL): 1 = IMAD
-// with a constant-bank multiplier (fma pipe); these kernels are alu-pipe-bound
 // most warps per CTA of image_moments_kernel: 16 leaves the cleaning code its 128
 // registers (24 would spill)
 #ifndef RTA_MOM_WARPS
 #define RTA_MOM_WARPS 16
 #endif
+// how the fused kernels form the arg-max keys (compute_results KEYMUL): 1 = IMAD
+// with a constant-bank multiplier (fma pipe); these kernels are alu-pipe-bound
 #ifndef RTA_IMG_KEYMODE
 #define RTA_IMG_KEYMODE 1
 #endif

@@ -93,6 +93,40 @@ def test_blob_images(P, E, seed):
     assert np.array_equal(got2[0], got[0]) and np.array_equal(got2[1].view(np.int32), got[1].view(np.int32))
 
 
+def test_symmetric_table_shortcut_equals_the_definition():
+    """On a symmetric neighbour table (every hex camera) the cleaning does both
+    steps in one pass over the core pixels; rta_debug_general_cleaning forces the
+    two steps as written. Same mask, same parameters, bit for bit — on blobs, on
+    dense images (every pixel core / every pixel above the boundary) and through
+    both fused kernels."""
+    import paper_1307_6489_b200 as rta
+    for P, seed in ((1855, 31), (469, 32), (37, 33)):
+        q, t, x, y, nbr = blob_images(40, P, seed)
+        q[5, :] = 20.0                      # every pixel core
+        q[6, :] = 5.0                       # every pixel above the boundary threshold only
+        q[7, ::3] = 50.0                    # a third of the camera core
+        want = oracle.image_moments(q, t, x, y, nbr, 8.0, 4.0)
+        fast = gpu_moments(q, t, x, y, nbr, 8.0, 4.0)
+        rta.rta_debug_general_cleaning(True)
+        try:
+            slow = gpu_moments(q, t, x, y, nbr, 8.0, 4.0)
+        finally:
+            rta.rta_debug_general_cleaning(False)
+        assert_image_parity(fast, want, x, y, "symmetric P=%d" % P)
+        for a, b in zip(fast, slow):
+            assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
+    cfg, wf, ped, gain, x, y, nbr, tp, tb = config_batch("C3", 40)
+    for generic in (False, True):
+        fast = gpu_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb, generic=generic)
+        rta.rta_debug_general_cleaning(True)
+        try:
+            slow = gpu_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb, generic=generic)
+        finally:
+            rta.rta_debug_general_cleaning(False)
+        for a, b in zip(fast, slow):
+            assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
+
+
 def test_thresholds_and_special_values():
     q, t, x, y, nbr = blob_images(24, 469, 11)
     q[3, :] = np.nan                       # NaN never passes a threshold
