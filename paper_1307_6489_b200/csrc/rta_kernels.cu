@@ -221,6 +221,213 @@ __global__ void __launch_bounds__(256)
   }
 }
 
+// ------------------------------------------- any shape, staged (runtime S, W) ----
+// The sliding-window extractor for shapes without a specialisation (a 60-sample
+// NectarCam-like readout, a 96-sample trace, another window width ...): the same
+// stage ring, TMA ingest and dynamic tile scheduler as extract_tile_kernel, with
+// S and W as kernel arguments. A thread still owns one unit (one trace, or two
+// when S is odd), but walks it in shared memory with 16-bit loads instead of a
+// register copy (register arrays need compile-time indices). What makes that
+// fast for any stride:
+//  * lanes l and l' hit the same bank with different words iff (l - l') * s = 0
+//    mod 32, s = words per unit; with g = gcd(s, 32) those are the lanes
+//    l + (32 / g) b, b = 0 .. g-1. Lane group b runs the sliding loop 2 b samples
+//    behind (one word): the loop has 2 (g - 1) more iterations than windows and
+//    every access of every iteration is conflict-free;
+//  * g is kept <= 4: units of a multiple of 32 bytes (g >= 8) are copied with
+//    16-byte cp.async into a layout padded by one chunk (as the S = 128 kernel),
+//    everything else arrives by one TMA bulk copy per tile.
+struct DynShape {
+  int32_t S, W, n_win;
+  int32_t tpt;          // traces per unit: 1 (S even) or 2
+  int32_t unit_bytes;   // 2 S tpt
+  int32_t unit_stride;  // unit_bytes (+ 16 when padded)
+  int32_t tile_bytes;   // blockDim.x * unit_bytes
+  int32_t stage_bytes;  // blockDim.x * unit_stride + slack, multiple of 128
+  int32_t stages;
+  int32_t g;            // gcd(unit_stride / 4, 32): 1, 2 or 4
+  int32_t kb;           // key bits: 2^kb >= n_win
+  uint32_t key_mul;     // 2^kb
+};
+constexpr int kDynMaxStages = 4;
+
+template <bool PAD>
+__global__ void __launch_bounds__(256)
+    extract_dyn_kernel(const uint8_t* __restrict__ wf, const uint32_t n_traces,
+                       const uint32_t n_pixels, const uint32_t pix_inv,
+                       const int* __restrict__ pedestal, const float* __restrict__ gain,
+                       int* __restrict__ out_sum, int* __restrict__ out_start,
+                       float* __restrict__ out_charge, float* __restrict__ out_time,
+                       uint32_t* __restrict__ sched, const __grid_constant__ DynShape sh) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t full_bar[kDynMaxStages];
+  __shared__ uint32_t tile_q[kDynMaxStages + 1];
+  const int tid = threadIdx.x, NT = blockDim.x;
+  const int STAGES = sh.stages, QN = STAGES + 1;
+  const uint32_t tile_traces = (uint32_t)(NT * sh.tpt);
+  const uint32_t n_full = n_traces / tile_traces;
+  const uint32_t rem = n_traces - n_full * tile_traces;
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t bar_base = smem_u32(full_bar);
+
+  constexpr uint32_t kMaxRun = 8;
+  const uint32_t dyn_base = (uint32_t)STAGES * gridDim.x;
+  uint32_t static_next = blockIdx.x, cur = 0, end = 0, nxt = 0, n_run = 0;
+  auto fetch_static = [&]() -> uint32_t {
+    const uint32_t t = static_next;
+    static_next = (t > 0xFFFFFFFFu - gridDim.x) ? 0xFFFFFFFFu : t + gridDim.x;
+    return t;
+  };
+  auto run_length = [&](const uint32_t seen) -> uint32_t {
+    const uint32_t left = n_full > seen ? n_full - seen : 0u;
+    const uint32_t k = left / (8u * gridDim.x);
+    return k < 1u ? 1u : (k > kMaxRun ? kMaxRun : k);
+  };
+  auto fetch = [&]() -> uint32_t {
+    if (sched == nullptr) return fetch_static();
+    if (cur == end) {
+      cur = nxt;
+      end = nxt + n_run;
+      n_run = run_length(cur);
+      nxt = dyn_base + atomicAdd(sched, n_run);
+    }
+    return cur++;
+  };
+
+  if (tid == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(bar_base + 8 * s, PAD ? NT : 1);
+      tile_q[s] = fetch_static();
+    }
+    fence_mbar_init();
+    if (sched != nullptr) {
+      n_run = run_length(dyn_base);
+      nxt = dyn_base + atomicAdd(sched, n_run);
+    }
+  }
+  __syncthreads();
+
+  const uint32_t chunks_per_unit = (uint32_t)sh.unit_bytes / 16u;  // PAD only
+  auto issue = [&](const uint32_t tile, const int stage) {
+    const uint8_t* src = wf + (size_t)tile * (size_t)sh.tile_bytes;
+    const uint32_t dst = smem_base + (uint32_t)(stage * sh.stage_bytes);
+    const uint32_t bar = bar_base + 8 * stage;
+    if constexpr (!PAD) {
+      if (tid == 0) {
+        mbar_expect_tx(bar, (uint32_t)sh.tile_bytes);
+        tma_bulk_g2s(dst, src, (uint32_t)sh.tile_bytes, bar);
+      }
+    } else {
+      // chunk c of the tile belongs to unit c / chunks_per_unit: one chunk of padding per unit
+      const uint32_t n_chunks = (uint32_t)sh.tile_bytes / 16u;
+      uint32_t u = (uint32_t)tid / chunks_per_unit, r = (uint32_t)tid - u * chunks_per_unit;
+      const uint32_t du = (uint32_t)NT / chunks_per_unit, dr = (uint32_t)NT - du * chunks_per_unit;
+      for (uint32_t c = tid; c < n_chunks; c += NT) {
+        cp_async16(dst + (c + u) * 16u, src + (size_t)c * 16u);
+        u += du;
+        r += dr;
+        if (r >= chunks_per_unit) r -= chunks_per_unit, ++u;
+      }
+      cp_async_mbar_arrive(bar);
+    }
+  };
+
+  for (int s = 0; s < STAGES; ++s) {
+    const uint32_t tile = tile_q[s];
+    if (tile < n_full) issue(tile, s);
+  }
+  uint32_t pre = 0;
+  if (tid == 0) pre = fetch();
+
+  const int S = sh.S, W = sh.W, n_win = sh.n_win;
+  const uint32_t KM = sh.key_mul - 1u;
+  // lane group b = lane * g / 32 runs 2 b samples behind; d_max = 2 (g - 1)
+  const int d = 2 * (((tid & 31) * sh.g) >> 5), d_max = 2 * (sh.g - 1);
+
+  // steps a2-a7 of one unit (its first n_valid traces) at `unit` in shared memory
+  auto compute = [&](const uint8_t* unit, const uint32_t g0, const uint32_t n_valid, uint32_t p) {
+    for (int j = 0; j < sh.tpt; ++j) {
+      const uint16_t* x = reinterpret_cast<const uint16_t*>(unit) + j * S;
+      uint32_t sum = 0;
+      for (int k = 0; k < W; ++k) sum += x[k];
+      uint32_t best = sum * sh.key_mul + KM;
+      // window t = i - d enters x[t + W - 1] and leaves x[t - 1]; lanes outside
+      // [1, n_win) read neighbouring bytes of the stage and discard them
+      const uint16_t* xe = x + (W - 1 - d);
+      const uint16_t* xl = x - (1 + d);
+      uint32_t low = KM + (uint32_t)d;  // KM - t at i = 0
+#pragma unroll 4
+      for (int i = 1; i < n_win + d_max; ++i) {
+        const uint32_t e = xe[i], l = xl[i];
+        --low;
+        if ((uint32_t)(i - d - 1) < (uint32_t)(n_win - 1)) {
+          sum = sum + e - l;
+          best = max(best, sum * sh.key_mul + low);
+        }
+      }
+      const int tstar = (int)(KM - (best & KM));
+      const int rawsum = (int)(best >> sh.kb);
+      int relnum = 0;
+      for (int k = 1; k < W; ++k) relnum += k * (int)x[tstar + k];
+      const Result r = finish_trace(W, rawsum, tstar, relnum, __ldg(pedestal + p), __ldg(gain + p),
+                                    W, (W * (W - 1)) / 2);
+      if ((uint32_t)j < n_valid) {
+        __stcs(out_sum + g0 + j, r.sum);
+        __stcs(out_start + g0 + j, r.start);
+        __stcs(out_charge + g0 + j, r.charge);
+        __stcs(out_time + g0 + j, r.time);
+      }
+      p = (p + 1 == n_pixels) ? 0u : p + 1;
+    }
+  };
+
+  uint32_t tile;
+  for (uint32_t j = 0;; ++j) {
+    tile = tile_q[j % QN];
+    if (tile >= n_full) break;
+    const int stage = (int)(j % (uint32_t)STAGES);
+    const uint32_t parity = (j / (uint32_t)STAGES) & 1u;
+    if (tid == 0) {
+      tile_q[(j + STAGES) % QN] = pre;
+      pre = fetch();
+    }
+    mbar_wait(bar_base + 8 * stage, parity);
+    const uint8_t* unit = smem + stage * sh.stage_bytes + tid * sh.unit_stride;
+    const uint32_t g0 = tile * tile_traces + (uint32_t)(tid * sh.tpt);
+    compute(unit, g0, (uint32_t)sh.tpt, fastmod(g0, n_pixels, pix_inv));
+    __syncthreads();
+    const uint32_t next = tile_q[(j + STAGES) % QN];
+    if (next < n_full) issue(next, stage);
+  }
+
+  // ragged tail (< one tile of traces): plain copies, by the CTA that drew index n_full
+  if (rem != 0 && tile == n_full) {
+    const uint8_t* src = wf + (size_t)n_full * (size_t)sh.tile_bytes;  // 16-byte aligned
+    const uint32_t n_hw = rem * (uint32_t)S;                          // halfwords
+    const uint32_t unit_hw = (uint32_t)sh.unit_bytes / 2u, pad_hw = (uint32_t)(sh.unit_stride - sh.unit_bytes) / 2u;
+    for (uint32_t i = tid; i < n_hw; i += NT) {
+      const uint32_t dsti = PAD ? i + (i / unit_hw) * pad_hw : i;
+      reinterpret_cast<uint16_t*>(smem)[dsti] = reinterpret_cast<const uint16_t*>(src)[i];
+    }
+    __syncthreads();
+    const uint32_t first = (uint32_t)(tid * sh.tpt);
+    if (first < rem) {
+      const uint8_t* unit = smem + tid * sh.unit_stride;
+      const uint32_t g0 = n_full * tile_traces + first;
+      compute(unit, g0, rem - first, fastmod(g0, n_pixels, pix_inv));
+    }
+  }
+
+  if (sched != nullptr && tid == 0) {
+    __threadfence();
+    if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) {
+      sched[0] = 0;
+      sched[1] = 0;
+      __threadfence();
+    }
+  }
+}
+
 // ------------------------------------------------- mixed-camera batches ----
 // SURVEY.md §8(f) NEXT-3 (readings R28-R30). The host plan cuts every
 // block (one telescope, one event) into tiles of at most TILE_TRACES traces of
@@ -592,6 +799,7 @@ const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16, int bits)
     if (S == 40 && W == 7) return "tile<S=40,W=7>";
     if (S == 25 && W == 4) return "tile<S=25,W=4>";
     if (S == 128 && W == 8) return "tile<S=128,W=8>";
+    if (S >= 1 && S <= ((S & 1) ? 288 : 576)) return "staged<any>";  // dyn_shape: units up to 1152 bytes
   }
   return "generic";
 }
@@ -626,6 +834,66 @@ cudaError_t launch_generic(const LaunchArgs& a, const ModeArgs& ma) {
   return cudaGetLastError();
 }
 
+// Shape of the any-shape staged kernel for (S, W); false = not eligible (units
+// above 1152 bytes: the generic kernel takes them).
+bool dyn_shape(int32_t S, int32_t W, DynShape* sh, int* threads) {
+  const int tpt = (S & 1) ? 2 : 1;
+  const long long ub = 2ll * S * tpt;
+  if (ub > 1152) return false;
+  const bool pad = (ub % 32 == 0);  // word stride a multiple of 8: one chunk of padding
+  const int stride = (int)ub + (pad ? 16 : 0);
+  int g = 1;
+  while (g < 32 && (stride / 4) % (2 * g) == 0) g *= 2;
+  if (g > 4) return false;  // cannot happen (see the kernel's header)
+  const int nt = stride <= 144 ? 256 : stride <= 288 ? 128 : stride <= 576 ? 64 : 32;
+  sh->S = S;
+  sh->W = W;
+  sh->n_win = S - W + 1;
+  sh->tpt = tpt;
+  sh->unit_bytes = (int)ub;
+  sh->unit_stride = stride;
+  sh->tile_bytes = nt * (int)ub;
+  sh->stage_bytes = ((nt * stride + 64 + 127) / 128) * 128;
+  sh->stages = sh->stage_bytes <= 24 * 1024 ? 3 : 2;
+  sh->g = g;
+  sh->kb = ilog2_ceil(sh->n_win);
+  sh->key_mul = 1u << sh->kb;
+  *threads = nt;
+  return true;
+}
+
+cudaError_t launch_dyn(const LaunchArgs& a, const DynShape& sh, int threads) {
+  int dev = 0, sms = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
+  const bool pad = sh.unit_stride != sh.unit_bytes;
+  const void* kernel = pad ? (const void*)extract_dyn_kernel<true> : (const void*)extract_dyn_kernel<false>;
+  const int smem = sh.stages * sh.stage_bytes;
+  // the dynamic shared-memory size depends on the shape: set per launch (cheap)
+  if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess)
+    return e;
+  int occ = 0;
+  if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem)) != cudaSuccess)
+    return e;
+  if (occ < 1) return cudaErrorLaunchOutOfResources;
+  const uint32_t n_full = a.n_traces / (uint32_t)(threads * sh.tpt);
+  uint32_t grid = (uint32_t)(sms * occ);
+  if (grid > n_full) grid = n_full;
+  if (grid < 1) grid = 1;
+  uint32_t* sched = g_static_schedule ? nullptr : sched_words(dev, a.stream);
+  if (pad)
+    extract_dyn_kernel<true><<<grid, threads, smem, a.stream>>>(
+        a.wf, a.n_traces, a.n_pixels, a.pix_inv, a.pedestal, a.gain, a.out_sum, a.out_start,
+        a.out_charge, a.out_time, sched, sh);
+  else
+    extract_dyn_kernel<false><<<grid, threads, smem, a.stream>>>(
+        a.wf, a.n_traces, a.n_pixels, a.pix_inv, a.pedestal, a.gain, a.out_sum, a.out_start,
+        a.out_charge, a.out_time, sched, sh);
+  rta_count_launch();
+  return cudaGetLastError();
+}
+
 #define RTA_TRY(CFG)                                                                          \
   if (a.S == CFG::S && a.W == CFG::W)                                                         \
     return TileLauncher<CFG, MODE>::launch(a.wf, a.n_traces, a.n_pixels, a.pix_inv,           \
@@ -638,6 +906,11 @@ cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
     RTA_TRY(CfgS40W7)
     RTA_TRY(CfgS25W4)
     RTA_TRY(CfgS128W8)
+    if constexpr (MODE == MODE_SLIDING) {
+      DynShape sh;
+      int threads = 0;
+      if (dyn_shape(a.S, a.W, &sh, &threads)) return launch_dyn(a, sh, threads);
+    }
   }
   return launch_generic<MODE, 16>(a, ma);
 }
