@@ -426,6 +426,45 @@ def ragged_leg(steps, peak, torch, dl0gen, rta, n_events=1000):
     return res
 
 
+def any_shape_leg(steps, peak, torch, dl0gen, rta):
+    """Shapes without a specialised kernel (not BASELINE configs: C2's and C4's
+    signal models with other readout lengths / window widths) through rta_extract:
+    the staged kernel with runtime (S, W), next to the old generic kernel."""
+    import dataclasses
+    c2, c4 = dl0gen.CONFIGS["C2"], dl0gen.CONFIGS["C4"]
+    shapes = [dataclasses.replace(c2, name="X60", label="10000x1855x60 W=7", seed=11, n_samples=60,
+                                  peak_lo=15.0, peak_hi=45.0),
+              dataclasses.replace(c2, name="X40w5", label="10000x1855x40 W=5", seed=12, W=5),
+              dataclasses.replace(c4, name="X96", label="10000x2048x96 W=8", seed=13, n_events=10_000,
+                                  n_samples=96, peak_lo=25.0, peak_hi=70.0),
+              dataclasses.replace(c4, name="X128w10", label="10000x2048x128 W=10", seed=14,
+                                  n_events=10_000, W=10)]
+    res = {}
+    for cfg in shapes:
+        d_wf, d_ped, d_gain, outs, ped, gain = device_batch(cfg, torch, dl0gen)
+        stream = torch.cuda.current_stream()
+        base = (d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain, cfg.W)
+        r = {"kernel": rta.rta_kernel_name(cfg.n_samples, cfg.W, True)}
+        ref = None
+        for name, generic in (("staged_any", False), ("generic", True)):
+            def run():
+                rta.rta_extract(*base, *outs, stream=stream, generic=generic)
+            for _ in range(3):
+                run()
+            torch.cuda.synchronize()
+            r[name] = summarise(cfg, time_steps(run, steps if not generic else 3, stream), peak)
+            got = [o.clone() for o in outs]
+            if ref is not None:
+                r["both_kernels_bit_identical"] = all(
+                    bool((a.view(torch.int32) == b.view(torch.int32)).all()) for a, b in zip(ref, got))
+            ref = got
+        r["speedup_vs_generic"] = r["generic"]["ms_avg"] / r["staged_any"]["ms_avg"]
+        res[cfg.name] = r
+        del d_wf, outs, ref, got
+        torch.cuda.empty_cache()
+    return res
+
+
 EVENT_OUT_BYTES = 36   # n_pix int32 + 8 fp32 parameters per event
 
 
@@ -839,6 +878,8 @@ def main():
                                       torch, dl0gen, rta)
                 torch.cuda.empty_cache()
             out["packed12"] = pk
+            out["any_shape"] = any_shape_leg(max(10, args.steps // 4), peak, torch, dl0gen, rta)
+            torch.cuda.empty_cache()
             out["ragged"] = ragged_leg(max(10, args.steps // 4), peak, torch, dl0gen, rta)
             torch.cuda.empty_cache()
             img = {}

@@ -251,7 +251,7 @@ struct DynShape {
 };
 constexpr int kDynMaxStages = 4;
 
-template <bool PAD>
+template <bool PAD, int G>
 __global__ void __launch_bounds__(256)
     extract_dyn_kernel(const uint8_t* __restrict__ wf, const uint32_t n_traces,
                        const uint32_t n_pixels, const uint32_t pix_inv,
@@ -342,13 +342,15 @@ __global__ void __launch_bounds__(256)
   const int S = sh.S, W = sh.W, n_win = sh.n_win;
   const uint32_t KM = sh.key_mul - 1u;
   // lane group b = lane * g / 32 runs 2 b samples behind; d_max = 2 (g - 1)
-  const int d = 2 * (((tid & 31) * sh.g) >> 5), d_max = 2 * (sh.g - 1);
+  const int d = 2 * (((tid & 31) * G) >> 5);
+  constexpr int d_max = 2 * (G - 1);
 
   // steps a2-a7 of one unit (its first n_valid traces) at `unit` in shared memory
   auto compute = [&](const uint8_t* unit, const uint32_t g0, const uint32_t n_valid, uint32_t p) {
     for (int j = 0; j < sh.tpt; ++j) {
       const uint16_t* x = reinterpret_cast<const uint16_t*>(unit) + j * S;
       uint32_t sum = 0;
+#pragma unroll 4
       for (int k = 0; k < W; ++k) sum += x[k];
       uint32_t best = sum * sh.key_mul + KM;
       // window t = i - d enters x[t + W - 1] and leaves x[t - 1]; lanes outside
@@ -356,18 +358,37 @@ __global__ void __launch_bounds__(256)
       const uint16_t* xe = x + (W - 1 - d);
       const uint16_t* xl = x - (1 + d);
       uint32_t low = KM + (uint32_t)d;  // KM - t at i = 0
-#pragma unroll 4
-      for (int i = 1; i < n_win + d_max; ++i) {
+      const uint32_t mul = sh.key_mul;
+      const auto guarded = [&](const int i) {  // a step some lane groups sit out
         const uint32_t e = xe[i], l = xl[i];
         --low;
         if ((uint32_t)(i - d - 1) < (uint32_t)(n_win - 1)) {
           sum = sum + e - l;
-          best = max(best, sum * sh.key_mul + low);
+          best = max(best, sum * mul + low);
         }
+      };
+      int i = 1;
+      if (n_win > d_max) {
+        // head: the lane groups start one after the other
+#pragma unroll
+        for (int h = 0; h < d_max; ++h) guarded(i++);
+        // steady state: every lane has a window, no predicates
+#pragma unroll 8
+        for (; i < n_win; ++i) {
+          sum = sum + xe[i] - xl[i];
+          --low;
+          best = max(best, sum * mul + low);
+        }
+        // tail: the lane groups finish one after the other
+#pragma unroll
+        for (int h = 0; h < d_max; ++h) guarded(i++);
+      } else {
+        for (; i < n_win + d_max; ++i) guarded(i);
       }
       const int tstar = (int)(KM - (best & KM));
       const int rawsum = (int)(best >> sh.kb);
       int relnum = 0;
+#pragma unroll 4
       for (int k = 1; k < W; ++k) relnum += k * (int)x[tstar + k];
       const Result r = finish_trace(W, rawsum, tstar, relnum, __ldg(pedestal + p), __ldg(gain + p),
                                     W, (W * (W - 1)) / 2);
@@ -844,7 +865,7 @@ bool dyn_shape(int32_t S, int32_t W, DynShape* sh, int* threads) {
   const int stride = (int)ub + (pad ? 16 : 0);
   int g = 1;
   while (g < 32 && (stride / 4) % (2 * g) == 0) g *= 2;
-  if (g > 4) return false;  // cannot happen (see the kernel's header)
+  if (g > 4 || (pad && g != 4)) return false;  // cannot happen (see the kernel's header)
   const int nt = stride <= 144 ? 256 : stride <= 288 ? 128 : stride <= 576 ? 64 : 32;
   sh->S = S;
   sh->W = W;
@@ -854,7 +875,7 @@ bool dyn_shape(int32_t S, int32_t W, DynShape* sh, int* threads) {
   sh->unit_stride = stride;
   sh->tile_bytes = nt * (int)ub;
   sh->stage_bytes = ((nt * stride + 64 + 127) / 128) * 128;
-  sh->stages = sh->stage_bytes <= 24 * 1024 ? 3 : 2;
+  sh->stages = 2;  // more resident CTAs beat a deeper ring (registers allow 32 warps per SM)
   sh->g = g;
   sh->kb = ilog2_ceil(sh->n_win);
   sh->key_mul = 1u << sh->kb;
@@ -868,7 +889,13 @@ cudaError_t launch_dyn(const LaunchArgs& a, const DynShape& sh, int threads) {
   if (e != cudaSuccess) return e;
   if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
   const bool pad = sh.unit_stride != sh.unit_bytes;
-  const void* kernel = pad ? (const void*)extract_dyn_kernel<true> : (const void*)extract_dyn_kernel<false>;
+  using Kernel = void (*)(const uint8_t*, uint32_t, uint32_t, uint32_t, const int*, const float*, int*,
+                          int*, float*, float*, uint32_t*, DynShape);
+  // unpadded layouts have g = 1, 2 or 4; the padded one always 4
+  const Kernel kernel = pad          ? extract_dyn_kernel<true, 4>
+                        : sh.g == 1 ? extract_dyn_kernel<false, 1>
+                        : sh.g == 2 ? extract_dyn_kernel<false, 2>
+                                    : extract_dyn_kernel<false, 4>;
   const int smem = sh.stages * sh.stage_bytes;
   // the dynamic shared-memory size depends on the shape: set per launch (cheap)
   if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess)
@@ -882,14 +909,9 @@ cudaError_t launch_dyn(const LaunchArgs& a, const DynShape& sh, int threads) {
   if (grid > n_full) grid = n_full;
   if (grid < 1) grid = 1;
   uint32_t* sched = g_static_schedule ? nullptr : sched_words(dev, a.stream);
-  if (pad)
-    extract_dyn_kernel<true><<<grid, threads, smem, a.stream>>>(
-        a.wf, a.n_traces, a.n_pixels, a.pix_inv, a.pedestal, a.gain, a.out_sum, a.out_start,
-        a.out_charge, a.out_time, sched, sh);
-  else
-    extract_dyn_kernel<false><<<grid, threads, smem, a.stream>>>(
-        a.wf, a.n_traces, a.n_pixels, a.pix_inv, a.pedestal, a.gain, a.out_sum, a.out_start,
-        a.out_charge, a.out_time, sched, sh);
+  kernel<<<grid, threads, smem, a.stream>>>(a.wf, a.n_traces, a.n_pixels, a.pix_inv, a.pedestal,
+                                            a.gain, a.out_sum, a.out_start, a.out_charge,
+                                            a.out_time, sched, sh);
   rta_count_launch();
   return cudaGetLastError();
 }

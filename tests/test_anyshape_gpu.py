@@ -1,0 +1,92 @@
+"""GPU parity of the any-shape staged kernel (runtime S and W)
+against the oracle, through rta_extract: every combination of the kernel's
+cases — word stride odd / 2 mod 4 / 0 mod 4 (lane groups skewed by one word),
+units of a multiple of 32 bytes (padded layout, 16-byte cp.async ingest), odd S
+(two traces per thread), fewer windows than the skew, W = 1 and W = S, several
+tiles per CTA plus a ragged tail, cameras smaller than a unit (the calibration
+index wraps inside a unit). The old generic kernel must agree bit for bit."""
+import numpy as np
+import pytest
+
+import oracle
+from tests._gpu import bit_identical, run_gpu
+
+pytestmark = pytest.mark.gpu
+
+# (S, W): words per unit s, g = gcd(s, 32) -> case
+SHAPES = [
+    (50, 8),     # s = 25, g = 1
+    (60, 7),     # s = 30, g = 2
+    (20, 3),     # s = 10, g = 2
+    (40, 5),     # s = 20, g = 4
+    (24, 24),    # s = 12, g = 4, one window
+    (40, 38),    # three windows, fewer than the skew of 6
+    (200, 9),    # s = 100, g = 4, 128 threads per CTA
+    (96, 8),     # 192-byte units: padded layout
+    (128, 10),   # 256-byte units: padded layout, 128 threads
+    (64, 1),     # padded, W = 1
+    (16, 5),     # 32-byte units: padded, 48-byte stride
+    (576, 12),   # the largest unit (1152 bytes), 32 threads per CTA
+    (33, 5),     # odd S: two traces per thread, s = 33
+    (27, 27),    # odd S, one window
+    (3, 2), (2, 1), (1, 1),
+    (287, 6),    # odd S, 1148-byte units
+]
+
+
+@pytest.mark.parametrize("S,W", SHAPES)
+@pytest.mark.parametrize("E,P", [(1, 1), (5, 3), (3, 700), (2, 5000)])
+def test_any_shape_random(S, W, E, P):
+    import paper_1307_6489_b200 as rta
+    assert rta.rta_kernel_name(S, W) == "staged<any>"
+    if E * P * S > 3_000_000:
+        E = 1
+    rng = np.random.default_rng(S * 1009 + W * 31 + E * P)
+    full = (S + W) % 2 == 0
+    hi = 65536 if full else 4096
+    wf = rng.integers(0, hi, size=(E, P, S)).astype(np.uint16)
+    wf[rng.random((E, P)) < 0.15] = hi - 1                     # all windows tie
+    wf[rng.random((E, P)) < 0.15] //= np.uint16(hi // 2)       # tie-heavy
+    ped = (rng.integers(-70000, 70000, P) if full else rng.integers(0, 600, P)).astype(np.int32)
+    gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
+    want = oracle.extract(wf, ped, gain, W)
+    got = run_gpu(wf, ped, gain, W)
+    assert (got[0] == want[0]).all() and (got[1] == want[1]).all()
+    assert bit_identical(got, want)
+    old = run_gpu(wf, ped, gain, W, generic=True)
+    assert bit_identical(got, old)
+
+
+@pytest.mark.parametrize("S,W", [(60, 7), (40, 5), (96, 8), (33, 5)])
+def test_any_shape_many_tiles_both_schedules(S, W):
+    """Several tiles per CTA, dynamic and static tile schedules, a ragged tail
+    of every length class (odd number of traces for the two-traces-per-thread case)."""
+    import paper_1307_6489_b200 as rta
+    rng = np.random.default_rng(S)
+    E, P = 37, 1855 + (S % 2)
+    wf = (400 + rng.normal(0, 4, (E, P, S))).round().clip(0, 4095).astype(np.uint16)
+    wf[:, ::11, S // 3: S // 3 + 4] += np.uint16(300)
+    ped = rng.integers(380, 421, P).astype(np.int32)
+    gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
+    want = oracle.extract(wf, ped, gain, W)
+    for static in (False, True):
+        rta.rta_debug_static_schedule(static)
+        try:
+            got = run_gpu(wf, ped, gain, W)
+        finally:
+            rta.rta_debug_static_schedule(False)
+        assert bit_identical(got, want)
+
+
+def test_any_shape_closed_forms():
+    """Delta at every position and constant traces (SURVEY.md pins P1, P2) for a
+    g = 4 shape: earliest of the tied windows through the skewed lane groups."""
+    S, W, ped = 40, 5, 100
+    wf = np.full((1, S + 1, S), ped, np.uint16)
+    for k in range(S):
+        wf[0, k, k] = ped + 50
+    wf[0, S, :] = 777
+    got = run_gpu(wf, np.full(S + 1, ped, np.int32), np.ones(S + 1, np.float32), W)
+    for k in range(S):
+        assert got[0][k] == 50 and got[1][k] == max(0, k - W + 1) and got[3][k] == np.float32(k)
+    assert got[0][S] == W * (777 - ped) and got[1][S] == 0 and got[3][S] == np.float32((W - 1) / 2)
