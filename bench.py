@@ -352,6 +352,9 @@ def family_leg(cfg, steps, peak, torch, dl0gen, rta):
         torch.cuda.synchronize()
         res[name] = summarise(cfg, time_steps(run, steps, stream), peak)
     res["fir"]["taps"] = taps
+    res["fixed"]["note"] = ("reads W samples per trace; traces longer than 96 bytes are gathered from global "
+                            "memory instead of streamed, so GB/s figures (which count the whole waveform) can "
+                            "exceed the HBM peak")
     return res
 
 

@@ -248,17 +248,19 @@ struct DynShape {
   int32_t g;            // gcd(unit_stride / 4, 32): 1, 2 or 4
   int32_t kb;           // key bits: 2^kb >= n_win
   uint32_t key_mul;     // 2^kb
+  uint32_t peak_mul;    // local peak: 2^ceil(log2 S)
 };
 constexpr int kDynMaxStages = 4;
 
-template <bool PAD, int G>
+template <bool PAD, int G, int MODE>
 __global__ void __launch_bounds__(256)
     extract_dyn_kernel(const uint8_t* __restrict__ wf, const uint32_t n_traces,
                        const uint32_t n_pixels, const uint32_t pix_inv,
                        const int* __restrict__ pedestal, const float* __restrict__ gain,
                        int* __restrict__ out_sum, int* __restrict__ out_start,
                        float* __restrict__ out_charge, float* __restrict__ out_time,
-                       uint32_t* __restrict__ sched, const __grid_constant__ DynShape sh) {
+                       uint32_t* __restrict__ sched, const __grid_constant__ DynShape sh,
+                       const __grid_constant__ ModeArgs ma) {
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ __align__(8) uint64_t full_bar[kDynMaxStages];
   __shared__ uint32_t tile_q[kDynMaxStages + 1];
@@ -349,49 +351,80 @@ __global__ void __launch_bounds__(256)
   auto compute = [&](const uint8_t* unit, const uint32_t g0, const uint32_t n_valid, uint32_t p) {
     for (int j = 0; j < sh.tpt; ++j) {
       const uint16_t* x = reinterpret_cast<const uint16_t*>(unit) + j * S;
-      uint32_t sum = 0;
-#pragma unroll 4
-      for (int k = 0; k < W; ++k) sum += x[k];
-      uint32_t best = sum * sh.key_mul + KM;
-      // window t = i - d enters x[t + W - 1] and leaves x[t - 1]; lanes outside
-      // [1, n_win) read neighbouring bytes of the stage and discard them
-      const uint16_t* xe = x + (W - 1 - d);
-      const uint16_t* xl = x - (1 + d);
-      uint32_t low = KM + (uint32_t)d;  // KM - t at i = 0
-      const uint32_t mul = sh.key_mul;
-      const auto guarded = [&](const int i) {  // a step some lane groups sit out
-        const uint32_t e = xe[i], l = xl[i];
-        --low;
-        if ((uint32_t)(i - d - 1) < (uint32_t)(n_win - 1)) {
-          sum = sum + e - l;
-          best = max(best, sum * mul + low);
+      int tstar = 0, rawsum = 0, relnum = 0;
+      // a loop of `n` steps in which lane group b handles index i - d at step i:
+      // `body(index)` for the lanes whose index lies in [first, first + n)
+      const auto skewed = [&](const int first, const int n, auto&& body) {
+        int i = first;
+        if (n > d_max) {
+#pragma unroll
+          for (int h = 0; h < d_max; ++h, ++i)  // head: the groups start one after the other
+            if ((uint32_t)(i - d - first) < (uint32_t)n) body(i - d);
+#pragma unroll 8
+          for (; i < first + n; ++i) body(i - d);  // steady state: no predicates
+#pragma unroll
+          for (int h = 0; h < d_max; ++h, ++i)  // tail: the groups finish one after the other
+            if ((uint32_t)(i - d - first) < (uint32_t)n) body(i - d);
+        } else {
+          for (; i < first + n + d_max; ++i)
+            if ((uint32_t)(i - d - first) < (uint32_t)n) body(i - d);
         }
       };
-      int i = 1;
-      if (n_win > d_max) {
-        // head: the lane groups start one after the other
-#pragma unroll
-        for (int h = 0; h < d_max; ++h) guarded(i++);
-        // steady state: every lane has a window, no predicates
-#pragma unroll 8
-        for (; i < n_win; ++i) {
-          sum = sum + xe[i] - xl[i];
+      if constexpr (MODE == MODE_SLIDING) {
+        uint32_t sum = 0;
+#pragma unroll 4
+        for (int k = 0; k < W; ++k) sum += x[k];
+        uint32_t best = sum * sh.key_mul + KM;
+        // window t enters x[t + W - 1] and leaves x[t - 1]; lanes outside [1, n_win)
+        // read neighbouring bytes of the stage and discard them
+        const uint32_t mul = sh.key_mul;
+        const uint16_t* xe = x + (W - 1);
+        const uint16_t* xl = x - 1;
+        uint32_t low = KM;  // KM - t: every lane visits t = 1, 2, ... in order
+        skewed(1, n_win - 1, [&](const int t) {
+          sum = sum + xe[t] - xl[t];
           --low;
           best = max(best, sum * mul + low);
-        }
-        // tail: the lane groups finish one after the other
-#pragma unroll
-        for (int h = 0; h < d_max; ++h) guarded(i++);
-      } else {
-        for (; i < n_win + d_max; ++i) guarded(i);
-      }
-      const int tstar = (int)(KM - (best & KM));
-      const int rawsum = (int)(best >> sh.kb);
-      int relnum = 0;
+        });
+        tstar = (int)(KM - (best & KM));
+        rawsum = (int)(best >> sh.kb);
 #pragma unroll 4
-      for (int k = 1; k < W; ++k) relnum += k * (int)x[tstar + k];
+        for (int k = 1; k < W; ++k) relnum += k * (int)x[tstar + k];
+      } else if constexpr (MODE == MODE_FIR) {
+        // response on raw samples; strict '>' scanning upwards = earliest on ties
+        int best = 0;
+        for (int k = 0; k < W; ++k) best += ma.taps[k] * (int)x[k];
+        skewed(1, n_win - 1, [&](const int t) {
+          int y = 0;
+#pragma unroll 4
+          for (int k = 0; k < W; ++k) y += ma.taps[k] * (int)x[t + k];
+          if (y > best) best = y, tstar = t;
+        });
+        rawsum = best;
+        for (int k = 1; k < W; ++k) relnum += k * ma.taps[k] * (int)x[tstar + k];
+      } else {
+        if constexpr (MODE == MODE_FIXED) {
+          tstar = clamp_start(__ldg(ma.window_start + p), S, W);
+        } else {  // MODE_LOCAL_PEAK: largest sample, earliest on ties
+          const uint32_t pmul = sh.peak_mul, PM = sh.peak_mul - 1u;
+          uint32_t best = (uint32_t)x[0] * pmul + PM;
+          skewed(1, S - 1, [&](const int k) {
+            best = max(best, (uint32_t)x[k] * pmul + (PM - (uint32_t)k));
+          });
+          tstar = clamp_start((int)(PM - (best & PM)) - ma.shift, S, W);
+        }
+        rawsum = (int)x[tstar];
+#pragma unroll 4
+        for (int k = 1; k < W; ++k) {
+          const int v = (int)x[tstar + k];
+          rawsum += v;
+          relnum += k * v;
+        }
+      }
+      const int c0 = (MODE == MODE_FIR) ? ma.c0 : W;
+      const int c1 = (MODE == MODE_FIR) ? ma.c1 : (W * (W - 1)) / 2;
       const Result r = finish_trace(W, rawsum, tstar, relnum, __ldg(pedestal + p), __ldg(gain + p),
-                                    W, (W * (W - 1)) / 2);
+                                    c0, c1);
       if ((uint32_t)j < n_valid) {
         __stcs(out_sum + g0 + j, r.sum);
         __stcs(out_start + g0 + j, r.start);
@@ -879,23 +912,25 @@ bool dyn_shape(int32_t S, int32_t W, DynShape* sh, int* threads) {
   sh->g = g;
   sh->kb = ilog2_ceil(sh->n_win);
   sh->key_mul = 1u << sh->kb;
+  sh->peak_mul = 1u << ilog2_ceil(S);
   *threads = nt;
   return true;
 }
 
-cudaError_t launch_dyn(const LaunchArgs& a, const DynShape& sh, int threads) {
+template <int MODE>
+cudaError_t launch_dyn(const LaunchArgs& a, const DynShape& sh, int threads, const ModeArgs& ma) {
   int dev = 0, sms = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
   const bool pad = sh.unit_stride != sh.unit_bytes;
   using Kernel = void (*)(const uint8_t*, uint32_t, uint32_t, uint32_t, const int*, const float*, int*,
-                          int*, float*, float*, uint32_t*, DynShape);
+                          int*, float*, float*, uint32_t*, DynShape, ModeArgs);
   // unpadded layouts have g = 1, 2 or 4; the padded one always 4
-  const Kernel kernel = pad          ? extract_dyn_kernel<true, 4>
-                        : sh.g == 1 ? extract_dyn_kernel<false, 1>
-                        : sh.g == 2 ? extract_dyn_kernel<false, 2>
-                                    : extract_dyn_kernel<false, 4>;
+  const Kernel kernel = pad          ? extract_dyn_kernel<true, 4, MODE>
+                        : sh.g == 1 ? extract_dyn_kernel<false, 1, MODE>
+                        : sh.g == 2 ? extract_dyn_kernel<false, 2, MODE>
+                                    : extract_dyn_kernel<false, 4, MODE>;
   const int smem = sh.stages * sh.stage_bytes;
   // the dynamic shared-memory size depends on the shape: set per launch (cheap)
   if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess)
@@ -911,7 +946,7 @@ cudaError_t launch_dyn(const LaunchArgs& a, const DynShape& sh, int threads) {
   uint32_t* sched = g_static_schedule ? nullptr : sched_words(dev, a.stream);
   kernel<<<grid, threads, smem, a.stream>>>(a.wf, a.n_traces, a.n_pixels, a.pix_inv, a.pedestal,
                                             a.gain, a.out_sum, a.out_start, a.out_charge,
-                                            a.out_time, sched, sh);
+                                            a.out_time, sched, sh, ma);
   rta_count_launch();
   return cudaGetLastError();
 }
@@ -923,16 +958,18 @@ cudaError_t launch_dyn(const LaunchArgs& a, const DynShape& sh, int threads) {
                                            a.out_charge, a.out_time, a.stream, ma);
 template <int MODE>
 cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
-  if (a.staged) {
+  // The fixed window touches W samples of a trace: beyond about three 32-byte
+  // sectors per trace, gathering them from global memory (the generic kernel)
+  // moves less than streaming whole tiles (S = 128: 0.99 ms against 1.69 ms).
+  const bool gather = (MODE == MODE_FIXED) && 2 * a.S > 96;
+  if (a.staged && !gather) {
     RTA_TRY(CfgS30W7)
     RTA_TRY(CfgS40W7)
     RTA_TRY(CfgS25W4)
     RTA_TRY(CfgS128W8)
-    if constexpr (MODE == MODE_SLIDING) {
-      DynShape sh;
-      int threads = 0;
-      if (dyn_shape(a.S, a.W, &sh, &threads)) return launch_dyn(a, sh, threads);
-    }
+    DynShape sh;
+    int threads = 0;
+    if (dyn_shape(a.S, a.W, &sh, &threads)) return launch_dyn<MODE>(a, sh, threads, ma);
   }
   return launch_generic<MODE, 16>(a, ma);
 }
