@@ -252,6 +252,106 @@ struct DynShape {
 };
 constexpr int kDynMaxStages = 4;
 
+// Steps a2-a7 of one unit (its first n_valid traces) at `unit` in shared memory,
+// shape and extractor as kernel arguments. p: calibration index of the unit's
+// first trace; it wraps to 0 after n_pixels - 1 (n_pixels = 0 never wraps).
+template <int G, int MODE>
+__device__ __forceinline__ void dyn_compute_unit(
+    const DynShape& sh, const ModeArgs& ma, const uint8_t* unit, const uint32_t g0,
+    const uint32_t n_valid, uint32_t p, const uint32_t n_pixels, const int* __restrict__ pedestal,
+    const float* __restrict__ gain, int* __restrict__ out_sum, int* __restrict__ out_start,
+    float* __restrict__ out_charge, float* __restrict__ out_time) {
+  const int S = sh.S, W = sh.W, n_win = sh.n_win;
+  const uint32_t KM = sh.key_mul - 1u;
+  // lane group b = lane * g / 32 runs 2 b samples behind; d_max = 2 (g - 1)
+  const int d = 2 * ((((int)threadIdx.x & 31) * G) >> 5);
+  constexpr int d_max = 2 * (G - 1);
+  for (int j = 0; j < sh.tpt; ++j) {
+    const uint16_t* x = reinterpret_cast<const uint16_t*>(unit) + j * S;
+    int tstar = 0, rawsum = 0, relnum = 0;
+    // a loop of `n` steps in which lane group b handles index i - d at step i:
+    // `body(index)` for the lanes whose index lies in [first, first + n)
+    const auto skewed = [&](const int first, const int n, auto&& body) {
+      int i = first;
+      if (n > d_max) {
+#pragma unroll
+        for (int h = 0; h < d_max; ++h, ++i)  // head: the groups start one after the other
+          if ((uint32_t)(i - d - first) < (uint32_t)n) body(i - d);
+#pragma unroll 8
+        for (; i < first + n; ++i) body(i - d);  // steady state: no predicates
+#pragma unroll
+        for (int h = 0; h < d_max; ++h, ++i)  // tail: the groups finish one after the other
+          if ((uint32_t)(i - d - first) < (uint32_t)n) body(i - d);
+      } else {
+        for (; i < first + n + d_max; ++i)
+          if ((uint32_t)(i - d - first) < (uint32_t)n) body(i - d);
+      }
+    };
+    if constexpr (MODE == MODE_SLIDING) {
+      uint32_t sum = 0;
+#pragma unroll 4
+      for (int k = 0; k < W; ++k) sum += x[k];
+      uint32_t best = sum * sh.key_mul + KM;
+      // window t enters x[t + W - 1] and leaves x[t - 1]; lanes outside [1, n_win)
+      // read neighbouring bytes of the stage and discard them
+      const uint32_t mul = sh.key_mul;
+      const uint16_t* xe = x + (W - 1);
+      const uint16_t* xl = x - 1;
+      uint32_t low = KM;  // KM - t: every lane visits t = 1, 2, ... in order
+      skewed(1, n_win - 1, [&](const int t) {
+        sum = sum + xe[t] - xl[t];
+        --low;
+        best = max(best, sum * mul + low);
+      });
+      tstar = (int)(KM - (best & KM));
+      rawsum = (int)(best >> sh.kb);
+#pragma unroll 4
+      for (int k = 1; k < W; ++k) relnum += k * (int)x[tstar + k];
+    } else if constexpr (MODE == MODE_FIR) {
+      // response on raw samples; strict '>' scanning upwards = earliest on ties
+      int best = 0;
+      for (int k = 0; k < W; ++k) best += ma.taps[k] * (int)x[k];
+      skewed(1, n_win - 1, [&](const int t) {
+        int y = 0;
+#pragma unroll 4
+        for (int k = 0; k < W; ++k) y += ma.taps[k] * (int)x[t + k];
+        if (y > best) best = y, tstar = t;
+      });
+      rawsum = best;
+      for (int k = 1; k < W; ++k) relnum += k * ma.taps[k] * (int)x[tstar + k];
+    } else {
+      if constexpr (MODE == MODE_FIXED) {
+        tstar = clamp_start(__ldg(ma.window_start + p), S, W);
+      } else {  // MODE_LOCAL_PEAK: largest sample, earliest on ties
+        const uint32_t pmul = sh.peak_mul, PM = sh.peak_mul - 1u;
+        uint32_t best = (uint32_t)x[0] * pmul + PM;
+        skewed(1, S - 1, [&](const int k) {
+          best = max(best, (uint32_t)x[k] * pmul + (PM - (uint32_t)k));
+        });
+        tstar = clamp_start((int)(PM - (best & PM)) - ma.shift, S, W);
+      }
+      rawsum = (int)x[tstar];
+#pragma unroll 4
+      for (int k = 1; k < W; ++k) {
+        const int v = (int)x[tstar + k];
+        rawsum += v;
+        relnum += k * v;
+      }
+    }
+    const int c0 = (MODE == MODE_FIR) ? ma.c0 : W;
+    const int c1 = (MODE == MODE_FIR) ? ma.c1 : (W * (W - 1)) / 2;
+    const Result r = finish_trace(W, rawsum, tstar, relnum, __ldg(pedestal + p), __ldg(gain + p),
+                                  c0, c1);
+    if ((uint32_t)j < n_valid) {
+      __stcs(out_sum + g0 + j, r.sum);
+      __stcs(out_start + g0 + j, r.start);
+      __stcs(out_charge + g0 + j, r.charge);
+      __stcs(out_time + g0 + j, r.time);
+    }
+    p = (p + 1 == n_pixels) ? 0u : p + 1;
+  }
+}
+
 template <bool PAD, int G, int MODE>
 __global__ void __launch_bounds__(256)
     extract_dyn_kernel(const uint8_t* __restrict__ wf, const uint32_t n_traces,
@@ -341,98 +441,11 @@ __global__ void __launch_bounds__(256)
   uint32_t pre = 0;
   if (tid == 0) pre = fetch();
 
-  const int S = sh.S, W = sh.W, n_win = sh.n_win;
-  const uint32_t KM = sh.key_mul - 1u;
-  // lane group b = lane * g / 32 runs 2 b samples behind; d_max = 2 (g - 1)
-  const int d = 2 * (((tid & 31) * G) >> 5);
-  constexpr int d_max = 2 * (G - 1);
+  const int S = sh.S;
 
-  // steps a2-a7 of one unit (its first n_valid traces) at `unit` in shared memory
-  auto compute = [&](const uint8_t* unit, const uint32_t g0, const uint32_t n_valid, uint32_t p) {
-    for (int j = 0; j < sh.tpt; ++j) {
-      const uint16_t* x = reinterpret_cast<const uint16_t*>(unit) + j * S;
-      int tstar = 0, rawsum = 0, relnum = 0;
-      // a loop of `n` steps in which lane group b handles index i - d at step i:
-      // `body(index)` for the lanes whose index lies in [first, first + n)
-      const auto skewed = [&](const int first, const int n, auto&& body) {
-        int i = first;
-        if (n > d_max) {
-#pragma unroll
-          for (int h = 0; h < d_max; ++h, ++i)  // head: the groups start one after the other
-            if ((uint32_t)(i - d - first) < (uint32_t)n) body(i - d);
-#pragma unroll 8
-          for (; i < first + n; ++i) body(i - d);  // steady state: no predicates
-#pragma unroll
-          for (int h = 0; h < d_max; ++h, ++i)  // tail: the groups finish one after the other
-            if ((uint32_t)(i - d - first) < (uint32_t)n) body(i - d);
-        } else {
-          for (; i < first + n + d_max; ++i)
-            if ((uint32_t)(i - d - first) < (uint32_t)n) body(i - d);
-        }
-      };
-      if constexpr (MODE == MODE_SLIDING) {
-        uint32_t sum = 0;
-#pragma unroll 4
-        for (int k = 0; k < W; ++k) sum += x[k];
-        uint32_t best = sum * sh.key_mul + KM;
-        // window t enters x[t + W - 1] and leaves x[t - 1]; lanes outside [1, n_win)
-        // read neighbouring bytes of the stage and discard them
-        const uint32_t mul = sh.key_mul;
-        const uint16_t* xe = x + (W - 1);
-        const uint16_t* xl = x - 1;
-        uint32_t low = KM;  // KM - t: every lane visits t = 1, 2, ... in order
-        skewed(1, n_win - 1, [&](const int t) {
-          sum = sum + xe[t] - xl[t];
-          --low;
-          best = max(best, sum * mul + low);
-        });
-        tstar = (int)(KM - (best & KM));
-        rawsum = (int)(best >> sh.kb);
-#pragma unroll 4
-        for (int k = 1; k < W; ++k) relnum += k * (int)x[tstar + k];
-      } else if constexpr (MODE == MODE_FIR) {
-        // response on raw samples; strict '>' scanning upwards = earliest on ties
-        int best = 0;
-        for (int k = 0; k < W; ++k) best += ma.taps[k] * (int)x[k];
-        skewed(1, n_win - 1, [&](const int t) {
-          int y = 0;
-#pragma unroll 4
-          for (int k = 0; k < W; ++k) y += ma.taps[k] * (int)x[t + k];
-          if (y > best) best = y, tstar = t;
-        });
-        rawsum = best;
-        for (int k = 1; k < W; ++k) relnum += k * ma.taps[k] * (int)x[tstar + k];
-      } else {
-        if constexpr (MODE == MODE_FIXED) {
-          tstar = clamp_start(__ldg(ma.window_start + p), S, W);
-        } else {  // MODE_LOCAL_PEAK: largest sample, earliest on ties
-          const uint32_t pmul = sh.peak_mul, PM = sh.peak_mul - 1u;
-          uint32_t best = (uint32_t)x[0] * pmul + PM;
-          skewed(1, S - 1, [&](const int k) {
-            best = max(best, (uint32_t)x[k] * pmul + (PM - (uint32_t)k));
-          });
-          tstar = clamp_start((int)(PM - (best & PM)) - ma.shift, S, W);
-        }
-        rawsum = (int)x[tstar];
-#pragma unroll 4
-        for (int k = 1; k < W; ++k) {
-          const int v = (int)x[tstar + k];
-          rawsum += v;
-          relnum += k * v;
-        }
-      }
-      const int c0 = (MODE == MODE_FIR) ? ma.c0 : W;
-      const int c1 = (MODE == MODE_FIR) ? ma.c1 : (W * (W - 1)) / 2;
-      const Result r = finish_trace(W, rawsum, tstar, relnum, __ldg(pedestal + p), __ldg(gain + p),
-                                    c0, c1);
-      if ((uint32_t)j < n_valid) {
-        __stcs(out_sum + g0 + j, r.sum);
-        __stcs(out_start + g0 + j, r.start);
-        __stcs(out_charge + g0 + j, r.charge);
-        __stcs(out_time + g0 + j, r.time);
-      }
-      p = (p + 1 == n_pixels) ? 0u : p + 1;
-    }
+  auto compute = [&](const uint8_t* unit, const uint32_t g0, const uint32_t n_valid, const uint32_t p) {
+    dyn_compute_unit<G, MODE>(sh, ma, unit, g0, n_valid, p, n_pixels, pedestal, gain, out_sum,
+                              out_start, out_charge, out_time);
   };
 
   uint32_t tile;
@@ -650,6 +663,155 @@ __global__ void __launch_bounds__(C::NT)
     __syncthreads();
     const uint32_t next = tile_q[(j + C::STAGES) % QN];
     if (next < n_tiles) issue((int)((j + C::STAGES) % QN), stage);
+  }
+
+  if (sched != nullptr && tid == 0) {
+    __threadfence();
+    if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) {
+      sched[0] = 0;
+      sched[1] = 0;
+      __threadfence();
+    }
+  }
+}
+
+// Mixed-camera blocks of a shape without a specialisation: the tile table and
+// ingest of extract_ragged_kernel with the runtime-shape walk of extract_dyn_kernel.
+template <bool PAD, int G>
+__global__ void __launch_bounds__(256)
+    extract_ragged_dyn_kernel(const uint8_t* __restrict__ wf, const RaggedTile* __restrict__ tiles,
+                              const uint32_t n_tiles, const int* __restrict__ pedestal,
+                              const float* __restrict__ gain, int* __restrict__ out_sum,
+                              int* __restrict__ out_start, float* __restrict__ out_charge,
+                              float* __restrict__ out_time, uint32_t* __restrict__ sched,
+                              const __grid_constant__ DynShape sh) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t full_bar[kDynMaxStages];
+  __shared__ uint32_t tile_q[kDynMaxStages + 1];
+  __shared__ RaggedTile desc_q[kDynMaxStages + 1];
+  const int tid = threadIdx.x, NT = blockDim.x;
+  const int STAGES = sh.stages, QN = STAGES + 1;
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t bar_base = smem_u32(full_bar);
+  const ModeArgs ma = {};
+
+  constexpr uint32_t kMaxRun = 8;
+  const uint32_t dyn_base = (uint32_t)STAGES * gridDim.x;
+  uint32_t static_next = blockIdx.x, cur = 0, end = 0, nxt = 0, n_run = 0;
+  auto fetch_static = [&]() -> uint32_t {
+    const uint32_t t = static_next;
+    static_next = (t > 0xFFFFFFFFu - gridDim.x) ? 0xFFFFFFFFu : t + gridDim.x;
+    return t;
+  };
+  auto run_length = [&](const uint32_t seen) -> uint32_t {
+    const uint32_t left = n_tiles > seen ? n_tiles - seen : 0u;
+    const uint32_t k = left / (8u * gridDim.x);
+    return k < 1u ? 1u : (k > kMaxRun ? kMaxRun : k);
+  };
+  auto fetch = [&]() -> uint32_t {
+    if (sched == nullptr) return fetch_static();
+    if (cur == end) {
+      cur = nxt;
+      end = nxt + n_run;
+      n_run = run_length(cur);
+      nxt = dyn_base + atomicAdd(sched, n_run);
+    }
+    return cur++;
+  };
+  const auto entry = [&](const uint32_t ti) -> RaggedTile {
+    if (ti < n_tiles) return tiles[ti];
+    return RaggedTile{0ull, 0u, 0u};
+  };
+  if (tid == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(bar_base + 8 * s, NT);
+      tile_q[s] = fetch_static();
+      desc_q[s] = entry(tile_q[s]);
+    }
+    fence_mbar_init();
+    if (sched != nullptr) {
+      n_run = run_length(dyn_base);
+      nxt = dyn_base + atomicAdd(sched, n_run);
+    }
+  }
+  __syncthreads();
+
+  const uint32_t UB = (uint32_t)sh.unit_bytes, PADB = (uint32_t)(sh.unit_stride - sh.unit_bytes);
+  const uint32_t TRACE_BYTES = 2u * (uint32_t)sh.S;
+  auto issue = [&](const int slot, const int stage) {
+    const RaggedTile t = desc_q[slot];
+    const uint8_t* src = wf + (size_t)(t.src & kRaggedOffMask);
+    const uint32_t bytes = (uint32_t)(t.src >> 48) * TRACE_BYTES;
+    uint8_t* dstp = smem + stage * sh.stage_bytes;
+    const uint32_t dst = smem_base + (uint32_t)(stage * sh.stage_bytes);
+    const uint32_t bar = bar_base + 8 * stage;
+    const uint32_t mis = (uint32_t)(reinterpret_cast<uintptr_t>(src) & 15u);
+    uint32_t done;  // bytes moved by the wide path; the rest goes halfword by halfword
+    if (mis == 0) {
+      if constexpr (!PAD) {
+        done = bytes & ~15u;
+        if (tid == 0 && done != 0) {
+          mbar_expect_tx_only(bar, done);
+          tma_bulk_g2s(dst, src, done, bar);
+        }
+      } else {
+        done = bytes & ~15u;  // whole units are whole chunks; a last half unit may not be
+        for (uint32_t c = tid; c < done / 16u; c += NT)
+          cp_async16(dst + (c + c / (UB / 16u)) * 16u, src + (size_t)c * 16u);
+      }
+    } else if ((mis & 3u) == 0) {
+      done = bytes & ~3u;
+      for (uint32_t c = tid; c < done / 4u; c += NT) {
+        uint32_t d = c * 4u;
+        if constexpr (PAD) d += (d / UB) * PADB;
+        cp_async4(dst + d, src + (size_t)c * 4u);
+      }
+    } else {
+      done = 0;
+    }
+    for (uint32_t b = done + 2u * tid; b < bytes; b += 2u * NT) {
+      uint32_t d = b;
+      if constexpr (PAD) d += (b / UB) * PADB;
+      *reinterpret_cast<uint16_t*>(dstp + d) = *reinterpret_cast<const uint16_t*>(src + b);
+    }
+    cp_async_mbar_arrive(bar);  // counts once this thread's cp.async copies have landed
+  };
+
+  for (int s = 0; s < STAGES; ++s) {
+    const uint32_t tile = tile_q[s];
+    if (tile < n_tiles) issue(s, s);
+  }
+  uint32_t pre = 0;
+  RaggedTile pre_d = {0ull, 0u, 0u};
+  if (tid == 0) {
+    pre = fetch();
+    pre_d = entry(pre);
+  }
+
+  for (uint32_t j = 0;; ++j) {
+    const uint32_t tile = tile_q[j % QN];
+    if (tile >= n_tiles) break;
+    const int stage = (int)(j % (uint32_t)STAGES);
+    const uint32_t parity = (j / (uint32_t)STAGES) & 1u;
+    if (tid == 0) {
+      tile_q[(j + STAGES) % QN] = pre;
+      desc_q[(j + STAGES) % QN] = pre_d;
+      pre = fetch();
+      pre_d = entry(pre);
+    }
+    const RaggedTile t = desc_q[j % QN];
+    const uint32_t n = (uint32_t)(t.src >> 48);
+    mbar_wait(bar_base + 8 * stage, parity);
+    const uint32_t first = (uint32_t)(tid * sh.tpt);
+    if (first < n) {
+      const uint8_t* unit = smem + stage * sh.stage_bytes + tid * sh.unit_stride;
+      dyn_compute_unit<G, MODE_SLIDING>(sh, ma, unit, t.out_base + first, n - first,
+                                        t.cal0 + first, 0u, pedestal, gain, out_sum, out_start,
+                                        out_charge, out_time);
+    }
+    __syncthreads();
+    const uint32_t next = tile_q[(j + STAGES) % QN];
+    if (next < n_tiles) issue((int)((j + STAGES) % QN), stage);
   }
 
   if (sched != nullptr && tid == 0) {
@@ -1035,6 +1197,9 @@ int rta_ragged_tile_traces(int32_t S, int32_t W) {
   if (S == CfgS40W7::S && W == CfgS40W7::W) return CfgS40W7::TILE_TRACES;
   if (S == CfgS25W4::S && W == CfgS25W4::W) return CfgS25W4::TILE_TRACES;
   if (S == CfgS128W8::S && W == CfgS128W8::W) return CfgS128W8::TILE_TRACES;
+  DynShape sh;
+  int threads = 0;
+  if (dyn_shape(S, W, &sh, &threads)) return threads * sh.tpt;  // extract_ragged_dyn_kernel
   return 256;  // extract_ragged_generic_kernel: one thread per trace, 256 threads
 }
 
@@ -1057,6 +1222,32 @@ cudaError_t rta_launch_ragged(const void* wf, const RtaRaggedTile* tiles_dev, ui
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
+  DynShape sh;
+  int threads = 0;
+  if (dyn_shape(S, W, &sh, &threads)) {
+    const bool pad = sh.unit_stride != sh.unit_bytes;
+    using Kernel = void (*)(const uint8_t*, const RaggedTile*, uint32_t, const int*, const float*,
+                            int*, int*, float*, float*, uint32_t*, DynShape);
+    const Kernel kernel = pad          ? extract_ragged_dyn_kernel<true, 4>
+                          : sh.g == 1 ? extract_ragged_dyn_kernel<false, 1>
+                          : sh.g == 2 ? extract_ragged_dyn_kernel<false, 2>
+                                      : extract_ragged_dyn_kernel<false, 4>;
+    const int smem = sh.stages * sh.stage_bytes;
+    if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) !=
+        cudaSuccess)
+      return e;
+    int occ = 0;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem)) != cudaSuccess)
+      return e;
+    if (occ < 1) return cudaErrorLaunchOutOfResources;
+    uint32_t grid = (uint32_t)(sms * occ);
+    if (grid > n_tiles) grid = n_tiles;
+    uint32_t* sched = g_static_schedule ? nullptr : sched_words(dev, stream);
+    kernel<<<grid, threads, smem, stream>>>(w, tiles_dev, n_tiles, pedestal, gain, out_sum, out_start,
+                                            out_charge, out_time, sched, sh);
+    rta_count_launch();
+    return cudaGetLastError();
+  }
   uint32_t grid = n_tiles;
   const uint32_t cap = (uint32_t)sms * 8u;
   if (grid > cap) grid = cap;

@@ -93,6 +93,22 @@ def test_random_mixed_batches(seed, gap, align):
     check(b)
 
 
+# shapes without a specialisation, one per case of the runtime-shape kernel
+# (word stride odd / 2 mod 4 / 0 mod 4, padded layout, odd S, blocks of several tiles)
+ANY_SHAPE = [((700, 60, 7), 2), ((300, 96, 8), 1), ((129, 64, 16), 1), ((77, 33, 5), 2),
+             ((1031, 50, 8), 1), ((515, 40, 5), 1), ((9, 128, 10), 2), ((3, 576, 12), 1)]
+
+
+@pytest.mark.parametrize("gap,align", [(0, 8), (5, 1), (6, 2), (9, 8)])
+@pytest.mark.parametrize("wf_shift", [0, 1, 2])
+def test_unspecialised_shapes_take_the_runtime_shape_kernel(gap, align, wf_shift):
+    """extract_ragged_dyn_kernel: every ingest path (TMA / 16-byte cp.async into
+    the padded layout, 4-byte cp.async, halfwords) for every bank-conflict class."""
+    b = make_batch(ANY_SHAPE, n_events=4, seed=3 + gap, gap=gap, align=align)
+    check(b, wf_shift=wf_shift)
+    check(b, wf_shift=wf_shift, static=True)
+
+
 @pytest.mark.parametrize("wf_shift", [0, 1, 2, 3, 4, 6])
 def test_every_alignment_of_the_waveform_buffer(wf_shift):
     """The same tables over a buffer that starts 0..12 bytes off a 16-byte boundary:
