@@ -299,7 +299,10 @@ void rta_ragged_plan_destroy(rta_ragged_plan* plan);
  * parameters (36 bytes per event, + the mask if asked for) are written. Shapes
  * (30,7), (40,7), (25,4), (128,8) with a 16-byte-aligned wf and every event
  * starting on a boundary the staged loads accept take the staged kernels; any
- * other shape or alignment a generic kernel. Same results either way
+ * other 16-byte-aligned shape with traces of at most 1152 bytes runs rta_extract's
+ * staged kernel into a stream-ordered scratch buffer (cudaMallocAsync, 16 bytes
+ * per trace, freed on the stream) followed by the moments kernel; anything else
+ * (or no scratch to be had) a generic fused kernel. Same results either way
  * (rta_image_kernel_name says which). rta_extract_image(...) equals
  * rta_extract(...) followed by rta_image_moments(out_charge, out_time, ...).
  * rta_extract_image_stream / _host: the host-fed variants, chunked and double
@@ -339,7 +342,7 @@ int rta_extract_image_host(const uint16_t* wf_host, int64_t n_events, int32_t n_
                            float thr_picture, float thr_boundary, int32_t* out_n_pix_host,
                            float* out_params_host, uint8_t* out_mask_host, size_t chunk_bytes);
 
-/* "image_tile<S=40,W=7>", ..., or "image_generic". */
+/* "image_tile<S=40,W=7>", ..., "staged<any>+image_moments" or "image_generic". */
 const char* rta_image_kernel_name(int32_t n_pixels, int32_t n_samples, int32_t W, int aligned16);
 int32_t rta_image_max_pixels(void);
 

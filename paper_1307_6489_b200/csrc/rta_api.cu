@@ -1014,6 +1014,7 @@ void rta_shutdown(void) {
     }
   }
   side_streams_release();
+  rta_image_release();
   rta_sched_release();
 }
 

@@ -43,6 +43,7 @@
 #include "rta_device.cuh"
 
 #include <atomic>
+#include <mutex>
 
 // most warps per CTA of image_moments_kernel: 16 leaves the cleaning code its 128
 // registers (24 would spill)
@@ -937,7 +938,51 @@ cudaError_t launch_moments(const float* charge, const float* time, uint32_t n_ev
   return cudaGetLastError();
 }
 
+// Library-owned stream-ordered memory pool of the current device for the scratch
+// of the two-kernel route of rta_launch_extract_image. Its release threshold is
+// unlimited, so the scratch of one call is reused by the next instead of going
+// back to the driver at every synchronisation. nullptr = no pool (generic route).
+constexpr int kMaxPoolDev = 32;
+std::mutex g_pool_mu;
+cudaMemPool_t g_pool[kMaxPoolDev] = {};
+bool g_pool_failed[kMaxPoolDev] = {};
+
+cudaMemPool_t scratch_pool() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxPoolDev) return nullptr;
+  std::lock_guard<std::mutex> lock(g_pool_mu);
+  if (g_pool[dev] == nullptr && !g_pool_failed[dev]) {
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t pool = nullptr;
+    unsigned long long keep = ~0ull;
+    if (cudaMemPoolCreate(&pool, &props) == cudaSuccess &&
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep) == cudaSuccess) {
+      g_pool[dev] = pool;
+    } else {
+      if (pool) cudaMemPoolDestroy(pool);
+      cudaGetLastError();
+      g_pool_failed[dev] = true;
+    }
+  }
+  return g_pool[dev];
+}
+
 }  // namespace
+
+// rta_shutdown: the caller has synchronised the devices in use
+void rta_image_release() {
+  std::lock_guard<std::mutex> lock(g_pool_mu);
+  for (int d = 0; d < kMaxPoolDev; ++d) {
+    if (g_pool[d]) cudaMemPoolDestroy(g_pool[d]);
+    g_pool[d] = nullptr;
+    g_pool_failed[d] = false;
+  }
+  cudaGetLastError();
+}
 
 void rta_set_general_cleaning(bool on) { g_general_cleaning.store(on); }
 
@@ -954,6 +999,7 @@ const char* rta_pick_image_kernel_name(int32_t P, int32_t S, int32_t W, bool ali
     if (S == 40 && W == 7 && staged_ok<ImgS40W7>(P)) return "image_tile<S=40,W=7>";
     if (S == 25 && W == 4 && staged_ok<ImgS25W4>(P)) return "image_tile<S=25,W=4>";
     if (S == 128 && W == 8 && staged_ok<ImgS128W8>(P)) return "image_tile<S=128,W=8>";
+    if (rta_dyn_eligible(S, W)) return "staged<any>+image_moments";
   }
   return "image_generic";
 }
@@ -990,6 +1036,30 @@ cudaError_t rta_launch_extract_image(const void* wf, int64_t n_events, int32_t n
     RTA_TRY(ImgS25W4)
     RTA_TRY(ImgS128W8)
 #undef RTA_TRY
+    // Any other shape the staged runtime-shape kernel takes: extraction into a
+    // stream-ordered scratch buffer (16 bytes per trace), then the moments kernel.
+    // Same charges and the same cleaning code, so the same bits as the generic
+    // fused kernel, 4-6 times faster (that kernel reads its traces with strided
+    // global loads). Falls through when the scratch cannot be had.
+    if (rta_dyn_eligible(S, W)) {
+      const size_t n_traces = (size_t)n_events * (size_t)n_pixels;
+      void* scratch = nullptr;
+      cudaMemPool_t pool = scratch_pool();
+      if (pool != nullptr &&
+          cudaMallocFromPoolAsync(&scratch, 16u * n_traces, pool, stream) == cudaSuccess) {
+        int32_t* o_sum = static_cast<int32_t*>(scratch);
+        int32_t* o_start = o_sum + n_traces;
+        float* o_charge = reinterpret_cast<float*>(o_start + n_traces);
+        float* o_time = o_charge + n_traces;
+        cudaError_t e = rta_launch_extract(wf, (int64_t)n_traces, n_pixels, S, pedestal, gain, W, o_sum,
+                                           o_start, o_charge, o_time, stream, false);
+        if (e == cudaSuccess)
+          e = rta_launch_image_moments(o_charge, o_time, n_events, n_pixels, cam, out, stream);
+        const cudaError_t ef = cudaFreeAsync(scratch, stream);
+        return e != cudaSuccess ? e : ef;
+      }
+      cudaGetLastError();
+    }
   }
   const size_t smem = 2u * EventBuf::bytes(n_pixels) + CleanScratch::bytes(n_pixels);
   if (smem + 1024u > kSmemLimit) return cudaErrorInvalidValue;

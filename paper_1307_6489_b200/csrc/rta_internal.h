@@ -29,6 +29,10 @@ cudaError_t rta_launch_extract(const void* wf, int64_t n_traces, int32_t n_pixel
                                cudaStream_t stream, bool force_generic,
                                const RtaMode* mode = nullptr, int sample_bits = 16);
 
+// Whether an unspecialised (S, W) takes the staged kernel with runtime shape
+// (extract_dyn_kernel) when the input is 16-byte aligned.
+bool rta_dyn_eligible(int32_t n_samples, int32_t W);
+
 // Name of the kernel the dispatcher picks (static string).
 const char* rta_pick_kernel_name(int32_t n_samples, int32_t W, bool aligned16, int bits = 16);
 
@@ -84,6 +88,7 @@ cudaError_t rta_launch_extract_image(const void* wf, int64_t n_events, int32_t n
 // Tests: never take the symmetric-neighbour-table shortcut of the cleaning (both
 // ways give the same mask on a symmetric table).
 void rta_set_general_cleaning(bool on);
+void rta_image_release();  // frees the scratch memory pools (rta_shutdown)
 int32_t rta_image_pixel_limit();  // charge, time and flags of one event must fit one CTA
 const char* rta_pick_image_kernel_name(int32_t n_pixels, int32_t n_samples, int32_t W,
                                        bool aligned16);

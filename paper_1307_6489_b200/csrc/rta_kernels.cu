@@ -1192,6 +1192,12 @@ int RaggedLauncher<C>::ctas_per_sm[kMaxDevices];
 
 }  // namespace
 
+bool rta_dyn_eligible(int32_t S, int32_t W) {
+  DynShape sh;
+  int threads = 0;
+  return S >= 1 && W >= 1 && W <= S && dyn_shape(S, W, &sh, &threads);
+}
+
 int rta_ragged_tile_traces(int32_t S, int32_t W) {
   if (S == CfgS30W7::S && W == CfgS30W7::W) return CfgS30W7::TILE_TRACES;
   if (S == CfgS40W7::S && W == CfgS40W7::W) return CfgS40W7::TILE_TRACES;

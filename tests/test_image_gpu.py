@@ -292,6 +292,35 @@ def test_fused_shapes_and_event_phases(S, W, P, E):
     assert_image_parity(got, want, x, y, "S=%d P=%d" % (S, P))
 
 
+@pytest.mark.parametrize("S,W,P,E", [(60, 7, 1855, 12), (96, 8, 300, 25), (33, 5, 400, 20), (50, 8, 37, 60)])
+def test_fused_unspecialised_shapes_run_extract_then_moments(S, W, P, E):
+    """Shapes without a fused specialisation: rta_extract's runtime-shape kernel
+    into a stream-ordered scratch buffer, then the moments kernel (two launches);
+    bit-identical to the generic fused kernel, repeatable (the scratch pool is reused)."""
+    import paper_1307_6489_b200 as rta
+    assert rta.rta_image_kernel_name(P, S, W) == "staged<any>+image_moments"
+    rng = np.random.default_rng(S + P)
+    x, y, nbr = dl0gen.hex_camera(P)
+    ped = rng.integers(380, 421, P).astype(np.int32)
+    gain = rng.uniform(0.9, 1.1, P).astype(F32)
+    wf = (400 + rng.normal(0, 4, (E, P, S))).round().clip(0, 4095).astype(np.uint16)
+    for e in range(E):
+        p = int(rng.integers(0, P))
+        for n in [p] + [int(v) for v in nbr[p] if v >= 0]:
+            wf[e, n, S // 2: S // 2 + W // 2] += np.uint16(rng.integers(20, 200))
+    want = oracle_extract_image(wf, ped, gain, W, x, y, nbr, 60.0, 30.0)
+    assert (want[0] > 0).any()
+    before = rta.rta_launch_count()
+    got = gpu_extract_image(wf, ped, gain, W, x, y, nbr, 60.0, 30.0)
+    assert rta.rta_launch_count() - before == 2
+    assert_image_parity(got, want, x, y, "S=%d P=%d" % (S, P))
+    gen = gpu_extract_image(wf, ped, gain, W, x, y, nbr, 60.0, 30.0, generic=True)
+    again = gpu_extract_image(wf, ped, gain, W, x, y, nbr, 60.0, 30.0)
+    for a, b, c in zip(got, gen, again):
+        assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
+        assert np.array_equal(a.view(np.uint8), c.view(np.uint8))
+
+
 def test_fused_unaligned_waveforms_take_the_generic_kernel():
     import torch
     cfg, wf, ped, gain, x, y, nbr, tp, tb = config_batch("C2", 20)
