@@ -51,7 +51,10 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C4"])
+    ap.add_argument("--workload", default="C2",
+                    choices=["C1", "C2", "C3", "C4", "X60", "X40w5", "X96", "X128w10"],
+                    help="C1..C4: BASELINE.json configs; X*: shapes without a specialised kernel "
+                         "(diagnostic runs of the runtime-shape kernel, imply --no-extra)")
     ap.add_argument("--input-format", default="u16", choices=["u16", "p12"],
                     help="u16: BASELINE.json's uint16 waveforms (the headline); p12: the same batch as "
                          "a packed 12-bit stream through rta_extract_packed12 (NEXT-2)")
@@ -202,7 +205,7 @@ def reference_arm(args):
     import numpy as np
     import dl0gen
     import oracle
-    cfg = dl0gen.CONFIGS[args.workload]
+    cfg = workload(args.workload, dl0gen)
     cores = os.cpu_count() or 1
     ped, gain = dl0gen.calib(cfg)
     # ~0.3 GB/s per core: size the per-step sample for about 1 s of all-cores work
@@ -429,10 +432,9 @@ def ragged_leg(steps, peak, torch, dl0gen, rta, n_events=1000):
     return res
 
 
-def any_shape_leg(steps, peak, torch, dl0gen, rta):
-    """Shapes without a specialised kernel (not BASELINE configs: C2's and C4's
-    signal models with other readout lengths / window widths) through rta_extract:
-    the staged kernel with runtime (S, W), next to the old generic kernel."""
+def extra_shapes(dl0gen):
+    """Workloads that are NOT BASELINE configs: C2's and C4's signal models with another
+    readout length or window width (shapes without a specialised kernel)."""
     import dataclasses
     c2, c4 = dl0gen.CONFIGS["C2"], dl0gen.CONFIGS["C4"]
     shapes = [dataclasses.replace(c2, name="X60", label="10000x1855x60 W=7", seed=11, n_samples=60,
@@ -442,8 +444,19 @@ def any_shape_leg(steps, peak, torch, dl0gen, rta):
                                   n_samples=96, peak_lo=25.0, peak_hi=70.0),
               dataclasses.replace(c4, name="X128w10", label="10000x2048x128 W=10", seed=14,
                                   n_events=10_000, W=10)]
+    return {c.name: c for c in shapes}
+
+
+def workload(name, dl0gen):
+    return dl0gen.CONFIGS[name] if name in dl0gen.CONFIGS else extra_shapes(dl0gen)[name]
+
+
+def any_shape_leg(steps, peak, torch, dl0gen, rta):
+    """Shapes without a specialised kernel (not BASELINE configs: C2's and C4's
+    signal models with other readout lengths / window widths) through rta_extract:
+    the staged kernel with runtime (S, W), next to the old generic kernel."""
     res = {}
-    for cfg in shapes:
+    for cfg in extra_shapes(dl0gen).values():
         d_wf, d_ped, d_gain, outs, ped, gain = device_batch(cfg, torch, dl0gen)
         stream = torch.cuda.current_stream()
         base = (d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain, cfg.W)
@@ -758,7 +771,7 @@ def main():
         torch.cuda.synchronize()
 
     rta.lib()
-    cfg = dl0gen.CONFIGS[args.workload]
+    cfg = workload(args.workload, dl0gen)
     peak, peak_src = hbm_peak()
 
     try:
@@ -770,7 +783,7 @@ def main():
     # Weak scaling: every rank extracts its own batch of the named workload
     # (independent events; no data-path collective).
     fmt = args.input_format
-    if fmt == "p12" or args.path != "extract":
+    if fmt == "p12" or args.path != "extract" or args.workload.startswith("X"):
         args.no_extra = True     # the packed / image main legs are profiling/diagnostic runs
     main_run = kernel_only(cfg, args.steps, args.warmup, torch, dl0gen, rta, barrier, sampler, fmt,
                            args.path)
