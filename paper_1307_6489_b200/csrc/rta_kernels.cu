@@ -1061,7 +1061,19 @@ bool dyn_shape(int32_t S, int32_t W, DynShape* sh, int* threads) {
   int g = 1;
   while (g < 32 && (stride / 4) % (2 * g) == 0) g *= 2;
   if (g > 4 || (pad && g != 4)) return false;  // cannot happen (see the kernel's header)
-  const int nt = stride <= 144 ? 256 : stride <= 288 ? 128 : stride <= 576 ? 64 : 32;
+  // threads per CTA: the candidate that keeps most warps resident (two stages per
+  // CTA in 227 KB of shared memory; about 62 registers per thread: 32 warps at most)
+  int nt = 32, best_warps = 0;
+  const int candidates[4] = {128, 256, 64, 32};  // ties go to the earlier entry (measured)
+  for (const int cand : candidates) {
+    const int stage = ((cand * stride + 64 + 127) / 128) * 128;
+    int ctas = (227 * 1024) / (2 * stage + 1024);
+    if (ctas > 32) ctas = 32;
+    int warps = ctas * (cand / 32);
+    if (warps > 32) warps = 32;
+    if (warps > best_warps) best_warps = warps, nt = cand;
+  }
+  if (best_warps == 0) return false;
   sh->S = S;
   sh->W = W;
   sh->n_win = S - W + 1;
