@@ -35,13 +35,70 @@
 
 namespace {
 
-// Tiles are handed out dynamically: SMs do not stream at the same rate (near /
-// far L2 die, DRAM channel load), and with a static round-robin the launch
-// ends when the slowest CTA has finished its fixed share (measured: 4-7 % of
-// SM-time idle). `sched` points at {next tile, CTAs done}, both zero on entry;
-// the last CTA to leave zeroes them again, so the pair is reusable by the next
-// launch on the same stream (and by CUDA-graph replays). sched == nullptr
-// selects the static round-robin (same code path, locally generated indices).
+// Tile indices of one CTA (used by its thread 0 only). Tiles are handed out
+// dynamically: SMs do not stream at the same rate (near / far L2 die, DRAM
+// channel load), and with a static round-robin the launch ends when the slowest
+// CTA has finished its fixed share (measured: 4-7 % of SM-time idle). `sched`
+// points at {next tile, CTAs done}, both zero on entry; the last CTA to leave
+// zeroes them again, so the pair is reusable by the next launch on the same
+// stream (and by CUDA-graph replays). sched == nullptr selects the static
+// round-robin (same code path, locally generated indices).
+// The first `stages` tiles of every CTA are the static round-robin ones (no
+// atomic round trip before the first load); the shared counter hands out the
+// tiles after those, in runs of up to kMaxRun consecutive tiles per atomic:
+// same-address atomics retire at only ~0.3 G/s on B200 (measured), which one
+// atomic per 10-20 KB tile would saturate. Runs shrink to single tiles near
+// the end so the CTAs still finish together.
+struct TileFeed {
+  static constexpr uint32_t kMaxRun = 8;
+  uint32_t* sched;
+  uint32_t n_tiles, dyn_base;
+  // static sequence, current run [cur, end), prefetched run [nxt, nxt + n_run)
+  uint32_t static_next, cur, end, nxt, n_run;
+
+  __device__ __forceinline__ TileFeed(uint32_t* sched_, const uint32_t n_tiles_, const int stages)
+      : sched(sched_), n_tiles(n_tiles_), dyn_base((uint32_t)stages * gridDim.x),
+        static_next(blockIdx.x), cur(0), end(0), nxt(0), n_run(0) {}
+  __device__ __forceinline__ uint32_t fetch_static() {
+    const uint32_t t = static_next;
+    // saturate: indices past the end must stay past the end
+    static_next = (t > 0xFFFFFFFFu - gridDim.x) ? 0xFFFFFFFFu : t + gridDim.x;
+    return t;
+  }
+  __device__ __forceinline__ uint32_t run_length(const uint32_t seen) const {
+    const uint32_t left = n_tiles > seen ? n_tiles - seen : 0u;
+    const uint32_t k = left / (8u * gridDim.x);
+    return k < 1u ? 1u : (k > kMaxRun ? kMaxRun : k);
+  }
+  // after the static tiles have been drawn: ask for the first dynamic run
+  __device__ __forceinline__ void prime() {
+    if (sched != nullptr) {
+      n_run = run_length(dyn_base);
+      nxt = dyn_base + atomicAdd(sched, n_run);
+    }
+  }
+  __device__ __forceinline__ uint32_t fetch() {
+    if (sched == nullptr) return fetch_static();
+    if (cur == end) {  // take the prefetched run, ask for the one after it
+      cur = nxt;
+      end = nxt + n_run;
+      n_run = run_length(cur);
+      nxt = dyn_base + atomicAdd(sched, n_run);
+    }
+    return cur++;
+  }
+  // hand the scheduler words back zeroed (all of this CTA's fetches precede this)
+  __device__ __forceinline__ void leave() const {
+    if (sched == nullptr) return;
+    __threadfence();
+    if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) {
+      sched[0] = 0;
+      sched[1] = 0;
+      __threadfence();
+    }
+  }
+};
+
 template <class C, int MODE>
 __global__ void __launch_bounds__(C::NT)
     extract_tile_kernel(const uint8_t* __restrict__ wf, const uint32_t n_traces,
@@ -61,49 +118,16 @@ __global__ void __launch_bounds__(C::NT)
   const uint32_t smem_base = smem_u32(smem);
   const uint32_t bar_base = smem_u32(full_bar);
 
-  // The first STAGES tiles of every CTA are the static round-robin ones (no
-  // atomic round trip before the first load); the shared counter hands out
-  // the tiles after those, in runs of up to kMaxRun consecutive tiles per
-  // atomic: same-address atomics retire at only ~0.3 G/s on B200 (measured),
-  // which one atomic per 10-20 KB tile would saturate. Runs shrink to single
-  // tiles near the end so the CTAs still finish together.
-  constexpr uint32_t kMaxRun = 8;
-  const uint32_t dyn_base = (uint32_t)C::STAGES * gridDim.x;
-  // thread 0 only: static sequence, current run [cur, end), prefetched run [nxt, nxt + n_run)
-  uint32_t static_next = blockIdx.x, cur = 0, end = 0, nxt = 0, n_run = 0;
-  auto fetch_static = [&]() -> uint32_t {
-    const uint32_t t = static_next;
-    // saturate: indices past the end must stay past the end
-    static_next = (t > 0xFFFFFFFFu - gridDim.x) ? 0xFFFFFFFFu : t + gridDim.x;
-    return t;
-  };
-  auto run_length = [&](const uint32_t seen) -> uint32_t {
-    const uint32_t left = n_full > seen ? n_full - seen : 0u;
-    const uint32_t k = left / (8u * gridDim.x);
-    return k < 1u ? 1u : (k > kMaxRun ? kMaxRun : k);
-  };
-  auto fetch = [&]() -> uint32_t {
-    if (sched == nullptr) return fetch_static();
-    if (cur == end) {  // take the prefetched run, ask for the one after it
-      cur = nxt;
-      end = nxt + n_run;
-      n_run = run_length(cur);
-      nxt = dyn_base + atomicAdd(sched, n_run);
-    }
-    return cur++;
-  };
+  TileFeed feed(sched, n_full, C::STAGES);  // thread 0 only
 
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < C::STAGES; ++s) {
       mbar_init(bar_base + 8 * s, C::PAD ? C::NT : 1);
-      tile_q[s] = fetch_static();
+      tile_q[s] = feed.fetch_static();
     }
     fence_mbar_init();
-    if (sched != nullptr) {
-      n_run = run_length(dyn_base);
-      nxt = dyn_base + atomicAdd(sched, n_run);
-    }
+    feed.prime();
   }
   __syncthreads();
 
@@ -135,7 +159,7 @@ __global__ void __launch_bounds__(C::NT)
   // thread 0 keeps one tile index in flight: fetched while a tile is being
   // computed, published one iteration later (the atomic's latency is hidden)
   uint32_t pre = 0;
-  if (tid == 0) pre = fetch();
+  if (tid == 0) pre = feed.fetch();
 
   uint32_t tile;
   for (uint32_t j = 0;; ++j) {
@@ -147,7 +171,7 @@ __global__ void __launch_bounds__(C::NT)
       // slot (j + STAGES) % QN == (j - 1) % QN was last read before the
       // previous iteration's barrier
       tile_q[(j + C::STAGES) % QN] = pre;
-      pre = fetch();
+      pre = feed.fetch();
     }
     mbar_wait(bar_base + 8 * stage, parity);
     const uint8_t* unit = smem + stage * C::STAGE_BYTES + tid * C::UNIT_STRIDE;
@@ -189,15 +213,7 @@ __global__ void __launch_bounds__(C::NT)
     }
   }
 
-  // hand the scheduler words back zeroed (all of this CTA's fetches precede this)
-  if (sched != nullptr && tid == 0) {
-    __threadfence();
-    if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) {
-      sched[0] = 0;
-      sched[1] = 0;
-      __threadfence();
-    }
-  }
+  if (tid == 0) feed.leave();
 }
 
 
@@ -372,40 +388,15 @@ __global__ void __launch_bounds__(256)
   const uint32_t smem_base = smem_u32(smem);
   const uint32_t bar_base = smem_u32(full_bar);
 
-  constexpr uint32_t kMaxRun = 8;
-  const uint32_t dyn_base = (uint32_t)STAGES * gridDim.x;
-  uint32_t static_next = blockIdx.x, cur = 0, end = 0, nxt = 0, n_run = 0;
-  auto fetch_static = [&]() -> uint32_t {
-    const uint32_t t = static_next;
-    static_next = (t > 0xFFFFFFFFu - gridDim.x) ? 0xFFFFFFFFu : t + gridDim.x;
-    return t;
-  };
-  auto run_length = [&](const uint32_t seen) -> uint32_t {
-    const uint32_t left = n_full > seen ? n_full - seen : 0u;
-    const uint32_t k = left / (8u * gridDim.x);
-    return k < 1u ? 1u : (k > kMaxRun ? kMaxRun : k);
-  };
-  auto fetch = [&]() -> uint32_t {
-    if (sched == nullptr) return fetch_static();
-    if (cur == end) {
-      cur = nxt;
-      end = nxt + n_run;
-      n_run = run_length(cur);
-      nxt = dyn_base + atomicAdd(sched, n_run);
-    }
-    return cur++;
-  };
+  TileFeed feed(sched, n_full, STAGES);  // thread 0 only
 
   if (tid == 0) {
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(bar_base + 8 * s, PAD ? NT : 1);
-      tile_q[s] = fetch_static();
+      tile_q[s] = feed.fetch_static();
     }
     fence_mbar_init();
-    if (sched != nullptr) {
-      n_run = run_length(dyn_base);
-      nxt = dyn_base + atomicAdd(sched, n_run);
-    }
+    feed.prime();
   }
   __syncthreads();
 
@@ -439,7 +430,7 @@ __global__ void __launch_bounds__(256)
     if (tile < n_full) issue(tile, s);
   }
   uint32_t pre = 0;
-  if (tid == 0) pre = fetch();
+  if (tid == 0) pre = feed.fetch();
 
   const int S = sh.S;
 
@@ -456,7 +447,7 @@ __global__ void __launch_bounds__(256)
     const uint32_t parity = (j / (uint32_t)STAGES) & 1u;
     if (tid == 0) {
       tile_q[(j + STAGES) % QN] = pre;
-      pre = fetch();
+      pre = feed.fetch();
     }
     mbar_wait(bar_base + 8 * stage, parity);
     const uint8_t* unit = smem + stage * sh.stage_bytes + tid * sh.unit_stride;
@@ -485,14 +476,7 @@ __global__ void __launch_bounds__(256)
     }
   }
 
-  if (sched != nullptr && tid == 0) {
-    __threadfence();
-    if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) {
-      sched[0] = 0;
-      sched[1] = 0;
-      __threadfence();
-    }
-  }
+  if (tid == 0) feed.leave();
 }
 
 // ------------------------------------------------- mixed-camera batches ----
@@ -535,29 +519,7 @@ __global__ void __launch_bounds__(C::NT)
 
   // tile indices: the first STAGES of a CTA are static (blockIdx.x + k * gridDim.x),
   // the rest come from the shared counter, one run of tiles per atomic
-  constexpr uint32_t kMaxRun = 8;
-  const uint32_t dyn_base = (uint32_t)C::STAGES * gridDim.x;
-  uint32_t static_next = blockIdx.x, cur = 0, end = 0, nxt = 0, n_run = 0;
-  auto fetch_static = [&]() -> uint32_t {
-    const uint32_t t = static_next;
-    static_next = (t > 0xFFFFFFFFu - gridDim.x) ? 0xFFFFFFFFu : t + gridDim.x;
-    return t;
-  };
-  auto run_length = [&](const uint32_t seen) -> uint32_t {
-    const uint32_t left = n_tiles > seen ? n_tiles - seen : 0u;
-    const uint32_t k = left / (8u * gridDim.x);
-    return k < 1u ? 1u : (k > kMaxRun ? kMaxRun : k);
-  };
-  auto fetch = [&]() -> uint32_t {
-    if (sched == nullptr) return fetch_static();
-    if (cur == end) {
-      cur = nxt;
-      end = nxt + n_run;
-      n_run = run_length(cur);
-      nxt = dyn_base + atomicAdd(sched, n_run);
-    }
-    return cur++;
-  };
+  TileFeed feed(sched, n_tiles, C::STAGES);  // thread 0 only
 
   const auto entry = [&](const uint32_t ti) -> RaggedTile {
     if (ti < n_tiles) return tiles[ti];
@@ -567,14 +529,11 @@ __global__ void __launch_bounds__(C::NT)
 #pragma unroll
     for (int s = 0; s < C::STAGES; ++s) {
       mbar_init(bar_base + 8 * s, C::NT);
-      tile_q[s] = fetch_static();
+      tile_q[s] = feed.fetch_static();
       desc_q[s] = entry(tile_q[s]);
     }
     fence_mbar_init();
-    if (sched != nullptr) {
-      n_run = run_length(dyn_base);
-      nxt = dyn_base + atomicAdd(sched, n_run);
-    }
+    feed.prime();
   }
   __syncthreads();
 
@@ -635,7 +594,7 @@ __global__ void __launch_bounds__(C::NT)
   uint32_t pre = 0;
   RaggedTile pre_d = {0ull, 0u, 0u};
   if (tid == 0) {
-    pre = fetch();
+    pre = feed.fetch();
     pre_d = entry(pre);
   }
 
@@ -647,7 +606,7 @@ __global__ void __launch_bounds__(C::NT)
     if (tid == 0) {
       tile_q[(j + C::STAGES) % QN] = pre;
       desc_q[(j + C::STAGES) % QN] = pre_d;
-      pre = fetch();
+      pre = feed.fetch();
       pre_d = entry(pre);
     }
     const RaggedTile t = desc_q[j % QN];
@@ -665,14 +624,7 @@ __global__ void __launch_bounds__(C::NT)
     if (next < n_tiles) issue((int)((j + C::STAGES) % QN), stage);
   }
 
-  if (sched != nullptr && tid == 0) {
-    __threadfence();
-    if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) {
-      sched[0] = 0;
-      sched[1] = 0;
-      __threadfence();
-    }
-  }
+  if (tid == 0) feed.leave();
 }
 
 // Mixed-camera blocks of a shape without a specialisation: the tile table and
@@ -695,29 +647,7 @@ __global__ void __launch_bounds__(256)
   const uint32_t bar_base = smem_u32(full_bar);
   const ModeArgs ma = {};
 
-  constexpr uint32_t kMaxRun = 8;
-  const uint32_t dyn_base = (uint32_t)STAGES * gridDim.x;
-  uint32_t static_next = blockIdx.x, cur = 0, end = 0, nxt = 0, n_run = 0;
-  auto fetch_static = [&]() -> uint32_t {
-    const uint32_t t = static_next;
-    static_next = (t > 0xFFFFFFFFu - gridDim.x) ? 0xFFFFFFFFu : t + gridDim.x;
-    return t;
-  };
-  auto run_length = [&](const uint32_t seen) -> uint32_t {
-    const uint32_t left = n_tiles > seen ? n_tiles - seen : 0u;
-    const uint32_t k = left / (8u * gridDim.x);
-    return k < 1u ? 1u : (k > kMaxRun ? kMaxRun : k);
-  };
-  auto fetch = [&]() -> uint32_t {
-    if (sched == nullptr) return fetch_static();
-    if (cur == end) {
-      cur = nxt;
-      end = nxt + n_run;
-      n_run = run_length(cur);
-      nxt = dyn_base + atomicAdd(sched, n_run);
-    }
-    return cur++;
-  };
+  TileFeed feed(sched, n_tiles, STAGES);  // thread 0 only
   const auto entry = [&](const uint32_t ti) -> RaggedTile {
     if (ti < n_tiles) return tiles[ti];
     return RaggedTile{0ull, 0u, 0u};
@@ -725,14 +655,11 @@ __global__ void __launch_bounds__(256)
   if (tid == 0) {
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(bar_base + 8 * s, NT);
-      tile_q[s] = fetch_static();
+      tile_q[s] = feed.fetch_static();
       desc_q[s] = entry(tile_q[s]);
     }
     fence_mbar_init();
-    if (sched != nullptr) {
-      n_run = run_length(dyn_base);
-      nxt = dyn_base + atomicAdd(sched, n_run);
-    }
+    feed.prime();
   }
   __syncthreads();
 
@@ -784,7 +711,7 @@ __global__ void __launch_bounds__(256)
   uint32_t pre = 0;
   RaggedTile pre_d = {0ull, 0u, 0u};
   if (tid == 0) {
-    pre = fetch();
+    pre = feed.fetch();
     pre_d = entry(pre);
   }
 
@@ -796,7 +723,7 @@ __global__ void __launch_bounds__(256)
     if (tid == 0) {
       tile_q[(j + STAGES) % QN] = pre;
       desc_q[(j + STAGES) % QN] = pre_d;
-      pre = fetch();
+      pre = feed.fetch();
       pre_d = entry(pre);
     }
     const RaggedTile t = desc_q[j % QN];
@@ -814,14 +741,7 @@ __global__ void __launch_bounds__(256)
     if (next < n_tiles) issue((int)((j + STAGES) % QN), stage);
   }
 
-  if (sched != nullptr && tid == 0) {
-    __threadfence();
-    if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) {
-      sched[0] = 0;
-      sched[1] = 0;
-      __threadfence();
-    }
-  }
+  if (tid == 0) feed.leave();
 }
 
 // Shapes without a specialisation: one thread per trace, one tile (<= 256 traces) per CTA pass.
