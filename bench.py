@@ -350,7 +350,7 @@ def family_leg(cfg, steps, peak, torch, dl0gen, rta):
     }
     res = {}
     for name, run in runs.items():
-        for _ in range(3):
+        for _ in range(LEG_WARMUP):
             run()
         torch.cuda.synchronize()
         res[name] = summarise(cfg, time_steps(run, steps, stream), peak)
@@ -376,7 +376,7 @@ def packed_leg(cfg, steps, peak, torch, dl0gen, rta):
     def run():
         rta.rta_extract_packed12(d_pk, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain,
                                  cfg.W, *outs, stream=stream)
-    for _ in range(3):
+    for _ in range(LEG_WARMUP):
         run()
     torch.cuda.synchronize()
     per = time_steps(run, steps, stream)
@@ -412,7 +412,7 @@ def ragged_leg(steps, peak, torch, dl0gen, rta, n_events=1000):
 
     def run():
         rta.rta_extract_ragged(plan, d_wf, d_ped, d_gain, *outs, stream=stream)
-    for _ in range(3):
+    for _ in range(LEG_WARMUP):
         run()
     torch.cuda.synchronize()
     before = rta.rta_launch_count()
@@ -465,7 +465,7 @@ def any_shape_leg(steps, peak, torch, dl0gen, rta):
         for name, generic in (("staged_any", False), ("generic", True)):
             def run():
                 rta.rta_extract(*base, *outs, stream=stream, generic=generic)
-            for _ in range(3):
+            for _ in range(LEG_WARMUP):
                 run()
             torch.cuda.synchronize()
             r[name] = summarise(cfg, time_steps(run, steps if not generic else 3, stream), peak)
@@ -482,6 +482,7 @@ def any_shape_leg(steps, peak, torch, dl0gen, rta):
 
 
 EVENT_OUT_BYTES = 36   # n_pix int32 + 8 fp32 parameters per event
+LEG_WARMUP = 10        # untimed launches in front of every secondary leg (the GPU idles while a leg sets up)
 
 
 def image_leg(cfg, steps, peak, torch, dl0gen, rta):
@@ -513,7 +514,7 @@ def image_leg(cfg, steps, peak, torch, dl0gen, rta):
         cfg.name, cfg.label, cam[3], cam[4]),
         "kernel": rta.rta_image_kernel_name(cfg.n_pixels, cfg.n_samples, cfg.W, True)}
     for name, run in (("fused", fused), ("two_calls", two_calls), ("moments", moments)):
-        for _ in range(3):
+        for _ in range(LEG_WARMUP):
             run()
         torch.cuda.synchronize()
         per = time_steps(run, steps, stream)
