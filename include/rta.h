@@ -53,8 +53,12 @@ enum {
  *   wf        DEVICE  uint16 [n_events][n_pixels][n_samples], dense, sample fastest.
  *                     Any uint16 value is accepted (12-bit data is a property of the
  *                     configs, not of the ABI). A 16-byte-aligned base pointer takes
- *                     the staged (TMA / cp.async) kernels; any other 2-byte-aligned
- *                     pointer takes the generic kernel. Same results either way.
+ *                     the staged (TMA / cp.async) kernels — a specialisation for the
+ *                     shapes (30,7), (40,7), (25,4), (128,8), a kernel with runtime
+ *                     (n_samples, W) for any other trace of at most 1152 bytes; any
+ *                     other 2-byte-aligned pointer, and longer traces, take the generic
+ *                     kernel (strided global loads: several times slower). Same
+ *                     results either way (rta_kernel_name says which).
  *   pedestal  DEVICE  int32  [n_pixels]; may exceed the samples (x can be negative).
  *   gain      DEVICE  float  [n_pixels]; NaN/Inf propagate into out_charge untouched.
  *   W         window width in samples, 1 <= W <= n_samples.
@@ -217,8 +221,9 @@ int rta_extract_host_packed12(const uint8_t* packed_host, int64_t n_events,
  *
  * rta_extract_ragged is asynchronous on `stream`: one launch per distinct
  * (n_samples, W) among the blocks (rta_ragged_plan_info(RTA_RAGGED_N_LAUNCHES)).
- * Shapes (30,7), (40,7), (25,4), (128,8) take the staged kernels; others a
- * generic kernel. Blocks starting on a 16-byte boundary of `wf` are fastest
+ * Shapes (30,7), (40,7), (25,4), (128,8) take the specialised staged kernels,
+ * other traces of at most 1152 bytes a staged kernel with runtime shape, longer
+ * ones a generic kernel. Blocks starting on a 16-byte boundary of `wf` are fastest
  * (TMA bulk copies); 4-byte-aligned ones use 4-byte cp.async; others plain loads.
  *
  * Errors (plan_create, before any CUDA call): NULL table with entries, or
@@ -353,8 +358,8 @@ const char* rta_strerror(int status);
  * (0 if none). */
 int rta_last_cuda_error(void);
 
-/* Which kernel a shape takes, for tests and profiles: writes a static string
- * such as "tile<S=40,W=7>" or "generic" for (n_samples, W, 16-byte-aligned?). */
+/* Which kernel a shape takes, for tests and profiles: a static string such as
+ * "tile<S=40,W=7>", "staged<any>" or "generic" for (n_samples, W, 16-byte-aligned?). */
 const char* rta_kernel_name(int32_t n_samples, int32_t W, int aligned16);
 /* Same for a P12 stream: "tile12<S=40,W=7>", "generic12", ... */
 const char* rta_kernel_name_packed12(int32_t n_samples, int32_t W, int aligned16);
