@@ -55,10 +55,15 @@ enum {
  *                     configs, not of the ABI). A 16-byte-aligned base pointer takes
  *                     the staged (TMA / cp.async) kernels — a specialisation for the
  *                     shapes (30,7), (40,7), (25,4), (128,8), a kernel with runtime
- *                     (n_samples, W) for any other trace of at most 1152 bytes; any
- *                     other 2-byte-aligned pointer, and longer traces, take the generic
+ *                     (n_samples, W) for any other trace of at most 1152 bytes. Any
+ *                     other 2-byte-aligned pointer takes that runtime-shape kernel
+ *                     too, unless the trace (pair of traces when n_samples is odd) is
+ *                     a multiple of 32 bytes; those, and longer traces, take the generic
  *                     kernel (strided global loads: several times slower). Same
- *                     results either way (rta_kernel_name says which).
+ *                     results either way (rta_kernel_name says which). With an
+ *                     unaligned base the first bulk copy starts at the 16-byte
+ *                     boundary below wf (inside the 16-byte line holding wf[0]);
+ *                     nothing past the last sample is read.
  *   pedestal  DEVICE  int32  [n_pixels]; may exceed the samples (x can be negative).
  *   gain      DEVICE  float  [n_pixels]; NaN/Inf propagate into out_charge untouched.
  *   W         window width in samples, 1 <= W <= n_samples.

@@ -401,14 +401,30 @@ __global__ void __launch_bounds__(256)
   __syncthreads();
 
   const uint32_t chunks_per_unit = (uint32_t)sh.unit_bytes / 16u;  // PAD only
+  // A base pointer that is only 2-byte aligned (dense layouts only): the bulk copy
+  // starts at the 16-byte boundary below the tile, so the tile lands `mis` bytes
+  // into the stage; the 16-bit walk does not care. The copy of the very last
+  // tile stops at the last boundary inside the caller's buffer and the final
+  // < 16 bytes go halfword by halfword: nothing past the buffer is read. (The
+  // first copy starts up to 14 bytes before `wf`, inside the 16-byte line that
+  // holds wf[0].)
+  const uint32_t mis = PAD ? 0u : (uint32_t)(reinterpret_cast<uintptr_t>(wf) & 15u);
   auto issue = [&](const uint32_t tile, const int stage) {
     const uint8_t* src = wf + (size_t)tile * (size_t)sh.tile_bytes;
     const uint32_t dst = smem_base + (uint32_t)(stage * sh.stage_bytes);
     const uint32_t bar = bar_base + 8 * stage;
     if constexpr (!PAD) {
       if (tid == 0) {
-        mbar_expect_tx(bar, (uint32_t)sh.tile_bytes);
-        tma_bulk_g2s(dst, src, (uint32_t)sh.tile_bytes, bar);
+        uint32_t len = (uint32_t)sh.tile_bytes + (mis ? 16u : 0u);
+        if (mis != 0 && (unsigned long long)(tile + 1u) * (unsigned long long)sh.tile_bytes + 16u - mis >
+                            (unsigned long long)n_traces * 2ull * (unsigned long long)sh.S) {
+          len = (uint32_t)sh.tile_bytes;  // whole 16-byte lines inside the buffer
+          uint8_t* d = smem + stage * sh.stage_bytes;
+          for (uint32_t b = len; b < mis + (uint32_t)sh.tile_bytes; b += 2u)
+            *reinterpret_cast<uint16_t*>(d + b) = *reinterpret_cast<const uint16_t*>(src - mis + b);
+        }
+        mbar_expect_tx(bar, len);
+        tma_bulk_g2s(dst, src - mis, len, bar);
       }
     } else {
       // chunk c of the tile belongs to unit c / chunks_per_unit: one chunk of padding per unit
@@ -450,7 +466,7 @@ __global__ void __launch_bounds__(256)
       pre = feed.fetch();
     }
     mbar_wait(bar_base + 8 * stage, parity);
-    const uint8_t* unit = smem + stage * sh.stage_bytes + tid * sh.unit_stride;
+    const uint8_t* unit = smem + stage * sh.stage_bytes + mis + tid * sh.unit_stride;
     const uint32_t g0 = tile * tile_traces + (uint32_t)(tid * sh.tpt);
     compute(unit, g0, (uint32_t)sh.tpt, fastmod(g0, n_pixels, pix_inv));
     __syncthreads();
@@ -460,8 +476,8 @@ __global__ void __launch_bounds__(256)
 
   // ragged tail (< one tile of traces): plain copies, by the CTA that drew index n_full
   if (rem != 0 && tile == n_full) {
-    const uint8_t* src = wf + (size_t)n_full * (size_t)sh.tile_bytes;  // 16-byte aligned
-    const uint32_t n_hw = rem * (uint32_t)S;                          // halfwords
+    const uint8_t* src = wf + (size_t)n_full * (size_t)sh.tile_bytes;
+    const uint32_t n_hw = rem * (uint32_t)S;  // halfwords
     const uint32_t unit_hw = (uint32_t)sh.unit_bytes / 2u, pad_hw = (uint32_t)(sh.unit_stride - sh.unit_bytes) / 2u;
     for (uint32_t i = tid; i < n_hw; i += NT) {
       const uint32_t dsti = PAD ? i + (i / unit_hw) * pad_hw : i;
@@ -936,6 +952,8 @@ const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16, int bits)
     if (S == 25 && W == 4) return "tile<S=25,W=4>";
     if (S == 128 && W == 8) return "tile<S=128,W=8>";
     if (S >= 1 && S <= ((S & 1) ? 288 : 576)) return "staged<any>";  // dyn_shape: units up to 1152 bytes
+  } else if (rta_dyn_eligible(S, W) && (2 * S * ((S & 1) ? 2 : 1)) % 32 != 0) {
+    return "staged<any>";  // dense layout: any 2-byte alignment (also for the specialised shapes)
   }
   return "generic";
 }
@@ -952,6 +970,7 @@ struct LaunchArgs {
   float *out_charge, *out_time;
   cudaStream_t stream;
   bool staged;  // 16-byte aligned input and not forced to the generic kernel
+  bool unaligned_staged;  // any other input not forced to the generic kernel
 };
 
 template <int MODE, int BITS>
@@ -1064,6 +1083,13 @@ cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
     DynShape sh;
     int threads = 0;
     if (dyn_shape(a.S, a.W, &sh, &threads)) return launch_dyn<MODE>(a, sh, threads, ma);
+  } else if (a.unaligned_staged && !gather) {
+    // a base that is only 2-byte aligned: the runtime-shape kernel with a dense
+    // layout takes it (the specialisations and the padded layout need 16 bytes)
+    DynShape sh;
+    int threads = 0;
+    if (dyn_shape(a.S, a.W, &sh, &threads) && sh.unit_stride == sh.unit_bytes)
+      return launch_dyn<MODE>(a, sh, threads, ma);
   }
   return launch_generic<MODE, 16>(a, ma);
 }
@@ -1219,6 +1245,7 @@ cudaError_t rta_launch_extract(const void* wf, int64_t n_traces64, int32_t n_pix
   a.out_time = out_time;
   a.stream = stream;
   a.staged = !force_generic && ((uintptr_t)wf % 16) == 0;
+  a.unaligned_staged = !force_generic && !a.staged && sample_bits == 16;
   ModeArgs ma = {};
   const int kind = mode ? mode->kind : RTA_MODE_SLIDING;
   if (sample_bits == 12)

@@ -88,13 +88,17 @@ def test_strerror_and_kernel_names():
     assert rta.rta_kernel_name(30, 7) == "tile<S=30,W=7>"
     assert rta.rta_kernel_name(25, 4) == "tile<S=25,W=4>"
     assert rta.rta_kernel_name(128, 8) == "tile<S=128,W=8>"
-    assert rta.rta_kernel_name(40, 7, aligned16=False) == "generic"
+    # a base that is only 2-byte aligned: dense layouts take the runtime-shape kernel,
+    # units of a multiple of 32 bytes (padded layout, 16-byte cp.async) the generic one
+    assert rta.rta_kernel_name(40, 7, aligned16=False) == "staged<any>"
+    assert rta.rta_kernel_name(128, 8, aligned16=False) == "generic"
     # any other shape with units up to 1152 bytes: the staged kernel with runtime (S, W)
     assert rta.rta_kernel_name(41, 7) == "staged<any>"
     assert rta.rta_kernel_name(60, 7) == "staged<any>"
     assert rta.rta_kernel_name(576, 9) == "staged<any>" and rta.rta_kernel_name(287, 9) == "staged<any>"
     assert rta.rta_kernel_name(578, 9) == "generic" and rta.rta_kernel_name(289, 9) == "generic"
-    assert rta.rta_kernel_name(60, 7, aligned16=False) == "generic"
+    assert rta.rta_kernel_name(60, 7, aligned16=False) == "staged<any>"
+    assert rta.rta_kernel_name(96, 8, aligned16=False) == "generic"
 
 
 def test_binding_raises_on_error_status():

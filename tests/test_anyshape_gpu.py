@@ -90,3 +90,34 @@ def test_any_shape_closed_forms():
     for k in range(S):
         assert got[0][k] == 50 and got[1][k] == max(0, k - W + 1) and got[3][k] == np.float32(k)
     assert got[0][S] == W * (777 - ped) and got[1][S] == 0 and got[3][S] == np.float32((W - 1) / 2)
+
+
+@pytest.mark.parametrize("S,W", [(30, 7), (40, 7), (25, 4), (60, 7), (50, 8), (200, 9), (33, 5), (128, 8), (96, 8)])
+@pytest.mark.parametrize("off", [1, 2, 3, 5, 7])
+def test_unaligned_base_pointers(S, W, off):
+    """A waveform pointer `off` halfwords past a 16-byte boundary: dense layouts
+    (the specialised shapes included) take the runtime-shape kernel with the tile
+    landing `mis` bytes into the stage, padded layouts the generic kernel. The
+    buffer ends exactly at the last sample and is followed by a guard whose value
+    must not matter; numbers of traces with and without a ragged tail."""
+    import torch
+    import paper_1307_6489_b200 as rta
+    from tests._gpu import alloc_outputs
+    rng = np.random.default_rng(S * 10 + off)
+    padded = (2 * S * (2 if S % 2 else 1)) % 32 == 0
+    assert rta.rta_kernel_name(S, W, aligned16=False) == ("generic" if padded else "staged<any>")
+    for E, P in ((3, 1855), (2, 512), (1, 5)):
+        wf = rng.integers(0, 4096, size=(E, P, S)).astype(np.uint16)
+        ped = rng.integers(0, 600, P).astype(np.int32)
+        gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
+        want = oracle.extract(wf, ped, gain, W)
+        for guard in (0, -1):
+            buf = torch.full((wf.size + off + 16,), guard, dtype=torch.int16, device="cuda")
+            assert buf.data_ptr() % 16 == 0
+            buf[off:off + wf.size] = torch.from_numpy(wf.reshape(-1).view(np.int16)).cuda()
+            view = buf[off:off + wf.size]
+            outs = alloc_outputs(E * P)
+            rta.rta_extract(view, E, P, S, torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda(),
+                            W, *outs)
+            torch.cuda.synchronize()
+            assert bit_identical(tuple(o.cpu().numpy() for o in outs), want), (E, P, guard)
