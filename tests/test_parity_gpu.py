@@ -151,7 +151,7 @@ def test_pedestals_at_the_edges_of_the_sample_range(S, W):
         assert bit_identical(got, want)
 
 
-def test_unaligned_input_takes_generic_kernel_and_agrees():
+def test_unaligned_input_agrees():
     import torch
     import paper_1307_6489_b200 as rta
     c = dl0gen.CONFIGS["C1"]
