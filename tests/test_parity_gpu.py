@@ -336,3 +336,44 @@ def test_cuda_graph_capture_and_replay():
         torch.cuda.synchronize()
         assert bit_identical(tuple(o.cpu().numpy() for o in outs),
                              oracle.extract(wf, ped, gain, c.W))
+
+
+@pytest.mark.parametrize("S,W,kernel", [(25, 4, "tile<S=25,W=4>"), (2, 1, "staged<any>")])
+def test_largest_trace_count(S, W, kernel):
+    """n_events * n_pixels just below the ABI guard 2^31 (R14): the 32-bit trace
+    indices, tile counts and the scheduler must hold up to the last trace. Sampled
+    blocks of traces (first, middle, last tiles and the ragged tail) against the oracle."""
+    import torch
+    import paper_1307_6489_b200 as rta
+    E, P = 1049088, 2047                       # 2 147 483 136 traces, 512 short of 2^31
+    n = E * P
+    need = n * (2 * S + 16) + (2 << 30)
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    if free < need:
+        pytest.skip("needs %.0f GB of device memory" % (need / 1e9))
+    assert rta.rta_kernel_name(S, W) == kernel
+    wf = torch.empty(n * S, dtype=torch.int16, device="cuda")
+    step = 1 << 28
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    for a in range(0, n * S, step):
+        b = min(a + step, n * S)
+        wf[a:b] = torch.randint(0, 4096, (b - a,), generator=gen, device="cuda", dtype=torch.int16)
+    rng = np.random.default_rng(9)
+    ped = rng.integers(0, 600, P).astype(np.int32)
+    gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
+    outs = [torch.full((n,), f, dtype=dt, device="cuda") for f, dt in
+            zip((-7, -7, -7.0, -7.0), (torch.int32, torch.int32, torch.float32, torch.float32))]
+    rta.rta_extract(wf, E, P, S, torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda(), W, *outs)
+    torch.cuda.synchronize()
+    assert int((outs[1] < 0).sum()) == 0        # every trace was written (a start is never negative)
+    blocks = [0, 1 << 20, n // 2 - 333, (1 << 31) - (1 << 16), n - 5000, n - 700]
+    for g0 in blocks:
+        m = min(3001, n - g0)
+        sub = wf[g0 * S:(g0 + m) * S].cpu().numpy().view(np.uint16).reshape(1, m, S)
+        pix = (g0 + np.arange(m)) % P
+        want = oracle.extract(sub, ped[pix], gain[pix], W)
+        got = tuple(o[g0:g0 + m].cpu().numpy() for o in outs)
+        assert bit_identical(got, want), g0
+    del wf, outs
+    torch.cuda.empty_cache()
