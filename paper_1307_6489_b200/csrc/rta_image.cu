@@ -471,20 +471,38 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   for (uint32_t e = blockIdx.x * WARPS + warp; e < n_events; e += stride) {
     const float* q = charge + (size_t)e * (size_t)P;
     constexpr int U = 16;  // loads in flight per lane: the sweep is one DRAM latency per 512 pixels
-    for (int p0 = 0; p0 < P; p0 += 32 * U) {
+    int p0 = 0;
+    // whole blocks of 32 U pixels: no bounds checks; lane u keeps word u of the
+    // block and lanes 0 .. U-1 store the block's words with one instruction each
+    for (; p0 + 32 * U <= P; p0 += 32 * U) {
+      float v[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) v[u] = __ldg(q + p0 + 32 * u + lane);
+      uint32_t mc = 0, ml = 0;
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const uint32_t c = __ballot_sync(0xFFFFFFFFu, v[u] >= thr_p);
+        const uint32_t l = __ballot_sync(0xFFFFFFFFu, v[u] >= thr_b);
+        if (lane == u) mc = c, ml = l;
+      }
+      if (lane < U) core_w[(p0 >> 5) + lane] = mc, low_w[(p0 >> 5) + lane] = ml;
+    }
+    if (p0 < P) {  // the last < 32 U pixels: the same block with bounds checks (loads still batched)
       float v[U];
 #pragma unroll
       for (int u = 0; u < U; ++u) {
         const int p = p0 + 32 * u + lane;
         v[u] = p < P ? __ldg(q + p) : 0.0f;
       }
+      uint32_t mc = 0, ml = 0;
 #pragma unroll
       for (int u = 0; u < U; ++u) {
         const bool in = p0 + 32 * u + lane < P;
         const uint32_t c = __ballot_sync(0xFFFFFFFFu, in && v[u] >= thr_p);
         const uint32_t l = __ballot_sync(0xFFFFFFFFu, in && v[u] >= thr_b);
-        if (lane == 0 && p0 + 32 * u < P) core_w[(p0 >> 5) + u] = c, low_w[(p0 >> 5) + u] = l;
+        if (lane == u) mc = c, ml = l;
       }
+      if (lane < U && p0 + 32 * lane < P) core_w[(p0 >> 5) + lane] = mc, low_w[(p0 >> 5) + lane] = ml;
     }
     __syncwarp();
     clean_event(e, P, q, time + (size_t)e * (size_t)P, core_w, low_w, sc, cam, out, symmetric, pd,
