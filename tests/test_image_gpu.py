@@ -319,6 +319,10 @@ def test_fused_unspecialised_shapes_run_extract_then_moments(S, W, P, E):
     for a, b, c in zip(got, gen, again):
         assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
         assert np.array_equal(a.view(np.uint8), c.view(np.uint8))
+    rta.rta_shutdown()                          # drops the scratch pool; the next call rebuilds it
+    after = gpu_extract_image(wf, ped, gain, W, x, y, nbr, 60.0, 30.0)
+    for a, b in zip(got, after):
+        assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
 
 
 def test_fused_unaligned_waveforms_take_the_generic_kernel():
