@@ -56,11 +56,7 @@ void rta_count_launch();
 // round-robin (tests compare the two). rta_sched_release frees the per-stream
 // scheduler words (rta_shutdown).
 void rta_set_static_schedule(bool on);
-bool rta_static_schedule();
 void rta_sched_release();
-// {next work item, CTAs done} pair owned by (device, stream), zero between
-// launches; nullptr = none available (use the static round-robin).
-uint32_t* rta_sched_words(int dev, cudaStream_t stream);
 cudaError_t rta_device_sms(int dev, int* sms);
 
 // Image cleaning + moments (include/rta.h rta_image_moments, rta_extract_image;

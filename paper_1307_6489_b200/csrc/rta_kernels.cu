@@ -912,9 +912,7 @@ int TileLauncher<C, MODE>::ctas_per_sm[kMaxDevices];
 }  // namespace
 
 void rta_set_static_schedule(bool on) { g_static_schedule.store(on); }
-bool rta_static_schedule() { return g_static_schedule.load(); }
 cudaError_t rta_device_sms(int dev, int* sms) { return device_sms(dev, sms); }
-uint32_t* rta_sched_words(int dev, cudaStream_t stream) { return sched_words(dev, stream); }
 
 // rta_shutdown: the caller has synchronised the device(s)
 void rta_sched_release() {
