@@ -871,6 +871,14 @@ struct ImgCfg {
   static constexpr int THREADS = G * C::NT + 32 * NCMAX;
   static constexpr size_t RING = (size_t)G * C::STAGES * (C::STAGE_BYTES + 16);
   static_assert(THREADS <= 1024, "one CTA");
+  // the register split of extract_image_kernel (same condition as there): the
+  // warpgroups trade registers inside what the CTA was launched with, which is
+  // the launch bound's cap (ptxas allocates it in full when setmaxnreg is used);
+  // a split that does not fit would leave setmaxnreg.inc waiting for ever
+  static constexpr bool REGSPLIT = ((G * C::NT) % 128 == 0) && (NCMAX == 4);
+  static constexpr int LAUNCH_REGS = ((65536 / THREADS) / 8) * 8;
+  static constexpr int SPLIT_REGS = G * C::NT * kExtractRegs + 32 * NCMAX * kCleanRegs;
+  static_assert(!REGSPLIT || SPLIT_REGS <= THREADS * LAUNCH_REGS, "register split exceeds the CTA's pool");
 };
 using ImgS30W7 = ImgCfg<TileCfg<30, 7, RTA_I30_NT, 2>, RTA_I30_G, RTA_IMG_NC>;
 using ImgS40W7 = ImgCfg<TileCfg<40, 7, RTA_I40_NT, 2>, RTA_I40_G, RTA_IMG_NC>;
@@ -920,6 +928,11 @@ struct FusedLauncher {
       smem += EventBuf::bytes(P);
     }
     auto kernel = extract_image_kernel<C, I::G, I::NCMAX>;
+    if (I::REGSPLIT) {  // never launch a split that the allocated registers cannot serve
+      cudaFuncAttributes fa;
+      if ((e = cudaFuncGetAttributes(&fa, kernel)) != cudaSuccess) return e;
+      if (fa.numRegs * I::THREADS < I::SPLIT_REGS) return cudaErrorLaunchOutOfResources;
+    }
     // the dynamic shared-memory size depends on n_pixels: set per launch (cheap)
     e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
