@@ -622,9 +622,9 @@ __global__ void __launch_bounds__(NT + 32)
 //   freeb[b]    one arrival by the cleaning warp per cleaned event; the extraction
 //               threads wait before the first write of event k >= NB
 constexpr int kMaxBuf = 8;
-constexpr int kCleanRegs = 152, kExtractRegs = 56;  // after the register split (multiples of 8)
+constexpr int kCleanRegs = 152;  // cleaning warpgroup after the register split (multiple of 8)
 
-template <class C, int G, int NCMAX>
+template <class C, int G, int NCMAX, int XREGS>
 __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
     extract_image_kernel(const uint8_t* __restrict__ wf, const uint32_t n_events, const int P,
                          const int* __restrict__ pedestal, const float* __restrict__ gain,
@@ -662,9 +662,9 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
   // event number k of this CTA. n_events < 2^31 and the walks stop a few items
   // past the end, so 32 bits hold every index that is formed
   const auto event_of = [&](const uint32_t k) -> uint32_t { return blockIdx.x + k * gridDim.x; };
-  // Register split (whole warpgroups only): the extraction code needs about 48
-  // registers, the cleaning code about 130; the CTA is launched with the same
-  // number for everyone and the warpgroups trade them here.
+  // Register split (whole warpgroups only): the extraction code needs 48-56
+  // registers (XREGS, tuned per shape), the cleaning code about 130; the CTA is
+  // launched with the same number for everyone and the warpgroups trade them here.
   constexpr bool REGSPLIT = (NX % 128 == 0) && (NCMAX == 4);
 
   if (tid >= NX) {  // ------------------------------------------------ cleaning warps
@@ -689,7 +689,7 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
   }
 
   // ---------------------------------------------------------------- extraction groups
-  if constexpr (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kExtractRegs));
+  if constexpr (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(XREGS));
   const int g = tid / NT, gt = tid - g * NT;
   const uint32_t ring = smem_u32(smem) + (uint32_t)(g * C::STAGES * STG);
   uint8_t* ringp = smem + (size_t)g * C::STAGES * STG;
@@ -864,10 +864,10 @@ std::atomic<bool> g_general_cleaning{false};  // tests: never take the symmetric
 #ifndef RTA_I128_NC
 #define RTA_I128_NC 2
 #endif
-template <class C_, int G_, int NCMAX_>
+template <class C_, int G_, int NCMAX_, int XREGS_ = 56>
 struct ImgCfg {
   using C = C_;
-  static constexpr int G = G_, NCMAX = NCMAX_;
+  static constexpr int G = G_, NCMAX = NCMAX_, XREGS = XREGS_;
   static constexpr int THREADS = G * C::NT + 32 * NCMAX;
   static constexpr size_t RING = (size_t)G * C::STAGES * (C::STAGE_BYTES + 16);
   static_assert(THREADS <= 1024, "one CTA");
@@ -877,11 +877,12 @@ struct ImgCfg {
   // a split that does not fit would leave setmaxnreg.inc waiting for ever
   static constexpr bool REGSPLIT = ((G * C::NT) % 128 == 0) && (NCMAX == 4);
   static constexpr int LAUNCH_REGS = ((65536 / THREADS) / 8) * 8;
-  static constexpr int SPLIT_REGS = G * C::NT * kExtractRegs + 32 * NCMAX * kCleanRegs;
+  static constexpr int SPLIT_REGS = G * C::NT * XREGS + 32 * NCMAX * kCleanRegs;
   static_assert(!REGSPLIT || SPLIT_REGS <= THREADS * LAUNCH_REGS, "register split exceeds the CTA's pool");
 };
 using ImgS30W7 = ImgCfg<TileCfg<30, 7, RTA_I30_NT, 2>, RTA_I30_G, RTA_IMG_NC>;
-using ImgS40W7 = ImgCfg<TileCfg<40, 7, RTA_I40_NT, 2>, RTA_I40_G, RTA_IMG_NC>;
+// 48 registers for the S = 40 extraction code: 0.253 ms on C2 against 0.268 ms at 56 (and 0.290 at 40)
+using ImgS40W7 = ImgCfg<TileCfg<40, 7, RTA_I40_NT, 2>, RTA_I40_G, RTA_IMG_NC, 48>;
 using ImgS25W4 = ImgCfg<TileCfg<25, 4, RTA_I25_NT, 2>, RTA_I25_G, RTA_IMG_NC>;
 using ImgS128W8 = ImgCfg<TileCfg<128, 8, RTA_I128_NT, 2>, RTA_I128_G, RTA_I128_NC>;
 
@@ -927,7 +928,7 @@ struct FusedLauncher {
       ++nb;
       smem += EventBuf::bytes(P);
     }
-    auto kernel = extract_image_kernel<C, I::G, I::NCMAX>;
+    auto kernel = extract_image_kernel<C, I::G, I::NCMAX, I::XREGS>;
     if (I::REGSPLIT) {  // never launch a split that the allocated registers cannot serve
       cudaFuncAttributes fa;
       if ((e = cudaFuncGetAttributes(&fa, kernel)) != cudaSuccess) return e;
