@@ -883,7 +883,10 @@ struct ImgCfg {
 using ImgS30W7 = ImgCfg<TileCfg<30, 7, RTA_I30_NT, 2>, RTA_I30_G, RTA_IMG_NC>;
 // 48 registers for the S = 40 extraction code: 0.253 ms on C2 against 0.268 ms at 56 (and 0.290 at 40)
 using ImgS40W7 = ImgCfg<TileCfg<40, 7, RTA_I40_NT, 2>, RTA_I40_G, RTA_IMG_NC, 48>;
-using ImgS25W4 = ImgCfg<TileCfg<25, 4, RTA_I25_NT, 2>, RTA_I25_G, RTA_IMG_NC>;
+#ifndef RTA_I25_XREGS
+#define RTA_I25_XREGS 64
+#endif
+using ImgS25W4 = ImgCfg<TileCfg<25, 4, RTA_I25_NT, 2>, RTA_I25_G, RTA_IMG_NC, RTA_I25_XREGS>;
 using ImgS128W8 = ImgCfg<TileCfg<128, 8, RTA_I128_NT, 2>, RTA_I128_G, RTA_I128_NC>;
 
 // Cleaning warps NC and event buffers NB = NC + 1 that fit behind the ring
