@@ -23,6 +23,12 @@ Prints ONE JSON line (rank 0). Keys beyond the driver's contract:
                 decoded inside the extraction kernel; sustained.packed12 is C5
                 fed as 22.26 GB of P12 through rta_extract_stream_packed12
   ragged        NEXT-3: a mixed-camera array through rta_extract_ragged
+  image         NEXT-4: rta_extract_image (extraction + cleaning + moments in one
+                kernel) next to rta_extract followed by rta_image_moments;
+                sustained.image is C5 through rta_extract_image_stream
+  any_shape     shapes without a specialised kernel (not BASELINE configs) through
+                the staged kernel with runtime (n_samples, W), next to the generic one
+Secondary legs are single-GPU diagnostics (N = 1 only) and run ten untimed launches first.
 """
 from __future__ import annotations
 
