@@ -1001,7 +1001,7 @@ bool dyn_shape(int32_t S, int32_t W, DynShape* sh, int* threads) {
   // threads per CTA: the candidate that keeps most warps resident (two stages per
   // CTA in 227 KB of shared memory; about 62 registers per thread: 32 warps at most)
   int nt = 32, best_warps = 0;
-  const int candidates[4] = {128, 256, 64, 32};  // ties go to the earlier entry (measured)
+  const int candidates[5] = {stride >= 160 ? 64 : 128, 128, 256, 64, 32};  // ties go to the earlier entry (measured: long units prefer small CTAs)
   for (const int cand : candidates) {
     const int stage = ((cand * stride + 64 + 127) / 128) * 128;
     int ctas = (227 * 1024) / (2 * stage + 1024);
