@@ -226,6 +226,10 @@ int rta_extract_host_packed12(const uint8_t* packed_host, int64_t n_events,
  *
  * rta_extract_ragged is asynchronous on `stream`: one launch per distinct
  * (n_samples, W) among the blocks (rta_ragged_plan_info(RTA_RAGGED_N_LAUNCHES)).
+ * The launches are independent; all but the first run on library-owned side
+ * streams that are forked from `stream` and joined back into it before the call
+ * returns, so the caller sees ordinary stream order: everything is complete when
+ * `stream` reaches the end of the call's work.
  * Shapes (30,7), (40,7), (25,4), (128,8) take the specialised staged kernels,
  * other traces of at most 1152 bytes a staged kernel with runtime shape, longer
  * ones a generic kernel. Blocks starting on a 16-byte boundary of `wf` are fastest
