@@ -265,6 +265,7 @@ struct DynShape {
   int32_t kb;           // key bits: 2^kb >= n_win
   uint32_t key_mul;     // 2^kb
   uint32_t peak_mul;    // local peak: 2^ceil(log2 S)
+  int32_t cpu_shift;    // padded layout: log2(16-byte chunks per unit) when that is a power of two, else -1
 };
 constexpr int kDynMaxStages = 4;
 
@@ -429,13 +430,19 @@ __global__ void __launch_bounds__(256)
     } else {
       // chunk c of the tile belongs to unit c / chunks_per_unit: one chunk of padding per unit
       const uint32_t n_chunks = (uint32_t)sh.tile_bytes / 16u;
-      uint32_t u = (uint32_t)tid / chunks_per_unit, r = (uint32_t)tid - u * chunks_per_unit;
-      const uint32_t du = (uint32_t)NT / chunks_per_unit, dr = (uint32_t)NT - du * chunks_per_unit;
-      for (uint32_t c = tid; c < n_chunks; c += NT) {
-        cp_async16(dst + (c + u) * 16u, src + (size_t)c * 16u);
-        u += du;
-        r += dr;
-        if (r >= chunks_per_unit) r -= chunks_per_unit, ++u;
+      if (sh.cpu_shift >= 0) {  // a power of two chunks per unit: the unit index is a shift
+#pragma unroll 4
+        for (uint32_t c = tid; c < n_chunks; c += NT)
+          cp_async16(dst + (c + (c >> sh.cpu_shift)) * 16u, src + (size_t)c * 16u);
+      } else {
+        uint32_t u = (uint32_t)tid / chunks_per_unit, r = (uint32_t)tid - u * chunks_per_unit;
+        const uint32_t du = (uint32_t)NT / chunks_per_unit, dr = (uint32_t)NT - du * chunks_per_unit;
+        for (uint32_t c = tid; c < n_chunks; c += NT) {
+          cp_async16(dst + (c + u) * 16u, src + (size_t)c * 16u);
+          u += du;
+          r += dr;
+          if (r >= chunks_per_unit) r -= chunks_per_unit, ++u;
+        }
       }
       cp_async_mbar_arrive(bar);
     }
@@ -1024,6 +1031,8 @@ bool dyn_shape(int32_t S, int32_t W, DynShape* sh, int* threads) {
   sh->kb = ilog2_ceil(sh->n_win);
   sh->key_mul = 1u << sh->kb;
   sh->peak_mul = 1u << ilog2_ceil(S);
+  const int cpu = (int)(ub / 16);
+  sh->cpu_shift = (pad && (cpu & (cpu - 1)) == 0) ? ilog2_ceil(cpu) : -1;
   *threads = nt;
   return true;
 }
