@@ -706,8 +706,20 @@ __global__ void __launch_bounds__(256)
         }
       } else {
         done = bytes & ~15u;  // whole units are whole chunks; a last half unit may not be
-        for (uint32_t c = tid; c < done / 16u; c += NT)
-          cp_async16(dst + (c + c / (UB / 16u)) * 16u, src + (size_t)c * 16u);
+        const uint32_t cpu = UB / 16u;  // chunks per unit: one chunk of padding after each
+        if (sh.cpu_shift >= 0) {
+          for (uint32_t c = tid; c < done / 16u; c += NT)
+            cp_async16(dst + (c + (c >> sh.cpu_shift)) * 16u, src + (size_t)c * 16u);
+        } else {
+          uint32_t u = (uint32_t)tid / cpu, r = (uint32_t)tid - u * cpu;
+          const uint32_t du = (uint32_t)NT / cpu, dr = (uint32_t)NT - du * cpu;
+          for (uint32_t c = tid; c < done / 16u; c += NT) {
+            cp_async16(dst + (c + u) * 16u, src + (size_t)c * 16u);
+            u += du;
+            r += dr;
+            if (r >= cpu) r -= cpu, ++u;
+          }
+        }
       }
     } else if ((mis & 3u) == 0) {
       done = bytes & ~3u;
