@@ -880,7 +880,10 @@ struct ImgCfg {
   static constexpr int SPLIT_REGS = G * C::NT * XREGS + 32 * NCMAX * kCleanRegs;
   static_assert(!REGSPLIT || SPLIT_REGS <= THREADS * LAUNCH_REGS, "register split exceeds the CTA's pool");
 };
-using ImgS30W7 = ImgCfg<TileCfg<30, 7, RTA_I30_NT, 2>, RTA_I30_G, RTA_IMG_NC>;
+#ifndef RTA_I30_XREGS
+#define RTA_I30_XREGS 56
+#endif
+using ImgS30W7 = ImgCfg<TileCfg<30, 7, RTA_I30_NT, 2>, RTA_I30_G, RTA_IMG_NC, RTA_I30_XREGS>;
 // 48 registers for the S = 40 extraction code: 0.253 ms on C2 against 0.268 ms at 56 (and 0.290 at 40)
 using ImgS40W7 = ImgCfg<TileCfg<40, 7, RTA_I40_NT, 2>, RTA_I40_G, RTA_IMG_NC, 48>;
 #ifndef RTA_I25_XREGS
