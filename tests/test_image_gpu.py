@@ -325,6 +325,25 @@ def test_fused_unspecialised_shapes_run_extract_then_moments(S, W, P, E):
         assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
 
 
+@pytest.mark.parametrize("name,n_events", [("C2", 1300), ("C3", 1500), ("C4", 700)])
+def test_fused_dense_images_and_buffer_reuse(name, n_events):
+    """Pedestals 25 counts too low make almost every pixel pass the picture threshold:
+    the cleaning warps become the bound, so the extraction groups wait for free event
+    buffers (several events per CTA: every buffer is reused) — the hand-off under the
+    opposite load of the sparse configs. Sampled events against the oracle, all events
+    against the generic fused kernel."""
+    cfg, wf, ped, gain, x, y, nbr, tp, tb = config_batch(name, n_events)
+    ped = (ped - 25).astype(np.int32)
+    got = gpu_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb)
+    assert got[0].mean() > 0.5 * cfg.n_pixels
+    gen = gpu_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb, generic=True)
+    for a, b in zip(got, gen):
+        assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
+    pick = np.r_[0:6, n_events // 2: n_events // 2 + 6, n_events - 6: n_events]
+    want = oracle_extract_image(wf[pick], ped, gain, cfg.W, x, y, nbr, tp, tb)
+    assert_image_parity(tuple(g[pick] for g in got), want, x, y, name + " dense")
+
+
 def test_fused_unaligned_waveforms_take_the_generic_kernel():
     import torch
     cfg, wf, ped, gain, x, y, nbr, tp, tb = config_batch("C2", 20)
