@@ -73,9 +73,11 @@ enum {
  * Asynchronous: validates, enqueues on `stream`, returns without synchronising.
  * Outputs are valid once `stream` has been synchronised. n_events == 0 is
  * RTA_OK with nothing enqueued and the outputs untouched. Thread-safe across
- * streams; capturable into a CUDA graph after one warm-up call on the device
- * (the first call allocates 128 KB of per-stream tile-scheduler words, owned by
- * the library and released by rta_shutdown). */
+ * streams. Capturable into a CUDA graph: a captured launch hands its tiles out
+ * in a fixed round-robin and touches no library state, so replays may run on
+ * any stream, next to one another and next to eager calls. (Eager calls use
+ * 128 KB of per-stream tile-scheduler words, allocated by the first eager call
+ * on a device, owned by the library and released by rta_shutdown.) */
 int rta_extract(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
                 int32_t n_samples, const int32_t* pedestal, const float* gain,
                 int32_t W, int32_t* out_sum, int32_t* out_start,

@@ -24,7 +24,12 @@ _SRCS = [_SRC, os.path.join(_HERE, "rta_oracle_windows.cpp"),
          os.path.join(_HERE, "rta_oracle_packed.cpp"),
          os.path.join(_HERE, "rta_oracle_ragged.cpp"),
          os.path.join(_HERE, "rta_oracle_image.cpp")]
-_LIB = os.path.join(_HERE, "librta_oracle.so")
+# RTA_ORACLE_SANITIZE=1: an instrumented build (-fsanitize=address,undefined) beside
+# the plain one, for a memory-safety pass of the CPU tests:
+#   LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 \
+#   RTA_ORACLE_SANITIZE=1 python -m pytest tests -q -m "not gpu"
+_SANITIZE = os.environ.get("RTA_ORACLE_SANITIZE", "") not in ("", "0")
+_LIB = os.path.join(_HERE, "librta_oracle_san.so" if _SANITIZE else "librta_oracle.so")
 _lock = threading.Lock()
 _lib = None
 
@@ -36,9 +41,11 @@ def build(force: bool = False) -> str:
                  or any(os.path.getmtime(_LIB) < os.path.getmtime(f) for f in _SRCS))
         if force or stale:
             tmp = _LIB + ".tmp%d" % os.getpid()
+            san = (["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=all"]
+                   if _SANITIZE else [])
             subprocess.check_call(
                 ["g++", "-std=c++17", "-O2", "-fPIC", "-shared",
-                 "-ffp-contract=off", "-o", tmp] + _SRCS)
+                 "-ffp-contract=off"] + san + ["-o", tmp] + _SRCS)
             os.replace(tmp, _LIB)
     return _LIB
 

@@ -23,6 +23,8 @@ RTA_ERR_NOMEM = 6
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lock = threading.Lock()
 _lib = None
+_test_lib = None
+_hooks_on: set = set()     # names of the rta_debug_* switches that are on (tests only)
 
 _VP = ctypes.c_void_p
 _EXTRACT_ARGS = [_VP, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, _VP, _VP,
@@ -36,90 +38,113 @@ class RtaError(RuntimeError):
         self.cuda_error = cuda_error
 
 
+def _declare(L: ctypes.CDLL, testing: bool) -> ctypes.CDLL:
+    for name in ("rta_extract",) + (("rta_extract_generic",) if testing else ()):
+        fn = getattr(L, name)
+        fn.restype = ctypes.c_int
+        fn.argtypes = _EXTRACT_ARGS + [_VP]
+    L.rta_extract_stream.restype = ctypes.c_int
+    L.rta_extract_stream.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t, _VP]
+    L.rta_extract_host.restype = ctypes.c_int
+    L.rta_extract_host.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t]
+    L.rta_extract_packed12.restype = ctypes.c_int
+    L.rta_extract_packed12.argtypes = _EXTRACT_ARGS + [_VP]
+    L.rta_extract_stream_packed12.restype = ctypes.c_int
+    L.rta_extract_stream_packed12.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t, _VP]
+    L.rta_extract_host_packed12.restype = ctypes.c_int
+    L.rta_extract_host_packed12.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t]
+    L.rta_kernel_name_packed12.restype = ctypes.c_char_p
+    L.rta_kernel_name_packed12.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int]
+    L.rta_extract_fixed.restype = ctypes.c_int
+    L.rta_extract_fixed.argtypes = _EXTRACT_ARGS[:7] + [_VP] + [_VP] * 4 + [_VP]
+    L.rta_extract_local_peak.restype = ctypes.c_int
+    L.rta_extract_local_peak.argtypes = _EXTRACT_ARGS[:7] + [ctypes.c_int32] + [_VP] * 4 + [_VP]
+    L.rta_extract_fir.restype = ctypes.c_int
+    L.rta_extract_fir.argtypes = _EXTRACT_ARGS[:6] + [_VP, ctypes.c_int32] + [_VP] * 4 + [_VP]
+    L.rta_strerror.restype = ctypes.c_char_p
+    L.rta_strerror.argtypes = [ctypes.c_int]
+    L.rta_last_cuda_error.restype = ctypes.c_int
+    L.rta_last_cuda_error.argtypes = []
+    L.rta_kernel_name.restype = ctypes.c_char_p
+    L.rta_kernel_name.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int]
+    L.rta_ragged_plan_create.restype = ctypes.c_int
+    L.rta_ragged_plan_create.argtypes = ([ctypes.c_int32] + [_VP] * 4 + [ctypes.c_int64]
+                                         + [_VP] * 3 + [ctypes.POINTER(_VP)])
+    L.rta_extract_ragged.restype = ctypes.c_int
+    L.rta_extract_ragged.argtypes = [_VP] * 9
+    L.rta_ragged_plan_info.restype = ctypes.c_int64
+    L.rta_ragged_plan_info.argtypes = [_VP, ctypes.c_int32]
+    L.rta_ragged_plan_destroy.restype = None
+    L.rta_ragged_plan_destroy.argtypes = [_VP]
+    _CAM = [_VP, _VP, _VP, ctypes.c_float, ctypes.c_float]
+    _IMG_OUT = [_VP, _VP, _VP]
+    L.rta_image_moments.restype = ctypes.c_int
+    L.rta_image_moments.argtypes = ([_VP, _VP, ctypes.c_int64, ctypes.c_int32] + _CAM
+                                    + _IMG_OUT + [_VP])
+    for name in ("rta_extract_image",) + (("rta_extract_image_generic",) if testing else ()):
+        fn = getattr(L, name)
+        fn.restype = ctypes.c_int
+        fn.argtypes = _EXTRACT_ARGS[:7] + _CAM + _IMG_OUT + [_VP]
+    L.rta_extract_image_stream.restype = ctypes.c_int
+    L.rta_extract_image_stream.argtypes = (_EXTRACT_ARGS[:7] + _CAM + _IMG_OUT
+                                           + [ctypes.c_size_t, _VP])
+    L.rta_extract_image_host.restype = ctypes.c_int
+    L.rta_extract_image_host.argtypes = (_EXTRACT_ARGS[:7] + _CAM + _IMG_OUT
+                                         + [ctypes.c_size_t])
+    L.rta_image_kernel_name.restype = ctypes.c_char_p
+    L.rta_image_kernel_name.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                        ctypes.c_int]
+    L.rta_image_max_pixels.restype = ctypes.c_int32
+    L.rta_image_max_pixels.argtypes = []
+    L.rta_chunk_events.restype = ctypes.c_int64
+    L.rta_chunk_events.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32,
+                                   ctypes.c_size_t, ctypes.c_int32]
+    L.rta_launch_count.restype = ctypes.c_uint64
+    L.rta_launch_count.argtypes = []
+    L.rta_shutdown.restype = None
+    L.rta_shutdown.argtypes = []
+    if testing:
+        for name in ("rta_debug_force_generic", "rta_debug_static_schedule",
+                     "rta_debug_serial_ragged", "rta_debug_general_cleaning"):
+            fn = getattr(L, name)
+            fn.restype = None
+            fn.argtypes = [ctypes.c_int]
+    return L
+
+
+def _load(testing: bool) -> ctypes.CDLL:
+    from . import build as _build
+    path = _build.build()
+    if testing:
+        path = _build.TEST_LIB
+    if not os.path.exists(path):
+        raise ImportError("%s is missing and could not be built" % path)
+    return _declare(ctypes.CDLL(path), testing)
+
+
 def lib() -> ctypes.CDLL:
-    """Load (building in-tree if stale) librta.so and declare its symbols."""
+    """Load (building in-tree if stale) librta.so and declare its symbols: the
+    ABI of include/rta.h, nothing else. While a test hook is switched on (see
+    :func:`testing_lib`) every call is routed to librta_testing.so instead."""
     global _lib
+    if _hooks_on:
+        return testing_lib()
     with _lock:
         if _lib is None:
-            from . import build as _build
-            path = _build.build()
-            if not os.path.exists(path):
-                raise ImportError("librta.so is missing and could not be built: " + path)
-            L = ctypes.CDLL(path)
-            for name in ("rta_extract", "rta_extract_generic"):
-                fn = getattr(L, name)
-                fn.restype = ctypes.c_int
-                fn.argtypes = _EXTRACT_ARGS + [_VP]
-            L.rta_extract_stream.restype = ctypes.c_int
-            L.rta_extract_stream.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t, _VP]
-            L.rta_extract_host.restype = ctypes.c_int
-            L.rta_extract_host.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t]
-            L.rta_extract_packed12.restype = ctypes.c_int
-            L.rta_extract_packed12.argtypes = _EXTRACT_ARGS + [_VP]
-            L.rta_extract_stream_packed12.restype = ctypes.c_int
-            L.rta_extract_stream_packed12.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t, _VP]
-            L.rta_extract_host_packed12.restype = ctypes.c_int
-            L.rta_extract_host_packed12.argtypes = _EXTRACT_ARGS + [ctypes.c_size_t]
-            L.rta_kernel_name_packed12.restype = ctypes.c_char_p
-            L.rta_kernel_name_packed12.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int]
-            L.rta_extract_fixed.restype = ctypes.c_int
-            L.rta_extract_fixed.argtypes = _EXTRACT_ARGS[:7] + [_VP] + [_VP] * 4 + [_VP]
-            L.rta_extract_local_peak.restype = ctypes.c_int
-            L.rta_extract_local_peak.argtypes = _EXTRACT_ARGS[:7] + [ctypes.c_int32] + [_VP] * 4 + [_VP]
-            L.rta_extract_fir.restype = ctypes.c_int
-            L.rta_extract_fir.argtypes = _EXTRACT_ARGS[:6] + [_VP, ctypes.c_int32] + [_VP] * 4 + [_VP]
-            L.rta_debug_force_generic.restype = None
-            L.rta_debug_force_generic.argtypes = [ctypes.c_int]
-            L.rta_strerror.restype = ctypes.c_char_p
-            L.rta_strerror.argtypes = [ctypes.c_int]
-            L.rta_last_cuda_error.restype = ctypes.c_int
-            L.rta_last_cuda_error.argtypes = []
-            L.rta_kernel_name.restype = ctypes.c_char_p
-            L.rta_kernel_name.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int]
-            L.rta_ragged_plan_create.restype = ctypes.c_int
-            L.rta_ragged_plan_create.argtypes = ([ctypes.c_int32] + [_VP] * 4 + [ctypes.c_int64]
-                                                 + [_VP] * 3 + [ctypes.POINTER(_VP)])
-            L.rta_extract_ragged.restype = ctypes.c_int
-            L.rta_extract_ragged.argtypes = [_VP] * 9
-            L.rta_ragged_plan_info.restype = ctypes.c_int64
-            L.rta_ragged_plan_info.argtypes = [_VP, ctypes.c_int32]
-            L.rta_ragged_plan_destroy.restype = None
-            L.rta_ragged_plan_destroy.argtypes = [_VP]
-            _CAM = [_VP, _VP, _VP, ctypes.c_float, ctypes.c_float]
-            _IMG_OUT = [_VP, _VP, _VP]
-            L.rta_image_moments.restype = ctypes.c_int
-            L.rta_image_moments.argtypes = ([_VP, _VP, ctypes.c_int64, ctypes.c_int32] + _CAM
-                                            + _IMG_OUT + [_VP])
-            for name in ("rta_extract_image", "rta_extract_image_generic"):
-                fn = getattr(L, name)
-                fn.restype = ctypes.c_int
-                fn.argtypes = _EXTRACT_ARGS[:7] + _CAM + _IMG_OUT + [_VP]
-            L.rta_extract_image_stream.restype = ctypes.c_int
-            L.rta_extract_image_stream.argtypes = (_EXTRACT_ARGS[:7] + _CAM + _IMG_OUT
-                                                   + [ctypes.c_size_t, _VP])
-            L.rta_extract_image_host.restype = ctypes.c_int
-            L.rta_extract_image_host.argtypes = (_EXTRACT_ARGS[:7] + _CAM + _IMG_OUT
-                                                 + [ctypes.c_size_t])
-            L.rta_image_kernel_name.restype = ctypes.c_char_p
-            L.rta_image_kernel_name.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
-                                                ctypes.c_int]
-            L.rta_image_max_pixels.restype = ctypes.c_int32
-            L.rta_image_max_pixels.argtypes = []
-            L.rta_chunk_events.restype = ctypes.c_int64
-            L.rta_chunk_events.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32,
-                                           ctypes.c_size_t, ctypes.c_int32]
-            L.rta_launch_count.restype = ctypes.c_uint64
-            L.rta_launch_count.argtypes = []
-            L.rta_shutdown.restype = None
-            L.rta_shutdown.argtypes = []
-            L.rta_debug_static_schedule.restype = None
-            L.rta_debug_static_schedule.argtypes = [ctypes.c_int]
-            L.rta_debug_serial_ragged.restype = None
-            L.rta_debug_serial_ragged.argtypes = [ctypes.c_int]
-            L.rta_debug_general_cleaning.restype = None
-            L.rta_debug_general_cleaning.argtypes = [ctypes.c_int]
-            _lib = L
+            _lib = _load(False)
     return _lib
+
+
+def testing_lib() -> ctypes.CDLL:
+    """librta_testing.so: the same sources built with -DRTA_TESTING, which adds
+    the entry points the tests need and the shipped library does not export
+    (rta_extract_generic, rta_extract_image_generic, rta_debug_*). The two
+    libraries share no state."""
+    global _test_lib
+    with _lock:
+        if _test_lib is None:
+            _test_lib = _load(True)
+    return _test_lib
 
 
 def _ptr(x) -> int | None:
@@ -155,7 +180,7 @@ def rta_extract(wf, n_events, n_pixels, n_samples, pedestal, gain, W,
                 generic: bool = False) -> None:
     """include/rta.h:rta_extract. Device pointers (tensors or addresses);
     asynchronous on ``stream`` (default: torch's current stream)."""
-    fn = lib().rta_extract_generic if generic else lib().rta_extract
+    fn = testing_lib().rta_extract_generic if generic else lib().rta_extract
     _check(fn(_ptr(wf), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain), W,
               _ptr(out_sum), _ptr(out_start), _ptr(out_charge), _ptr(out_time),
               _stream_handle(stream)))
@@ -306,7 +331,7 @@ def rta_extract_image(wf, n_events, n_pixels, n_samples, pedestal, gain, W, pix_
                       neighbors, thr_picture, thr_boundary, out_n_pix, out_params,
                       out_mask=None, stream=None, *, generic: bool = False) -> None:
     """include/rta.h:rta_extract_image. Device pointers; asynchronous on ``stream``."""
-    fn = lib().rta_extract_image_generic if generic else lib().rta_extract_image
+    fn = testing_lib().rta_extract_image_generic if generic else lib().rta_extract_image
     _check(fn(_ptr(wf), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain), W,
               _ptr(pix_x), _ptr(pix_y), _ptr(neighbors), float(thr_picture),
               float(thr_boundary), _ptr(out_n_pix), _ptr(out_params), _ptr(out_mask),
@@ -375,27 +400,33 @@ def rta_shutdown() -> None:
     lib().rta_shutdown()
 
 
+def _hook(name: str, on: bool) -> None:
+    getattr(testing_lib(), name)(1 if on else 0)
+    (_hooks_on.add if on else _hooks_on.discard)(name)
+
+
 def rta_debug_force_generic(on: bool) -> None:
-    """Test hook: route rta_extract_fixed/_local_peak/_fir/_packed12 to the generic kernel."""
-    lib().rta_debug_force_generic(1 if on else 0)
+    """Test hook (librta_testing.so): route rta_extract_fixed/_local_peak/_fir/_packed12
+    to the generic kernel."""
+    _hook("rta_debug_force_generic", on)
 
 
 def rta_debug_static_schedule(on: bool) -> None:
-    """Test hook: force the static round-robin tile schedule of the staged
-    kernels (default is dynamic). Results are identical either way."""
-    lib().rta_debug_static_schedule(1 if on else 0)
+    """Test hook (librta_testing.so): force the static round-robin tile schedule of the
+    staged kernels (default is dynamic). Results are identical either way."""
+    _hook("rta_debug_static_schedule", on)
 
 
 def rta_debug_serial_ragged(on: bool) -> None:
-    """Test hook: rta_extract_ragged issues its launches one after the other on
-    the caller's stream instead of forking side streams. Same results."""
-    lib().rta_debug_serial_ragged(1 if on else 0)
+    """Test hook (librta_testing.so): rta_extract_ragged issues its launches one after
+    the other on the caller's stream instead of forking side streams. Same results."""
+    _hook("rta_debug_serial_ragged", on)
 
 
 def rta_debug_general_cleaning(on: bool) -> None:
-    """Test hook: the image cleaning runs the two steps of its definition even
-    when the neighbour table is symmetric (same masks either way)."""
-    lib().rta_debug_general_cleaning(1 if on else 0)
+    """Test hook (librta_testing.so): the image cleaning runs the two steps of its
+    definition even when the neighbour table is symmetric (same masks either way)."""
+    _hook("rta_debug_general_cleaning", on)
 
 
 def shard_events(n_events: int, world_size: int, rank: int) -> tuple[int, int]:

@@ -3,7 +3,28 @@
 // page-locked transfer experiment of PAPER.md:133/139 §5 is its ancestor).
 // No CPU fallback exists here: every compute call ends in a kernel launch or
 // in an error code.
+// The library is built with -fvisibility=hidden: what it exports is what
+// include/rta.h declares (plus the test hooks below in librta_testing.so).
+#pragma GCC visibility push(default)
 #include "../../include/rta.h"
+#ifdef RTA_TESTING
+extern "C" {
+int rta_extract_generic(const uint16_t* wf, int64_t n_events, int32_t n_pixels, int32_t n_samples,
+                        const int32_t* pedestal, const float* gain, int32_t W, int32_t* out_sum,
+                        int32_t* out_start, float* out_charge, float* out_time, void* stream);
+int rta_extract_image_generic(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
+                              int32_t n_samples, const int32_t* pedestal, const float* gain,
+                              int32_t W, const float* pix_x, const float* pix_y,
+                              const int32_t* neighbors, float thr_picture, float thr_boundary,
+                              int32_t* out_n_pix, float* out_params, uint8_t* out_mask,
+                              void* stream);
+void rta_debug_serial_ragged(int on);
+void rta_debug_force_generic(int on);
+void rta_debug_static_schedule(int on);
+void rta_debug_general_cleaning(int on);
+}
+#endif
+#pragma GCC visibility pop
 
 #include <cuda_runtime.h>
 
@@ -178,6 +199,7 @@ ChunkPlan plan_chunks(int64_t n_events, int32_t n_pixels, int32_t n_samples, siz
   const int64_t ev_samples = (int64_t)n_pixels * (int64_t)n_samples;
   p.event_bits = (size_t)ev_samples * (size_t)bits;
   if (chunk_bytes == 0) chunk_bytes = (size_t)1 << 30;
+  if (chunk_bytes > ((size_t)1 << 48)) chunk_bytes = (size_t)1 << 48;  // the products below stay far from 2^64
   const int64_t m = bits == 12 ? 32 / gcd64(ev_samples, 32) : 1;
   int64_t ce = (int64_t)((chunk_bytes / p.event_bits) * 8u +
                          ((chunk_bytes % p.event_bits) * 8u) / p.event_bits);  // whole events
@@ -458,8 +480,10 @@ int rta_extract(const uint16_t* wf, int64_t n_events, int32_t n_pixels, int32_t 
   return e == cudaSuccess ? RTA_OK : fail_cuda(e);
 }
 
-// Same as rta_extract but always through the generic kernel. Exported for the
-// tests (two independent device paths must agree); not in the public header.
+#ifdef RTA_TESTING
+// Same as rta_extract but always through the generic kernel. Only in
+// librta_testing.so (built with -DRTA_TESTING; two independent device paths
+// must agree); the shipped librta.so exports include/rta.h and nothing else.
 int rta_extract_generic(const uint16_t* wf, int64_t n_events, int32_t n_pixels, int32_t n_samples,
                         const int32_t* pedestal, const float* gain, int32_t W, int32_t* out_sum,
                         int32_t* out_start, float* out_charge, float* out_time, void* stream) {
@@ -471,6 +495,7 @@ int rta_extract_generic(const uint16_t* wf, int64_t n_events, int32_t n_pixels, 
                          out_sum, out_start, out_charge, out_time, (cudaStream_t)stream, true);
   return e == cudaSuccess ? RTA_OK : fail_cuda(e);
 }
+#endif  // RTA_TESTING
 
 // ---- the other members of the extractor family (NEXT-1; readings R22-R24) ----
 int rta_extract_fixed(const uint16_t* wf, int64_t n_events, int32_t n_pixels, int32_t n_samples,
@@ -637,6 +662,12 @@ int rta_ragged_plan_create(int32_t n_tel, const int32_t* tel_n_pixels,
       return RTA_ERR_SHAPE;
     }
     const int64_t P = tel_n_pixels[k], S = tel_n_samples[k];
+    // range checks before any arithmetic on the offsets: an offset near 2^62
+    // would wrap (P * S < 2^46 by the telescope checks above)
+    if (blk_wf_offset[b] >= (1ll << 47) || blk_out_offset[b] >= (1ll << 31)) {
+      delete pl;
+      return RTA_ERR_UNSUPPORTED;
+    }
     const int64_t end_bytes = (blk_wf_offset[b] + P * S) * 2;
     if (blk_out_offset[b] + P >= (1ll << 31) || end_bytes >= (1ll << 48)) {
       delete pl;
@@ -874,7 +905,8 @@ int rta_extract_image(const uint16_t* wf, int64_t n_events, int32_t n_pixels, in
                               out_mask, stream, false);
 }
 
-// Same through the generic fused kernel. Exported for the tests; not in the public header.
+#ifdef RTA_TESTING
+// Same through the generic fused kernel (librta_testing.so only).
 int rta_extract_image_generic(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
                               int32_t n_samples, const int32_t* pedestal, const float* gain,
                               int32_t W, const float* pix_x, const float* pix_y,
@@ -885,6 +917,7 @@ int rta_extract_image_generic(const uint16_t* wf, int64_t n_events, int32_t n_pi
                               neighbors, thr_picture, thr_boundary, out_n_pix, out_params,
                               out_mask, stream, true);
 }
+#endif  // RTA_TESTING
 
 int rta_extract_image_stream(const uint16_t* wf_host, int64_t n_events, int32_t n_pixels,
                              int32_t n_samples, const int32_t* pedestal, const float* gain,
@@ -995,6 +1028,7 @@ int64_t rta_chunk_events(int64_t n_events, int32_t n_pixels, int32_t n_samples,
                          size_t chunk_bytes, int32_t sample_bits) {
   if (n_events < 0 || n_pixels < 1 || n_samples < 1 || (sample_bits != 16 && sample_bits != 12))
     return -1;
+  if ((int64_t)n_pixels * (int64_t)n_samples >= (1ll << 46)) return -1;  // event_bits must fit
   return plan_chunks(n_events, n_pixels, n_samples, chunk_bytes, sample_bits).chunk_events;
 }
 
@@ -1018,20 +1052,24 @@ void rta_shutdown(void) {
   rta_sched_release();
 }
 
-// Test hook (not in the public header): 1 = rta_extract_ragged issues every
-// launch on the caller's stream, one after the other.
+#ifdef RTA_TESTING
+// Test hooks: process-global switches that exist in librta_testing.so only, so
+// that no program linked against the shipped library can flip the dispatch of
+// another thread's calls.
+// 1 = rta_extract_ragged issues every launch on the caller's stream, one after the other.
 void rta_debug_serial_ragged(int on) { g_serial_ragged.store(on != 0); }
 
-// Test hook (not in the public header): 1 = rta_extract_fixed / _local_peak / _fir /
+// 1 = rta_extract_fixed / _local_peak / _fir /
 // _packed12 take the generic kernel whatever the shape (two device paths must agree).
 void rta_debug_force_generic(int on) { g_force_generic.store(on != 0); }
 
-// Test hook (not in the public header): 1 = static round-robin tile schedule,
+// 1 = static round-robin tile schedule,
 // 0 = dynamic (default). Results are identical; only the tile->CTA map changes.
 void rta_debug_static_schedule(int on) { rta_set_static_schedule(on != 0); }
 
-// Test hook (not in the public header): 1 = the image cleaning runs the two
+// 1 = the image cleaning runs the two
 // steps of its definition even when the neighbour table is symmetric.
 void rta_debug_general_cleaning(int on) { rta_set_general_cleaning(on != 0); }
+#endif  // RTA_TESTING
 
 }  // extern "C"

@@ -940,9 +940,8 @@ struct FusedLauncher {
       if ((e = cudaFuncGetAttributes(&fa, kernel)) != cudaSuccess) return e;
       if (fa.numRegs * I::THREADS < I::SPLIT_REGS) return cudaErrorLaunchOutOfResources;
     }
-    // the dynamic shared-memory size depends on n_pixels: set per launch (cheap)
-    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    // the dynamic shared-memory size depends on n_pixels
+    if ((e = rta_func_allow_max_smem((const void*)kernel, dev)) != cudaSuccess) return e;
     uint32_t grid = (uint32_t)sms;
     if (grid > n_events) grid = n_events;
     ModeArgs ma = {};  // constant-bank operands of compute_results (KEYMUL)
@@ -964,9 +963,8 @@ cudaError_t launch_moments(const float* charge, const float* time, uint32_t n_ev
   if (e != cudaSuccess) return e;
   if ((e = rta_device_sms(dev, &sms)) != cudaSuccess) return e;
   const size_t smem = WARPS * moments_warp_bytes(P);
-  e = cudaFuncSetAttribute(image_moments_kernel<WARPS>,
-                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
+  if ((e = rta_func_allow_max_smem((const void*)image_moments_kernel<WARPS>, dev)) != cudaSuccess)
+    return e;
   uint32_t grid = (uint32_t)sms;  // one CTA per SM (launch bounds)
   const uint32_t need = (n_events + WARPS - 1u) / WARPS;
   if (grid > need) grid = need;
@@ -1106,8 +1104,7 @@ cudaError_t rta_launch_extract_image(const void* wf, int64_t n_events, int32_t n
   if (e != cudaSuccess) return e;
   if ((e = rta_device_sms(dev, &sms)) != cudaSuccess) return e;
   auto kernel = extract_image_generic_kernel<kGenericNT>;
-  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
+  if ((e = rta_func_allow_max_smem((const void*)kernel, dev)) != cudaSuccess) return e;
   int occ = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, kGenericNT + 32, smem);
   if (e != cudaSuccess) return e;

@@ -58,6 +58,8 @@ void rta_count_launch();
 void rta_set_static_schedule(bool on);
 void rta_sched_release();
 cudaError_t rta_device_sms(int dev, int* sms);
+// Allow `func` up to 227 KB of dynamic shared memory on `dev` (set once per kernel and device).
+cudaError_t rta_func_allow_max_smem(const void* func, int dev);
 
 // Image cleaning + moments (include/rta.h rta_image_moments, rta_extract_image;
 // DESIGN.md readings R31-R35). Device pointers, already validated.

@@ -41,8 +41,8 @@ namespace {
 // CTA has finished its fixed share (measured: 4-7 % of SM-time idle). `sched`
 // points at {next tile, CTAs done}, both zero on entry; the last CTA to leave
 // zeroes them again, so the pair is reusable by the next launch on the same
-// stream (and by CUDA-graph replays). sched == nullptr selects the static
-// round-robin (same code path, locally generated indices).
+// stream. sched == nullptr selects the static round-robin (same code path,
+// locally generated indices); launches captured into a CUDA graph use it.
 // The first `stages` tiles of every CTA are the static round-robin ones (no
 // atomic round trip before the first load); the shared counter hands out the
 // tiles after those, in runs of up to kMaxRun consecutive tiles per atomic:
@@ -638,9 +638,11 @@ __global__ void __launch_bounds__(C::NT)
     const uint32_t first = (uint32_t)tid * C::TPT;
     if (first < n) {
       const uint8_t* unit = smem + stage * C::STAGE_BYTES + tid * C::UNIT_STRIDE;
-      compute_unit<C, MODE_SLIDING>(unit, t.out_base + first, n - first, t.cal0 + first, 0u,
-                                    pedestal, gain, out_sum, out_start, out_charge, out_time,
-                                    vec_store != 0 && (t.out_base & 1u) == 0, ma);
+      // the calibration index "wraps" after the tile's last trace, so the discarded
+      // second trace of an odd tile reads pedestal[0], never past the arrays
+      compute_unit<C, MODE_SLIDING>(unit, t.out_base + first, n - first, t.cal0 + first,
+                                    t.cal0 + n, pedestal, gain, out_sum, out_start, out_charge,
+                                    out_time, vec_store != 0 && (t.out_base & 1u) == 0, ma);
     }
     __syncthreads();
     const uint32_t next = tile_q[(j + C::STAGES) % QN];
@@ -768,8 +770,8 @@ __global__ void __launch_bounds__(256)
     if (first < n) {
       const uint8_t* unit = smem + stage * sh.stage_bytes + tid * sh.unit_stride;
       dyn_compute_unit<G, MODE_SLIDING>(sh, ma, unit, t.out_base + first, n - first,
-                                        t.cal0 + first, 0u, pedestal, gain, out_sum, out_start,
-                                        out_charge, out_time);
+                                        t.cal0 + first, t.cal0 + n, pedestal, gain, out_sum,
+                                        out_start, out_charge, out_time);  // wrap: see above
     }
     __syncthreads();
     const uint32_t next = tile_q[(j + STAGES) % QN];
@@ -829,8 +831,9 @@ cudaError_t device_sms(int dev, int* sms) {
 }
 
 // ---- scheduler words: one {next tile, CTAs done} pair per (device, stream) ----
-// Launches on one stream run one after the other, so a pair owned by a stream
-// is never shared by two running kernels; the kernel leaves it zeroed.
+// Eager launches on one stream run one after the other, so a pair owned by a
+// stream is never shared by two running kernels; the kernel leaves it zeroed.
+// Launches recorded into a CUDA graph get no pair (sched_words).
 constexpr int kSchedSlots = 1024;      // distinct streams per device before falling back
 constexpr int kSchedSlotWords = 32;    // 128 bytes apart: one L2 line per pair
 
@@ -845,6 +848,16 @@ SchedPool g_sched;
 // nullptr = no pair available (static round-robin is used instead)
 uint32_t* sched_words(int dev, cudaStream_t stream) {
   if (stream == cudaStreamPerThread) return nullptr;  // one handle, many streams
+  // A captured launch keeps its kernel arguments for every replay, and replays
+  // may run on any stream, next to eager calls on the capture stream or to other
+  // graphs captured on it: two running grids would then draw from one counter.
+  // Captured launches therefore take the static round-robin (no shared state).
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(stream, &cap) != cudaSuccess) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  if (cap != cudaStreamCaptureStatusNone) return nullptr;
   std::lock_guard<std::mutex> lock(g_sched.mu);
   if (g_sched.failed[dev]) return nullptr;
   if (g_sched.base[dev] == nullptr) {
@@ -872,6 +885,27 @@ uint32_t* sched_words(int dev, cudaStream_t stream) {
   }
   return g_sched.base[dev] + (size_t)slot * kSchedSlotWords;
 }
+
+}  // namespace
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize of `func` on `dev`, raised once to
+// the most a CTA can have (227 KB) for kernels whose dynamic shared memory
+// depends on the call (shape, camera size): a per-launch set would let one host
+// thread lower it between another thread's set and its launch.
+cudaError_t rta_func_allow_max_smem(const void* func, int dev) {
+  static std::mutex mu;
+  static std::unordered_map<uintptr_t, uint32_t> done;  // kernel -> bit per device
+  if (dev < 0 || dev >= 32) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(mu);
+  uint32_t& bits = done[(uintptr_t)func];
+  if (bits & (1u << dev)) return cudaSuccess;
+  const cudaError_t e =
+      cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+  if (e == cudaSuccess) bits |= 1u << dev;
+  return e;
+}
+
+namespace {
 
 template <class C, int MODE>
 struct TileLauncher {
@@ -1064,9 +1098,8 @@ cudaError_t launch_dyn(const LaunchArgs& a, const DynShape& sh, int threads, con
                         : sh.g == 2 ? extract_dyn_kernel<false, 2, MODE>
                                     : extract_dyn_kernel<false, 4, MODE>;
   const int smem = sh.stages * sh.stage_bytes;
-  // the dynamic shared-memory size depends on the shape: set per launch (cheap)
-  if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess)
-    return e;
+  // the dynamic shared-memory size depends on the shape
+  if ((e = rta_func_allow_max_smem((const void*)kernel, dev)) != cudaSuccess) return e;
   int occ = 0;
   if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem)) != cudaSuccess)
     return e;
@@ -1216,9 +1249,7 @@ cudaError_t rta_launch_ragged(const void* wf, const RtaRaggedTile* tiles_dev, ui
                           : sh.g == 2 ? extract_ragged_dyn_kernel<false, 2>
                                       : extract_ragged_dyn_kernel<false, 4>;
     const int smem = sh.stages * sh.stage_bytes;
-    if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) !=
-        cudaSuccess)
-      return e;
+    if ((e = rta_func_allow_max_smem((const void*)kernel, dev)) != cudaSuccess) return e;
     int occ = 0;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem)) != cudaSuccess)
       return e;

@@ -15,7 +15,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def declared_symbols():
     text = open(os.path.join(ROOT, "include", "rta.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(rta_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(rta_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_library_exports_every_declared_symbol():
@@ -26,6 +26,28 @@ def test_library_exports_every_declared_symbol():
             "rta_shutdown"} <= set(names)
     for n in names:
         assert hasattr(L, n), n
+
+
+def test_shipped_library_exports_exactly_the_header():
+    """librta.so is built with hidden visibility: its defined dynamic function
+    symbols are the functions include/rta.h declares, no test hook, no internal
+    C++ symbol. The hooks exist in librta_testing.so only."""
+    import subprocess
+    from paper_1307_6489_b200 import build as b
+
+    def exported(path):
+        out = subprocess.run(["nm", "-D", "--defined-only", path], capture_output=True,
+                             text=True, check=True).stdout
+        return sorted(f[2] for f in (ln.split() for ln in out.splitlines())
+                      if len(f) == 3 and f[1] == "T")
+    rta.lib()
+    assert exported(b.LIB) == declared_symbols()
+    hooks = {"rta_extract_generic", "rta_extract_image_generic", "rta_debug_force_generic",
+             "rta_debug_static_schedule", "rta_debug_serial_ragged", "rta_debug_general_cleaning"}
+    assert set(exported(b.TEST_LIB)) == set(declared_symbols()) | hooks
+    T = rta.testing_lib()
+    for n in hooks:
+        assert hasattr(T, n) and not hasattr(rta.lib(), n), n
 
 
 def test_library_links_no_torch():

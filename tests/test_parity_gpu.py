@@ -310,8 +310,7 @@ def test_concurrent_streams_have_their_own_scheduler_words():
 
 
 def test_cuda_graph_capture_and_replay():
-    """rta_extract is capturable: the scheduler words are reset by the kernel
-    itself, so a replayed graph sees them zeroed again."""
+    """rta_extract is capturable (a captured launch takes the static tile schedule)."""
     import torch
     import paper_1307_6489_b200 as rta
     c = dl0gen.CONFIGS["C2"]
@@ -336,6 +335,53 @@ def test_cuda_graph_capture_and_replay():
         torch.cuda.synchronize()
         assert bit_identical(tuple(o.cpu().numpy() for o in outs),
                              oracle.extract(wf, ped, gain, c.W))
+
+
+def test_graph_replays_run_next_to_eager_calls_and_to_each_other():
+    """Two graphs captured on ONE stream, replayed on two other streams at the
+    same time as eager calls on the capture stream, 50 rounds: a captured launch
+    must not share tile-scheduler state with anything (it takes the static
+    round-robin), or tiles are skipped and outputs stay unwritten. Batches are
+    small enough for several grids to be resident together."""
+    import torch
+    import paper_1307_6489_b200 as rta
+    c = dl0gen.CONFIGS["C2"]
+    ped, gain = dl0gen.calib(c)
+    d_ped, d_gain = torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda()
+    A, B, C = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    jobs = []
+    for i, n_ev in enumerate((37, 41, 29)):               # graph 1, graph 2, eager
+        wf = dl0gen.events_cpu(c, 500 * i, n_ev, threads=4)
+        jobs.append((n_ev, to_dev_u16(wf), alloc_outputs(n_ev * c.n_pixels),
+                     oracle.extract(wf, ped, gain, c.W)))
+
+    def call(j):
+        n_ev, d_wf, outs, _ = jobs[j]
+        rta.rta_extract(d_wf, n_ev, c.n_pixels, c.n_samples, d_ped, d_gain, c.W, *outs)
+    with torch.cuda.stream(A):                            # warm-up on the capture stream
+        call(2)
+    torch.cuda.synchronize()
+    graphs = []
+    for j in (0, 1):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=A):
+            call(j)
+        graphs.append(g)
+    for rnd in range(50):
+        for n_ev, d_wf, outs, want in jobs:
+            for o in outs:
+                o.fill_(-3)
+        torch.cuda.synchronize()
+        for _ in range(4):                                # several of each in flight
+            with torch.cuda.stream(B):
+                graphs[0].replay()
+            with torch.cuda.stream(C):
+                graphs[1].replay()
+            with torch.cuda.stream(A):
+                call(2)
+        torch.cuda.synchronize()
+        for j, (n_ev, d_wf, outs, want) in enumerate(jobs):
+            assert bit_identical(tuple(o.cpu().numpy() for o in outs), want), (rnd, j)
 
 
 @pytest.mark.parametrize("S,W,kernel", [(25, 4, "tile<S=25,W=4>"), (2, 1, "staged<any>")])

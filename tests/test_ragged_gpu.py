@@ -32,10 +32,12 @@ def run_gpu(b, wf=None, wf_shift=0, streams=1, static=False, serial=False):
     n = b.n_out + 3
     outs = [torch.full((n,), f, dtype=dt, device="cuda")
             for f, dt in zip(FILL, (torch.int32, torch.int32, torch.float32, torch.float32))]
+    # the hooks live in librta_testing.so; while one is on the binding routes every
+    # call there, so the plan is made and destroyed under the same switches
+    rta.rta_debug_static_schedule(static)
+    rta.rta_debug_serial_ragged(serial)
     plan = rta.rta_ragged_plan_create(*b.tables())
     try:
-        rta.rta_debug_static_schedule(static)
-        rta.rta_debug_serial_ragged(serial)
         before = rta.rta_launch_count()
         rta.rta_extract_ragged(plan, d_wf, d_ped, d_gain, *outs)
         torch.cuda.synchronize()
@@ -43,9 +45,9 @@ def run_gpu(b, wf=None, wf_shift=0, streams=1, static=False, serial=False):
         assert rta.rta_ragged_plan_info(plan, rta.RTA_RAGGED_N_TRACES) == sum(
             b.tel_n_pixels[k] for k in b.blk_tel)
     finally:
+        rta.rta_ragged_plan_destroy(plan)
         rta.rta_debug_static_schedule(False)
         rta.rta_debug_serial_ragged(False)
-        rta.rta_ragged_plan_destroy(plan)
     return tuple(o.cpu().numpy() for o in outs)
 
 
