@@ -889,7 +889,7 @@ uint32_t* sched_words(int dev, cudaStream_t stream) {
 }  // namespace
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize of `func` on `dev`, raised once to
-// the most a CTA can have (227 KB) for kernels whose dynamic shared memory
+// the most a CTA can have (227 KB with its static part) for kernels whose dynamic shared memory
 // depends on the call (shape, camera size): a per-launch set would let one host
 // thread lower it between another thread's set and its launch.
 cudaError_t rta_func_allow_max_smem(const void* func, int dev) {
@@ -899,8 +899,15 @@ cudaError_t rta_func_allow_max_smem(const void* func, int dev) {
   std::lock_guard<std::mutex> lock(mu);
   uint32_t& bits = done[(uintptr_t)func];
   if (bits & (1u << dev)) return cudaSuccess;
-  const cudaError_t e =
-      cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+  // the opt-in limit covers static + dynamic shared memory
+  cudaFuncAttributes fa;
+  cudaError_t e = cudaFuncGetAttributes(&fa, func);
+  if (e != cudaSuccess) return e;
+  int optin = 0;
+  if ((e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev)) != cudaSuccess)
+    return e;
+  e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           optin - (int)fa.sharedSizeBytes);
   if (e == cudaSuccess) bits |= 1u << dev;
   return e;
 }

@@ -13,6 +13,7 @@ import pytest
 import dl0gen
 import oracle
 from tests._checks import check_invariants
+from tests._full import alloc_filled_outputs, compare_every_event, slabs
 from tests._gpu import alloc_outputs, assert_parity, bit_identical, run_gpu, to_dev_u16
 
 pytestmark = pytest.mark.gpu
@@ -211,12 +212,14 @@ def test_config_models_small_batches(name, n_ev):
 
 
 @pytest.mark.parametrize("name", ["C2", "C3", "C4"])
-def test_full_size_configs_sampled_against_oracle(name):
+def test_full_size_configs_every_event_against_oracle(name):
     """BASELINE.json's full sizes, in the launch configuration bench.py times
     (one rta_extract over the whole device-resident batch): generate on the
-    GPU, extract, then compare sampled event blocks with the oracle run on the
-    same bytes regenerated on the host, and check the size-independent
-    invariants (P8/P9) on them."""
+    GPU, extract into sentinel-filled outputs, then compare EVERY event with the
+    oracle run on the same bytes (copied back in ~1 GB slabs, all host cores):
+    a tile dropped or duplicated anywhere in the launch fails here. A few event
+    blocks are also regenerated on the host (device bytes == host generator's
+    bytes) and put through the size-independent invariants (P8/P9)."""
     import torch
     import paper_1307_6489_b200 as rta
     c = dl0gen.CONFIGS[name]
@@ -225,25 +228,24 @@ def test_full_size_configs_sampled_against_oracle(name):
     dl0gen.events_cuda(c, d_wf.data_ptr(), 0, c.n_events, torch.cuda.current_stream().cuda_stream)
     d_ped = torch.from_numpy(ped).cuda()
     d_gain = torch.from_numpy(gain).cuda()
-    outs = alloc_outputs(c.n_traces)
+    outs = alloc_filled_outputs(c.n_traces)
+    before = rta.rta_launch_count()
     rta.rta_extract(d_wf, c.n_events, c.n_pixels, c.n_samples, d_ped, d_gain, c.W, *outs)
     torch.cuda.synchronize()
+    assert rta.rta_launch_count() == before + 1
+    n = compare_every_event(
+        c.n_events, c.n_pixels, slabs(c.n_events, c.n_pixels * c.n_samples * 2),
+        lambda e0, k: d_wf[e0:e0 + k].cpu().numpy().view(np.uint16),
+        lambda wf, a, b: oracle.extract(wf[a:b], ped, gain, c.W), outs)
+    assert n == c.n_events
     rng = np.random.default_rng(5)
-    blocks = [0, c.n_events - 12] + sorted(rng.integers(12, c.n_events - 24, 6).tolist())
-    for e0 in blocks:
+    for e0 in [0, c.n_events - 12] + sorted(rng.integers(12, c.n_events - 24, 2).tolist()):
         wf = dl0gen.events_cpu(c, e0, 12, threads=4)
-        # the device bytes are the host generator's bytes
         assert (d_wf[e0:e0 + 12].cpu().numpy().view(np.uint16) == wf).all()
-        want = oracle.extract(wf, ped, gain, c.W)
         lo, hi = e0 * c.n_pixels, (e0 + 12) * c.n_pixels
         got = tuple(o[lo:hi].cpu().numpy() for o in outs)
-        assert_parity(got, want, "%s events %d.." % (name, e0))
-        assert bit_identical(got, want)
+        assert_parity(got, oracle.extract(wf, ped, gain, c.W), "%s events %d.." % (name, e0))
         check_invariants(wf, ped, gain, c.W, *got)
-    # whole-batch properties that hold at any size
-    s, t = outs[0], outs[1]
-    assert int(t.min()) >= 0 and int(t.max()) <= c.n_samples - c.W
-    assert bool(torch.isfinite(outs[3]).all()) and bool(torch.isfinite(outs[2]).all())
 
 
 # ---- tile scheduler (dynamic by default) ---------------
