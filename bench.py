@@ -29,6 +29,13 @@ Prints ONE JSON line (rank 0). Keys beyond the driver's contract:
   any_shape     shapes without a specialised kernel (not BASELINE configs) through
                 the staged kernel with runtime (n_samples, W), next to the generic one
 Secondary legs are single-GPU diagnostics (N = 1 only) and run ten untimed launches first.
+
+`--gpus N` without a torchrun environment re-executes itself under
+`python -m torch.distributed.run --standalone --nproc-per-node N` (one rank per
+GPU, NCCL for the barrier and the MAX over ranks only; no data-path collective).
+At N > 1 every rank also runs the host-fed `sustained` leg on its own pinned
+buffer (each GPU has its own host link); `value` there is the aggregate over
+ranks on the slowest rank's time.
 """
 from __future__ import annotations
 
@@ -83,13 +90,50 @@ def hbm_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def csrc_sha256():
+    """Content hash of the kernel sources: ties an ncu capture to the code it measured
+    (the GPU box has no .git)."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_1307_6489_b200", "csrc")
+    h = hashlib.sha256()
+    for n in sorted(os.listdir(d)):
+        if n.endswith((".cu", ".cuh", ".h")):
+            h.update(n.encode())
+            h.update(open(os.path.join(d, n), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def ncu_traffic(name):
-    """DRAM bytes per launch from the committed ncu --set full capture, if any."""
+    """DRAM bytes per launch from the committed ncu --set full capture
+    (profiles/traffic.json), or None when the kernel sources have changed since
+    that capture. Returns (bytes or None, commit of the capture, stale?)."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     try:
-        return json.load(open(p)).get(name)
+        t = json.load(open(p))
     except Exception:
-        return None
+        return None, None, None
+    stale = t.get("csrc_sha256") != csrc_sha256()
+    return (None if stale else t.get("kernels", {}).get(name)), t.get("commit"), stale
+
+
+def oracle_sample_events(cfg):
+    """The ONE sampling rule for timing the oracle (both arms): the whole workload
+    when its input is at most 2 GB (C1, C2, C3), else the first 2 GB of events."""
+    ev_bytes = cfg.n_pixels * cfg.n_samples * 2
+    return min(cfg.n_events, max(1, int(2e9 // ev_bytes)))
+
+
+def event_slabs(n_events, event_bytes, slab_bytes=1 << 30):
+    step = max(1, slab_bytes // event_bytes)
+    for e0 in range(0, n_events, step):
+        yield e0, min(step, n_events - e0)
+
+
+def bits_equal(torch, dev_out, want, lo, hi):
+    """device outputs [lo, hi) == oracle outputs, bit for bit (floats as int32)."""
+    import numpy as np
+    return all(np.array_equal(o[lo:hi].cpu().numpy().view(np.int32), w.view(np.int32))
+               for o, w in zip(dev_out, want))
 
 
 class ClockSampler:
@@ -214,20 +258,23 @@ def reference_arm(args):
     cfg = workload(args.workload, dl0gen)
     cores = os.cpu_count() or 1
     ped, gain = dl0gen.calib(cfg)
-    # ~0.3 GB/s per core: size the per-step sample for about 1 s of all-cores work
-    n_ev = max(cores, min(cfg.n_events, 200 * cores))
+    n_ev = oracle_sample_events(cfg)      # the same sample as the b200 arm's cpu_baseline
     wf = dl0gen.events_cpu(cfg, 0, n_ev, threads=cores)
-    for _ in range(max(1, min(args.warmup, 2))):
+    for _ in range(max(1, min(args.warmup, 1))):
         oracle.extract_threads(wf, ped, gain, cfg.W, cores)
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
+    # bounded: at most `steps` passes and about two minutes of oracle time
+    steps, t_used = 0, 0.0
+    while steps < args.steps and (steps == 0 or t_used < 120.0):
+        t0 = time.perf_counter()
         oracle.extract_threads(wf, ped, gain, cfg.W, cores)
-    dt = (time.perf_counter() - t0) / args.steps
+        t_used += time.perf_counter() - t0
+        steps += 1
+    dt = t_used / steps
     val = wf.nbytes / dt / 1e9
     sample = "first %d of %d events of %s per step, %d threads" % (n_ev, cfg.n_events, cfg.name, cores)
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT,
-        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "n_gpus": args.gpus, "steps": steps, "warmup": args.warmup,
         "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int64", "data": "synthetic",
         "config": {"workload": "%s: %s" % (cfg.name, cfg.label), "sample": sample},
@@ -361,9 +408,26 @@ def family_leg(cfg, steps, peak, torch, dl0gen, rta):
         torch.cuda.synchronize()
         res[name] = summarise(cfg, time_steps(run, steps, stream), peak)
     res["fir"]["taps"] = taps
-    res["fixed"]["note"] = ("reads W samples per trace; traces longer than 96 bytes are gathered from global "
-                            "memory instead of streamed, so GB/s figures (which count the whole waveform) can "
-                            "exceed the HBM peak")
+    if 2 * cfg.n_samples > 96:
+        # rta_extract_fixed GATHERS for traces longer than 96 bytes (rta_kernels.cu launch_mode): it
+        # touches only the W-sample window of a trace, so its algorithmic bytes are the 32-byte
+        # sectors that window overlaps (+ 16 bytes out), not the whole waveform
+        st = start.cpu().numpy().astype(np.int64)
+        g = np.arange(min(cfg.n_traces, 64 * cfg.n_pixels), dtype=np.int64)
+        lo = g * (2 * cfg.n_samples) + 2 * st[g % cfg.n_pixels]
+        sectors = (lo + 2 * cfg.W - 1) // 32 - lo // 32 + 1
+        per_trace = 32.0 * float(sectors.mean()) + ALGO_BYTES_PER_TRACE_OUT
+        f = res["fixed"]
+        algo = per_trace * cfg.n_traces
+        f["route"] = "gather (generic kernel): W samples of each trace from global memory"
+        f["bytes_per_trace"] = per_trace
+        f["mean_sectors_per_trace"] = float(sectors.mean())
+        f["streamed_equivalent_GBps"] = f["algorithmic_GBps"]
+        f["algorithmic_GBps"] = algo / f["ms_avg"] / 1e6
+        f["frac_of_measured_hbm"] = f["algorithmic_GBps"] / peak
+        f["frac_of_nominal_8TBps"] = f["algorithmic_GBps"] / 8000.0
+    else:
+        res["fixed"]["route"] = "streamed (staged kernel): whole tiles cross HBM"
     return res
 
 
@@ -586,136 +650,238 @@ def e2e_leg(cfg, keep, steps, chunk_mb, torch, rta):
             "api": "rta_extract_host (pinned host in/out, double-buffered H2D, D2H on a third stream)"}
 
 
-def sustained_leg(torch, dl0gen, rta, link_gbs):
-    """BASELINE.json:configs[4]: C5 in pinned host memory, 1 GiB chunks."""
-    cfg = dl0gen.CONFIGS["C5"]
+def mem_available_bytes():
     try:
-        avail_kb = int([l for l in open("/proc/meminfo") if l.startswith("MemAvailable")][0].split()[1])
+        return 1024 * int([l for l in open("/proc/meminfo") if l.startswith("MemAvailable")][0].split()[1])
     except Exception:
-        avail_kb = 0
-    if avail_kb < 44 * 1024 * 1024:
-        return {"skipped": "needs 29.68 GB of pinned host memory; MemAvailable=%d MB" % (avail_kb // 1024)}
+        return 0
+
+
+def bind_to_gpu_numa_node(torch, local):
+    """Best effort: run this rank's host threads (and first-touch its pinned buffer)
+    on the NUMA node the GPU hangs off. Returns a note for the JSON line."""
+    try:
+        bus = torch.cuda.get_device_properties(local).pci_bus_id
+        dom = torch.cuda.get_device_properties(local).pci_domain_id
+        dev = torch.cuda.get_device_properties(local).pci_device_id
+        path = "/sys/bus/pci/devices/%04x:%02x:%02x.0/numa_node" % (dom, bus, dev)
+        node = int(open(path).read())
+        if node < 0:
+            return "numa node unknown"
+        cpus = set()
+        for part in open("/sys/devices/system/node/node%d/cpulist" % node).read().strip().split(","):
+            lo, _, hi = part.partition("-")
+            cpus.update(range(int(lo), int(hi or lo) + 1))
+        cpus &= os.sched_getaffinity(0)
+        if cpus:
+            os.sched_setaffinity(0, cpus)
+            return "bound to numa node %d (%d cpus)" % (node, len(cpus))
+        return "numa node %d has no allowed cpu" % node
+    except Exception as ex:
+        return "not bound (%s)" % type(ex).__name__
+
+
+def sustained_leg(torch, dl0gen, rta, link_gbs, world=1, rank=0, dist=None, verify=True):
+    """BASELINE.json:configs[4]: C5 in pinned host memory, 1 GiB chunks. At
+    world > 1 every rank feeds its own GPU from its own pinned buffer (sized so
+    that all ranks fit the host's memory); the aggregate is all ranks' bytes over
+    the slowest rank's device time."""
+    import numpy as np
+    cfg = dl0gen.CONFIGS["C5"]
+    ev_bytes = cfg.n_pixels * cfg.n_samples * 2
+    avail = mem_available_bytes()
+    n_events = cfg.n_events
+    if world > 1:
+        # every rank's pinned buffer plus slack must fit: at most 70 % of the host's memory in all
+        n_events = int(min(cfg.n_events, 0.7 * avail / world / ev_bytes))
+        n_events -= n_events % 1000
+        t = torch.tensor([n_events], device="cuda", dtype=torch.int64)
+        dist.all_reduce(t, op=dist.ReduceOp.MIN)
+        n_events = int(t.item())
+    elif avail < 44 << 30:
+        return {"skipped": "needs 29.68 GB of pinned host memory; MemAvailable=%d MB" % (avail >> 20)}
+    if n_events < 1000:
+        return {"skipped": "host memory too small for %d ranks; MemAvailable=%d MB" % (world, avail >> 20)}
+    n_traces = n_events * cfg.n_pixels
+    input_bytes = n_events * ev_bytes
     t0 = time.perf_counter()
-    host = torch.empty((cfg.n_events, cfg.n_pixels, cfg.n_samples), dtype=torch.int16, pin_memory=True)
+    host = torch.empty((n_events, cfg.n_pixels, cfg.n_samples), dtype=torch.int16, pin_memory=True)
     t_alloc = time.perf_counter() - t0
-    gen_ev = 10_000
+    gen_ev = 10_000 if n_events % 10_000 == 0 else 1000
     stage = torch.empty((gen_ev, cfg.n_pixels, cfg.n_samples), dtype=torch.int16, device="cuda")
     st = torch.cuda.current_stream().cuda_stream
-    for e0 in range(0, cfg.n_events, gen_ev):
-        dl0gen.events_cuda(cfg, stage.data_ptr(), e0, gen_ev, st)
+    first = rank * n_events                        # every rank streams its own events of C5's model
+    for e0 in range(0, n_events, gen_ev):
+        dl0gen.events_cuda(cfg, stage.data_ptr(), first + e0, gen_ev, st)
         host[e0:e0 + gen_ev].copy_(stage)
     torch.cuda.synchronize()
     del stage
     ped, gain = dl0gen.calib(cfg)
     d_ped, d_gain = torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda()
-    outs = [torch.empty(cfg.n_traces, dtype=dt, device="cuda")
-            for dt in (torch.int32, torch.int32, torch.float32, torch.float32)]
+    outs = [torch.full((n_traces,), f, dtype=dt, device="cuda") for f, dt in
+            ((-7, torch.int32), (-7, torch.int32), (-7.0, torch.float32), (-7.0, torch.float32))]
     stream = torch.cuda.current_stream()
 
+    def timed(run, reps=2):
+        """device time (CUDA events on the compute stream, which every chunk's kernel and
+        therefore every copy is ordered into) and host wall time; best of `reps`; with
+        several ranks the MAX over ranks of each repetition"""
+        best = None
+        for _ in range(reps):
+            torch.cuda.synchronize()
+            if dist is not None:
+                dist.barrier()
+                torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0 = time.perf_counter()
+            a.record(stream)
+            run()
+            b.record(stream)
+            torch.cuda.synchronize()
+            wall = time.perf_counter() - t0
+            dev = a.elapsed_time(b) / 1e3
+            if dist is not None:
+                t = torch.tensor([dev, wall], device="cuda", dtype=torch.float64)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                dev, wall = float(t[0]), float(t[1])
+            if best is None or dev < best[0]:
+                best = (dev, wall)
+        return best
+
     def run():
-        rta.rta_extract_stream(host, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain,
+        rta.rta_extract_stream(host, n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain,
                                cfg.W, *outs, chunk_bytes=1 << 30, stream=stream)
     run()                                        # warm-up: allocates the workspace
     torch.cuda.synchronize()
-    times = []
     before = rta.rta_launch_count()
-    for _ in range(2):
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()                 # first cudaMemcpyAsync issue ...
-        run()
-        torch.cuda.synchronize()                 # ... to completion of the last kernel
-        times.append(time.perf_counter() - t0)
+    dt, wall = timed(run)
     launches = (rta.rta_launch_count() - before) // 2
-    dt = min(times)
-    val = cfg.input_bytes / dt / 1e9
-    res = {"workload": "%s: %s" % (cfg.name, cfg.label), "value": val, "unit": UNIT,
-           "seconds": dt, "traces_per_s": cfg.n_traces / dt, "chunk_bytes": 1 << 30,
-           "chunks": launches, "h2d_bytes": cfg.input_bytes,
-           "host_link_GBps_measured": link_gbs, "frac_of_host_link": val / link_gbs,
+    val = world * input_bytes / dt / 1e9
+    res = {"workload": "%s: %s" % (cfg.name, cfg.label) + ("" if n_events == cfg.n_events else
+                                                         " (%d events per rank)" % n_events),
+           "value": val, "unit": UNIT, "ranks": world,
+           "seconds": dt, "seconds_wall": wall, "timing": "CUDA events on the compute stream, max over ranks",
+           "traces_per_s": world * n_traces / dt, "chunk_bytes": 1 << 30,
+           "chunks": launches, "h2d_bytes": world * input_bytes,
+           "host_link_GBps_measured": link_gbs, "frac_of_host_link": val / world / link_gbs,
            "paper_array_rate_GBps": list(PAPER_RATE_GBS),
            "x_paper_max_rate": val / PAPER_RATE_GBS[1],
-           "pinned_alloc_s": t_alloc, "outputs": "stay on device (5.94 GB)"}
+           "pinned_alloc_s": t_alloc, "outputs": "stay on device (%.2f GB per rank)" % (16e-9 * n_traces)}
+    if world > 1:                              # the single-rank extras below are N = 1 diagnostics
+        del host, outs
+        rta.rta_shutdown()
+        return res
+
+    h = host.numpy().view(np.uint16)
+    if verify:
+        # every one of the 200 000 events against the oracle, on the pinned buffer's own bytes
+        # (chunk-sized slabs, all host cores): the full-size verification pass of SURVEY.md 8(d)
+        import oracle
+        cores = os.cpu_count() or 1
+        t0 = time.perf_counter()
+        ok, done = True, 0
+        for e0, k in event_slabs(n_events, ev_bytes):
+            want = oracle.extract_threads(h[e0:e0 + k], ped, gain, cfg.W, cores)
+            ok = ok and bits_equal(torch, outs, want, e0 * cfg.n_pixels, (e0 + k) * cfg.n_pixels)
+            done += k
+        tv = time.perf_counter() - t0
+        res["verified_events"] = done
+        res["all_outputs_bit_identical_to_oracle"] = ok
+        res["verify_seconds"] = tv
+        res["oracle_all_cores_GBps_incl_compare"] = input_bytes / tv / 1e9
+    # the same stream from PAGEABLE host memory (PAPER.md:133 is a page-locked-versus-not
+    # transfer test): the first 8 GiB of the buffer copied into ordinary memory
+    try:
+        n_pg = min(n_events, 8 * ((1 << 30) // ev_bytes))
+        pg = np.empty((n_pg, cfg.n_pixels, cfg.n_samples), np.int16)
+        pg[...] = host[:n_pg].numpy()
+        pg_outs = [torch.empty(n_pg * cfg.n_pixels, dtype=o.dtype, device="cuda") for o in outs]
+
+        def run_pg():
+            rta.rta_extract_stream(pg, n_pg, cfg.n_pixels, cfg.n_samples, d_ped, d_gain, cfg.W,
+                                   *pg_outs, chunk_bytes=1 << 30, stream=stream)
+        run_pg()
+        torch.cuda.synchronize()
+        same = all(bool((a == b[:a.numel()]).all()) for a, b in zip(pg_outs[:2], outs[:2]))
+        dtp, _ = timed(run_pg)
+        res["pageable"] = {"value": pg.nbytes / dtp / 1e9, "unit": UNIT, "seconds": dtp,
+                           "h2d_bytes": pg.nbytes, "events": n_pg,
+                           "frac_of_host_link": pg.nbytes / dtp / 1e9 / link_gbs,
+                           "source": "pageable numpy array (staged through library-owned pinned buffers)",
+                           "equals_pinned_result": same}
+        del pg, pg_outs
+    except Exception as ex:
+        res["pageable"] = {"error": repr(ex)}
     # NEXT-4: the same pinned buffer through rta_extract_image_stream: waveforms in at
     # link speed, 36 bytes of event parameters per event out (they stay on the device)
     try:
         cam = camera_on_device(cfg, torch, dl0gen)
-        n_pix = torch.empty(cfg.n_events, dtype=torch.int32, device="cuda")
-        par = torch.empty((cfg.n_events, 8), dtype=torch.float32, device="cuda")
+        n_pix = torch.empty(n_events, dtype=torch.int32, device="cuda")
+        par = torch.empty((n_events, 8), dtype=torch.float32, device="cuda")
 
         def run_img():
-            rta.rta_extract_image_stream(host, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped,
+            rta.rta_extract_image_stream(host, n_events, cfg.n_pixels, cfg.n_samples, d_ped,
                                          d_gain, cfg.W, *cam, n_pix, par, None,
                                          chunk_bytes=1 << 30, stream=stream)
         run_img()
         torch.cuda.synchronize()
-        # the first events again from the per-trace outputs of the uint16 leg above
-        n64, p64 = image_outputs(dl0gen.CONFIGS["C1"], torch)            # 64 events
-        rta.rta_image_moments(outs[2], outs[3], 64, cfg.n_pixels, *cam, n64, p64, None, stream=stream)
+        # every event again from the (verified) per-trace outputs of the uint16 leg above
+        n_all = torch.empty(n_events, dtype=torch.int32, device="cuda")
+        p_all = torch.empty((n_events, 8), dtype=torch.float32, device="cuda")
+        rta.rta_image_moments(outs[2], outs[3], n_events, cfg.n_pixels, *cam, n_all, p_all, None,
+                              stream=stream)
         torch.cuda.synchronize()
-        same_img = bool((n_pix[:64] == n64).all()) and bool(
-            (par[:64].view(torch.int32) == p64.view(torch.int32)).all())
-        times = []
-        for _ in range(2):
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            run_img()
-            torch.cuda.synchronize()
-            times.append(time.perf_counter() - t0)
-        dti = min(times)
+        same_img = bool((n_pix == n_all).all()) and bool(
+            (par.view(torch.int32) == p_all.view(torch.int32)).all())
+        dti, _ = timed(run_img)
         res["image"] = {
-            "value": cfg.input_bytes / dti / 1e9, "unit": UNIT, "seconds": dti,
+            "value": input_bytes / dti / 1e9, "unit": UNIT, "seconds": dti,
             "api": "rta_extract_image_stream (extraction + cleaning + moments in one kernel per chunk)",
-            "events_per_s": cfg.n_events / dti, "frac_of_host_link": cfg.input_bytes / dti / 1e9 / link_gbs,
-            "result_bytes": EVENT_OUT_BYTES * cfg.n_events,
+            "events_per_s": n_events / dti, "frac_of_host_link": input_bytes / dti / 1e9 / link_gbs,
+            "result_bytes": EVENT_OUT_BYTES * n_events,
             "mean_pixels_in_image": float(n_pix.float().mean()),
-            "first_64_events_equal_extract_then_moments": same_img}
-        del n_pix, par
+            "all_events_equal_extract_then_moments": same_img}
+        del n_pix, par, n_all, p_all
     except Exception as ex:
         res["image"] = {"error": repr(ex)}
     # NEXT-2: the same 200 000 events as a P12 stream (22.26 GB) in the same pinned
     # buffer, through rta_extract_stream_packed12 (chunks of 9644 events = 1.07 GB)
     try:
         ev_samples = cfg.n_pixels * cfg.n_samples
-        nb = dl0gen.packed12_nbytes(cfg.n_traces * cfg.n_samples)
+        nb = dl0gen.packed12_nbytes(n_traces * cfg.n_samples)
         hp = host.view(-1).view(torch.uint8)[:nb]
         stage = torch.empty((gen_ev, cfg.n_pixels, cfg.n_samples), dtype=torch.int16, device="cuda")
         stage_pk = torch.empty(gen_ev * ev_samples * 3 // 2, dtype=torch.uint8, device="cuda")
-        for e0 in range(0, cfg.n_events, gen_ev):
+        for e0 in range(0, n_events, gen_ev):
             dl0gen.events_cuda(cfg, stage.data_ptr(), e0, gen_ev, st)
             dl0gen.pack12_cuda(stage.data_ptr(), gen_ev * ev_samples, stage_pk.data_ptr(), st)
             b0 = e0 * ev_samples * 3 // 2
             hp[b0:b0 + stage_pk.numel()].copy_(stage_pk)
         torch.cuda.synchronize()
         del stage, stage_pk
-        want = [o[:64 * cfg.n_pixels].clone() for o in outs]     # uint16-path result, first events
+        want = [o.clone() for o in outs]          # the (verified) uint16-path result, every trace
         for o in outs:
             o.zero_()
 
         def run12():
-            rta.rta_extract_stream_packed12(hp, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped,
+            rta.rta_extract_stream_packed12(hp, n_events, cfg.n_pixels, cfg.n_samples, d_ped,
                                             d_gain, cfg.W, *outs, chunk_bytes=1 << 30, stream=stream)
         run12()
         torch.cuda.synchronize()
-        same = all(bool((o[:64 * cfg.n_pixels] == w).all()) for o, w in zip(outs, want))
-        times = []
+        same = all(bool((o.view(torch.int32) == w.view(torch.int32)).all()) for o, w in zip(outs, want))
+        del want
         before = rta.rta_launch_count()
-        for _ in range(2):
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            run12()
-            torch.cuda.synchronize()
-            times.append(time.perf_counter() - t0)
-        dt12 = min(times)
+        dt12, _ = timed(run12)
         res["packed12"] = {
-            "value": cfg.input_bytes / dt12 / 1e9, "unit": UNIT,
+            "value": input_bytes / dt12 / 1e9, "unit": UNIT,
             "meaning": "raw-waveform-equivalent GB/s (2 bytes per sample) of the same 200000 events",
             "seconds": dt12, "h2d_bytes": nb, "link_GBps": nb / dt12 / 1e9,
             "frac_of_host_link": nb / dt12 / 1e9 / link_gbs,
             "chunks": (rta.rta_launch_count() - before) // 2,
-            "chunk_events": rta.rta_chunk_events(cfg.n_events, cfg.n_pixels, cfg.n_samples, 1 << 30, 12),
-            "traces_per_s": cfg.n_traces / dt12, "x_paper_max_rate": cfg.input_bytes / dt12 / 1e9 / PAPER_RATE_GBS[1],
+            "chunk_events": rta.rta_chunk_events(n_events, cfg.n_pixels, cfg.n_samples, 1 << 30, 12),
+            "traces_per_s": n_traces / dt12, "x_paper_max_rate": input_bytes / dt12 / 1e9 / PAPER_RATE_GBS[1],
             "speedup_vs_uint16_feed": dt / dt12,
-            "first_64_events_equal_uint16_path": same}
+            "all_events_equal_uint16_path": same}
     except Exception as ex:  # the uint16 leg above stands on its own
         res["packed12"] = {"error": repr(ex)}
     del host, outs
@@ -723,39 +889,68 @@ def sustained_leg(torch, dl0gen, rta, link_gbs):
     return res
 
 
-def cpu_baseline_leg(cfg, keep, dl0gen):
-    """The oracle, as it stands, on this box's host cores, on the same bytes."""
+def cpu_baseline_leg(cfg, keep, dl0gen, torch):
+    """The oracle, as it stands, on this box's host cores, on the same bytes the
+    GPU extracted: all cores on `oracle_sample_events` events (the whole batch
+    for C2: the timing run doubles as the verification pass), one thread on an
+    eighth of that. Every event of the batch is then compared with the device
+    result (the events beyond the timed sample in untimed slabs)."""
     import numpy as np
     import oracle
     d_wf, _, _, outs, ped, gain = keep
     cores = os.cpu_count() or 1
-    # bounded sample: ~0.28 GB/s per thread -> about 5 s single-threaded
-    n_ev = min(cfg.n_events, max(64, int(1.4e9 // (cfg.n_pixels * cfg.n_samples * 2))))
+    ev_bytes = cfg.n_pixels * cfg.n_samples * 2
+    n_ev = oracle_sample_events(cfg)
     wf = d_wf[:n_ev].cpu().numpy().view(np.uint16)
     t0 = time.perf_counter()
-    r1 = oracle.extract(wf, ped, gain, cfg.W)
-    t1 = time.perf_counter() - t0
-    t0 = time.perf_counter()
-    oracle.extract_threads(wf, ped, gain, cfg.W, cores)
+    rn = oracle.extract_threads(wf, ped, gain, cfg.W, cores)
     tn = time.perf_counter() - t0
+    n1 = max(1, n_ev // 8)
+    t0 = time.perf_counter()
+    oracle.extract(wf[:n1], ped, gain, cfg.W)
+    t1 = time.perf_counter() - t0
     n = n_ev * cfg.n_pixels
-    ints_equal = bool((outs[0][:n].cpu().numpy() == r1[0]).all()
-                      and (outs[1][:n].cpu().numpy() == r1[1]).all())
-    floats_equal = bool((outs[2][:n].cpu().numpy() == r1[2]).all()
-                        and (outs[3][:n].cpu().numpy() == r1[3]).all())
-    return {"value": wf.nbytes / tn / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+    ints_equal = bits_equal(torch, outs[:2], rn[:2], 0, n)
+    floats_equal = bits_equal(torch, outs[2:], rn[2:], 0, n)
+    verified = n_ev
+    del wf, rn
+    for e0, k in event_slabs(cfg.n_events - n_ev, ev_bytes):      # the rest of the batch, untimed
+        e0 += n_ev
+        w = d_wf[e0:e0 + k].cpu().numpy().view(np.uint16)
+        r = oracle.extract_threads(w, ped, gain, cfg.W, cores)
+        lo, hi = e0 * cfg.n_pixels, (e0 + k) * cfg.n_pixels
+        ints_equal = ints_equal and bits_equal(torch, outs[:2], r[:2], lo, hi)
+        floats_equal = floats_equal and bits_equal(torch, outs[2:], r[2:], lo, hi)
+        verified += k
+    return {"value": n_ev * ev_bytes / tn / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": "first %d of %d events of %s (%.2f GB), same bytes as the GPU run"
-                      % (n_ev, cfg.n_events, cfg.name, wf.nbytes / 1e9),
-            "single_thread_value": wf.nbytes / t1 / 1e9,
-            "traces_per_s": n / tn, "single_thread_traces_per_s": n / t1,
-            "gpu_matches_oracle_on_sample": {"ints_bit_exact": ints_equal,
-                                             "floats_bit_exact": floats_equal}}
+                      % (n_ev, cfg.n_events, cfg.name, n_ev * ev_bytes / 1e9),
+            "seconds": tn,
+            "single_thread_value": n1 * ev_bytes / t1 / 1e9,
+            "single_thread_sample": "first %d events" % n1,
+            "traces_per_s": n / tn, "single_thread_traces_per_s": n1 * cfg.n_pixels / t1,
+            "verified_events": verified, "n_events": cfg.n_events,
+            "gpu_matches_oracle_on_every_event": {"ints_bit_exact": ints_equal,
+                                                  "floats_bit_exact": floats_equal}}
+
+
+def multi_rank_command(n_gpus, argv):
+    """The command `python bench.py --gpus N` re-executes itself as when no
+    torchrun environment is present (rendezvous on 127.0.0.1: the container's
+    hostname may not resolve)."""
+    return [sys.executable, "-m", "torch.distributed.run", "--standalone", "--nnodes=1",
+            "--nproc-per-node", str(int(n_gpus)), "--local-addr", "127.0.0.1",
+            os.path.join(ROOT, "bench.py")] + list(argv)
 
 
 def main():
     args = parse_args()
     if args.impl == "reference":
         return reference_arm(args)
+
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # plain `python bench.py --gpus N`: one rank per GPU under torchrun, same arguments
+        return subprocess.call(multi_rank_command(args.gpus, sys.argv[1:]))
 
     import torch
     import dl0gen
@@ -768,8 +963,10 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
     torch.cuda.set_device(local)
     dist = None
+    numa = None
     if world > 1:
         import torch.distributed as dist
+        numa = bind_to_gpu_numa_node(torch, local)      # before any pinned allocation
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     def barrier():
@@ -856,10 +1053,19 @@ def main():
             "algorithmic_bytes_per_launch": algo_bytes,
             "bytes_per_trace": bytes_per_trace,
             "avg_launch_ms": summ["ms_avg"],
-            "traffic": ncu_traffic(kname),
             "frac_of_nominal_8TBps": summ["frac_of_nominal_8TBps"],
         },
     }
+    traffic, t_commit, t_stale = ncu_traffic(kname)
+    out["roofline"]["traffic"] = traffic
+    out["roofline"]["traffic_commit"] = t_commit
+    out["roofline"]["traffic_source"] = (
+        "no capture" if t_commit is None else
+        "null: csrc changed since the ncu capture of that commit" if t_stale else
+        "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch, captured at that "
+        "commit with the same kernel sources (profiles/)")
+    if numa is not None:
+        out["config"]["host_affinity"] = numa
 
     if not args.no_extra:
         # host-fed leg on every rank (each GPU has its own host link); max over ranks
@@ -874,9 +1080,18 @@ def main():
             e2e["h2d_bytes_per_step"] *= world
             e2e["d2h_bytes_per_step"] *= world
         out["e2e"] = e2e
+        if world > 1 and not args.no_sustained:
+            # the host-fed number is the one that scales with the GPU count (one host link
+            # per GPU) until host memory bandwidth saturates: every rank feeds its own GPU
+            main_run["keep"] = keep = None
+            torch.cuda.empty_cache()
+            link = host_link_bandwidth(torch)
+            t = torch.tensor([link], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MIN)
+            out["sustained"] = sustained_leg(torch, dl0gen, rta, float(t.item()), world, rank, dist)
         if rank == 0 and world == 1:
             if not args.no_cpu:
-                out["cpu_baseline"] = cpu_baseline_leg(cfg, keep, dl0gen)
+                out["cpu_baseline"] = cpu_baseline_leg(cfg, keep, dl0gen, torch)
             main_run["keep"] = keep = None
             torch.cuda.empty_cache()
             others = {}

@@ -12,6 +12,7 @@ import pytest
 
 import dl0gen
 import oracle
+from tests._full import alloc_filled_outputs, bits_equal, first_mismatch, slabs, split_events
 from tests._gpu import alloc_outputs, assert_parity, bit_identical, to_dev_u16
 
 pytestmark = pytest.mark.gpu
@@ -173,9 +174,10 @@ def test_family_on_config_models(name, n_ev):
 
 
 @pytest.mark.parametrize("name", ["C2", "C4"])
-def test_family_full_size_sampled(name):
-    """BASELINE.json's full sizes in one launch per extractor; sampled event
-    blocks against the oracle on host-regenerated bytes."""
+def test_family_full_size_every_event(name):
+    """BASELINE.json's full sizes in one launch per extractor into sentinel-filled
+    outputs; EVERY event against the oracle on the same bytes (copied back in
+    ~1 GB slabs, all host cores)."""
     import torch
     import paper_1307_6489_b200 as rta
     c = dl0gen.CONFIGS[name]
@@ -186,10 +188,12 @@ def test_family_full_size_sampled(name):
     rng = np.random.default_rng(9)
     start = rng.integers(0, c.n_samples - c.W + 1, c.n_pixels).astype(np.int32)
     taps = np.array([1, 2, 3, 4, 3, 2, 1, 1][:c.W], np.int32)
-    blocks = [0, c.n_events - 8] + sorted(rng.integers(8, c.n_events - 16, 3).tolist())
-    for kind, kw in (("fixed", dict(W=c.W, window_start=start)),
-                     ("local_peak", dict(W=c.W, shift=2)), ("fir", dict(taps=taps))):
-        outs = alloc_outputs(c.n_traces)
+    kinds = (("fixed", dict(W=c.W, window_start=start)),
+             ("local_peak", dict(W=c.W, shift=2)), ("fir", dict(taps=taps)))
+    results = {}
+    for kind, kw in kinds:
+        outs = alloc_filled_outputs(c.n_traces)
+        before = rta.rta_launch_count()
         if kind == "fixed":
             rta.rta_extract_fixed(d_wf, c.n_events, c.n_pixels, c.n_samples, d_ped, d_gain, c.W,
                                   torch.from_numpy(start).cuda(), *outs)
@@ -199,11 +203,14 @@ def test_family_full_size_sampled(name):
         else:
             rta.rta_extract_fir(d_wf, c.n_events, c.n_pixels, c.n_samples, d_ped, d_gain, taps, *outs)
         torch.cuda.synchronize()
-        for e0 in blocks:
-            wf = dl0gen.events_cpu(c, e0, 8, threads=4)
-            want = want_family(kind, wf, ped, gain, **kw)
-            lo, hi = e0 * c.n_pixels, (e0 + 8) * c.n_pixels
-            got = tuple(o[lo:hi].cpu().numpy() for o in outs)
-            assert_parity(got, want, "%s %s events %d.." % (name, kind, e0))
-            assert bit_identical(got, want)
-        del outs
+        assert rta.rta_launch_count() == before + 1
+        results[kind] = outs
+    # one pass over the input slabs serves the three extractors
+    for e0, k in slabs(c.n_events, c.n_pixels * c.n_samples * 2):
+        wf = d_wf[e0:e0 + k].cpu().numpy().view(np.uint16)
+        lo, hi = e0 * c.n_pixels, (e0 + k) * c.n_pixels
+        for kind, kw in kinds:
+            want = split_events(k, lambda a, b: want_family(kind, wf[a:b], ped, gain, **kw))
+            got = tuple(o[lo:hi].cpu().numpy() for o in results[kind])
+            assert bits_equal(got, want), "%s %s events %d..%d: %s" % (
+                name, kind, e0, e0 + k, first_mismatch(got, want))

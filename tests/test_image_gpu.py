@@ -442,13 +442,17 @@ def test_stream_and_host_variants_match_the_device_call():
     rta.rta_shutdown()
 
 
-# ------------------------------------------------------ bench-sized, sampled events
+# ------------------------------------------------------ bench-sized, every event
 @pytest.mark.parametrize("name", ["C2", "C3", "C4"])
-def test_fused_at_full_size_sampled_events(name):
-    """BASELINE.json configs at full size, generated on the device; the oracle
-    checks event blocks regenerated on the host (same bytes: tests/test_dl0gen.py)."""
+def test_fused_and_two_call_route_at_full_size_every_event(name):
+    """BASELINE.json configs at full size, generated on the device, in the launch
+    configurations bench.py times: one rta_extract_image (no mask), and rta_extract
+    followed by rta_image_moments (with the mask). EVERY event of both is compared
+    with the oracle (extraction + cleaning + moments) run on the same bytes, copied
+    back in ~1 GB slabs, on all host cores."""
     import torch
     import paper_1307_6489_b200 as rta
+    from tests._full import alloc_filled_outputs, slabs, split_events
     cfg = dl0gen.CONFIGS[name]
     ped, gain = dl0gen.calib(cfg)
     x, y, nbr = dl0gen.hex_camera(cfg.n_pixels)
@@ -456,18 +460,28 @@ def test_fused_at_full_size_sampled_events(name):
     E, P, S = cfg.n_events, cfg.n_pixels, cfg.n_samples
     d_wf = torch.empty((E, P, S), dtype=torch.int16, device="cuda")
     dl0gen.events_cuda(cfg, d_wf.data_ptr(), 0, E, torch.cuda.current_stream().cuda_stream)
-    outs = image_outputs(E, P, mask=False)
+    cam = (dev(x), dev(y), dev(nbr), tp, tb)
+    d_ped, d_gain = dev(ped, np.int32), dev(gain, F32)
+    fused = image_outputs(E, P, mask=False)
     before = rta.rta_launch_count()
-    rta.rta_extract_image(d_wf, E, P, S, dev(ped, np.int32), dev(gain, F32), cfg.W, dev(x), dev(y),
-                          dev(nbr), tp, tb, *outs)
-    n, par, _ = host(outs)
+    rta.rta_extract_image(d_wf, E, P, S, d_ped, d_gain, cfg.W, *cam, *fused)
     assert rta.rta_launch_count() == before + 1
-    del d_wf
-    assert (n >= 0).all() and (n <= P).all() and np.isfinite(par).all()
-    assert ((par == 0).all(1) == (n == 0)).all()              # positive thresholds: empty <=> zero
-    nb = 6 if name != "C4" else 3
-    for first in [0, E - 8] + [int(v) for v in np.random.default_rng(1).integers(8, E - 16, nb)]:
-        wf = dl0gen.events_cpu(cfg, first, 8, threads=8)
-        want = oracle_extract_image(wf, ped, gain, cfg.W, x, y, nbr, tp, tb)
-        assert_image_parity((n[first:first + 8], par[first:first + 8], None), want, x, y,
-                            "%s events %d.." % (name, first))
+    per_trace = alloc_filled_outputs(E * P)
+    two = image_outputs(E, P, mask=True)
+    rta.rta_extract(d_wf, E, P, S, d_ped, d_gain, cfg.W, *per_trace)
+    rta.rta_image_moments(per_trace[2], per_trace[3], E, P, *cam, *two)
+    fn, fpar, _ = host(fused)
+    tn, tpar, tmask = host(two)
+    del per_trace, two, fused
+    assert ((fpar == 0).all(1) == (fn == 0)).all()            # positive thresholds: empty <=> zero
+    done = 0
+    for e0, k in slabs(E, P * S * 2):
+        wf = d_wf[e0:e0 + k].cpu().numpy().view(np.uint16)
+        want = split_events(k, lambda a, b: oracle_extract_image(wf[a:b], ped, gain, cfg.W, x, y,
+                                                                 nbr, tp, tb))
+        what = "%s events %d..%d" % (name, e0, e0 + k)
+        assert_image_parity((fn[e0:e0 + k], fpar[e0:e0 + k], None), want, x, y, what + " fused")
+        assert_image_parity((tn[e0:e0 + k], tpar[e0:e0 + k], tmask[e0:e0 + k]), want, x, y,
+                            what + " extract + moments")
+        done += k
+    assert done == E

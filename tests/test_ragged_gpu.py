@@ -182,36 +182,49 @@ def test_uniform_batch_through_the_ragged_path_equals_rta_extract():
     rta.rta_ragged_plan_destroy(plan)
 
 
-def test_bench_sized_mixed_array_sampled_against_oracle():
-    """The mixed array bench.py times (4 LST-, 10 MST-, 6 SST-like telescopes, every
-    event triggers all, blocks on 16-byte boundaries): generated on the GPU, one
-    rta_extract_ragged, sampled blocks against the oracle on host-regenerated bytes."""
+def test_bench_sized_mixed_array_every_block_against_oracle():
+    """The mixed array bench.py times (1000 events x (4 LST-, 10 MST-, 6 SST-like
+    telescopes), every event triggers all, blocks on 16-byte boundaries): generated
+    on the GPU, one rta_extract_ragged into sentinel-filled outputs, then EVERY block
+    against oracle.extract_ragged on the same bytes (copied back in slabs of whole
+    events, all host cores). A few blocks are also regenerated on the host."""
     import torch
     import dl0gen
     import paper_1307_6489_b200 as rta
-    m = dl0gen.MixedArray(n_events=400)
+    from tests._full import alloc_filled_outputs, bits_equal, first_mismatch, slabs, split_events
+    m = dl0gen.MixedArray(n_events=1000)
     ped, gain = m.calib()
     d_wf = torch.zeros(m.n_samples_total, dtype=torch.int16, device="cuda")
     m.fill_cuda(torch, d_wf)
-    outs = [torch.empty(m.n_traces, dtype=dt, device="cuda")
-            for dt in (torch.int32, torch.int32, torch.float32, torch.float32)]
+    outs = alloc_filled_outputs(m.n_traces)
     plan = rta.rta_ragged_plan_create(*m.tables())
     assert rta.rta_ragged_plan_info(plan, rta.RTA_RAGGED_N_LAUNCHES) == 3
     assert rta.rta_ragged_plan_info(plan, rta.RTA_RAGGED_WF_BYTES) == m.wf_bytes
     rta.rta_extract_ragged(plan, d_wf, torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda(), *outs)
     torch.cuda.synchronize()
     rta.rta_ragged_plan_destroy(plan)
+    n_slots, tpe, stride = len(m.slots), m.traces_per_event, m.event_stride
+
+    def oracle_events(wf, a, b):                       # events [a, b) of the slab `wf`
+        idx = range((b - a) * n_slots)
+        tel = [i % n_slots for i in idx]
+        wo = [(i // n_slots) * stride + m.slot_offset[i % n_slots] for i in idx]
+        oo = [(i // n_slots) * tpe + m.slot_out[i % n_slots] for i in idx]
+        return oracle.extract_ragged(wf[a * stride:b * stride], m.tel_n_pixels, m.tel_n_samples,
+                                     m.tel_W, m.tel_calib_offset, tel, wo, oo, ped, gain,
+                                     (b - a) * tpe)
+    done = 0
+    for e0, k in slabs(m.n_events, stride * 2):
+        wf = d_wf[e0 * stride:(e0 + k) * stride].cpu().numpy().view(np.uint16)
+        want = split_events(k, lambda a, b: oracle_events(wf, a, b))
+        got = tuple(o[e0 * tpe:(e0 + k) * tpe].cpu().numpy() for o in outs)
+        assert bits_equal(got, want), "events %d..%d: %s" % (e0, e0 + k, first_mismatch(got, want))
+        done += k
+    assert done == m.n_events
     rng = np.random.default_rng(8)
-    picks = [(0, 0), (m.n_events - 1, len(m.slots) - 1)] + [
-        (int(rng.integers(0, m.n_events)), int(rng.integers(0, len(m.slots)))) for _ in range(24)]
-    for e, j in picks:
+    for e, j in [(0, 0), (m.n_events - 1, n_slots - 1)] + [
+            (int(rng.integers(0, m.n_events)), int(rng.integers(0, n_slots))) for _ in range(6)]:
         blk = m.block_cpu(e, j)
-        P, S, W, c = m.tel_n_pixels[j], m.tel_n_samples[j], m.tel_W[j], m.tel_calib_offset[j]
-        w0 = e * m.event_stride + m.slot_offset[j]
+        P, S = m.tel_n_pixels[j], m.tel_n_samples[j]
+        w0 = e * stride + m.slot_offset[j]
         assert (d_wf[w0:w0 + P * S].cpu().numpy().view(np.uint16) == blk.ravel()).all()
-        want = oracle.extract(blk[None], ped[c:c + P], gain[c:c + P], W)
-        o0 = e * m.traces_per_event + m.slot_out[j]
-        got = tuple(o[o0:o0 + P].cpu().numpy() for o in outs)
-        assert_parity(got, want, "event %d slot %d" % (e, j))
-        assert bit_identical(got, want)
-    assert int(outs[1].min()) >= 0 and bool(torch.isfinite(outs[3]).all())
