@@ -114,9 +114,13 @@ def _declare(L: ctypes.CDLL, testing: bool) -> ctypes.CDLL:
 
 def _load(testing: bool) -> ctypes.CDLL:
     from . import build as _build
-    path = _build.build()
-    if testing:
-        path = _build.TEST_LIB
+    # RTA_LIBRARY: load a prebuilt library (a -DRTA_TESTING build serves both roles)
+    # instead of building in-tree
+    path = os.environ.get("RTA_LIBRARY")
+    if not path:
+        path = _build.build()
+        if testing:
+            path = _build.TEST_LIB
     if not os.path.exists(path):
         raise ImportError("%s is missing and could not be built" % path)
     return _declare(ctypes.CDLL(path), testing)

@@ -45,10 +45,10 @@
 #include <atomic>
 #include <mutex>
 
-// most warps per CTA of image_moments_kernel: 16 leaves the cleaning code its 128
-// registers (24 would spill)
+// most warps per CTA of image_moments_kernel (the launch bound caps the registers
+// per thread at 65536 / (32 warps))
 #ifndef RTA_MOM_WARPS
-#define RTA_MOM_WARPS 16
+#define RTA_MOM_WARPS 24
 #endif
 // how the fused kernels form the arg-max keys (compute_results KEYMUL): 1 = IMAD
 // with a constant-bank multiplier (fma pipe); these kernels are alu-pipe-bound
@@ -108,30 +108,39 @@ struct EventBuf {
   }
 };
 
-// Scratch owned by a cleaning warp: keep / mask bit words and one pixel list.
+// Scratch owned by a cleaning warp: keep / mask bit words and one pixel list of
+// `cap` entries (cap >= 384 = 32 lanes x 12 words, the most one lane's run of
+// words can hold for P <= 12288). A list longer than cap is produced and
+// consumed in rounds (compact_bits); sparse images need one round.
 struct CleanScratch {
   uint32_t* keep_w;
   uint32_t* mask_w;
-  uint16_t* list;  // [P], pixel indices (< 2^16: rta_image_pixel_limit)
-  static __host__ __device__ size_t bytes(int P) {
-    return 2u * r16(4u * mask_words(P)) + r16(2u * (size_t)P);
+  uint16_t* list;  // [cap], pixel indices (< 2^16: rta_image_pixel_limit)
+  int cap;
+  static __host__ __device__ size_t bytes(int P, int cap) {
+    return 2u * r16(4u * mask_words(P)) + r16(2u * (size_t)cap);
   }
-  __device__ __forceinline__ CleanScratch(uint8_t* base, const int P) {
+  __device__ __forceinline__ CleanScratch(uint8_t* base, const int P, const int cap_) : cap(cap_) {
     keep_w = reinterpret_cast<uint32_t*>(base);
     mask_w = reinterpret_cast<uint32_t*>(base + r16(4u * mask_words(P)));
     list = reinterpret_cast<uint16_t*>(base + 2u * r16(4u * mask_words(P)));
   }
 };
+constexpr int kListCapMin = 512;
 
-// Pixel indices of the set bits of word(w), w = 0 .. NW-1, in ascending order
-// into list[]; returns their number (same value in every lane). One warp: lane
-// l owns the K = ceil(NW / 32) consecutive words l K .. l K + K - 1, so one
-// prefix sum over the lanes' bit counts places every lane's run.
+// Pixel indices of the set bits of word(w), w = w_begin .. NW-1, in ascending
+// order into list[], at most `cap` of them; returns their number (same value in
+// every lane) and moves w_begin to the first word not covered (NW when done).
+// One warp: lane l owns the K = ceil(NW / 32) consecutive words from
+// w_begin + l K, so one prefix sum over the lanes' bit counts places every
+// lane's run; a round ends before the first lane whose run would pass `cap`
+// (cap >= 32 K, so every round covers at least lane 0's words).
 template <class F>
-__device__ __forceinline__ int compact_bits(const int NW, uint16_t* __restrict__ list, F word) {
+__device__ __forceinline__ int compact_bits(const int NW, int& w_begin, uint16_t* __restrict__ list,
+                                            const int cap, F word) {
   const int lane = threadIdx.x & 31;
   const int K = (NW + 31) >> 5;
-  const int w_lo = lane * K, w_hi = min(w_lo + K, NW);
+  const int w_lo = min(w_begin + lane * K, NW), w_hi = min(w_lo + K, NW);
   int c = 0;
   for (int w = w_lo; w < w_hi; ++w) c += __popc(word(w));
   int incl = c;
@@ -140,47 +149,66 @@ __device__ __forceinline__ int compact_bits(const int NW, uint16_t* __restrict__
     const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
     if (lane >= o) incl += v;
   }
-  int off = incl - c;
-  for (int w = w_lo; w < w_hi; ++w) {
-    uint32_t bits = word(w);
-    while (bits) {
-      const int b = __ffs((int)bits) - 1;
-      bits &= bits - 1u;
-      list[off++] = (uint16_t)(32 * w + b);
+  const uint32_t over = __ballot_sync(0xFFFFFFFFu, incl > cap);
+  const int n_lanes = over ? __ffs((int)over) - 1 : 32;  // lanes whose runs fit
+  if (lane < n_lanes) {
+    int off = incl - c;
+    for (int w = w_lo; w < w_hi; ++w) {
+      uint32_t bits = word(w);
+      while (bits) {
+        const int b = __ffs((int)bits) - 1;
+        bits &= bits - 1u;
+        list[off++] = (uint16_t)(32 * w + b);
+      }
     }
   }
-  const int total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+  const int total = __shfl_sync(0xFFFFFFFFu, incl, max(n_lanes, 1) - 1);
+  w_begin = min(w_begin + n_lanes * K, NW);
   __syncwarp();
-  return total;
+  return n_lanes ? total : 0;
 }
 
 __device__ __forceinline__ bool test_bit(const uint32_t* w, const int n) {
   return (w[n >> 5] >> (n & 31)) & 1u;
 }
 
-// nb8: the table is 8-byte aligned, so a 24-byte row is three 8-byte loads
-__device__ __forceinline__ void load_row(const int32_t* __restrict__ nbr, const bool nb8,
-                                         const int p, int (&nb)[6]) {
-  const int32_t* row = nbr + 6u * (size_t)p;
-  if (nb8) {
+// The neighbour table as the cleaning code reads it: the caller's int32 [P][6]
+// in global memory, or a copy as uint16 [P][6] in shared memory (0xFFFF = none;
+// 12 bytes per pixel) that the CTA makes when it starts and there is room.
+struct NbrTable {
+  const int32_t* g;    // global, as given
+  const uint16_t* s;   // shared copy, or nullptr
+  bool g8;             // g is 8-byte aligned: a 24-byte row is three 8-byte loads
+  __device__ __forceinline__ void row(const int p, int (&nb)[6]) const {
+    if (s != nullptr) {
+      const uint32_t* r = reinterpret_cast<const uint32_t*>(s + 6 * p);  // 12 p: word aligned
 #pragma unroll
-    for (int j = 0; j < 3; ++j) {
-      const int2 v = __ldg(reinterpret_cast<const int2*>(row) + j);
-      nb[2 * j] = v.x, nb[2 * j + 1] = v.y;
+      for (int j = 0; j < 3; ++j) {
+        const uint32_t v = r[j];
+        nb[2 * j] = (int)(v & 0xFFFFu), nb[2 * j + 1] = (int)(v >> 16);
+      }
+    } else {
+      const int32_t* r = g + 6u * (size_t)p;
+      if (g8) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+          const int2 v = __ldg(reinterpret_cast<const int2*>(r) + j);
+          nb[2 * j] = v.x, nb[2 * j + 1] = v.y;
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 6; ++j) nb[j] = __ldg(r + j);
+      }
     }
-  } else {
-#pragma unroll
-    for (int j = 0; j < 6; ++j) nb[j] = __ldg(row + j);
   }
-}
+};
 
 // For the n listed pixels: hit = some neighbour's bit is set in in_w; hits set
 // the pixel's bit in out_w. Two list entries per lane are in flight at once
 // (their neighbour rows are loaded before any is used). Returns "any hit" per lane.
 __device__ __forceinline__ int neighbour_pass(const int n, const uint16_t* __restrict__ list,
-                                              const int32_t* __restrict__ nbr, const bool nb8,
-                                              const int P, const uint32_t* in_w,
-                                              uint32_t* out_w) {
+                                              const NbrTable& nbr, const int P,
+                                              const uint32_t* in_w, uint32_t* out_w) {
   const int lane = threadIdx.x & 31;
   constexpr int U = 2;
   int any = 0;
@@ -193,7 +221,7 @@ __device__ __forceinline__ int neighbour_pass(const int n, const uint16_t* __res
     }
 #pragma unroll
     for (int u = 0; u < U; ++u)
-      if (p[u] >= 0) load_row(nbr, nb8, p[u], nb[u]);
+      if (p[u] >= 0) nbr.row(p[u], nb[u]);
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       if (p[u] >= 0) {
@@ -212,15 +240,29 @@ __device__ __forceinline__ int neighbour_pass(const int n, const uint16_t* __res
   return any;
 }
 
+// "q[n] >= thr_boundary" for the symmetric pass: from the bit mask the producer
+// of the event made, or straight from a charge row in shared memory (the
+// moments kernel, which then never builds that mask for a symmetric table).
+struct LowFromBits {
+  const uint32_t* low_w;
+  __device__ __forceinline__ bool operator()(const int n) const { return test_bit(low_w, n); }
+};
+struct LowFromRow {
+  const float* row;
+  float thr;
+  __device__ __forceinline__ bool operator()(const int n) const { return row[n] >= thr; }
+};
+
 // Symmetric neighbour table (p in nbr[n] whenever n in nbr[p]): "n has a kept
 // neighbour" is the same as "a kept pixel lists n", so one pass over the core
 // pixels does both steps of the cleaning. A core pixel with a core neighbour is
 // kept: its own bit goes into mask_w, and so does every neighbour that passes
 // the boundary threshold. Returns "any pixel kept" per lane.
+template <class Low>
 __device__ __forceinline__ int symmetric_pass(const int n, const uint16_t* __restrict__ list,
-                                              const int32_t* __restrict__ nbr, const bool nb8,
-                                              const int P, const uint32_t* core_w,
-                                              const uint32_t* low_w, uint32_t* mask_w) {
+                                              const NbrTable& nbr, const int P,
+                                              const uint32_t* core_w, const Low& low,
+                                              uint32_t* mask_w) {
   const int lane = threadIdx.x & 31;
   constexpr int U = 2;
   int any = 0;
@@ -233,7 +275,7 @@ __device__ __forceinline__ int symmetric_pass(const int n, const uint16_t* __res
     }
 #pragma unroll
     for (int u = 0; u < U; ++u)
-      if (p[u] >= 0) load_row(nbr, nb8, p[u], nb[u]);
+      if (p[u] >= 0) nbr.row(p[u], nb[u]);
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       if (p[u] >= 0) {
@@ -242,10 +284,10 @@ __device__ __forceinline__ int symmetric_pass(const int n, const uint16_t* __res
 #pragma unroll
         for (int j = 0; j < 6; ++j) {
           const bool ok = (unsigned)nb[u][j] < (unsigned)P;
-          const int w = ok ? (nb[u][j] >> 5) : 0;
-          const uint32_t bit = ok ? (1u << (nb[u][j] & 31)) : 0u;
-          if (core_w[w] & bit) hit = true;
-          lw[j] = low_w[w] & bit;
+          const int m = ok ? nb[u][j] : 0;
+          const uint32_t bit = ok ? (1u << (m & 31)) : 0u;
+          if (core_w[m >> 5] & bit) hit = true;
+          lw[j] = (ok && low(m)) ? bit : 0u;
         }
         if (hit) {
           atomicOr(&mask_w[p[u] >> 5], 1u << (p[u] & 31));
@@ -262,32 +304,64 @@ __device__ __forceinline__ int symmetric_pass(const int n, const uint16_t* __res
 }
 
 // Every thread of the CTA: is the neighbour table symmetric? One (pixel, slot)
-// entry per thread and step; the answer is the same in every thread. Contains
-// __syncthreads.
+// entry per thread and step, four steps' loads in flight at once; the answer
+// is the same in every thread. Contains __syncthreads.
 __device__ __forceinline__ int table_is_symmetric(const int32_t* __restrict__ nbr, const int P) {
   int ok = 1;
   const int n_entries = 6 * P;
-  for (int i = threadIdx.x; i < n_entries; i += blockDim.x) {
-    const int n = __ldg(nbr + i);
-    if ((unsigned)n < (unsigned)P) {
-      const int p = i / 6;
-      const int32_t* r = nbr + 6u * (size_t)n;
+  constexpr int U = 4;
+  for (int i0 = threadIdx.x; i0 < n_entries; i0 += U * blockDim.x) {
+    int n[U], r[U][6];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int i = i0 + u * blockDim.x;
+      n[u] = i < n_entries ? __ldg(nbr + i) : -1;
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int32_t* row = nbr + 6u * (size_t)((unsigned)n[u] < (unsigned)P ? n[u] : 0);
+#pragma unroll
+      for (int j = 0; j < 6; ++j) r[u][j] = __ldg(row + j);
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int p = (i0 + u * (int)blockDim.x) / 6;
       bool back = false;
 #pragma unroll
-      for (int j = 0; j < 6; ++j) back |= (__ldg(r + j) == p);
+      for (int j = 0; j < 6; ++j) back |= (r[u][j] == p);
+      if ((unsigned)n[u] < (unsigned)P && !back) ok = 0;
+    }
+  }
+  return __syncthreads_and(ok);
+}
+
+// The same on a uint16 copy of the table in shared memory (complete and visible
+// to the CTA; 0xFFFF = none). Contains __syncthreads.
+__device__ __forceinline__ int table_is_symmetric_s16(const uint16_t* nbr, const int P) {
+  int ok = 1;
+  const int n_entries = 6 * P;
+  for (int i = threadIdx.x; i < n_entries; i += blockDim.x) {
+    const int n = nbr[i];
+    if (n < P) {
+      const int p = i / 6;
+      const uint16_t* r = nbr + 6 * n;
+      bool back = false;
+#pragma unroll
+      for (int j = 0; j < 6; ++j) back |= ((int)r[j] == p);
       if (!back) ok = 0;
     }
   }
   return __syncthreads_and(ok);
 }
 
-// The sums of one event, parked in one lane until 32 events are finished together.
-struct Pending {
-  double s0, sx, sy, st, sxx, syy, sxy;  // about the origin (x0, y0)
+// The sums of one event (readings R33 / R34), about the origin (x0, y0).
+struct EventSums {
+  double s0, sx, sy, st, sxx, syy, sxy;
   float x0, y0, qm;
   int n_pix;
   uint32_t e;
 };
+using Pending = EventSums;  // parked in one lane until 32 events are finished together
 
 // One lane, one event: the scalar tail of readings R33 / R34.
 __device__ __forceinline__ void finish_event(const Pending& pd, const RtaImageOut& out) {
@@ -335,102 +409,109 @@ __device__ __forceinline__ double shfl_xor_f64(const double v, const int o) {
 }
 
 // Cleaning and moment sums of event e (readings R31-R35), executed by one whole
-// warp. core_w / low_w are in shared memory and complete; q and t point at the
-// event's charges and peak times (shared or global memory). The event's sums go
-// into lane n_pend's `pd`; after 32 events the warp finishes them together.
-__device__ __forceinline__ void clean_event(const uint32_t e, const int P, const float* q,
-                                            const float* t, const uint32_t* core_w,
-                                            const uint32_t* low_w, const CleanScratch& sc,
-                                            const RtaCamera& cam, const RtaImageOut& out,
-                                            const bool symmetric, Pending& pd, int& n_pend) {
+// warp; the sums come back in every lane. core_w (and low_w for the general
+// path) are in shared memory and complete; `low(n)` answers q[n] >= thr_boundary
+// for the symmetric pass; q and t point at the event's charges and peak times
+// (shared or global memory). `after_pass()` runs once the threshold tests are
+// over (the moments kernel hands its row buffer back to the copy engine there).
+template <class Low, class AfterPass>
+__device__ __forceinline__ void clean_event_sums(const uint32_t e, const int P, const float* q,
+                                                 const float* t, const uint32_t* core_w,
+                                                 const uint32_t* low_w, const Low& low,
+                                                 const CleanScratch& sc, const NbrTable& nbr,
+                                                 const RtaCamera& cam, const RtaImageOut& out,
+                                                 const bool symmetric, AfterPass after_pass,
+                                                 EventSums& cur) {
   const int lane = threadIdx.x & 31;
   const int NW = (int)mask_words(P);
-  const bool nb8 = (reinterpret_cast<uintptr_t>(cam.neighbors) & 7u) == 0;
   uint8_t* mrow = out.mask ? out.mask + (size_t)e * (size_t)P : nullptr;
 
-  Pending cur;
   cur.s0 = cur.sx = cur.sy = cur.st = cur.sxx = cur.syy = cur.sxy = 0.0;
   cur.x0 = cur.y0 = cur.qm = 0.0f;
   cur.n_pix = 0;
   cur.e = e;
 
-  const int n_core = compact_bits(NW, sc.list, [&](int w) { return core_w[w]; });
-  int kept;
+  int kept = 0;
   if (symmetric) {
     for (int w = lane; w < NW; w += 32) sc.mask_w[w] = 0u;
     __syncwarp();
-    kept = symmetric_pass(n_core, sc.list, cam.neighbors, nb8, P, core_w, low_w, sc.mask_w);
+    for (int wb = 0; wb < NW;) {
+      const int n_core = compact_bits(NW, wb, sc.list, sc.cap, [&](int w) { return core_w[w]; });
+      kept |= symmetric_pass(n_core, sc.list, nbr, P, core_w, low, sc.mask_w);
+    }
   } else {
     // keep[p] = core[p] and some neighbour is core (isolated core pixels drop)
     for (int w = lane; w < NW; w += 32) sc.keep_w[w] = 0u;
     __syncwarp();
-    kept = neighbour_pass(n_core, sc.list, cam.neighbors, nb8, P, core_w, sc.keep_w);
-  }
-  if (__any_sync(0xFFFFFFFFu, kept)) {
-    if (!symmetric) {
-      // mask[p] = keep[p] or (q[p] >= thr_boundary and some neighbour is kept)
-      for (int w = lane; w < NW; w += 32) sc.mask_w[w] = sc.keep_w[w];
-      const int n_cand =
-          compact_bits(NW, sc.list, [&](int w) { return low_w[w] & ~sc.keep_w[w]; });
-      neighbour_pass(n_cand, sc.list, cam.neighbors, nb8, P, sc.keep_w, sc.mask_w);
+    for (int wb = 0; wb < NW;) {
+      const int n_core = compact_bits(NW, wb, sc.list, sc.cap, [&](int w) { return core_w[w]; });
+      kept |= neighbour_pass(n_core, sc.list, nbr, P, core_w, sc.keep_w);
     }
+  }
+  kept = __any_sync(0xFFFFFFFFu, kept);
+  if (kept && !symmetric) {
+    // mask[p] = keep[p] or (q[p] >= thr_boundary and some neighbour is kept)
+    for (int w = lane; w < NW; w += 32) sc.mask_w[w] = sc.keep_w[w];
+    __syncwarp();
+    for (int wb = 0; wb < NW;) {
+      const int n_cand = compact_bits(NW, wb, sc.list, sc.cap,
+                                      [&](int w) { return low_w[w] & ~sc.keep_w[w]; });
+      neighbour_pass(n_cand, sc.list, nbr, P, sc.keep_w, sc.mask_w);
+    }
+  }
+  after_pass();
+  if (kept) {
     if (mrow)
       for (int p = lane; p < P; p += 32) mrow[p] = test_bit(sc.mask_w, p) ? 1 : 0;
 
-    // one pass over the mask pixels in ascending pixel order: lane i takes
-    // entries i, i + 32, ...; origin = the first mask pixel (lane 0's first entry)
-    const int n_pix = compact_bits(NW, sc.list, [&](int w) { return sc.mask_w[w]; });
-    float qm = -INFINITY;
-    float fx = 0.0f, fy = 0.0f, fq = 0.0f, ft = 0.0f;
-    if (lane < n_pix) {
-      const int p = sc.list[lane];
-      fq = q[p];
-      ft = t[p];
-      fx = __ldg(cam.pix_x + p);
-      fy = __ldg(cam.pix_y + p);
-      qm = fq;
-    }
-    const float x0 = __shfl_sync(0xFFFFFFFFu, fx, 0), y0 = __shfl_sync(0xFFFFFFFFu, fy, 0);
-    const double X0 = (double)x0, Y0 = (double)y0;
-    double s0, sx, sy, st, sxx, syy, sxy;
-    {
-      const double w = (double)fq;  // 0 for lanes past the list
-      const double dx = __dsub_rn((double)fx, X0), dy = __dsub_rn((double)fy, Y0);
-      const double wx = __dmul_rn(w, dx), wy = __dmul_rn(w, dy);
-      s0 = lane < n_pix ? w : 0.0;
-      sx = lane < n_pix ? wx : 0.0;
-      sy = lane < n_pix ? wy : 0.0;
-      st = lane < n_pix ? __dmul_rn(w, (double)ft) : 0.0;
-      sxx = lane < n_pix ? __dmul_rn(wx, dx) : 0.0;
-      syy = lane < n_pix ? __dmul_rn(wy, dy) : 0.0;
-      sxy = lane < n_pix ? __dmul_rn(wx, dy) : 0.0;
-    }
-    for (int i = lane + 32; i < n_pix; i += 32) {
-      const int p = sc.list[i];
-      const float qp = q[p];
-      const double w = (double)qp;
-      const double dx = __dsub_rn((double)__ldg(cam.pix_x + p), X0);
-      const double dy = __dsub_rn((double)__ldg(cam.pix_y + p), Y0);
-      const double wx = __dmul_rn(w, dx), wy = __dmul_rn(w, dy);
-      s0 = __dadd_rn(s0, w);
-      sx = __dadd_rn(sx, wx);
-      sy = __dadd_rn(sy, wy);
-      st = __fma_rn(w, (double)t[p], st);
-      sxx = __fma_rn(wx, dx, sxx);
-      syy = __fma_rn(wy, dy, syy);
-      sxy = __fma_rn(wx, dy, sxy);
-      qm = fmaxf(qm, qp);
+    // one pass over the mask pixels in ascending pixel order: in every round lane i
+    // takes entries i, i + 32, ...; origin = the first mask pixel
+    float qm = -INFINITY, x0 = 0.0f, y0 = 0.0f;
+    double X0 = 0.0, Y0 = 0.0;
+    double s0 = 0.0, sx = 0.0, sy = 0.0, st = 0.0, sxx = 0.0, syy = 0.0, sxy = 0.0;
+    int n_pix = 0;
+    for (int wb = 0; wb < NW;) {
+      const int n = compact_bits(NW, wb, sc.list, sc.cap, [&](int w) { return sc.mask_w[w]; });
+      // lane i's first entry of the round is entry i: its loads go out before anything
+      // waits, and lane 0's coordinates become the origin in the first non-empty round
+      int p = lane < n ? (int)sc.list[lane] : 0;
+      float qp = 0.0f, tp = 0.0f, xp = 0.0f, yp = 0.0f;
+      if (lane < n) qp = q[p], tp = t[p], xp = __ldg(cam.pix_x + p), yp = __ldg(cam.pix_y + p);
+      if (n_pix == 0 && n > 0) {
+        x0 = __shfl_sync(0xFFFFFFFFu, xp, 0), y0 = __shfl_sync(0xFFFFFFFFu, yp, 0);
+        X0 = (double)x0, Y0 = (double)y0;
+      }
+      n_pix += n;
+      for (int i = lane; i < n; i += 32) {
+        if (i != lane) {
+          p = sc.list[i];
+          qp = q[p], tp = t[p], xp = __ldg(cam.pix_x + p), yp = __ldg(cam.pix_y + p);
+        }
+        const double w = (double)qp;
+        const double dx = __dsub_rn((double)xp, X0);
+        const double dy = __dsub_rn((double)yp, Y0);
+        const double wx = __dmul_rn(w, dx), wy = __dmul_rn(w, dy);
+        s0 = __dadd_rn(s0, w);
+        sx = __dadd_rn(sx, wx);
+        sy = __dadd_rn(sy, wy);
+        sxx = __fma_rn(wx, dx, sxx);
+        syy = __fma_rn(wy, dy, syy);
+        sxy = __fma_rn(wx, dy, sxy);
+        qm = fmaxf(qm, qp);
+        st = __fma_rn(w, (double)tp, st);  // last: the peak time comes from furthest away
+      }
+      __syncwarp();  // the list is rewritten by the next round
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       s0 = __dadd_rn(s0, shfl_xor_f64(s0, o));
       sx = __dadd_rn(sx, shfl_xor_f64(sx, o));
       sy = __dadd_rn(sy, shfl_xor_f64(sy, o));
-      st = __dadd_rn(st, shfl_xor_f64(st, o));
       sxx = __dadd_rn(sxx, shfl_xor_f64(sxx, o));
       syy = __dadd_rn(syy, shfl_xor_f64(syy, o));
       sxy = __dadd_rn(sxy, shfl_xor_f64(sxy, o));
       qm = fmaxf(qm, __shfl_xor_sync(0xFFFFFFFFu, qm, o));
+      st = __dadd_rn(st, shfl_xor_f64(st, o));
     }
     cur.s0 = s0, cur.sx = sx, cur.sy = sy, cur.st = st;
     cur.sxx = sxx, cur.syy = syy, cur.sxy = sxy;
@@ -439,77 +520,235 @@ __device__ __forceinline__ void clean_event(const uint32_t e, const int P, const
   } else if (mrow) {  // no surviving core pixel: the mask is empty
     for (int p = lane; p < P; p += 32) mrow[p] = 0;
   }
-  if (lane == n_pend) pd = cur;
+}
+
+// The fused kernels' cleaning warps: threshold masks from the producer, the
+// neighbour table in global memory, sums parked in lane n_pend's `pd`; after 32
+// events the warp finishes them together.
+__device__ __forceinline__ void clean_event(const uint32_t e, const int P, const float* q,
+                                            const float* t, const uint32_t* core_w,
+                                            const uint32_t* low_w, const CleanScratch& sc,
+                                            const RtaCamera& cam, const RtaImageOut& out,
+                                            const bool symmetric, Pending& pd, int& n_pend) {
+  const NbrTable nbr{cam.neighbors, nullptr, (reinterpret_cast<uintptr_t>(cam.neighbors) & 7u) == 0};
+  EventSums cur;
+  clean_event_sums(e, P, q, t, core_w, low_w, LowFromBits{low_w}, sc, nbr, cam, out, symmetric,
+                   [] {}, cur);
+  if ((int)(threadIdx.x & 31) == n_pend) pd = cur;
   if (++n_pend == 32) flush_pending(pd, n_pend, out);
 }
 
 // ------------------------------------------------ cleaning on HBM arrays ----
-// One warp per event. The warp sweeps the charge row once with coalesced loads
-// (lane = pixel mod 32, so a ballot is a word of the bit mask) and then cleans
-// with charge / peak time of the few mask pixels gathered from L2. Shared
-// memory per warp: two threshold bit masks and the cleaning scratch only.
-size_t moments_warp_bytes(int32_t P) { return 2u * r16(4u * mask_words(P)) + CleanScratch::bytes(P); }
+// One warp per event, one persistent CTA per SM, as many warps as shared memory
+// holds (about 20 for an 1800-pixel camera).
+//  * Every warp owns a row buffer that ONE bulk copy (TMA, mbarrier complete_tx)
+//    fills with the charge row of the warp's next event while the warp is still
+//    cleaning the current one: the row loads of all warps are always in flight
+//    and no warp spends issue slots or a DRAM latency on them. Rows start at any
+//    multiple of 4 bytes: the copy starts at the 16-byte boundary below the row
+//    (the row lands `mis` bytes into the buffer) and stops at the last boundary
+//    inside the array; the final < 16 bytes of the array are read with plain loads.
+//  * The sweep builds ONE bit mask (q >= thr_picture; lane = pixel mod 32, so a
+//    ballot is a word). With a symmetric neighbour table the boundary threshold
+//    is only ever asked of the neighbours of kept pixels, which the symmetric
+//    pass reads straight from the row buffer; the buffer goes back to the copy
+//    engine right after that pass.
+//  * The CTA copies the neighbour table into shared memory as uint16 (12 bytes
+//    per pixel) when there is room: the table look-up is the one dependent load
+//    in front of every bit test.
+//  * The scalar tail (divisions, square roots, atan2: about 400 dependent
+//    instructions) is never run per event: a warp pushes the event's sums into a
+//    CTA-wide queue in shared memory, and whichever warp completes a batch of 32
+//    records finishes them, one event per lane; the last partial batch is
+//    finished after a __syncthreads. No cleaning warp keeps parked sums in
+//    registers.
+constexpr int kQueueBatches = 4;   // batch slots of 32 records
+struct FinishQueue {
+  uint32_t head;                     // records claimed so far
+  uint32_t written[kQueueBatches];   // records completely written, per slot
+  uint32_t freed[kQueueBatches];     // batches read out of the slot so far
+  uint32_t pad[7];
+  float4 rec[kQueueBatches * 32][5];  // 80 bytes per record
+};
+static_assert(sizeof(FinishQueue) % 16 == 0, "the per-warp buffers behind it stay 16-byte aligned");
 
-template <int WARPS>
+// lanes < n: read record `first + lane` and run the scalar tail for it
+__device__ __forceinline__ void queue_finish(FinishQueue& Q, const uint32_t slot, const int n,
+                                             const RtaImageOut& out) {
+  const int lane = threadIdx.x & 31;
+  Pending pd;
+  if (lane < n) {
+    const float4* r = Q.rec[slot * 32u + (uint32_t)lane];
+    const float4 a = r[0], b = r[1], c = r[2], d = r[3], f = r[4];
+    pd.s0 = __hiloint2double(__float_as_int(a.y), __float_as_int(a.x));
+    pd.sx = __hiloint2double(__float_as_int(a.w), __float_as_int(a.z));
+    pd.sy = __hiloint2double(__float_as_int(b.y), __float_as_int(b.x));
+    pd.st = __hiloint2double(__float_as_int(b.w), __float_as_int(b.z));
+    pd.sxx = __hiloint2double(__float_as_int(c.y), __float_as_int(c.x));
+    pd.syy = __hiloint2double(__float_as_int(c.w), __float_as_int(c.z));
+    pd.sxy = __hiloint2double(__float_as_int(d.y), __float_as_int(d.x));
+    pd.x0 = d.z, pd.y0 = d.w, pd.qm = f.x;
+    pd.n_pix = __float_as_int(f.y);
+    pd.e = (uint32_t)__float_as_int(f.z);
+  }
+  __syncwarp();
+  if (lane == 0) {  // the slot may be refilled
+    __threadfence_block();
+    Q.written[slot] = 0u;
+    atomicAdd(&Q.freed[slot], 1u);
+  }
+  if (lane < n) finish_event(pd, out);
+  __syncwarp();
+}
+
+// whole warp; `cur` holds the same sums in every lane
+__device__ __forceinline__ void queue_push(FinishQueue& Q, const EventSums& cur,
+                                           const RtaImageOut& out) {
+  const int lane = threadIdx.x & 31;
+  uint32_t done = 0, slot = 0;
+  if (lane == 0) {
+    const uint32_t idx = atomicAdd(&Q.head, 1u);
+    const uint32_t batch = idx >> 5;
+    slot = batch % kQueueBatches;
+    // the batch that used this slot before must have been read out (it almost always has)
+    while (*reinterpret_cast<volatile uint32_t*>(&Q.freed[slot]) < batch / kQueueBatches) __nanosleep(64);
+    __threadfence_block();
+    float4* r = Q.rec[slot * 32u + (idx & 31u)];
+    const auto lo = [](double v) { return __int_as_float(__double2loint(v)); };
+    const auto hi = [](double v) { return __int_as_float(__double2hiint(v)); };
+    r[0] = make_float4(lo(cur.s0), hi(cur.s0), lo(cur.sx), hi(cur.sx));
+    r[1] = make_float4(lo(cur.sy), hi(cur.sy), lo(cur.st), hi(cur.st));
+    r[2] = make_float4(lo(cur.sxx), hi(cur.sxx), lo(cur.syy), hi(cur.syy));
+    r[3] = make_float4(lo(cur.sxy), hi(cur.sxy), cur.x0, cur.y0);
+    r[4] = make_float4(cur.qm, __int_as_float(cur.n_pix), __int_as_float((int)cur.e), 0.0f);
+    __threadfence_block();
+    done = atomicAdd(&Q.written[slot], 1u) + 1u;
+  }
+  done = __shfl_sync(0xFFFFFFFFu, done, 0);
+  if (done == 32u) {
+    slot = __shfl_sync(0xFFFFFFFFu, slot, 0);
+    __threadfence_block();
+    queue_finish(Q, slot, 32, out);
+  }
+}
+
+size_t moments_row_bytes(int32_t P) { return r16(4u * (size_t)P) + 32u; }
+size_t moments_warp_bytes(int32_t P) {
+  return moments_row_bytes(P) + 2u * r16(4u * mask_words(P)) + CleanScratch::bytes(P, kListCapMin);
+}
+size_t moments_table_bytes(int32_t P) { return r16(12u * (size_t)P); }
+
+template <int WARPS, bool S16>
 __global__ void __launch_bounds__(32 * WARPS, 1)
     image_moments_kernel(const float* __restrict__ charge, const float* __restrict__ time,
                          const uint32_t n_events, const int P,
                          const __grid_constant__ RtaCamera cam,
                          const __grid_constant__ RtaImageOut out, const int force_general) {
   extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t row_bar[WARPS];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  FinishQueue& Q = *reinterpret_cast<FinishQueue*>(smem);
+  uint16_t* nbr16 = reinterpret_cast<uint16_t*>(smem + sizeof(FinishQueue));
   const size_t wb = r16(4u * mask_words(P));
-  uint8_t* mine = smem + (size_t)warp * (2u * wb + CleanScratch::bytes(P));
-  uint32_t* core_w = reinterpret_cast<uint32_t*>(mine);
-  uint32_t* low_w = reinterpret_cast<uint32_t*>(mine + wb);
-  const CleanScratch sc(mine + 2u * wb, P);
-  const bool symmetric = table_is_symmetric(cam.neighbors, P) && !force_general;
-  const float thr_p = cam.thr_picture, thr_b = cam.thr_boundary;
-  const uint32_t stride = gridDim.x * WARPS;
-  Pending pd = {};
-  int n_pend = 0;
-  for (uint32_t e = blockIdx.x * WARPS + warp; e < n_events; e += stride) {
-    const float* q = charge + (size_t)e * (size_t)P;
-    constexpr int U = 16;  // loads in flight per lane: the sweep is one DRAM latency per 512 pixels
-    int p0 = 0;
-    // whole blocks of 32 U pixels: no bounds checks; lane u keeps word u of the
-    // block and lanes 0 .. U-1 store the block's words with one instruction each
-    for (; p0 + 32 * U <= P; p0 += 32 * U) {
-      float v[U];
-#pragma unroll
-      for (int u = 0; u < U; ++u) v[u] = __ldg(q + p0 + 32 * u + lane);
-      uint32_t mc = 0, ml = 0;
-#pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const uint32_t c = __ballot_sync(0xFFFFFFFFu, v[u] >= thr_p);
-        const uint32_t l = __ballot_sync(0xFFFFFFFFu, v[u] >= thr_b);
-        if (lane == u) mc = c, ml = l;
-      }
-      if (lane < U) core_w[(p0 >> 5) + lane] = mc, low_w[(p0 >> 5) + lane] = ml;
-    }
-    if (p0 < P) {  // the last < 32 U pixels: the same block with bounds checks (loads still batched)
-      float v[U];
-#pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const int p = p0 + 32 * u + lane;
-        v[u] = p < P ? __ldg(q + p) : 0.0f;
-      }
-      uint32_t mc = 0, ml = 0;
-#pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const bool in = p0 + 32 * u + lane < P;
-        const uint32_t c = __ballot_sync(0xFFFFFFFFu, in && v[u] >= thr_p);
-        const uint32_t l = __ballot_sync(0xFFFFFFFFu, in && v[u] >= thr_b);
-        if (lane == u) mc = c, ml = l;
-      }
-      if (lane < U && p0 + 32 * lane < P) core_w[(p0 >> 5) + lane] = mc, low_w[(p0 >> 5) + lane] = ml;
-    }
-    __syncwarp();
-    clean_event(e, P, q, time + (size_t)e * (size_t)P, core_w, low_w, sc, cam, out, symmetric, pd,
-                n_pend);
-    __syncwarp();
+  const size_t rb = r16(4u * (size_t)P) + 32u;
+  const size_t per_warp = rb + 2u * wb + CleanScratch::bytes(P, kListCapMin);
+  uint8_t* mine = smem + sizeof(FinishQueue) + (S16 ? r16(12u * (size_t)P) : 0u) + (size_t)warp * per_warp;
+  uint32_t* core_w = reinterpret_cast<uint32_t*>(mine + rb);
+  uint32_t* low_w = reinterpret_cast<uint32_t*>(mine + rb + wb);
+  const CleanScratch sc(mine + rb + 2u * wb, P, kListCapMin);
+  const uint32_t bar = smem_u32(&row_bar[warp]);
+  const uint32_t row_s = smem_u32(mine);
+  if (threadIdx.x < (sizeof(FinishQueue) - sizeof(Q.rec)) / 4u)
+    reinterpret_cast<uint32_t*>(smem)[threadIdx.x] = 0u;  // head, written[], freed[]
+  if (lane == 0) {
+    mbar_init(bar, 1);
+    fence_mbar_init();
   }
-  flush_pending(pd, n_pend, out);
+  __syncwarp();
+
+  const uintptr_t base = reinterpret_cast<uintptr_t>(charge);
+  const uintptr_t end_all = base + (uintptr_t)n_events * (uintptr_t)P * 4u;
+  const uint32_t row_bytes = 4u * (uint32_t)P;
+  // lane 0: start the copy of event e's row into this warp's buffer
+  const auto issue = [&](const uint32_t e) {
+    const uintptr_t a = base + (uintptr_t)e * row_bytes;
+    const uint32_t mis = (uint32_t)(a & 15u);
+    const uintptr_t lo = a - mis;
+    uint32_t len = (mis + row_bytes + 15u) & ~15u;
+    if (lo + len > end_all) {  // the last row of the array: whole 16-byte lines, then words
+      len = (uint32_t)((end_all - lo) & ~(uintptr_t)15u);
+      for (uint32_t b = len; b < mis + row_bytes; b += 4u)
+        *reinterpret_cast<float*>(mine + b) = *reinterpret_cast<const float*>(lo + b);
+    }
+    mbar_expect_tx(bar, len);
+    if (len != 0) tma_bulk_g2s(row_s, reinterpret_cast<const void*>(lo), len, bar);
+  };
+
+  const uint32_t stride = gridDim.x * WARPS;
+  uint32_t e = blockIdx.x * WARPS + warp;
+  if (lane == 0 && e < n_events) issue(e);
+  // the table copy and check overlap the first loads
+  bool symmetric;
+  if constexpr (S16) {
+    for (int i = threadIdx.x; i < 6 * P; i += 32 * WARPS) {
+      const int n = __ldg(cam.neighbors + i);
+      nbr16[i] = (unsigned)n < (unsigned)P ? (uint16_t)n : (uint16_t)0xFFFFu;
+    }
+    __syncthreads();
+    symmetric = table_is_symmetric_s16(nbr16, P) && !force_general;
+  } else {
+    symmetric = table_is_symmetric(cam.neighbors, P) && !force_general;  // contains __syncthreads
+  }
+  const NbrTable nbr{cam.neighbors, S16 ? nbr16 : nullptr,
+                     (reinterpret_cast<uintptr_t>(cam.neighbors) & 7u) == 0};
+  const float thr_p = cam.thr_picture, thr_b = cam.thr_boundary;
+  const int NW = (int)mask_words(P), NWF = P >> 5;  // words, full words
+  for (uint32_t k = 0; e < n_events; e += stride, ++k) {
+    const uint32_t mis = (uint32_t)((base + (uintptr_t)e * row_bytes) & 15u);
+    const float* row = reinterpret_cast<const float*>(mine + mis);
+    mbar_wait(bar, k & 1u);
+    // sweep: word w of a mask = ballot over pixels 32 w .. 32 w + 31; four words per
+    // step (loads first), lane 0 stores them with one 16-byte store
+    const auto sweep = [&](const float thr, uint32_t* words) {
+      int w = 0;
+#pragma unroll 2
+      for (; w + 4 <= NWF; w += 4) {
+        float v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = row[32 * (w + u) + lane];
+        uint4 m;
+        m.x = __ballot_sync(0xFFFFFFFFu, v[0] >= thr);
+        m.y = __ballot_sync(0xFFFFFFFFu, v[1] >= thr);
+        m.z = __ballot_sync(0xFFFFFFFFu, v[2] >= thr);
+        m.w = __ballot_sync(0xFFFFFFFFu, v[3] >= thr);
+        if (lane == 0) *reinterpret_cast<uint4*>(words + w) = m;
+      }
+      for (; w < NW; ++w) {  // the last words; the very last may be partial
+        const int p = 32 * w + lane;
+        const float v = p < P ? row[p] : 0.0f;
+        const uint32_t m = __ballot_sync(0xFFFFFFFFu, p < P && v >= thr);
+        if (lane == 0) words[w] = m;
+      }
+    };
+    sweep(thr_p, core_w);
+    if (!symmetric) sweep(thr_b, low_w);  // the general path asks for every boundary candidate
+    __syncwarp();
+    EventSums cur;
+    clean_event_sums(
+        e, P, charge + (size_t)e * (size_t)P, time + (size_t)e * (size_t)P, core_w, low_w,
+        LowFromRow{row, thr_b}, sc, nbr, cam, out, symmetric,
+        [&] {  // every lane is done with the row: the buffer goes back to the copy engine
+          __syncwarp();
+          if (lane == 0 && e + stride < n_events) issue(e + stride);
+        },
+        cur);
+    queue_push(Q, cur, out);
+  }
+  __syncthreads();
+  if (warp == 0) {  // the last, partial batch
+    const uint32_t total = *reinterpret_cast<volatile uint32_t*>(&Q.head);
+    if (total & 31u) queue_finish(Q, (total >> 5) % kQueueBatches, (int)(total & 31u), out);
+  }
 }
 
 // ------------------------------------------------- producer / cleaner hand-off ----
@@ -532,7 +771,7 @@ __device__ __forceinline__ void cleaner_loop(const int P, uint8_t* ev_base, uint
                                              volatile FusedShared& fs, const RtaCamera& cam,
                                              const RtaImageOut& out, const bool symmetric) {
   const size_t eb = EventBuf::bytes(P);
-  const CleanScratch sc(sc_base, P);
+  const CleanScratch sc(sc_base, P, P);
   Pending pd = {};
   int n_pend = 0;
   for (uint32_t k = 0;; ++k) {
@@ -672,7 +911,7 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
     const bool symmetric = table_is_symmetric(cam.neighbors, P) && !force_general;
     const int c = (tid - NX) >> 5;
     if (c >= NC) return;
-    const CleanScratch sc(ev_base + (size_t)NB * eb + (size_t)c * CleanScratch::bytes(P), P);
+    const CleanScratch sc(ev_base + (size_t)NB * eb + (size_t)c * CleanScratch::bytes(P, P), P, P);
     Pending pd = {};
     int n_pend = 0;
     for (uint32_t k = (uint32_t)c; event_of(k) < n_events; k += (uint32_t)NC) {
@@ -898,7 +1137,7 @@ template <class I>
 int fused_cleaners(int32_t P) {
   for (int nc = I::NCMAX; nc >= 1; --nc) {
     const size_t need = I::RING + (size_t)(nc + 1) * EventBuf::bytes(P) +
-                        (size_t)nc * CleanScratch::bytes(P) + 1024u;
+                        (size_t)nc * CleanScratch::bytes(P, P) + 1024u;
     if (need <= kSmemLimit) return nc;
   }
   return 0;
@@ -928,7 +1167,7 @@ struct FusedLauncher {
     if ((e = rta_device_sms(dev, &sms)) != cudaSuccess) return e;
     const int nc = fused_cleaners<I>(P);
     int nb = nc + 1;
-    size_t smem = I::RING + (size_t)nb * EventBuf::bytes(P) + (size_t)nc * CleanScratch::bytes(P);
+    size_t smem = I::RING + (size_t)nb * EventBuf::bytes(P) + (size_t)nc * CleanScratch::bytes(P, P);
     // one more buffer when there is room: the extraction groups run further ahead
     if (nb + 1 <= kMaxBuf && smem + EventBuf::bytes(P) + 1024u <= kSmemLimit) {
       ++nb;
@@ -955,21 +1194,22 @@ struct FusedLauncher {
   }
 };
 
-template <int WARPS>
+template <int WARPS, bool S16>
 cudaError_t launch_moments(const float* charge, const float* time, uint32_t n_events, int32_t P,
                            const RtaCamera& cam, const RtaImageOut& out, cudaStream_t stream) {
   int dev = 0, sms = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if ((e = rta_device_sms(dev, &sms)) != cudaSuccess) return e;
-  const size_t smem = WARPS * moments_warp_bytes(P);
-  if ((e = rta_func_allow_max_smem((const void*)image_moments_kernel<WARPS>, dev)) != cudaSuccess)
-    return e;
+  const size_t smem = sizeof(FinishQueue) + (S16 ? moments_table_bytes(P) : 0u) +
+                      WARPS * moments_warp_bytes(P);
+  auto kernel = image_moments_kernel<WARPS, S16>;
+  if ((e = rta_func_allow_max_smem((const void*)kernel, dev)) != cudaSuccess) return e;
   uint32_t grid = (uint32_t)sms;  // one CTA per SM (launch bounds)
   const uint32_t need = (n_events + WARPS - 1u) / WARPS;
   if (grid > need) grid = need;
-  image_moments_kernel<WARPS><<<grid, 32 * WARPS, smem, stream>>>(
-      charge, time, n_events, P, cam, out, g_general_cleaning.load() ? 1 : 0);
+  kernel<<<grid, 32 * WARPS, smem, stream>>>(charge, time, n_events, P, cam, out,
+                                             g_general_cleaning.load() ? 1 : 0);
   rta_count_launch();
   return cudaGetLastError();
 }
@@ -1044,16 +1284,27 @@ cudaError_t rta_launch_image_moments(const float* charge, const float* time, int
                                      int32_t n_pixels, const RtaCamera& cam,
                                      const RtaImageOut& out, cudaStream_t stream) {
   if (n_events <= 0) return cudaSuccess;
-  // as many warps as one CTA's shared memory holds, up to RTA_MOM_WARPS
+  // As many warps as one CTA's shared memory holds (row buffer + masks + scratch
+  // per warp, behind the finish queue). The uint16 copy of the neighbour table
+  // goes in front when at least 12 warps still fit behind it.
   const size_t per_warp = moments_warp_bytes(n_pixels);
-  const size_t room = kSmemLimit - 2048u;
+  const size_t room = kSmemLimit - 1024u - sizeof(FinishQueue);
+  const size_t table = moments_table_bytes(n_pixels);
   const uint32_t E = (uint32_t)n_events;
-#if RTA_MOM_WARPS >= 24
-  if (24u * per_warp <= room) return launch_moments<24>(charge, time, E, n_pixels, cam, out, stream);
-#endif
-  if (16u * per_warp <= room) return launch_moments<16>(charge, time, E, n_pixels, cam, out, stream);
-  if (8u * per_warp <= room) return launch_moments<8>(charge, time, E, n_pixels, cam, out, stream);
-  return launch_moments<4>(charge, time, E, n_pixels, cam, out, stream);
+  if (table + 12u * per_warp <= room) {
+#define RTA_TRY(W) \
+  if (W <= RTA_MOM_WARPS && table + (size_t)W * per_warp <= room) \
+    return launch_moments<W, true>(charge, time, E, n_pixels, cam, out, stream);
+    RTA_TRY(24) RTA_TRY(22) RTA_TRY(20) RTA_TRY(18) RTA_TRY(16)
+    return launch_moments<12, true>(charge, time, E, n_pixels, cam, out, stream);
+#undef RTA_TRY
+  }
+#define RTA_TRY(W) \
+  if (W <= RTA_MOM_WARPS && (size_t)W * per_warp <= room) \
+    return launch_moments<W, false>(charge, time, E, n_pixels, cam, out, stream);
+  RTA_TRY(24) RTA_TRY(20) RTA_TRY(16) RTA_TRY(12) RTA_TRY(8) RTA_TRY(4) RTA_TRY(2)
+#undef RTA_TRY
+  return launch_moments<1, false>(charge, time, E, n_pixels, cam, out, stream);
 }
 
 cudaError_t rta_launch_extract_image(const void* wf, int64_t n_events, int32_t n_pixels,
@@ -1097,7 +1348,7 @@ cudaError_t rta_launch_extract_image(const void* wf, int64_t n_events, int32_t n
       cudaGetLastError();
     }
   }
-  const size_t smem = 2u * EventBuf::bytes(n_pixels) + CleanScratch::bytes(n_pixels);
+  const size_t smem = 2u * EventBuf::bytes(n_pixels) + CleanScratch::bytes(n_pixels, n_pixels);
   if (smem + 1024u > kSmemLimit) return cudaErrorInvalidValue;
   int dev = 0, sms = 0;
   cudaError_t e = cudaGetDevice(&dev);
