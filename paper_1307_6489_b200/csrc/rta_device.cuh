@@ -132,6 +132,29 @@ __device__ __forceinline__ Result finish_trace(const int W, const int rawsum, co
   return r;
 }
 
+// Steps a5-a6 only (all-ones window): sum and charge as finish_trace forms them;
+// `time` carries the bits of t* for a later finish_trace on the same trace.
+__device__ __forceinline__ Result finish_charge(const int W, const int rawsum, const int tstar,
+                                                const int ped, const float gain) {
+  Result r;
+  r.start = tstar;
+  r.time = __int_as_float(tstar);
+  constexpr int lim = 1 << 24;
+  if ((unsigned)ped <= 65535u) {
+    const int sum = rawsum - W * ped;
+    r.sum = sum;
+    r.charge = ((unsigned)(sum + (lim - 1)) < (unsigned)(2 * lim - 1))
+                   ? __fmul_rn((float)sum, gain)
+                   : (float)((double)sum * (double)gain);
+    return r;
+  }
+  const long long sum64 = (long long)rawsum - (long long)W * (long long)ped;
+  r.sum = (int)sum64;
+  r.charge = (sum64 > -lim && sum64 < lim) ? __fmul_rn((float)(int)sum64, gain)
+                                           : (float)((double)sum64 * (double)gain);
+  return r;
+}
+
 // ---- the extractor family (readings R22-R24): how t* is chosen ----
 enum : int { MODE_SLIDING = 0, MODE_FIXED = 1, MODE_LOCAL_PEAK = 2, MODE_FIR = 3 };
 
@@ -286,7 +309,10 @@ struct WindowReader {
 // (a uniform batch runs through the camera again; n_pixels = 0 never wraps).
 // KEYMUL != 0: `ma` comes from the launch (constant bank) and carries key_mul /
 // one / minus_one, which lets part of the integer work run on the fma pipe.
-template <class C, int MODE, int KEYMUL = 0>
+// WANT_TIME = false (sliding extractor only): step a7 is left out. res[].time then
+// holds the BITS of t* (the caller recomputes the peak time where it is needed:
+// the fused image kernel, for the few pixels that survive the cleaning).
+template <class C, int MODE, int KEYMUL = 0, bool WANT_TIME = true>
 __device__ __forceinline__ void compute_results(const uint8_t* __restrict__ unit,
                                                 const uint32_t p0, const uint32_t n_pixels,
                                                 const int* __restrict__ pedestal,
@@ -356,10 +382,12 @@ __device__ __forceinline__ void compute_results(const uint8_t* __restrict__ unit
       }
       tstar = (int)(C::KM - (best & C::KM));
       rawsum = (int)(best >> C::KB);
-      // a7 numerator: re-read the winning window (dynamic index -> shared memory)
-      const WindowReader<C> tr(unit, h0 + tstar);
+      if constexpr (WANT_TIME) {
+        // a7 numerator: re-read the winning window (dynamic index -> shared memory)
+        const WindowReader<C> tr(unit, h0 + tstar);
 #pragma unroll
-      for (int k = 1; k < W; ++k) relnum += k * tr.read(k);
+        for (int k = 1; k < W; ++k) relnum += k * tr.read(k);
+      }
     } else if constexpr (MODE == MODE_FIR) {
       // response on raw samples (the pedestal shifts every y(t) by the same
       // c0*ped); signed compare, strict '>' scanning upwards = earliest on ties
@@ -435,7 +463,10 @@ __device__ __forceinline__ void compute_results(const uint8_t* __restrict__ unit
     }
     const int ped = __ldg(pedestal + p);
     const float gn = __ldg(gain + p);
-    if constexpr (MODE == MODE_FIR)
+    if constexpr (!WANT_TIME) {
+      static_assert(WANT_TIME || MODE == MODE_SLIDING, "only the sliding extractor defers a7");
+      res[j] = finish_charge(W, rawsum, tstar, ped, gn);
+    } else if constexpr (MODE == MODE_FIR)
       res[j] = finish_trace(W, rawsum, tstar, relnum, ped, gn, ma.c0, ma.c1);
     else
       res[j] = finish_trace(W, rawsum, tstar, relnum, ped, gn, W, (W * (W - 1)) / 2);

@@ -240,6 +240,35 @@ __device__ __forceinline__ int neighbour_pass(const int n, const uint16_t* __res
   return any;
 }
 
+// Peak time of pixel p for the moment sums: from an array, or recomputed from the
+// waveform for the fused staged kernel, whose extraction threads leave step a7
+// out (only the few mask pixels of an event ever need a peak time; the samples
+// are still in L2). tstar[p] holds the bits of t*; the same finish_trace as in
+// the extraction gives the same bits.
+struct TimeFromArray {
+  const float* t;
+  __device__ __forceinline__ float operator()(const int p) const { return t[p]; }
+};
+struct TimeFromWaveform {
+  const uint16_t* wf;  // the event's first sample (global memory)
+  const float* tstar;  // [P], bit patterns of t*
+  const int* pedestal;
+  const float* gain;
+  int S, W;
+  __device__ __forceinline__ float operator()(const int p) const {
+    const int ts = __float_as_int(tstar[p]);
+    const uint16_t* x = wf + (size_t)p * (size_t)S + ts;
+    int rawsum = 0, relnum = 0;
+    for (int k = 0; k < W; ++k) {
+      const int v = (int)__ldg(x + k);
+      rawsum += v;
+      relnum += k * v;
+    }
+    return finish_trace(W, rawsum, ts, relnum, __ldg(pedestal + p), __ldg(gain + p), W,
+                        (W * (W - 1)) / 2).time;
+  }
+};
+
 // "q[n] >= thr_boundary" for the symmetric pass: from the bit mask the producer
 // of the event made, or straight from a charge row in shared memory (the
 // moments kernel, which then never builds that mask for a symmetric table).
@@ -411,12 +440,12 @@ __device__ __forceinline__ double shfl_xor_f64(const double v, const int o) {
 // Cleaning and moment sums of event e (readings R31-R35), executed by one whole
 // warp; the sums come back in every lane. core_w (and low_w for the general
 // path) are in shared memory and complete; `low(n)` answers q[n] >= thr_boundary
-// for the symmetric pass; q and t point at the event's charges and peak times
-// (shared or global memory). `after_pass()` runs once the threshold tests are
+// for the symmetric pass; q points at the event's charges (shared or global
+// memory) and t(p) gives pixel p's peak time. `after_pass()` runs once the threshold tests are
 // over (the moments kernel hands its row buffer back to the copy engine there).
-template <class Low, class AfterPass>
+template <class Time, class Low, class AfterPass>
 __device__ __forceinline__ void clean_event_sums(const uint32_t e, const int P, const float* q,
-                                                 const float* t, const uint32_t* core_w,
+                                                 const Time& t, const uint32_t* core_w,
                                                  const uint32_t* low_w, const Low& low,
                                                  const CleanScratch& sc, const NbrTable& nbr,
                                                  const RtaCamera& cam, const RtaImageOut& out,
@@ -476,7 +505,7 @@ __device__ __forceinline__ void clean_event_sums(const uint32_t e, const int P, 
       // waits, and lane 0's coordinates become the origin in the first non-empty round
       int p = lane < n ? (int)sc.list[lane] : 0;
       float qp = 0.0f, tp = 0.0f, xp = 0.0f, yp = 0.0f;
-      if (lane < n) qp = q[p], tp = t[p], xp = __ldg(cam.pix_x + p), yp = __ldg(cam.pix_y + p);
+      if (lane < n) qp = q[p], tp = t(p), xp = __ldg(cam.pix_x + p), yp = __ldg(cam.pix_y + p);
       if (n_pix == 0 && n > 0) {
         x0 = __shfl_sync(0xFFFFFFFFu, xp, 0), y0 = __shfl_sync(0xFFFFFFFFu, yp, 0);
         X0 = (double)x0, Y0 = (double)y0;
@@ -485,7 +514,7 @@ __device__ __forceinline__ void clean_event_sums(const uint32_t e, const int P, 
       for (int i = lane; i < n; i += 32) {
         if (i != lane) {
           p = sc.list[i];
-          qp = q[p], tp = t[p], xp = __ldg(cam.pix_x + p), yp = __ldg(cam.pix_y + p);
+          qp = q[p], tp = t(p), xp = __ldg(cam.pix_x + p), yp = __ldg(cam.pix_y + p);
         }
         const double w = (double)qp;
         const double dx = __dsub_rn((double)xp, X0);
@@ -525,8 +554,9 @@ __device__ __forceinline__ void clean_event_sums(const uint32_t e, const int P, 
 // The fused kernels' cleaning warps: threshold masks from the producer, the
 // neighbour table in global memory, sums parked in lane n_pend's `pd`; after 32
 // events the warp finishes them together.
+template <class Time>
 __device__ __forceinline__ void clean_event(const uint32_t e, const int P, const float* q,
-                                            const float* t, const uint32_t* core_w,
+                                            const Time& t, const uint32_t* core_w,
                                             const uint32_t* low_w, const CleanScratch& sc,
                                             const RtaCamera& cam, const RtaImageOut& out,
                                             const bool symmetric, Pending& pd, int& n_pend) {
@@ -735,7 +765,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
     __syncwarp();
     EventSums cur;
     clean_event_sums(
-        e, P, charge + (size_t)e * (size_t)P, time + (size_t)e * (size_t)P, core_w, low_w,
+        e, P, charge + (size_t)e * (size_t)P, TimeFromArray{time + (size_t)e * (size_t)P}, core_w, low_w,
         LowFromRow{row, thr_b}, sc, nbr, cam, out, symmetric,
         [&] {  // every lane is done with the row: the buffer goes back to the copy engine
           __syncwarp();
@@ -780,7 +810,8 @@ __device__ __forceinline__ void cleaner_loop(const int P, uint8_t* ev_base, uint
     const uint32_t e = fs.ev_id[b];
     if (e == kNoEvent) break;
     const EventBuf buf(ev_base + (size_t)b * eb, P);
-    clean_event(e, P, buf.q, buf.t, buf.core_w, buf.low_w, sc, cam, out, symmetric, pd, n_pend);
+    clean_event(e, P, buf.q, TimeFromArray{buf.t}, buf.core_w, buf.low_w, sc, cam, out, symmetric,
+                pd, n_pend);
     __syncwarp();
     named_arrive(BAR_FREE + b, NT + 32);
   }
@@ -918,8 +949,10 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
       const uint32_t b = k % (uint32_t)NB, use = k / (uint32_t)NB;
       mbar_wait_idle(ready0 + 8 * b, use & 1u);
       const EventBuf buf(ev_base + (size_t)b * eb, P);
-      clean_event(event_of(k), P, buf.q, buf.t, buf.core_w, buf.low_w, sc, cam, out, symmetric,
-                  pd, n_pend);
+      const uint32_t ev = event_of(k);
+      const TimeFromWaveform tw{reinterpret_cast<const uint16_t*>(wf) + (size_t)ev * (size_t)P * C::S,
+                                buf.t, pedestal, gain, C::S, C::W};
+      clean_event(ev, P, buf.q, tw, buf.core_w, buf.low_w, sc, cam, out, symmetric, pd, n_pend);
       __syncwarp();
       if (lane == 0) mbar_arrive(free0 + 8 * b);
     }
@@ -1025,7 +1058,8 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
       if constexpr (!C::PAD) mis = (ev * EB32) & 15u;  // TILE_BYTES is a multiple of 16
       const uint8_t* unit = ringp + stage * STG + mis + gt * C::UNIT_STRIDE;
       Result res[C::TPT];
-      compute_results<C, MODE_SLIDING, RTA_IMG_KEYMODE>(unit, p0, 0u, pedestal, gain, ma, res);
+      // step a7 is left to the cleaning warp (TimeFromWaveform): res[].time = bits of t*
+      compute_results<C, MODE_SLIDING, RTA_IMG_KEYMODE, false>(unit, p0, 0u, pedestal, gain, ma, res);
 #pragma unroll
       for (int i = 0; i < C::TPT; ++i) {  // P is a multiple of TPT: the unit is whole
         buf.q[p0 + i] = qv[i] = res[i].charge;
@@ -1060,8 +1094,12 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
     __syncwarp();
     if (lane == 0) mbar_arrive(ready0 + 8 * b);  // release: this warp's share of the tile is in the buffer
     named_sync(1 + g, NT);                       // every thread of the group is done with the stage
-    if (pc.ev < n_events) issue(pc.ev, pc.tile, stage);
-    advance(pc);
+    // (an empty-stage mbarrier that only the issuing thread waits on, so that the other
+    // warps run ahead, was measured: no gain on C2, 4 % slower on C3)
+    if (C::PAD || gt == 0) {  // dense layouts: only the thread that issues the bulk copy keeps the producer cursor
+      if (pc.ev < n_events) issue(pc.ev, pc.tile, stage);
+      advance(pc);
+    }
     advance(cc);
   }
 }
@@ -1124,7 +1162,10 @@ struct ImgCfg {
 #endif
 using ImgS30W7 = ImgCfg<TileCfg<30, 7, RTA_I30_NT, 2>, RTA_I30_G, RTA_IMG_NC, RTA_I30_XREGS>;
 // 48 registers for the S = 40 extraction code: 0.253 ms on C2 against 0.268 ms at 56 (and 0.290 at 40)
-using ImgS40W7 = ImgCfg<TileCfg<40, 7, RTA_I40_NT, 2>, RTA_I40_G, RTA_IMG_NC, 48>;
+#ifndef RTA_I40_XREGS
+#define RTA_I40_XREGS 56
+#endif
+using ImgS40W7 = ImgCfg<TileCfg<40, 7, RTA_I40_NT, 2>, RTA_I40_G, RTA_IMG_NC, RTA_I40_XREGS>;
 #ifndef RTA_I25_XREGS
 #define RTA_I25_XREGS 64
 #endif
