@@ -105,7 +105,7 @@ def _declare(L: ctypes.CDLL, testing: bool) -> ctypes.CDLL:
     L.rta_shutdown.argtypes = []
     if testing:
         for name in ("rta_debug_force_generic", "rta_debug_static_schedule",
-                     "rta_debug_serial_ragged", "rta_debug_general_cleaning"):
+                     "rta_debug_serial_ragged", "rta_debug_general_cleaning", "rta_debug_jit"):
             fn = getattr(L, name)
             fn.restype = None
             fn.argtypes = [ctypes.c_int]
@@ -431,6 +431,13 @@ def rta_debug_general_cleaning(on: bool) -> None:
     """Test hook (librta_testing.so): the image cleaning runs the two steps of its
     definition even when the neighbour table is symmetric (same masks either way)."""
     _hook("rta_debug_general_cleaning", on)
+
+
+def rta_debug_jit(on: bool) -> None:
+    """Test hook (librta_testing.so): False = no run-time (NVRTC) specialisations, so that
+    unspecialised shapes take the runtime-shape kernel, as without libnvrtc; True = default."""
+    testing_lib().rta_debug_jit(1 if on else 0)
+    (_hooks_on.discard if on else _hooks_on.add)("rta_debug_jit")
 
 
 def shard_events(n_events: int, world_size: int, rank: int) -> tuple[int, int]:

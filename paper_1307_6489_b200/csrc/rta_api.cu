@@ -22,6 +22,7 @@ void rta_debug_serial_ragged(int on);
 void rta_debug_force_generic(int on);
 void rta_debug_static_schedule(int on);
 void rta_debug_general_cleaning(int on);
+void rta_debug_jit(int on);
 }
 #endif
 #pragma GCC visibility pop
@@ -1080,6 +1081,7 @@ void rta_shutdown(void) {
   }
   side_streams_release();
   rta_image_release();
+  rta_jit_release();
   rta_sched_release();
 }
 
@@ -1101,6 +1103,10 @@ void rta_debug_static_schedule(int on) { rta_set_static_schedule(on != 0); }
 // 1 = the image cleaning runs the two
 // steps of its definition even when the neighbour table is symmetric.
 void rta_debug_general_cleaning(int on) { rta_set_general_cleaning(on != 0); }
+
+// 0 = no run-time specialisations: unspecialised shapes take the runtime-shape kernel
+// (staged<any>), as they do when libnvrtc is not available. 1 = back on.
+void rta_debug_jit(int on) { rta_jit_enable(on != 0); }
 #endif  // RTA_TESTING
 
 }  // extern "C"

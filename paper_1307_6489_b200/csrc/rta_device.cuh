@@ -56,7 +56,7 @@ __device__ __forceinline__ void cp_async_mbar_arrive(uint32_t bar) {
 }
 
 // ------------------------------------------------------------ utilities ----
-constexpr int ilog2_ceil(int n) {
+__host__ __device__ constexpr int ilog2_ceil(int n) {
   int b = 0;
   while ((1 << b) < n) ++b;
   return b;

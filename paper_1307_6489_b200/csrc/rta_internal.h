@@ -3,11 +3,23 @@
 #ifndef RTA_INTERNAL_H
 #define RTA_INTERNAL_H
 
-#include <cuda_runtime.h>
-#include <stdint.h>
-
 // The extractor family (readings R22-R24): how the window is chosen.
 #define RTA_MAX_TAPS 32
+
+#ifdef __CUDACC_RTC__
+// Run-time compilation of a specialised tile kernel (rta_jit.cu): device code
+// only, no host headers. NVRTC predefines size_t and the CUDA built-ins.
+typedef unsigned char uint8_t;
+typedef unsigned short uint16_t;
+typedef unsigned int uint32_t;
+typedef int int32_t;
+typedef unsigned long long uint64_t;
+typedef long long int64_t;
+typedef unsigned long long uintptr_t;
+#else
+#include <cuda_runtime.h>
+#include <stdint.h>
+#endif
 enum { RTA_MODE_SLIDING = 0, RTA_MODE_FIXED = 1, RTA_MODE_LOCAL_PEAK = 2, RTA_MODE_FIR = 3 };
 struct RtaMode {
   int kind;
@@ -17,6 +29,7 @@ struct RtaMode {
   int32_t taps[RTA_MAX_TAPS];   // RTA_MODE_FIR
 };
 
+#ifndef __CUDACC_RTC__
 // Enqueue the extraction of `n_traces` traces starting at global trace index 0
 // of `wf` on `stream`. Arguments are already validated. Returns a cudaError_t.
 // `force_generic` routes every shape to the generic kernel (tests use it to
@@ -90,5 +103,27 @@ void rta_image_release();  // frees the scratch memory pools (rta_shutdown)
 int32_t rta_image_pixel_limit();  // charge, time and flags of one event must fit one CTA
 const char* rta_pick_image_kernel_name(int32_t n_pixels, int32_t n_samples, int32_t W,
                                        bool aligned16);
+
+// Run-time specialisation (rta_jit.cu): the staged tile kernel compiled by NVRTC
+// for one (n_samples, W, extractor) the first time that shape is seen, cached
+// per process. rta_jit_launch returns cudaErrorNotSupported when the shape is
+// not eligible or the compiler is not available (the caller then takes the
+// runtime-shape kernel); any other error is a launch error.
+struct RtaJitArgs {
+  const void* wf;
+  uint32_t n_traces, n_pixels, pix_inv;
+  const int32_t* pedestal;
+  const float* gain;
+  int32_t *out_sum, *out_start;
+  float *out_charge, *out_time;
+  uint32_t* sched;
+};
+bool rta_jit_eligible(int32_t n_samples, int32_t W);   // shape fits a register copy, JIT enabled
+bool rta_jit_available();                              // ... and libnvrtc could be loaded
+cudaError_t rta_jit_launch(int32_t n_samples, int32_t W, int mode, const RtaJitArgs& a,
+                           const void* mode_args, size_t mode_args_bytes, cudaStream_t stream);
+void rta_jit_enable(bool on);   // tests: switch the run-time specialisations off / on
+void rta_jit_release();         // rta_shutdown
+#endif  // __CUDACC_RTC__
 
 #endif

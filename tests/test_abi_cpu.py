@@ -43,7 +43,8 @@ def test_shipped_library_exports_exactly_the_header():
     rta.lib()
     assert exported(b.LIB) == declared_symbols()
     hooks = {"rta_extract_generic", "rta_extract_image_generic", "rta_debug_force_generic",
-             "rta_debug_static_schedule", "rta_debug_serial_ragged", "rta_debug_general_cleaning"}
+             "rta_debug_static_schedule", "rta_debug_serial_ragged", "rta_debug_general_cleaning",
+             "rta_debug_jit"}
     assert set(exported(b.TEST_LIB)) == set(declared_symbols()) | hooks
     T = rta.testing_lib()
     for n in hooks:
@@ -114,9 +115,17 @@ def test_strerror_and_kernel_names():
     # units of a multiple of 32 bytes (padded layout, 16-byte cp.async) the generic one
     assert rta.rta_kernel_name(40, 7, aligned16=False) == "staged<any>"
     assert rta.rta_kernel_name(128, 8, aligned16=False) == "generic"
-    # any other shape with units up to 1152 bytes: the staged kernel with runtime (S, W)
-    assert rta.rta_kernel_name(41, 7) == "staged<any>"
-    assert rta.rta_kernel_name(60, 7) == "staged<any>"
+    # any other shape: units up to 320 bytes are compiled for their (S, W) at first use when
+    # libnvrtc can be loaded (staged<jit>); otherwise, and for units up to 1152 bytes, the
+    # staged kernel with runtime (S, W)
+    assert rta.rta_kernel_name(41, 7) in ("staged<jit>", "staged<any>")
+    assert rta.rta_kernel_name(60, 7) == rta.rta_kernel_name(160, 9) == rta.rta_kernel_name(41, 7)
+    assert rta.rta_kernel_name(162, 9) == "staged<any>"
+    rta.rta_debug_jit(False)
+    try:
+        assert rta.rta_kernel_name(41, 7) == rta.rta_kernel_name(60, 7) == "staged<any>"
+    finally:
+        rta.rta_debug_jit(True)
     assert rta.rta_kernel_name(576, 9) == "staged<any>" and rta.rta_kernel_name(287, 9) == "staged<any>"
     assert rta.rta_kernel_name(578, 9) == "generic" and rta.rta_kernel_name(289, 9) == "generic"
     assert rta.rta_kernel_name(60, 7, aligned16=False) == "staged<any>"

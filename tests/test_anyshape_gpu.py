@@ -38,7 +38,8 @@ SHAPES = [
 @pytest.mark.parametrize("E,P", [(1, 1), (5, 3), (3, 700), (2, 5000)])
 def test_any_shape_random(S, W, E, P):
     import paper_1307_6489_b200 as rta
-    assert rta.rta_kernel_name(S, W) == "staged<any>"
+    jit = 2 * S * (2 if S % 2 else 1) <= 320        # the unit fits a register copy: run-time specialisation
+    assert rta.rta_kernel_name(S, W) == ("staged<jit>" if jit else "staged<any>")
     if E * P * S > 3_000_000:
         E = 1
     rng = np.random.default_rng(S * 1009 + W * 31 + E * P)
@@ -50,9 +51,15 @@ def test_any_shape_random(S, W, E, P):
     ped = (rng.integers(-70000, 70000, P) if full else rng.integers(0, 600, P)).astype(np.int32)
     gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
     want = oracle.extract(wf, ped, gain, W)
-    got = run_gpu(wf, ped, gain, W)
+    got = run_gpu(wf, ped, gain, W)                  # NVRTC specialisation where eligible
     assert (got[0] == want[0]).all() and (got[1] == want[1]).all()
     assert bit_identical(got, want)
+    rta.rta_debug_jit(False)                         # the runtime-shape kernel (no libnvrtc needed)
+    try:
+        assert rta.rta_kernel_name(S, W) == "staged<any>"
+        assert bit_identical(run_gpu(wf, ped, gain, W), want)
+    finally:
+        rta.rta_debug_jit(True)
     old = run_gpu(wf, ped, gain, W, generic=True)
     assert bit_identical(got, old)
 
@@ -69,13 +76,16 @@ def test_any_shape_many_tiles_both_schedules(S, W):
     ped = rng.integers(380, 421, P).astype(np.int32)
     gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
     want = oracle.extract(wf, ped, gain, W)
-    for static in (False, True):
-        rta.rta_debug_static_schedule(static)
-        try:
-            got = run_gpu(wf, ped, gain, W)
-        finally:
-            rta.rta_debug_static_schedule(False)
-        assert bit_identical(got, want)
+    for jit in (True, False):                        # run-time specialisation / runtime-shape kernel
+        for static in (False, True):
+            rta.rta_debug_static_schedule(static)
+            rta.rta_debug_jit(jit)
+            try:
+                got = run_gpu(wf, ped, gain, W)
+            finally:
+                rta.rta_debug_static_schedule(False)
+                rta.rta_debug_jit(True)
+            assert bit_identical(got, want), (jit, static)
 
 
 def test_any_shape_closed_forms():
@@ -86,10 +96,16 @@ def test_any_shape_closed_forms():
     for k in range(S):
         wf[0, k, k] = ped + 50
     wf[0, S, :] = 777
-    got = run_gpu(wf, np.full(S + 1, ped, np.int32), np.ones(S + 1, np.float32), W)
-    for k in range(S):
-        assert got[0][k] == 50 and got[1][k] == max(0, k - W + 1) and got[3][k] == np.float32(k)
-    assert got[0][S] == W * (777 - ped) and got[1][S] == 0 and got[3][S] == np.float32((W - 1) / 2)
+    import paper_1307_6489_b200 as rta
+    for jit in (True, False):
+        rta.rta_debug_jit(jit)
+        try:
+            got = run_gpu(wf, np.full(S + 1, ped, np.int32), np.ones(S + 1, np.float32), W)
+        finally:
+            rta.rta_debug_jit(True)
+        for k in range(S):
+            assert got[0][k] == 50 and got[1][k] == max(0, k - W + 1) and got[3][k] == np.float32(k)
+        assert got[0][S] == W * (777 - ped) and got[1][S] == 0 and got[3][S] == np.float32((W - 1) / 2)
 
 
 @pytest.mark.parametrize("S,W", [(30, 7), (40, 7), (25, 4), (60, 7), (50, 8), (200, 9), (33, 5), (128, 8), (96, 8)])
