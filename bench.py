@@ -65,7 +65,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="C2",
-                    choices=["C1", "C2", "C3", "C4", "X60", "X40w5", "X96", "X128w10"],
+                    choices=["C1", "C2", "C3", "C4", "X60", "X40w5", "X96", "X128w10", "X2048"],
                     help="C1..C4: BASELINE.json configs; X*: shapes without a specialised kernel "
                          "(diagnostic runs of the runtime-shape kernel, imply --no-extra)")
     ap.add_argument("--input-format", default="u16", choices=["u16", "p12"],
@@ -513,7 +513,10 @@ def extra_shapes(dl0gen):
               dataclasses.replace(c4, name="X96", label="10000x2048x96 W=8", seed=13, n_events=10_000,
                                   n_samples=96, peak_lo=25.0, peak_hi=70.0),
               dataclasses.replace(c4, name="X128w10", label="10000x2048x128 W=10", seed=14,
-                                  n_events=10_000, W=10)]
+                                  n_events=10_000, W=10),
+              # traces too long for one thread (4096 bytes): a warp per trace
+              dataclasses.replace(c4, name="X2048", label="1000x2048x2048 W=12", seed=15,
+                                  n_events=1000, n_samples=2048, W=12, peak_lo=200.0, peak_hi=1800.0)]
     return {c.name: c for c in shapes}
 
 

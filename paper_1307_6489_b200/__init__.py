@@ -105,7 +105,8 @@ def _declare(L: ctypes.CDLL, testing: bool) -> ctypes.CDLL:
     L.rta_shutdown.argtypes = []
     if testing:
         for name in ("rta_debug_force_generic", "rta_debug_static_schedule",
-                     "rta_debug_serial_ragged", "rta_debug_general_cleaning", "rta_debug_jit"):
+                     "rta_debug_serial_ragged", "rta_debug_general_cleaning", "rta_debug_jit",
+                     "rta_debug_lanes_per_trace"):
             fn = getattr(L, name)
             fn.restype = None
             fn.argtypes = [ctypes.c_int]
@@ -438,6 +439,13 @@ def rta_debug_jit(on: bool) -> None:
     unspecialised shapes take the runtime-shape kernel, as without libnvrtc; True = default."""
     testing_lib().rta_debug_jit(1 if on else 0)
     (_hooks_on.discard if on else _hooks_on.add)("rta_debug_jit")
+
+
+def rta_debug_lanes_per_trace(lpt: int) -> None:
+    """Test / measurement hook (librta_testing.so): 4, 8, 16 or 32 = rta_extract runs the
+    several-lanes-per-trace kernel with that many lanes wherever it can; 0 = normal dispatch."""
+    testing_lib().rta_debug_lanes_per_trace(int(lpt))
+    (_hooks_on.add if lpt else _hooks_on.discard)("rta_debug_lanes_per_trace")
 
 
 def shard_events(n_events: int, world_size: int, rank: int) -> tuple[int, int]:

@@ -23,6 +23,7 @@ void rta_debug_force_generic(int on);
 void rta_debug_static_schedule(int on);
 void rta_debug_general_cleaning(int on);
 void rta_debug_jit(int on);
+void rta_debug_lanes_per_trace(int lpt);
 }
 #endif
 #pragma GCC visibility pop
@@ -1107,6 +1108,10 @@ void rta_debug_general_cleaning(int on) { rta_set_general_cleaning(on != 0); }
 // 0 = no run-time specialisations: unspecialised shapes take the runtime-shape kernel
 // (staged<any>), as they do when libnvrtc is not available. 1 = back on.
 void rta_debug_jit(int on) { rta_jit_enable(on != 0); }
+
+// 4 / 8 / 16 / 32 = rta_extract runs the several-lanes-per-trace kernel with that many lanes
+// per trace wherever it can (measurements of DESIGN.md section 5g); 0 = normal dispatch.
+void rta_debug_lanes_per_trace(int lpt) { rta_set_lanes_per_trace(lpt); }
 #endif  // RTA_TESTING
 
 }  // extern "C"

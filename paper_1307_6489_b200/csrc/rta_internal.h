@@ -69,6 +69,9 @@ void rta_count_launch();
 // round-robin (tests compare the two). rta_sched_release frees the per-stream
 // scheduler words (rta_shutdown).
 void rta_set_static_schedule(bool on);
+// Measurements / tests: 4, 8, 16 or 32 = the sliding extractor runs the several-lanes-per-trace
+// kernel with that many lanes wherever it can (n_samples a multiple of 8, aligned base); 0 = normal.
+void rta_set_lanes_per_trace(int lpt);
 void rta_sched_release();
 cudaError_t rta_device_sms(int dev, int* sms);
 // Allow `func` up to 227 KB of dynamic shared memory on `dev` (set once per kernel and device).

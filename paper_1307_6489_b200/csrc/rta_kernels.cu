@@ -624,8 +624,119 @@ __global__ void __launch_bounds__(256)
   }
 }
 
+// ------------------------------------------ several lanes per trace ----
+// LPT lanes own one trace (32 / LPT traces per warp at a time): the formulation
+// with warp-shuffle prefix sums that BASELINE.json:north_star (b) names. Lane j
+// of a group loads the 16-byte chunks j, j + LPT, ... of the trace straight
+// from global memory (coalesced), forms the inclusive prefix sums of its 8
+// samples, a shuffle scan over the group's lanes adds the lanes in front and a
+// carry the rounds before, and the exclusive prefix array X[i] = x[0] + ... + x[i-1]
+// goes to shared memory. Window sums are then X[t + W] - X[t] (a lane takes four
+// consecutive t per step with a 16-byte load), the arg-max key is reduced over the group
+// by shuffles, and lane 0 of the group finishes the trace. Any n_samples that
+// is a multiple of 8 on a 16-byte-aligned base, any W: this is the kernel for
+// traces too long for a thread (units above 1152 bytes), where the alternative
+// is the strided generic kernel; on S = 128 it was measured against the
+// thread-per-trace specialisation.
+template <int LPT>
+__global__ void __launch_bounds__(256)
+    extract_lanes_kernel(const uint8_t* __restrict__ wf, const uint32_t n_traces, const int S,
+                         const int W, const int kb, const uint32_t n_pixels,
+                         const uint32_t pix_inv, const int* __restrict__ pedestal,
+                         const float* __restrict__ gain, int* __restrict__ out_sum,
+                         int* __restrict__ out_start, float* __restrict__ out_charge,
+                         float* __restrict__ out_time) {
+  extern __shared__ __align__(16) uint32_t lanes_smem[];
+  const int lane = threadIdx.x & 31, j = lane % LPT;
+  const uint32_t gmask = LPT == 32 ? 0xFFFFFFFFu : (((1u << (LPT & 31)) - 1u) << (lane - j));
+  const uint32_t groups = blockDim.x / LPT, gi = threadIdx.x / LPT;
+  // per group: the EXCLUSIVE prefix sums X[i] = x[0] + ... + x[i-1], i = 0 .. S (X[0] = 0),
+  // 16-byte aligned, padded so that the 4-window steps below may read up to X[S + 6]
+  const uint32_t pstride = (uint32_t)S + 12u;
+  uint32_t* X = lanes_smem + gi * pstride;
+  const int n_chunks = S >> 3, n_win = S - W + 1;
+  const uint32_t key_mul = 1u << kb, KM = key_mul - 1u;
+  constexpr int U = 4;  // chunks in flight per lane: the loads of a step go out before any is used
+  for (uint32_t g = blockIdx.x * groups + gi; g < n_traces; g += gridDim.x * groups) {
+    const uint4* src = reinterpret_cast<const uint4*>(wf + (size_t)g * (size_t)S * 2u);
+    uint32_t carry = 0;
+    for (int c0 = 0; c0 < n_chunks; c0 += U * LPT) {
+      uint4 v[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int c = c0 + u * LPT + j;
+        v[u] = c < n_chunks ? __ldcs(src + c) : make_uint4(0u, 0u, 0u, 0u);
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int c = c0 + u * LPT + j;
+        uint4 lo, hi;  // exclusive prefix sums inside the chunk, then its total
+        lo.x = 0u;
+        lo.y = v[u].x & 0xFFFFu;
+        lo.z = lo.y + (v[u].x >> 16);
+        lo.w = lo.z + (v[u].y & 0xFFFFu);
+        hi.x = lo.w + (v[u].y >> 16);
+        hi.y = hi.x + (v[u].z & 0xFFFFu);
+        hi.z = hi.y + (v[u].z >> 16);
+        hi.w = hi.z + (v[u].w & 0xFFFFu);
+        const uint32_t total = hi.w + (v[u].w >> 16);
+        uint32_t incl = total;  // scan of the chunk totals over the group's lanes
+#pragma unroll
+        for (int o = 1; o < LPT; o <<= 1) {
+          const uint32_t up = __shfl_up_sync(gmask, incl, o, LPT);
+          if (j >= o) incl += up;
+        }
+        const uint32_t base = carry + incl - total;
+        if (c < n_chunks) {
+          uint4* dst = reinterpret_cast<uint4*>(X + 8 * c);
+          dst[0] = make_uint4(base, base + lo.y, base + lo.z, base + lo.w);
+          dst[1] = make_uint4(base + hi.x, base + hi.y, base + hi.z, base + hi.w);
+        }
+        carry += __shfl_sync(gmask, incl, LPT - 1, LPT);
+      }
+    }
+    if (j == 0) X[S] = carry;  // the sum of the whole trace
+    __syncwarp(gmask);
+    // a3 + a4: Sum(t) = X[t + W] - X[t], four consecutive windows per lane and step
+    // (16-byte loads; windows past the end are masked), packed (sum, earliest) key
+    uint32_t best = 0;  // every key is >= 0 and window 0 exists
+    for (int t = 4 * j; t < n_win; t += 4 * LPT) {
+      const uint4 a = *reinterpret_cast<const uint4*>(X + t);
+      const uint32_t* e = X + t + W;
+      const uint32_t k0 = (e[0] - a.x) * key_mul + (KM - (uint32_t)t);
+      const uint32_t k1 = (e[1] - a.y) * key_mul + (KM - (uint32_t)t - 1u);
+      const uint32_t k2 = (e[2] - a.z) * key_mul + (KM - (uint32_t)t - 2u);
+      const uint32_t k3 = (e[3] - a.w) * key_mul + (KM - (uint32_t)t - 3u);
+      best = max(best, k0);
+      if (t + 1 < n_win) best = max(best, k1);
+      if (t + 2 < n_win) best = max(best, k2);
+      if (t + 3 < n_win) best = max(best, k3);
+    }
+#pragma unroll
+    for (int o = LPT / 2; o > 0; o >>= 1) best = max(best, __shfl_xor_sync(gmask, best, o, LPT));
+    const int tstar = (int)(KM - (best & KM));
+    const int rawsum = (int)(best >> kb);
+    // a7 numerator: sum_k k raw[t* + k], raw[i] = X[i + 1] - X[i]
+    int relnum = 0;
+    for (int k = j; k < W; k += LPT) relnum += k * (int)(X[tstar + k + 1] - X[tstar + k]);
+#pragma unroll
+    for (int o = LPT / 2; o > 0; o >>= 1) relnum += __shfl_xor_sync(gmask, relnum, o, LPT);
+    if (j == 0) {
+      const uint32_t p = fastmod(g, n_pixels, pix_inv);
+      const Result r = finish_trace(W, rawsum, tstar, relnum, __ldg(pedestal + p), __ldg(gain + p),
+                                    W, (W * (W - 1)) / 2);
+      __stcs(out_sum + g, r.sum);
+      __stcs(out_start + g, r.start);
+      __stcs(out_charge + g, r.charge);
+      __stcs(out_time + g, r.time);
+    }
+    __syncwarp(gmask);  // the prefix array is rewritten by the next trace
+  }
+}
+
 // ------------------------------------------------------------- dispatch ----
 constexpr int kMaxDevices = 32;
+std::atomic<int> g_force_lanes{0};  // tests / measurements: lanes per trace to use wherever the lanes kernel can run
 std::atomic<bool> g_static_schedule{false};  // tests: force the static round-robin
 
 struct DeviceInfo {
@@ -790,6 +901,7 @@ int TileLauncher<C, MODE>::ctas_per_sm[kMaxDevices];
 }  // namespace
 
 void rta_set_static_schedule(bool on) { g_static_schedule.store(on); }
+void rta_set_lanes_per_trace(int lpt) { g_force_lanes.store(lpt); }
 cudaError_t rta_device_sms(int dev, int* sms) { return device_sms(dev, sms); }
 
 // rta_shutdown: the caller has synchronised the device(s)
@@ -832,6 +944,8 @@ const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16, int bits)
   } else if (rta_dyn_eligible(S, W) && (2 * S * ((S & 1) ? 2 : 1)) % 32 != 0) {
     return "staged<any>";  // dense layout: any 2-byte alignment (also for the specialised shapes)
   }
+  if (aligned16 && S >= 8 && S % 8 == 0 && 4u * ((size_t)S + 12u) <= 200u * 1024u)
+    return "lanes<32>";  // a warp per trace: traces too long for one thread
   return "generic";
 }
 
@@ -942,6 +1056,39 @@ cudaError_t launch_dyn(const LaunchArgs& a, const DynShape& sh, int threads, con
   return cudaGetLastError();
 }
 
+// The lanes kernel takes the sliding extractor on a 16-byte-aligned base when n_samples
+// is a multiple of 8 and one group's prefix array fits a CTA.
+bool lanes_eligible(const LaunchArgs& a) {
+  return a.staged && a.S >= 8 && a.S % 8 == 0 && 4u * ((size_t)a.S + 12u) <= 200u * 1024u;
+}
+
+template <int LPT>
+cudaError_t launch_lanes(const LaunchArgs& a) {
+  int dev = 0, sms = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
+  const size_t per_group = 4u * ((size_t)a.S + 12u);
+  int threads = 256;  // as many groups per CTA as fit about a third of an SM's shared memory
+  while (threads > LPT && (size_t)(threads / LPT) * per_group > 72u * 1024u) threads /= 2;
+  const size_t smem = (size_t)(threads / LPT) * per_group;
+  auto kernel = extract_lanes_kernel<LPT>;
+  if ((e = rta_func_allow_max_smem((const void*)kernel, dev)) != cudaSuccess) return e;
+  int occ = 0;
+  if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem)) != cudaSuccess)
+    return e;
+  if (occ < 1) return cudaErrorLaunchOutOfResources;
+  const uint32_t groups = (uint32_t)(threads / LPT);
+  uint32_t grid = (uint32_t)(sms * occ);
+  const uint32_t need = (a.n_traces + groups - 1u) / groups;
+  if (grid > need) grid = need;
+  kernel<<<grid, threads, smem, a.stream>>>(a.wf, a.n_traces, a.S, a.W, ilog2_ceil(a.S - a.W + 1),
+                                            a.n_pixels, a.pix_inv, a.pedestal, a.gain, a.out_sum,
+                                            a.out_start, a.out_charge, a.out_time);
+  rta_count_launch();
+  return cudaGetLastError();
+}
+
 #define RTA_TRY(CFG)                                                                          \
   if (a.S == CFG::S && a.W == CFG::W)                                                         \
     return TileLauncher<CFG, MODE>::launch(a.wf, a.n_traces, a.n_pixels, a.pix_inv,           \
@@ -953,6 +1100,15 @@ cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
   // sectors per trace, gathering them from global memory (the generic kernel)
   // moves less than streaming whole tiles (S = 128: 0.99 ms against 1.69 ms).
   const bool gather = (MODE == MODE_FIXED) && 2 * a.S > 96;
+  if (MODE == MODE_SLIDING && lanes_eligible(a)) {
+    switch (g_force_lanes.load(std::memory_order_relaxed)) {  // measurements only (0 in production)
+      case 4: return launch_lanes<4>(a);
+      case 8: return launch_lanes<8>(a);
+      case 16: return launch_lanes<16>(a);
+      case 32: return launch_lanes<32>(a);
+      default: break;
+    }
+  }
   if (a.staged && !gather) {
     RTA_TRY(CfgS30W7)
     RTA_TRY(CfgS40W7)
@@ -986,6 +1142,8 @@ cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
     if (dyn_shape(a.S, a.W, &sh, &threads) && sh.unit_stride == sh.unit_bytes)
       return launch_dyn<MODE>(a, sh, threads, ma);
   }
+  // traces too long for one thread: a warp per trace (shuffle scan, prefix array in shared memory)
+  if (MODE == MODE_SLIDING && lanes_eligible(a)) return launch_lanes<32>(a);
   return launch_generic<MODE, 16>(a, ma);
 }
 

@@ -137,3 +137,50 @@ def test_unaligned_base_pointers(S, W, off):
                             W, *outs)
             torch.cuda.synchronize()
             assert bit_identical(tuple(o.cpu().numpy() for o in outs), want), (E, P, guard)
+
+
+# ---- several lanes per trace (shuffle prefix sums): long traces, and any S % 8 == 0 on request
+def _tie_heavy(rng, E, P, S, hi):
+    wf = rng.integers(0, hi, size=(E, P, S)).astype(np.uint16)
+    wf[rng.random((E, P)) < 0.15] = hi - 1                     # all windows tie
+    wf[rng.random((E, P)) < 0.15] //= np.uint16(hi // 2)       # tie-heavy
+    return wf
+
+
+@pytest.mark.parametrize("S,W", [(584, 9), (1000, 32), (2048, 12), (2048, 1), (4096, 7), (8192, 3), (800, 40), (1024, 1024 // 512)])
+def test_long_traces_take_a_warp_per_trace(S, W):
+    """Units above 1152 bytes with n_samples a multiple of 8: lanes<32> (one warp per
+    trace, shuffle scan + prefix array in shared memory) instead of the strided generic
+    kernel; both against the oracle, full uint16 range where the ABI guard allows."""
+    import paper_1307_6489_b200 as rta
+    assert rta.rta_kernel_name(S, W) == "lanes<32>"
+    rng = np.random.default_rng(S + W)
+    for E, P in ((1, 1), (3, 37), (2, 700)):
+        hi = 65536 if S * W * 65535 < 2 ** 31 and W % 2 else 4096
+        wf = _tie_heavy(rng, E, P, S, hi)
+        ped = rng.integers(0, 600, P).astype(np.int32)
+        gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
+        want = oracle.extract(wf, ped, gain, W)
+        assert bit_identical(run_gpu(wf, ped, gain, W), want), (E, P)
+        assert bit_identical(run_gpu(wf, ped, gain, W, generic=True), want), (E, P)
+
+
+@pytest.mark.parametrize("lpt", [4, 8, 16, 32])
+@pytest.mark.parametrize("S,W", [(128, 8), (40, 7), (8, 8), (16, 1), (96, 9), (256, 20)])
+def test_lanes_per_trace_on_short_traces(lpt, S, W):
+    """The same kernel with 4, 8, 16 or 32 lanes per trace on shapes that normally take a
+    thread per trace (the measurement of DESIGN.md section 5g): bit-identical to the oracle,
+    trace counts that leave groups and warps partly empty."""
+    import paper_1307_6489_b200 as rta
+    rng = np.random.default_rng(lpt * 1000 + S)
+    for E, P in ((1, 1), (2, 37), (3, 1855)):
+        wf = _tie_heavy(rng, E, P, S, 4096)
+        ped = rng.integers(-70000, 70000, P).astype(np.int32)
+        gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
+        want = oracle.extract(wf, ped, gain, W)
+        rta.rta_debug_lanes_per_trace(lpt)
+        try:
+            got = run_gpu(wf, ped, gain, W)
+        finally:
+            rta.rta_debug_lanes_per_trace(0)
+        assert bit_identical(got, want), (E, P)
