@@ -75,9 +75,16 @@ def parse_args():
                     help="main leg: rta_extract (default, the BASELINE metric); 'image' = "
                          "rta_extract_image, 'moments' = rta_image_moments (diagnostic runs "
                          "for profiling, imply --no-extra)")
+    ap.add_argument("--extractor", default="sliding", choices=["sliding", "fixed", "local_peak", "fir"],
+                    help="main leg with --path extract: rta_extract (default, the BASELINE metric) or one "
+                         "of the NEXT-1 extractors (diagnostic / profiling runs; secondary legs are skipped)")
     ap.add_argument("--no-extra", action="store_true", help="skip configs/e2e/sustained/cpu legs")
     ap.add_argument("--no-sustained", action="store_true", help="skip the 29.68 GB C5 leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--legs", default="all",
+                    help="comma list of the secondary single-GPU legs to run: configs, family, packed12, "
+                         "any_shape, ragged, image (default: all; the profiling commands in profiles/ "
+                         "name one leg each)")
     ap.add_argument("--e2e-chunk-mb", type=int, default=64)
     return ap.parse_args()
 
@@ -322,8 +329,37 @@ def image_outputs(cfg, torch):
             torch.empty((cfg.n_events, 8), dtype=torch.float32, device="cuda"))
 
 
+def family_runs(cfg, base, outs, stream, torch, rta):
+    """The three NEXT-1 extractors on one device batch: per-pixel fixed window starts
+    (seeded), local peak with shift W/2, FIR with triangular taps."""
+    import numpy as np
+    start = torch.from_numpy(np.random.default_rng(cfg.seed).integers(
+        0, cfg.n_samples - cfg.W + 1, cfg.n_pixels).astype(np.int32)).cuda()
+    taps = [1, 2, 3, 4, 3, 2, 1, 1][:cfg.W]
+    runs = {
+        "fixed": lambda: rta.rta_extract_fixed(*base, cfg.W, start, *outs, stream=stream),
+        "local_peak": lambda: rta.rta_extract_local_peak(*base, cfg.W, cfg.W // 2, *outs, stream=stream),
+        "fir": lambda: rta.rta_extract_fir(*base, taps, *outs, stream=stream),
+    }
+    return runs, start, taps
+
+
+def fixed_gather_bytes_per_trace(cfg, start):
+    """rta_extract_fixed GATHERS for traces longer than 96 bytes (rta_kernels.cu launch_mode): it
+    touches only the W-sample window of a trace, so its algorithmic bytes are the 32-byte sectors
+    that window overlaps (+ 16 bytes out), not the whole waveform. None when it streams."""
+    import numpy as np
+    if 2 * cfg.n_samples <= 96:
+        return None, None
+    st = start.cpu().numpy().astype(np.int64)
+    g = np.arange(min(cfg.n_traces, 64 * cfg.n_pixels), dtype=np.int64)
+    lo = g * (2 * cfg.n_samples) + 2 * st[g % cfg.n_pixels]
+    sectors = (lo + 2 * cfg.W - 1) // 32 - lo // 32 + 1
+    return 32.0 * float(sectors.mean()) + ALGO_BYTES_PER_TRACE_OUT, float(sectors.mean())
+
+
 def kernel_only(cfg, steps, warmup, torch, dl0gen, rta, barrier=None, sampler=None, fmt="u16",
-                path="extract"):
+                path="extract", extractor="sliding"):
     d_wf, d_ped, d_gain, outs, ped, gain = device_batch(cfg, torch, dl0gen)
     stream = torch.cuda.current_stream()
     if path in ("image", "moments"):
@@ -349,6 +385,10 @@ def kernel_only(cfg, steps, warmup, torch, dl0gen, rta, barrier=None, sampler=No
         def run():
             rta.rta_extract_packed12(d_pk, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped,
                                      d_gain, cfg.W, *outs, stream=stream)
+    elif extractor != "sliding":
+        runs, fam_start, _ = family_runs(
+            cfg, (d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain), outs, stream, torch, rta)
+        run = runs[extractor]
     else:
         def run():
             rta.rta_extract(d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain,
@@ -367,7 +407,7 @@ def kernel_only(cfg, steps, warmup, torch, dl0gen, rta, barrier=None, sampler=No
         barrier()
     checksum = int(d_wf.view(-1)[: min(d_wf.numel(), 1 << 26)].sum(dtype=torch.int64))
     return {"per_launch_ms": per, "launches": launches, "checksum_first_64Mi_samples": checksum,
-            "marks": (m0, m1),
+            "marks": (m0, m1), "fixed_start": fam_start if extractor == "fixed" else None,
             "keep": (d_wf, d_ped, d_gain, outs, ped, gain)}
 
 
@@ -392,15 +432,8 @@ def family_leg(cfg, steps, peak, torch, dl0gen, rta):
     import numpy as np
     d_wf, d_ped, d_gain, outs, ped, gain = device_batch(cfg, torch, dl0gen)
     stream = torch.cuda.current_stream()
-    start = torch.from_numpy(np.random.default_rng(cfg.seed).integers(
-        0, cfg.n_samples - cfg.W + 1, cfg.n_pixels).astype(np.int32)).cuda()
-    taps = [1, 2, 3, 4, 3, 2, 1, 1][:cfg.W]
     base = (d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain)
-    runs = {
-        "fixed": lambda: rta.rta_extract_fixed(*base, cfg.W, start, *outs, stream=stream),
-        "local_peak": lambda: rta.rta_extract_local_peak(*base, cfg.W, cfg.W // 2, *outs, stream=stream),
-        "fir": lambda: rta.rta_extract_fir(*base, taps, *outs, stream=stream),
-    }
+    runs, start, taps = family_runs(cfg, base, outs, stream, torch, rta)
     res = {}
     for name, run in runs.items():
         for _ in range(LEG_WARMUP):
@@ -408,20 +441,13 @@ def family_leg(cfg, steps, peak, torch, dl0gen, rta):
         torch.cuda.synchronize()
         res[name] = summarise(cfg, time_steps(run, steps, stream), peak)
     res["fir"]["taps"] = taps
-    if 2 * cfg.n_samples > 96:
-        # rta_extract_fixed GATHERS for traces longer than 96 bytes (rta_kernels.cu launch_mode): it
-        # touches only the W-sample window of a trace, so its algorithmic bytes are the 32-byte
-        # sectors that window overlaps (+ 16 bytes out), not the whole waveform
-        st = start.cpu().numpy().astype(np.int64)
-        g = np.arange(min(cfg.n_traces, 64 * cfg.n_pixels), dtype=np.int64)
-        lo = g * (2 * cfg.n_samples) + 2 * st[g % cfg.n_pixels]
-        sectors = (lo + 2 * cfg.W - 1) // 32 - lo // 32 + 1
-        per_trace = 32.0 * float(sectors.mean()) + ALGO_BYTES_PER_TRACE_OUT
+    per_trace, mean_sectors = fixed_gather_bytes_per_trace(cfg, start)
+    if per_trace is not None:
         f = res["fixed"]
         algo = per_trace * cfg.n_traces
         f["route"] = "gather (generic kernel): W samples of each trace from global memory"
         f["bytes_per_trace"] = per_trace
-        f["mean_sectors_per_trace"] = float(sectors.mean())
+        f["mean_sectors_per_trace"] = mean_sectors
         f["streamed_equivalent_GBps"] = f["algorithmic_GBps"]
         f["algorithmic_GBps"] = algo / f["ms_avg"] / 1e6
         f["frac_of_measured_hbm"] = f["algorithmic_GBps"] / peak
@@ -554,6 +580,7 @@ def any_shape_leg(steps, peak, torch, dl0gen, rta):
     return res
 
 
+SECONDARY_LEGS = ("configs", "family", "packed12", "any_shape", "ragged", "image")
 EVENT_OUT_BYTES = 36   # n_pix int32 + 8 fp32 parameters per event
 LEG_WARMUP = 10        # untimed launches in front of every secondary leg (the GPU idles while a leg sets up)
 
@@ -990,10 +1017,13 @@ def main():
     # Weak scaling: every rank extracts its own batch of the named workload
     # (independent events; no data-path collective).
     fmt = args.input_format
-    if fmt == "p12" or args.path != "extract" or args.workload.startswith("X"):
-        args.no_extra = True     # the packed / image main legs are profiling/diagnostic runs
+    if (fmt == "p12" or args.path != "extract" or args.workload.startswith("X")
+            or args.extractor != "sliding"):
+        args.no_extra = True     # the packed / image / family main legs are profiling/diagnostic runs
+    if args.extractor != "sliding" and (fmt != "u16" or args.path != "extract"):
+        raise SystemExit("--extractor goes with --path extract --input-format u16")
     main_run = kernel_only(cfg, args.steps, args.warmup, torch, dl0gen, rta, barrier, sampler, fmt,
-                           args.path)
+                           args.path, args.extractor)
     clocks = sampler.stop(*main_run["marks"])
     t_local = sum(main_run["per_launch_ms"])
     t_max = t_local
@@ -1016,6 +1046,18 @@ def main():
         summ["algorithmic_GBps"] = algo_bytes / avg / 1e6
         summ["frac_of_measured_hbm"] = algo_bytes / avg / 1e6 / peak
         summ["frac_of_nominal_8TBps"] = algo_bytes / avg / 1e6 / 8000.0
+    if args.extractor != "sliding":
+        kname = "%s:%s" % (args.extractor, kname)
+        per_trace, _ = (fixed_gather_bytes_per_trace(cfg, main_run["fixed_start"])
+                        if args.extractor == "fixed" else (None, None))
+        if per_trace is not None:     # the gathering route: sectors touched, not whole traces
+            kname = "fixed:gather(generic)"
+            bytes_per_trace = per_trace
+            algo_bytes = per_trace * cfg.n_traces
+            avg = summ["ms_avg"]
+            summ["algorithmic_GBps"] = algo_bytes / avg / 1e6
+            summ["frac_of_measured_hbm"] = algo_bytes / avg / 1e6 / peak
+            summ["frac_of_nominal_8TBps"] = algo_bytes / avg / 1e6 / 8000.0
     if args.path != "extract":
         ev_bytes = EVENT_OUT_BYTES * cfg.n_events
         if args.path == "image":
@@ -1037,6 +1079,7 @@ def main():
         "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
         "config": {
             "workload": "%s: %s" % (cfg.name, cfg.label) + (" as a P12 stream" if fmt == "p12" else "")
+                        + ("" if args.extractor == "sliding" else " through rta_extract_" + args.extractor)
                         + {"extract": "", "image": " through rta_extract_image",
                            "moments": " charges through rta_image_moments"}[args.path],
             "per_gpu": "%d events x %d pixels x %d samples uint16, W=%d" % (
@@ -1097,38 +1140,48 @@ def main():
                 out["cpu_baseline"] = cpu_baseline_leg(cfg, keep, dl0gen, torch)
             main_run["keep"] = keep = None
             torch.cuda.empty_cache()
+            legs = set(SECONDARY_LEGS if args.legs == "all" else
+                       [x for x in args.legs.split(",") if x])
+            if legs - set(SECONDARY_LEGS):
+                raise SystemExit("--legs: unknown leg(s) %s" % sorted(legs - set(SECONDARY_LEGS)))
             others = {}
             for name in ("C3", "C4"):
-                if name == cfg.name:
+                if name == cfg.name or "configs" not in legs:
                     continue
                 c = dl0gen.CONFIGS[name]
                 r = kernel_only(c, max(10, args.steps // 2), 3, torch, dl0gen, rta)
                 others[name] = summarise(c, r["per_launch_ms"], peak)
                 r = None
                 torch.cuda.empty_cache()
-            out["configs"] = others
+            if "configs" in legs:
+                out["configs"] = others
             fam = {}
-            for name in ("C2", "C3", "C4"):
+            for name in ("C2", "C3", "C4") if "family" in legs else ():
                 fam[name] = family_leg(dl0gen.CONFIGS[name], max(10, args.steps // 4), peak,
                                        torch, dl0gen, rta)
                 torch.cuda.empty_cache()
-            out["family"] = fam
+            if fam:
+                out["family"] = fam
             pk = {}
-            for name in ("C2", "C3", "C4"):
+            for name in ("C2", "C3", "C4") if "packed12" in legs else ():
                 pk[name] = packed_leg(dl0gen.CONFIGS[name], max(10, args.steps // 4), peak,
                                       torch, dl0gen, rta)
                 torch.cuda.empty_cache()
-            out["packed12"] = pk
-            out["any_shape"] = any_shape_leg(max(10, args.steps // 4), peak, torch, dl0gen, rta)
-            torch.cuda.empty_cache()
-            out["ragged"] = ragged_leg(max(10, args.steps // 4), peak, torch, dl0gen, rta)
-            torch.cuda.empty_cache()
+            if pk:
+                out["packed12"] = pk
+            if "any_shape" in legs:
+                out["any_shape"] = any_shape_leg(max(10, args.steps // 4), peak, torch, dl0gen, rta)
+                torch.cuda.empty_cache()
+            if "ragged" in legs:
+                out["ragged"] = ragged_leg(max(10, args.steps // 4), peak, torch, dl0gen, rta)
+                torch.cuda.empty_cache()
             img = {}
-            for name in ("C2", "C3", "C4"):
+            for name in ("C2", "C3", "C4") if "image" in legs else ():
                 img[name] = image_leg(dl0gen.CONFIGS[name], max(10, args.steps // 4), peak,
                                       torch, dl0gen, rta)
                 torch.cuda.empty_cache()
-            out["image"] = img
+            if img:
+                out["image"] = img
             link = host_link_bandwidth(torch)
             out["e2e"]["host_link_GBps_measured"] = link
             out["e2e"]["frac_of_host_link"] = out["e2e"]["value"] / link
