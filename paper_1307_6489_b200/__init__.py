@@ -110,6 +110,8 @@ def _declare(L: ctypes.CDLL, testing: bool) -> ctypes.CDLL:
             fn = getattr(L, name)
             fn.restype = None
             fn.argtypes = [ctypes.c_int]
+        L.rta_debug_seg_tuning.restype = None
+        L.rta_debug_seg_tuning.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]
     return L
 
 
@@ -446,6 +448,14 @@ def rta_debug_lanes_per_trace(lpt: int) -> None:
     several-lanes-per-trace kernel with that many lanes wherever it can; 0 = normal dispatch."""
     testing_lib().rta_debug_lanes_per_trace(int(lpt))
     (_hooks_on.add if lpt else _hooks_on.discard)("rta_debug_lanes_per_trace")
+
+
+def rta_debug_seg_tuning(L: int = 0, TR: int = 0, NT: int = 0, stages: int = 0) -> None:
+    """Test / measurement hook (librta_testing.so): window starts per segment (2 * odd), traces
+    per tile, threads per CTA and ring stages of the segment kernel (0 = chosen per shape). A non-zero L
+    sends every sliding rta_extract on a 16-byte-aligned base to that kernel."""
+    testing_lib().rta_debug_seg_tuning(int(L), int(TR), int(NT), int(stages))
+    (_hooks_on.add if (L or TR or NT or stages) else _hooks_on.discard)("rta_debug_seg_tuning")
 
 
 def shard_events(n_events: int, world_size: int, rank: int) -> tuple[int, int]:

@@ -24,6 +24,7 @@ void rta_debug_static_schedule(int on);
 void rta_debug_general_cleaning(int on);
 void rta_debug_jit(int on);
 void rta_debug_lanes_per_trace(int lpt);
+void rta_debug_seg_tuning(int L, int TR, int NT, int stages);
 }
 #endif
 #pragma GCC visibility pop
@@ -1112,6 +1113,10 @@ void rta_debug_jit(int on) { rta_jit_enable(on != 0); }
 // 4 / 8 / 16 / 32 = rta_extract runs the several-lanes-per-trace kernel with that many lanes
 // per trace wherever it can (measurements of DESIGN.md section 5g); 0 = normal dispatch.
 void rta_debug_lanes_per_trace(int lpt) { rta_set_lanes_per_trace(lpt); }
+
+// Segment kernel: window starts per segment (2 * odd), traces per tile, threads per CTA, stages; 0 =
+// chosen per shape. A non-zero L sends every sliding call on an aligned base to that kernel.
+void rta_debug_seg_tuning(int L, int TR, int NT, int stages) { rta_set_seg_tuning(L, TR, NT, stages); }
 #endif  // RTA_TESTING
 
 }  // extern "C"

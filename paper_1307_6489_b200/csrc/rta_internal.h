@@ -72,6 +72,11 @@ void rta_set_static_schedule(bool on);
 // Measurements / tests: 4, 8, 16 or 32 = the sliding extractor runs the several-lanes-per-trace
 // kernel with that many lanes wherever it can (n_samples a multiple of 8, aligned base); 0 = normal.
 void rta_set_lanes_per_trace(int lpt);
+// Measurements / tests: segment length (2 * odd), traces per tile and threads per CTA of the
+// segment kernel; 0 = chosen per shape. A non-zero L sends every sliding call on an aligned
+// base to that kernel.
+void rta_set_seg_tuning(int L, int TR, int NT, int stages);
+bool rta_seg_eligible(int32_t n_samples, int32_t W);
 void rta_sched_release();
 cudaError_t rta_device_sms(int dev, int* sms);
 // Allow `func` up to 227 KB of dynamic shared memory on `dev` (set once per kernel and device).

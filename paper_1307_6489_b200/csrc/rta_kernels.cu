@@ -734,10 +734,242 @@ __global__ void __launch_bounds__(256)
   }
 }
 
+// ------------------------------------------ long traces: a thread per segment ----
+// Traces too long for one thread (units above 1152 bytes). A tile is TR whole
+// traces in a ring of 2-4 stages (mbarrier per stage, dynamic tile scheduler as
+// in the other staged kernels). The n_win windows of a trace are cut into
+// segments of L consecutive window starts; a thread takes one segment: it sums
+// the first window (W loads) and then slides like the runtime-shape kernel (two
+// 16-bit shared-memory loads per window; the samples up to W - 1 past its
+// segment belong to the same trace), keeping the packed (sum, earliest) key of
+// its segment. The keys of a trace meet in one atomicMax on a shared-memory word
+// per trace: the packed key orders by sum first and earlier start second across
+// segments exactly as inside one. After a barrier thread i finishes trace i of
+// the tile (a5-a7).
+// Banks: L / 2 is odd, so consecutive segments of a trace start on consecutive
+// (odd-stride) banks. When n_samples is a multiple of 8 every trace is copied by
+// its own bulk copy to a stride of `trace_stride` bytes chosen so that segment 0
+// of the next trace continues that bank sequence (slots per trace nslot = nseg
+// rounded up to a multiple of 4, stride = nslot L / 2 words mod 32): 32
+// consecutive slots never share a bank. Other n_samples keep the dense layout
+// (one bulk copy per tile, TR n_samples a multiple of 8 so tiles start on
+// 16-byte boundaries; a last tile whose byte count is not a multiple of 16 gets
+// its last bytes halfword by halfword from the issuing thread).
+struct SegShape {
+  int32_t S, W, n_win;
+  int32_t L;             // window starts per segment
+  int32_t nseg;          // ceil(n_win / L)
+  int32_t nslot;         // thread slots per trace (>= nseg; the extra ones idle)
+  uint32_t nslot_inv;    // min(floor(2^32 / nslot), 2^32 - 1)
+  int32_t TR;            // traces per tile
+  int32_t trace_stride;  // bytes between traces in a stage: 2 S (dense) or padded
+  int32_t stage_bytes;   // multiple of 128
+  int32_t stages;
+  int32_t kb;
+  uint32_t key_mul;
+};
+constexpr int kSegMaxStages = 4;
+constexpr int kSegMaxTR = 64;
+
+// The windows 1 .. nw-1 of a segment whose window 0 starts at x (sum = its sum, low = the
+// low key bits of window 0): the best packed key of the segment.
+// 16-bit loads, any alignment: window i enters x[W-1+i] and leaves x[i-1].
+__device__ __forceinline__ uint32_t seg_slide_u16(const uint16_t* x, const int W, const int nw,
+                                                  uint32_t sum, const uint32_t mul, uint32_t low) {
+  uint32_t best = sum * mul + low;
+  const uint16_t* xe = x + (W - 1);
+  const uint16_t* xl = x - 1;
+  // one add-sub per window, in order: left to the compiler the unrolled sums are
+  // re-associated into a tree that costs twice the adds (measured)
+#pragma unroll 8
+  for (int i = 1; i < nw; ++i) {
+    const uint32_t e = xe[i], l = xl[i];
+    asm("{ .reg .u32 t; add.u32 t, %0, %1; sub.u32 %0, t, %2; }" : "+r"(sum) : "r"(e), "r"(l));
+    --low;
+    best = max(best, sum * mul + low);
+  }
+  return best;
+}
+
+// x on a 4-byte boundary: two windows per step from one 32-bit load per stream. The
+// leaving pair (x[2m], x[2m+1]) is word m; the entering pair (x[W+2m], x[W+2m+1]) is
+// word W/2 + m, or for odd W the funnel shift of two consecutive words (the second is
+// kept for the next step). Both window sums come from the sum two windows back by
+// dp2a (IDP.2A): + e.lo - l.lo and + e.lo + e.hi - l.lo - l.hi.
+template <bool WODD>
+__device__ __forceinline__ uint32_t seg_slide_pairs(const uint16_t* x, const int W, const int nw,
+                                                    uint32_t sum, const uint32_t mul, uint32_t low) {
+  uint32_t best = sum * mul + low;
+  const uint32_t* xl = reinterpret_cast<const uint32_t*>(x);
+  const uint32_t* xe = xl + (W >> 1);
+  constexpr uint32_t kPlus = 0x01010001u;   // bytes (1, 0 | 1, 1): .lo adds a.lo, .hi adds a.lo + a.hi
+  constexpr uint32_t kMinus = 0xFFFF00FFu;  // bytes (-1, 0 | -1, -1)
+  const int np = (nw - 1) >> 1;
+  uint32_t ecur = WODD ? xe[0] : 0u;
+  int s = (int)sum;
+#pragma unroll 4
+  for (int m = 0; m < np; ++m) {
+    const uint32_t lw = xl[m];
+    uint32_t ew;
+    if constexpr (WODD) {
+      const uint32_t enext = xe[m + 1];
+      ew = __funnelshift_r(ecur, enext, 16);
+      ecur = enext;
+    } else {
+      ew = xe[m];
+    }
+    const int s1 = dp2a_u16_s8<0>(lw, kMinus, dp2a_u16_s8<0>(ew, kPlus, s));
+    s = dp2a_u16_s8<1>(lw, kMinus, dp2a_u16_s8<1>(ew, kPlus, s));
+    low -= 2u;
+    best = max(best, (uint32_t)s1 * mul + (low + 1u));
+    best = max(best, (uint32_t)s * mul + low);
+  }
+  if ((nw - 1) & 1) {  // the last window of an even-length segment
+    const int i = nw - 1;
+    s += (int)x[W - 1 + i] - (int)x[i - 1];
+    best = max(best, (uint32_t)s * mul + (low - 1u));
+  }
+  return best;
+}
+
+__global__ void __launch_bounds__(256)
+    extract_seg_kernel(const uint8_t* __restrict__ wf, const uint32_t n_traces,
+                       const uint32_t n_pixels, const uint32_t pix_inv,
+                       const int* __restrict__ pedestal, const float* __restrict__ gain,
+                       int* __restrict__ out_sum, int* __restrict__ out_start,
+                       float* __restrict__ out_charge, float* __restrict__ out_time,
+                       uint32_t* __restrict__ sched, const __grid_constant__ SegShape sh) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t full_bar[kSegMaxStages];
+  __shared__ uint32_t tile_q[kSegMaxStages + 1];
+  __shared__ uint32_t bestk[kSegMaxTR];
+  const int tid = threadIdx.x, NT = blockDim.x;
+  const int STAGES = sh.stages, QN = STAGES + 1;
+  const int S = sh.S, W = sh.W;
+  const uint32_t TR = (uint32_t)sh.TR;
+  const uint32_t n_tiles = (n_traces + TR - 1u) / TR;
+  const uint32_t trace_bytes = 2u * (uint32_t)S;
+  const bool dense = (uint32_t)sh.trace_stride == trace_bytes;
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t bar_base = smem_u32(full_bar);
+
+  TileFeed feed(sched, n_tiles, STAGES);  // thread 0 only
+
+  if (tid == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(bar_base + 8 * s, 1);
+      tile_q[s] = feed.fetch_static();
+    }
+    fence_mbar_init();
+    feed.prime();
+  }
+  if (tid < kSegMaxTR) bestk[tid] = 0u;  // every key is >= 0 and window 0 of a trace always exists
+  __syncthreads();
+
+  auto tile_traces = [&](const uint32_t tile) {
+    const uint32_t left = n_traces - tile * TR;
+    return left < TR ? left : TR;
+  };
+  auto issue = [&](const uint32_t tile, const int stage) {  // thread 0
+    const uint8_t* src = wf + (size_t)tile * (size_t)TR * (size_t)trace_bytes;
+    const uint32_t n_tr = tile_traces(tile);
+    const uint32_t bar = bar_base + 8 * stage;
+    const uint32_t dst = smem_base + (uint32_t)(stage * sh.stage_bytes);
+    if (dense) {
+      const uint32_t bytes = n_tr * trace_bytes;
+      const uint32_t len = bytes & ~15u;
+      uint8_t* d = smem + stage * sh.stage_bytes;
+      for (uint32_t b = len; b < bytes; b += 2u)  // the last tile only: nothing past the buffer is read
+        *reinterpret_cast<uint16_t*>(d + b) = *reinterpret_cast<const uint16_t*>(src + b);
+      mbar_expect_tx(bar, len);
+      if (len != 0) tma_bulk_g2s(dst, src, len, bar);
+    } else {  // one copy per trace (a multiple of 16 bytes each) to the padded stride
+      mbar_expect_tx(bar, n_tr * trace_bytes);
+      for (uint32_t i = 0; i < n_tr; ++i)
+        tma_bulk_g2s(dst + i * (uint32_t)sh.trace_stride, src + (size_t)i * trace_bytes, trace_bytes, bar);
+    }
+  };
+
+  if (tid == 0) {
+    for (int s = 0; s < STAGES; ++s)
+      if (tile_q[s] < n_tiles) issue(tile_q[s], s);
+  }
+  uint32_t pre = 0;
+  if (tid == 0) pre = feed.fetch();
+
+  const uint32_t mul = sh.key_mul, KM = sh.key_mul - 1u;
+  const uint32_t stride_hw = (uint32_t)sh.trace_stride / 2u;
+  // every segment starts on a 4-byte boundary (L is even) when the traces do
+  const bool pairs = (stride_hw & 1u) == 0u;
+  for (uint32_t j = 0;; ++j) {
+    const uint32_t tile = tile_q[j % QN];
+    if (tile >= n_tiles) break;
+    const int stage = (int)(j % (uint32_t)STAGES);
+    const uint32_t parity = (j / (uint32_t)STAGES) & 1u;
+    if (tid == 0) {
+      tile_q[(j + STAGES) % QN] = pre;
+      pre = feed.fetch();
+    }
+    const uint32_t n_tr = tile_traces(tile);
+    // the thread that will finish trace `tid` of the tile asks for its calibration now
+    int ped = 0;
+    float gn = 0.0f;
+    if ((uint32_t)tid < n_tr) {
+      const uint32_t p = fastmod(tile * TR + (uint32_t)tid, n_pixels, pix_inv);
+      ped = __ldg(pedestal + p), gn = __ldg(gain + p);
+    }
+    mbar_wait(bar_base + 8 * stage, parity);
+    const uint16_t* base = reinterpret_cast<const uint16_t*>(smem + stage * sh.stage_bytes);
+    const uint32_t n_q = n_tr * (uint32_t)sh.nslot;
+    for (uint32_t q = tid; q < n_q; q += NT) {
+      uint32_t tr = __umulhi(q, sh.nslot_inv);
+      uint32_t seg = q - tr * (uint32_t)sh.nslot;
+      if (seg >= (uint32_t)sh.nslot) seg -= (uint32_t)sh.nslot, ++tr;
+      if (seg >= (uint32_t)sh.nseg) continue;  // a padding slot
+      const int t0 = (int)seg * sh.L;
+      const int nw = min(sh.L, sh.n_win - t0);
+      const uint16_t* x = base + tr * stride_hw + t0;
+      uint32_t sum = 0;
+#pragma unroll 4
+      for (int k = 0; k < W; ++k) sum += x[k];
+      const uint32_t best = pairs ? ((W & 1) ? seg_slide_pairs<true>(x, W, nw, sum, mul, KM - (uint32_t)t0)
+                                             : seg_slide_pairs<false>(x, W, nw, sum, mul, KM - (uint32_t)t0))
+                                  : seg_slide_u16(x, W, nw, sum, mul, KM - (uint32_t)t0);
+      atomicMax(&bestk[tr], best);
+    }
+    __syncthreads();
+    if ((uint32_t)tid < n_tr) {
+      const uint32_t best = bestk[tid];
+      bestk[tid] = 0u;
+      const int tstar = (int)(KM - (best & KM));
+      const int rawsum = (int)(best >> sh.kb);
+      const uint16_t* x = base + (uint32_t)tid * stride_hw + tstar;
+      int relnum = 0;
+#pragma unroll 4
+      for (int k = 1; k < W; ++k) relnum += k * (int)x[k];
+      const uint32_t g = tile * TR + (uint32_t)tid;
+      const Result r = finish_trace(W, rawsum, tstar, relnum, ped, gn, W, (W * (W - 1)) / 2);
+      __stcs(out_sum + g, r.sum);
+      __stcs(out_start + g, r.start);
+      __stcs(out_charge + g, r.charge);
+      __stcs(out_time + g, r.time);
+    }
+    __syncthreads();  // the stage is free and bestk is zero again
+    if (tid == 0) {
+      const uint32_t next = tile_q[(j + STAGES) % QN];
+      if (next < n_tiles) issue(next, stage);
+    }
+  }
+  if (tid == 0) feed.leave();
+}
+
 // ------------------------------------------------------------- dispatch ----
 constexpr int kMaxDevices = 32;
 std::atomic<int> g_force_lanes{0};  // tests / measurements: lanes per trace to use wherever the lanes kernel can run
 std::atomic<bool> g_static_schedule{false};  // tests: force the static round-robin
+// tests / measurements: segment length, traces per tile and threads per CTA of the segment
+// kernel (0 = chosen per shape); a forced L also sends shapes that have a faster kernel there
+std::atomic<int> g_seg_L{0}, g_seg_TR{0}, g_seg_NT{0}, g_seg_ST{0};
 
 struct DeviceInfo {
   std::atomic<int> ready{0};
@@ -902,6 +1134,12 @@ int TileLauncher<C, MODE>::ctas_per_sm[kMaxDevices];
 
 void rta_set_static_schedule(bool on) { g_static_schedule.store(on); }
 void rta_set_lanes_per_trace(int lpt) { g_force_lanes.store(lpt); }
+void rta_set_seg_tuning(int L, int TR, int NT, int stages) {
+  g_seg_L.store(L);
+  g_seg_TR.store(TR);
+  g_seg_NT.store(NT);
+  g_seg_ST.store(stages);
+}
 cudaError_t rta_device_sms(int dev, int* sms) { return device_sms(dev, sms); }
 
 // rta_shutdown: the caller has synchronised the device(s)
@@ -924,6 +1162,19 @@ void rta_sched_release() {
   cudaGetLastError();
 }
 
+// The segment kernel takes the sliding extractor on a 16-byte-aligned base when two
+// stages of at least one tile-aligned group of traces fit a CTA and the window is
+// not much wider than the longest segment (the first window of every segment costs
+// W loads; the lanes kernel does not care about W).
+bool rta_seg_eligible(int32_t S, int32_t W) {
+  if (S < 1 || W < 1 || W > S || W - 1 > 2 * 258) return false;
+  int step = 1;  // traces per tile in the dense layout: tiles start on 16-byte boundaries
+  if (S % 8 != 0)
+    while (((long long)step * S) % 8 != 0) step *= 2;
+  const long long stage = (((long long)step * (2 * S + 128) + 127) / 128) * 128;
+  return 2 * stage <= 200 * 1024;
+}
+
 const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16, int bits) {
   if (bits == 12) {
     if (aligned16) {
@@ -944,8 +1195,9 @@ const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16, int bits)
   } else if (rta_dyn_eligible(S, W) && (2 * S * ((S & 1) ? 2 : 1)) % 32 != 0) {
     return "staged<any>";  // dense layout: any 2-byte alignment (also for the specialised shapes)
   }
+  if (aligned16 && rta_seg_eligible(S, W)) return "segments";  // a thread per segment of a long trace
   if (aligned16 && S >= 8 && S % 8 == 0 && 4u * ((size_t)S + 12u) <= 200u * 1024u)
-    return "lanes<32>";  // a warp per trace: traces too long for one thread
+    return "lanes<32>";  // a warp per trace: very wide windows or very long traces
   return "generic";
 }
 
@@ -1089,6 +1341,94 @@ cudaError_t launch_lanes(const LaunchArgs& a) {
   return cudaGetLastError();
 }
 
+// Shape of the segment kernel for (S, W); false = not eligible. L is 2 * odd (bank
+// spread), a tile is at most 64 traces, TR * S is a multiple of 8 when the layout is
+// dense (tiles start on 16-byte boundaries).
+bool seg_shape_for(int32_t S, int32_t W, int L, int TR, int NT, int stages, SegShape* sh, int* threads) {
+  if (S < 1 || W < 1 || W > S || L < 2 || (L / 2) % 2 == 0 || L % 2 != 0) return false;
+  if (TR < 1 || TR > kSegMaxTR) return false;
+  if (NT < 32 || NT > 256 || NT % 32 != 0 || NT < TR) return false;
+  if (stages < 2 || stages > kSegMaxStages) return false;
+  const bool per_trace = S % 8 == 0;
+  if (!per_trace && ((long long)TR * S) % 8 != 0) return false;
+  sh->S = S;
+  sh->W = W;
+  sh->n_win = S - W + 1;
+  sh->L = L;
+  sh->nseg = (sh->n_win + L - 1) / L;
+  sh->nslot = per_trace ? ((sh->nseg + 3) / 4) * 4 : sh->nseg;
+  sh->nslot_inv = sh->nslot == 1 ? 0xFFFFFFFFu : (uint32_t)(0x100000000ull / (unsigned long long)sh->nslot);
+  long long stride = 2ll * S;
+  if (per_trace) {
+    // words between traces = nslot L / 2 (mod 32), at least S / 2, a multiple of 4
+    const int want = (int)(((long long)sh->nslot * (L / 2)) % 32);
+    long long w = S / 2;
+    while (w % 32 != want) w += 4;  // S / 2 and `want` are multiples of 4: at most 7 steps
+    stride = 4 * w;
+  }
+  const long long stage = (((long long)TR * stride + 127) / 128) * 128;
+  if (stages * stage > 200 * 1024) return false;
+  sh->TR = TR;
+  sh->trace_stride = (int32_t)stride;
+  sh->stage_bytes = (int32_t)stage;
+  sh->stages = stages;
+  sh->kb = ilog2_ceil(sh->n_win);
+  sh->key_mul = 1u << sh->kb;
+  *threads = NT;
+  return true;
+}
+
+// The shape the dispatch uses: segments of 66 window starts (130 and 258 for wide
+// windows), tiles of about 16 KB in two stages (measured: more resident warps beat a
+// deeper ring), as many threads as the tile has slots.
+bool seg_shape(int32_t S, int32_t W, SegShape* sh, int* threads) {
+  const int fL = g_seg_L.load(std::memory_order_relaxed), fTR = g_seg_TR.load(std::memory_order_relaxed);
+  const int fNT = g_seg_NT.load(std::memory_order_relaxed), fST = g_seg_ST.load(std::memory_order_relaxed);
+  const int L = fL ? fL : (W - 1 <= 66 ? 66 : W - 1 <= 130 ? 130 : 258);
+  int step = 1;  // TR must be a multiple of this in the dense layout
+  if (S % 8 != 0)
+    while (((long long)step * S) % 8 != 0) step *= 2;
+  int TR = fTR ? fTR : (int)((16 * 1024) / (2ll * S) / step) * step;
+  if (TR < step) TR = step;
+  if (TR > kSegMaxTR) TR = (kSegMaxTR / step) * step;
+  const int n_win = S - W + 1;
+  const int nseg = (n_win + L - 1) / L;
+  const int nslot = S % 8 == 0 ? ((nseg + 3) / 4) * 4 : nseg;
+  int NT = fNT;
+  if (!NT) {
+    const long long slots = (long long)TR * nslot;
+    NT = slots <= 32 ? 32 : slots <= 64 ? 64 : slots <= 128 ? 128 : 256;
+    if (NT < TR) NT = ((TR + 31) / 32) * 32;
+  }
+  for (int stages = fST ? fST : 2; stages >= 2; --stages)
+    if (seg_shape_for(S, W, L, TR, NT, stages, sh, threads)) return true;
+  return false;
+}
+
+cudaError_t launch_seg(const LaunchArgs& a, const SegShape& sh, int threads) {
+  int dev = 0, sms = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
+  const int smem = sh.stages * sh.stage_bytes;
+  if ((e = rta_func_allow_max_smem((const void*)extract_seg_kernel, dev)) != cudaSuccess) return e;
+  int occ = 0;
+  if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, extract_seg_kernel, threads, smem)) !=
+      cudaSuccess)
+    return e;
+  if (occ < 1) return cudaErrorLaunchOutOfResources;
+  const uint32_t n_tiles = (a.n_traces + (uint32_t)sh.TR - 1u) / (uint32_t)sh.TR;
+  uint32_t grid = (uint32_t)(sms * occ);
+  if (grid > n_tiles) grid = n_tiles;
+  if (grid < 1) grid = 1;
+  uint32_t* sched = g_static_schedule ? nullptr : sched_words(dev, a.stream);
+  extract_seg_kernel<<<grid, threads, smem, a.stream>>>(a.wf, a.n_traces, a.n_pixels, a.pix_inv,
+                                                        a.pedestal, a.gain, a.out_sum, a.out_start,
+                                                        a.out_charge, a.out_time, sched, sh);
+  rta_count_launch();
+  return cudaGetLastError();
+}
+
 #define RTA_TRY(CFG)                                                                          \
   if (a.S == CFG::S && a.W == CFG::W)                                                         \
     return TileLauncher<CFG, MODE>::launch(a.wf, a.n_traces, a.n_pixels, a.pix_inv,           \
@@ -1100,6 +1440,11 @@ cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
   // sectors per trace, gathering them from global memory (the generic kernel)
   // moves less than streaming whole tiles (S = 128: 0.99 ms against 1.69 ms).
   const bool gather = (MODE == MODE_FIXED) && 2 * a.S > 96;
+  if (MODE == MODE_SLIDING && a.staged && g_seg_L.load(std::memory_order_relaxed) != 0) {
+    SegShape sg;  // measurements / tests only: the segment kernel on any shape
+    int threads = 0;
+    if (seg_shape(a.S, a.W, &sg, &threads)) return launch_seg(a, sg, threads);
+  }
   if (MODE == MODE_SLIDING && lanes_eligible(a)) {
     switch (g_force_lanes.load(std::memory_order_relaxed)) {  // measurements only (0 in production)
       case 4: return launch_lanes<4>(a);
@@ -1142,7 +1487,14 @@ cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
     if (dyn_shape(a.S, a.W, &sh, &threads) && sh.unit_stride == sh.unit_bytes)
       return launch_dyn<MODE>(a, sh, threads, ma);
   }
-  // traces too long for one thread: a warp per trace (shuffle scan, prefix array in shared memory)
+  // traces too long for one thread: a thread per segment of a trace; windows much wider
+  // than a segment, or traces too long for a stage, a warp per trace (shuffle scan,
+  // prefix array in shared memory: its cost does not depend on W)
+  if (MODE == MODE_SLIDING && a.staged) {
+    SegShape sg;
+    int threads = 0;
+    if (rta_seg_eligible(a.S, a.W) && seg_shape(a.S, a.W, &sg, &threads)) return launch_seg(a, sg, threads);
+  }
   if (MODE == MODE_SLIDING && lanes_eligible(a)) return launch_lanes<32>(a);
   return launch_generic<MODE, 16>(a, ma);
 }

@@ -44,7 +44,7 @@ def test_shipped_library_exports_exactly_the_header():
     assert exported(b.LIB) == declared_symbols()
     hooks = {"rta_extract_generic", "rta_extract_image_generic", "rta_debug_force_generic",
              "rta_debug_static_schedule", "rta_debug_serial_ragged", "rta_debug_general_cleaning",
-             "rta_debug_jit", "rta_debug_lanes_per_trace"}
+             "rta_debug_jit", "rta_debug_lanes_per_trace", "rta_debug_seg_tuning"}
     assert set(exported(b.TEST_LIB)) == set(declared_symbols()) | hooks
     T = rta.testing_lib()
     for n in hooks:
@@ -127,9 +127,12 @@ def test_strerror_and_kernel_names():
     finally:
         rta.rta_debug_jit(True)
     assert rta.rta_kernel_name(576, 9) == "staged<any>" and rta.rta_kernel_name(287, 9) == "staged<any>"
-    # longer traces: a warp per trace when n_samples is a multiple of 8, else the generic kernel
-    assert rta.rta_kernel_name(578, 9) == "generic" and rta.rta_kernel_name(289, 9) == "generic"
-    assert rta.rta_kernel_name(584, 9) == "lanes<32>" and rta.rta_kernel_name(2048, 12) == "lanes<32>"
+    # longer traces: a thread per segment of a trace (any S that the ABI guard n_samples * W *
+    # 65535 < 2^31 admits; the names below are what the dispatch would pick past that guard)
+    assert rta.rta_kernel_name(578, 9) == "segments" and rta.rta_kernel_name(289, 9) == "segments"
+    assert rta.rta_kernel_name(584, 9) == "segments" and rta.rta_kernel_name(2048, 12) == "segments"
+    assert rta.rta_kernel_name(2048, 1000) == "lanes<32>" and rta.rta_kernel_name(2047, 1000) == "generic"
+    assert rta.rta_kernel_name(65536, 4) == "generic" and rta.rta_kernel_name(40000, 4) == "segments"
     assert rta.rta_kernel_name(2048, 12, aligned16=False) == "generic"
     assert rta.rta_kernel_name(60, 7, aligned16=False) == "staged<any>"
     assert rta.rta_kernel_name(96, 8, aligned16=False) == "generic"

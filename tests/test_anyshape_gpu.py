@@ -147,22 +147,62 @@ def _tie_heavy(rng, E, P, S, hi):
     return wf
 
 
-@pytest.mark.parametrize("S,W", [(584, 9), (1000, 32), (2048, 12), (2048, 1), (4096, 7), (8192, 3), (800, 40), (1024, 1024 // 512)])
-def test_long_traces_take_a_warp_per_trace(S, W):
-    """Units above 1152 bytes with n_samples a multiple of 8: lanes<32> (one warp per
-    trace, shuffle scan + prefix array in shared memory) instead of the strided generic
-    kernel; both against the oracle, full uint16 range where the ABI guard allows."""
+@pytest.mark.parametrize("S,W", [(584, 9), (1000, 32), (2048, 12), (2048, 1), (4096, 7), (8192, 3), (800, 40),
+                                 (1024, 1024 // 512), (578, 9), (289, 9), (601, 2), (1001, 30), (3000, 10),
+                                 (20000, 1), (16000, 2), (2050, 15), (2050, 12), (2052, 9)])
+def test_long_traces_take_a_thread_per_segment(S, W):
+    """Units above 1152 bytes: the segment kernel (a thread per run of window starts, keys of
+    a trace merged by a shared-memory atomicMax) instead of the strided generic kernel, for
+    any n_samples (odd ones included: the tile then holds a multiple of 8 traces); both
+    against the oracle, full uint16 range where the ABI guard allows; trace counts that
+    leave the last tile partly empty and not a multiple of 16 bytes long."""
     import paper_1307_6489_b200 as rta
-    assert rta.rta_kernel_name(S, W) == "lanes<32>"
+    assert rta.rta_kernel_name(S, W) == "segments"
     rng = np.random.default_rng(S + W)
-    for E, P in ((1, 1), (3, 37), (2, 700)):
+    for E, P in ((1, 1), (3, 37), (2, 700), (1, 67)):
+        if E * P * S > 3_000_000:
+            P = max(1, 3_000_000 // (E * S))
         hi = 65536 if S * W * 65535 < 2 ** 31 and W % 2 else 4096
+        if S * W * (hi - 1) >= 2 ** 31:
+            hi = max(2, (2 ** 31 - 1) // (S * W))
         wf = _tie_heavy(rng, E, P, S, hi)
         ped = rng.integers(0, 600, P).astype(np.int32)
         gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
         want = oracle.extract(wf, ped, gain, W)
         assert bit_identical(run_gpu(wf, ped, gain, W), want), (E, P)
+        for static in (True,):
+            rta.rta_debug_static_schedule(static)
+            try:
+                assert bit_identical(run_gpu(wf, ped, gain, W), want), (E, P, "static")
+            finally:
+                rta.rta_debug_static_schedule(False)
         assert bit_identical(run_gpu(wf, ped, gain, W, generic=True), want), (E, P)
+
+
+@pytest.mark.parametrize("L,TR,NT,ST", [(34, 8, 128, 2), (66, 0, 0, 0), (130, 16, 256, 4), (2, 8, 32, 3), (6, 64, 64, 2),
+                                         (258, 0, 0, 0), (66, 1, 32, 4)])
+@pytest.mark.parametrize("S,W", [(128, 8), (40, 7), (25, 4), (33, 33), (96, 1), (1000, 32), (2048, 12)])
+def test_segment_kernel_on_any_shape(L, TR, NT, ST, S, W):
+    """The segment kernel forced onto shapes that normally take a thread per trace, with
+    segment lengths from 2 window starts (every segment is one or two windows) to more
+    than a trace (one segment), several traces per thread pass, tiles of 1 to 64 traces, two
+    to four stages; n_samples a multiple of 8 (one bulk copy per trace, padded stride) or not
+    (dense tiles)."""
+    import paper_1307_6489_b200 as rta
+    rng = np.random.default_rng(L * 1000 + S)
+    for E, P in ((1, 1), (2, 37), (3, 1855)):
+        if E * P * S > 3_000_000:
+            P = max(1, 3_000_000 // (E * S))
+        wf = _tie_heavy(rng, E, P, S, 4096)
+        ped = rng.integers(-70000, 70000, P).astype(np.int32)
+        gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
+        want = oracle.extract(wf, ped, gain, W)
+        rta.rta_debug_seg_tuning(L, TR, NT, ST)
+        try:
+            got = run_gpu(wf, ped, gain, W)
+        finally:
+            rta.rta_debug_seg_tuning(0, 0, 0, 0)
+        assert bit_identical(got, want), (E, P)
 
 
 @pytest.mark.parametrize("lpt", [4, 8, 16, 32])
