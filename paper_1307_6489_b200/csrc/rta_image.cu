@@ -714,15 +714,29 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
     if (len != 0) tma_bulk_g2s(row_s, reinterpret_cast<const void*>(lo), len, bar);
   };
 
-  const uint32_t stride = gridDim.x * WARPS;
-  uint32_t e = blockIdx.x * WARPS + warp;
-  if (lane == 0 && e < n_events) issue(e);
+  // The CTA owns a contiguous range of events; its warps draw them from a shared-memory
+  // counter (with a fixed warp -> event map the CTA waits for the warps that have one
+  // event more than the others: 7 against 6.1 on C3). Lane 0 draws the next index when
+  // it hands the row buffer back, so the copy of that row is issued a whole event ahead.
+  __shared__ uint32_t next_event;
+  const uint32_t ev_lo = (uint32_t)(((uint64_t)n_events * blockIdx.x) / gridDim.x);
+  const uint32_t ev_hi = (uint32_t)(((uint64_t)n_events * (blockIdx.x + 1u)) / gridDim.x);
+  if (threadIdx.x == 0) next_event = ev_lo + WARPS;
+  uint32_t e = ev_lo + warp, e_next = ev_hi;
+  if (lane == 0 && e < ev_hi) issue(e);
   // the table copy and check overlap the first loads
   bool symmetric;
   if constexpr (S16) {
-    for (int i = threadIdx.x; i < 6 * P; i += 32 * WARPS) {
-      const int n = __ldg(cam.neighbors + i);
-      nbr16[i] = (unsigned)n < (unsigned)P ? (uint16_t)n : (uint16_t)0xFFFFu;
+    // eight loads in flight per thread (one at a time this copy was 8 % of the kernel)
+    constexpr int step = 32 * WARPS;
+    for (int i0 = threadIdx.x; i0 < 6 * P; i0 += 8 * step) {
+      int v[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) v[u] = i0 + u * step < 6 * P ? __ldg(cam.neighbors + i0 + u * step) : -1;
+#pragma unroll
+      for (int u = 0; u < 8; ++u)
+        if (i0 + u * step < 6 * P)
+          nbr16[i0 + u * step] = (unsigned)v[u] < (unsigned)P ? (uint16_t)v[u] : (uint16_t)0xFFFFu;
     }
     __syncthreads();
     symmetric = table_is_symmetric_s16(nbr16, P) && !force_general;
@@ -733,7 +747,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
                      (reinterpret_cast<uintptr_t>(cam.neighbors) & 7u) == 0};
   const float thr_p = cam.thr_picture, thr_b = cam.thr_boundary;
   const int NW = (int)mask_words(P), NWF = P >> 5;  // words, full words
-  for (uint32_t k = 0; e < n_events; e += stride, ++k) {
+  for (uint32_t k = 0; e < ev_hi; e = __shfl_sync(0xFFFFFFFFu, e_next, 0), ++k) {
     const uint32_t mis = (uint32_t)((base + (uintptr_t)e * row_bytes) & 15u);
     const float* row = reinterpret_cast<const float*>(mine + mis);
     mbar_wait(bar, k & 1u);
@@ -769,7 +783,10 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
         LowFromRow{row, thr_b}, sc, nbr, cam, out, symmetric,
         [&] {  // every lane is done with the row: the buffer goes back to the copy engine
           __syncwarp();
-          if (lane == 0 && e + stride < n_events) issue(e + stride);
+          if (lane == 0) {
+            e_next = atomicAdd(&next_event, 1u);
+            if (e_next < ev_hi) issue(e_next);
+          }
         },
         cur);
     queue_push(Q, cur, out);
