@@ -489,11 +489,12 @@ def packed_leg(cfg, steps, peak, torch, dl0gen, rta):
             "traces_per_s": cfg.n_traces / avg * 1e3}
 
 
-def ragged_leg(steps, peak, torch, dl0gen, rta, n_events=1000):
+def ragged_leg(steps, peak, torch, dl0gen, rta, n_events=1000, slots=None, label=None):
     """NEXT-3: a mixed-camera array (4 LST-, 10 MST-, 6 SST-like telescopes, the
     cameras of C2/C3/C4), every event holding one block per telescope, through
-    one rta_extract_ragged call (one launch per camera shape)."""
-    m = dl0gen.MixedArray(n_events=n_events)
+    one rta_extract_ragged call (one launch per camera shape). `slots` names
+    another array (the second measurement: cameras without a specialised kernel)."""
+    m = dl0gen.MixedArray(n_events=n_events) if slots is None else dl0gen.MixedArray(slots, n_events)
     ped, gain = m.calib()
     d_wf = torch.zeros(m.n_samples_total, dtype=torch.int16, device="cuda")
     m.fill_cuda(torch, d_wf)
@@ -516,8 +517,8 @@ def ragged_leg(steps, peak, torch, dl0gen, rta, n_events=1000):
     launches = (rta.rta_launch_count() - before) // steps
     avg = sum(per) / len(per)
     algo = m.wf_bytes + 16 * m.n_traces
-    res = {"workload": "mixed array: %d events x (4 x 1855x40 W7 + 10 x 1764x25 W4 + 6 x 2048x128 W8), "
-                       "%d blocks on 16-byte boundaries" % (m.n_events, len(m.blk_tel)),
+    res = {"workload": "mixed array: %d events x (%s), %d blocks on 16-byte boundaries" % (
+               m.n_events, label or "4 x 1855x40 W7 + 10 x 1764x25 W4 + 6 x 2048x128 W8", len(m.blk_tel)),
            "ms_avg": avg, "ms_median": statistics.median(per), "ms_best": min(per),
            "launches_per_call": launches, "tiles": rta.rta_ragged_plan_info(plan, rta.RTA_RAGGED_N_TILES),
            "waveform_bytes": m.wf_bytes, "algorithmic_bytes_per_call": algo,
@@ -1067,7 +1068,7 @@ def main():
         else:
             # the charge row is read once; peak times are gathered for the mask pixels only
             algo_bytes = 4 * cfg.n_traces + ev_bytes
-            kname = "image_moments"
+            kname = "image_moments:%s" % cfg.name      # its DRAM traffic depends on the camera
             bytes_per_trace = 4 + EVENT_OUT_BYTES / cfg.n_pixels
         avg = summ["ms_avg"]
         summ["algorithmic_GBps"] = algo_bytes / avg / 1e6
@@ -1174,6 +1175,11 @@ def main():
                 torch.cuda.empty_cache()
             if "ragged" in legs:
                 out["ragged"] = ragged_leg(max(10, args.steps // 4), peak, torch, dl0gen, rta)
+                torch.cuda.empty_cache()
+                xs = extra_shapes(dl0gen)      # cameras without a specialised kernel: extract_ragged_dyn_kernel
+                out["ragged"]["unspecialised"] = ragged_leg(
+                    max(10, args.steps // 4), peak, torch, dl0gen, rta, n_events=1000,
+                    slots=((xs["X60"], 6), (xs["X96"], 6)), label="6 x 1855x60 W7 + 6 x 2048x96 W8")
                 torch.cuda.empty_cache()
             img = {}
             for name in ("C2", "C3", "C4") if "image" in legs else ():

@@ -244,9 +244,9 @@ class MixedArray:
     def __init__(self, slots=(("C2", 4), ("C3", 10), ("C4", 6)), n_events=1000, align=8):
         self.n_events = int(n_events)
         self.slots = []                                   # (config, rank among its camera)
-        for name, count in slots:
+        for name, count in slots:                         # a config name, or a Config of another shape
             for j in range(count):
-                self.slots.append((CONFIGS[name], j))
+                self.slots.append((CONFIGS[name] if isinstance(name, str) else name, j))
         self.tel_n_pixels = [c.n_pixels for c, _ in self.slots]
         self.tel_n_samples = [c.n_samples for c, _ in self.slots]
         self.tel_W = [c.W for c, _ in self.slots]
