@@ -199,7 +199,11 @@ class ClockSampler:
             try:
                 mhz = float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
                 mask = int(n.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle))
-                self.samples.append((mhz, mask))
+                try:
+                    watts = n.nvmlDeviceGetPowerUsage(self.handle) / 1000.0
+                except Exception:
+                    watts = None
+                self.samples.append((mhz, mask, watts))
             except Exception:
                 pass
             time.sleep(0.001)
@@ -212,6 +216,18 @@ class ClockSampler:
         """Number of samples so far: bracket the timed region with two marks."""
         return len(self.samples) if self.nvml else len(self.lines)
 
+    def window(self, lo, hi):
+        """Clocks and power of the samples [lo, hi) of a running sampler (NVML only), for the
+        secondary legs: an arithmetic-bound leg late in a long run can meet lower clocks."""
+        if not self.nvml or hi <= lo:
+            return None
+        sel = self.samples[lo:hi]
+        sm = [x[0] for x in sel]
+        w = [x[2] for x in sel if x[2] is not None]
+        cap = self.nvml.nvmlClocksThrottleReasonSwPowerCap
+        return {"sm_mhz": statistics.median(sm), "sm_min_mhz": min(sm), "watts_max": max(w) if w else None,
+                "sw_power_cap": any(x[1] & cap for x in sel), "samples": len(sm)}
+
     def stop(self, lo=0, hi=None):
         if self.nvml:
             self.stop_flag.set()
@@ -222,8 +238,8 @@ class ClockSampler:
                     "hw_thermal_slowdown": n.nvmlClocksThrottleReasonHwThermalSlowdown,
                     "sw_thermal_slowdown": n.nvmlClocksThrottleReasonSwThermalSlowdown,
                     "sw_power_cap": n.nvmlClocksThrottleReasonSwPowerCap}
-            reasons = sorted(k for k, b in bits.items() if any(m & b for _, m in sel))
-            sm = [x for x, _ in sel]
+            reasons = sorted(k for k, b in bits.items() if any(x[1] & b for x in sel))
+            sm = [x[0] for x in sel]
             return {"sm_mhz": statistics.median(sm) if sm else None, "sm_min_mhz": min(sm) if sm else None,
                     "sm_max_mhz": self.sm_max, "samples": len(sm), "source": "nvml, timed region only",
                     "reasons": reasons}
@@ -1143,6 +1159,17 @@ def main():
             torch.cuda.empty_cache()
             legs = set(SECONDARY_LEGS if args.legs == "all" else
                        [x for x in args.legs.split(",") if x])
+            leg_sampler = ClockSampler(local, uuid)
+            leg_sampler.start()
+            leg_clocks = {}
+
+            def timed_leg(name, fn):
+                lo = leg_sampler.mark()
+                r = fn()
+                c = leg_sampler.window(lo, leg_sampler.mark())
+                if c:
+                    leg_clocks[name] = c
+                return r
             if legs - set(SECONDARY_LEGS):
                 raise SystemExit("--legs: unknown leg(s) %s" % sorted(legs - set(SECONDARY_LEGS)))
             others = {}
@@ -1165,8 +1192,8 @@ def main():
                 out["family"] = fam
             pk = {}
             for name in ("C2", "C3", "C4") if "packed12" in legs else ():
-                pk[name] = packed_leg(dl0gen.CONFIGS[name], max(10, args.steps // 4), peak,
-                                      torch, dl0gen, rta)
+                pk[name] = timed_leg("packed12." + name, lambda: packed_leg(
+                    dl0gen.CONFIGS[name], max(10, args.steps // 4), peak, torch, dl0gen, rta))
                 torch.cuda.empty_cache()
             if pk:
                 out["packed12"] = pk
@@ -1183,11 +1210,14 @@ def main():
                 torch.cuda.empty_cache()
             img = {}
             for name in ("C2", "C3", "C4") if "image" in legs else ():
-                img[name] = image_leg(dl0gen.CONFIGS[name], max(10, args.steps // 4), peak,
-                                      torch, dl0gen, rta)
+                img[name] = timed_leg("image." + name, lambda: image_leg(
+                    dl0gen.CONFIGS[name], max(10, args.steps // 4), peak, torch, dl0gen, rta))
                 torch.cuda.empty_cache()
             if img:
                 out["image"] = img
+            leg_sampler.stop()
+            if leg_clocks:
+                out["leg_clocks"] = leg_clocks   # whole leg (set-up included): sm clock, peak power
             link = host_link_bandwidth(torch)
             out["e2e"]["host_link_GBps_measured"] = link
             out["e2e"]["frac_of_host_link"] = out["e2e"]["value"] / link

@@ -842,7 +842,7 @@ __global__ void __launch_bounds__(256)
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ __align__(8) uint64_t full_bar[kSegMaxStages];
   __shared__ uint32_t tile_q[kSegMaxStages + 1];
-  __shared__ uint32_t bestk[kSegMaxTR];
+  __shared__ uint32_t bestk_all[kSegMaxStages][kSegMaxTR];  // per stage: tile j + 1 collects keys while tile j is finished
   const int tid = threadIdx.x, NT = blockDim.x;
   const int STAGES = sh.stages, QN = STAGES + 1;
   const int S = sh.S, W = sh.W;
@@ -863,7 +863,7 @@ __global__ void __launch_bounds__(256)
     fence_mbar_init();
     feed.prime();
   }
-  if (tid < kSegMaxTR) bestk[tid] = 0u;  // every key is >= 0 and window 0 of a trace always exists
+  for (int i = tid; i < kSegMaxStages * kSegMaxTR; i += NT) (&bestk_all[0][0])[i] = 0u;  // every key is >= 0 and window 0 always exists
   __syncthreads();
 
   auto tile_traces = [&](const uint32_t tile) {
@@ -920,22 +920,39 @@ __global__ void __launch_bounds__(256)
     }
     mbar_wait(bar_base + 8 * stage, parity);
     const uint16_t* base = reinterpret_cast<const uint16_t*>(smem + stage * sh.stage_bytes);
+    uint32_t* bestk = bestk_all[stage];
     const uint32_t n_q = n_tr * (uint32_t)sh.nslot;
-    for (uint32_t q = tid; q < n_q; q += NT) {
+    const int lane = tid & 31;
+    for (uint32_t q0 = (uint32_t)(tid - lane); q0 < n_q; q0 += NT) {  // whole warps: the key reduction needs every lane
+      const uint32_t q = q0 + (uint32_t)lane;
       uint32_t tr = __umulhi(q, sh.nslot_inv);
       uint32_t seg = q - tr * (uint32_t)sh.nslot;
       if (seg >= (uint32_t)sh.nslot) seg -= (uint32_t)sh.nslot, ++tr;
-      if (seg >= (uint32_t)sh.nseg) continue;  // a padding slot
-      const int t0 = (int)seg * sh.L;
-      const int nw = min(sh.L, sh.n_win - t0);
-      const uint16_t* x = base + tr * stride_hw + t0;
-      uint32_t sum = 0;
+      const bool active = q < n_q && seg < (uint32_t)sh.nseg;  // not past the tile, not a padding slot
+      uint32_t best = 0u;  // every real key is >= 0
+      if (active) {
+        const int t0 = (int)seg * sh.L;
+        const int nw = min(sh.L, sh.n_win - t0);
+        const uint16_t* x = base + tr * stride_hw + t0;
+        uint32_t sum = 0;
 #pragma unroll 4
-      for (int k = 0; k < W; ++k) sum += x[k];
-      const uint32_t best = pairs ? ((W & 1) ? seg_slide_pairs<true>(x, W, nw, sum, mul, KM - (uint32_t)t0)
-                                             : seg_slide_pairs<false>(x, W, nw, sum, mul, KM - (uint32_t)t0))
-                                  : seg_slide_u16(x, W, nw, sum, mul, KM - (uint32_t)t0);
-      atomicMax(&bestk[tr], best);
+        for (int k = 0; k < W; ++k) sum += x[k];
+        best = pairs ? ((W & 1) ? seg_slide_pairs<true>(x, W, nw, sum, mul, KM - (uint32_t)t0)
+                                : seg_slide_pairs<false>(x, W, nw, sum, mul, KM - (uint32_t)t0))
+                     : seg_slide_u16(x, W, nw, sum, mul, KM - (uint32_t)t0);
+      }
+      // the segments of a trace meet in bestk[tr]: one REDUX + one atomic per warp when the warp's
+      // lanes all work on one trace (32 same-address atomics serialise), else one atomic per lane
+      const uint32_t act = __ballot_sync(0xFFFFFFFFu, active);
+      if (act != 0u) {
+        const uint32_t tr_ref = __shfl_sync(0xFFFFFFFFu, tr, __ffs((int)act) - 1);
+        if (__all_sync(0xFFFFFFFFu, !active || tr == tr_ref)) {
+          const uint32_t m = __reduce_max_sync(0xFFFFFFFFu, best);
+          if (lane == 0) atomicMax(&bestk[tr_ref], m);
+        } else if (active) {
+          atomicMax(&bestk[tr], best);
+        }
+      }
     }
     __syncthreads();
     if ((uint32_t)tid < n_tr) {
@@ -954,7 +971,10 @@ __global__ void __launch_bounds__(256)
       __stcs(out_charge + g, r.charge);
       __stcs(out_time + g, r.time);
     }
-    __syncthreads();  // the stage is free and bestk is zero again
+    // The stage may be refilled once the finishing threads are done with it. They all sit in
+    // warp 0 when a tile holds at most 32 traces: the other warps go on to the next tile (its
+    // own stage and key words) without waiting; the next barrier orders everything else.
+    if (TR > 32u) __syncthreads(); else __syncwarp();
     if (tid == 0) {
       const uint32_t next = tile_q[(j + STAGES) % QN];
       if (next < n_tiles) issue(next, stage);
