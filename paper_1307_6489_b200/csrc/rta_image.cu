@@ -108,6 +108,27 @@ struct EventBuf {
   }
 };
 
+// The same for the staged fused kernel, whose extraction threads hand over the start t* of
+// the winning window instead of the peak time (TimeFromWaveform): one byte per pixel
+// (n_samples <= 256), so that more event buffers fit behind the stage rings.
+struct EventBuf8 {
+  float* q;          // [P]
+  uint8_t* tstar;    // [P]
+  uint32_t* core_w;
+  uint32_t* low_w;
+  static __host__ __device__ size_t bytes(int P) {
+    return r16(4u * (size_t)P) + r16((size_t)P) + 2u * r16(4u * mask_words(P));
+  }
+  __device__ __forceinline__ EventBuf8(uint8_t* base, const int P) {
+    q = reinterpret_cast<float*>(base);
+    base += r16(4u * (size_t)P);
+    tstar = base;
+    base += r16((size_t)P);
+    core_w = reinterpret_cast<uint32_t*>(base);
+    low_w = reinterpret_cast<uint32_t*>(base + r16(4u * mask_words(P)));
+  }
+};
+
 // Scratch owned by a cleaning warp: keep / mask bit words and one pixel list of
 // `cap` entries (cap >= 384 = 32 lanes x 12 words, the most one lane's run of
 // words can hold for P <= 12288). A list longer than cap is produced and
@@ -139,6 +160,37 @@ template <class F>
 __device__ __forceinline__ int compact_bits(const int NW, int& w_begin, uint16_t* __restrict__ list,
                                             const int cap, F word) {
   const int lane = threadIdx.x & 31;
+  if (NW <= 64 && w_begin == 0) {
+    // cameras of up to 2048 pixels (every BASELINE shape): lane l owns words 2 l and 2 l + 1,
+    // read once into registers; one round unless the list is too short for the bits
+    const int w0 = 2 * lane;
+    uint32_t b0 = w0 < NW ? word(w0) : 0u, b1 = w0 + 1 < NW ? word(w0 + 1) : 0u;
+    const int c = __popc(b0) + __popc(b1);
+    int incl = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+      if (lane >= o) incl += v;
+    }
+    const int total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    if (total <= cap) {
+      int off = incl - c;
+      const int base = 64 * lane;
+      while (b0) {
+        const int b = __ffs((int)b0) - 1;
+        b0 &= b0 - 1u;
+        list[off++] = (uint16_t)(base + b);
+      }
+      while (b1) {
+        const int b = __ffs((int)b1) - 1;
+        b1 &= b1 - 1u;
+        list[off++] = (uint16_t)(base + 32 + b);
+      }
+      w_begin = NW;
+      __syncwarp();
+      return total;
+    }
+  }
   const int K = (NW + 31) >> 5;
   const int w_lo = min(w_begin + lane * K, NW), w_hi = min(w_lo + K, NW);
   int c = 0;
@@ -243,7 +295,7 @@ __device__ __forceinline__ int neighbour_pass(const int n, const uint16_t* __res
 // Peak time of pixel p for the moment sums: from an array, or recomputed from the
 // waveform for the fused staged kernel, whose extraction threads leave step a7
 // out (only the few mask pixels of an event ever need a peak time; the samples
-// are still in L2). tstar[p] holds the bits of t*; the same finish_trace as in
+// are still in L2). tstar[p] holds t*; the same finish_trace as in
 // the extraction gives the same bits.
 struct TimeFromArray {
   const float* t;
@@ -251,12 +303,12 @@ struct TimeFromArray {
 };
 struct TimeFromWaveform {
   const uint16_t* wf;  // the event's first sample (global memory)
-  const float* tstar;  // [P], bit patterns of t*
+  const uint8_t* tstar;  // [P], t*
   const int* pedestal;
   const float* gain;
   int S, W;
   __device__ __forceinline__ float operator()(const int p) const {
-    const int ts = __float_as_int(tstar[p]);
+    const int ts = (int)tstar[p];
     const uint16_t* x = wf + (size_t)p * (size_t)S + ts;
     int rawsum = 0, relnum = 0;
     for (int k = 0; k < W; ++k) {
@@ -287,8 +339,13 @@ struct LowFromRow {
 // pixels does both steps of the cleaning. A core pixel with a core neighbour is
 // kept: its own bit goes into mask_w, and so does every neighbour that passes
 // the boundary threshold. Returns "any pixel kept" per lane.
+// Two forms with the same result. One pass (symmetric_pass_one): every core pixel tests its
+// neighbours for both thresholds at once: the shorter chain of dependent steps, which is
+// what the fused kernels' few cleaning warps are bound by (their table is in global
+// memory). Two phases (symmetric_pass): fewer instructions (the boundary tests run for the
+// kept pixels only), which is what image_moments_kernel is bound by (measured both ways).
 template <class Low>
-__device__ __forceinline__ int symmetric_pass(const int n, const uint16_t* __restrict__ list,
+__device__ __forceinline__ int symmetric_pass_one(const int n, const uint16_t* __restrict__ list,
                                               const NbrTable& nbr, const int P,
                                               const uint32_t* core_w, const Low& low,
                                               uint32_t* mask_w) {
@@ -330,6 +387,68 @@ __device__ __forceinline__ int symmetric_pass(const int n, const uint16_t* __res
   }
   __syncwarp();
   return any;
+}
+
+template <class Low>
+__device__ __forceinline__ int symmetric_pass(const int n, uint16_t* __restrict__ list,
+                                              const NbrTable& nbr, const int P,
+                                              const uint32_t* core_w, const Low& low,
+                                              uint32_t* mask_w) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t lt = (1u << lane) - 1u;
+  constexpr int U = 2;
+  // Phase A: which core pixels have a core neighbour? Those are kept: their own mask bit is
+  // set and they move to the front of the list (most core pixels of a sparse image are
+  // isolated noise, so the boundary tests and mask updates below run for a few entries only).
+  int n_kept = 0;
+  for (int i0 = 0; i0 < n; i0 += 32 * U) {
+    int p[U];
+    bool hit[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int i = i0 + 32 * u + lane;
+      p[u] = i < n ? (int)list[i] : -1;
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      hit[u] = false;
+      if (p[u] >= 0) {
+        int nb[6];
+        nbr.row(p[u], nb);
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+          const bool ok = (unsigned)nb[j] < (unsigned)P;
+          const int m = ok ? nb[j] : 0;
+          if (ok && ((core_w[m >> 5] >> (m & 31)) & 1u)) hit[u] = true;
+        }
+      }
+    }
+    __syncwarp();  // every entry of the round has been read: the front of the list may be rewritten
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const uint32_t bal = __ballot_sync(0xFFFFFFFFu, hit[u]);
+      if (hit[u]) {
+        list[n_kept + __popc(bal & lt)] = (uint16_t)p[u];
+        atomicOr(&mask_w[p[u] >> 5], 1u << (p[u] & 31));
+      }
+      n_kept += __popc(bal);
+    }
+  }
+  __syncwarp();
+  // Phase B: every kept pixel marks those of its neighbours that pass the boundary threshold.
+  for (int i = lane; i < n_kept; i += 32) {
+    const int p = (int)list[i];
+    int nb[6];
+    nbr.row(p, nb);
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+      const bool ok = (unsigned)nb[j] < (unsigned)P;
+      const int m = ok ? nb[j] : 0;
+      if (ok && low(m)) atomicOr(&mask_w[m >> 5], 1u << (m & 31));
+    }
+  }
+  __syncwarp();
+  return n_kept;  // the same in every lane
 }
 
 // Every thread of the CTA: is the neighbour table symmetric? One (pixel, slot)
@@ -443,7 +562,7 @@ __device__ __forceinline__ double shfl_xor_f64(const double v, const int o) {
 // for the symmetric pass; q points at the event's charges (shared or global
 // memory) and t(p) gives pixel p's peak time. `after_pass()` runs once the threshold tests are
 // over (the moments kernel hands its row buffer back to the copy engine there).
-template <class Time, class Low, class AfterPass>
+template <bool TWO_PHASE, class Time, class Low, class AfterPass>
 __device__ __forceinline__ void clean_event_sums(const uint32_t e, const int P, const float* q,
                                                  const Time& t, const uint32_t* core_w,
                                                  const uint32_t* low_w, const Low& low,
@@ -466,7 +585,8 @@ __device__ __forceinline__ void clean_event_sums(const uint32_t e, const int P, 
     __syncwarp();
     for (int wb = 0; wb < NW;) {
       const int n_core = compact_bits(NW, wb, sc.list, sc.cap, [&](int w) { return core_w[w]; });
-      kept |= symmetric_pass(n_core, sc.list, nbr, P, core_w, low, sc.mask_w);
+      kept |= TWO_PHASE ? symmetric_pass(n_core, sc.list, nbr, P, core_w, low, sc.mask_w)
+                        : symmetric_pass_one(n_core, sc.list, nbr, P, core_w, low, sc.mask_w);
     }
   } else {
     // keep[p] = core[p] and some neighbour is core (isolated core pixels drop)
@@ -562,7 +682,7 @@ __device__ __forceinline__ void clean_event(const uint32_t e, const int P, const
                                             const bool symmetric, Pending& pd, int& n_pend) {
   const NbrTable nbr{cam.neighbors, nullptr, (reinterpret_cast<uintptr_t>(cam.neighbors) & 7u) == 0};
   EventSums cur;
-  clean_event_sums(e, P, q, t, core_w, low_w, LowFromBits{low_w}, sc, nbr, cam, out, symmetric,
+  clean_event_sums<false>(e, P, q, t, core_w, low_w, LowFromBits{low_w}, sc, nbr, cam, out, symmetric,
                    [] {}, cur);
   if ((int)(threadIdx.x & 31) == n_pend) pd = cur;
   if (++n_pend == 32) flush_pending(pd, n_pend, out);
@@ -778,7 +898,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
     if (!symmetric) sweep(thr_b, low_w);  // the general path asks for every boundary candidate
     __syncwarp();
     EventSums cur;
-    clean_event_sums(
+    clean_event_sums<true>(
         e, P, charge + (size_t)e * (size_t)P, TimeFromArray{time + (size_t)e * (size_t)P}, core_w, low_w,
         LowFromRow{row, thr_b}, sc, nbr, cam, out, symmetric,
         [&] {  // every lane is done with the row: the buffer goes back to the copy engine
@@ -908,10 +1028,11 @@ __global__ void __launch_bounds__(NT + 32)
 //               nt * NT / 32 arrivals per phase; the cleaning warp waits
 //   freeb[b]    one arrival by the cleaning warp per cleaned event; the extraction
 //               threads wait before the first write of event k >= NB
-constexpr int kMaxBuf = 8;
-constexpr int kCleanRegs = 152;  // cleaning warpgroup after the register split (multiple of 8)
+constexpr int kMaxBuf = 12;
+constexpr int kFusedListCap = 512;  // entries of a cleaning warp's pixel list (longer lists go in rounds)
 
-template <class C, int G, int NCMAX, int XREGS>
+// XREGS / CREGS: registers per thread of the extraction / cleaning warpgroups after the split
+template <class C, int G, int NCMAX, int XREGS, int CREGS>
 __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
     extract_image_kernel(const uint8_t* __restrict__ wf, const uint32_t n_events, const int P,
                          const int* __restrict__ pedestal, const float* __restrict__ gain,
@@ -921,6 +1042,7 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
   static_assert(C::BITS == 16 && C::STAGES >= 2, "uint16 samples, at least two stages");
   static_assert(C::TPT == 1 || C::TPT == 2, "one or two traces per thread");
   static_assert(G >= 1 && G <= 14, "named barriers 1 .. G");
+  static_assert(C::S <= 256, "t* travels as one byte");
   // an event may start at any multiple of VEC bytes: the copy starts at the
   // 16-byte boundary below it, so a stage holds up to 16 bytes more than a tile
   constexpr int STG = C::STAGE_BYTES + 16;
@@ -933,7 +1055,7 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
   const int tid = threadIdx.x, lane = tid & 31;
   const uint32_t nt = ((uint32_t)P + C::TILE_TRACES - 1u) / C::TILE_TRACES;  // tiles per event
   uint8_t* ev_base = smem + (size_t)G * C::STAGES * STG;
-  const size_t eb = EventBuf::bytes(P);
+  const size_t eb = EventBuf8::bytes(P);
   const uint32_t ready0 = smem_u32(ready_bar), free0 = smem_u32(free_bar);
 
   if (tid == 0) {
@@ -952,23 +1074,24 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
   // Register split (whole warpgroups only): the extraction code needs 48-56
   // registers (XREGS, tuned per shape), the cleaning code about 130; the CTA is
   // launched with the same number for everyone and the warpgroups trade them here.
-  constexpr bool REGSPLIT = (NX % 128 == 0) && (NCMAX == 4);
+  constexpr bool REGSPLIT = (NX % 128 == 0) && (NCMAX % 4 == 0);
 
   if (tid >= NX) {  // ------------------------------------------------ cleaning warps
-    if constexpr (REGSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kCleanRegs));
+    if constexpr (REGSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(CREGS));
     const bool symmetric = table_is_symmetric(cam.neighbors, P) && !force_general;
     const int c = (tid - NX) >> 5;
     if (c >= NC) return;
-    const CleanScratch sc(ev_base + (size_t)NB * eb + (size_t)c * CleanScratch::bytes(P, P), P, P);
+    const CleanScratch sc(ev_base + (size_t)NB * eb + (size_t)c * CleanScratch::bytes(P, kFusedListCap), P,
+                          kFusedListCap);
     Pending pd = {};
     int n_pend = 0;
     for (uint32_t k = (uint32_t)c; event_of(k) < n_events; k += (uint32_t)NC) {
       const uint32_t b = k % (uint32_t)NB, use = k / (uint32_t)NB;
       mbar_wait_idle(ready0 + 8 * b, use & 1u);
-      const EventBuf buf(ev_base + (size_t)b * eb, P);
+      const EventBuf8 buf(ev_base + (size_t)b * eb, P);
       const uint32_t ev = event_of(k);
       const TimeFromWaveform tw{reinterpret_cast<const uint16_t*>(wf) + (size_t)ev * (size_t)P * C::S,
-                                buf.t, pedestal, gain, C::S, C::W};
+                                buf.tstar, pedestal, gain, C::S, C::W};
       clean_event(ev, P, buf.q, tw, buf.core_w, buf.low_w, sc, cam, out, symmetric, pd, n_pend);
       __syncwarp();
       if (lane == 0) mbar_arrive(free0 + 8 * b);
@@ -1063,7 +1186,7 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
       cur_ev = ev;
       if (cc.use != 0) mbar_wait(free0 + 8 * b, (cc.use - 1u) & 1u);
     }
-    const EventBuf buf(ev_base + (size_t)b * eb, P);
+    const EventBuf8 buf(ev_base + (size_t)b * eb, P);
     mbar_wait(bar_base + 8 * stage, parity);
     const uint32_t p0 = tile * C::TILE_TRACES + (uint32_t)gt * C::TPT;
     float qv[C::TPT];
@@ -1080,7 +1203,7 @@ __global__ void __launch_bounds__(G * C::NT + 32 * NCMAX, 1)
 #pragma unroll
       for (int i = 0; i < C::TPT; ++i) {  // P is a multiple of TPT: the unit is whole
         buf.q[p0 + i] = qv[i] = res[i].charge;
-        buf.t[p0 + i] = res[i].time;
+        buf.tstar[p0 + i] = (uint8_t)__float_as_int(res[i].time);
       }
     }
     // threshold bits of this warp's 32 * TPT pixels (warps past the camera's end write nothing)
@@ -1158,10 +1281,10 @@ std::atomic<bool> g_general_cleaning{false};  // tests: never take the symmetric
 #ifndef RTA_I128_NC
 #define RTA_I128_NC 2
 #endif
-template <class C_, int G_, int NCMAX_, int XREGS_ = 56>
+template <class C_, int G_, int NCMAX_, int XREGS_ = 56, int CREGS_ = 152>
 struct ImgCfg {
   using C = C_;
-  static constexpr int G = G_, NCMAX = NCMAX_, XREGS = XREGS_;
+  static constexpr int G = G_, NCMAX = NCMAX_, XREGS = XREGS_, CREGS = CREGS_;
   static constexpr int THREADS = G * C::NT + 32 * NCMAX;
   static constexpr size_t RING = (size_t)G * C::STAGES * (C::STAGE_BYTES + 16);
   static_assert(THREADS <= 1024, "one CTA");
@@ -1169,24 +1292,33 @@ struct ImgCfg {
   // warpgroups trade registers inside what the CTA was launched with, which is
   // the launch bound's cap (ptxas allocates it in full when setmaxnreg is used);
   // a split that does not fit would leave setmaxnreg.inc waiting for ever
-  static constexpr bool REGSPLIT = ((G * C::NT) % 128 == 0) && (NCMAX == 4);
+  static constexpr bool REGSPLIT = ((G * C::NT) % 128 == 0) && (NCMAX % 4 == 0);
   static constexpr int LAUNCH_REGS = ((65536 / THREADS) / 8) * 8;
-  static constexpr int SPLIT_REGS = G * C::NT * XREGS + 32 * NCMAX * kCleanRegs;
+  static constexpr int SPLIT_REGS = G * C::NT * XREGS + 32 * NCMAX * CREGS;
   static_assert(!REGSPLIT || SPLIT_REGS <= THREADS * LAUNCH_REGS, "register split exceeds the CTA's pool");
 };
 #ifndef RTA_I30_XREGS
 #define RTA_I30_XREGS 56
 #endif
-using ImgS30W7 = ImgCfg<TileCfg<30, 7, RTA_I30_NT, 2>, RTA_I30_G, RTA_IMG_NC, RTA_I30_XREGS>;
+#ifndef RTA_I30_CREGS
+#define RTA_I30_CREGS 152
+#endif
+using ImgS30W7 = ImgCfg<TileCfg<30, 7, RTA_I30_NT, 2>, RTA_I30_G, RTA_IMG_NC, RTA_I30_XREGS, RTA_I30_CREGS>;
 // 48 registers for the S = 40 extraction code: 0.253 ms on C2 against 0.268 ms at 56 (and 0.290 at 40)
 #ifndef RTA_I40_XREGS
 #define RTA_I40_XREGS 56
 #endif
-using ImgS40W7 = ImgCfg<TileCfg<40, 7, RTA_I40_NT, 2>, RTA_I40_G, RTA_IMG_NC, RTA_I40_XREGS>;
+#ifndef RTA_I40_CREGS
+#define RTA_I40_CREGS 152
+#endif
+using ImgS40W7 = ImgCfg<TileCfg<40, 7, RTA_I40_NT, 2>, RTA_I40_G, RTA_IMG_NC, RTA_I40_XREGS, RTA_I40_CREGS>;
 #ifndef RTA_I25_XREGS
 #define RTA_I25_XREGS 64
 #endif
-using ImgS25W4 = ImgCfg<TileCfg<25, 4, RTA_I25_NT, 2>, RTA_I25_G, RTA_IMG_NC, RTA_I25_XREGS>;
+#ifndef RTA_I25_CREGS
+#define RTA_I25_CREGS 152
+#endif
+using ImgS25W4 = ImgCfg<TileCfg<25, 4, RTA_I25_NT, 2>, RTA_I25_G, RTA_IMG_NC, RTA_I25_XREGS, RTA_I25_CREGS>;
 using ImgS128W8 = ImgCfg<TileCfg<128, 8, RTA_I128_NT, 2>, RTA_I128_G, RTA_I128_NC>;
 
 // Cleaning warps NC and event buffers NB = NC + 1 that fit behind the ring
@@ -1194,8 +1326,8 @@ using ImgS128W8 = ImgCfg<TileCfg<128, 8, RTA_I128_NT, 2>, RTA_I128_G, RTA_I128_N
 template <class I>
 int fused_cleaners(int32_t P) {
   for (int nc = I::NCMAX; nc >= 1; --nc) {
-    const size_t need = I::RING + (size_t)(nc + 1) * EventBuf::bytes(P) +
-                        (size_t)nc * CleanScratch::bytes(P, P) + 1024u;
+    const size_t need = I::RING + (size_t)(nc + 1) * EventBuf8::bytes(P) +
+                        (size_t)nc * CleanScratch::bytes(P, kFusedListCap) + 1024u;
     if (need <= kSmemLimit) return nc;
   }
   return 0;
@@ -1225,13 +1357,14 @@ struct FusedLauncher {
     if ((e = rta_device_sms(dev, &sms)) != cudaSuccess) return e;
     const int nc = fused_cleaners<I>(P);
     int nb = nc + 1;
-    size_t smem = I::RING + (size_t)nb * EventBuf::bytes(P) + (size_t)nc * CleanScratch::bytes(P, P);
-    // one more buffer when there is room: the extraction groups run further ahead
-    if (nb + 1 <= kMaxBuf && smem + EventBuf::bytes(P) + 1024u <= kSmemLimit) {
+    size_t smem = I::RING + (size_t)nb * EventBuf8::bytes(P) +
+                  (size_t)nc * CleanScratch::bytes(P, kFusedListCap);
+    // more buffers while there is room: the extraction groups run further ahead
+    while (nb + 1 <= kMaxBuf && nb < nc + 3 && smem + EventBuf8::bytes(P) + 1024u <= kSmemLimit) {
       ++nb;
-      smem += EventBuf::bytes(P);
+      smem += EventBuf8::bytes(P);
     }
-    auto kernel = extract_image_kernel<C, I::G, I::NCMAX, I::XREGS>;
+    auto kernel = extract_image_kernel<C, I::G, I::NCMAX, I::XREGS, I::CREGS>;
     if (I::REGSPLIT) {  // never launch a split that the allocated registers cannot serve
       cudaFuncAttributes fa;
       if ((e = cudaFuncGetAttributes(&fa, kernel)) != cudaSuccess) return e;
