@@ -662,6 +662,7 @@ struct rta_ragged_plan {
   RtaRaggedTile* tiles_dev = nullptr;  // all classes, one after the other
   struct Class {
     int32_t S, W;
+    int32_t tile_traces;    // what the class's tiles were cut for (rta_ragged_tile_traces at plan time)
     uint32_t first, count;  // range in tiles_dev
   };
   std::vector<Class> classes;
@@ -689,6 +690,7 @@ int rta_ragged_plan_create(int32_t n_tel, const int32_t* tel_n_pixels,
   if (!pl) return RTA_ERR_NOMEM;
   // tiles grouped by shape class, blocks in table order inside a class
   std::map<std::pair<int32_t, int32_t>, std::vector<RtaRaggedTile>> by_shape;
+  std::map<std::pair<int32_t, int32_t>, int> tile_of;  // tile size per shape class, asked once
   for (int64_t b = 0; b < n_blocks; ++b) {
     const int32_t k = blk_tel[b];
     if (k < 0 || k >= n_tel || blk_wf_offset[b] < 0 || blk_out_offset[b] < 0) {
@@ -707,8 +709,12 @@ int rta_ragged_plan_create(int32_t n_tel, const int32_t* tel_n_pixels,
       delete pl;
       return RTA_ERR_UNSUPPORTED;
     }
-    const int64_t tt = rta_ragged_tile_traces((int32_t)S, tel_W[k]);
-    std::vector<RtaRaggedTile>& v = by_shape[std::make_pair((int32_t)S, tel_W[k])];
+    const auto shape = std::make_pair((int32_t)S, tel_W[k]);
+    auto tile_it = tile_of.find(shape);
+    if (tile_it == tile_of.end())
+      tile_it = tile_of.emplace(shape, rta_ragged_tile_traces((int32_t)S, tel_W[k])).first;
+    const int64_t tt = tile_it->second;
+    std::vector<RtaRaggedTile>& v = by_shape[shape];
     for (int64_t t0 = 0; t0 < P; t0 += tt) {
       const int64_t n = (P - t0 < tt) ? P - t0 : tt;
       RtaRaggedTile t;
@@ -732,6 +738,7 @@ int rta_ragged_plan_create(int32_t n_tel, const int32_t* tel_n_pixels,
     rta_ragged_plan::Class c;
     c.S = kv.first.first;
     c.W = kv.first.second;
+    c.tile_traces = tile_of[kv.first];
     c.first = (uint32_t)all.size();
     c.count = (uint32_t)kv.second.size();
     pl->classes.push_back(c);
@@ -853,7 +860,7 @@ int rta_extract_ragged(const rta_ragged_plan* plan, const uint16_t* wf, const in
         used = k + 1;
       }
     }
-    e = rta_launch_ragged(wf, plan->tiles_dev + c.first, c.count, c.S, c.W, pedestal, gain,
+    e = rta_launch_ragged(wf, plan->tiles_dev + c.first, c.count, c.S, c.W, c.tile_traces, pedestal, gain,
                           out_sum, out_start, out_charge, out_time, st);
     if (e != cudaSuccess && first_err == cudaSuccess) first_err = e;
   }

@@ -20,6 +20,12 @@ typedef unsigned long long uintptr_t;
 #include <cuda_runtime.h>
 #include <stdint.h>
 #endif
+// Mixed-camera batches: one entry per tile (at most rta_ragged_tile_traces(S, W) traces of one block).
+struct alignas(16) RtaRaggedTile {
+  unsigned long long src;  // byte offset of the tile's first trace in wf | n_traces << 48
+  uint32_t out_base;       // flat output index of the first trace
+  uint32_t cal0;           // calibration index of the first trace
+};
 enum { RTA_MODE_SLIDING = 0, RTA_MODE_FIXED = 1, RTA_MODE_LOCAL_PEAK = 2, RTA_MODE_FIR = 3 };
 struct RtaMode {
   int kind;
@@ -49,17 +55,15 @@ bool rta_dyn_eligible(int32_t n_samples, int32_t W);
 // Name of the kernel the dispatcher picks (static string).
 const char* rta_pick_kernel_name(int32_t n_samples, int32_t W, bool aligned16, int bits = 16);
 
-// Mixed-camera batches (include/rta.h rta_ragged_plan_*): one entry per tile of
-// at most rta_ragged_tile_traces(S, W) traces of one block.
-struct alignas(16) RtaRaggedTile {
-  unsigned long long src;  // byte offset of the tile's first trace in wf | n_traces << 48
-  uint32_t out_base;       // flat output index of the first trace
-  uint32_t cal0;           // calibration index of the first trace
-};
+// Mixed-camera batches (include/rta.h rta_ragged_plan_*): how many traces of one block a
+// tile of shape (S, W) holds at most, decided when the plan is made: the tile of the
+// ahead-of-time kernel, else of the run-time specialisation (when the compiler is there),
+// else of the runtime-shape kernel.
 int rta_ragged_tile_traces(int32_t n_samples, int32_t W);
 // One launch over a device-resident tile table whose tiles all have shape (S, W).
+// `tile_traces` is what rta_ragged_tile_traces gave when the table was cut.
 cudaError_t rta_launch_ragged(const void* wf, const RtaRaggedTile* tiles_dev, uint32_t n_tiles,
-                              int32_t n_samples, int32_t W, const int32_t* pedestal,
+                              int32_t n_samples, int32_t W, int32_t tile_traces, const int32_t* pedestal,
                               const float* gain, int32_t* out_sum, int32_t* out_start,
                               float* out_charge, float* out_time, cudaStream_t stream);
 
@@ -130,6 +134,21 @@ bool rta_jit_eligible(int32_t n_samples, int32_t W);   // shape fits a register 
 bool rta_jit_available();                              // ... and libnvrtc could be loaded
 cudaError_t rta_jit_launch(int32_t n_samples, int32_t W, int mode, const RtaJitArgs& a,
                            const void* mode_args, size_t mode_args_bytes, cudaStream_t stream);
+// The same for a tile table of a mixed-camera batch (sliding extractor). rta_jit_tile_traces:
+// traces per tile of the specialisation of (S, W), 0 when there is none (not eligible, no compiler).
+struct RtaJitRaggedArgs {
+  const void* wf;
+  const RtaRaggedTile* tiles;
+  uint32_t n_tiles;
+  const int32_t* pedestal;
+  const float* gain;
+  int32_t *out_sum, *out_start;
+  float *out_charge, *out_time;
+  uint32_t* sched;
+};
+int rta_jit_tile_traces(int32_t n_samples, int32_t W);
+cudaError_t rta_jit_launch_ragged(int32_t n_samples, int32_t W, const RtaJitRaggedArgs& a,
+                                  cudaStream_t stream);
 void rta_jit_enable(bool on);   // tests: switch the run-time specialisations off / on
 void rta_jit_release();         // rta_shutdown
 #endif  // __CUDACC_RTC__

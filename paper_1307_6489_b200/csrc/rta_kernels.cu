@@ -329,14 +329,8 @@ __global__ void __launch_bounds__(256)
 // S = 128 layout); a 4-byte-aligned one by 4-byte cp.async; anything else by
 // plain halfword copies. Every thread arrives on the stage's mbarrier through
 // cp.async.mbarrier.arrive, so the three ways share one completion mechanism.
-using RaggedTile = RtaRaggedTile;  // rta_internal.h: {src offset | n << 48, out_base, cal0}
-constexpr unsigned long long kRaggedOffMask = (1ull << 48) - 1ull;
-
-__device__ __forceinline__ void mbar_expect_tx_only(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes)
-               : "memory");
-}
-
+// (RaggedTile, the ingest helpers and the kernel body live in rta_tile_kernel.cuh: the run-time
+// specialisations compile the same source)
 template <class C>
 __global__ void __launch_bounds__(C::NT)
     extract_ragged_kernel(const uint8_t* __restrict__ wf, const RaggedTile* __restrict__ tiles,
@@ -345,129 +339,8 @@ __global__ void __launch_bounds__(C::NT)
                           int* __restrict__ out_start, float* __restrict__ out_charge,
                           float* __restrict__ out_time, const int vec_store,
                           uint32_t* __restrict__ sched) {
-  static_assert(C::BITS == 16 && C::STAGES >= 2, "uint16 blocks, at least two stages");
-  extern __shared__ __align__(128) uint8_t smem[];
-  __shared__ __align__(8) uint64_t full_bar[C::STAGES];
-  constexpr int QN = C::STAGES + 1;
-  __shared__ uint32_t tile_q[QN];
-  // the table entry of every queued tile, fetched by thread 0 one iteration
-  // ahead together with the index: no thread waits on a dependent global load
-  __shared__ RaggedTile desc_q[QN];
-  const int tid = threadIdx.x;
-  const uint32_t smem_base = smem_u32(smem);
-  const uint32_t bar_base = smem_u32(full_bar);
-  const ModeArgs ma = {};
-
-  // tile indices: the first STAGES of a CTA are static (blockIdx.x + k * gridDim.x),
-  // the rest come from the shared counter, one run of tiles per atomic
-  TileFeed feed(sched, n_tiles, C::STAGES);  // thread 0 only
-
-  const auto entry = [&](const uint32_t ti) -> RaggedTile {
-    if (ti < n_tiles) return tiles[ti];
-    return RaggedTile{0ull, 0u, 0u};
-  };
-  if (tid == 0) {
-#pragma unroll
-    for (int s = 0; s < C::STAGES; ++s) {
-      mbar_init(bar_base + 8 * s, C::NT);
-      tile_q[s] = feed.fetch_static();
-      desc_q[s] = entry(tile_q[s]);
-    }
-    fence_mbar_init();
-    feed.prime();
-  }
-  __syncthreads();
-
-  constexpr uint32_t UB = C::UNIT_BYTES, PADB = C::UNIT_STRIDE - C::UNIT_BYTES;
-  constexpr uint32_t TRACE_BYTES = C::TRACE_BITS / 8;
-  auto issue = [&](const int slot, const int stage) {
-    const RaggedTile t = desc_q[slot];
-    const uint8_t* src = wf + (size_t)(t.src & kRaggedOffMask);
-    const uint32_t bytes = (uint32_t)(t.src >> 48) * TRACE_BYTES;
-    uint8_t* dstp = smem + stage * C::STAGE_BYTES;
-    const uint32_t dst = smem_base + stage * C::STAGE_BYTES;
-    const uint32_t bar = bar_base + 8 * stage;
-    const uint32_t mis = (uint32_t)(reinterpret_cast<uintptr_t>(src) & 15u);
-    uint32_t done;  // bytes moved by the wide path; the rest goes halfword by halfword
-    if (mis == 0) {
-      if constexpr (!C::PAD) {
-        done = bytes & ~15u;
-        if (tid == 0 && done != 0) {
-          mbar_expect_tx_only(bar, done);
-          tma_bulk_g2s(dst, src, done, bar);
-        }
-      } else {
-        done = bytes;  // a padded unit is a whole number of 16-byte chunks
-        if (bytes == (uint32_t)C::TILE_BYTES) {  // full tile: compile-time trip count, as the uniform kernel
-#pragma unroll 4
-          for (int c = tid; c < C::TILE_BYTES / 16; c += C::NT) {
-            const int u = c / C::NVEC;
-            cp_async16(dst + (uint32_t)(c + u) * 16u, src + (size_t)c * 16);
-          }
-        } else {
-          for (uint32_t c = tid; c < bytes / 16u; c += C::NT)
-            cp_async16(dst + (c + c / (UB / 16u)) * 16u, src + (size_t)c * 16u);
-        }
-      }
-    } else if ((mis & 3u) == 0) {
-      done = bytes & ~3u;
-      for (uint32_t c = tid; c < done / 4u; c += C::NT) {
-        uint32_t d = c * 4u;
-        if constexpr (C::PAD) d += (d / UB) * PADB;
-        cp_async4(dst + d, src + (size_t)c * 4u);
-      }
-    } else {
-      done = 0;
-    }
-    for (uint32_t b = done + 2u * tid; b < bytes; b += 2u * C::NT) {
-      uint32_t d = b;
-      if constexpr (C::PAD) d += (b / UB) * PADB;
-      *reinterpret_cast<uint16_t*>(dstp + d) = *reinterpret_cast<const uint16_t*>(src + b);
-    }
-    cp_async_mbar_arrive(bar);  // counts once this thread's cp.async copies have landed
-  };
-
-#pragma unroll
-  for (int s = 0; s < C::STAGES; ++s) {
-    const uint32_t tile = tile_q[s];
-    if (tile < n_tiles) issue(s, s);
-  }
-  uint32_t pre = 0;
-  RaggedTile pre_d = {0ull, 0u, 0u};
-  if (tid == 0) {
-    pre = feed.fetch();
-    pre_d = entry(pre);
-  }
-
-  for (uint32_t j = 0;; ++j) {
-    const uint32_t tile = tile_q[j % QN];
-    if (tile >= n_tiles) break;
-    const int stage = (int)(j % C::STAGES);
-    const uint32_t parity = (j / C::STAGES) & 1u;
-    if (tid == 0) {
-      tile_q[(j + C::STAGES) % QN] = pre;
-      desc_q[(j + C::STAGES) % QN] = pre_d;
-      pre = feed.fetch();
-      pre_d = entry(pre);
-    }
-    const RaggedTile t = desc_q[j % QN];
-    const uint32_t n = (uint32_t)(t.src >> 48);
-    mbar_wait(bar_base + 8 * stage, parity);
-    const uint32_t first = (uint32_t)tid * C::TPT;
-    if (first < n) {
-      const uint8_t* unit = smem + stage * C::STAGE_BYTES + tid * C::UNIT_STRIDE;
-      // the calibration index "wraps" after the tile's last trace, so the discarded
-      // second trace of an odd tile reads pedestal[0], never past the arrays
-      compute_unit<C, MODE_SLIDING>(unit, t.out_base + first, n - first, t.cal0 + first,
-                                    t.cal0 + n, pedestal, gain, out_sum, out_start, out_charge,
-                                    out_time, vec_store != 0 && (t.out_base & 1u) == 0, ma);
-    }
-    __syncthreads();
-    const uint32_t next = tile_q[(j + C::STAGES) % QN];
-    if (next < n_tiles) issue((int)((j + C::STAGES) % QN), stage);
-  }
-
-  if (tid == 0) feed.leave();
+  ragged_kernel_body<C>(wf, tiles, n_tiles, pedestal, gain, out_sum, out_start, out_charge, out_time,
+                        vec_store, sched);
 }
 
 // Mixed-camera blocks of a shape without a specialisation: the tile table and
@@ -1254,7 +1127,7 @@ cudaError_t launch_generic(const LaunchArgs& a, const ModeArgs& ma) {
 
 // Shape of the any-shape staged kernel for (S, W); false = not eligible (units
 // above 1152 bytes: the generic kernel takes them).
-bool dyn_shape(int32_t S, int32_t W, DynShape* sh, int* threads) {
+bool dyn_shape(int32_t S, int32_t W, DynShape* sh, int* threads, int force_threads = 0) {
   const int tpt = (S & 1) ? 2 : 1;
   const long long ub = 2ll * S * tpt;
   if (ub > 1152) return false;
@@ -1275,7 +1148,14 @@ bool dyn_shape(int32_t S, int32_t W, DynShape* sh, int* threads) {
     if (warps > 32) warps = 32;
     if (warps > best_warps) best_warps = warps, nt = cand;
   }
-  if (best_warps == 0) return false;
+  if (force_threads != 0) {  // a tile table cut for another tile size (mixed-camera plans)
+    if (force_threads % 32 != 0 || force_threads > 256 ||
+        2 * (((force_threads * stride + 64 + 127) / 128) * 128) + 1024 > 227 * 1024)
+      return false;
+    nt = force_threads;
+  } else if (best_warps == 0) {
+    return false;
+  }
   sh->S = S;
   sh->W = W;
   sh->n_win = S - W + 1;
@@ -1586,6 +1466,8 @@ int rta_ragged_tile_traces(int32_t S, int32_t W) {
   if (S == CfgS40W7::S && W == CfgS40W7::W) return CfgS40W7::TILE_TRACES;
   if (S == CfgS25W4::S && W == CfgS25W4::W) return CfgS25W4::TILE_TRACES;
   if (S == CfgS128W8::S && W == CfgS128W8::W) return CfgS128W8::TILE_TRACES;
+  const int jit = rta_jit_tile_traces(S, W);  // the run-time specialisation of the tile-table kernel
+  if (jit > 0) return jit;
   DynShape sh;
   int threads = 0;
   if (dyn_shape(S, W, &sh, &threads)) return threads * sh.tpt;  // extract_ragged_dyn_kernel
@@ -1593,7 +1475,8 @@ int rta_ragged_tile_traces(int32_t S, int32_t W) {
 }
 
 cudaError_t rta_launch_ragged(const void* wf, const RtaRaggedTile* tiles_dev, uint32_t n_tiles,
-                              int32_t S, int32_t W, const int32_t* pedestal, const float* gain,
+                              int32_t S, int32_t W, int32_t tile_traces, const int32_t* pedestal,
+                              const float* gain,
                               int32_t* out_sum, int32_t* out_start, float* out_charge,
                               float* out_time, cudaStream_t stream) {
   if (n_tiles == 0) return cudaSuccess;
@@ -1611,9 +1494,19 @@ cudaError_t rta_launch_ragged(const void* wf, const RtaRaggedTile* tiles_dev, ui
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
+  // the run-time specialisation, when the table was cut for its tile
+  if (tile_traces == rta_jit_tile_traces(S, W)) {
+    const RtaJitRaggedArgs ja{w, tiles_dev, n_tiles, pedestal, gain, out_sum, out_start, out_charge, out_time,
+                              g_static_schedule ? nullptr : sched_words(dev, stream)};
+    e = rta_jit_launch_ragged(S, W, ja, stream);
+    if (e != cudaErrorNotSupported) return e;
+  }
+  // the runtime-shape kernel with as many threads as a tile has units (the table may have been
+  // cut for the specialisation's tile while the compiler has gone away since)
   DynShape sh;
   int threads = 0;
-  if (dyn_shape(S, W, &sh, &threads)) {
+  const int tpt = (S & 1) ? 2 : 1;
+  if (tile_traces % tpt == 0 && dyn_shape(S, W, &sh, &threads, tile_traces / tpt)) {
     const bool pad = sh.unit_stride != sh.unit_bytes;
     using Kernel = void (*)(const uint8_t*, const RaggedTile*, uint32_t, const int*, const float*,
                             int*, int*, float*, float*, uint32_t*, DynShape);

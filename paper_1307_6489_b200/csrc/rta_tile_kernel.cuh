@@ -192,6 +192,149 @@ __device__ __forceinline__ void tile_kernel_body(
   if (tid == 0) feed.leave();
 }
 
+using RaggedTile = RtaRaggedTile;  // rta_internal.h: {src offset | n << 48, out_base, cal0}
+constexpr unsigned long long kRaggedOffMask = (1ull << 48) - 1ull;
+
+__device__ __forceinline__ void mbar_expect_tx_only(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes)
+               : "memory");
+}
+
+// The body of the mixed-camera tile kernel (one launch per shape class walks its tile
+// table): ahead-of-time for the four BASELINE shapes (extract_ragged_kernel in
+// rta_kernels.cu) and, like the uniform kernel, compiled at run time for any other shape
+// whose unit fits a register copy (rta_jit.cu).
+template <class C>
+__device__ __forceinline__ void ragged_kernel_body(
+    const uint8_t* __restrict__ wf, const RaggedTile* __restrict__ tiles, const uint32_t n_tiles,
+    const int* __restrict__ pedestal, const float* __restrict__ gain, int* __restrict__ out_sum,
+    int* __restrict__ out_start, float* __restrict__ out_charge, float* __restrict__ out_time,
+    const int vec_store, uint32_t* __restrict__ sched) {
+  static_assert(C::BITS == 16 && C::STAGES >= 2, "uint16 blocks, at least two stages");
+  extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t full_bar[C::STAGES];
+  constexpr int QN = C::STAGES + 1;
+  __shared__ uint32_t tile_q[QN];
+  // the table entry of every queued tile, fetched by thread 0 one iteration
+  // ahead together with the index: no thread waits on a dependent global load
+  __shared__ RaggedTile desc_q[QN];
+  const int tid = threadIdx.x;
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t bar_base = smem_u32(full_bar);
+  const ModeArgs ma = {};
+
+  // tile indices: the first STAGES of a CTA are static (blockIdx.x + k * gridDim.x),
+  // the rest come from the shared counter, one run of tiles per atomic
+  TileFeed feed(sched, n_tiles, C::STAGES);  // thread 0 only
+
+  const auto entry = [&](const uint32_t ti) -> RaggedTile {
+    if (ti < n_tiles) return tiles[ti];
+    return RaggedTile{0ull, 0u, 0u};
+  };
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < C::STAGES; ++s) {
+      mbar_init(bar_base + 8 * s, C::NT);
+      tile_q[s] = feed.fetch_static();
+      desc_q[s] = entry(tile_q[s]);
+    }
+    fence_mbar_init();
+    feed.prime();
+  }
+  __syncthreads();
+
+  constexpr uint32_t UB = C::UNIT_BYTES, PADB = C::UNIT_STRIDE - C::UNIT_BYTES;
+  constexpr uint32_t TRACE_BYTES = C::TRACE_BITS / 8;
+  auto issue = [&](const int slot, const int stage) {
+    const RaggedTile t = desc_q[slot];
+    const uint8_t* src = wf + (size_t)(t.src & kRaggedOffMask);
+    const uint32_t bytes = (uint32_t)(t.src >> 48) * TRACE_BYTES;
+    uint8_t* dstp = smem + stage * C::STAGE_BYTES;
+    const uint32_t dst = smem_base + stage * C::STAGE_BYTES;
+    const uint32_t bar = bar_base + 8 * stage;
+    const uint32_t mis = (uint32_t)(reinterpret_cast<uintptr_t>(src) & 15u);
+    uint32_t done;  // bytes moved by the wide path; the rest goes halfword by halfword
+    if (mis == 0) {
+      if constexpr (!C::PAD) {
+        done = bytes & ~15u;
+        if (tid == 0 && done != 0) {
+          mbar_expect_tx_only(bar, done);
+          tma_bulk_g2s(dst, src, done, bar);
+        }
+      } else {
+        done = bytes;  // a padded unit is a whole number of 16-byte chunks
+        if (bytes == (uint32_t)C::TILE_BYTES) {  // full tile: compile-time trip count, as the uniform kernel
+#pragma unroll 4
+          for (int c = tid; c < C::TILE_BYTES / 16; c += C::NT) {
+            const int u = c / C::NVEC;
+            cp_async16(dst + (uint32_t)(c + u) * 16u, src + (size_t)c * 16);
+          }
+        } else {
+          for (uint32_t c = tid; c < bytes / 16u; c += C::NT)
+            cp_async16(dst + (c + c / (UB / 16u)) * 16u, src + (size_t)c * 16u);
+        }
+      }
+    } else if ((mis & 3u) == 0) {
+      done = bytes & ~3u;
+      for (uint32_t c = tid; c < done / 4u; c += C::NT) {
+        uint32_t d = c * 4u;
+        if constexpr (C::PAD) d += (d / UB) * PADB;
+        cp_async4(dst + d, src + (size_t)c * 4u);
+      }
+    } else {
+      done = 0;
+    }
+    for (uint32_t b = done + 2u * tid; b < bytes; b += 2u * C::NT) {
+      uint32_t d = b;
+      if constexpr (C::PAD) d += (b / UB) * PADB;
+      *reinterpret_cast<uint16_t*>(dstp + d) = *reinterpret_cast<const uint16_t*>(src + b);
+    }
+    cp_async_mbar_arrive(bar);  // counts once this thread's cp.async copies have landed
+  };
+
+#pragma unroll
+  for (int s = 0; s < C::STAGES; ++s) {
+    const uint32_t tile = tile_q[s];
+    if (tile < n_tiles) issue(s, s);
+  }
+  uint32_t pre = 0;
+  RaggedTile pre_d = {0ull, 0u, 0u};
+  if (tid == 0) {
+    pre = feed.fetch();
+    pre_d = entry(pre);
+  }
+
+  for (uint32_t j = 0;; ++j) {
+    const uint32_t tile = tile_q[j % QN];
+    if (tile >= n_tiles) break;
+    const int stage = (int)(j % C::STAGES);
+    const uint32_t parity = (j / C::STAGES) & 1u;
+    if (tid == 0) {
+      tile_q[(j + C::STAGES) % QN] = pre;
+      desc_q[(j + C::STAGES) % QN] = pre_d;
+      pre = feed.fetch();
+      pre_d = entry(pre);
+    }
+    const RaggedTile t = desc_q[j % QN];
+    const uint32_t n = (uint32_t)(t.src >> 48);
+    mbar_wait(bar_base + 8 * stage, parity);
+    const uint32_t first = (uint32_t)tid * C::TPT;
+    if (first < n) {
+      const uint8_t* unit = smem + stage * C::STAGE_BYTES + tid * C::UNIT_STRIDE;
+      // the calibration index "wraps" after the tile's last trace, so the discarded
+      // second trace of an odd tile reads pedestal[0], never past the arrays
+      compute_unit<C, MODE_SLIDING>(unit, t.out_base + first, n - first, t.cal0 + first,
+                                    t.cal0 + n, pedestal, gain, out_sum, out_start, out_charge,
+                                    out_time, vec_store != 0 && (t.out_base & 1u) == 0, ma);
+    }
+    __syncthreads();
+    const uint32_t next = tile_q[(j + C::STAGES) % QN];
+    if (next < n_tiles) issue((int)((j + C::STAGES) % QN), stage);
+  }
+
+  if (tid == 0) feed.leave();
+}
+
 template <class C, int MODE>
 __global__ void __launch_bounds__(C::NT)
     extract_tile_kernel(const uint8_t* __restrict__ wf, const uint32_t n_traces,

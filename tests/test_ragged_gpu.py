@@ -18,7 +18,7 @@ GOLD = os.path.join(os.path.dirname(__file__), "golden", "ragged.json")
 FILL = (-7, -7, -7.0, -7.0)
 
 
-def run_gpu(b, wf=None, wf_shift=0, streams=1, static=False, serial=False):
+def run_gpu(b, wf=None, wf_shift=0, streams=1, static=False, serial=False, jit=True, jit_at_launch=None):
     """wf_shift: place the waveform buffer that many samples into a 256-byte-aligned
     allocation (so block alignments change without touching the tables)."""
     import torch
@@ -34,10 +34,14 @@ def run_gpu(b, wf=None, wf_shift=0, streams=1, static=False, serial=False):
             for f, dt in zip(FILL, (torch.int32, torch.int32, torch.float32, torch.float32))]
     # the hooks live in librta_testing.so; while one is on the binding routes every
     # call there, so the plan is made and destroyed under the same switches
+    # jit: are the run-time specialisations (NVRTC) on when the plan is made (the plan cuts the
+    # tiles of an unspecialised shape for the kernel it expects); jit_at_launch: and at the launch
     rta.rta_debug_static_schedule(static)
     rta.rta_debug_serial_ragged(serial)
+    rta.rta_debug_jit(jit)
     plan = rta.rta_ragged_plan_create(*b.tables())
     try:
+        rta.rta_debug_jit(jit if jit_at_launch is None else jit_at_launch)
         before = rta.rta_launch_count()
         rta.rta_extract_ragged(plan, d_wf, d_ped, d_gain, *outs)
         torch.cuda.synchronize()
@@ -48,6 +52,7 @@ def run_gpu(b, wf=None, wf_shift=0, streams=1, static=False, serial=False):
         rta.rta_ragged_plan_destroy(plan)
         rta.rta_debug_static_schedule(False)
         rta.rta_debug_serial_ragged(False)
+        rta.rta_debug_jit(True)
     return tuple(o.cpu().numpy() for o in outs)
 
 
@@ -104,11 +109,27 @@ ANY_SHAPE = [((700, 60, 7), 2), ((300, 96, 8), 1), ((129, 64, 16), 1), ((77, 33,
 @pytest.mark.parametrize("gap,align", [(0, 8), (5, 1), (6, 2), (9, 8)])
 @pytest.mark.parametrize("wf_shift", [0, 1, 2])
 def test_unspecialised_shapes_take_the_runtime_shape_kernel(gap, align, wf_shift):
-    """extract_ragged_dyn_kernel: every ingest path (TMA / 16-byte cp.async into
-    the padded layout, 4-byte cp.async, halfwords) for every bank-conflict class."""
+    """extract_ragged_dyn_kernel (run-time specialisations off): every ingest path (TMA /
+    16-byte cp.async into the padded layout, 4-byte cp.async, halfwords) for every
+    bank-conflict class."""
+    b = make_batch(ANY_SHAPE, n_events=4, seed=3 + gap, gap=gap, align=align)
+    check(b, wf_shift=wf_shift, jit=False)
+    check(b, wf_shift=wf_shift, static=True, jit=False)
+
+
+@pytest.mark.parametrize("gap,align", [(0, 8), (5, 1), (6, 2), (9, 8)])
+@pytest.mark.parametrize("wf_shift", [0, 1, 2])
+def test_unspecialised_shapes_take_the_run_time_specialisation(gap, align, wf_shift):
+    """The tile-table kernel compiled for the shape at first use (units up to 320 bytes; the
+    576-sample camera of the batch keeps the runtime-shape kernel): the same batches, both
+    tile schedules; and a plan cut for the specialisation's tiles that is launched after the
+    compiler has gone away (the runtime-shape kernel with as many threads as a tile has units),
+    and the other way round."""
     b = make_batch(ANY_SHAPE, n_events=4, seed=3 + gap, gap=gap, align=align)
     check(b, wf_shift=wf_shift)
     check(b, wf_shift=wf_shift, static=True)
+    check(b, wf_shift=wf_shift, jit=True, jit_at_launch=False)
+    check(b, wf_shift=wf_shift, jit=False, jit_at_launch=True)
 
 
 @pytest.mark.parametrize("wf_shift", [0, 1, 2, 3, 4, 6])
