@@ -53,13 +53,18 @@ enum {
  *   wf        DEVICE  uint16 [n_events][n_pixels][n_samples], dense, sample fastest.
  *                     Any uint16 value is accepted (12-bit data is a property of the
  *                     configs, not of the ABI). A 16-byte-aligned base pointer takes
- *                     the staged (TMA / cp.async) kernels — a specialisation for the
- *                     shapes (30,7), (40,7), (25,4), (128,8), a kernel with runtime
- *                     (n_samples, W) for any other trace of at most 1152 bytes. Any
- *                     other 2-byte-aligned pointer takes that runtime-shape kernel
- *                     too, unless the trace (pair of traces when n_samples is odd) is
- *                     a multiple of 32 bytes; those, and longer traces, take the generic
- *                     kernel (strided global loads: several times slower). Same
+ *                     the staged (TMA / cp.async) kernels — ahead-of-time
+ *                     specialisations for the shapes (30,7), (40,7), (25,4), (128,8);
+ *                     for any other trace (pair of traces when n_samples is odd) of at
+ *                     most 320 bytes the same kernel compiled for the shape at first use
+ *                     (NVRTC through dlopen("libnvrtc.so"): 0.3-0.6 s once per shape and
+ *                     process; never inside a stream capture; RTA_JIT=0 turns it off);
+ *                     without the compiler, and up to 1152 bytes, a kernel with runtime
+ *                     (n_samples, W); longer traces a kernel that gives a thread a run of
+ *                     window starts. Any other 2-byte-aligned pointer takes the
+ *                     runtime-shape kernel too, unless the trace (pair) is a multiple of
+ *                     32 bytes; those take the generic kernel (strided global loads:
+ *                     several times slower). Same
  *                     results either way (rta_kernel_name says which). With an
  *                     unaligned base the first bulk copy starts at the 16-byte
  *                     boundary below wf (inside the 16-byte line holding wf[0]);
@@ -370,9 +375,11 @@ const char* rta_strerror(int status);
 int rta_last_cuda_error(void);
 
 /* Which kernel a shape takes, for tests and profiles: a static string such as
- * "tile<S=40,W=7>", "staged<any>" or "generic" for (n_samples, W, 16-byte-aligned?). */
+ * "tile<S=40,W=7>", "staged<jit>", "staged<any>", "segments" or "generic" for
+ * (n_samples, W, 16-byte-aligned?). */
 const char* rta_kernel_name(int32_t n_samples, int32_t W, int aligned16);
-/* Same for a P12 stream: "tile12<S=40,W=7>", "generic12", ... */
+/* Same for a P12 stream: "tile12<S=40,W=7>", "tile12<jit>" (packed units of at most 320
+ * bytes, compiled at first use), "generic12". */
 const char* rta_kernel_name_packed12(int32_t n_samples, int32_t W, int aligned16);
 
 /* Events per chunk the host-fed calls use for this shape and `chunk_bytes`

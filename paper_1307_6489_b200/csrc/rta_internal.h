@@ -130,10 +130,11 @@ struct RtaJitArgs {
   float *out_charge, *out_time;
   uint32_t* sched;
 };
-bool rta_jit_eligible(int32_t n_samples, int32_t W);   // shape fits a register copy, JIT enabled
+bool rta_jit_eligible(int32_t n_samples, int32_t W, int bits = 16);   // shape fits a register copy, JIT enabled
 bool rta_jit_available();                              // ... and libnvrtc could be loaded
 cudaError_t rta_jit_launch(int32_t n_samples, int32_t W, int mode, const RtaJitArgs& a,
-                           const void* mode_args, size_t mode_args_bytes, cudaStream_t stream);
+                           const void* mode_args, size_t mode_args_bytes, cudaStream_t stream,
+                           int bits = 16);
 // The same for a tile table of a mixed-camera batch (sliding extractor). rta_jit_tile_traces:
 // traces per tile of the specialisation of (S, W), 0 when there is none (not eligible, no compiler).
 struct RtaJitRaggedArgs {

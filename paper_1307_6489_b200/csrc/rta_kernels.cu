@@ -1075,6 +1075,7 @@ const char* rta_pick_kernel_name(int32_t S, int32_t W, bool aligned16, int bits)
       if (S == 40 && W == 7) return "tile12<S=40,W=7>";
       if (S == 25 && W == 4) return "tile12<S=25,W=4>";
       if (S == 128 && W == 8) return "tile12<S=128,W=8>";
+      if (rta_jit_eligible(S, W, 12) && rta_jit_available()) return "tile12<jit>";  // compiled at first use
     }
     return "generic12";
   }
@@ -1407,6 +1408,22 @@ cudaError_t launch_packed12(const LaunchArgs& a, const ModeArgs& ma) {
     RTA_TRY(CfgP40W7)
     RTA_TRY(CfgP25W4)
     RTA_TRY(CfgP128W8)
+    // any other shape whose packed unit fits a register copy: compiled for (S, W) at first use
+    if (rta_jit_eligible(a.S, a.W, 12)) {
+      int dev = 0;
+      cudaError_t e = cudaGetDevice(&dev);
+      if (e != cudaSuccess) return e;
+      ModeArgs m = ma;
+      m.key_mul = 1u << ilog2_ceil(a.S - a.W + 1);
+      m.one = 1u;
+      m.minus_one = 0xFFFFFFFFu;
+      const RtaJitArgs ja{a.wf,      a.n_traces,  a.n_pixels,  a.pix_inv,
+                          a.pedestal, a.gain,      a.out_sum,   a.out_start,
+                          a.out_charge, a.out_time,
+                          g_static_schedule ? nullptr : sched_words(dev, a.stream)};
+      e = rta_jit_launch(a.S, a.W, MODE, ja, &m, sizeof m, a.stream, 12);
+      if (e != cudaErrorNotSupported) return e;
+    }
   }
   return launch_generic<MODE, 12>(a, ma);
 }

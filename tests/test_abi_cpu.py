@@ -238,7 +238,13 @@ def test_packed12_kernel_names():
     assert rta.rta_kernel_name_packed12(25, 4) == "tile12<S=25,W=4>"
     assert rta.rta_kernel_name_packed12(128, 8) == "tile12<S=128,W=8>"
     assert rta.rta_kernel_name_packed12(40, 7, aligned16=False) == "generic12"
-    assert rta.rta_kernel_name_packed12(41, 7) == "generic12"
+    assert rta.rta_kernel_name_packed12(41, 7) in ("tile12<jit>", "generic12")   # with / without libnvrtc
+    assert rta.rta_kernel_name_packed12(300, 7) == "generic12"                   # 450-byte units: no register copy
+    rta.rta_debug_jit(False)
+    try:
+        assert rta.rta_kernel_name_packed12(41, 7) == "generic12"
+    finally:
+        rta.rta_debug_jit(True)
 
 
 def test_chunk_events_planning():

@@ -72,6 +72,16 @@ def all_paths(wf12, ped, gain, W):
         got = run_packed(packed, E, P, S, ped, gain, W, **kw)
         assert_parity(got, want, str(kw))
         assert bit_identical(got, want), kw
+    import paper_1307_6489_b200 as rta
+    if rta.rta_kernel_name_packed12(S, W) == "tile12<jit>":
+        # a shape without an ahead-of-time kernel: the run above took the run-time specialisation;
+        # without it (no libnvrtc) the same call takes generic12
+        rta.rta_debug_jit(False)
+        try:
+            assert rta.rta_kernel_name_packed12(S, W) == "generic12"
+            assert bit_identical(run_packed(packed, E, P, S, ped, gain, W), want), "jit off"
+        finally:
+            rta.rta_debug_jit(True)
     return want
 
 
