@@ -330,3 +330,37 @@ def test_extract_host_packed_end_to_end(chunk_events):
     outs2 = tuple(np.zeros_like(o) for o in outs)
     rta.rta_extract_host_packed12(pk, 37, c.n_pixels, c.n_samples, ped, gain, c.W, *outs2)
     assert bit_identical(outs2, want)
+
+
+@pytest.mark.parametrize("S,W,P", [(60, 7, 1855), (31, 5, 333), (96, 8, 512)])
+def test_stream_and_host_variants_on_shapes_without_an_ahead_of_time_kernel(S, W, P):
+    """The host-fed P12 calls on shapes that take the run-time specialisation of the P12
+    kernel (or generic12 without the compiler): several chunks, every chunk a kernel launch on
+    a 16-byte-aligned slice of the stream, against the bit-by-bit oracle."""
+    import torch
+    import paper_1307_6489_b200 as rta
+    rng = np.random.default_rng(S * 100 + W)
+    n_ev = 37
+    wf = rng.integers(0, 4096, size=(n_ev, P, S)).astype(np.uint16)
+    wf[rng.random((n_ev, P)) < 0.1] = 4095
+    ped = rng.integers(0, 600, P).astype(np.int32)
+    gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
+    pk = dl0gen.pack12_cpu(wf)
+    want = oracle.extract_packed12(pk, n_ev, ped, gain, S, W)
+    d_ped, d_gain = torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda()
+    ev_bytes = P * S * 3 // 2
+    for chunk_events in (5, 16, 1000):
+        outs = alloc_outputs(n_ev * P)
+        rta.rta_extract_stream_packed12(torch.from_numpy(pk).pin_memory(), n_ev, P, S, d_ped, d_gain, W, *outs,
+                                        chunk_bytes=chunk_events * ev_bytes + 3)
+        torch.cuda.synchronize()
+        assert bit_identical(tuple(o.cpu().numpy() for o in outs), want), chunk_events
+    rta.rta_debug_jit(False)
+    try:
+        outs = alloc_outputs(n_ev * P)
+        rta.rta_extract_stream_packed12(torch.from_numpy(pk), n_ev, P, S, d_ped, d_gain, W, *outs,
+                                        chunk_bytes=9 * ev_bytes)
+        torch.cuda.synchronize()
+        assert bit_identical(tuple(o.cpu().numpy() for o in outs), want), "jit off"
+    finally:
+        rta.rta_debug_jit(True)

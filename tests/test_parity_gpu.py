@@ -339,6 +339,43 @@ def test_cuda_graph_capture_and_replay():
                              oracle.extract(wf, ped, gain, c.W))
 
 
+@pytest.mark.parametrize("S,W,warm", [(52, 6, True), (54, 9, False), (2048, 12, False)])
+def test_cuda_graph_capture_of_shapes_without_an_ahead_of_time_kernel(S, W, warm):
+    """A shape whose specialisation is compiled at first use: captured after an eager call the
+    graph holds the compiled kernel; captured as the very first call of the shape nothing is
+    compiled inside the capture (the runtime-shape kernel is recorded instead). Long traces
+    (the segment kernel) are capturable too. Replays on other data must match the oracle."""
+    import torch
+    import paper_1307_6489_b200 as rta
+    rng = np.random.default_rng(S)
+    E, P = 3, 1500 if S < 1000 else 40
+    ped = rng.integers(0, 600, P).astype(np.int32)
+    gain = rng.uniform(0.9, 1.1, P).astype(np.float32)
+    d_ped, d_gain = torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda()
+    wfs = [rng.integers(0, 4096, size=(E, P, S)).astype(np.uint16) for _ in range(3)]
+    d_wf = to_dev_u16(wfs[0])
+    outs = alloc_outputs(E * P)
+    side = torch.cuda.Stream()
+    if warm:
+        with torch.cuda.stream(side):
+            rta.rta_extract(d_wf, E, P, S, d_ped, d_gain, W, *outs)
+        torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        rta.rta_extract(d_wf, E, P, S, d_ped, d_gain, W, *outs)
+    for wf in wfs[::-1]:
+        d_wf.copy_(to_dev_u16(wf))
+        for o in outs:
+            o.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert bit_identical(tuple(o.cpu().numpy() for o in outs), oracle.extract(wf, ped, gain, W))
+    # and eagerly afterwards (the shape that was first seen inside a capture compiles now)
+    rta.rta_extract(d_wf, E, P, S, d_ped, d_gain, W, *outs)
+    torch.cuda.synchronize()
+    assert bit_identical(tuple(o.cpu().numpy() for o in outs), oracle.extract(wfs[0], ped, gain, W))
+
+
 def test_graph_replays_run_next_to_eager_calls_and_to_each_other():
     """Two graphs captured on ONE stream, replayed on two other streams at the
     same time as eager calls on the capture stream, 50 rounds: a captured launch
