@@ -45,7 +45,8 @@ enum {
   RTA_ERR_UNSUPPORTED = 3, /* n_events*n_pixels >= 2^31, or n_samples*W*65535 >= 2^31 (int32 guard) */
   RTA_ERR_ALIGN = 4,       /* wf is not 2-byte aligned / an output is not 4-byte aligned (P12: any byte) */
   RTA_ERR_CUDA = 5,        /* CUDA runtime failure; see rta_last_cuda_error() */
-  RTA_ERR_NOMEM = 6        /* workspace allocation failed (device or pinned host) */
+  RTA_ERR_NOMEM = 6,       /* workspace allocation failed (device or pinned host) */
+  RTA_ERR_TOO_LARGE = 7    /* more work than the fixed scratch of rta_extract_image_noalloc holds */
 };
 
 /* Kernel-only path.
@@ -362,6 +363,52 @@ int rta_extract_image_host(const uint16_t* wf_host, int64_t n_events, int32_t n_
                            const float* pix_y_host, const int32_t* neighbors_host,
                            float thr_picture, float thr_boundary, int32_t* out_n_pix_host,
                            float* out_params_host, uint8_t* out_mask_host, size_t chunk_bytes);
+
+/* rta_extract_image for callers that must not allocate device memory.
+ *
+ * Two kinds of caller are meant. A reconstruction thread during data taking
+ * (§4.2, event by event while the telescopes acquire): cudaMalloc and
+ * cudaFree synchronise the whole device, so an allocation on the analysis side
+ * stalls the copies that bring the next events in. And a process whose device
+ * memory is spoken for in full (a framework allocator told to take everything, a
+ * GPU partition sized to the job), where an allocation behind the owner's back
+ * fails or breaks the owner's budget. rta_extract_image itself is no good to
+ * them on a shape without a fused kernel: it takes 16 bytes of scratch per trace
+ * from a stream-ordered pool, may compile a kernel at first use, and its tile
+ * scheduler lives in a cudaMalloc'ed pool.
+ *
+ * This call computes the same thing with the same arguments (extraction by the
+ * runtime-shape staged kernel into scratch, then the moments kernel) and calls
+ * no cudaMalloc, cudaFree, memory pool, run-time compiler or other allocating
+ * routine. Its scratch is a static device array inside the library image:
+ * 256 bytes of scheduler words + 16 bytes per trace for at most
+ * RTA_NOALLOC_MAX_TRACES traces = 16 MiB + 256 bytes, held by every GPU that
+ * loads librta.so from module load until the process exits, called or not.
+ *
+ *  - n_events * n_pixels > RTA_NOALLOC_MAX_TRACES -> RTA_ERR_TOO_LARGE, nothing
+ *    enqueued (split the batch: events are independent).
+ *  - wf must be 16-byte aligned (else RTA_ERR_ALIGN) and a trace (a pair of
+ *    traces when n_samples is odd) at most 1152 bytes, i.e. n_samples <= 576
+ *    even / 288 odd (else RTA_ERR_UNSUPPORTED). All four BASELINE shapes qualify.
+ *    Every other rule of rta_extract_image applies unchanged.
+ *  - The first call on a device looks the array's device address up
+ *    (cudaGetSymbolAddress, once per device, with that device current) and sets
+ *    kernel attributes; make that first call outside any stream capture.
+ *  - The array is shared by every call on the device and keeps the previous
+ *    call's bytes. The library zeroes the scheduler words on `stream` before each
+ *    launch; the per-trace part is fully rewritten before it is read. Two calls
+ *    whose kernels can run at the same time (unordered streams, two host threads)
+ *    race on the array and return garbage: keep such calls on one stream or order
+ *    them with events. Results equal rta_extract_image's (same integer
+ *    extraction, same cleaning and moments code).
+ * Asynchronous on `stream`; n_events == 0 -> RTA_OK. */
+#define RTA_NOALLOC_MAX_TRACES 1048576
+int rta_extract_image_noalloc(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
+                              int32_t n_samples, const int32_t* pedestal, const float* gain,
+                              int32_t W, const float* pix_x, const float* pix_y,
+                              const int32_t* neighbors, float thr_picture, float thr_boundary,
+                              int32_t* out_n_pix, float* out_params, uint8_t* out_mask,
+                              void* stream);
 
 /* "image_tile<S=40,W=7>", ..., "staged<any>+image_moments" or "image_generic". */
 const char* rta_image_kernel_name(int32_t n_pixels, int32_t n_samples, int32_t W, int aligned16);

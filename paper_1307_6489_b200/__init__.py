@@ -19,6 +19,8 @@ RTA_ERR_UNSUPPORTED = 3
 RTA_ERR_ALIGN = 4
 RTA_ERR_CUDA = 5
 RTA_ERR_NOMEM = 6
+RTA_ERR_TOO_LARGE = 7
+RTA_NOALLOC_MAX_TRACES = 1 << 20   # include/rta.h
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _lock = threading.Lock()
@@ -81,7 +83,8 @@ def _declare(L: ctypes.CDLL, testing: bool) -> ctypes.CDLL:
     L.rta_image_moments.restype = ctypes.c_int
     L.rta_image_moments.argtypes = ([_VP, _VP, ctypes.c_int64, ctypes.c_int32] + _CAM
                                     + _IMG_OUT + [_VP])
-    for name in ("rta_extract_image",) + (("rta_extract_image_generic",) if testing else ()):
+    for name in ("rta_extract_image", "rta_extract_image_noalloc") + (
+            ("rta_extract_image_generic",) if testing else ()):
         fn = getattr(L, name)
         fn.restype = ctypes.c_int
         fn.argtypes = _EXTRACT_ARGS[:7] + _CAM + _IMG_OUT + [_VP]
@@ -343,6 +346,19 @@ def rta_extract_image(wf, n_events, n_pixels, n_samples, pedestal, gain, W, pix_
               _ptr(pix_x), _ptr(pix_y), _ptr(neighbors), float(thr_picture),
               float(thr_boundary), _ptr(out_n_pix), _ptr(out_params), _ptr(out_mask),
               _stream_handle(stream)))
+
+
+def rta_extract_image_noalloc(wf, n_events, n_pixels, n_samples, pedestal, gain, W, pix_x, pix_y,
+                              neighbors, thr_picture, thr_boundary, out_n_pix, out_params,
+                              out_mask=None, stream=None) -> None:
+    """include/rta.h:rta_extract_image_noalloc: rta_extract_image for callers that must
+    not allocate device memory (fixed scratch inside the library, at most
+    RTA_NOALLOC_MAX_TRACES traces per call, calls that overlap on the GPU race).
+    Device pointers; asynchronous on ``stream``."""
+    _check(lib().rta_extract_image_noalloc(
+        _ptr(wf), n_events, n_pixels, n_samples, _ptr(pedestal), _ptr(gain), W,
+        _ptr(pix_x), _ptr(pix_y), _ptr(neighbors), float(thr_picture), float(thr_boundary),
+        _ptr(out_n_pix), _ptr(out_params), _ptr(out_mask), _stream_handle(stream)))
 
 
 def rta_extract_image_stream(wf_host, n_events, n_pixels, n_samples, pedestal, gain, W, pix_x,

@@ -946,6 +946,30 @@ int rta_extract_image(const uint16_t* wf, int64_t n_events, int32_t n_pixels, in
                               out_mask, stream, false);
 }
 
+// The same for callers that cannot allocate device memory (include/rta.h): fixed
+// scratch inside the library image, see rta_noalloc.cu. Validation happens here,
+// before the first CUDA call.
+int rta_extract_image_noalloc(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
+                              int32_t n_samples, const int32_t* pedestal, const float* gain,
+                              int32_t W, const float* pix_x, const float* pix_y,
+                              const int32_t* neighbors, float thr_picture, float thr_boundary,
+                              int32_t* out_n_pix, float* out_params, uint8_t* out_mask,
+                              void* stream) {
+  int v = validate_fused(wf, n_events, n_pixels, n_samples, pedestal, gain, W);
+  if (v != RTA_OK) return v;
+  v = validate_image(n_events, n_pixels, pix_x, pix_y, neighbors, out_n_pix, out_params, out_mask);
+  if (v != RTA_OK || n_events == 0) return v;
+  if (n_events * (int64_t)n_pixels > (int64_t)RTA_NOALLOC_MAX_TRACES) return RTA_ERR_TOO_LARGE;
+  if ((uintptr_t)wf % 16 != 0) return RTA_ERR_ALIGN;
+  if (!rta_dyn_eligible(n_samples, W)) return RTA_ERR_UNSUPPORTED;
+  const RtaCamera cam{pix_x, pix_y, neighbors, thr_picture, thr_boundary};
+  const RtaImageOut out{out_n_pix, out_params, out_mask};
+  const cudaError_t e = rta_launch_extract_image_noalloc(wf, n_events, n_pixels, n_samples, pedestal,
+                                                         gain, W, cam, out, (cudaStream_t)stream);
+  if (e == cudaErrorNotSupported) return RTA_ERR_UNSUPPORTED;
+  return e == cudaSuccess ? RTA_OK : fail_cuda(e);
+}
+
 #ifdef RTA_TESTING
 // Same through the generic fused kernel (librta_testing.so only).
 int rta_extract_image_generic(const uint16_t* wf, int64_t n_events, int32_t n_pixels,
@@ -1051,6 +1075,9 @@ const char* rta_strerror(int status) {
     case RTA_ERR_ALIGN: return "misaligned pointer (wf: 2 bytes; calibration and outputs: 4 bytes)";
     case RTA_ERR_CUDA: return "CUDA runtime error (see rta_last_cuda_error)";
     case RTA_ERR_NOMEM: return "out of device or pinned host memory";
+    case RTA_ERR_TOO_LARGE:
+      return "too many traces for the fixed scratch of rta_extract_image_noalloc "
+             "(n_events*n_pixels > RTA_NOALLOC_MAX_TRACES): split the batch";
     default: return "unknown status";
   }
 }

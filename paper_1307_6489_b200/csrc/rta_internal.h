@@ -52,6 +52,15 @@ cudaError_t rta_launch_extract(const void* wf, int64_t n_traces, int32_t n_pixel
 // (extract_dyn_kernel) when the input is 16-byte aligned.
 bool rta_dyn_eligible(int32_t n_samples, int32_t W);
 
+// The sliding extractor through the runtime-shape staged kernel, with the tile
+// scheduler's two words supplied by the caller (zero when the kernel starts) instead
+// of the library's cudaMalloc'ed per-stream pool. cudaErrorNotSupported unless
+// rta_dyn_eligible(n_samples, W) and wf is 16-byte aligned.
+cudaError_t rta_launch_extract_dyn_sched(const void* wf, int64_t n_traces, int32_t n_pixels,
+                                         int32_t n_samples, const int32_t* pedestal,
+                                         const float* gain, int32_t W, int32_t* out_sum,
+                                         int32_t* out_start, float* out_charge, float* out_time,
+                                         cudaStream_t stream, uint32_t* sched);
 // Name of the kernel the dispatcher picks (static string).
 const char* rta_pick_kernel_name(int32_t n_samples, int32_t W, bool aligned16, int bits = 16);
 
@@ -108,6 +117,13 @@ cudaError_t rta_launch_extract_image(const void* wf, int64_t n_events, int32_t n
                                      const float* gain, int32_t W, const RtaCamera& cam,
                                      const RtaImageOut& out, cudaStream_t stream,
                                      bool force_generic);
+// rta_noalloc.cu: rta_extract_image_noalloc behind its validation (include/rta.h).
+// cudaErrorNotSupported: shape or alignment outside what that call takes.
+cudaError_t rta_launch_extract_image_noalloc(const void* wf, int64_t n_events, int32_t n_pixels,
+                                             int32_t n_samples, const int32_t* pedestal,
+                                             const float* gain, int32_t W,
+                                             const RtaCamera& cam,
+                                             const RtaImageOut& out, cudaStream_t stream);
 // Tests: never take the symmetric-neighbour-table shortcut of the cleaning (both
 // ways give the same mask on a symmetric table).
 void rta_set_general_cleaning(bool on);

@@ -1478,6 +1478,54 @@ bool rta_dyn_eligible(int32_t S, int32_t W) {
   return S >= 1 && W >= 1 && W <= S && dyn_shape(S, W, &sh, &threads);
 }
 
+// The sliding extractor through the runtime-shape staged kernel with scheduler words
+// the caller owns (rta_noalloc.cu: words in a static device array, zeroed on the
+// stream ahead of this launch). Nothing here allocates device memory: no per-stream
+// scheduler pool, no run-time compile. A separate copy of launch_dyn's body so that
+// the dispatch above stays as it is. cudaErrorNotSupported: (S, W) is not
+// rta_dyn_eligible, or wf is not 16-byte aligned.
+cudaError_t rta_launch_extract_dyn_sched(const void* wf, int64_t n_traces64, int32_t n_pixels,
+                                         int32_t S, const int32_t* pedestal, const float* gain,
+                                         int32_t W, int32_t* out_sum, int32_t* out_start,
+                                         float* out_charge, float* out_time, cudaStream_t stream,
+                                         uint32_t* sched) {
+  if (n_traces64 <= 0) return cudaSuccess;
+  DynShape sh;
+  int threads = 0;
+  if (((uintptr_t)wf % 16) != 0 || S < 1 || W < 1 || W > S || !dyn_shape(S, W, &sh, &threads))
+    return cudaErrorNotSupported;
+  int dev = 0, sms = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if ((e = device_sms(dev, &sms)) != cudaSuccess) return e;
+  const bool pad = sh.unit_stride != sh.unit_bytes;
+  using Kernel = void (*)(const uint8_t*, uint32_t, uint32_t, uint32_t, const int*, const float*, int*,
+                          int*, float*, float*, uint32_t*, DynShape, ModeArgs);
+  const Kernel kernel = pad          ? extract_dyn_kernel<true, 4, MODE_SLIDING>
+                        : sh.g == 1 ? extract_dyn_kernel<false, 1, MODE_SLIDING>
+                        : sh.g == 2 ? extract_dyn_kernel<false, 2, MODE_SLIDING>
+                                    : extract_dyn_kernel<false, 4, MODE_SLIDING>;
+  const int smem = sh.stages * sh.stage_bytes;
+  if ((e = rta_func_allow_max_smem((const void*)kernel, dev)) != cudaSuccess) return e;
+  int occ = 0;
+  if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem)) != cudaSuccess)
+    return e;
+  if (occ < 1) return cudaErrorLaunchOutOfResources;
+  const uint32_t n_traces = (uint32_t)n_traces64, P = (uint32_t)n_pixels;
+  const uint32_t n_full = n_traces / (uint32_t)(threads * sh.tpt);
+  uint32_t grid = (uint32_t)(sms * occ);
+  if (grid > n_full) grid = n_full;
+  if (grid < 1) grid = 1;
+  const uint64_t inv64 = (1ull << 32) / P;
+  const uint32_t pix_inv = inv64 > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)inv64;
+  const ModeArgs ma = {};
+  kernel<<<grid, threads, smem, stream>>>(static_cast<const uint8_t*>(wf), n_traces, P, pix_inv,
+                                          pedestal, gain, out_sum, out_start, out_charge, out_time,
+                                          sched, sh, ma);
+  rta_count_launch();
+  return cudaGetLastError();
+}
+
 int rta_ragged_tile_traces(int32_t S, int32_t W) {
   if (S == CfgS30W7::S && W == CfgS30W7::W) return CfgS30W7::TILE_TRACES;
   if (S == CfgS40W7::S && W == CfgS40W7::W) return CfgS40W7::TILE_TRACES;
