@@ -745,6 +745,9 @@ __device__ __forceinline__ void queue_finish(FinishQueue& Q, const uint32_t slot
   if (lane == 0) {  // the slot may be refilled
     __threadfence_block();
     Q.written[slot] = 0u;
+    // the reset must be visible before the slot is handed back: a writer of the next
+    // batch waits on `freed` and then counts itself into `written`
+    __threadfence_block();
     atomicAdd(&Q.freed[slot], 1u);
   }
   if (lane < n) finish_event(pd, out);

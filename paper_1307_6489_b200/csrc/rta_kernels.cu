@@ -484,11 +484,12 @@ __global__ void __launch_bounds__(256)
   for (uint32_t ti = blockIdx.x; ti < n_tiles; ti += gridDim.x) {
     const RaggedTile t = tiles[ti];
     const uint32_t n = (uint32_t)(t.src >> 48);
-    if (threadIdx.x < n) {
-      const GlobalTrace<16> tr(wf + (size_t)(t.src & kRaggedOffMask), threadIdx.x, S);
-      const Result r =
-          generic_trace<MODE_SLIDING, 16>(tr, S, W, t.cal0 + threadIdx.x, pedestal, gain, ma);
-      const uint32_t g = t.out_base + threadIdx.x;
+    // a tile may hold more traces than the CTA has threads (tables cut for the 512-trace
+    // tiles of the staged kernels can end up here when those are not available)
+    for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+      const GlobalTrace<16> tr(wf + (size_t)(t.src & kRaggedOffMask), i, S);
+      const Result r = generic_trace<MODE_SLIDING, 16>(tr, S, W, t.cal0 + i, pedestal, gain, ma);
+      const uint32_t g = t.out_base + i;
       out_sum[g] = r.sum;
       out_start[g] = r.start;
       out_charge[g] = r.charge;
