@@ -425,6 +425,36 @@ int rta_last_cuda_error(void);
  * "tile<S=40,W=7>", "staged<jit>", "staged<any>", "segments" or "generic" for
  * (n_samples, W, 16-byte-aligned?). */
 const char* rta_kernel_name(int32_t n_samples, int32_t W, int aligned16);
+/* Take the run-time compile off the data path. A shape without an ahead-of-time
+ * kernel is compiled for its (n_samples, W, extractor, sample format) the first
+ * time a call meets it: 0.3-0.6 s on the host inside that call, and never inside
+ * a stream capture (a first call that is being captured records the slower
+ * runtime-shape kernel instead). An on-site pipeline that knows its cameras
+ * (three telescope types; re-pointing within 90 s)
+ * calls this once per shape at configuration time, with the device current that
+ * will run the data, before any capture:
+ *
+ *   extractor    RTA_EXTRACTOR_SLIDING (rta_extract, rta_extract_ragged, the
+ *                _stream / _host / _image calls), _FIXED, _LOCAL_PEAK or _FIR
+ *                (W = n_taps)
+ *   sample_bits  16 (uint16 samples) or 12 (P12 stream; sliding only)
+ *
+ * RTA_OK: a kernel specialised for the shape is compiled, loaded and set up on
+ * the current device (or was built ahead of time); calls of this shape compile
+ * nothing from now on. RTA_ERR_UNSUPPORTED: the shape has no specialisation
+ * (trace too long for one, libnvrtc not found, RTA_JIT=0) and runs the
+ * runtime-shape kernels, which need no preparation either; also P12 with another
+ * extractor, and the int32 guard of rta_extract. RTA_ERR_SHAPE: bad n_samples /
+ * W / extractor / sample_bits. Thread-safe; compiling one shape does not delay
+ * launches of other shapes. rta_shutdown unloads what was compiled. */
+enum {
+  RTA_EXTRACTOR_SLIDING = 0,
+  RTA_EXTRACTOR_FIXED = 1,
+  RTA_EXTRACTOR_LOCAL_PEAK = 2,
+  RTA_EXTRACTOR_FIR = 3
+};
+int rta_prepare(int32_t n_samples, int32_t W, int32_t extractor, int32_t sample_bits);
+
 /* Same for a P12 stream: "tile12<S=40,W=7>", "tile12<jit>" (packed units of at most 320
  * bytes, compiled at first use), "generic12". */
 const char* rta_kernel_name_packed12(int32_t n_samples, int32_t W, int aligned16);

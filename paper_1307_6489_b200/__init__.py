@@ -99,6 +99,8 @@ def _declare(L: ctypes.CDLL, testing: bool) -> ctypes.CDLL:
                                         ctypes.c_int]
     L.rta_image_max_pixels.restype = ctypes.c_int32
     L.rta_image_max_pixels.argtypes = []
+    L.rta_prepare.restype = ctypes.c_int
+    L.rta_prepare.argtypes = [ctypes.c_int32] * 4
     L.rta_chunk_events.restype = ctypes.c_int64
     L.rta_chunk_events.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32,
                                    ctypes.c_size_t, ctypes.c_int32]
@@ -391,6 +393,21 @@ def rta_image_kernel_name(n_pixels: int, n_samples: int, W: int, aligned16: bool
 
 def rta_image_max_pixels() -> int:
     return int(lib().rta_image_max_pixels())
+
+
+RTA_EXTRACTOR_SLIDING, RTA_EXTRACTOR_FIXED, RTA_EXTRACTOR_LOCAL_PEAK, RTA_EXTRACTOR_FIR = 0, 1, 2, 3
+
+
+def rta_prepare(n_samples: int, W: int, extractor: int = RTA_EXTRACTOR_SLIDING,
+                sample_bits: int = 16) -> bool:
+    """include/rta.h:rta_prepare. True: a kernel specialised for the shape is ready on the
+    current device (nothing will be compiled on the data path); False: the shape has no
+    specialisation and runs the runtime-shape kernels. Other statuses raise."""
+    st = lib().rta_prepare(n_samples, W, extractor, sample_bits)
+    if st == RTA_ERR_UNSUPPORTED:
+        return False
+    _check(st)
+    return True
 
 
 def rta_strerror(status: int) -> str:

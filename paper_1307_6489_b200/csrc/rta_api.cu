@@ -1088,6 +1088,26 @@ const char* rta_kernel_name(int32_t n_samples, int32_t W, int aligned16) {
   return rta_pick_kernel_name(n_samples, W, aligned16 != 0);
 }
 
+int rta_prepare(int32_t n_samples, int32_t W, int32_t extractor, int32_t sample_bits) {
+  static_assert((int)RTA_EXTRACTOR_SLIDING == (int)RTA_MODE_SLIDING &&
+                    (int)RTA_EXTRACTOR_FIXED == (int)RTA_MODE_FIXED &&
+                    (int)RTA_EXTRACTOR_LOCAL_PEAK == (int)RTA_MODE_LOCAL_PEAK &&
+                    (int)RTA_EXTRACTOR_FIR == (int)RTA_MODE_FIR,
+                "the public extractor numbers are the internal modes");
+  if (n_samples < 1 || W < 1 || W > n_samples) return RTA_ERR_SHAPE;
+  if (extractor < RTA_EXTRACTOR_SLIDING || extractor > RTA_EXTRACTOR_FIR) return RTA_ERR_SHAPE;
+  if (sample_bits != 16 && sample_bits != 12) return RTA_ERR_SHAPE;
+  if ((int64_t)n_samples * (int64_t)W * 65535ll >= (1ll << 31)) return RTA_ERR_UNSUPPORTED;
+  if (sample_bits == 12 && extractor != RTA_EXTRACTOR_SLIDING) return RTA_ERR_UNSUPPORTED;
+  if (extractor == RTA_EXTRACTOR_FIR && W > RTA_MAX_TAPS) return RTA_ERR_UNSUPPORTED;
+  // the four BASELINE shapes were compiled with the library
+  if (std::strncmp(rta_pick_kernel_name(n_samples, W, true, sample_bits), "tile", 4) == 0) return RTA_OK;
+  const cudaError_t e = rta_jit_prepare(n_samples, W, extractor, sample_bits);
+  if (e == cudaSuccess) return RTA_OK;
+  if (e == cudaErrorNotSupported) return RTA_ERR_UNSUPPORTED;
+  return fail_cuda(e);
+}
+
 const char* rta_kernel_name_packed12(int32_t n_samples, int32_t W, int aligned16) {
   return rta_pick_kernel_name(n_samples, W, aligned16 != 0, 12);
 }

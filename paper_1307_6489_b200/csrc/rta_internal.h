@@ -151,6 +151,9 @@ bool rta_jit_available();                              // ... and libnvrtc could
 cudaError_t rta_jit_launch(int32_t n_samples, int32_t W, int mode, const RtaJitArgs& a,
                            const void* mode_args, size_t mode_args_bytes, cudaStream_t stream,
                            int bits = 16);
+// Compile / load / set up the specialisation of a shape on the current device now
+// (rta_prepare); cudaErrorNotSupported when the shape has none.
+cudaError_t rta_jit_prepare(int32_t n_samples, int32_t W, int mode, int bits);
 // The same for a tile table of a mixed-camera batch (sliding extractor). rta_jit_tile_traces:
 // traces per tile of the specialisation of (S, W), 0 when there is none (not eligible, no compiler).
 struct RtaJitRaggedArgs {

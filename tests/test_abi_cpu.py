@@ -322,3 +322,29 @@ def test_ragged_plan_validation_before_any_cuda_call():
     assert rta.rta_ragged_plan_info(plan, rta.RTA_RAGGED_N_LAUNCHES) == 0
     assert rta.rta_ragged_plan_info(plan, 99) == -1
     rta.rta_ragged_plan_destroy(plan)
+
+
+def test_prepare_validates_before_any_cuda_call():
+    """include/rta.h:rta_prepare: argument errors and the ahead-of-time shapes are decided
+    on the host; only a shape that needs compiling reaches CUDA (and fails here, without a
+    device, as every compute call does)."""
+    L = rta.lib()
+    assert L.rta_prepare(0, 1, rta.RTA_EXTRACTOR_SLIDING, 16) == rta.RTA_ERR_SHAPE
+    assert L.rta_prepare(30, 31, rta.RTA_EXTRACTOR_SLIDING, 16) == rta.RTA_ERR_SHAPE
+    assert L.rta_prepare(30, 7, 4, 16) == rta.RTA_ERR_SHAPE          # no such extractor
+    assert L.rta_prepare(30, 7, -1, 16) == rta.RTA_ERR_SHAPE
+    assert L.rta_prepare(30, 7, rta.RTA_EXTRACTOR_SLIDING, 8) == rta.RTA_ERR_SHAPE
+    assert L.rta_prepare(2048, 17, rta.RTA_EXTRACTOR_SLIDING, 16) == rta.RTA_ERR_UNSUPPORTED
+    assert L.rta_prepare(36, 5, rta.RTA_EXTRACTOR_FIXED, 12) == rta.RTA_ERR_UNSUPPORTED
+    assert L.rta_prepare(64, 33, rta.RTA_EXTRACTOR_FIR, 16) == rta.RTA_ERR_UNSUPPORTED
+    for S, W in ((30, 7), (40, 7), (25, 4), (128, 8)):               # built with the library
+        for bits in (16, 12):
+            assert L.rta_prepare(S, W, rta.RTA_EXTRACTOR_SLIDING, bits) == rta.RTA_OK
+    try:
+        import torch
+        has_gpu = torch.cuda.is_available()
+    except Exception:
+        has_gpu = False
+    if not has_gpu:
+        assert L.rta_prepare(36, 5, rta.RTA_EXTRACTOR_SLIDING, 16) in (
+            rta.RTA_ERR_CUDA, rta.RTA_ERR_NOMEM, rta.RTA_ERR_UNSUPPORTED)
