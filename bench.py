@@ -17,7 +17,8 @@ Prints ONE JSON line (rank 0). Keys beyond the driver's contract:
                 fed through rta_extract_stream in 1 GiB chunks, against the
                 host-link bandwidth measured in the same run and the paper's
                 0.5-8 GB/s array data rate
-  configs       kernel-only numbers for the other single-GPU configs (C3, C4)
+  configs       kernel-only numbers for the other single-GPU configs (C3, C4) and the
+                small case C1 (eager and CUDA-graph replay, L2 flushed and resident)
   family        the other extractors (NEXT-1) on the same batches
   packed12      NEXT-2: the same batches as P12 streams (12 bits per sample),
                 decoded inside the extraction kernel; sustained.packed12 is C5
@@ -26,6 +27,8 @@ Prints ONE JSON line (rank 0). Keys beyond the driver's contract:
   image         NEXT-4: rta_extract_image (extraction + cleaning + moments in one
                 kernel) next to rta_extract followed by rta_image_moments;
                 sustained.image is C5 through rta_extract_image_stream
+  latency       host wall time per call (p50 / p99) for 1 .. 4096 events of the C2 camera:
+                rta_extract eager and as a graph replay, rta_extract_host, rta_extract_image_host
   any_shape     shapes without a specialised kernel (not BASELINE configs) through
                 the staged kernel with runtime (n_samples, W), next to the generic one
 Secondary legs are single-GPU diagnostics (N = 1 only) and run ten untimed launches first.
@@ -597,7 +600,7 @@ def any_shape_leg(steps, peak, torch, dl0gen, rta):
     return res
 
 
-SECONDARY_LEGS = ("configs", "family", "packed12", "any_shape", "ragged", "image")
+SECONDARY_LEGS = ("configs", "family", "packed12", "any_shape", "ragged", "image", "latency")
 EVENT_OUT_BYTES = 36   # n_pix int32 + 8 fp32 parameters per event
 LEG_WARMUP = 10        # untimed launches in front of every secondary leg (the GPU idles while a leg sets up)
 
@@ -695,6 +698,159 @@ def e2e_leg(cfg, keep, steps, chunk_mb, torch, rta):
             "d2h_bytes_per_step": cfg.output_bytes, "steps": k, "chunk_bytes": chunk,
             "launches_per_step": launches, "matches_device_result": ok,
             "api": "rta_extract_host (pinned host in/out, double-buffered H2D, D2H on a third stream)"}
+
+
+def read_stream_peak(torch, nbytes=2 << 30, reps=10):
+    """A read-only stream over 2 GiB (torch.sum over float64 / int64 / float32 views: a library
+    reduction, used here as a yardstick only), best of `reps`. The driver's
+    MEASURED_PEAKS.json figure is a copy (half reads, half writes); the extraction
+    kernels are 5:1 reads, and HBM sustains more on reads than on a 1:1 mix, so their
+    fraction of the copy peak can exceed 1. This is the second denominator."""
+    x = torch.empty(nbytes, dtype=torch.uint8, device="cuda").random_(0, 255)
+    best, how = None, None
+    # 8-byte elements read fastest (6.89 TB/s against 6.52 TB/s for float32 on this pool)
+    for name, v in (("float64", x.view(torch.float64)), ("int64", x.view(torch.int64)),
+                    ("float32", x.view(torch.float32))):
+        for _ in range(3):
+            torch.sum(v)
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            torch.sum(v)
+            b.record()
+            torch.cuda.synchronize()
+            ms = a.elapsed_time(b)
+            if best is None or ms < best:
+                best, how = ms, name
+    del x
+    return nbytes / best / 1e6, "torch.sum over 2 GiB as %s, best of %d (read-only stream)" % (how, reps)
+
+
+def small_batch_leg(cfg, steps, peak, torch, dl0gen, rta):
+    """BASELINE.json configs[0] (C1, 64 events, 7 MB): launch-latency-bound. Device time
+    per launch, eager and as a CUDA-graph replay, with L2 flushed between launches
+    (a 256 MB write, outside the event pair) and, for contrast, L2-resident."""
+    d_wf, d_ped, d_gain, outs, _, _ = device_batch(cfg, torch, dl0gen)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    side = torch.cuda.Stream()
+
+    def run(stream):
+        rta.rta_extract(d_wf, cfg.n_events, cfg.n_pixels, cfg.n_samples, d_ped, d_gain, cfg.W,
+                        *outs, stream=stream)
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        for _ in range(LEG_WARMUP):
+            run(side)
+        side.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            run(side)
+    torch.cuda.synchronize()
+
+    def timed(launch, flushed):
+        st = torch.cuda.current_stream()
+        per = []
+        for _ in range(3 + steps):
+            if flushed:
+                flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(st)
+            launch(st)
+            b.record(st)
+            per.append((a, b))
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in per[3:]]
+    res = {"workload": "%s: %s" % (cfg.name, cfg.label),
+           "l2": "input %.1f MB fits the L2: 'flushed' rows write 256 MB between launches, "
+                 "'resident' rows do not" % (cfg.input_bytes / 1e6)}
+    for name, launch in (("eager", run), ("graph_replay", lambda st: graph.replay())):
+        for flushed in (True, False):
+            sm = summarise(cfg, timed(launch, flushed), peak)
+            res["%s_%s" % (name, "flushed" if flushed else "resident")] = {
+                k: sm[k] for k in ("ms_avg", "ms_median", "ms_best", "waveform_GBps",
+                                   "frac_of_measured_hbm")}
+    return res
+
+
+def latency_leg(cfg, torch, dl0gen, rta, sizes=(1, 8, 64, 512, 4096), calls=1000):
+    """What ONE call costs on small batches (the RTA works event by event
+    during data taking; 30 s alert budget). Host wall time per call, p50 and
+    p99 over `calls` calls, for n_events of the C2 camera: (i) rta_extract + stream
+    synchronise, eager; (ii) the same launch as a CUDA-graph replay + synchronise;
+    (iii) rta_extract_host, pinned host buffers in and out; (iv) rta_extract_image_host.
+    The ABI is called through ctypes with the pointers prepared beforehand; `abi_call_us`
+    is what an empty call (rta_launch_count) costs that way."""
+    import ctypes
+    import numpy as np
+    L = rta.lib()
+    P, S, W = cfg.n_pixels, cfg.n_samples, cfg.W
+    n_max = max(sizes)
+    d_wf = torch.empty((n_max, P, S), dtype=torch.int16, device="cuda")
+    dl0gen.events_cuda(cfg, d_wf.data_ptr(), 0, n_max, torch.cuda.current_stream().cuda_stream)
+    ped, gain = dl0gen.calib(cfg)
+    x, y, nbr = dl0gen.hex_camera(P)
+    tp, tb = dl0gen.IMAGE_THRESHOLDS[cfg.name]
+    d_ped, d_gain = torch.from_numpy(ped).cuda(), torch.from_numpy(gain).cuda()
+    outs = [torch.empty(n_max * P, dtype=dt, device="cuda")
+            for dt in (torch.int32, torch.int32, torch.float32, torch.float32)]
+    h_wf = torch.empty(d_wf.shape, dtype=torch.int16, pin_memory=True)
+    h_wf.copy_(d_wf)
+    h_out = [torch.empty(n_max * P, dtype=o.dtype, pin_memory=True) for o in outs]
+    h_np, h_par = (torch.empty(n_max, dtype=torch.int32, pin_memory=True),
+                   torch.empty((n_max, 8), dtype=torch.float32, pin_memory=True))
+    host = [np.ascontiguousarray(a) for a in (ped, gain, x, y, nbr)]
+    hp = [a.ctypes.data for a in host]
+    stream = torch.cuda.Stream()
+    sh = stream.cuda_stream
+    sync = stream.synchronize
+    o = [t.data_ptr() for t in outs]
+    ho = [t.data_ptr() for t in h_out]
+    torch.cuda.synchronize()
+
+    def pct(ns):
+        ns = sorted(ns)
+        return {"p50_us": ns[len(ns) // 2] / 1e3, "p99_us": ns[(len(ns) * 99) // 100] / 1e3,
+                "min_us": ns[0] / 1e3}
+
+    def wall(fn, n):
+        for _ in range(20):
+            fn()
+        t = []
+        clock = time.perf_counter_ns
+        for _ in range(n):
+            t0 = clock()
+            fn()
+            t.append(clock() - t0)
+        return pct(t)
+    res = {"calls": calls, "camera": "%d pixels x %d samples, W=%d" % (P, S, W),
+           "abi_call_us": wall(lambda: L.rta_launch_count(), calls)["p50_us"],
+           "stream_sync_us": wall(sync, calls)["p50_us"]}
+    for n in sizes:
+        def eager():
+            L.rta_extract(d_wf.data_ptr(), n, P, S, d_ped.data_ptr(), d_gain.data_ptr(), W, *o, sh)
+            sync()
+        with torch.cuda.stream(stream):
+            eager()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=stream):
+                L.rta_extract(d_wf.data_ptr(), n, P, S, d_ped.data_ptr(), d_gain.data_ptr(), W, *o, sh)
+
+            def replay():
+                graph.replay()
+                sync()
+
+            def host_call():
+                L.rta_extract_host(h_wf.data_ptr(), n, P, S, hp[0], hp[1], W, *ho, 0)
+
+            def image_host():
+                L.rta_extract_image_host(h_wf.data_ptr(), n, P, S, hp[0], hp[1], W, hp[2], hp[3], hp[4],
+                                         tp, tb, h_np.data_ptr(), h_par.data_ptr(), None, 0)
+            k = calls if n <= 512 else max(200, calls // 5)
+            res["n%d" % n] = {"input_bytes": n * P * S * 2,
+                              "extract_eager": wall(eager, k), "extract_graph_replay": wall(replay, k),
+                              "extract_host": wall(host_call, k), "extract_image_host": wall(image_host, k)}
+            del graph
+    return res
 
 
 def mem_available_bytes():
@@ -981,6 +1137,56 @@ def cpu_baseline_leg(cfg, keep, dl0gen, torch):
                                                   "floats_bit_exact": floats_equal}}
 
 
+def compact_summary(out):
+    """Every leg as [ms per launch, fraction of the measured HBM copy peak] (host-fed legs:
+    [GB/s, fraction of the measured host link]; latency: p50 microseconds per call), short
+    enough to survive in the tail of the line. `cap` lists the legs during which the driver
+    reported sw_power_cap."""
+    r3 = lambda v: None if v is None else round(float(v), 3)
+    pair = lambda d: [round(d["ms_avg"], 4), r3(d.get("frac_of_measured_hbm"))]
+    sm = {"main": [round(out["roofline"]["avg_launch_ms"], 4), r3(out["roofline"]["frac"]),
+                   r3(out["roofline"].get("frac_of_read_stream_peak"))]}
+    for name, d in out.get("configs", {}).items():
+        if name == "C1":
+            sm["C1"] = {k.replace("_flushed", "_fl").replace("_resident", "_l2"): pair(v)
+                        for k, v in d.items() if isinstance(v, dict)}
+        else:
+            sm[name] = pair(d)
+    for leg in ("family", "packed12"):
+        for name, d in out.get(leg, {}).items():
+            if leg == "family":
+                sm["fam." + name] = {k: pair(v) for k, v in d.items()}
+            else:
+                sm["p12." + name] = pair(d)
+    for name, d in out.get("image", {}).items():
+        peak = out["roofline"]["peak"]
+        sm["img." + name] = {k: [round(d[k]["ms_avg"], 4), r3(d[k].get("frac_of_measured_hbm"))]
+                             for k in ("fused", "moments", "two_calls") if k in d}
+    if "ragged" in out:
+        sm["ragged"] = pair(out["ragged"])
+        if "unspecialised" in out["ragged"]:
+            sm["ragged.unspec"] = pair(out["ragged"]["unspecialised"])
+    for name, d in out.get("any_shape", {}).items():
+        if isinstance(d, dict) and "staged_any" in d:
+            sm["any." + name] = pair(d["staged_any"])
+    e = out.get("e2e", {})
+    if e.get("value") is not None:
+        sm["e2e"] = [r3(e["value"]), r3(e.get("frac_of_host_link"))]
+    su = out.get("sustained", {})
+    if su:
+        sm["sus"] = [r3(su["value"]), r3(su.get("frac_of_host_link"))]
+        for k in ("pageable", "image", "packed12"):
+            if k in su:
+                sm["sus." + k] = [r3(su[k]["value"]), r3(su[k].get("frac_of_host_link"))]
+    lat = out.get("latency", {})
+    for k, d in lat.items():
+        if k.startswith("n") and isinstance(d, dict):
+            sm["lat." + k] = [round(d[m]["p50_us"], 1) for m in
+                              ("extract_eager", "extract_graph_replay", "extract_host", "extract_image_host")]
+    sm["cap"] = sorted(k for k, c in out.get("leg_clocks", {}).items() if c.get("sw_power_cap"))
+    return sm
+
+
 def multi_rank_command(n_gpus, argv):
     """The command `python bench.py --gpus N` re-executes itself as when no
     torchrun environment is present (rendezvous on 127.0.0.1: the container's
@@ -1182,7 +1388,13 @@ def main():
                 r = None
                 torch.cuda.empty_cache()
             if "configs" in legs:
+                # C1 is configs[0]: the small case, bound by launch latency, not by HBM
+                others["C1"] = small_batch_leg(dl0gen.CONFIGS["C1"], max(20, args.steps), peak,
+                                               torch, dl0gen, rta)
                 out["configs"] = others
+            if "latency" in legs:
+                out["latency"] = latency_leg(dl0gen.CONFIGS["C2"], torch, dl0gen, rta)
+                torch.cuda.empty_cache()
             fam = {}
             for name in ("C2", "C3", "C4") if "family" in legs else ():
                 fam[name] = family_leg(dl0gen.CONFIGS[name], max(10, args.steps // 4), peak,
@@ -1215,6 +1427,14 @@ def main():
                 torch.cuda.empty_cache()
             if img:
                 out["image"] = img
+            rs_peak, rs_how = read_stream_peak(torch)
+            r = out["roofline"]
+            r["read_stream_peak"] = rs_peak
+            r["read_stream_peak_source"] = rs_how
+            r["frac_of_read_stream_peak"] = r["achieved"] / rs_peak
+            r["note"] = ("`peak` is the driver's copy figure (1:1 reads and writes); this kernel is 5:1 "
+                         "reads, which HBM serves faster, so `frac` can pass 1; frac_of_read_stream_peak "
+                         "divides by a read-only stream measured in this run")
             leg_sampler.stop()
             if leg_clocks:
                 out["leg_clocks"] = leg_clocks   # whole leg (set-up included): sm clock, peak power
@@ -1227,6 +1447,8 @@ def main():
         out["e2e"] = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0,
                       "d2h_bytes_per_step": 0, "note": "skipped by --no-extra"}
     if rank == 0:
+        if world == 1 and not args.no_extra:
+            out["summary"] = compact_summary(out)   # last key: the tail of the line carries every leg
         print(json.dumps(out))
     if dist is not None:
         dist.barrier()

@@ -85,3 +85,43 @@ def test_extra_shapes_are_not_baseline_configs():
         assert name not in dl0gen.CONFIGS and c.n_samples * c.W * 65535 < 2 ** 31
         assert bench.workload(name, dl0gen) is not None
     assert bench.workload("C2", dl0gen) is dl0gen.CONFIGS["C2"]
+
+
+def test_compact_summary_is_short_and_carries_every_leg():
+    """The driver keeps the tail of the bench line: the last key must hold every leg as
+    [ms, fraction] in well under 2 KB ("only C2 is in the record")."""
+    import json
+    import bench
+    leg = lambda ms, f: {"ms_avg": ms, "frac_of_measured_hbm": f}
+    lat = {m: {"p50_us": 12.345, "p99_us": 20.0, "min_us": 10.0} for m in
+           ("extract_eager", "extract_graph_replay", "extract_host", "extract_image_host")}
+    out = {
+        "roofline": {"avg_launch_ms": 0.26, "frac": 1.046, "peak": 6546.6, "frac_of_read_stream_peak": 0.93},
+        "configs": {"C3": leg(0.336, 1.057), "C4": leg(1.734, 0.98),
+                    "C1": {"workload": "C1", "l2": "x", "eager_flushed": leg(0.01, 0.1),
+                           "eager_resident": leg(0.008, 0.2), "graph_replay_flushed": leg(0.009, 0.1),
+                           "graph_replay_resident": leg(0.007, 0.2)}},
+        "family": {c: {k: leg(0.3, 0.9) for k in ("fixed", "local_peak", "fir")} for c in ("C2", "C3", "C4")},
+        "packed12": {c: leg(0.3, 0.9) for c in ("C2", "C3", "C4")},
+        "image": {c: {k: leg(0.3, 0.9) for k in ("fused", "moments", "two_calls")} for c in ("C2", "C3", "C4")},
+        "ragged": dict(leg(0.83, 0.95), unspecialised=leg(0.66, 0.93)),
+        "any_shape": {n: {"kernel": "staged<jit>", "staged_any": leg(0.36, 1.0), "generic": leg(2.0, 0.2)}
+                      for n in ("X60", "X40w5", "X96", "X128w10", "X2048")},
+        "e2e": {"value": 53.8, "frac_of_host_link": 0.97},
+        "sustained": {"value": 55.2, "frac_of_host_link": 0.99,
+                      "pageable": {"value": 44.0, "frac_of_host_link": 0.8},
+                      "image": {"value": 55.0, "frac_of_host_link": 0.99},
+                      "packed12": {"value": 73.0, "frac_of_host_link": 0.99}},
+        "latency": dict({"calls": 1000, "abi_call_us": 0.4}, **{"n%d" % n: lat for n in (1, 8, 64, 512, 4096)}),
+        "leg_clocks": {"packed12.C4": {"sw_power_cap": True}, "image.C2": {"sw_power_cap": False}},
+    }
+    sm = bench.compact_summary(out)
+    text = json.dumps(sm)
+    assert len(text) < 2000, len(text)
+    assert sm["C3"] == [0.336, 1.057] and sm["C4"] == [1.734, 0.98]
+    assert sm["main"] == [0.26, 1.046, 0.93]
+    assert sm["C1"]["graph_replay_l2"] == [0.007, 0.2]
+    assert sm["fam.C4"]["fixed"] == [0.3, 0.9] and sm["p12.C2"] == [0.3, 0.9]
+    assert sm["img.C3"]["moments"] == [0.3, 0.9] and sm["ragged.unspec"] == [0.66, 0.93]
+    assert sm["sus.packed12"] == [73.0, 0.99] and sm["lat.n64"] == [12.3, 12.3, 12.3, 12.3]
+    assert sm["cap"] == ["packed12.C4"]
