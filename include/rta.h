@@ -62,7 +62,12 @@ enum {
  *                     process; never inside a stream capture; RTA_JIT=0 turns it off);
  *                     without the compiler, and up to 1152 bytes, a kernel with runtime
  *                     (n_samples, W); longer traces a kernel that gives a thread a run of
- *                     window starts. Any other 2-byte-aligned pointer takes the
+ *                     window starts ("segments"), or a warp per trace ("lanes<32>":
+ *                     n_samples a multiple of 8 with a window much wider than a
+ *                     segment, or a trace too long for a segment stage) — these two
+ *                     for rta_extract only; the other extractors, P12 input, mixed
+ *                     batches and the image calls run the generic kernel on traces
+ *                     above 1152 bytes. Any other 2-byte-aligned pointer takes the
  *                     runtime-shape kernel too, unless the trace (pair) is a multiple of
  *                     32 bytes; those take the generic kernel (strided global loads:
  *                     several times slower). Same
@@ -422,7 +427,7 @@ const char* rta_strerror(int status);
 int rta_last_cuda_error(void);
 
 /* Which kernel a shape takes, for tests and profiles: a static string such as
- * "tile<S=40,W=7>", "staged<jit>", "staged<any>", "segments" or "generic" for
+ * "tile<S=40,W=7>", "staged<jit>", "staged<any>", "segments", "lanes<32>" or "generic" for
  * (n_samples, W, 16-byte-aligned?). */
 const char* rta_kernel_name(int32_t n_samples, int32_t W, int aligned16);
 /* Take the run-time compile off the data path. A shape without an ahead-of-time

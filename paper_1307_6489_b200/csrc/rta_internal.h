@@ -81,6 +81,7 @@ void rta_count_launch();
 // Tile scheduling of the staged kernels: dynamic (default) or the static
 // round-robin (tests compare the two). rta_sched_release frees the per-stream
 // scheduler words (rta_shutdown).
+// (the three setters below exist in librta_testing.so only: rta_kernels.cu -DRTA_TESTING)
 void rta_set_static_schedule(bool on);
 // Measurements / tests: 4, 8, 16 or 32 = the sliding extractor runs the several-lanes-per-trace
 // kernel with that many lanes wherever it can (n_samples a multiple of 8, aligned base); 0 = normal.

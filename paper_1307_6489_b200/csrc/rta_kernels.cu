@@ -859,11 +859,24 @@ __global__ void __launch_bounds__(256)
 
 // ------------------------------------------------------------- dispatch ----
 constexpr int kMaxDevices = 32;
+#ifdef RTA_TESTING
+// Process-wide dispatch switches: in librta_testing.so only (this file is compiled a
+// second time with -DRTA_TESTING for it).
 std::atomic<int> g_force_lanes{0};  // tests / measurements: lanes per trace to use wherever the lanes kernel can run
 std::atomic<bool> g_static_schedule{false};  // tests: force the static round-robin
 // tests / measurements: segment length, traces per tile and threads per CTA of the segment
 // kernel (0 = chosen per shape); a forced L also sends shapes that have a faster kernel there
 std::atomic<int> g_seg_L{0}, g_seg_TR{0}, g_seg_NT{0}, g_seg_ST{0};
+#else
+// The shipped library has no switches: every read below is the constant 0 / false, and
+// what only a switch could select (the lanes kernel with fewer than 32 lanes, the
+// segment kernel on shapes that have a faster one) is not compiled into it.
+struct NoSwitch {
+  constexpr int load(std::memory_order = std::memory_order_relaxed) const { return 0; }
+  constexpr operator bool() const { return false; }
+};
+constexpr NoSwitch g_static_schedule{}, g_seg_L{}, g_seg_TR{}, g_seg_NT{}, g_seg_ST{};
+#endif
 
 struct DeviceInfo {
   std::atomic<int> ready{0};
@@ -1026,6 +1039,7 @@ int TileLauncher<C, MODE>::ctas_per_sm[kMaxDevices];
 
 }  // namespace
 
+#ifdef RTA_TESTING
 void rta_set_static_schedule(bool on) { g_static_schedule.store(on); }
 void rta_set_lanes_per_trace(int lpt) { g_force_lanes.store(lpt); }
 void rta_set_seg_tuning(int L, int TR, int NT, int stages) {
@@ -1034,6 +1048,7 @@ void rta_set_seg_tuning(int L, int TR, int NT, int stages) {
   g_seg_NT.store(NT);
   g_seg_ST.store(stages);
 }
+#endif
 cudaError_t rta_device_sms(int dev, int* sms) { return device_sms(dev, sms); }
 
 // rta_shutdown: the caller has synchronised the device(s)
@@ -1342,13 +1357,14 @@ cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
   // sectors per trace, gathering them from global memory (the generic kernel)
   // moves less than streaming whole tiles (S = 128: 0.99 ms against 1.69 ms).
   const bool gather = (MODE == MODE_FIXED) && 2 * a.S > 96;
+#ifdef RTA_TESTING
   if (MODE == MODE_SLIDING && a.staged && g_seg_L.load(std::memory_order_relaxed) != 0) {
     SegShape sg;  // measurements / tests only: the segment kernel on any shape
     int threads = 0;
     if (seg_shape(a.S, a.W, &sg, &threads)) return launch_seg(a, sg, threads);
   }
   if (MODE == MODE_SLIDING && lanes_eligible(a)) {
-    switch (g_force_lanes.load(std::memory_order_relaxed)) {  // measurements only (0 in production)
+    switch (g_force_lanes.load(std::memory_order_relaxed)) {  // measurements only
       case 4: return launch_lanes<4>(a);
       case 8: return launch_lanes<8>(a);
       case 16: return launch_lanes<16>(a);
@@ -1356,6 +1372,7 @@ cudaError_t launch_mode(const LaunchArgs& a, const ModeArgs& ma) {
       default: break;
     }
   }
+#endif
   if (a.staged && !gather) {
     RTA_TRY(CfgS30W7)
     RTA_TRY(CfgS40W7)
