@@ -22,8 +22,10 @@
  *  - The caller owns every pointer it passes; the library never frees or
  *    retains them. The library owns only rta_extract_stream's workspace (two
  *    device chunk buffers, two pinned staging buffers when the source is
- *    pageable, one copy stream, events), created lazily, reused, and released
- *    by rta_shutdown().
+ *    pageable, one copy stream, events), one per device, created lazily by the
+ *    first host-fed call on that device, reused, and released by
+ *    rta_shutdown(). Host-fed calls on one device serialise on that device's
+ *    workspace; calls on different devices do not wait for one another.
  *  - There is no CPU fallback: without a CUDA device every compute call
  *    returns RTA_ERR_CUDA.
  *  - The library links the CUDA runtime only (no libtorch).

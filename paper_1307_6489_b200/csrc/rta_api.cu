@@ -95,7 +95,27 @@ struct Workspace {
   bool returned_valid[2] = {false, false};
   cudaStream_t host_stream = nullptr;            // compute stream of rta_extract_host
 };
-Workspace g_ws;
+// One workspace per device, each behind its own mutex: host threads that feed different
+// GPUs of one process neither wait for one another nor tear down each other's buffers
+// (until round 3 there was one workspace per process, rebuilt whenever the current device
+// changed). A workspace is created by the first host-fed call on its device.
+constexpr int kMaxWsDevices = 32;
+Workspace g_ws_tab[kMaxWsDevices];
+
+// Which workspace serves `dev`; nullptr = a device index outside the table.
+Workspace* ws_for_device(int dev) {
+  return (dev >= 0 && dev < kMaxWsDevices) ? &g_ws_tab[dev] : nullptr;
+}
+
+// The workspace of the current device (not yet locked or prepared).
+Workspace* ws_current(cudaError_t* err) {
+  int dev = 0;
+  *err = cudaGetDevice(&dev);
+  if (*err != cudaSuccess) return nullptr;
+  Workspace* w = ws_for_device(dev);
+  if (w == nullptr) *err = cudaErrorInvalidDevice;
+  return w;
+}
 
 void ws_release(Workspace& w) {
   for (int b = 0; b < 2; ++b) {
@@ -381,8 +401,11 @@ int host_impl(const void* wf_host, int64_t n_events, int32_t n_pixels, int32_t n
                          out_sum_host, out_start_host, out_charge_host, out_time_host,
                          bits == 12 ? 1 : 2);
   if (v != RTA_OK || n_events == 0) return v;
-  std::lock_guard<std::mutex> lock(g_ws.mu);
-  Workspace& w = g_ws;
+  cudaError_t e0 = cudaSuccess;
+  Workspace* wsp = ws_current(&e0);
+  if (wsp == nullptr) return fail_cuda(e0);
+  Workspace& w = *wsp;
+  std::lock_guard<std::mutex> lock(w.mu);
   cudaError_t e = ws_prepare(w);
   if (e != cudaSuccess) return fail_cuda(e);
   const size_t calib_bytes = (size_t)n_pixels * 8u;
@@ -601,10 +624,14 @@ int rta_extract_stream(const uint16_t* wf_host, int64_t n_events, int32_t n_pixe
   const int v = validate(wf_host, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum,
                          out_start, out_charge, out_time);
   if (v != RTA_OK || n_events == 0) return v;
-  std::lock_guard<std::mutex> lock(g_ws.mu);
-  cudaError_t e = ws_prepare(g_ws);
+  cudaError_t e = cudaSuccess;
+  Workspace* wsp = ws_current(&e);
+  if (wsp == nullptr) return fail_cuda(e);
+  Workspace& ws = *wsp;
+  std::lock_guard<std::mutex> lock(ws.mu);
+  e = ws_prepare(ws);
   if (e != cudaSuccess) return fail_cuda(e);
-  return stream_impl(g_ws, wf_host, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum,
+  return stream_impl(ws, wf_host, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum,
                      out_start, out_charge, out_time, chunk_bytes, (cudaStream_t)stream, nullptr);
 }
 
@@ -639,10 +666,14 @@ int rta_extract_stream_packed12(const uint8_t* packed_host, int64_t n_events, in
   const int v = validate(packed_host, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum,
                          out_start, out_charge, out_time, 1);
   if (v != RTA_OK || n_events == 0) return v;
-  std::lock_guard<std::mutex> lock(g_ws.mu);
-  cudaError_t e = ws_prepare(g_ws);
+  cudaError_t e = cudaSuccess;
+  Workspace* wsp = ws_current(&e);
+  if (wsp == nullptr) return fail_cuda(e);
+  Workspace& ws = *wsp;
+  std::lock_guard<std::mutex> lock(ws.mu);
+  e = ws_prepare(ws);
   if (e != cudaSuccess) return fail_cuda(e);
-  return stream_impl(g_ws, packed_host, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum,
+  return stream_impl(ws, packed_host, n_events, n_pixels, n_samples, pedestal, gain, W, out_sum,
                      out_start, out_charge, out_time, chunk_bytes, (cudaStream_t)stream, nullptr,
                      12);
 }
@@ -994,12 +1025,16 @@ int rta_extract_image_stream(const uint16_t* wf_host, int64_t n_events, int32_t 
   if (v != RTA_OK) return v;
   v = validate_image(n_events, n_pixels, pix_x, pix_y, neighbors, out_n_pix, out_params, out_mask);
   if (v != RTA_OK || n_events == 0) return v;
-  std::lock_guard<std::mutex> lock(g_ws.mu);
-  cudaError_t e = ws_prepare(g_ws);
+  cudaError_t e = cudaSuccess;
+  Workspace* wsp = ws_current(&e);
+  if (wsp == nullptr) return fail_cuda(e);
+  Workspace& ws = *wsp;
+  std::lock_guard<std::mutex> lock(ws.mu);
+  e = ws_prepare(ws);
   if (e != cudaSuccess) return fail_cuda(e);
   const RtaCamera cam{pix_x, pix_y, neighbors, thr_picture, thr_boundary};
   const RtaImageOut out{out_n_pix, out_params, out_mask};
-  return image_stream_impl(g_ws, wf_host, n_events, n_pixels, n_samples, pedestal, gain, W, cam,
+  return image_stream_impl(ws, wf_host, n_events, n_pixels, n_samples, pedestal, gain, W, cam,
                            out, chunk_bytes, (cudaStream_t)stream, nullptr);
 }
 
@@ -1014,8 +1049,11 @@ int rta_extract_image_host(const uint16_t* wf_host, int64_t n_events, int32_t n_
   v = validate_image(n_events, n_pixels, pix_x_host, pix_y_host, neighbors_host, out_n_pix_host,
                      out_params_host, out_mask_host);
   if (v != RTA_OK || n_events == 0) return v;
-  std::lock_guard<std::mutex> lock(g_ws.mu);
-  Workspace& w = g_ws;
+  cudaError_t e0 = cudaSuccess;
+  Workspace* wsp = ws_current(&e0);
+  if (wsp == nullptr) return fail_cuda(e0);
+  Workspace& w = *wsp;
+  std::lock_guard<std::mutex> lock(w.mu);
   cudaError_t e = ws_prepare(w);
   if (e != cudaSuccess) return fail_cuda(e);
   // pedestal, gain, pix_x, pix_y: 4 bytes per pixel each; neighbours: 24
@@ -1123,18 +1161,19 @@ int64_t rta_chunk_events(int64_t n_events, int32_t n_pixels, int32_t n_samples,
 uint64_t rta_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 void rta_shutdown(void) {
-  std::lock_guard<std::mutex> lock(g_ws.mu);
-  if (g_ws.device >= 0) {
-    int cur = 0;
-    if (cudaGetDevice(&cur) == cudaSuccess) {
-      cudaSetDevice(g_ws.device);
+  int cur = 0;
+  const bool have_cur = cudaGetDevice(&cur) == cudaSuccess;
+  for (int d = 0; d < kMaxWsDevices; ++d) {
+    Workspace& w = g_ws_tab[d];
+    std::lock_guard<std::mutex> lock(w.mu);
+    if (w.device < 0) continue;
+    if (cudaSetDevice(w.device) == cudaSuccess) {
       cudaDeviceSynchronize();
-      ws_release(g_ws);
-      cudaSetDevice(cur);
-    } else {
-      cudaGetLastError();
+      ws_release(w);
     }
   }
+  if (have_cur) cudaSetDevice(cur);
+  cudaGetLastError();
   side_streams_release();
   rta_image_release();
   rta_jit_release();
